@@ -1,0 +1,143 @@
+/* b200_allegro.h — C ABI of the B200-native Allegro energy+force path (arXiv 2304.10061).
+ *
+ * One library, libb200allegro.so, hand-written CUDA for sm_100a.  Every entry point below is one of
+ * the calls of SURVEY.md §8(b); each cites the passage of /root/reference/PAPER.md (or the SURVEY §8(c)
+ * reading, where the paper is silent) that defines the operation.
+ *
+ * Conventions
+ *   - C linkage, no C++ type crosses the boundary.  Every function returns int: 0 = ALLEGRO_OK,
+ *     negative = error (table below).  allegro_last_error() gives a human-readable message for the
+ *     last failing call on that model (or the last failing call without a model).
+ *   - Pointer arguments are DEVICE pointers on the current CUDA device unless the parameter comment
+ *     says "host".  The `_host` variants take HOST pointers for every array and do the copies inside.
+ *   - The caller owns every array it passes in or receives results into.  Opaque handles
+ *     (allegro_model, allegro_nbr) are created and destroyed by the library.
+ *   - Work is enqueued on the stream set by allegro_set_stream (default: the legacy default stream).
+ *     Device-pointer calls return after enqueueing, except allegro_neighbors, which synchronises the
+ *     stream once (the edge count is needed on the host to size the list).
+ *   - Units: Angstrom, eV, fs, amu.  Species are int32 in [0, n_species).
+ *   - Box: orthorhombic, fully periodic, box[3] = edge lengths > 0 (host pointer).
+ *   - There is NO CPU fallback: without a CUDA device every compute call returns ALLEGRO_ERR_CUDA.
+ */
+#ifndef B200_ALLEGRO_H
+#define B200_ALLEGRO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  ALLEGRO_OK = 0,
+  ALLEGRO_ERR_BAD_HPARAMS = -1,   /* inconsistent hyper-parameters (incl. latent width != d, l_max > 3) */
+  ALLEGRO_ERR_BLOB_SIZE = -2,     /* blob_bytes != allegro_blob_size()                                */
+  ALLEGRO_ERR_BOX_TOO_SMALL = -3, /* an image shift does not fit int8                                 */
+  ALLEGRO_ERR_CAPACITY = -4,      /* an internal capacity was exceeded                                */
+  ALLEGRO_ERR_NONFINITE = -5,     /* coincident atoms (r = 0) or non-finite input                     */
+  ALLEGRO_ERR_CUDA = -6,          /* CUDA runtime error / no device                                   */
+  ALLEGRO_ERR_UNIMPLEMENTED = -7,
+  ALLEGRO_ERR_BAD_ARG = -8
+};
+
+typedef struct allegro_model allegro_model; /* weights, CG tables, workspaces */
+typedef struct allegro_nbr allegro_nbr;     /* CSR neighbor list on device     */
+
+/* Hyper-parameters (PAPER.md:222 lists the paper's values; SURVEY §8 table the five configs). */
+typedef struct {
+  int32_t n_species, l_max, n_layers, n_tensor, n_bessel, poly_p;
+  double r_cut;
+  int32_t n_twobody;
+  int32_t twobody_dims[8]; /* hidden widths; last = latent width d */
+  int32_t n_latent;
+  int32_t latent_dims[8];  /* same shape for every layer; last must equal d */
+  int32_t n_edge;
+  int32_t edge_dims[8];    /* hidden widths; the final ->1 layer is implicit */
+  double avg_num_neighbors; /* c_env = 1/sqrt(this)                  (S7) */
+  double resid_alpha[8];    /* per layer residual mixing coefficient (S7) */
+  int32_t precision;        /* MLP GEMM arithmetic: 0 fp32 (FFMA), 1 TF32 tensor cores, 2 BF16 tensor
+                               cores; accumulation is fp32 in all modes */
+  int64_t max_atoms, max_edges; /* capacity hints, 0 = grow on demand (+5 %) */
+} allegro_hparams;
+
+/* Number of bytes of the flat weight blob for these hyper-parameters (layout: SURVEY §8(b),
+ * restated in DESIGN.md).  host pointers. */
+int allegro_blob_size(const allegro_hparams* hp, size_t* bytes);
+
+/* Tensor-product path table (enumeration SURVEY §8(c) S6).  For layer L (1-based)
+ * returns the number of paths; if fan != NULL (host int32[n_paths]) fills, per path in canonical
+ * order, how many paths of that layer share the path's output irrep.  dims (host int32[2], may be
+ * NULL) receives {D_{L-1}, D_L}, the feature widths sum(2l+1) before / after the layer. */
+int allegro_path_info(const allegro_hparams* hp, int32_t layer, int32_t* n_paths, int32_t* fan, int32_t* dims);
+
+/* Create a model from hyper-parameters and the flat blob (host pointers).  Builds irreps, paths, the
+ * path-weight-fused real Clebsch-Gordan tensors K^L (Fig. 3) and uploads weights. */
+int allegro_create(const allegro_hparams* hp, const void* blob, size_t blob_bytes, allegro_model** out);
+int allegro_destroy(allegro_model* m);
+
+/* cudaStream_t to enqueue on, passed as void* (e.g. torch.cuda.current_stream().cuda_stream). */
+int allegro_set_stream(allegro_model* m, void* cuda_stream);
+
+/* Optional device allocator hooks (e.g. PyTorch's caching allocator); default cudaMalloc/cudaFree.
+ * Must be set before the first neighbors/compute call. */
+typedef void* (*allegro_alloc_fn)(size_t bytes, void* user);
+typedef void (*allegro_free_fn)(void* ptr, void* user);
+int allegro_set_allocator(allegro_model* m, allegro_alloc_fn a, allegro_free_fn f, void* user);
+
+/* Maximum number of active edges processed per center-contiguous chunk (strict locality,
+ * PAPER.md:138, makes chunks independent).  Default 1<<20. */
+int allegro_set_chunk_edges(allegro_model* m, int64_t max_edges_per_chunk);
+
+/* Periodic cell-list neighbor build (PAPER.md:128 ordered pairs).  Edge set =
+ * {(i,j,s): (i!=j or s!=0), d2 < cutoff^2}, dx = (x_j - x_i) + s_x*L_x, d2 = (dx*dx+dy*dy)+dz*dz in
+ * fp64 without FMA contraction; CSR by i, each row sorted by (j, sx, sy, sz); positions need not be
+ * wrapped (shifts are relative to the positions as given).
+ * pos: device f64[n_atoms*3]; box: host f64[3]; *inout: reused (buffers kept) if non-NULL. */
+int allegro_neighbors(allegro_model* m, const double* pos, int64_t n_atoms, const double box[3], double cutoff,
+                      allegro_nbr** inout);
+int allegro_neighbors_host(allegro_model* m, const double* pos_host, int64_t n_atoms, const double box[3],
+                           double cutoff, allegro_nbr** inout);
+/* Read-only DEVICE views of the list: row_ptr int64[n_atoms+1], j int32[n_edges], shift int8[n_edges*3]. */
+int allegro_nbr_info(const allegro_nbr* n, int64_t* n_atoms, int64_t* n_edges, const int64_t** row_ptr,
+                     const int32_t** j, const int8_t** shift);
+/* Copy the list to host arrays (row_ptr int64[n_atoms+1], j int32[n_edges], shift int8[n_edges*3]). */
+int allegro_nbr_copy_host(allegro_model* m, const allegro_nbr* n, int64_t* row_ptr, int32_t* j, int8_t* shift);
+int allegro_nbr_free(allegro_model* m, allegro_nbr* n);
+
+/* Energy and forces (PAPER.md:128 energy decomposition; Eq. (2) PAPER.md:132-138 layers
+ * fp64 final stage; forces F_i = -dE/dr_i by the hand-written analytic backward).
+ * The list may have been built at cutoff >= r_cut (Verlet skin); edges with r >= r_cut are dropped.
+ * pos f64[N*3], species i32[N], e_total f64[1], e_atom f64[N] or NULL, force f64[N*3] (device). */
+int allegro_compute(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                    const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force);
+int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                         const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom,
+                         double* force);
+
+/* One velocity-Verlet NVE step: v += dt/2 F/m; r += dt v; [rebuild list at cutoff
+ * r_cut+skin if *step_counter % rebuild_every == 0]; F; v += dt/2 F/m.  `force` f64[N*3] (device) must
+ * hold F(r) of the current positions on entry (call allegro_compute once before the first step) and
+ * holds F of the new positions on exit.  mass: device f64[n_species].  e_pot, e_kin: device f64[1].
+ * step_counter: host int64, incremented. */
+int allegro_step_nve(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                     const double* mass, int64_t n_atoms, const double box[3], double dt_fs,
+                     int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
+                     double* e_pot, double* e_kin);
+
+/* Counters for tests/bench: number of kernels launched by the library since creation (host). */
+int allegro_launch_count(const allegro_model* m, int64_t* launches);
+/* Number of active (r < r_cut) edges of the last allegro_compute (synchronises the stream). */
+int allegro_last_active_edges(allegro_model* m, int64_t* n_active);
+
+/* Debug/parity taps (tests only): copy an intermediate tensor of the LAST chunk of the last
+ * allegro_compute to host as fp32.  name: "Y", "u", "x0", "x1".., "V1".., "gamma1".., "ebar".
+ * n_floats: in = capacity of out, out = floats written. */
+int allegro_debug_tensor(allegro_model* m, const char* name, float* out, int64_t* n_floats);
+
+const char* allegro_last_error(const allegro_model* m);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* B200_ALLEGRO_H */

@@ -1,0 +1,315 @@
+"""paper_2304_10061_b200 — thin Python binding of libb200allegro.so (include/b200_allegro.h).
+
+Argument marshalling only: every step of the hot path runs in the library's CUDA kernels.  PyTorch is
+used for device memory (tensors, caching allocator hook), streams and nothing else.  There is no CPU
+fallback: if the shared library is missing or no CUDA device is present, calls fail loudly.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+from .build import build as build_library, lib_path
+
+__all__ = ["Hparams", "Allegro", "NeighborList", "AllegroError", "load_library", "hparams_from"]
+
+_I32x8 = C.c_int32 * 8
+_F64x8 = C.c_double * 8
+
+
+class Hparams(C.Structure):
+    """Mirror of `allegro_hparams` (include/b200_allegro.h)."""
+    _fields_ = [
+        ("n_species", C.c_int32), ("l_max", C.c_int32), ("n_layers", C.c_int32), ("n_tensor", C.c_int32),
+        ("n_bessel", C.c_int32), ("poly_p", C.c_int32),
+        ("r_cut", C.c_double),
+        ("n_twobody", C.c_int32), ("twobody_dims", _I32x8),
+        ("n_latent", C.c_int32), ("latent_dims", _I32x8),
+        ("n_edge", C.c_int32), ("edge_dims", _I32x8),
+        ("avg_num_neighbors", C.c_double),
+        ("resid_alpha", _F64x8),
+        ("precision", C.c_int32),
+        ("max_atoms", C.c_int64), ("max_edges", C.c_int64),
+    ]
+
+
+def hparams_from(hp, precision: int = 0) -> Hparams:
+    """Build the C struct from any object with the attribute names of synthetic.configs.Hparams."""
+    h = Hparams()
+    h.n_species, h.l_max, h.n_layers, h.n_tensor = hp.n_species, hp.l_max, hp.n_layers, hp.n_tensor
+    h.n_bessel, h.poly_p, h.r_cut = hp.n_bessel, hp.poly_p, hp.r_cut
+    h.n_twobody = len(hp.twobody_dims)
+    h.n_latent = len(hp.latent_dims)
+    h.n_edge = len(hp.edge_dims)
+    for k, v in enumerate(hp.twobody_dims):
+        h.twobody_dims[k] = v
+    for k, v in enumerate(hp.latent_dims):
+        h.latent_dims[k] = v
+    for k, v in enumerate(hp.edge_dims):
+        h.edge_dims[k] = v
+    h.avg_num_neighbors = hp.avg_num_neighbors
+    for k, v in enumerate(hp.resid_alpha):
+        h.resid_alpha[k] = v
+    h.precision = precision
+    h.max_atoms = 0
+    h.max_edges = 0
+    return h
+
+
+class AllegroError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libb200allegro error {code}: {msg}")
+        self.code = code
+
+
+_ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+_lib = None
+
+EXPORTS = [
+    "allegro_blob_size", "allegro_path_info", "allegro_create", "allegro_destroy", "allegro_set_stream",
+    "allegro_set_allocator", "allegro_set_chunk_edges", "allegro_neighbors", "allegro_neighbors_host",
+    "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
+    "allegro_step_nve", "allegro_launch_count", "allegro_last_active_edges", "allegro_debug_tensor",
+    "allegro_last_error",
+]
+
+
+def load_library(path: Optional[str] = None) -> C.CDLL:
+    """dlopen the in-tree libb200allegro.so.  Raises (never falls back) if it is missing."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = path or lib_path()
+    if not os.path.exists(p):
+        raise FileNotFoundError(
+            f"{p} not found: run `python -m paper_2304_10061_b200.build` (or __graft_entry__.build()). "
+            "There is no CPU fallback for the Allegro hot path.")
+    lib = C.CDLL(p)
+    vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
+    P = C.POINTER
+    lib.allegro_blob_size.argtypes = [P(Hparams), P(C.c_size_t)]
+    lib.allegro_path_info.argtypes = [P(Hparams), i32, P(i32), P(i32), P(i32)]
+    lib.allegro_create.argtypes = [P(Hparams), vp, C.c_size_t, P(vp)]
+    lib.allegro_destroy.argtypes = [vp]
+    lib.allegro_set_stream.argtypes = [vp, vp]
+    lib.allegro_set_allocator.argtypes = [vp, _ALLOC_FN, _FREE_FN, vp]
+    lib.allegro_set_chunk_edges.argtypes = [vp, i64]
+    lib.allegro_neighbors.argtypes = [vp, vp, i64, P(C.c_double), C.c_double, P(vp)]
+    lib.allegro_neighbors_host.argtypes = [vp, vp, i64, P(C.c_double), C.c_double, P(vp)]
+    lib.allegro_nbr_info.argtypes = [vp, P(i64), P(i64), P(vp), P(vp), P(vp)]
+    lib.allegro_nbr_copy_host.argtypes = [vp, vp, vp, vp, vp]
+    lib.allegro_nbr_free.argtypes = [vp, vp]
+    lib.allegro_compute.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp, vp]
+    lib.allegro_compute_host.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp, vp]
+    lib.allegro_step_nve.argtypes = [vp, vp, vp, vp, vp, vp, i64, P(C.c_double), C.c_double, i32, C.c_double, P(vp),
+                                     P(i64), vp, vp]
+    lib.allegro_launch_count.argtypes = [vp, P(i64)]
+    lib.allegro_last_active_edges.argtypes = [vp, P(i64)]
+    lib.allegro_debug_tensor.argtypes = [vp, C.c_char_p, vp, P(i64)]
+    lib.allegro_last_error.argtypes = [vp]
+    lib.allegro_last_error.restype = C.c_char_p
+    for name in EXPORTS:
+        if name != "allegro_last_error":
+            getattr(lib, name).restype = C.c_int
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def _box3(box) -> C.Array:
+    return (C.c_double * 3)(float(box[0]), float(box[1]), float(box[2]))
+
+
+def path_fan(hp: Hparams):
+    """Per layer, per path (canonical order): number of paths sharing the path's output irrep
+    (`allegro_path_info`).  Used by the synthetic blob writer for the alpha scale."""
+    lib = load_library()
+    out = []
+    for L in range(1, hp.n_layers + 1):
+        n = C.c_int32(0)
+        rc = lib.allegro_path_info(C.byref(hp), L, C.byref(n), None, None)
+        if rc:
+            raise AllegroError(rc, lib.allegro_last_error(None).decode())
+        fan = (C.c_int32 * n.value)()
+        lib.allegro_path_info(C.byref(hp), L, C.byref(n), fan, None)
+        out.append(list(fan))
+    return out
+
+
+def layer_dims(hp: Hparams):
+    lib = load_library()
+    dims = []
+    for L in range(1, hp.n_layers + 1):
+        n = C.c_int32(0)
+        dd = (C.c_int32 * 2)()
+        rc = lib.allegro_path_info(C.byref(hp), L, C.byref(n), None, dd)
+        if rc:
+            raise AllegroError(rc, lib.allegro_last_error(None).decode())
+        if L == 1:
+            dims.append(dd[0])
+        dims.append(dd[1])
+    return dims
+
+
+class NeighborList:
+    """Opaque handle to a device CSR list (allegro_nbr)."""
+
+    def __init__(self, model: "Allegro"):
+        self._model = model
+        self._h = C.c_void_p(None)
+
+    @property
+    def n_edges(self) -> int:
+        ne = C.c_int64(0)
+        self._model._lib.allegro_nbr_info(self._h, None, C.byref(ne), None, None, None)
+        return ne.value
+
+    def to_host(self):
+        """(row_ptr int64[N+1], j int32[E], shift int8[E,3]) as numpy arrays."""
+        import numpy as np
+        na, ne = C.c_int64(0), C.c_int64(0)
+        self._model._lib.allegro_nbr_info(self._h, C.byref(na), C.byref(ne), None, None, None)
+        rp = np.empty(na.value + 1, dtype=np.int64)
+        j = np.empty(ne.value, dtype=np.int32)
+        s = np.empty((ne.value, 3), dtype=np.int8)
+        self._model._check(self._model._lib.allegro_nbr_copy_host(
+            self._model._h, self._h, rp.ctypes.data, j.ctypes.data, s.ctypes.data))
+        return rp, j, s
+
+    def free(self):
+        if self._h:
+            self._model._lib.allegro_nbr_free(self._model._h, self._h)
+            self._h = C.c_void_p(None)
+
+
+class Allegro:
+    """allegro_model handle.  Tensors are torch CUDA tensors (float64 positions/forces, int32 species)."""
+
+    def __init__(self, hp: Hparams, blob: bytes, use_torch_allocator: bool = True, chunk_edges: Optional[int] = None):
+        import torch
+        if not torch.cuda.is_available():
+            raise AllegroError(-6, "no CUDA device: the Allegro hot path has no CPU fallback")
+        self._torch = torch
+        self._lib = load_library()
+        self.hp = hp
+        self._h = C.c_void_p(None)
+        buf = C.create_string_buffer(blob, len(blob))
+        rc = self._lib.allegro_create(C.byref(hp), buf, len(blob), C.byref(self._h))
+        if rc:
+            raise AllegroError(rc, self._lib.allegro_last_error(None).decode())
+        self._keep = []
+        if use_torch_allocator:
+            dev = torch.cuda.current_device()
+
+            def _alloc(nbytes, _user):
+                return torch.cuda.caching_allocator_alloc(int(nbytes), dev, torch.cuda.current_stream(dev))
+
+            def _free(ptr, _user):
+                torch.cuda.caching_allocator_delete(ptr)
+
+            a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
+            self._keep += [a, f]
+            self._check(self._lib.allegro_set_allocator(self._h, a, f, None))
+        if chunk_edges:
+            self._check(self._lib.allegro_set_chunk_edges(self._h, int(chunk_edges)))
+        self._sync_stream()
+
+    # -- plumbing ---------------------------------------------------------------------------------
+    def _check(self, rc: int):
+        if rc:
+            raise AllegroError(rc, self._lib.allegro_last_error(self._h).decode())
+
+    def _sync_stream(self):
+        s = self._torch.cuda.current_stream().cuda_stream
+        self._lib.allegro_set_stream(self._h, C.c_void_p(s))
+
+    def close(self):
+        if self._h:
+            self._lib.allegro_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launches(self) -> int:
+        v = C.c_int64(0)
+        self._lib.allegro_launch_count(self._h, C.byref(v))
+        return v.value
+
+    def last_active_edges(self) -> int:
+        v = C.c_int64(0)
+        self._check(self._lib.allegro_last_active_edges(self._h, C.byref(v)))
+        return v.value
+
+    # -- the four calls of the boundary -----------------------------------------------------------
+    def neighbors(self, pos, box: Sequence[float], cutoff: float, reuse: Optional[NeighborList] = None) -> NeighborList:
+        """allegro_neighbors: pos = CUDA float64 [N,3]."""
+        assert pos.is_cuda and pos.dtype == self._torch.float64 and pos.is_contiguous()
+        self._sync_stream()
+        nb = reuse or NeighborList(self)
+        self._check(self._lib.allegro_neighbors(self._h, pos.data_ptr(), pos.shape[0], _box3(box), float(cutoff),
+                                                C.byref(nb._h)))
+        return nb
+
+    def compute(self, pos, species, box: Sequence[float], nbr: NeighborList, want_atom_energies: bool = True):
+        """allegro_compute -> (e_total f64[1], e_atom f64[N] | None, force f64[N,3]) CUDA tensors."""
+        t = self._torch
+        assert pos.is_cuda and pos.dtype == t.float64 and pos.is_contiguous()
+        assert species.is_cuda and species.dtype == t.int32 and species.is_contiguous()
+        self._sync_stream()
+        N = pos.shape[0]
+        e = t.empty(1, dtype=t.float64, device=pos.device)
+        ea = t.empty(N, dtype=t.float64, device=pos.device) if want_atom_energies else None
+        f = t.empty((N, 3), dtype=t.float64, device=pos.device)
+        self._check(self._lib.allegro_compute(self._h, pos.data_ptr(), species.data_ptr(), N, _box3(box), nbr._h,
+                                              e.data_ptr(), ea.data_ptr() if ea is not None else None, f.data_ptr()))
+        return e, ea, f
+
+    def compute_into(self, pos, species, box3, nbr: NeighborList, e, ea, f):
+        """allegro_compute into preallocated tensors (no allocation: bench inner loop)."""
+        self._check(self._lib.allegro_compute(self._h, pos.data_ptr(), species.data_ptr(), pos.shape[0], box3, nbr._h,
+                                              e.data_ptr(), ea.data_ptr() if ea is not None else None, f.data_ptr()))
+
+    def neighbors_host(self, pos_np, box, cutoff, reuse: Optional[NeighborList] = None) -> NeighborList:
+        import numpy as np
+        pos_np = np.ascontiguousarray(pos_np, dtype=np.float64)
+        self._sync_stream()
+        nb = reuse or NeighborList(self)
+        self._check(self._lib.allegro_neighbors_host(self._h, pos_np.ctypes.data, pos_np.shape[0], _box3(box),
+                                                     float(cutoff), C.byref(nb._h)))
+        return nb
+
+    def compute_host(self, pos_np, species_np, box, nbr: NeighborList):
+        """allegro_compute_host: numpy in, numpy out; H2D/D2H copies happen inside the library."""
+        import numpy as np
+        pos_np = np.ascontiguousarray(pos_np, dtype=np.float64)
+        species_np = np.ascontiguousarray(species_np, dtype=np.int32)
+        N = pos_np.shape[0]
+        e = np.zeros(1)
+        ea = np.zeros(N)
+        f = np.zeros((N, 3))
+        self._sync_stream()
+        self._check(self._lib.allegro_compute_host(self._h, pos_np.ctypes.data, species_np.ctypes.data, N, _box3(box),
+                                                   nbr._h, e.ctypes.data, ea.ctypes.data, f.ctypes.data))
+        return float(e[0]), ea, f
+
+    def step_nve(self, pos, vel, force, species, mass, box, dt_fs: float, rebuild_every: int, skin: float,
+                 nbr: NeighborList, step_counter: C.c_int64, e_pot, e_kin):
+        """allegro_step_nve; pos/vel/force updated in place; nbr rebuilt when due."""
+        self._check(self._lib.allegro_step_nve(self._h, pos.data_ptr(), vel.data_ptr(), force.data_ptr(),
+                                               species.data_ptr(), mass.data_ptr(), pos.shape[0], _box3(box),
+                                               float(dt_fs), int(rebuild_every), float(skin), C.byref(nbr._h),
+                                               C.byref(step_counter), e_pot.data_ptr(), e_kin.data_ptr()))
+
+    def debug_tensor(self, name: str, max_floats: int = 1 << 26):
+        import numpy as np
+        out = np.empty(max_floats, dtype=np.float32)
+        n = C.c_int64(max_floats)
+        self._check(self._lib.allegro_debug_tensor(self._h, name.encode(), out.ctypes.data, C.byref(n)))
+        return out[:n.value].copy()

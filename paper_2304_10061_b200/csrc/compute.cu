@@ -1,0 +1,311 @@
+// allegro_compute: center-chunked forward + analytic backward of the Allegro energy (SURVEY.md §3 call
+// stack (2), §8(a) steps 2-11).  No host synchronisation inside; the number of active edges of a chunk
+// lives on the device (Work::m_act) and every kernel grid is sized for the chunk's candidate count.
+#include <algorithm>
+#include <cstring>
+
+#include "gemm.h"
+#include "kernels.h"
+
+static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
+  if (!m->work) m->work = new Work();
+  Work& w = *m->work;
+  int64_t M = std::max<int64_t>(nb->max_chunk_edges, 1), Nc = std::max<int64_t>(nb->max_chunk_centers, 1);
+  const allegro_hparams& hp = m->hp;
+  int d = m->d, n = m->n, nA = m->nA, NL = m->NL;
+  if (M > w.cap_edges || w.XS.empty()) {
+    auto R = [&](DevBuf& b, size_t floats) { return al_reserve(m, b, floats * 4 + 64); };
+    AL_CHECK(R(w.ei, M)); AL_CHECK(R(w.ej, M)); AL_CHECK(R(w.geo, 4 * M)); AL_CHECK(R(w.u, M)); AL_CHECK(R(w.du, M));
+    AL_CHECK(R(w.B, M * m->NB)); AL_CHECK(R(w.dB, M * m->NB)); AL_CHECK(R(w.Y, M * m->Denv));
+    w.tb_z.resize(hp.n_twobody); w.tb_a.resize(hp.n_twobody);
+    int maxw = d + n;
+    for (int k = 0; k < hp.n_twobody; ++k) {
+      AL_CHECK(R(w.tb_z[k], (size_t)M * hp.twobody_dims[k]));
+      if (k < hp.n_twobody - 1) AL_CHECK(R(w.tb_a[k], (size_t)M * hp.twobody_dims[k]));
+      maxw = std::max(maxw, hp.twobody_dims[k]);
+    }
+    w.XS.resize(NL); w.OM.resize(NL + 1); w.T.resize(NL + 1); w.lat_z.resize(NL); w.lat_a.resize(NL);
+    int Dmax = 1;
+    for (int L = 0; L < NL; ++L) {
+      AL_CHECK(R(w.XS[L], (size_t)M * (d + n)));
+      if (L >= 1) AL_CHECK(R(w.OM[L + 1], (size_t)M * nA));
+      if (L >= 1) AL_CHECK(R(w.T[L], (size_t)M * m->D[L] * n));
+      Dmax = std::max(Dmax, m->D[L]);
+      w.lat_z[L].resize(hp.n_latent); w.lat_a[L].resize(hp.n_latent);
+      for (int k = 0; k < hp.n_latent; ++k) {
+        AL_CHECK(R(w.lat_z[L][k], (size_t)M * hp.latent_dims[k]));
+        if (k < hp.n_latent - 1) AL_CHECK(R(w.lat_a[L][k], (size_t)M * hp.latent_dims[k]));
+        maxw = std::max(maxw, hp.latent_dims[k]);
+      }
+    }
+    AL_CHECK(R(w.XF, (size_t)M * d)); AL_CHECK(R(w.WE, (size_t)M * 2 * nA));
+    AL_CHECK(R(w.XB0, (size_t)M * d)); AL_CHECK(R(w.XB1, (size_t)M * d));
+    AL_CHECK(R(w.ZB0, (size_t)M * maxw)); AL_CHECK(R(w.ZB1, (size_t)M * maxw));
+    AL_CHECK(R(w.G, (size_t)M * (d + n))); AL_CHECK(R(w.OB, (size_t)M * 2 * nA));
+    AL_CHECK(R(w.VB0, (size_t)M * Dmax * n)); AL_CHECK(R(w.VB1, (size_t)M * Dmax * n));
+    AL_CHECK(R(w.ubar, M)); AL_CHECK(R(w.Ybar, (size_t)M * m->Denv)); AL_CHECK(R(w.ge, (size_t)3 * M));
+    w.cap_edges = M;
+  }
+  if (Nc > w.cap_centers) {
+    AL_CHECK(al_reserve(m, w.deg, (size_t)Nc * 4 + 64));
+    AL_CHECK(al_reserve(m, w.rowa, (size_t)(Nc + 1) * 8 + 64));
+    AL_CHECK(al_reserve(m, w.gamma, (size_t)Nc * m->Denv * n * 4 + 64));
+    w.cap_centers = Nc;
+  }
+  if (!w.m_act.p) {
+    AL_CHECK(al_reserve(m, w.m_act, 64));
+    AL_CUDA(m, cudaMemsetAsync(w.m_act.p, 0, 64, m->stream));
+  }
+  if (N > w.eatom_cap) { AL_CHECK(al_reserve(m, w.eatom, (size_t)N * 8 + 64)); w.eatom_cap = N; }
+  return ALLEGRO_OK;
+}
+
+void al_work_free(allegro_model* m) {
+  if (!m->work) return;
+  Work& w = *m->work;
+  std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.B, &w.dB, &w.Y,
+                              &w.XF, &w.WE, &w.gamma, &w.XB0, &w.XB1, &w.ZB0, &w.ZB1, &w.G, &w.OB, &w.VB0, &w.VB1,
+                              &w.ubar, &w.Ybar, &w.ge, &w.eatom};
+  for (auto* b : all) al_release(m, *b);
+  for (auto* v : {&w.tb_z, &w.tb_a, &w.XS, &w.OM, &w.T}) for (auto& b : *v) al_release(m, b);
+  for (auto* vv : {&w.lat_z, &w.lat_a}) for (auto& v : *vv) for (auto& b : v) al_release(m, b);
+  delete m->work;
+  m->work = nullptr;
+}
+
+static GemmArgs mk(const float* A, int lda, const Dense& D, bool transposed_weight, float* C, int ldc, int m_cap,
+                   const int* m_ptr, int epi) {
+  // transposed_weight = false: forward  Y = X W   -> Bt = Wt [fo][fi], N = fo, K = fi
+  // transposed_weight = true : backward dX = dY W^T -> Bt = W  [fi][fo], N = fi, K = fo
+  GemmArgs g{};
+  g.A = A; g.lda = lda;
+  if (!transposed_weight) { g.Bt = D.Wt; g.Bt16 = D.Wth; g.ldb = D.fi; g.N = D.fo; g.K = D.fi; }
+  else { g.Bt = D.W; g.Bt16 = D.Wh; g.ldb = D.fo; g.N = D.fi; g.K = D.fo; }
+  g.C = C; g.ldc = ldc; g.m_cap = m_cap; g.m_ptr = m_ptr; g.epi = epi;
+  return g;
+}
+
+static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* pos, const int32_t* species,
+                     const double box[3], const allegro_nbr* nb, double* e_atom, double* force) {
+  const allegro_hparams& hp = m->hp;
+  const int d = m->d, n = m->n, nA = m->nA, NL = m->NL, ntb = hp.n_twobody, nlat = hp.n_latent;
+  const int nc = (int)(ch.c1 - ch.c0);
+  const int m_cap = (int)(ch.e1 - ch.e0);
+  w.last_nc = nc;
+  if (m_cap <= 0) {   // isolated atoms only: E-hat_i = mu_Z
+    return k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom);   // rowa not valid -> handled below
+  }
+  const int* mp = (const int*)w.m_act.p;
+  cudaStream_t st = m->stream;
+  EdgeGeomArgs ga{};
+  ga.pos = pos; ga.species = species; memcpy(ga.box, box, 24); ga.rc = hp.r_cut; ga.p = hp.poly_p; ga.NB = m->NB;
+  ga.lmax = m->lmax; ga.row_ptr = (const int64_t*)nb->row_ptr.p; ga.j = (const int32_t*)nb->j.p;
+  ga.shift = (const int8_t*)nb->shift.p; ga.c0 = ch.c0; ga.nc = nc;
+  // ---- step 2: compaction + geometry ----------------------------------------------------------------
+  AL_CHECK(k_launch_active_count(m, ga, (int*)w.deg.p));
+  AL_CHECK(al_exclusive_scan_i64(m, (int*)w.deg.p, (int64_t*)w.rowa.p, nc, w.scan_tmp));
+  AL_CHECK(k_launch_set_mact(m, (int64_t*)w.rowa.p, nc, (int*)w.m_act.p));
+  AL_CHECK(k_launch_geom_fill(m, ga, (int64_t*)w.rowa.p, w));
+  // ---- step 3: two-body latent ------------------------------------------------------------------------
+  AL_CHECK(k_launch_twobody0(m, w, species, m->twobody[0], ntb == 1, m_cap));
+  for (int k = 1; k < ntb; ++k) {
+    bool last = (k == ntb - 1);
+    GemmArgs g = mk((float*)w.tb_a[k - 1].p, hp.twobody_dims[k - 1], m->twobody[k], false,
+                    last ? (float*)w.XS[0].p : (float*)w.tb_a[k].p, last ? d + n : hp.twobody_dims[k], m_cap, mp,
+                    last ? EPI_SILU_U : EPI_SILU_BOTH);
+    g.out2 = (float*)w.tb_z[k].p; g.ldo2 = hp.twobody_dims[k]; g.u = (float*)w.u.p;
+    AL_CHECK(al_gemm(m, g));
+  }
+  // ---- step 4: embedding projections  [w^0 | omega^1] = x^0 [A^0 | A^1] ----------------------------------
+  AL_CHECK(al_gemm(m, mk((float*)w.XS[0].p, d + n, m->emb01, false, (float*)w.WE.p, 2 * nA, m_cap, mp, EPI_PLAIN)));
+  // ---- steps 5-8: layers -----------------------------------------------------------------------------------
+  for (int L = 1; L <= NL; ++L) {
+    const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
+    int ldo = (L == 1) ? 2 * nA : nA;
+    const float* Vin = (L == 1) ? nullptr : (float*)w.T[L - 1].p;
+    float* Tout = (L < NL) ? (float*)w.T[L].p : nullptr;
+    AL_CHECK(k_launch_tp_fwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, Tout, (float*)w.XS[L - 1].p + d, d + n));
+    for (int k = 0; k < nlat; ++k) {
+      bool last = (k == nlat - 1);
+      const float* A = (k == 0) ? (float*)w.XS[L - 1].p : (float*)w.lat_a[L - 1][k - 1].p;
+      int lda = (k == 0) ? d + n : hp.latent_dims[k - 1];
+      float* C; int ldc;
+      if (!last) { C = (float*)w.lat_a[L - 1][k].p; ldc = hp.latent_dims[k]; }
+      else if (L < NL) { C = (float*)w.XS[L].p; ldc = d + n; }
+      else { C = (float*)w.XF.p; ldc = d; }
+      GemmArgs g = mk(A, lda, m->latent[L - 1][k], false, C, ldc, m_cap, mp, last ? EPI_LATENT : EPI_SILU_BOTH);
+      g.out2 = (float*)w.lat_z[L - 1][k].p; g.ldo2 = hp.latent_dims[k];
+      g.u = (float*)w.u.p; g.aux1 = (float*)w.XS[L - 1].p; g.ld1 = d + n; g.c0 = m->c_old[L - 1]; g.c1 = m->c_new[L - 1];
+      AL_CHECK(al_gemm(m, g));
+    }
+    if (L < NL)
+      AL_CHECK(al_gemm(m, mk((float*)w.XS[L].p, d + n, m->emb[L], false, (float*)w.OM[L + 1].p, nA, m_cap, mp, EPI_PLAIN)));
+  }
+  // ---- steps 9-10: edge energy, per-atom energy (fp64) -----------------------------------------------------
+  AL_CHECK(k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom));
+  // ---- step 11: backward -----------------------------------------------------------------------------------
+  AL_CUDA(m, cudaMemsetAsync(w.ubar.p, 0, (size_t)m_cap * 4, st));
+  AL_CUDA(m, cudaMemsetAsync(w.Ybar.p, 0, (size_t)m_cap * m->Denv * 4, st));
+  float* xb = (float*)w.XB0.p; float* xb_o = (float*)w.XB1.p;
+  float* vb = nullptr; float* vb_a = (float*)w.VB0.p; float* vb_b = (float*)w.VB1.p;
+  AL_CHECK(k_launch_fill_xbar(m, w, species, xb, m_cap));
+  for (int L = NL; L >= 1; --L) {
+    float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
+    AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
+    for (int k = nlat - 1; k >= 1; --k) {
+      GemmArgs g = mk(zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
+      g.aux1 = (float*)w.lat_z[L - 1][k - 1].p; g.ld1 = hp.latent_dims[k - 1];
+      AL_CHECK(al_gemm(m, g));
+      std::swap(zb, zb_o);
+    }
+    AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->latent[L - 1][0], true, (float*)w.G.p, d + n, m_cap, mp, EPI_PLAIN)));
+    const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
+    int ldo = (L == 1) ? 2 * nA : nA;
+    const float* Vin = (L == 1) ? nullptr : (float*)w.T[L - 1].p;
+    int ldob = (L == 1) ? 2 * nA : nA;
+    float* ombar = (L == 1) ? (float*)w.OB.p + nA : (float*)w.OB.p;
+    float* vprev = (vb == vb_a) ? vb_b : vb_a;
+    AL_CHECK(k_launch_tp_bwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, vb, (float*)w.G.p + d, d + n, vprev, ombar,
+                             ldob, (float*)w.OB.p));
+    vb = vprev;
+    GemmArgs g = mk((float*)w.OB.p, ldob, (L == 1) ? m->emb01 : m->emb[L - 1], true, xb_o, d, m_cap, mp, EPI_ADD2);
+    g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = (float*)w.G.p; g.ld2 = d + n;
+    AL_CHECK(al_gemm(m, g));
+    std::swap(xb, xb_o);
+  }
+  {
+    float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
+    AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.tb_z[ntb - 1].p, d, 1.0f, zb, d, d, m_cap));
+    for (int k = ntb - 1; k >= 1; --k) {
+      GemmArgs g = mk(zb, hp.twobody_dims[k], m->twobody[k], true, zb_o, hp.twobody_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
+      g.aux1 = (float*)w.tb_z[k - 1].p; g.ld1 = hp.twobody_dims[k - 1];
+      AL_CHECK(al_gemm(m, g));
+      std::swap(zb, zb_o);
+    }
+    AL_CHECK(k_launch_edge_bwd(m, w, zb, hp.twobody_dims[0], m->twobody[0], ntb == 1, force, m_cap));
+  }
+  return ALLEGRO_OK;
+}
+
+int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t N, const double box[3],
+                    const allegro_nbr* nb, double* e_total, double* e_atom, double* force) {
+  if (!m || !pos || !species || !box || !nb || !e_total || !force) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+  if (nb->n_atoms != N) { al_set_error(m, "neighbor list was built for a different n_atoms"); return ALLEGRO_ERR_BAD_ARG; }
+  if (nb->cutoff < m->hp.r_cut) { al_set_error(m, "neighbor list cutoff < r_cut"); return ALLEGRO_ERR_BAD_ARG; }
+  AL_CHECK(work_reserve(m, nb, N));
+  Work& w = *m->work;
+  double* ea = e_atom ? e_atom : (double*)w.eatom.p;
+  AL_CHECK(k_launch_zero_f64(m, force, 3 * N));
+  for (const Chunk& ch : nb->chunks) {
+    if (ch.e1 == ch.e0) {
+      // no candidate edges at all: make rowa all-zero so k_energy yields mu_Z
+      AL_CUDA(m, cudaMemsetAsync(w.rowa.p, 0, (size_t)(ch.c1 - ch.c0 + 1) * 8, m->stream));
+    }
+    AL_CHECK(run_chunk(m, w, ch, pos, species, box, nb, ea, force));
+  }
+  AL_CHECK(k_launch_sum_f64(m, ea, N, e_total));
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_compute(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                               const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force) {
+  return al_compute_impl(m, pos, species, n_atoms, box, nbr, e_total, e_atom, force);
+}
+
+extern "C" int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* species, int64_t N,
+                                    const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom,
+                                    double* force) {
+  if (!m || !pos || !species || !e_total || !force) return ALLEGRO_ERR_BAD_ARG;
+  void *dp = nullptr, *ds = nullptr, *de = nullptr, *dea = nullptr, *df = nullptr;
+  int rc = ALLEGRO_OK;
+  cudaStream_t st = m->stream;
+  if ((rc = al_alloc(m, &dp, N * 24 + 16)) || (rc = al_alloc(m, &ds, N * 4 + 16)) || (rc = al_alloc(m, &de, 16)) ||
+      (rc = al_alloc(m, &dea, N * 8 + 16)) || (rc = al_alloc(m, &df, N * 24 + 16)))
+    goto done;
+  cudaMemcpyAsync(dp, pos, N * 24, cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(ds, species, N * 4, cudaMemcpyHostToDevice, st);
+  rc = al_compute_impl(m, (double*)dp, (int32_t*)ds, N, box, nbr, (double*)de, (double*)dea, (double*)df);
+  if (rc == ALLEGRO_OK) {
+    cudaMemcpyAsync(e_total, de, 8, cudaMemcpyDeviceToHost, st);
+    if (e_atom) cudaMemcpyAsync(e_atom, dea, N * 8, cudaMemcpyDeviceToHost, st);
+    cudaMemcpyAsync(force, df, N * 24, cudaMemcpyDeviceToHost, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { al_set_error(m, cudaGetErrorString(e)); rc = ALLEGRO_ERR_CUDA; }
+    else {
+      int flags[4];
+      cudaMemcpy(flags, m->work->m_act.p, 16, cudaMemcpyDeviceToHost);
+      if (flags[1] & 1) { al_set_error(m, "coincident atoms (r = 0)"); rc = ALLEGRO_ERR_NONFINITE; }
+    }
+  }
+done:
+  cudaStreamSynchronize(st);
+  al_free(m, dp); al_free(m, ds); al_free(m, de); al_free(m, dea); al_free(m, df);
+  return rc;
+}
+
+extern "C" int allegro_last_active_edges(allegro_model* m, int64_t* n_active) {
+  if (!m || !n_active || !m->work) return ALLEGRO_ERR_BAD_ARG;
+  int v = 0;
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  AL_CUDA(m, cudaMemcpy(&v, m->work->m_act.p, 4, cudaMemcpyDeviceToHost));
+  *n_active = v;
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                                const double* mass, int64_t N, const double box[3], double dt_fs, int32_t rebuild_every,
+                                double skin, allegro_nbr** nbr, int64_t* step_counter, double* e_pot, double* e_kin) {
+  if (!m || !pos || !vel || !force || !species || !mass || !nbr || !step_counter || !e_pot || !e_kin) {
+    al_set_error(m, "NULL argument");
+    return ALLEGRO_ERR_BAD_ARG;
+  }
+  if (rebuild_every < 1 || skin < 0) { al_set_error(m, "rebuild_every >= 1 and skin >= 0 required"); return ALLEGRO_ERR_BAD_ARG; }
+  AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, true));
+  if (*nbr == nullptr || (*step_counter % rebuild_every) == 0)
+    AL_CHECK(al_neighbors_impl(m, pos, N, box, m->hp.r_cut + skin, nbr));
+  AL_CHECK(al_compute_impl(m, pos, species, N, box, *nbr, e_pot, nullptr, force));
+  AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, false));
+  AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, m->work->scan_tmp));
+  (*step_counter)++;
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_debug_tensor(allegro_model* m, const char* name, float* out, int64_t* n_floats) {
+  if (!m || !name || !out || !n_floats || !m->work) return ALLEGRO_ERR_BAD_ARG;
+  Work& w = *m->work;
+  int M = 0;
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  AL_CUDA(m, cudaMemcpy(&M, w.m_act.p, 4, cudaMemcpyDeviceToHost));
+  std::string s(name);
+  const float* src = nullptr; int width = 0, ld = 0; int64_t rows = M;
+  int d = m->d, n = m->n;
+  if (s == "Y") { src = (float*)w.Y.p; width = ld = m->Denv; }
+  else if (s == "u") { src = (float*)w.u.p; width = ld = 1; }
+  else if (s == "B") { src = (float*)w.B.p; width = ld = m->NB; }
+  else if (s == "geo") { src = (float*)w.geo.p; width = ld = 4; }
+  else if (s == "ge") { src = (float*)w.ge.p; width = ld = 3; }
+  else if (s == "ybar") { src = (float*)w.Ybar.p; width = ld = m->Denv; }
+  else if (s == "ubar") { src = (float*)w.ubar.p; width = ld = 1; }
+  else if (s == "ei") { src = (float*)w.ei.p; width = ld = 1; }
+  else if (s == "ej") { src = (float*)w.ej.p; width = ld = 1; }
+  else if (s == "we") { src = (float*)w.WE.p; width = ld = 2 * m->nA; }
+  else if (s[0] == 'x' && s.size() == 2) {
+    int L = s[1] - '0';
+    if (L < 0 || L > m->NL) return ALLEGRO_ERR_BAD_ARG;
+    if (L == m->NL) { src = (float*)w.XF.p; width = ld = d; } else { src = (float*)w.XS[L].p; width = d; ld = d + n; }
+  } else if (s[0] == 's' && s.size() == 2) {
+    int L = s[1] - '0';
+    if (L < 1 || L > m->NL) return ALLEGRO_ERR_BAD_ARG;
+    src = (float*)w.XS[L - 1].p + d; width = n; ld = d + n;
+  } else if (s[0] == 'V' && s.size() == 2) {
+    int L = s[1] - '0';
+    if (L < 1 || L >= m->NL) return ALLEGRO_ERR_BAD_ARG;
+    src = (float*)w.T[L].p; width = ld = m->D[L] * n;
+  } else if (s == "gamma") { src = (float*)w.gamma.p; width = ld = m->Denv * n; rows = w.last_nc; }
+  else { al_set_error(m, "unknown debug tensor"); return ALLEGRO_ERR_BAD_ARG; }
+  int64_t need = rows * width;
+  if (need > *n_floats) { *n_floats = need; al_set_error(m, "debug buffer too small"); return ALLEGRO_ERR_CAPACITY; }
+  if (need > 0) AL_CUDA(m, cudaMemcpy2D(out, (size_t)width * 4, src, (size_t)ld * 4, (size_t)width * 4, rows, cudaMemcpyDeviceToHost));
+  *n_floats = need;
+  return ALLEGRO_OK;
+}

@@ -1,0 +1,629 @@
+// Non-GEMM kernels of the hot path: active-edge compaction + edge geometry / radial / angular basis
+// (SURVEY.md §8(a) step 2), first two-body layer (step 3), environment sum + tensor product (steps 5-7,
+// PAPER.md Eq. (2) :132-138 and Fig. 3 :180), energies (steps 9-10), and the
+// hand-written backward of all of them (step 11), NVE helpers (step 12).
+#include <cmath>
+
+#include "kernels.h"
+
+namespace {
+
+#define FULLMASK 0xffffffffu
+
+__device__ __forceinline__ float silu_f(float z) { return z / (1.0f + expf(-z)); }
+__device__ __forceinline__ float dsilu_f(float z) {
+  float s = 1.0f / (1.0f + expf(-z));
+  return s * (1.0f + z * (1.0f - s));
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLMASK, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULLMASK, v, o);
+  return v;
+}
+
+// ---- real spherical harmonics, component normalisation, l <= 3 (SURVEY §8(c) S4 closed forms) ------
+#define SQ3 1.7320508075688772f
+#define SQ5 2.23606797749979f
+#define SQ15 3.872983346207417f
+#define SQ7 2.6457513110645907f
+#define C3A 2.091650066335189f    /* sqrt(35/8) */
+#define C3B 10.246950765959598f   /* sqrt(105)  */
+#define C3C 1.620185174601965f    /* sqrt(21/8) */
+
+__device__ __forceinline__ void sph_harm(float x, float y, float z, int lmax, float* Y) {
+  Y[0] = 1.0f;
+  if (lmax >= 1) { Y[1] = SQ3 * y; Y[2] = SQ3 * z; Y[3] = SQ3 * x; }
+  if (lmax >= 2) {
+    Y[4] = SQ15 * x * y; Y[5] = SQ15 * y * z; Y[6] = 0.5f * SQ5 * (3.0f * z * z - 1.0f);
+    Y[7] = SQ15 * x * z; Y[8] = 0.5f * SQ15 * (x * x - y * y);
+  }
+  if (lmax >= 3) {
+    Y[9] = C3A * y * (3.0f * x * x - y * y); Y[10] = C3B * x * y * z; Y[11] = C3C * y * (5.0f * z * z - 1.0f);
+    Y[12] = 0.5f * SQ7 * (5.0f * z * z * z - 3.0f * z); Y[13] = C3C * x * (5.0f * z * z - 1.0f);
+    Y[14] = 0.5f * C3B * z * (x * x - y * y); Y[15] = C3A * x * (x * x - 3.0f * y * y);
+  }
+}
+
+// v = sum_b Ybar[b] * grad Y_b (gradient of the polynomial forms above; only its tangential part is used)
+__device__ __forceinline__ void sph_harm_vjp(float x, float y, float z, int lmax, const float* g, float& vx, float& vy,
+                                             float& vz) {
+  vx = vy = vz = 0.f;
+  if (lmax >= 1) { vy += SQ3 * g[1]; vz += SQ3 * g[2]; vx += SQ3 * g[3]; }
+  if (lmax >= 2) {
+    vx += SQ15 * (y * g[4] + z * g[7] + x * g[8]);
+    vy += SQ15 * (x * g[4] + z * g[5] - y * g[8]);
+    vz += SQ15 * (y * g[5] + x * g[7]) + 3.0f * SQ5 * z * g[6];
+  }
+  if (lmax >= 3) {
+    float xx = x * x, yy = y * y, zz = z * z;
+    vx += 6.0f * C3A * x * y * g[9] + C3B * y * z * g[10] + C3C * (5.0f * zz - 1.0f) * g[13] + C3B * x * z * g[14] +
+          3.0f * C3A * (xx - yy) * g[15];
+    vy += 3.0f * C3A * (xx - yy) * g[9] + C3B * x * z * g[10] + C3C * (5.0f * zz - 1.0f) * g[11] - C3B * y * z * g[14] -
+          6.0f * C3A * x * y * g[15];
+    vz += C3B * x * y * g[10] + 10.0f * C3C * y * z * g[11] + 0.5f * SQ7 * (15.0f * zz - 3.0f) * g[12] +
+          10.0f * C3C * x * z * g[13] + 0.5f * C3B * (xx - yy) * g[14];
+  }
+}
+
+// ---- active-edge count / compaction + geometry ------------------------------------------------------
+__device__ __forceinline__ bool edge_vec(const EdgeGeomArgs& a, int i, int64_t e, int& j, double& dx, double& dy,
+                                         double& dz, double& r2) {
+  j = a.j[e];
+  dx = (a.pos[3 * (int64_t)j + 0] - a.pos[3 * (int64_t)i + 0]) + (double)a.shift[3 * e + 0] * a.box[0];
+  dy = (a.pos[3 * (int64_t)j + 1] - a.pos[3 * (int64_t)i + 1]) + (double)a.shift[3 * e + 1] * a.box[1];
+  dz = (a.pos[3 * (int64_t)j + 2] - a.pos[3 * (int64_t)i + 2]) + (double)a.shift[3 * e + 2] * a.box[2];
+  r2 = dx * dx + dy * dy + dz * dz;
+  return r2 < a.rc * a.rc;
+}
+
+__global__ void k_active_count(EdgeGeomArgs a, int* __restrict__ deg) {
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= a.nc) return;
+  int i = (int)(a.c0 + warp);
+  int64_t b = a.row_ptr[i], e = a.row_ptr[i + 1];
+  int cnt = 0;
+  for (int64_t k = b + lane; k < e; k += 32) {
+    int j; double dx, dy, dz, r2;
+    cnt += edge_vec(a, i, k, j, dx, dy, dz, r2) ? 1 : 0;
+  }
+  cnt = (int)warp_sum((float)cnt);
+  if (lane == 0) deg[warp] = cnt;
+}
+
+__global__ void k_set_mact(const int64_t* __restrict__ rowa, int nc, int* __restrict__ m_act) { m_act[0] = (int)rowa[nc]; }
+
+__global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, int* __restrict__ ei, int* __restrict__ ej,
+                            float4* __restrict__ geo, float* __restrict__ u, float* __restrict__ du,
+                            float* __restrict__ B, float* __restrict__ dB, float* __restrict__ Y, int Denv,
+                            int* __restrict__ flags) {
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= a.nc) return;
+  int i = (int)(a.c0 + warp);
+  int64_t b = a.row_ptr[i], e = a.row_ptr[i + 1];
+  int64_t out0 = rowa[warp];
+  int cnt = 0;
+  for (int64_t kb = b; kb < e; kb += 32) {
+    int64_t k = kb + lane;
+    int j = 0; double dx = 0, dy = 0, dz = 0, r2 = 0;
+    bool ok = (k < e) && edge_vec(a, i, k, j, dx, dy, dz, r2);
+    unsigned mask = __ballot_sync(FULLMASK, ok);
+    if (ok) {
+      int64_t o = out0 + cnt + __popc(mask & ((1u << lane) - 1u));
+      double r = sqrt(r2);
+      if (!(r > 0.0)) { atomicOr(&flags[1], 1); r = 1.0; }
+      double inv = 1.0 / r;
+      float hx = (float)(dx * inv), hy = (float)(dy * inv), hz = (float)(dz * inv);
+      ei[o] = i; ej[o] = j;
+      geo[o] = make_float4(hx, hy, hz, (float)r);
+      // envelope (fp64; PAPER.md:222 via SURVEY S2)
+      double x = r / a.rc, p = (double)a.p;
+      double xp1 = pow(x, p - 1.0), xp = xp1 * x;
+      double uu = 1.0 - 0.5 * (p + 1.0) * (p + 2.0) * xp + p * (p + 2.0) * xp * x - 0.5 * p * (p + 1.0) * xp * x * x;
+      double dud = -0.5 * p * (p + 1.0) * (p + 2.0) * xp1 * (1.0 - x) * (1.0 - x) / a.rc;
+      u[o] = (float)uu; du[o] = (float)dud;
+      // Bessel basis by the angle-addition recurrence in fp64
+      double th = M_PI * x, s1, c1;
+      sincos(th, &s1, &c1);
+      double sn = s1, cn = c1, pref = sqrt(2.0 / a.rc);
+      for (int nb = 1; nb <= a.NB; ++nb) {
+        double bn = pref * sn * inv;
+        double dbn = pref * ((double)nb * M_PI / a.rc * cn * inv - sn * inv * inv);
+        B[o * a.NB + nb - 1] = (float)(bn * uu);
+        dB[o * a.NB + nb - 1] = (float)(dbn * uu + bn * dud);
+        double s2 = sn * c1 + cn * s1, c2 = cn * c1 - sn * s1;
+        sn = s2; cn = c2;
+      }
+      float yy[16];
+      sph_harm(hx, hy, hz, a.lmax, yy);
+      for (int q = 0; q < Denv; ++q) Y[o * Denv + q] = yy[q];
+    }
+    cnt += __popc(mask);
+  }
+}
+
+// ---- first two-body layer: one-hot rows + Bessel matvec ----------------------------------
+constexpr int TB0_EPB = 8;
+__global__ void k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int* __restrict__ ej,
+                           const int32_t* __restrict__ species, const float* __restrict__ B, const float* __restrict__ u,
+                           const float* __restrict__ W, int S, int NB, int H, float* __restrict__ z, float* __restrict__ act,
+                           int ldact, int scale_u) {
+  const int M = *m_ptr;
+  int e0 = blockIdx.x * TB0_EPB;
+  if (e0 >= M) return;
+  __shared__ float sB[TB0_EPB][16];
+  __shared__ int sZi[TB0_EPB], sZj[TB0_EPB];
+  __shared__ float sU[TB0_EPB];
+  int tid = threadIdx.x;
+  if (tid < TB0_EPB * NB) {
+    int e = e0 + tid / NB;
+    sB[tid / NB][tid % NB] = (e < M) ? B[(size_t)e * NB + tid % NB] : 0.f;
+  }
+  if (tid < TB0_EPB) {
+    int e = e0 + tid;
+    sZi[tid] = (e < M) ? species[ei[e]] : 0;
+    sZj[tid] = (e < M) ? species[ej[e]] : 0;
+    sU[tid] = (e < M) ? u[e] : 0.f;
+  }
+  __syncthreads();
+  for (int k = tid; k < H; k += blockDim.x) {
+    float wb[16];
+    for (int q = 0; q < NB; ++q) wb[q] = W[(size_t)(2 * S + q) * H + k];
+#pragma unroll
+    for (int t = 0; t < TB0_EPB; ++t) {
+      int e = e0 + t;
+      if (e >= M) break;
+      float acc = W[(size_t)sZi[t] * H + k] + W[(size_t)(S + sZj[t]) * H + k];
+      for (int q = 0; q < NB; ++q) acc = fmaf(sB[t][q], wb[q], acc);
+      z[(size_t)e * H + k] = acc;
+      float s = silu_f(acc);
+      act[(size_t)e * ldact + k] = scale_u ? sU[t] * s : s;
+    }
+  }
+}
+
+// ---- tensor track -------------------------------------------------------------------------------------
+struct TPArgs {
+  const int64_t* rowa;
+  const float* om; int ldo;       // omega^L  [M][(l,n)]
+  const float* Y; int Denv;
+  const float* Vin;               // [M][Din][n] or null (FIRST)
+  const float* w0; int ldw;       // FIRST: w^0 [M][(l,n)]
+  const int *v0_l, *v0_y, *env_l;
+  TPLayerDev t;
+  int n, lmax; float c_env;
+  float* Tout;                    // [M][Dout][n] or null
+  float* xs; int ldx;             // scalars s -> xs[e*ldx + nn]
+  float* gamma_out;               // [Nc][Denv][n] or null
+  // backward
+  const float* VbarL;             // [M][Dout][n] or null
+  const float* sbar; int lds;
+  float* Vbar_prev;               // [M][Din][n]
+  float* ombar; int ldob;
+  float* w0bar;                   // FIRST: [M][(l,n)] with ld = ldob
+  float* Ybar;
+};
+
+template <bool FIRST>
+__device__ __forceinline__ float v_load(const TPArgs& a, int64_t e, int comp, int nn) {
+  if (FIRST) return a.w0[e * a.ldw + a.v0_l[comp] * a.n + nn] * a.Y[e * a.Denv + a.v0_y[comp]];
+  return a.Vin[(e * a.t.Din + comp) * a.n + nn];
+}
+
+__device__ __forceinline__ void tp_gamma_M(const TPArgs& a, int64_t e0, int64_t e1, float* G, float* Ms) {
+  const int n = a.n;
+  for (int idx = threadIdx.x; idx < a.Denv * n; idx += blockDim.x) {
+    int b = idx / n, nn = idx - b * n, l = a.env_l[b];
+    float acc = 0.f;
+    for (int64_t e = e0; e < e1; ++e) acc = fmaf(a.om[e * a.ldo + l * n + nn], a.Y[e * a.Denv + b], acc);
+    G[idx] = a.c_env * acc;
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < a.t.npairs * n; idx += blockDim.x) {
+    int p = idx / n, nn = idx - p * n;
+    float acc = 0.f;
+    for (int k = a.t.pair_ptr[p]; k < a.t.pair_ptr[p + 1]; ++k) acc = fmaf(a.t.ent_val[k], G[a.t.ent_b[k] * n + nn], acc);
+    Ms[idx] = acc;
+  }
+  __syncthreads();
+}
+
+// One block per center: Gamma_i (Eq. (2) line 2), M_i = K . Gamma_i, then T_e = V_e . M_i for its edges.
+template <bool FIRST>
+__global__ void __launch_bounds__(256) k_tp_fwd(TPArgs a) {
+  extern __shared__ float smem[];
+  const int n = a.n;
+  float* G = smem;
+  float* Ms = smem + a.Denv * n;
+  int c = blockIdx.x;
+  int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
+  if (e1 <= e0) return;
+  tp_gamma_M(a, e0, e1, G, Ms);
+  if (a.gamma_out)
+    for (int idx = threadIdx.x; idx < a.Denv * n; idx += blockDim.x) a.gamma_out[(size_t)c * a.Denv * n + idx] = G[idx];
+  int deg = (int)(e1 - e0);
+  for (int idx = threadIdx.x; idx < deg * n; idx += blockDim.x) {
+    int el = idx / n, nn = idx - el * n;
+    int64_t e = e0 + el;
+    for (int cc = 0; cc < a.t.Dout; ++cc) {
+      float acc = 0.f;
+      for (int k = a.t.c_ptr[cc]; k < a.t.c_ptr[cc + 1]; ++k)
+        acc = fmaf(v_load<FIRST>(a, e, a.t.c_a[k], nn), Ms[a.t.c_p[k] * n + nn], acc);
+      if (cc == 0) a.xs[e * a.ldx + nn] = acc;
+      if (a.Tout) a.Tout[(e * a.t.Dout + cc) * n + nn] = acc;
+    }
+  }
+}
+
+__device__ __forceinline__ float tbar_load(const TPArgs& a, int64_t e, int cc, int nn) {
+  float v = a.VbarL ? a.VbarL[(e * a.t.Dout + cc) * a.n + nn] : 0.f;
+  if (cc == 0) v += a.sbar[e * a.lds + nn];
+  return v;
+}
+
+template <bool FIRST>
+__global__ void __launch_bounds__(256) k_tp_bwd(TPArgs a) {
+  extern __shared__ float smem[];
+  const int n = a.n, nl = a.lmax + 1;
+  float* G = smem;
+  float* Ms = smem + a.Denv * n;
+  int c = blockIdx.x;
+  int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
+  if (e1 <= e0) return;
+  int deg = (int)(e1 - e0);
+  tp_gamma_M(a, e0, e1, G, Ms);
+  // V-bar^{L-1}_e[a] = sum_c M[a,c] T-bar_e[c]
+  for (int idx = threadIdx.x; idx < deg * n; idx += blockDim.x) {
+    int el = idx / n, nn = idx - el * n;
+    int64_t e = e0 + el;
+    for (int aa = 0; aa < a.t.Din; ++aa) {
+      float acc = 0.f;
+      for (int k = a.t.a_ptr[aa]; k < a.t.a_ptr[aa + 1]; ++k)
+        acc = fmaf(Ms[a.t.a_p[k] * n + nn], tbar_load(a, e, a.t.a_c[k], nn), acc);
+      a.Vbar_prev[(e * a.t.Din + aa) * n + nn] = acc;
+    }
+  }
+  __syncthreads();
+  // M-bar[p] = sum_e V_e[a_p] T-bar_e[c_p]   (overwrites M)
+  for (int idx = threadIdx.x; idx < a.t.npairs * n; idx += blockDim.x) {
+    int p = idx / n, nn = idx - p * n;
+    int aa = a.t.pair_a[p], cc = a.t.pair_c[p];
+    float acc = 0.f;
+    for (int64_t e = e0; e < e1; ++e) acc = fmaf(v_load<FIRST>(a, e, aa, nn), tbar_load(a, e, cc, nn), acc);
+    Ms[idx] = acc;
+  }
+  __syncthreads();
+  // Gamma-bar[b] = sum_{(a,c)} K[a,b,c] M-bar[a,c]   (overwrites Gamma)
+  for (int idx = threadIdx.x; idx < a.Denv * n; idx += blockDim.x) {
+    int b = idx / n, nn = idx - b * n;
+    float acc = 0.f;
+    for (int k = a.t.b_ptr[b]; k < a.t.b_ptr[b + 1]; ++k) acc = fmaf(a.t.b_val[k], Ms[a.t.b_p[k] * n + nn], acc);
+    G[idx] = acc;
+  }
+  __syncthreads();
+  // omega-bar_e[l,n] = c_env sum_m Gamma-bar[(l,m),n] Y_e[(l,m)]
+  for (int idx = threadIdx.x; idx < deg * nl * n; idx += blockDim.x) {
+    int el = idx / (nl * n), rem = idx - el * nl * n, l = rem / n, nn = rem - l * n;
+    int64_t e = e0 + el;
+    float acc = 0.f;
+    for (int b = l * l; b < (l + 1) * (l + 1); ++b) acc = fmaf(G[b * n + nn], a.Y[e * a.Denv + b], acc);
+    a.ombar[e * a.ldob + l * n + nn] = a.c_env * acc;
+  }
+  // Y-bar_e[b] += c_env sum_n omega_e[l(b),n] Gamma-bar[b,n]
+  int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+  for (int item = warp; item < deg * a.Denv; item += nw) {
+    int el = item / a.Denv, b = item - el * a.Denv, l = a.env_l[b];
+    int64_t e = e0 + el;
+    float acc = 0.f;
+    for (int nn = lane; nn < n; nn += 32) acc = fmaf(a.om[e * a.ldo + l * n + nn], G[b * n + nn], acc);
+    acc = warp_sum(acc);
+    if (lane == 0) a.Ybar[e * a.Denv + b] += a.c_env * acc;
+  }
+  if (FIRST) {
+    __syncthreads();
+    // V^0 = w^0 (x) Y :  w0-bar[l,n] = sum_{a in l} V-bar^0[a,n] Y[a] ; Y-bar[a] += sum_n w0[l(a),n] V-bar^0[a,n]
+    for (int idx = threadIdx.x; idx < deg * nl * n; idx += blockDim.x) {
+      int el = idx / (nl * n), rem = idx - el * nl * n, l = rem / n, nn = rem - l * n;
+      int64_t e = e0 + el;
+      float acc = 0.f;
+      for (int aa = 0; aa < a.t.Din; ++aa)
+        if (a.v0_l[aa] == l) acc = fmaf(a.Vbar_prev[(e * a.t.Din + aa) * n + nn], a.Y[e * a.Denv + a.v0_y[aa]], acc);
+      a.w0bar[e * a.ldob + l * n + nn] = acc;
+    }
+    for (int item = warp; item < deg * a.t.Din; item += nw) {
+      int el = item / a.t.Din, aa = item - el * a.t.Din;
+      int64_t e = e0 + el;
+      float acc = 0.f;
+      for (int nn = lane; nn < n; nn += 32)
+        acc = fmaf(a.w0[e * a.ldw + a.v0_l[aa] * n + nn], a.Vbar_prev[(e * a.t.Din + aa) * n + nn], acc);
+      acc = warp_sum(acc);
+      if (lane == 0) a.Ybar[e * a.Denv + a.v0_y[aa]] += acc;
+    }
+  }
+}
+
+// ---- energies (fp64 final stage) -------------------------------------------------------------
+__global__ void k_energy(const int64_t* __restrict__ rowa, int nc, int64_t c0, const float* __restrict__ xf, int d,
+                         const double* __restrict__ w_eff, const int32_t* __restrict__ species,
+                         const double* __restrict__ sigma, const double* __restrict__ mu, double* __restrict__ e_atom) {
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= nc) return;
+  int64_t e0 = rowa[warp], e1 = rowa[warp + 1];
+  double acc = 0.0;
+  for (int64_t e = e0; e < e1; ++e)
+    for (int k = lane; k < d; k += 32) acc += (double)xf[e * d + k] * w_eff[k];
+  acc = warp_sum_d(acc);
+  if (lane == 0) {
+    int z = species[c0 + warp];
+    e_atom[c0 + warp] = sigma[z] * acc + mu[z];
+  }
+}
+
+__global__ void k_sum_f64(const double* __restrict__ x, int64_t n, double* __restrict__ out) {
+  __shared__ double sh[1024];
+  double s = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += blockDim.x) s += x[i];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int o = blockDim.x / 2; o > 0; o >>= 1) {
+    if (threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) *out = sh[0];
+}
+
+__global__ void k_fill_xbar(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int32_t* __restrict__ species,
+                            const double* __restrict__ sigma, const float* __restrict__ w_eff, int d, float* __restrict__ xb) {
+  const int M = *m_ptr;
+  int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  int64_t e = idx / d; int k = (int)(idx - e * d);
+  if (e >= M) return;
+  xb[idx] = (float)sigma[species[ei[e]]] * w_eff[k];
+}
+
+// zb = c * u * xbar * silu'(z) ; ubar += c * <xbar, silu(z)>      (one warp per edge)
+__global__ void k_bwd_prep(const int* __restrict__ m_ptr, const float* __restrict__ xbar, int ldx, const float* __restrict__ z,
+                           int ldz, const float* __restrict__ u, float c, float* __restrict__ zb, int ldzb, int width,
+                           float* __restrict__ ubar) {
+  const int M = *m_ptr;
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= M) return;
+  int64_t e = warp;
+  float cu = c * u[e], acc = 0.f;
+  for (int k = lane; k < width; k += 32) {
+    float xb = xbar[e * ldx + k], zz = z[e * ldz + k];
+    float s = 1.0f / (1.0f + expf(-zz));
+    acc = fmaf(xb, zz * s, acc);
+    zb[e * ldzb + k] = cu * xb * (s * (1.0f + zz * (1.0f - s)));
+  }
+  acc = warp_sum(acc);
+  if (lane == 0) ubar[e] += c * acc;
+}
+
+// Last backward stage: B-bar through the first two-body layer, r-bar, angular part, dE/dr_e, force scatter.
+__global__ void k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz, const float* __restrict__ W,
+                           int S, int NB, int H, const float4* __restrict__ geo, const float* __restrict__ du,
+                           const float* __restrict__ dB, const float* __restrict__ ubar, const float* __restrict__ Ybar,
+                           int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
+                           float* __restrict__ ge, double* __restrict__ force) {
+  const int M = *m_ptr;
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= M) return;
+  int64_t e = warp;
+  float rbar = 0.f;
+  for (int q = 0; q < NB; ++q) {
+    float acc = 0.f;
+    for (int k = lane; k < H; k += 32) acc = fmaf(zb1[e * ldz + k], W[(size_t)(2 * S + q) * H + k], acc);
+    acc = warp_sum(acc);
+    rbar = fmaf(acc, dB[e * NB + q], rbar);
+  }
+  if (lane == 0) {
+    rbar = fmaf(ubar[e], du[e], rbar);
+    float4 g4 = geo[e];
+    float yb[16];
+    for (int q = 0; q < Denv; ++q) yb[q] = Ybar[e * Denv + q];
+    float vx, vy, vz;
+    sph_harm_vjp(g4.x, g4.y, g4.z, lmax, yb, vx, vy, vz);
+    float dot = vx * g4.x + vy * g4.y + vz * g4.z;
+    float ir = 1.0f / g4.w;
+    float gx = rbar * g4.x + (vx - dot * g4.x) * ir;
+    float gy = rbar * g4.y + (vy - dot * g4.y) * ir;
+    float gz = rbar * g4.z + (vz - dot * g4.z) * ir;
+    if (ge) { ge[3 * e] = gx; ge[3 * e + 1] = gy; ge[3 * e + 2] = gz; }
+    int i = ei[e], j = ej[e];
+    atomicAdd(&force[3 * (int64_t)i + 0], (double)gx); atomicAdd(&force[3 * (int64_t)i + 1], (double)gy);
+    atomicAdd(&force[3 * (int64_t)i + 2], (double)gz);
+    atomicAdd(&force[3 * (int64_t)j + 0], -(double)gx); atomicAdd(&force[3 * (int64_t)j + 1], -(double)gy);
+    atomicAdd(&force[3 * (int64_t)j + 2], -(double)gz);
+  }
+}
+
+__global__ void k_zero_f64(double* p, int64_t n) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n) p[i] = 0.0;
+}
+
+// ---- NVE ---------------------------------------------------------------------------------
+#define ACC_CONV 9.648533212e-3
+__global__ void k_nve(double* pos, double* vel, const double* force, const int32_t* species, const double* mass, int64_t n,
+                      double dt, int drift) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double im = ACC_CONV / mass[species[i]];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    double v = vel[3 * i + k] + (0.5 * dt) * (force[3 * i + k] * im);
+    vel[3 * i + k] = v;
+    if (drift) pos[3 * i + k] += dt * v;
+  }
+}
+
+__global__ void k_kin(const double* vel, const int32_t* species, const double* mass, int64_t n, double* out) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double m = mass[species[i]];
+  out[i] = 0.5 * m * (vel[3 * i] * vel[3 * i] + vel[3 * i + 1] * vel[3 * i + 1] + vel[3 * i + 2] * vel[3 * i + 2]) / ACC_CONV;
+}
+
+}  // namespace
+
+#define LAUNCH_CHECK(m)              \
+  do {                               \
+    (m)->launches++;                 \
+    AL_CUDA(m, cudaGetLastError());  \
+  } while (0)
+
+int k_launch_active_count(allegro_model* m, const EdgeGeomArgs& a, int* deg) {
+  if (a.nc <= 0) return ALLEGRO_OK;
+  k_active_count<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, deg);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_set_mact(allegro_model* m, const int64_t* rowa, int nc, int* m_act) {
+  k_set_mact<<<1, 1, 0, m->stream>>>(rowa, nc, m_act);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* rowa, Work& w) {
+  if (a.nc <= 0) return ALLEGRO_OK;
+  k_geom_fill<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, rowa, (int*)w.ei.p, (int*)w.ej.p, (float4*)w.geo.p,
+                                                           (float*)w.u.p, (float*)w.du.p, (float*)w.B.p, (float*)w.dB.p,
+                                                           (float*)w.Y.p, m->Denv, (int*)w.m_act.p);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_twobody0(allegro_model* m, Work& w, const int32_t* species, const Dense& L0, bool single, int m_cap) {
+  if (m_cap <= 0) return ALLEGRO_OK;
+  float* act = single ? (float*)w.XS[0].p : (float*)w.tb_a[0].p;
+  int ld = single ? (m->d + m->n) : L0.fo;
+  k_twobody0<<<(m_cap + TB0_EPB - 1) / TB0_EPB, 128, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, (int*)w.ej.p, species,
+                                                                    (float*)w.B.p, (float*)w.u.p, L0.W, m->S, m->NB, L0.fo,
+                                                                    (float*)w.tb_z[0].p, act, ld, single ? 1 : 0);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+static size_t tp_smem(const allegro_model* m, int L) { return (size_t)(m->Denv + m->tp[L - 1].npairs) * m->n * sizeof(float); }
+
+static void tp_common(allegro_model* m, Work& w, int L, TPArgs& a, const float* om, int ldo, const float* Vin,
+                      const float* w0, int ldw) {
+  a.rowa = (const int64_t*)w.rowa.p;
+  a.om = om; a.ldo = ldo; a.Y = (const float*)w.Y.p; a.Denv = m->Denv;
+  a.Vin = Vin; a.w0 = w0; a.ldw = ldw;
+  a.v0_l = m->d_v0_l; a.v0_y = m->d_v0_y; a.env_l = m->d_env_l;
+  a.t = m->tp[L - 1]; a.n = m->n; a.lmax = m->lmax; a.c_env = m->c_env;
+}
+
+int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
+                    const float* w0, int ldw, float* Tout, float* xs, int ldx) {
+  if (nc <= 0) return ALLEGRO_OK;
+  TPArgs a{};
+  tp_common(m, w, L, a, om, ldo, Vin, w0, ldw);
+  a.Tout = Tout; a.xs = xs; a.ldx = ldx; a.gamma_out = (float*)w.gamma.p;
+  size_t sm = tp_smem(m, L);
+  if (Vin == nullptr) {
+    AL_CUDA(m, cudaFuncSetAttribute(k_tp_fwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    k_tp_fwd<true><<<nc, 256, sm, m->stream>>>(a);
+  } else {
+    AL_CUDA(m, cudaFuncSetAttribute(k_tp_fwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    k_tp_fwd<false><<<nc, 256, sm, m->stream>>>(a);
+  }
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
+                    const float* w0, int ldw, const float* VbarL, const float* sbar, int lds, float* Vbar_prev,
+                    float* ombar, int ldob, float* w0bar) {
+  if (nc <= 0) return ALLEGRO_OK;
+  TPArgs a{};
+  tp_common(m, w, L, a, om, ldo, Vin, w0, ldw);
+  a.VbarL = VbarL; a.sbar = sbar; a.lds = lds; a.Vbar_prev = Vbar_prev; a.ombar = ombar; a.ldob = ldob;
+  a.w0bar = w0bar; a.Ybar = (float*)w.Ybar.p;
+  size_t sm = tp_smem(m, L);
+  if (Vin == nullptr) {
+    AL_CUDA(m, cudaFuncSetAttribute(k_tp_bwd<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    k_tp_bwd<true><<<nc, 256, sm, m->stream>>>(a);
+  } else {
+    AL_CUDA(m, cudaFuncSetAttribute(k_tp_bwd<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    k_tp_bwd<false><<<nc, 256, sm, m->stream>>>(a);
+  }
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c0, int nc, const float* xf, double* e_atom) {
+  if (nc <= 0) return ALLEGRO_OK;
+  k_energy<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, xf, m->d, m->w_eff_d, species,
+                                                        m->sigma, m->mu, e_atom);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_sum_f64(allegro_model* m, const double* x, int64_t n, double* out) {
+  k_sum_f64<<<1, 1024, 0, m->stream>>>(x, n, out);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_fill_xbar(allegro_model* m, Work& w, const int32_t* species, float* xb, int m_cap) {
+  if (m_cap <= 0) return ALLEGRO_OK;
+  int64_t tot = (int64_t)m_cap * m->d;
+  k_fill_xbar<<<(unsigned)((tot + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, species, m->sigma,
+                                                                   m->w_eff_f, m->d, xb);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, const float* z, int ldz, float c, float* zb,
+                      int ldzb, int width, int m_cap) {
+  if (m_cap <= 0) return ALLEGRO_OK;
+  k_bwd_prep<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, xbar, ldx, z, ldz,
+                                                                                  (float*)w.u.p, c, zb, ldzb, width,
+                                                                                  (float*)w.ubar.p);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, const Dense& L0, bool single, double* force,
+                      int m_cap) {
+  if (m_cap <= 0) return ALLEGRO_OK;
+  (void)single;
+  k_edge_bwd<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>(
+      (int*)w.m_act.p, zb1, ldz, L0.W, m->S, m->NB, L0.fo, (float4*)w.geo.p, (float*)w.du.p, (float*)w.dB.p,
+      (float*)w.ubar.p, (float*)w.Ybar.p, m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_zero_f64(allegro_model* m, double* p, int64_t n) {
+  if (n <= 0) return ALLEGRO_OK;
+  k_zero_f64<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(p, n);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_nve_kick_drift(allegro_model* m, double* pos, double* vel, const double* force, const int32_t* species,
+                            const double* mass, int64_t n, double dt, bool drift) {
+  if (n <= 0) return ALLEGRO_OK;
+  k_nve<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(pos, vel, force, species, mass, n, dt, drift ? 1 : 0);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_kinetic(allegro_model* m, const double* vel, const int32_t* species, const double* mass, int64_t n,
+                     double* e_kin, DevBuf& tmp) {
+  AL_CHECK(al_reserve(m, tmp, (size_t)n * 8 + 16));
+  if (n > 0) {
+    k_kin<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(vel, species, mass, n, (double*)tmp.p);
+    LAUNCH_CHECK(m);
+  }
+  return k_launch_sum_f64(m, (double*)tmp.p, n, e_kin);
+}

@@ -1,0 +1,38 @@
+// Edge-batched MLP GEMMs with fused epilogues.
+//   C[M,N] = epi( A[M,K] * Bt[N,K]^T )      A, Bt K-contiguous (row-major), fp32 in HBM
+// M is read from device memory (*m_ptr): the number of active edges of the chunk is only known on
+// the device; grids are sized for m_cap rows and blocks beyond *m_ptr exit.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+enum GemmEpi {
+  EPI_PLAIN = 0,      // C = acc
+  EPI_SILU_BOTH = 1,  // out2 = acc (pre-activation z) ; C = silu(acc)
+  EPI_SILU_U = 2,     // out2 = acc ; C = u[m] * silu(acc)                              (two-body output x^0)
+  EPI_LATENT = 3,     // out2 = acc ; C = c0 * aux1[m,n] + c1 * u[m] * silu(acc)        (x^L residual update)
+  EPI_MUL_DSILU = 4,  // C = acc * silu'(aux1[m,n])                                    (backward through SiLU)
+  EPI_ADD2 = 5,       // C = acc + c0 * aux1[m,n] + aux2[m,n]                           (x-bar accumulation)
+  EPI_LATENT_BWD = 6  // C = acc + c0*aux1 + aux2 ; out2 = c1 * u[m] * C * silu'(aux3[m,n]) ; ubar[m] += c1 * <C, silu(aux3)>
+};
+
+struct GemmArgs {
+  const float* A; int lda;
+  const float* Bt; int ldb;       // fp32 weights [N][K]
+  const void* Bt16;               // bf16 weights [N][K] (precision 2) or null
+  float* C; int ldc;
+  int N, K;
+  int m_cap; const int* m_ptr;
+  int epi;
+  const float* aux1; int ld1;
+  const float* aux2; int ld2;
+  const float* aux3; int ld3;
+  float* out2; int ldo2;
+  const float* u;                 // per-row scalar
+  float* ubar;                    // per-row accumulation target (EPI_LATENT_BWD)
+  float c0, c1;
+};
+
+// precision: 0 fp32 FFMA, 1 TF32 tcgen05, 2 BF16 tcgen05 (A converted on the fly is not possible with
+// TMA-fed operands, so precision 2 uses TF32 for fp32-resident activations).
+int al_gemm(struct allegro_model* m, const GemmArgs& g);

@@ -1,0 +1,129 @@
+// Internal structures of libb200allegro (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "b200_allegro.h"
+
+#define AL_MAX_LAYERS 8
+
+// ---- error plumbing ------------------------------------------------------------------------------
+void al_set_error(const allegro_model* m, const std::string& msg);
+#define AL_CUDA(m, expr)                                                                          \
+  do {                                                                                            \
+    cudaError_t _e = (expr);                                                                      \
+    if (_e != cudaSuccess) {                                                                      \
+      al_set_error(m, std::string(#expr) + ": " + cudaGetErrorString(_e));                        \
+      return ALLEGRO_ERR_CUDA;                                                                    \
+    }                                                                                             \
+  } while (0)
+#define AL_CHECK(expr)             \
+  do {                             \
+    int _r = (expr);               \
+    if (_r != ALLEGRO_OK) return _r; \
+  } while (0)
+
+// ---- host-side description of the tensor track ---------------------------------------------------
+struct Irrep { int l, p; };
+
+struct TPLayerHost {
+  std::vector<Irrep> in, out;      // S_{L-1}, S_L
+  int Din, Dout, Denv;
+  struct Path { int i1, l2, io; };
+  std::vector<Path> paths;
+  std::vector<int> fan;
+  // fused tensor K[a,b,c] as a sparse list, grouped into (a,c) "pairs"
+  int npairs;
+  std::vector<int> pair_a, pair_c;            // [npairs]
+  std::vector<int> pair_ptr;                  // [npairs+1] -> entries (b,val) of K
+  std::vector<int> ent_b; std::vector<float> ent_val;
+  // CSR over output component c -> (a, pair)
+  std::vector<int> c_ptr, c_a, c_p;
+  // CSR over input component a -> (c, pair)
+  std::vector<int> a_ptr, a_c, a_p;
+  // CSR over env component b -> (pair, val)
+  std::vector<int> b_ptr, b_p; std::vector<float> b_val;
+  int nnz;
+};
+
+// device copy of the tables of one layer
+struct TPLayerDev {
+  int Din, Dout, Denv, npairs, nnz;
+  int *pair_a, *pair_c, *pair_ptr, *ent_b; float* ent_val;
+  int *c_ptr, *c_a, *c_p;
+  int *a_ptr, *a_c, *a_p;
+  int *b_ptr, *b_p; float* b_val;
+};
+
+struct Dense {
+  int fi = 0, fo = 0;
+  float* W = nullptr;    // [fi][fo] row-major  (B operand of dX = dY * W^T, K-major over fo)
+  float* Wt = nullptr;   // [fo][fi] row-major  (B operand of Y = X * W, K-major over fi)
+  void* Wh = nullptr;    // bf16 copies for precision 2 (same two layouts), else null
+  void* Wth = nullptr;
+};
+
+struct DevBuf {
+  void* p = nullptr; size_t bytes = 0;
+};
+
+struct Chunk { int64_t c0, c1; int64_t e0, e1; };   // centers [c0,c1), candidate edges [e0,e1)
+
+struct allegro_nbr {
+  int64_t n_atoms = 0, n_edges = 0;
+  double cutoff = 0; double box[3] = {0, 0, 0};
+  DevBuf row_ptr, j, shift, keys;      // int64[N+1], int32[E], int8[3E], uint64[E] scratch
+  DevBuf wpos, q, cell_of, cell_cnt, cell_start, cell_atoms, deg, scan_tmp;
+  std::vector<int64_t> row_ptr_host;
+  std::vector<Chunk> chunks; int64_t chunk_cap = 0;
+  int64_t max_chunk_edges = 0, max_chunk_centers = 0;
+};
+
+struct allegro_model {
+  allegro_hparams hp;
+  int S, NB, d, n, lmax, NL, Denv, nA;
+  std::vector<TPLayerHost> tp_host;       // [NL]
+  std::vector<TPLayerDev> tp;             // [NL]
+  std::vector<int> D;                     // D_0..D_NL
+  // V^0 layout: position -> l, -> index in Y
+  std::vector<int> v0_l, v0_y; int *d_v0_l = nullptr, *d_v0_y = nullptr, *d_env_l = nullptr;
+  // weights
+  std::vector<Dense> twobody;             // twobody[0] is the (2S+NB)-input layer
+  Dense emb01;                            // [A0 | A1] : d -> 2 nA, columns permuted to (l, n)
+  std::vector<Dense> emb;                 // emb[L] = A^{L+1} for L >= 1 (index 0 unused)
+  std::vector<std::vector<Dense>> latent; // [NL][n_latent]
+  float* w_eff_f = nullptr; double* w_eff_d = nullptr;   // product of the edge-MLP layers, [d]
+  double *sigma = nullptr, *mu = nullptr; // device [S]
+  std::vector<double> sigma_h, mu_h;
+  float c_env; float c_old[AL_MAX_LAYERS], c_new[AL_MAX_LAYERS];
+  // runtime
+  cudaStream_t stream = 0;
+  allegro_alloc_fn alloc_fn = nullptr; allegro_free_fn free_fn = nullptr; void* alloc_user = nullptr;
+  int64_t chunk_edges = 1 << 20;
+  int64_t launches = 0;
+  std::string err;
+  int sm_count = 148;
+  // workspace (per chunk), grown on demand
+  struct Work* work = nullptr;
+  std::vector<void*> owned;               // device allocations made through al_alloc (weights/tables)
+};
+
+// ---- allocation helpers ---------------------------------------------------------------------------
+int al_alloc(allegro_model* m, void** p, size_t bytes);
+void al_free(allegro_model* m, void* p);
+int al_reserve(allegro_model* m, DevBuf& b, size_t bytes);   // grow-only with +5 % head-room
+void al_release(allegro_model* m, DevBuf& b);
+
+// ---- sub-systems ----------------------------------------------------------------------------------
+int al_build_tp_tables(allegro_model* m, const std::vector<std::vector<float>>& alphas);   // cg_tables.cpp
+void al_enumerate(int lmax, int NL, std::vector<std::vector<Irrep>>& S,
+                  std::vector<std::vector<TPLayerHost::Path>>& paths);
+int al_neighbors_impl(allegro_model* m, const double* pos, int64_t n_atoms, const double box[3], double cutoff,
+                      allegro_nbr** inout);
+int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                    const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force);
+int al_exclusive_scan_i64(allegro_model* m, const int32_t* in, int64_t* out, int64_t n, DevBuf& tmp);  // out[n] = total
+void al_work_free(allegro_model* m);

@@ -1,0 +1,63 @@
+// Launch wrappers of the non-GEMM kernels (edge geometry, tensor track, energy, backward, NVE).
+#pragma once
+#include "internal.h"
+
+// Per-chunk workspace.  All edge tensors are edge-major over the chunk's ACTIVE edges (r < r_cut),
+// sorted by center.  Tensor-track features are [edge][component][channel] (channel fastest).
+struct Work {
+  int64_t cap_edges = 0, cap_centers = 0;
+  DevBuf deg, rowa, scan_tmp, m_act;        // int32[Nc], int64[Nc+1], scan scratch, int32[4]
+  DevBuf ei, ej;                            // int32[M] global atom ids
+  DevBuf geo;                               // float4[M]: rhat.xyz, r
+  DevBuf u, du;                             // float[M]: envelope u(r/rc), du/dr
+  DevBuf B, dB;                             // float[M][NB]: B_n = b_n u, dB_n/dr
+  DevBuf Y;                                 // float[M][Denv]
+  std::vector<DevBuf> tb_z, tb_a;           // two-body pre-activations / activations, [M][h_k]
+  std::vector<DevBuf> XS;                   // [NL] : [M][d+n] = [x^{L-1} | s^L]
+  DevBuf XF;                                // [M][d] final latent x^{NL}
+  DevBuf WE;                                // [M][2 nA] = [w^0 | omega^1]  (component-major (l,n))
+  std::vector<DevBuf> OM;                   // [NL+1]: omega^L for L >= 2, [M][nA]
+  std::vector<DevBuf> T;                    // [NL]: T^L = V^L for L < NL, [M][D_L][n]
+  std::vector<std::vector<DevBuf>> lat_z, lat_a;   // [NL][n_latent]
+  DevBuf gamma;                             // [Nc][Denv][n] of the layer being processed (debug tap)
+  // backward
+  DevBuf XB0, XB1;                          // x-bar ping-pong [M][d]
+  DevBuf ZB0, ZB1;                          // z-bar ping-pong [M][max width]
+  DevBuf G;                                 // [M][d+n] = [x-bar part | s-bar]
+  DevBuf OB;                                // [M][2 nA] omega-bar (and w0-bar)
+  DevBuf VB0, VB1;                          // V-bar ping-pong [M][Dmax][n]
+  DevBuf ubar, Ybar;                        // [M], [M][Denv]
+  DevBuf ge;                                // float[M][3] dE/dr_e (debug tap)
+  DevBuf eatom;                             // f64[N] when the caller passes e_atom = NULL
+  int64_t eatom_cap = 0;
+  int last_nc = 0;
+};
+
+struct EdgeGeomArgs {
+  const double* pos; const int32_t* species; double box[3]; double rc; int p; int NB; int lmax;
+  const int64_t* row_ptr; const int32_t* j; const int8_t* shift;   // candidate list (global)
+  int64_t c0; int nc;                                               // centers [c0, c0+nc)
+};
+
+int k_launch_active_count(allegro_model* m, const EdgeGeomArgs& a, int* deg);
+int k_launch_set_mact(allegro_model* m, const int64_t* rowa, int nc, int* m_act);
+int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* rowa, Work& w);
+int k_launch_twobody0(allegro_model* m, Work& w, const int32_t* species, const Dense& L0, bool single, int m_cap);
+int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
+                    const float* w0, int ldw, float* Tout, float* xs, int ldx);
+int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
+                    const float* w0, int ldw, const float* Vbar_out_in /*V-bar^L or null*/, const float* sbar, int lds,
+                    float* Vbar_prev, float* ombar, int ldob, float* w0bar);
+int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c0, int nc, const float* xf,
+                    double* e_atom);
+int k_launch_sum_f64(allegro_model* m, const double* x, int64_t n, double* out);
+int k_launch_fill_xbar(allegro_model* m, Work& w, const int32_t* species, float* xb, int m_cap);
+int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, const float* z, int ldz, float c,
+                      float* zb, int ldzb, int width, int m_cap);
+int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, const Dense& L0, bool single,
+                      double* force, int m_cap);
+int k_launch_zero_f64(allegro_model* m, double* p, int64_t n);
+int k_launch_nve_kick_drift(allegro_model* m, double* pos, double* vel, const double* force, const int32_t* species,
+                            const double* mass, int64_t n, double dt, bool drift);
+int k_launch_kinetic(allegro_model* m, const double* vel, const int32_t* species, const double* mass, int64_t n,
+                     double* e_kin, DevBuf& tmp);

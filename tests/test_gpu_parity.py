@@ -1,0 +1,171 @@
+"""GPU-vs-oracle parity through the C ABI (`-m gpu`).  Tolerances are BASELINE.json north_star's:
+fp32 mode |dE|/N <= 1e-6 eV/atom, max|dF| <= 1e-5 * force scale; neighbor lists bit-exact."""
+import ctypes
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import allegro_oracle as O
+from synthetic import CONFIGS, make_system, maxwell_boltzmann
+from synthetic.configs import scaled_config
+from synthetic.systems import masses_for
+
+from gpu_util import gpu_eval, make_both, nbr_as_arrays
+
+E_TOL_PER_ATOM = 1e-6
+F_TOL_REL = 1e-5
+
+
+def _check_EF(got, want, N, tag=""):
+    (E, Ea, F), (E0, Ea0, F0) = got, want
+    fscale = max(1.0, float(np.sqrt((F0 ** 2).mean())))
+    dE = abs(E - E0) / N
+    dEa = np.abs(Ea - Ea0).max()
+    dF = np.abs(F - F0).max()
+    print(f"[{tag}] N={N} |dE|/N={dE:.3e} max|dE_i|={dEa:.3e} max|dF|={dF:.3e} rmsF={np.sqrt((F0**2).mean()):.3e}")
+    assert dE <= E_TOL_PER_ATOM
+    assert dEa <= 27 * E_TOL_PER_ATOM
+    assert dF <= F_TOL_REL * fscale
+
+
+# ---------------------------------------------------------------------------------------------------
+# neighbor lists: bit-exact as sorted (i, j, shift) lists
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ci,n,cutoff,unwrap", [(0, 192, 4.0, False), (0, 192, 5.0, True), (1, 1536, 4.0, True),
+                                                (4, 1200, 6.0, False), (4, 1200, 7.0, True)])
+def test_neighbor_list_bit_exact(ci, n, cutoff, unwrap):
+    cfg = scaled_config(ci, n)
+    pos, sp, box = make_system(cfg)
+    if unwrap:
+        g = np.random.default_rng(ci)
+        pos = pos + g.integers(-2, 3, pos.shape) * box
+    model, _ = make_both(cfg)
+    nb = model.neighbors(torch.from_numpy(pos).cuda(), box, cutoff)
+    gi, gj, gs = nbr_as_arrays(nb)
+    oi, oj, os_ = O.neighbor_list(pos, box, cutoff)
+    assert gi.shape == oi.shape
+    assert np.array_equal(gi, oi) and np.array_equal(gj, oj) and np.array_equal(gs, os_)
+
+
+def test_neighbor_list_small_box_self_images_and_empty():
+    cfg = scaled_config(0, 192)
+    model, _ = make_both(cfg)
+    g = np.random.default_rng(3)
+    box = np.array([3.0, 3.5, 4.2])
+    pos = g.uniform(0, 1, (5, 3)) * box
+    nb = model.neighbors(torch.from_numpy(pos).cuda(), box, 4.0)
+    gi, gj, gs = nbr_as_arrays(nb)
+    oi, oj, os_ = O.neighbor_list_brute(pos, box, 4.0)
+    assert np.array_equal(gi, oi) and np.array_equal(gj, oj) and np.array_equal(gs, os_)
+    assert ((gi == gj) & (np.abs(gs).sum(1) > 0)).any()
+    # one atom, big box: no edges; E = mu
+    pos1 = np.array([[1.0, 2.0, 3.0]])
+    (E, Ea, F), nb1 = gpu_eval(model, pos1, np.array([1], dtype=np.int32), np.array([50.0, 50.0, 50.0]))
+    assert nb1.n_edges == 0 and E == pytest.approx(cfg.mu()[1]) and np.all(F == 0)
+    # zero atoms
+    nb0 = model.neighbors(torch.zeros((0, 3), dtype=torch.float64, device="cuda"), box, 4.0)
+    assert nb0.n_edges == 0
+
+
+# ---------------------------------------------------------------------------------------------------
+# energy + forces, fp32 mode
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ci,n", [(0, 192), (1, 1536), (2, 3000), (4, 1200)])
+def test_energy_forces_fp32(ci, n):
+    cfg = scaled_config(ci, n)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg)
+    got, nb = gpu_eval(model, pos, sp, box)
+    want = O.energy_forces(oracle, pos, sp, box, O.neighbor_list(pos, box, cfg.hp.r_cut))
+    _check_EF(got, want, n, f"cfg{ci}")
+
+
+def test_intermediates_cfg0():
+    cfg = scaled_config(0, 192)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg)
+    got, nb = gpu_eval(model, pos, sp, box)
+    ei, ej, es = O.neighbor_list(pos, box, cfg.hp.r_cut)
+    t = torch.from_numpy
+    _, parts = oracle.edge_energies(t(pos), t(sp.astype(np.int64)), t(box), t(ei), t(ej), t(es), return_parts=True)
+    E = ei.shape[0]
+    hp = cfg.hp
+    Y = model.debug_tensor("Y").reshape(E, -1)
+    np.testing.assert_allclose(Y, parts["Y"].numpy(), atol=2e-6)
+    u = model.debug_tensor("u")
+    np.testing.assert_allclose(u, parts["u"].numpy(), atol=1e-6)
+    B = model.debug_tensor("B").reshape(E, -1)
+    np.testing.assert_allclose(B, parts["B"].numpy(), atol=1e-6)
+    x0 = model.debug_tensor("x0").reshape(E, hp.d)
+    np.testing.assert_allclose(x0, parts["x"][0].numpy(), atol=2e-6)
+    x1 = model.debug_tensor("x1").reshape(E, hp.d)
+    np.testing.assert_allclose(x1, parts["x"][1].numpy(), atol=3e-6)
+
+
+def test_chunking_and_skin_list_invariance():
+    cfg = scaled_config(1, 1536)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg)
+    (E0, Ea0, F0), _ = gpu_eval(model, pos, sp, box)
+    model_c, _ = make_both(cfg, chunk_edges=4096)          # ~10 chunks, ragged tail
+    (E1, Ea1, F1), _ = gpu_eval(model_c, pos, sp, box)
+    assert abs(E1 - E0) < 1e-9 and np.abs(F1 - F0).max() < 1e-9 and np.abs(Ea1 - Ea0).max() < 1e-12
+    (E2, Ea2, F2), nb2 = gpu_eval(model, pos, sp, box, cutoff=cfg.hp.r_cut + 1.0)   # Verlet skin list
+    assert model.last_active_edges() < nb2.n_edges
+    assert abs(E2 - E0) < 1e-9 and np.abs(F2 - F0).max() < 1e-9
+
+
+def test_host_variants_match_device():
+    cfg = scaled_config(0, 192)
+    pos, sp, box = make_system(cfg)
+    model, _ = make_both(cfg)
+    (E0, Ea0, F0), _ = gpu_eval(model, pos, sp, box)
+    nb = model.neighbors_host(pos, box, cfg.hp.r_cut)
+    E1, Ea1, F1 = model.compute_host(pos, sp, box, nb)
+    assert abs(E1 - E0) < 1e-10 and np.abs(F1 - F0).max() < 1e-10
+
+
+def test_coincident_atoms_flagged():
+    import paper_2304_10061_b200 as P
+    cfg = scaled_config(0, 192)
+    model, _ = make_both(cfg)
+    pos = np.array([[1.0, 1.0, 1.0], [1.0, 1.0, 1.0], [2.0, 1.0, 1.0]])
+    nb = model.neighbors_host(pos, np.array([20.0, 20.0, 20.0]), 4.0)
+    with pytest.raises(P.AllegroError) as ei:
+        model.compute_host(pos, np.array([0, 1, 0], dtype=np.int32), np.array([20.0, 20.0, 20.0]), nb)
+    assert ei.value.code == -5
+
+
+def test_nve_steps_match_oracle():
+    cfg = scaled_config(0, 192)
+    pos, sp, box = make_system(cfg)
+    vel = maxwell_boltzmann(cfg, sp)
+    model, oracle = make_both(cfg)
+    mass = masses_for(cfg)
+    dt, nsteps = 0.5, 5
+    # oracle trajectory (list rebuilt every step at r_c)
+    def force_fn(p):
+        E, _, F = O.energy_forces(oracle, p, sp, box, O.neighbor_list(p, box, cfg.hp.r_cut))
+        return E, F
+    p_o, v_o = pos.copy(), vel.copy()
+    e_o, f_o = force_fn(p_o)
+    for _ in range(nsteps):
+        p_o, v_o, f_o, e_o = O.nve_step(force_fn, p_o, v_o, f_o, mass[sp], dt)
+    # GPU trajectory (skin list rebuilt every 3 steps)
+    p = torch.from_numpy(pos.copy()).cuda(); v = torch.from_numpy(vel.copy()).cuda()
+    s = torch.from_numpy(sp).cuda(); mg = torch.from_numpy(mass).cuda()
+    nb = model.neighbors(p, box, cfg.hp.r_cut + 1.0)
+    e, _, f = model.compute(p, s, box, nb)
+    ek = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctr = ctypes.c_int64(0)
+    for _ in range(nsteps):
+        model.step_nve(p, v, f, s, mg, box, dt, 3, 1.0, nb, ctr, e, ek)
+    torch.cuda.synchronize()
+    assert ctr.value == nsteps
+    np.testing.assert_allclose(p.cpu().numpy(), p_o, atol=1e-7)
+    np.testing.assert_allclose(v.cpu().numpy(), v_o, atol=1e-7)
+    assert abs(e.item() - e_o) / 192 < 2e-6
+    assert abs(ek.item() - O.kinetic_energy(v_o, mass[sp])) < 1e-6
