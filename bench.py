@@ -1,0 +1,276 @@
+#!/usr/bin/env python
+"""bench.py — atom-steps/s of the Allegro energy+force hot path on B200 (BASELINE.json metric).
+
+A "step" is one pass of the whole hot path: one velocity-Verlet NVE step
+through the C ABI (`allegro_step_nve`): half-kick + drift, neighbor rebuild when due (every
+`rebuild_every` steps at r_c + skin), active-edge compaction + edge basis, two-body MLP, Allegro layers,
+edge energies, fp64 sums, analytic backward, force scatter, half-kick, kinetic energy.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--precision 1] [--impl ours|reference]
+
+N > 1: launched by torchrun, one rank per GPU.  The path does not shard in this build (north_star: one
+GPU, no collectives) -> "replicas only": every rank runs an independent replica of the same workload;
+value = sum of atom-steps over ranks / max-over-ranks device time.
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+FFMA_LANES_PER_SM = 128          # B200_PROFILING.md / blackwell guide: 4 SMSP x 32 fp32 FMA lanes
+TF32_OVER_BF16 = 0.5             # nominal dense ratio (B200_PROFILING.md table: 1.1 vs 2.25 PFLOP/s)
+
+
+def gemm_macs_per_edge(hp):
+    """Algorithmic MACs per ACTIVE edge of the GEMM kernel group, forward + backward (dX only)."""
+    d, n, nA = hp.twobody_dims[-1], hp.n_tensor, hp.n_tensor * (hp.l_max + 1)
+    tb = sum(a * b for a, b in zip(hp.twobody_dims[:-1], hp.twobody_dims[1:]))
+    lat = (d + n) * hp.latent_dims[0] + sum(a * b for a, b in zip(hp.latent_dims[:-1], hp.latent_dims[1:]))
+    fwd = tb + d * 2 * nA + hp.n_layers * lat + (hp.n_layers - 1) * d * nA
+    bwd = tb + hp.n_layers * lat + 2 * nA * d + (hp.n_layers - 1) * nA * d
+    return fwd + bwd
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        super().__init__(daemon=True)
+        self.gpu, self.samples, self.stop_flag = gpu_index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(s[2 + k].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return {"hbm_gbs": j["hbm_gbs"], "bf16_burst": j["bf16_tflops"], "bf16_sustained": j["bf16_tflops_sustained"],
+                "sm_max_mhz": j.get("sm_max_mhz", 1965.0), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+def oracle_sample(cfg, pos, sp, box, n_centers):
+    """Energy + forces of `n_centers` contiguous centres by the fp64 oracle (cpu_baseline / reference arm)."""
+    import torch
+    from oracle import allegro_oracle as O
+    from synthetic import make_blob
+    hp = cfg.hp
+    blob = make_blob(hp, O.path_fan(hp.l_max, hp.n_layers), [cfg.sigma] * hp.n_species, cfg.mu(), cfg.weight_seed)
+    om = O.OracleModel(hp, blob)
+    nbr = O.neighbor_list(pos, box, hp.r_cut)
+    centers = np.arange(min(n_centers, pos.shape[0]))
+
+    def run():
+        t0 = time.perf_counter()
+        O.energy_forces(om, pos, sp, box, nbr, centers=centers)
+        return time.perf_counter() - t0
+    return run, centers.size, torch.get_num_threads()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--precision", type=int, default=1, help="0 fp32 FFMA, 1 TF32 tensor cores")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    K, W = args.steps, max(args.warmup, 3)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from synthetic import CONFIGS, make_blob, make_system, maxwell_boltzmann
+    from synthetic.systems import masses_for
+    cfg = CONFIGS[args.config]
+    workload = f"config{cfg.index}:{cfg.name}"
+    metric, unit = "atom-steps/s (energy+forces, 1 B200)", "atom-steps/s"
+
+    # ---------------------------------------------------------------- reference arm = the oracle on host cores
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        pos, sp, box = make_system(cfg)
+        n_c = {0: 192, 1: 96, 2: 32, 3: 32, 4: 24}[cfg.index]
+        run, n_c, cores = oracle_sample(cfg, pos, sp, box, n_c)
+        for _ in range(min(W, 3)):
+            run()
+        t = sum(run() for _ in range(K))
+        val = n_c * K / t
+        print(json.dumps({
+            "impl": "reference", "metric": metric, "value": val, "unit": unit, "n_gpus": args.gpus, "steps": K,
+            "warmup": min(W, 3), "ms_per_step": 1e3 * t / K, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload, "n_atoms": int(pos.shape[0]), "sample": f"{n_c} contiguous centres per step"},
+            "cpu_baseline": {"value": val, "unit": unit, "cores": cores, "kind": "oracle",
+                             "sample": f"energy+forces of {n_c} centres (all their edges) of {workload}, per step"},
+            "e2e": {"value": val, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+        return
+
+    # ---------------------------------------------------------------- our arm
+    import torch
+    import paper_2304_10061_b200 as P
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device: the hot path has no CPU fallback"
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    pos, sp, box = make_system(cfg)
+    vel = maxwell_boltzmann(cfg, sp)
+    N = pos.shape[0]
+    chp = P.hparams_from(cfg.hp, args.precision)
+    blob = make_blob(cfg.hp, P.path_fan(chp), [cfg.sigma] * cfg.hp.n_species, cfg.mu(), cfg.weight_seed)
+    model = P.Allegro(chp, blob)
+    dev = torch.device("cuda", local_rank)
+    p = torch.from_numpy(pos.copy()).to(dev); v = torch.from_numpy(vel.copy()).to(dev)
+    s = torch.from_numpy(sp).to(dev); mass = torch.from_numpy(masses_for(cfg)).to(dev)
+    nb = model.neighbors(p, box, cfg.hp.r_cut + cfg.skin)
+    e, _, f = model.compute(p, s, box, nb, want_atom_energies=False)
+    ek = torch.zeros(1, dtype=torch.float64, device=dev)
+    ctr = ctypes.c_int64(0)
+
+    def step():
+        model.step_nve(p, v, f, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, e, ek)
+
+    for _ in range(W):
+        step()
+    barrier()
+    l0 = model.launches
+    sampler = ClockSampler(local_rank); sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    for _ in range(K):
+        step()
+    ev1.record()
+    barrier()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
+    launches = model.launches - l0
+    n_active = model.last_active_edges()
+    e_pot, e_kin = float(e.item()), float(ek.item())
+    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_max = float(t_ms.item())
+    value = world * N * K / (ms_max * 1e-3)
+
+    # ---- e2e: the same step through the C ABI with HOST (pinned) buffers, copies inside the timed region
+    hp_ = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    ph, vh, fh = hp_(p.cpu().numpy()), hp_(v.cpu().numpy()), hp_(f.cpu().numpy())
+    sh, mh = hp_(sp), hp_(masses_for(cfg))
+    eh, ekh = torch.zeros(1, dtype=torch.float64).pin_memory(), torch.zeros(1, dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        model.step_nve_host(ph, vh, fh, sh, mh, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, eh, ekh)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(K):
+        model.step_nve_host(ph, vh, fh, sh, mh, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, eh, ekh)
+    torch.cuda.synchronize()
+    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
+    e2e_val = world * N * K / float(t_e2e.item())
+    h2d = 3 * N * 24 + N * 4 + cfg.hp.n_species * 8
+    d2h = 3 * N * 24 + 16
+
+    # ---- roofline of the dominant kernel group: second pass of K steps with per-group CUDA events
+    groups = ["gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd", "neighbors", "nve"]
+    model.profile_enable(True)
+    for _ in range(K):
+        model.step_nve(p, v, f, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, e, ek)
+    prof = {g: model.profile_read(g) for g in groups}
+    model.profile_enable(False)
+    tot_prof = sum(t for t, _ in prof.values())
+    pk = peaks()
+    gemm_ms, gemm_n = prof["gemm"]
+    flops_per_step = 2.0 * gemm_macs_per_edge(cfg.hp) * n_active
+    gemm_tflops = flops_per_step * K / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+    if args.precision == 0:
+        # fp32 FFMA peak = SMs x 128 lanes x 2 flop x max SM clock (unit counts: blackwell guide; clock: MEASURED_PEAKS)
+        nsm = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak, bound = nsm * FFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12, "alu"
+        peak_note = f"{nsm} SMs x {FFMA_LANES_PER_SM} FFMA lanes x 2 x {pk['sm_max_mhz']} MHz"
+    else:
+        peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16, "tensor"
+        peak_note = f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16}"
+    roofline = {"bound": bound, "kernel": "MLP GEMM group (fwd+bwd)", "achieved": gemm_tflops, "peak": peak,
+                "unit": "TFLOP/s", "frac": gemm_tflops / peak if peak else None, "traffic": None,
+                "peak_note": peak_note, "launches_per_step": gemm_n / K, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
+                "share_of_step": gemm_ms / tot_prof if tot_prof else None,
+                "groups_ms_per_step": {g: round(t / K, 4) for g, (t, _) in prof.items()}}
+
+    out = {
+        "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
+        "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {0: "f32", 1: "tf32", 2: "bf16"}[args.precision], "data": "synthetic",
+        "config": {"workload": workload, "n_atoms": N, "active_edges": n_active, "candidate_edges": nb.n_edges,
+                   "precision_mode": args.precision, "dt_fs": cfg.dt_fs, "rebuild_every": cfg.rebuild_every, "skin": cfg.skin,
+                   "l2": "per-step working set (edge activations, several GB) is far larger than the 126 MB L2",
+                   "parallelism": "replicas only" if world > 1 else "single GPU"},
+        "timesteps_per_s": K / (ms_max * 1e-3), "ns_per_day": K / (ms_max * 1e-3) * cfg.dt_fs * 0.0864,
+        "e_pot": e_pot, "e_kin": e_kin,
+        "gpu_launches": launches,
+        "clocks": sampler.summary(),
+        "e2e": {"value": e2e_val, "unit": unit, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "roofline": roofline,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        run, n_c, cores = oracle_sample(cfg, pos, sp, box, {0: 192, 1: 3072, 2: 512, 3: 512, 4: 256}[cfg.index])
+        run()
+        reps, tt = 0, 0.0
+        while tt < 10.0 and reps < 200:
+            tt += run(); reps += 1
+        out["cpu_baseline"] = {"value": n_c * reps / tt, "unit": unit, "cores": cores, "kind": "oracle",
+                               "sample": f"energy+forces of {n_c} contiguous centres (all their edges) of {workload}, "
+                                         f"{reps} repeats, {tt:.1f} s"}
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

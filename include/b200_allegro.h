@@ -125,6 +125,23 @@ int allegro_step_nve(allegro_model* m, double* pos, double* vel, double* force, 
                      int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
                      double* e_pot, double* e_kin);
 
+/* Same step with HOST arrays (pos, vel, force f64[N*3], species i32[N], mass f64[n_species], e_pot,
+ * e_kin f64[1]): copies state host->device, runs allegro_step_nve, copies state and energies back,
+ * and synchronises.  Pinned host memory makes the copies asynchronous. */
+int allegro_step_nve_host(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                          const double* mass, int64_t n_atoms, const double box[3], double dt_fs,
+                          int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
+                          double* e_pot, double* e_kin);
+
+/* Per-kernel-group device timing (bench roofline).  While enabled, every kernel group launched by the
+ * library is bracketed by CUDA events on the launching stream.  allegro_profile_read synchronises and
+ * returns, for group `name` ("gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem",
+ * "edge_bwd", "neighbors", "nve"), the summed milliseconds and the launch count since enable, plus for
+ * "gemm" the summed algorithmic FLOPs (2*M*N*K with M the chunk's candidate-edge capacity is NOT used:
+ * flops are computed by the caller from allegro_last_active_edges).  host pointers. */
+int allegro_profile_enable(allegro_model* m, int32_t on);
+int allegro_profile_read(allegro_model* m, const char* name, double* ms, int64_t* launches);
+
 /* Counters for tests/bench: number of kernels launched by the library since creation (host). */
 int allegro_launch_count(const allegro_model* m, int64_t* launches);
 /* Number of active (r < r_cut) edges of the last allegro_compute (synchronises the stream). */

@@ -71,7 +71,8 @@ EXPORTS = [
     "allegro_blob_size", "allegro_path_info", "allegro_create", "allegro_destroy", "allegro_set_stream",
     "allegro_set_allocator", "allegro_set_chunk_edges", "allegro_neighbors", "allegro_neighbors_host",
     "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
-    "allegro_step_nve", "allegro_launch_count", "allegro_last_active_edges", "allegro_debug_tensor",
+    "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
+    "allegro_launch_count", "allegro_last_active_edges", "allegro_debug_tensor",
     "allegro_last_error",
 ]
 
@@ -105,6 +106,9 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_compute_host.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp, vp]
     lib.allegro_step_nve.argtypes = [vp, vp, vp, vp, vp, vp, i64, P(C.c_double), C.c_double, i32, C.c_double, P(vp),
                                      P(i64), vp, vp]
+    lib.allegro_step_nve_host.argtypes = lib.allegro_step_nve.argtypes
+    lib.allegro_profile_enable.argtypes = [vp, i32]
+    lib.allegro_profile_read.argtypes = [vp, C.c_char_p, P(C.c_double), P(i64)]
     lib.allegro_launch_count.argtypes = [vp, P(i64)]
     lib.allegro_last_active_edges.argtypes = [vp, P(i64)]
     lib.allegro_debug_tensor.argtypes = [vp, C.c_char_p, vp, P(i64)]
@@ -306,6 +310,23 @@ class Allegro:
                                                species.data_ptr(), mass.data_ptr(), pos.shape[0], _box3(box),
                                                float(dt_fs), int(rebuild_every), float(skin), C.byref(nbr._h),
                                                C.byref(step_counter), e_pot.data_ptr(), e_kin.data_ptr()))
+
+    def step_nve_host(self, pos, vel, force, species, mass, box, dt_fs, rebuild_every, skin, nbr, step_counter,
+                      e_pot, e_kin):
+        """allegro_step_nve_host: all arrays are HOST buffers (numpy arrays or pinned CPU torch tensors)."""
+        ptr = lambda a: a.ctypes.data if hasattr(a, "ctypes") else a.data_ptr()
+        self._check(self._lib.allegro_step_nve_host(self._h, ptr(pos), ptr(vel), ptr(force), ptr(species), ptr(mass),
+                                                    pos.shape[0], _box3(box), float(dt_fs), int(rebuild_every),
+                                                    float(skin), C.byref(nbr._h), C.byref(step_counter), ptr(e_pot),
+                                                    ptr(e_kin)))
+
+    def profile_enable(self, on: bool):
+        self._check(self._lib.allegro_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self, name: str):
+        ms, n = C.c_double(0), C.c_int64(0)
+        self._check(self._lib.allegro_profile_read(self._h, name.encode(), C.byref(ms), C.byref(n)))
+        return ms.value, n.value
 
     def debug_tensor(self, name: str, max_floats: int = 1 << 26):
         import numpy as np

@@ -270,6 +270,33 @@ extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, doub
   return ALLEGRO_OK;
 }
 
+extern "C" int allegro_step_nve_host(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                                     const double* mass, int64_t N, const double box[3], double dt_fs,
+                                     int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
+                                     double* e_pot, double* e_kin) {
+  if (!m || !pos || !vel || !force || !species || !mass || !e_pot || !e_kin) return ALLEGRO_ERR_BAD_ARG;
+  static thread_local DevBuf stage;   // [pos | vel | force | e_pot, e_kin | mass | species]
+  size_t b3 = (size_t)N * 24, off_e = 3 * b3, off_m = off_e + 16, off_s = off_m + (size_t)m->S * 8;
+  AL_CHECK(al_reserve(m, stage, off_s + (size_t)N * 4 + 64));
+  char* d = (char*)stage.p;
+  cudaStream_t st = m->stream;
+  AL_CUDA(m, cudaMemcpyAsync(d, pos, b3, cudaMemcpyHostToDevice, st));
+  AL_CUDA(m, cudaMemcpyAsync(d + b3, vel, b3, cudaMemcpyHostToDevice, st));
+  AL_CUDA(m, cudaMemcpyAsync(d + 2 * b3, force, b3, cudaMemcpyHostToDevice, st));
+  AL_CUDA(m, cudaMemcpyAsync(d + off_m, mass, (size_t)m->S * 8, cudaMemcpyHostToDevice, st));
+  AL_CUDA(m, cudaMemcpyAsync(d + off_s, species, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+  AL_CHECK(allegro_step_nve(m, (double*)d, (double*)(d + b3), (double*)(d + 2 * b3), (const int32_t*)(d + off_s),
+                            (const double*)(d + off_m), N, box, dt_fs, rebuild_every, skin, nbr, step_counter,
+                            (double*)(d + off_e), (double*)(d + off_e + 8)));
+  AL_CUDA(m, cudaMemcpyAsync(pos, d, b3, cudaMemcpyDeviceToHost, st));
+  AL_CUDA(m, cudaMemcpyAsync(vel, d + b3, b3, cudaMemcpyDeviceToHost, st));
+  AL_CUDA(m, cudaMemcpyAsync(force, d + 2 * b3, b3, cudaMemcpyDeviceToHost, st));
+  AL_CUDA(m, cudaMemcpyAsync(e_pot, d + off_e, 8, cudaMemcpyDeviceToHost, st));
+  AL_CUDA(m, cudaMemcpyAsync(e_kin, d + off_e + 8, 8, cudaMemcpyDeviceToHost, st));
+  AL_CUDA(m, cudaStreamSynchronize(st));
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_debug_tensor(allegro_model* m, const char* name, float* out, int64_t* n_floats) {
   if (!m || !name || !out || !n_floats || !m->work) return ALLEGRO_ERR_BAD_ARG;
   Work& w = *m->work;

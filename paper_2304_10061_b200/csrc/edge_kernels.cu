@@ -478,6 +478,7 @@ __global__ void k_kin(const double* vel, const int32_t* species, const double* m
   } while (0)
 
 int k_launch_active_count(allegro_model* m, const EdgeGeomArgs& a, int* deg) {
+  ProfScope _ps(m, PC_GEOM);
   if (a.nc <= 0) return ALLEGRO_OK;
   k_active_count<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, deg);
   LAUNCH_CHECK(m);
@@ -485,12 +486,14 @@ int k_launch_active_count(allegro_model* m, const EdgeGeomArgs& a, int* deg) {
 }
 
 int k_launch_set_mact(allegro_model* m, const int64_t* rowa, int nc, int* m_act) {
+  ProfScope _ps(m, PC_GEOM);
   k_set_mact<<<1, 1, 0, m->stream>>>(rowa, nc, m_act);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
 
 int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* rowa, Work& w) {
+  ProfScope _ps(m, PC_GEOM);
   if (a.nc <= 0) return ALLEGRO_OK;
   k_geom_fill<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, rowa, (int*)w.ei.p, (int*)w.ej.p, (float4*)w.geo.p,
                                                            (float*)w.u.p, (float*)w.du.p, (float*)w.B.p, (float*)w.dB.p,
@@ -500,6 +503,7 @@ int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* r
 }
 
 int k_launch_twobody0(allegro_model* m, Work& w, const int32_t* species, const Dense& L0, bool single, int m_cap) {
+  ProfScope _ps(m, PC_TWOBODY0);
   if (m_cap <= 0) return ALLEGRO_OK;
   float* act = single ? (float*)w.XS[0].p : (float*)w.tb_a[0].p;
   int ld = single ? (m->d + m->n) : L0.fo;
@@ -523,6 +527,7 @@ static void tp_common(allegro_model* m, Work& w, int L, TPArgs& a, const float* 
 
 int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
                     const float* w0, int ldw, float* Tout, float* xs, int ldx) {
+  ProfScope _ps(m, PC_TP_FWD);
   if (nc <= 0) return ALLEGRO_OK;
   TPArgs a{};
   tp_common(m, w, L, a, om, ldo, Vin, w0, ldw);
@@ -542,6 +547,7 @@ int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
 int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
                     const float* w0, int ldw, const float* VbarL, const float* sbar, int lds, float* Vbar_prev,
                     float* ombar, int ldob, float* w0bar) {
+  ProfScope _ps(m, PC_TP_BWD);
   if (nc <= 0) return ALLEGRO_OK;
   TPArgs a{};
   tp_common(m, w, L, a, om, ldo, Vin, w0, ldw);
@@ -560,6 +566,7 @@ int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
 }
 
 int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c0, int nc, const float* xf, double* e_atom) {
+  ProfScope _ps(m, PC_ENERGY);
   if (nc <= 0) return ALLEGRO_OK;
   k_energy<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, xf, m->d, m->w_eff_d, species,
                                                         m->sigma, m->mu, e_atom);
@@ -568,12 +575,14 @@ int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c
 }
 
 int k_launch_sum_f64(allegro_model* m, const double* x, int64_t n, double* out) {
+  ProfScope _ps(m, PC_ENERGY);
   k_sum_f64<<<1, 1024, 0, m->stream>>>(x, n, out);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
 
 int k_launch_fill_xbar(allegro_model* m, Work& w, const int32_t* species, float* xb, int m_cap) {
+  ProfScope _ps(m, PC_BWD_ELEM);
   if (m_cap <= 0) return ALLEGRO_OK;
   int64_t tot = (int64_t)m_cap * m->d;
   k_fill_xbar<<<(unsigned)((tot + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, species, m->sigma,
@@ -584,6 +593,7 @@ int k_launch_fill_xbar(allegro_model* m, Work& w, const int32_t* species, float*
 
 int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, const float* z, int ldz, float c, float* zb,
                       int ldzb, int width, int m_cap) {
+  ProfScope _ps(m, PC_BWD_ELEM);
   if (m_cap <= 0) return ALLEGRO_OK;
   k_bwd_prep<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, xbar, ldx, z, ldz,
                                                                                   (float*)w.u.p, c, zb, ldzb, width,
@@ -594,6 +604,7 @@ int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, con
 
 int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, const Dense& L0, bool single, double* force,
                       int m_cap) {
+  ProfScope _ps(m, PC_EDGE_BWD);
   if (m_cap <= 0) return ALLEGRO_OK;
   (void)single;
   k_edge_bwd<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>(
@@ -604,6 +615,7 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
 }
 
 int k_launch_zero_f64(allegro_model* m, double* p, int64_t n) {
+  ProfScope _ps(m, PC_EDGE_BWD);
   if (n <= 0) return ALLEGRO_OK;
   k_zero_f64<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(p, n);
   LAUNCH_CHECK(m);
@@ -612,6 +624,7 @@ int k_launch_zero_f64(allegro_model* m, double* p, int64_t n) {
 
 int k_launch_nve_kick_drift(allegro_model* m, double* pos, double* vel, const double* force, const int32_t* species,
                             const double* mass, int64_t n, double dt, bool drift) {
+  ProfScope _ps(m, PC_NVE);
   if (n <= 0) return ALLEGRO_OK;
   k_nve<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(pos, vel, force, species, mass, n, dt, drift ? 1 : 0);
   LAUNCH_CHECK(m);
@@ -620,6 +633,7 @@ int k_launch_nve_kick_drift(allegro_model* m, double* pos, double* vel, const do
 
 int k_launch_kinetic(allegro_model* m, const double* vel, const int32_t* species, const double* mass, int64_t n,
                      double* e_kin, DevBuf& tmp) {
+  ProfScope _ps(m, PC_NVE);
   AL_CHECK(al_reserve(m, tmp, (size_t)n * 8 + 16));
   if (n > 0) {
     k_kin<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(vel, species, mass, n, (double*)tmp.p);

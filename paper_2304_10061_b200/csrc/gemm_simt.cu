@@ -113,6 +113,7 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
 }  // namespace
 
 int al_gemm(allegro_model* m, const GemmArgs& g) {
+  ProfScope _ps(m, PC_GEMM);
   if (g.m_cap <= 0) return ALLEGRO_OK;
   if ((g.K & 3) || (g.N & 3) || (g.lda & 3) || (g.ldb & 3) || (g.ldc & 3)) {
     al_set_error(m, "gemm: dimensions must be multiples of 4");

@@ -108,7 +108,21 @@ struct allegro_model {
   int sm_count = 148;
   // workspace (per chunk), grown on demand
   struct Work* work = nullptr;
+  // per-kernel-group event timing (allegro_profile_*)
+  bool prof = false;
+  struct ProfRec { int cat; cudaEvent_t a, b; };
+  std::vector<ProfRec> prof_recs;
+  std::vector<cudaEvent_t> prof_pool;
   std::vector<void*> owned;               // device allocations made through al_alloc (weights/tables)
+};
+
+// ---- profiling ------------------------------------------------------------------------------------
+enum ProfCat { PC_GEMM = 0, PC_TP_FWD, PC_TP_BWD, PC_GEOM, PC_TWOBODY0, PC_ENERGY, PC_BWD_ELEM, PC_EDGE_BWD, PC_NEIGHBORS,
+               PC_NVE, PC_COUNT };
+struct ProfScope {
+  allegro_model* m; int cat; cudaEvent_t a = nullptr;
+  ProfScope(allegro_model* m_, int cat_);
+  ~ProfScope();
 };
 
 // ---- allocation helpers ---------------------------------------------------------------------------

@@ -271,6 +271,8 @@ extern "C" int allegro_destroy(allegro_model* m) {
   if (!m) return ALLEGRO_OK;
   cudaDeviceSynchronize();
   al_work_free(m);
+  for (auto& r : m->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto e : m->prof_pool) cudaEventDestroy(e);
   for (void* p : m->owned) cudaFree(p);
   delete m;
   return ALLEGRO_OK;
@@ -298,5 +300,42 @@ extern "C" int allegro_set_chunk_edges(allegro_model* m, int64_t e) {
 extern "C" int allegro_launch_count(const allegro_model* m, int64_t* l) {
   if (!m || !l) return ALLEGRO_ERR_BAD_ARG;
   *l = m->launches;
+  return ALLEGRO_OK;
+}
+
+// ---- per-kernel-group event timing ---------------------------------------------------------------------
+static cudaEvent_t prof_event(allegro_model* m) {
+  if (!m->prof_pool.empty()) { cudaEvent_t e = m->prof_pool.back(); m->prof_pool.pop_back(); return e; }
+  cudaEvent_t e; cudaEventCreate(&e); return e;
+}
+ProfScope::ProfScope(allegro_model* m_, int cat_) : m(m_), cat(cat_) {
+  if (m && m->prof) { a = prof_event(m); cudaEventRecord(a, m->stream); }
+}
+ProfScope::~ProfScope() {
+  if (a) { cudaEvent_t b = prof_event(m); cudaEventRecord(b, m->stream); m->prof_recs.push_back({cat, a, b}); }
+}
+
+static const char* kProfNames[PC_COUNT] = {"gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd",
+                                           "neighbors", "nve"};
+
+extern "C" int allegro_profile_enable(allegro_model* m, int32_t on) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  cudaStreamSynchronize(m->stream);
+  for (auto& r : m->prof_recs) { m->prof_pool.push_back(r.a); m->prof_pool.push_back(r.b); }
+  m->prof_recs.clear();
+  m->prof = on != 0;
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_profile_read(allegro_model* m, const char* name, double* ms, int64_t* launches) {
+  if (!m || !name || !ms || !launches) return ALLEGRO_ERR_BAD_ARG;
+  int cat = -1;
+  for (int k = 0; k < PC_COUNT; ++k) if (std::string(name) == kProfNames[k]) cat = k;
+  if (cat < 0) { al_set_error(m, "unknown profile group"); return ALLEGRO_ERR_BAD_ARG; }
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  double tot = 0; int64_t cnt = 0;
+  for (auto& r : m->prof_recs)
+    if (r.cat == cat) { float t = 0; cudaEventElapsedTime(&t, r.a, r.b); tot += t; cnt++; }
+  *ms = tot; *launches = cnt;
   return ALLEGRO_OK;
 }

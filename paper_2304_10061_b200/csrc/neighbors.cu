@@ -206,6 +206,7 @@ int al_exclusive_scan_i64(allegro_model* m, const int32_t* in, int64_t* out, int
 
 int al_neighbors_impl(allegro_model* m, const double* pos, int64_t N, const double box[3], double cutoff,
                       allegro_nbr** inout) {
+  ProfScope _ps(m, PC_NEIGHBORS);
   if (!m || (!pos && N > 0) || !inout || !box) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
   if (N < 0 || N > 2000000000LL) { al_set_error(m, "n_atoms out of range"); return ALLEGRO_ERR_BAD_ARG; }
   if (!(cutoff > 0) || !(box[0] > 0) || !(box[1] > 0) || !(box[2] > 0)) { al_set_error(m, "cutoff and box must be > 0"); return ALLEGRO_ERR_BAD_ARG; }
