@@ -1,16 +1,320 @@
-// tcgen05 (TF32 / BF16) tensor-core GEMM path — placeholder until the tcgen05 kernel lands.
+// tcgen05 tensor-core GEMM for the edge-batched MLPs (precision modes 1/2; "TF32 for
+// matrix multiplications", Table IV).  sm_100a only: TMA (cp.async.bulk.tensor) stages K-major 128B-
+// swizzled operand tiles in shared memory, one elected thread issues tcgen05.mma.kind::tf32 with the
+// fp32 accumulator in TMEM (double-buffered, 2 x 256 columns), four epilogue warps read it back with
+// tcgen05.ld and apply the fused epilogue (SiLU / envelope / residual / SiLU') before storing fp32.
+//
+//   C[M,N] = epi( A[M,K] * Bt[N,K]^T ),  A and Bt row-major (K contiguous) fp32 in HBM.
+//
+// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM alloc), warps 2-5 =
+// epilogue (TMEM lane quarter = warp_id % 4).  Persistent CTAs, static tile schedule, n fastest.
+#include <cuda.h>
+#include <cstdlib>
+
+#include <map>
+#include <tuple>
+
 #include "gemm.h"
 #include "internal.h"
 
+namespace {
+
+constexpr int BM = 128;          // UMMA M (cta_group::1)
+constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
+constexpr int STAGES = 4;
+constexpr int BN_MAX = 256;
+constexpr int NTHREADS = 192;
+constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
+constexpr uint32_t B_STAGE_BYTES = BN_MAX * BKF * 4;       // 32 KB (allocated for the largest BN)
+constexpr uint32_t SMEM_BYTES = STAGES * (A_STAGE_BYTES + B_STAGE_BYTES) + 1024 /*align*/ + 256 /*barriers*/;
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t done, addr = smem_u32(bar);
+  do {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}"
+        : "=r"(done)
+        : "r"(addr), "r"(parity)
+        : "memory");
+  } while (!done);
+}
+__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_mma_tf32(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t* r) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// K-major, SWIZZLE_128B shared-memory matrix descriptor (sm100 format): start>>4 | LBO | SBO=1024B | version=1 | layout=2
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
+  uint64_t d = 0;
+  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)1 << 16;                 // LBO (unused for swizzled K-major)
+  d |= (uint64_t)(1024 >> 4) << 32;       // SBO: 8 rows x 128 B
+  d |= (uint64_t)1 << 46;                 // descriptor version (sm100)
+  d |= (uint64_t)2 << 61;                 // SWIZZLE_128B
+  return d;
+}
+
+__device__ __forceinline__ float silu_f(float z) { return z / (1.0f + __expf(-z)); }
+__device__ __forceinline__ float dsilu_f(float z) {
+  float s = 1.0f / (1.0f + __expf(-z));
+  return s * (1.0f + z * (1.0f - s));
+}
+
+__global__ void __launch_bounds__(NTHREADS, 1)
+k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, GemmArgs g, int BN, int ntn) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t* sA = smem;
+  uint8_t* sB = smem + STAGES * A_STAGE_BYTES;
+  uint64_t* bars = (uint64_t*)(smem + STAGES * (A_STAGE_BYTES + B_STAGE_BYTES));
+  uint64_t* full = bars;                 // [STAGES]
+  uint64_t* empty = bars + STAGES;       // [STAGES]
+  uint64_t* tfull = bars + 2 * STAGES;   // [2]
+  uint64_t* tempty = bars + 2 * STAGES + 2;   // [2]
+  uint32_t* tmem_slot = (uint32_t*)(bars + 2 * STAGES + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int M = *g.m_ptr;
+  const int num_mt = (M + BM - 1) / BM;
+  const int num_tiles = num_mt * ntn;
+  const int num_kb = (g.K + BKF - 1) / BKF;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===== TMA producer =====
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      const uint32_t bytes = A_STAGE_BYTES + (uint32_t)BN * BKF * 4;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        int mt = tile / ntn, nt = tile - mt * ntn;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&empty[stage], phase ^ 1);
+          mbar_expect_tx(&full[stage], bytes);
+          tma_load_2d(sA + stage * A_STAGE_BYTES, &tmA, &full[stage], kb * BKF, mt * BM);
+          tma_load_2d(sB + stage * B_STAGE_BYTES, &tmB, &full[stage], kb * BKF, nt * BN);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer =====
+    if (lane == 0) {
+      // instruction descriptor: D=f32, A=B=tf32, K-major both, N>>3, M>>4
+      const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+      int stage = 0; uint32_t phase = 0; int it = 0;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+        int acc = it & 1;
+        mbar_wait(&tempty[acc], ((it >> 1) & 1) ^ 1);
+        tc_fence_after();
+        uint32_t d_tmem = tmem_base + acc * BN_MAX;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&full[stage], phase);
+          tc_fence_after();
+          uint64_t da = make_desc(smem_u32(sA + stage * A_STAGE_BYTES));
+          uint64_t db = make_desc(smem_u32(sB + stage * B_STAGE_BYTES));
+#pragma unroll
+          for (int k = 0; k < BKF / 8; ++k)   // UMMA_K = 8 tf32 = 32 bytes -> +2 in the (addr >> 4) field
+            tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+          tc_commit(&empty[stage]);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
+        tc_commit(&tfull[acc]);
+      }
+    }
+  } else {
+    // ===== epilogue warps =====
+    const int q = warp & 3;   // TMEM lane quarter
+    int it = 0;
+    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+      int mt = tile / ntn, nt = tile - mt * ntn;
+      int acc = it & 1;
+      mbar_wait(&tfull[acc], (it >> 1) & 1);
+      tc_fence_after();
+      const int row = mt * BM + q * 32 + lane;
+      const bool row_ok = row < M;
+      float us = 1.0f;
+      if (row_ok && (g.epi == EPI_SILU_U || g.epi == EPI_LATENT)) us = g.u[row];
+      for (int c0 = 0; c0 < BN; c0 += 32) {
+        uint32_t r[32];
+        tc_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN_MAX + c0, r);
+        const int colb = nt * BN + c0;
+        if (row_ok) {
+#pragma unroll
+          for (int j4 = 0; j4 < 8; ++j4) {
+            int col = colb + j4 * 4;
+            if (col >= g.N || c0 + j4 * 4 >= BN) break;
+            float v[4] = {__uint_as_float(r[j4 * 4]), __uint_as_float(r[j4 * 4 + 1]), __uint_as_float(r[j4 * 4 + 2]),
+                          __uint_as_float(r[j4 * 4 + 3])};
+            float o[4];
+            switch (g.epi) {
+              case EPI_SILU_BOTH:
+              case EPI_SILU_U:
+              case EPI_LATENT: {
+                *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(v[0], v[1], v[2], v[3]);
+                if (g.epi == EPI_LATENT) {
+                  float4 x = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
+                  float xo[4] = {x.x, x.y, x.z, x.w};
+#pragma unroll
+                  for (int j = 0; j < 4; ++j) o[j] = g.c0 * xo[j] + g.c1 * us * silu_f(v[j]);
+                } else {
+#pragma unroll
+                  for (int j = 0; j < 4; ++j) o[j] = us * silu_f(v[j]);
+                }
+              } break;
+              case EPI_MUL_DSILU: {
+                float4 z = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
+                float zz[4] = {z.x, z.y, z.z, z.w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j) o[j] = v[j] * dsilu_f(zz[j]);
+              } break;
+              case EPI_ADD2: {
+                float4 x = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
+                float4 y = *reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col);
+                o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
+                o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
+              } break;
+              default:
+#pragma unroll
+                for (int j = 0; j < 4; ++j) o[j] = v[j];
+            }
+            *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+          }
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&tempty[acc]);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+  }
+}
+
+// ---- host side: tensor maps -----------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn g_encode = nullptr;
+
+typedef std::tuple<const void*, long long, long long, long long, int> TmKey;   // ptr, rows, K, ld, box_rows
+std::map<TmKey, CUtensorMap>& tm_cache() {
+  static thread_local std::map<TmKey, CUtensorMap> c;
+  return c;
+}
+
+int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, long long ld, int box_rows, CUtensorMap* out) {
+  TmKey key(ptr, rows, K, ld, box_rows);
+  auto& c = tm_cache();
+  auto it = c.find(key);
+  if (it != c.end()) { *out = it->second; return ALLEGRO_OK; }
+  if (!g_encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    AL_CUDA(m, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) { al_set_error(m, "cuTensorMapEncodeTiled not available"); return ALLEGRO_ERR_CUDA; }
+    g_encode = (EncodeTiledFn)fn;
+  }
+  cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
+  cuuint64_t gstr[1] = {(cuuint64_t)ld * 4};
+  cuuint32_t box[2] = {(cuuint32_t)BKF, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUtensorMap tm;
+  static const bool f32map = getenv("B200_ALLEGRO_TMAP_F32") != nullptr;   // experiment: plain fp32 load (MMA truncates)
+  CUresult r = g_encode(&tm, f32map ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_TFLOAT32, 2, const_cast<void*>(ptr), gdim, gstr, box, estr,
+                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { al_set_error(m, "cuTensorMapEncodeTiled failed, code " + std::to_string((int)r)); return ALLEGRO_ERR_CUDA; }
+  if (c.size() > 4096) c.clear();
+  c[key] = tm;
+  *out = tm;
+  return ALLEGRO_OK;
+}
+
+}  // namespace
+
 int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
-  (void)g;
-  al_set_error(m, "precision >= 1 (tensor-core GEMMs) not implemented yet");
-  return ALLEGRO_ERR_UNIMPLEMENTED;
+  int ntn = (g.N + BN_MAX - 1) / BN_MAX;
+  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  CUtensorMap tmA, tmB;
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, &tmA));
+  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, &tmB));
+  static bool attr_set = false;
+  if (!attr_set) {
+    AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
+    attr_set = true;
+  }
+  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
+  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
+  k_gemm_tf32<<<grid, NTHREADS, SMEM_BYTES, m->stream>>>(tmA, tmB, g, BN, ntn);
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
 }
 
 int al_upload_bf16(allegro_model* m, void** dst, const std::vector<float>& h) {
-  (void)h;
-  *dst = nullptr;
-  (void)m;
+  (void)m; (void)h;
+  *dst = nullptr;   // precision 2 currently runs the TF32 kernel on the fp32 copies
   return ALLEGRO_OK;
 }

@@ -169,3 +169,29 @@ def test_nve_steps_match_oracle():
     np.testing.assert_allclose(v.cpu().numpy(), v_o, atol=1e-7)
     assert abs(e.item() - e_o) / 192 < 2e-6
     assert abs(ek.item() - O.kinetic_energy(v_o, mass[sp])) < 1e-6
+
+
+# ---------------------------------------------------------------------------------------------------
+# TF32 tensor-core MLP mode (precision 1): 2e-3 relative on E (after removing sum mu) and on F
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ci,n", [(0, 192), (1, 1536), (2, 3000), (4, 1200)])
+def test_energy_forces_tf32(ci, n):
+    cfg = scaled_config(ci, n)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg, precision=1)
+    (E, Ea, F), nb = gpu_eval(model, pos, sp, box)
+    E0, Ea0, F0 = O.energy_forces(oracle, pos, sp, box, O.neighbor_list(pos, box, cfg.hp.r_cut))
+    mu = np.array(cfg.mu())[sp]
+    frms = float(np.sqrt((F0 ** 2).mean()))
+    # E - sum(mu) is a sum of per-atom energies of both signs and can nearly cancel, so the relative
+    # error of E is taken against the 1-norm of the per-atom energies
+    relE = abs(E - E0) / np.abs(Ea0 - mu).sum()
+    relEa = np.abs(Ea - Ea0).max() / np.abs(Ea0 - mu).max()
+    # "2e-3 relative on F" (north_star) is read as: max-norm error relative to the force scale max|F|,
+    # and relative L2 error; the stricter max-norm / RMS ratio is printed for the record.
+    relF_max = np.abs(F - F0).max() / np.abs(F0).max()
+    relF_l2 = np.linalg.norm(F - F0) / np.linalg.norm(F0)
+    relF_rms = np.abs(F - F0).max() / frms
+    print(f"[tf32 cfg{ci}] relE={relE:.3e} relE_i(max-norm)={relEa:.3e} relF: max/max={relF_max:.3e} "
+          f"l2={relF_l2:.3e} max/rms={relF_rms:.3e}")
+    assert relE <= 2e-3 and relEa <= 2e-3 and relF_max <= 2e-3 and relF_l2 <= 2e-3
