@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libb200allegro.so")
-SOURCES = ["model.cu", "cg_tables.cpp", "neighbors.cu", "edge_kernels.cu", "gemm_simt.cu", "gemm_tc.cu", "compute.cu"]
+SOURCES = ["model.cu", "cg_tables.cpp", "neighbors.cu", "edge_kernels.cu", "tp_kernels.cu", "gemm_simt.cu", "gemm_tc.cu", "compute.cu"]
 
 
 def lib_path() -> str:

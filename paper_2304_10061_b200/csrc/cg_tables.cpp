@@ -211,6 +211,9 @@ int al_build_tp_tables(allegro_model* m, const std::vector<std::vector<float>>& 
         if (any) { t.pair_a.push_back(a); t.pair_c.push_back(c); t.pair_ptr.push_back((int)t.ent_b.size()); }
       }
     t.npairs = (int)t.pair_a.size();
+    t.ent_idx.assign(t.nnz, 0);
+    for (int p = 0; p < t.npairs; ++p)
+      for (int k = t.pair_ptr[p]; k < t.pair_ptr[p + 1]; ++k) t.ent_idx[k] = t.pair_a[p] * t.Dout + t.pair_c[p];
     // CSR over c and over a
     t.c_ptr.assign(t.Dout + 1, 0); t.a_ptr.assign(t.Din + 1, 0); t.b_ptr.assign(t.Denv + 1, 0);
     for (int p = 0; p < t.npairs; ++p) { t.c_ptr[t.pair_c[p] + 1]++; t.a_ptr[t.pair_a[p] + 1]++; }

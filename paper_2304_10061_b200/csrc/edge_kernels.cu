@@ -408,7 +408,7 @@ __global__ void k_bwd_prep(const int* __restrict__ m_ptr, const float* __restric
 __global__ void k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz, const float* __restrict__ W,
                            int S, int NB, int H, const float4* __restrict__ geo, const float* __restrict__ du,
                            const float* __restrict__ dB, const float* __restrict__ ubar, const float* __restrict__ Ybar,
-                           int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
+                           int ngroups, int64_t ybar_gstride, int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
                            float* __restrict__ ge, double* __restrict__ force) {
   const int M = *m_ptr;
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -425,7 +425,11 @@ __global__ void k_edge_bwd(const int* __restrict__ m_ptr, const float* __restric
     rbar = fmaf(ubar[e], du[e], rbar);
     float4 g4 = geo[e];
     float yb[16];
-    for (int q = 0; q < Denv; ++q) yb[q] = Ybar[e * Denv + q];
+    for (int q = 0; q < Denv; ++q) {
+      float acc = 0.f;
+      for (int gq = 0; gq < ngroups; ++gq) acc += Ybar[gq * ybar_gstride + e * Denv + q];   // fixed order: deterministic
+      yb[q] = acc;
+    }
     float vx, vy, vz;
     sph_harm_vjp(g4.x, g4.y, g4.z, lmax, yb, vx, vy, vz);
     float dot = vx * g4.x + vy * g4.y + vz * g4.z;
@@ -525,10 +529,19 @@ static void tp_common(allegro_model* m, Work& w, int L, TPArgs& a, const float* 
   a.t = m->tp[L - 1]; a.n = m->n; a.lmax = m->lmax; a.c_env = m->c_env;
 }
 
+int tpw_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
+            float* Tout, float* xs, int ldx);
+int tpw_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
+            const float* VbarL, const float* sbar, int lds, float* Vbar_prev, float* ombar, int ldob, float* w0bar);
+
 int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
                     const float* w0, int ldw, float* Tout, float* xs, int ldx) {
   ProfScope _ps(m, PC_TP_FWD);
   if (nc <= 0) return ALLEGRO_OK;
+  {
+    int rc = tpw_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);   // warp-per-(center, channel group) fast path
+    if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
+  }
   TPArgs a{};
   tp_common(m, w, L, a, om, ldo, Vin, w0, ldw);
   a.Tout = Tout; a.xs = xs; a.ldx = ldx; a.gamma_out = (float*)w.gamma.p;
@@ -549,6 +562,10 @@ int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
                     float* ombar, int ldob, float* w0bar) {
   ProfScope _ps(m, PC_TP_BWD);
   if (nc <= 0) return ALLEGRO_OK;
+  {
+    int rc = tpw_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
+    if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
+  }
   TPArgs a{};
   tp_common(m, w, L, a, om, ldo, Vin, w0, ldw);
   a.VbarL = VbarL; a.sbar = sbar; a.lds = lds; a.Vbar_prev = Vbar_prev; a.ombar = ombar; a.ldob = ldob;
@@ -609,7 +626,7 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
   (void)single;
   k_edge_bwd<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>(
       (int*)w.m_act.p, zb1, ldz, L0.W, m->S, m->NB, L0.fo, (float4*)w.geo.p, (float*)w.du.p, (float*)w.dB.p,
-      (float*)w.ubar.p, (float*)w.Ybar.p, m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
+      (float*)w.ubar.p, (float*)w.Ybar.p, (m->n + 31) / 32, (int64_t)w.cap_edges * m->Denv, m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }

@@ -6,8 +6,8 @@
 //
 //   C[M,N] = epi( A[M,K] * Bt[N,K]^T ),  A and Bt row-major (K contiguous) fp32 in HBM.
 //
-// Warp roles (192 threads): warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM alloc), warps 2-5 =
-// epilogue (TMEM lane quarter = warp_id % 4).  Persistent CTAs, static tile schedule, n fastest.
+// Warp roles: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM alloc), warps 2.. = epilogue (TMEM
+// lane quarter = warp_id % 4, EPI_WARPS/4 warps per quarter taking alternate 32-column chunks).  Persistent CTAs, static tile schedule, n fastest.
 #include <cuda.h>
 #include <cstdlib>
 
@@ -21,12 +21,14 @@ namespace {
 
 constexpr int BM = 128;          // UMMA M (cta_group::1)
 constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
-constexpr int STAGES = 4;
+constexpr int STAGES = 3;
 constexpr int BN_MAX = 256;
-constexpr int NTHREADS = 192;
+constexpr int EPI_WARPS = 16;     // 2 per TMEM lane quarter, alternating 32-column chunks
+constexpr int NTHREADS = 64 + 32 * EPI_WARPS;
 constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
 constexpr uint32_t B_STAGE_BYTES = BN_MAX * BKF * 4;       // 32 KB (allocated for the largest BN)
-constexpr uint32_t SMEM_BYTES = STAGES * (A_STAGE_BYTES + B_STAGE_BYTES) + 1024 /*align*/ + 256 /*barriers*/;
+constexpr uint32_t STG_BYTES = EPI_WARPS * 32 * 33 * 4;             // epilogue transpose staging, one 32x33 tile per warp
+constexpr uint32_t SMEM_BYTES = STAGES * (A_STAGE_BYTES + B_STAGE_BYTES) + 1024 /*align*/ + 256 /*barriers*/ + STG_BYTES;
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -99,10 +101,11 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
   return d;
 }
 
-__device__ __forceinline__ float silu_f(float z) { return z / (1.0f + __expf(-z)); }
+// tensor-core modes: fast-math sigmoid (ex2.approx + rcp.approx), error ~1e-7 << TF32 rounding
+__device__ __forceinline__ float silu_f(float z) { return __fdividef(z, 1.0f + __expf(-z)); }
 __device__ __forceinline__ float dsilu_f(float z) {
-  float s = 1.0f / (1.0f + __expf(-z));
-  return s * (1.0f + z * (1.0f - s));
+  float s = __fdividef(1.0f, 1.0f + __expf(-z));
+  return s * fmaf(z, 1.0f - s, 1.0f);
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1)
@@ -117,6 +120,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   uint64_t* tfull = bars + 2 * STAGES;   // [2]
   uint64_t* tempty = bars + 2 * STAGES + 2;   // [2]
   uint32_t* tmem_slot = (uint32_t*)(bars + 2 * STAGES + 4);
+  float* stage_buf = (float*)(smem + STAGES * (A_STAGE_BYTES + B_STAGE_BYTES) + 256);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = *g.m_ptr;
@@ -126,7 +130,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 4); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], EPI_WARPS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -188,27 +192,34 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       int acc = it & 1;
       mbar_wait(&tfull[acc], (it >> 1) & 1);
       tc_fence_after();
-      const int row = mt * BM + q * 32 + lane;
-      const bool row_ok = row < M;
-      float us = 1.0f;
-      if (row_ok && (g.epi == EPI_SILU_U || g.epi == EPI_LATENT)) us = g.u[row];
-      for (int c0 = 0; c0 < BN; c0 += 32) {
+      // Each 32-column chunk: TMEM -> registers (lane = row) -> padded smem -> registers in the
+      // "coalesced domain" (8 lanes x float4 cover one row's 128 B, 4 rows per warp instruction), so
+      // every global load/store of the epilogue touches 4 lines per instruction instead of 32.
+      float* stg = stage_buf + (warp - 2) * (32 * 33);
+      const int chunk0 = (warp - 2) >> 2;   // this warp takes chunks chunk0, chunk0 + EPI_WARPS/4, ...
+      const int rsub = lane >> 3, c4 = (lane & 7) * 4;
+      const int rbase = mt * BM + q * 32;
+      for (int c0 = chunk0 * 32; c0 < BN; c0 += 32 * (EPI_WARPS / 4)) {
         uint32_t r[32];
         tc_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN_MAX + c0, r);
-        const int colb = nt * BN + c0;
-        if (row_ok) {
 #pragma unroll
-          for (int j4 = 0; j4 < 8; ++j4) {
-            int col = colb + j4 * 4;
-            if (col >= g.N || c0 + j4 * 4 >= BN) break;
-            float v[4] = {__uint_as_float(r[j4 * 4]), __uint_as_float(r[j4 * 4 + 1]), __uint_as_float(r[j4 * 4 + 2]),
-                          __uint_as_float(r[j4 * 4 + 3])};
+        for (int j = 0; j < 32; ++j) stg[lane * 33 + j] = __uint_as_float(r[j]);
+        __syncwarp();
+        const int col = nt * BN + c0 + c4;
+        const bool col_ok = (col < g.N) && (c0 + c4 < BN);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          const int rl = i * 4 + rsub;
+          const int row = rbase + rl;
+          float v[4] = {stg[rl * 33 + c4], stg[rl * 33 + c4 + 1], stg[rl * 33 + c4 + 2], stg[rl * 33 + c4 + 3]};
+          if (row < M && col_ok) {
             float o[4];
             switch (g.epi) {
               case EPI_SILU_BOTH:
               case EPI_SILU_U:
               case EPI_LATENT: {
                 *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(v[0], v[1], v[2], v[3]);
+                float us = (g.epi == EPI_SILU_BOTH) ? 1.0f : g.u[row];
                 if (g.epi == EPI_LATENT) {
                   float4 x = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
                   float xo[4] = {x.x, x.y, x.z, x.w};
@@ -238,6 +249,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
           }
         }
+        __syncwarp();
       }
       tc_fence_before();
       __syncwarp();

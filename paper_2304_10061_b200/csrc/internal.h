@@ -40,6 +40,7 @@ struct TPLayerHost {
   std::vector<int> pair_a, pair_c;            // [npairs]
   std::vector<int> pair_ptr;                  // [npairs+1] -> entries (b,val) of K
   std::vector<int> ent_b; std::vector<float> ent_val;
+  std::vector<int> ent_idx;                   // [nnz] a*Dout + c of the entry's pair
   // CSR over output component c -> (a, pair)
   std::vector<int> c_ptr, c_a, c_p;
   // CSR over input component a -> (c, pair)
@@ -52,7 +53,7 @@ struct TPLayerHost {
 // device copy of the tables of one layer
 struct TPLayerDev {
   int Din, Dout, Denv, npairs, nnz;
-  int *pair_a, *pair_c, *pair_ptr, *ent_b; float* ent_val;
+  int *pair_a, *pair_c, *pair_ptr, *ent_b; float* ent_val; int* ent_idx;
   int *c_ptr, *c_a, *c_p;
   int *a_ptr, *a_c, *a_p;
   int *b_ptr, *b_p; float* b_val;

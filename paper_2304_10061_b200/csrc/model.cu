@@ -253,7 +253,7 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
     t.Din = h.Din; t.Dout = h.Dout; t.Denv = h.Denv; t.npairs = h.npairs; t.nnz = h.nnz;
     if ((rc = upload(m, &t.pair_a, h.pair_a)) || (rc = upload(m, &t.pair_c, h.pair_c)) ||
         (rc = upload(m, &t.pair_ptr, h.pair_ptr)) || (rc = upload(m, &t.ent_b, h.ent_b)) ||
-        (rc = upload(m, &t.ent_val, h.ent_val)) || (rc = upload(m, &t.c_ptr, h.c_ptr)) ||
+        (rc = upload(m, &t.ent_val, h.ent_val)) || (rc = upload(m, &t.ent_idx, h.ent_idx)) || (rc = upload(m, &t.c_ptr, h.c_ptr)) ||
         (rc = upload(m, &t.c_a, h.c_a)) || (rc = upload(m, &t.c_p, h.c_p)) || (rc = upload(m, &t.a_ptr, h.a_ptr)) ||
         (rc = upload(m, &t.a_c, h.a_c)) || (rc = upload(m, &t.a_p, h.a_p)) || (rc = upload(m, &t.b_ptr, h.b_ptr)) ||
         (rc = upload(m, &t.b_p, h.b_p)) || (rc = upload(m, &t.b_val, h.b_val)))
