@@ -15,7 +15,7 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
   int d = m->d, n = m->n, nA = m->nA, NL = m->NL;
   if (M > w.cap_edges || w.XS.empty()) {
     auto R = [&](DevBuf& b, size_t floats) { return al_reserve(m, b, floats * 4 + 64); };
-    AL_CHECK(R(w.ei, M)); AL_CHECK(R(w.ej, M)); AL_CHECK(R(w.geo, 4 * M)); AL_CHECK(R(w.u, M)); AL_CHECK(R(w.du, M));
+    AL_CHECK(R(w.ei, M)); AL_CHECK(R(w.ej, M)); AL_CHECK(R(w.geo, 4 * M)); AL_CHECK(R(w.u, M)); AL_CHECK(R(w.du, M)); AL_CHECK(R(w.sig, M));
     AL_CHECK(R(w.B, M * m->NB)); AL_CHECK(R(w.dB, M * m->NB)); AL_CHECK(R(w.Y, M * m->Denv));
     w.tb_z.resize(hp.n_twobody); w.tb_a.resize(hp.n_twobody);
     int maxw = d + n;
@@ -63,7 +63,7 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
 void al_work_free(allegro_model* m) {
   if (!m->work) return;
   Work& w = *m->work;
-  std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.B, &w.dB, &w.Y,
+  std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.sig, &w.B, &w.dB, &w.Y,
                               &w.XF, &w.WE, &w.gamma, &w.XB0, &w.XB1, &w.ZB0, &w.ZB1, &w.G, &w.OB, &w.VB0, &w.VB1,
                               &w.ubar, &w.Ybar, &w.ge, &w.eatom};
   for (auto* b : all) al_release(m, *b);
@@ -149,10 +149,10 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     AL_CUDA(m, cudaMemsetAsync((float*)w.Ybar.p + (size_t)gq * w.cap_edges * m->Denv, 0, (size_t)m_cap * m->Denv * 4, st));
   float* xb = (float*)w.XB0.p; float* xb_o = (float*)w.XB1.p;
   float* vb = nullptr; float* vb_a = (float*)w.VB0.p; float* vb_b = (float*)w.VB1.p;
-  AL_CHECK(k_launch_fill_xbar(m, w, species, xb, m_cap));
+  bool rank1 = true;   // x-bar^{NL} = sigma_e * w_eff is never materialised
   for (int L = NL; L >= 1; --L) {
     float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
-    AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
+    AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
     for (int k = nlat - 1; k >= 1; --k) {
       GemmArgs g = mk(zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
       g.aux1 = (float*)w.lat_z[L - 1][k - 1].p; g.ld1 = hp.latent_dims[k - 1];
@@ -169,10 +169,13 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     AL_CHECK(k_launch_tp_bwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, vb, (float*)w.G.p + d, d + n, vprev, ombar,
                              ldob, (float*)w.OB.p));
     vb = vprev;
-    GemmArgs g = mk((float*)w.OB.p, ldob, (L == 1) ? m->emb01 : m->emb[L - 1], true, xb_o, d, m_cap, mp, EPI_ADD2);
+    GemmArgs g = mk((float*)w.OB.p, ldob, (L == 1) ? m->emb01 : m->emb[L - 1], true, xb_o, d, m_cap, mp,
+                    rank1 ? EPI_ADD2R : EPI_ADD2);
     g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = (float*)w.G.p; g.ld2 = d + n;
+    g.u = (float*)w.sig.p; g.aux3 = m->w_eff_f;
     AL_CHECK(al_gemm(m, g));
     std::swap(xb, xb_o);
+    rank1 = false;
   }
   {
     float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;

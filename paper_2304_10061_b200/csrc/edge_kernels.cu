@@ -100,7 +100,7 @@ __global__ void k_set_mact(const int64_t* __restrict__ rowa, int nc, int* __rest
 __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, int* __restrict__ ei, int* __restrict__ ej,
                             float4* __restrict__ geo, float* __restrict__ u, float* __restrict__ du,
                             float* __restrict__ B, float* __restrict__ dB, float* __restrict__ Y, int Denv,
-                            int* __restrict__ flags) {
+                            int* __restrict__ flags, float* __restrict__ sig, const double* __restrict__ sigma) {
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= a.nc) return;
   int i = (int)(a.c0 + warp);
@@ -119,6 +119,7 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
       double inv = 1.0 / r;
       float hx = (float)(dx * inv), hy = (float)(dy * inv), hz = (float)(dz * inv);
       ei[o] = i; ej[o] = j;
+      sig[o] = (float)sigma[a.species[i]];
       geo[o] = make_float4(hx, hy, hz, (float)r);
       // envelope (fp64; PAPER.md:222 via SURVEY S2)
       double x = r / a.rc, p = (double)a.p;
@@ -376,29 +377,29 @@ __global__ void k_sum_f64(const double* __restrict__ x, int64_t n, double* __res
   if (threadIdx.x == 0) *out = sh[0];
 }
 
-__global__ void k_fill_xbar(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int32_t* __restrict__ species,
-                            const double* __restrict__ sigma, const float* __restrict__ w_eff, int d, float* __restrict__ xb) {
-  const int M = *m_ptr;
-  int64_t idx = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
-  int64_t e = idx / d; int k = (int)(idx - e * d);
-  if (e >= M) return;
-  xb[idx] = (float)sigma[species[ei[e]]] * w_eff[k];
-}
-
-// zb = c * u * xbar * silu'(z) ; ubar += c * <xbar, silu(z)>      (one warp per edge)
+// zb = c * u * xbar * silu'(z) ; ubar += c * <xbar, silu(z)>      (one warp per edge, float4 lanes)
+// xbar == nullptr: the incoming gradient is the rank-1 x-bar^{NL}_e = sigma_{Z_i(e)} * w_eff (never materialised).
 __global__ void k_bwd_prep(const int* __restrict__ m_ptr, const float* __restrict__ xbar, int ldx, const float* __restrict__ z,
                            int ldz, const float* __restrict__ u, float c, float* __restrict__ zb, int ldzb, int width,
-                           float* __restrict__ ubar) {
+                           float* __restrict__ ubar, const float* __restrict__ sig, const float* __restrict__ w_eff) {
   const int M = *m_ptr;
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= M) return;
   int64_t e = warp;
   float cu = c * u[e], acc = 0.f;
-  for (int k = lane; k < width; k += 32) {
-    float xb = xbar[e * ldx + k], zz = z[e * ldz + k];
-    float s = 1.0f / (1.0f + expf(-zz));
-    acc = fmaf(xb, zz * s, acc);
-    zb[e * ldzb + k] = cu * xb * (s * (1.0f + zz * (1.0f - s)));
+  float sg = xbar ? 0.f : sig[e];
+  for (int k = lane * 4; k < width; k += 128) {
+    float4 x4 = xbar ? *reinterpret_cast<const float4*>(xbar + e * ldx + k) : *reinterpret_cast<const float4*>(w_eff + k);
+    float4 z4 = *reinterpret_cast<const float4*>(z + e * ldz + k);
+    float xb[4] = {x4.x, x4.y, x4.z, x4.w}, zz[4] = {z4.x, z4.y, z4.z, z4.w}, o[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      if (!xbar) xb[j] *= sg;
+      float s = 1.0f / (1.0f + expf(-zz[j]));
+      acc = fmaf(xb[j], zz[j] * s, acc);
+      o[j] = cu * xb[j] * (s * (1.0f + zz[j] * (1.0f - s)));
+    }
+    *reinterpret_cast<float4*>(zb + e * ldzb + k) = make_float4(o[0], o[1], o[2], o[3]);
   }
   acc = warp_sum(acc);
   if (lane == 0) ubar[e] += c * acc;
@@ -501,7 +502,7 @@ int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* r
   if (a.nc <= 0) return ALLEGRO_OK;
   k_geom_fill<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, rowa, (int*)w.ei.p, (int*)w.ej.p, (float4*)w.geo.p,
                                                            (float*)w.u.p, (float*)w.du.p, (float*)w.B.p, (float*)w.dB.p,
-                                                           (float*)w.Y.p, m->Denv, (int*)w.m_act.p);
+                                                           (float*)w.Y.p, m->Denv, (int*)w.m_act.p, (float*)w.sig.p, m->sigma);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
@@ -598,23 +599,13 @@ int k_launch_sum_f64(allegro_model* m, const double* x, int64_t n, double* out) 
   return ALLEGRO_OK;
 }
 
-int k_launch_fill_xbar(allegro_model* m, Work& w, const int32_t* species, float* xb, int m_cap) {
-  ProfScope _ps(m, PC_BWD_ELEM);
-  if (m_cap <= 0) return ALLEGRO_OK;
-  int64_t tot = (int64_t)m_cap * m->d;
-  k_fill_xbar<<<(unsigned)((tot + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, species, m->sigma,
-                                                                   m->w_eff_f, m->d, xb);
-  LAUNCH_CHECK(m);
-  return ALLEGRO_OK;
-}
-
 int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, const float* z, int ldz, float c, float* zb,
                       int ldzb, int width, int m_cap) {
   ProfScope _ps(m, PC_BWD_ELEM);
   if (m_cap <= 0) return ALLEGRO_OK;
   k_bwd_prep<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, xbar, ldx, z, ldz,
                                                                                   (float*)w.u.p, c, zb, ldzb, width,
-                                                                                  (float*)w.ubar.p);
+                                                                                  (float*)w.ubar.p, (float*)w.sig.p, m->w_eff_f);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }

@@ -13,7 +13,7 @@ enum GemmEpi {
   EPI_LATENT = 3,     // out2 = acc ; C = c0 * aux1[m,n] + c1 * u[m] * silu(acc)        (x^L residual update)
   EPI_MUL_DSILU = 4,  // C = acc * silu'(aux1[m,n])                                    (backward through SiLU)
   EPI_ADD2 = 5,       // C = acc + c0 * aux1[m,n] + aux2[m,n]                           (x-bar accumulation)
-  EPI_LATENT_BWD = 6  // C = acc + c0*aux1 + aux2 ; out2 = c1 * u[m] * C * silu'(aux3[m,n]) ; ubar[m] += c1 * <C, silu(aux3)>
+  EPI_ADD2R = 6       // C = acc + c0 * u[m] * aux3[n] + aux2[m,n]   (rank-1 incoming gradient sigma_e * w_eff)
 };
 
 struct GemmArgs {

@@ -102,6 +102,13 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
         o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
         o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
       } break;
+      case EPI_ADD2R: {
+        float4 x = *reinterpret_cast<const float4*>(g.aux3 + col);
+        float4 y = *reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col);
+        float cs = g.c0 * g.u[row];
+        o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
+        o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
+      } break;
       default:
 #pragma unroll
         for (int j = 0; j < 4; ++j) o[j] = v[j];

@@ -10,6 +10,7 @@ struct Work {
   DevBuf ei, ej;                            // int32[M] global atom ids
   DevBuf geo;                               // float4[M]: rhat.xyz, r
   DevBuf u, du;                             // float[M]: envelope u(r/rc), du/dr
+  DevBuf sig;                               // float[M]: sigma_{Z_i(e)}
   DevBuf B, dB;                             // float[M][NB]: B_n = b_n u, dB_n/dr
   DevBuf Y;                                 // float[M][Denv]
   std::vector<DevBuf> tb_z, tb_a;           // two-body pre-activations / activations, [M][h_k]
@@ -51,7 +52,6 @@ int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
 int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c0, int nc, const float* xf,
                     double* e_atom);
 int k_launch_sum_f64(allegro_model* m, const double* x, int64_t n, double* out);
-int k_launch_fill_xbar(allegro_model* m, Work& w, const int32_t* species, float* xb, int m_cap);
 int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, const float* z, int ldz, float c,
                       float* zb, int ldzb, int width, int m_cap);
 int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, const Dense& L0, bool single,
