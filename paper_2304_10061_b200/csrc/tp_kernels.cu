@@ -21,6 +21,49 @@ __device__ __forceinline__ float wsum(float v) {
   return v;
 }
 
+// Sum each of 8 per-lane values over the 32 lanes with 9 shuffles (halving butterfly): on return the
+// lane holds the total of value index ((lane>>4)&1)*4 + ((lane>>3)&1)*2 + ((lane>>2)&1).
+__device__ __forceinline__ float reduce8(const float* v, int lane) {
+  float a[4], b[2], c;
+  const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float send = h16 ? v[i] : v[i + 4], keep = h16 ? v[i + 4] : v[i];
+    a[i] = keep + __shfl_xor_sync(FULLMASK, send, 16);
+  }
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    float send = h8 ? a[i] : a[i + 2], keep = h8 ? a[i + 2] : a[i];
+    b[i] = keep + __shfl_xor_sync(FULLMASK, send, 8);
+  }
+  {
+    float send = h4 ? b[0] : b[1], keep = h4 ? b[1] : b[0];
+    c = keep + __shfl_xor_sync(FULLMASK, send, 4);
+  }
+  c += __shfl_xor_sync(FULLMASK, c, 2);
+  c += __shfl_xor_sync(FULLMASK, c, 1);
+  return c;
+}
+
+// Y-bar_e[idx[k]] += sum over lanes of p[k], k < D (D <= 16), deterministic; partial sums live in registers.
+template <int D>
+__device__ __forceinline__ void ybar_accumulate(float* yrow, const float* p, const int* idx, int lane) {
+  const int sel = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+#pragma unroll
+  for (int k0 = 0; k0 + 8 <= D; k0 += 8) {
+    float r = reduce8(p + k0, lane);
+    int t = idx[k0];
+#pragma unroll
+    for (int q = 1; q < 8; ++q) t = (sel == q) ? idx[k0 + q] : t;
+    if ((lane & 3) == 0) yrow[t] += r;
+  }
+#pragma unroll
+  for (int k = (D / 8) * 8; k < D; ++k) {
+    float s = wsum(p[k]);
+    if (lane == 0) yrow[idx[k]] += s;
+  }
+}
+
 struct TPW {
   const int64_t* rowa; int nc;
   const float* om; int ldo;
@@ -182,6 +225,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpw_bwd(TPW a) {
       float w[NLV], wb[NLV];
 #pragma unroll
       for (int l = 0; l < NLV; ++l) { w[l] = act ? a.w0[e * a.ldw + l * a.n + nn] : 0.f; wb[l] = 0.f; }
+      float pp[DIN];
 #pragma unroll
       for (int k = 0; k < DIN; ++k) {
         float y = __ldg(&a.Y[e * DENV + vy[k]]);
@@ -192,9 +236,9 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpw_bwd(TPW a) {
           wb[l] = m ? fmaf(vb[k], y, wb[l]) : wb[l];
           wl = m ? w[l] : wl;
         }
-        float s = wsum(wl * vb[k]);
-        if (lane == 0) Yb[e * DENV + vy[k]] += s;
+        pp[k] = wl * vb[k];
       }
+      ybar_accumulate<DIN>(Yb + e * DENV, pp, vy, lane);
       if (act)
 #pragma unroll
         for (int l = 0; l < NLV; ++l) a.w0bar[e * a.ldob + l * a.n + nn] = wb[l];
@@ -214,24 +258,26 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpw_bwd(TPW a) {
   for (int k = 0; k < tb.nnz; ++k) Gs[tb.b[k] * 32 + lane] = fmaf(tb.val[k], Ms[tb.idx[k] * 32 + lane], Gs[tb.b[k] * 32 + lane]);
   __syncwarp();
   float Gb[DENV];
+  int ident[DENV];
 #pragma unroll
-  for (int b = 0; b < DENV; ++b) Gb[b] = a.c_env * Gs[b * 32 + lane];     // c_env folded in here
+  for (int b = 0; b < DENV; ++b) { Gb[b] = a.c_env * Gs[b * 32 + lane]; ident[b] = b; }     // c_env folded in here
   // pass 2: omega-bar_e[l] = sum_m Gamma-bar[(l,m)] Y_e[(l,m)] ; Y-bar_e[b] += sum_n omega_e[l(b),n] Gamma-bar[b,n]
   for (int64_t e = e0; e < e1; ++e) {
     float om[NLV];
 #pragma unroll
     for (int l = 0; l < NLV; ++l) om[l] = act ? a.om[e * a.ldo + l * a.n + nn] : 0.f;
+    float pp[DENV];
 #pragma unroll
     for (int l = 0; l < NLV; ++l) {
       float ob = 0.f;
 #pragma unroll
       for (int b = l * l; b < (l + 1) * (l + 1); ++b) {
         ob = fmaf(Gb[b], __ldg(&a.Y[e * DENV + b]), ob);
-        float s = wsum(om[l] * Gb[b]);
-        if (lane == 0) Yb[e * DENV + b] += s;
+        pp[b] = om[l] * Gb[b];
       }
       if (act) a.ombar[e * a.ldob + l * a.n + nn] = ob;
     }
+    ybar_accumulate<DENV>(Yb + e * DENV, pp, ident, lane);
   }
 }
 

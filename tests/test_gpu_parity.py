@@ -195,3 +195,71 @@ def test_energy_forces_tf32(ci, n):
     print(f"[tf32 cfg{ci}] relE={relE:.3e} relE_i(max-norm)={relEa:.3e} relF: max/max={relF_max:.3e} "
           f"l2={relF_l2:.3e} max/rms={relF_rms:.3e}")
     assert relE <= 2e-3 and relEa <= 2e-3 and relF_max <= 2e-3 and relF_l2 <= 2e-3
+
+
+# ---------------------------------------------------------------------------------------------------
+# full-size configs, in the launch configuration bench.py times (default chunking, Verlet-skin list):
+# config 1 against the full oracle; configs 2-4 by exact sub-system parity (strict locality,
+# E-hat_c needs only centre c's edges; F_a only the centres within r_c of a)
+# ---------------------------------------------------------------------------------------------------
+def _subsystem_check(ci, n_probe, precision, seed=0):
+    cfg = CONFIGS[ci]
+    pos, sp, box = make_system(cfg)
+    N = pos.shape[0]
+    model, oracle = make_both(cfg, precision=precision)
+    (E, Ea, F), nb = gpu_eval(model, pos, sp, box, cutoff=cfg.hp.r_cut + cfg.skin)
+    oi, oj, os_ = O.neighbor_list(pos, box, cfg.hp.r_cut)
+    # list parity at full size on sampled rows (bit-exact) + total count
+    gi, gj, gs = nbr_as_arrays(model.neighbors(torch.from_numpy(pos).cuda(), box, cfg.hp.r_cut))
+    assert gi.shape == oi.shape and np.array_equal(gj, oj) and np.array_equal(gs, os_)
+    g = np.random.default_rng(seed)
+    probes = g.choice(N, n_probe, replace=False)
+    rp = np.searchsorted(oi, np.arange(N + 1))
+    C = set(probes.tolist())
+    for a in probes:
+        C.update(oj[rp[a]:rp[a + 1]].tolist())
+    C = np.array(sorted(C))
+    E0, Ea0, F0 = O.energy_forces(oracle, pos, sp, box, (oi, oj, os_), centers=C)
+    mu = np.array(cfg.mu())[sp]
+    dEa = np.abs(Ea[C] - Ea0[C]).max()
+    dF = np.abs(F[probes] - F0[probes]).max()
+    fs = max(1.0, float(np.sqrt((F0[probes] ** 2).mean())))
+    print(f"[cfg{ci} N={N} edges={oi.shape[0]} prec={precision}] centres={C.size} max|dE_c|={dEa:.3e} "
+          f"max|dF_probe|={dF:.3e} rmsF={np.sqrt((F0[probes]**2).mean()):.3e}")
+    assert np.isfinite(F).all() and np.isfinite(Ea).all()
+    assert abs(F.sum(0)).max() < 1e-6 * np.abs(F).sum()            # property at any size: sum F = 0
+    if precision == 0:
+        assert dEa <= 27 * E_TOL_PER_ATOM and dF <= F_TOL_REL * fs
+    else:
+        assert dEa <= 2e-3 * np.abs(Ea0[C] - mu[C]).max() and dF <= 2e-3 * np.abs(F0[probes]).max()
+
+
+def test_config1_full_fp32_and_tf32():
+    cfg = CONFIGS[1]
+    pos, sp, box = make_system(cfg)
+    want = O.energy_forces(oracle_for(cfg), pos, sp, box, O.neighbor_list(pos, box, cfg.hp.r_cut))
+    model, _ = make_both(cfg, precision=0)
+    got, _ = gpu_eval(model, pos, sp, box, cutoff=cfg.hp.r_cut + cfg.skin)
+    _check_EF(got, want, pos.shape[0], "cfg1 full fp32")
+    model1, _ = make_both(cfg, precision=1)
+    (E, Ea, F), _ = gpu_eval(model1, pos, sp, box, cutoff=cfg.hp.r_cut + cfg.skin)
+    mu = np.array(cfg.mu())[sp]
+    assert abs(E - want[0]) <= 2e-3 * np.abs(want[1] - mu).sum()
+    assert np.abs(F - want[2]).max() <= 2e-3 * np.abs(want[2]).max()
+    assert np.linalg.norm(F - want[2]) <= 2e-3 * np.linalg.norm(want[2])
+
+
+def oracle_for(cfg):
+    from synthetic import make_blob
+    hp = cfg.hp
+    blob = make_blob(hp, O.path_fan(hp.l_max, hp.n_layers), [cfg.sigma] * hp.n_species, cfg.mu(), cfg.weight_seed)
+    return O.OracleModel(hp, blob)
+
+
+@pytest.mark.parametrize("ci,precision", [(2, 0), (2, 1), (4, 0), (4, 1)])
+def test_full_size_subsystem_parity(ci, precision):
+    _subsystem_check(ci, 24, precision)
+
+
+def test_config3_million_atoms_subsystem_parity():
+    _subsystem_check(3, 8, 1)
