@@ -82,6 +82,18 @@ def peaks():
     return {"hbm_gbs": 6650.0, "bf16_burst": 1590.0, "bf16_sustained": 1400.0, "sm_max_mhz": 1965.0, "src": "fallback"}
 
 
+def aggregate_over_ranks(ms_local, atoms_local, steps, dist=None, device="cpu"):
+    """Whole-job throughput for N independent replicas ("replicas only"): units summed over ranks divided by
+    the MAX over ranks of the device time.  Returns (atom-steps/s, max ms)."""
+    import torch
+    t = torch.tensor([float(ms_local)], dtype=torch.float64, device=device)
+    a = torch.tensor([float(atoms_local)], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(a, op=dist.ReduceOp.SUM)
+    return float(a.item()) * steps / (float(t.item()) * 1e-3), float(t.item())
+
+
 def oracle_sample(cfg, pos, sp, box, n_centers):
     """Energy + forces of `n_centers` contiguous centres by the fp64 oracle (cpu_baseline / reference arm)."""
     import torch
@@ -126,7 +138,7 @@ def main():
         if rank != 0:
             return
         pos, sp, box = make_system(cfg)
-        n_c = {0: 192, 1: 96, 2: 32, 3: 32, 4: 24}[cfg.index]
+        n_c = {0: 192, 1: 3072, 2: 512, 3: 512, 4: 256}[cfg.index]
         run, n_c, cores = oracle_sample(cfg, pos, sp, box, n_c)
         for _ in range(min(W, 3)):
             run()
@@ -191,11 +203,7 @@ def main():
     launches = model.launches - l0
     n_active = model.last_active_edges()
     e_pot, e_kin = float(e.item()), float(ek.item())
-    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    ms_max = float(t_ms.item())
-    value = world * N * K / (ms_max * 1e-3)
+    value, ms_max = aggregate_over_ranks(ms, N, K, dist, dev)
 
     # ---- e2e: the same step through the C ABI with HOST (pinned) buffers, copies inside the timed region
     hp_ = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -209,10 +217,7 @@ def main():
     for _ in range(K):
         model.step_nve_host(ph, vh, fh, sh, mh, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, eh, ekh)
     torch.cuda.synchronize()
-    t_e2e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t_e2e, op=dist.ReduceOp.MAX)
-    e2e_val = world * N * K / float(t_e2e.item())
+    e2e_val, _ = aggregate_over_ranks((time.perf_counter() - t0) * 1e3, N, K, dist, dev)
     h2d = 3 * N * 24 + N * 4 + cfg.hp.n_species * 8
     d2h = 3 * N * 24 + 16
 
