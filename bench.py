@@ -43,6 +43,33 @@ def gemm_macs_per_edge(hp):
     return fwd + bwd
 
 
+def gemm_bytes_per_edge(hp):
+    """Algorithmic HBM bytes per ACTIVE edge of the GEMM kernel group (fp32 storage): every launch reads its A
+    operand once and writes its outputs once; aux operands of the fused epilogues are read once.  Weights are
+    L2-resident and not counted.  Mirrors the launch list of csrc/compute.cu::run_chunk."""
+    d, n, nA, NL = hp.twobody_dims[-1], hp.n_tensor, hp.n_tensor * (hp.l_max + 1), hp.n_layers
+    tb, lat = list(hp.twobody_dims), list(hp.latent_dims)
+    fl = 0
+    for k in range(1, len(tb)):                       # two-body forward: A, C (activation), out2 (pre-activation)
+        fl += tb[k - 1] + 2 * tb[k]
+    fl += d + 2 * nA                                  # [w0 | omega1]
+    for L in range(1, NL + 1):
+        for k in range(len(lat)):
+            K = d + n if k == 0 else lat[k - 1]
+            fl += K + 2 * lat[k] + (d if k == len(lat) - 1 else 0)      # last: residual x^{L-1} read
+        if L < NL:
+            fl += d + nA
+    for L in range(NL, 0, -1):                        # backward
+        for k in range(len(lat) - 1, 0, -1):
+            fl += lat[k] + 2 * lat[k - 1]             # A, aux z, C
+        fl += lat[0] + (d + n)
+        Kx = 2 * nA if L == 1 else nA
+        fl += Kx + d * (2 if L == NL else 3)          # A, aux2 (+ aux1 unless rank-1), C
+    for k in range(len(tb) - 1, 0, -1):
+        fl += tb[k] + 2 * tb[k - 1]
+    return 4 * fl
+
+
 class ClockSampler(threading.Thread):
     """Samples nvidia-smi clocks and throttle reasons during the timed region."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -241,9 +268,16 @@ def main():
     else:
         peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16, "tensor"
         peak_note = f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16}"
-    roofline = {"bound": bound, "kernel": "MLP GEMM group (fwd+bwd)", "achieved": gemm_tflops, "peak": peak,
-                "unit": "TFLOP/s", "frac": gemm_tflops / peak if peak else None, "traffic": None,
-                "peak_note": peak_note, "launches_per_step": gemm_n / K, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
+    gemm_gbs = gemm_bytes_per_edge(cfg.hp) * n_active * K / (gemm_ms * 1e-3) / 1e9 if gemm_ms > 0 else 0.0
+    f_compute, f_hbm = gemm_tflops / peak, gemm_gbs / pk["hbm_gbs"]
+    comp = {"bound": bound, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s", "frac": f_compute, "peak_note": peak_note}
+    hbm = {"bound": "hbm", "achieved": gemm_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm,
+           "peak_note": f"copy bandwidth ({pk['src']}); algorithmic bytes = {gemm_bytes_per_edge(cfg.hp)} B per active edge"}
+    top = hbm if f_hbm > f_compute else comp       # the binding roofline is the one with the larger fraction
+    roofline = {"bound": top["bound"], "kernel": "MLP GEMM group (fwd+bwd), k_gemm_tf32" if args.precision else "MLP GEMM group (fwd+bwd), k_gemm_simt",
+                "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"], "traffic": None,
+                "peak_note": top["peak_note"], "compute_roofline": comp, "hbm_roofline": hbm,
+                "launches_per_step": gemm_n / K, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
                 "share_of_step": gemm_ms / tot_prof if tot_prof else None,
                 "groups_ms_per_step": {g: round(t / K, 4) for g, (t, _) in prof.items()}}
 

@@ -144,7 +144,7 @@ int allegro_profile_read(allegro_model* m, const char* name, double* ms, int64_t
 
 /* Counters for tests/bench: number of kernels launched by the library since creation (host). */
 int allegro_launch_count(const allegro_model* m, int64_t* launches);
-/* Number of active (r < r_cut) edges of the last allegro_compute (synchronises the stream). */
+/* Total number of active (r < r_cut) edges, over all chunks, of the last allegro_compute (synchronises the stream). */
 int allegro_last_active_edges(allegro_model* m, int64_t* n_active);
 
 /* Debug/parity taps (tests only): copy an intermediate tensor of the LAST chunk of the last

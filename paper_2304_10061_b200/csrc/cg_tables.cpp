@@ -214,6 +214,22 @@ int al_build_tp_tables(allegro_model* m, const std::vector<std::vector<float>>& 
     t.ent_idx.assign(t.nnz, 0);
     for (int p = 0; p < t.npairs; ++p)
       for (int k = t.pair_ptr[p]; k < t.pair_ptr[p + 1]; ++k) t.ent_idx[k] = t.pair_a[p] * t.Dout + t.pair_c[p];
+    // packed entry lists sorted by c (already the entry order) and by a
+    t.ce_pack.assign(t.nnz, 0); t.ce_val = t.ent_val; t.cent_ptr.assign(t.Dout + 1, 0);
+    for (int p = 0; p < t.npairs; ++p)
+      for (int k = t.pair_ptr[p]; k < t.pair_ptr[p + 1]; ++k) {
+        t.ce_pack[k] = t.pair_a[p] | (t.pair_c[p] << 8) | (t.ent_b[k] << 16);
+        t.cent_ptr[t.pair_c[p] + 1]++;
+      }
+    for (int c = 0; c < t.Dout; ++c) t.cent_ptr[c + 1] += t.cent_ptr[c];
+    t.aent_ptr.assign(t.Din + 1, 0);
+    for (int k = 0; k < t.nnz; ++k) t.aent_ptr[(t.ce_pack[k] & 255) + 1]++;
+    for (int a = 0; a < t.Din; ++a) t.aent_ptr[a + 1] += t.aent_ptr[a];
+    t.ae_pack.assign(t.nnz, 0); t.ae_val.assign(t.nnz, 0.f);
+    {
+      std::vector<int> af(t.aent_ptr.begin(), t.aent_ptr.end() - 1);
+      for (int k = 0; k < t.nnz; ++k) { int a = t.ce_pack[k] & 255; t.ae_pack[af[a]] = t.ce_pack[k]; t.ae_val[af[a]++] = t.ce_val[k]; }
+    }
     // CSR over c and over a
     t.c_ptr.assign(t.Dout + 1, 0); t.a_ptr.assign(t.Din + 1, 0); t.b_ptr.assign(t.Denv + 1, 0);
     for (int p = 0; p < t.npairs; ++p) { t.c_ptr[t.pair_c[p] + 1]++; t.a_ptr[t.pair_a[p] + 1]++; }

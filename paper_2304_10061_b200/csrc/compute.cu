@@ -200,6 +200,7 @@ int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species,
   Work& w = *m->work;
   double* ea = e_atom ? e_atom : (double*)w.eatom.p;
   AL_CHECK(k_launch_zero_f64(m, force, 3 * N));
+  AL_CUDA(m, cudaMemsetAsync((int*)w.m_act.p + 2, 0, 8, m->stream));   // total active edges of this call
   for (const Chunk& ch : nb->chunks) {
     if (ch.e1 == ch.e0) {
       // no candidate edges at all: make rowa all-zero so k_energy yields mu_Z
@@ -249,9 +250,9 @@ done:
 
 extern "C" int allegro_last_active_edges(allegro_model* m, int64_t* n_active) {
   if (!m || !n_active || !m->work) return ALLEGRO_ERR_BAD_ARG;
-  int v = 0;
+  long long v = 0;
   AL_CUDA(m, cudaStreamSynchronize(m->stream));
-  AL_CUDA(m, cudaMemcpy(&v, m->work->m_act.p, 4, cudaMemcpyDeviceToHost));
+  AL_CUDA(m, cudaMemcpy(&v, (int*)m->work->m_act.p + 2, 8, cudaMemcpyDeviceToHost));
   *n_active = v;
   return ALLEGRO_OK;
 }

@@ -95,7 +95,11 @@ __global__ void k_active_count(EdgeGeomArgs a, int* __restrict__ deg) {
   if (lane == 0) deg[warp] = cnt;
 }
 
-__global__ void k_set_mact(const int64_t* __restrict__ rowa, int nc, int* __restrict__ m_act) { m_act[0] = (int)rowa[nc]; }
+// m_act[0] = active edges of this chunk; (int64*)(m_act + 2) accumulates the total over the chunks of one compute call
+__global__ void k_set_mact(const int64_t* __restrict__ rowa, int nc, int* __restrict__ m_act) {
+  m_act[0] = (int)rowa[nc];
+  *reinterpret_cast<long long*>(m_act + 2) += (long long)rowa[nc];
+}
 
 __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, int* __restrict__ ei, int* __restrict__ ej,
                             float4* __restrict__ geo, float* __restrict__ u, float* __restrict__ du,

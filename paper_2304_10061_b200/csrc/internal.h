@@ -41,6 +41,8 @@ struct TPLayerHost {
   std::vector<int> pair_ptr;                  // [npairs+1] -> entries (b,val) of K
   std::vector<int> ent_b; std::vector<float> ent_val;
   std::vector<int> ent_idx;                   // [nnz] a*Dout + c of the entry's pair
+  // packed entry lists (a | c<<8 | b<<16, val): sorted by c (ce_*, cent_ptr[Dout+1]) and by a (ae_*, aent_ptr[Din+1])
+  std::vector<int> ce_pack, cent_ptr, ae_pack, aent_ptr; std::vector<float> ce_val, ae_val;
   // CSR over output component c -> (a, pair)
   std::vector<int> c_ptr, c_a, c_p;
   // CSR over input component a -> (c, pair)
@@ -57,6 +59,7 @@ struct TPLayerDev {
   int *c_ptr, *c_a, *c_p;
   int *a_ptr, *a_c, *a_p;
   int *b_ptr, *b_p; float* b_val;
+  int *ce_pack, *cent_ptr, *ae_pack, *aent_ptr; float *ce_val, *ae_val;
 };
 
 struct Dense {

@@ -256,7 +256,9 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
         (rc = upload(m, &t.ent_val, h.ent_val)) || (rc = upload(m, &t.ent_idx, h.ent_idx)) || (rc = upload(m, &t.c_ptr, h.c_ptr)) ||
         (rc = upload(m, &t.c_a, h.c_a)) || (rc = upload(m, &t.c_p, h.c_p)) || (rc = upload(m, &t.a_ptr, h.a_ptr)) ||
         (rc = upload(m, &t.a_c, h.a_c)) || (rc = upload(m, &t.a_p, h.a_p)) || (rc = upload(m, &t.b_ptr, h.b_ptr)) ||
-        (rc = upload(m, &t.b_p, h.b_p)) || (rc = upload(m, &t.b_val, h.b_val)))
+        (rc = upload(m, &t.b_p, h.b_p)) || (rc = upload(m, &t.b_val, h.b_val)) ||
+        (rc = upload(m, &t.ce_pack, h.ce_pack)) || (rc = upload(m, &t.cent_ptr, h.cent_ptr)) || (rc = upload(m, &t.ce_val, h.ce_val)) ||
+        (rc = upload(m, &t.ae_pack, h.ae_pack)) || (rc = upload(m, &t.aent_ptr, h.aent_ptr)) || (rc = upload(m, &t.ae_val, h.ae_val)))
       return fail(rc);
   }
   std::vector<int> env_l;

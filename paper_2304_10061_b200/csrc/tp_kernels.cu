@@ -281,6 +281,263 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpw_bwd(TPW a) {
   }
 }
 
+// =====================================================================================================
+// Blocked variants for wide features (l_max = 3: D = 16 / 31).  M_i no longer fits next to the other live
+// values, so the forward walks C-BLOCKS of the output (M block in registers: D_in x CB <= 128) and the
+// backward walks A-BLOCKS of the input (M-bar block in registers: AB x D_out <= 128, M block in the warp's
+// shared slice).  Entries of the sparse fused tensor are staged per block, sorted by c resp. by a.
+// =====================================================================================================
+struct PackedTables { const int* pack; const float* val; const int* ptr; };
+
+__device__ __forceinline__ PackedTables load_packed(const int* gpack, const float* gval, const int* gptr, int nnz, int nptr,
+                                                    float* smem_tab) {
+  int* sp = (int*)smem_tab; float* sv = (float*)(sp + nnz); int* spt = (int*)(sv + nnz);
+  for (int k = threadIdx.x; k < nnz; k += blockDim.x) { sp[k] = gpack[k]; sv[k] = gval[k]; }
+  for (int k = threadIdx.x; k < nptr; k += blockDim.x) spt[k] = gptr[k];
+  __syncthreads();
+  return PackedTables{sp, sv, spt};
+}
+
+template <int DENV>
+__device__ __forceinline__ void gamma_only(const TPW& a, int64_t e0, int64_t e1, int nn, bool act, int lane, float* Gs) {
+  constexpr int NLV = (DENV == 1) ? 1 : (DENV == 4) ? 2 : (DENV == 9) ? 3 : 4;
+  float G[DENV];
+#pragma unroll
+  for (int b = 0; b < DENV; ++b) G[b] = 0.f;
+#pragma unroll 2
+  for (int64_t e = e0; e < e1; ++e) {
+    float om[NLV];
+#pragma unroll
+    for (int l = 0; l < NLV; ++l) om[l] = act ? a.om[e * a.ldo + l * a.n + nn] : 0.f;
+#pragma unroll
+    for (int l = 0; l < NLV; ++l)
+#pragma unroll
+      for (int b = l * l; b < (l + 1) * (l + 1); ++b) G[b] = fmaf(om[l], __ldg(&a.Y[e * DENV + b]), G[b]);
+  }
+#pragma unroll
+  for (int b = 0; b < DENV; ++b) Gs[b * 32 + lane] = a.c_env * G[b];
+  __syncwarp();
+}
+
+template <int DENV, int DIN, int DOUT, int CB, bool FIRST>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpb_fwd(TPW a) {
+  extern __shared__ float smem[];
+  constexpr int WSL = (DENV + DIN * CB) * 32;          // floats per warp slice
+  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const PackedTables tb = load_packed(a.t.ce_pack, a.t.ce_val, a.t.cent_ptr, a.t.nnz, DOUT + 1, smem + WARPS_PER_BLOCK * WSL);
+  const int64_t wg = (int64_t)blockIdx.x * WARPS_PER_BLOCK + wib;
+  if (wg >= (int64_t)a.nc * a.ngroups) return;
+  const int c = (int)(wg / a.ngroups), grp = (int)(wg - (int64_t)c * a.ngroups);
+  const int nn = grp * 32 + lane;
+  const bool act = nn < a.n;
+  float* Gs = smem + wib * WSL;
+  float* Ms = Gs + DENV * 32;
+  const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
+  if (e1 <= e0) return;
+  gamma_only<DENV>(a, e0, e1, nn, act, lane, Gs);
+  if (a.gamma_out && act)
+#pragma unroll
+    for (int b = 0; b < DENV; ++b) a.gamma_out[((size_t)c * DENV + b) * a.n + nn] = Gs[b * 32 + lane];
+  int vl[DIN], vy[DIN];
+#pragma unroll
+  for (int k = 0; k < DIN; ++k) { vl[k] = FIRST ? a.v0_l[k] : 0; vy[k] = FIRST ? a.v0_y[k] : 0; }
+  for (int cb = 0; cb < DOUT; cb += CB) {
+    const int cend = (cb + CB < DOUT) ? cb + CB : DOUT;
+#pragma unroll
+    for (int k = 0; k < DIN * CB; ++k) Ms[k * 32 + lane] = 0.f;
+    __syncwarp();
+    for (int k = tb.ptr[cb]; k < tb.ptr[cend]; ++k) {
+      int pk = tb.pack[k];
+      int idx = (pk & 255) * CB + (((pk >> 8) & 255) - cb);
+      Ms[idx * 32 + lane] = fmaf(tb.val[k], Gs[(pk >> 16) * 32 + lane], Ms[idx * 32 + lane]);
+    }
+    __syncwarp();
+    float Mr[DIN * CB];
+#pragma unroll
+    for (int k = 0; k < DIN * CB; ++k) Mr[k] = Ms[k * 32 + lane];
+    for (int64_t e = e0; e < e1; ++e) {
+      float v[DIN];
+      load_v<DENV, DIN, FIRST>(a, e, nn, act, vl, vy, v);
+      float acc[CB];
+#pragma unroll
+      for (int cc = 0; cc < CB; ++cc) acc[cc] = 0.f;
+#pragma unroll
+      for (int k = 0; k < DIN; ++k)
+#pragma unroll
+        for (int cc = 0; cc < CB; ++cc) acc[cc] = fmaf(v[k], Mr[k * CB + cc], acc[cc]);
+      if (act) {
+        if (cb == 0) a.xs[e * a.ldx + nn] = acc[0];
+        if (a.Tout)
+#pragma unroll
+          for (int cc = 0; cc < CB; ++cc)
+            if (cb + cc < DOUT) a.Tout[(e * DOUT + cb + cc) * a.n + nn] = acc[cc];
+      }
+    }
+    __syncwarp();
+  }
+}
+
+template <int DENV, int DIN, int DOUT, int AB, bool FIRST>
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpb_bwd(TPW a) {
+  extern __shared__ float smem[];
+  constexpr int NLV = (DENV == 1) ? 1 : (DENV == 4) ? 2 : (DENV == 9) ? 3 : 4;
+  constexpr int WSL = (2 * DENV + AB * DOUT) * 32;
+  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const PackedTables tb = load_packed(a.t.ae_pack, a.t.ae_val, a.t.aent_ptr, a.t.nnz, DIN + 1, smem + WARPS_PER_BLOCK * WSL);
+  const int64_t wg = (int64_t)blockIdx.x * WARPS_PER_BLOCK + wib;
+  if (wg >= (int64_t)a.nc * a.ngroups) return;
+  const int c = (int)(wg / a.ngroups), grp = (int)(wg - (int64_t)c * a.ngroups);
+  const int nn = grp * 32 + lane;
+  const bool act = nn < a.n;
+  float* Gs = smem + wib * WSL;
+  float* Gbs = Gs + DENV * 32;
+  float* Ms = Gbs + DENV * 32;
+  const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
+  if (e1 <= e0) return;
+  gamma_only<DENV>(a, e0, e1, nn, act, lane, Gs);
+#pragma unroll
+  for (int b = 0; b < DENV; ++b) Gbs[b * 32 + lane] = 0.f;
+  float* Yb = a.Ybar + (size_t)grp * a.ybar_gstride;
+  if (FIRST && act)
+    for (int64_t e = e0; e < e1; ++e)
+#pragma unroll
+      for (int l = 0; l < NLV; ++l) a.w0bar[e * a.ldob + l * a.n + nn] = 0.f;
+  for (int ab = 0; ab < DIN; ab += AB) {
+    const int aend = (ab + AB < DIN) ? ab + AB : DIN;
+    int vl[AB], vy[AB];
+#pragma unroll
+    for (int k = 0; k < AB; ++k) {
+      int aa = (ab + k < DIN) ? ab + k : DIN - 1;
+      vl[k] = FIRST ? a.v0_l[aa] : 0; vy[k] = FIRST ? a.v0_y[aa] : 0;
+    }
+    // M block [AB][DOUT] -> smem slice
+#pragma unroll
+    for (int k = 0; k < AB * DOUT; ++k) Ms[k * 32 + lane] = 0.f;
+    __syncwarp();
+    for (int k = tb.ptr[ab]; k < tb.ptr[aend]; ++k) {
+      int pk = tb.pack[k];
+      int idx = ((pk & 255) - ab) * DOUT + ((pk >> 8) & 255);
+      Ms[idx * 32 + lane] = fmaf(tb.val[k], Gs[(pk >> 16) * 32 + lane], Ms[idx * 32 + lane]);
+    }
+    __syncwarp();
+    float Mb[AB * DOUT];
+#pragma unroll
+    for (int k = 0; k < AB * DOUT; ++k) Mb[k] = 0.f;
+    for (int64_t e = e0; e < e1; ++e) {
+      float tbar[DOUT];
+#pragma unroll
+      for (int cc = 0; cc < DOUT; ++cc) tbar[cc] = (a.VbarL && act) ? a.VbarL[(e * DOUT + cc) * a.n + nn] : 0.f;
+      if (act) tbar[0] += a.sbar[e * a.lds + nn];
+      float v[AB], vb[AB];
+      float w[NLV];
+      if (FIRST) {
+#pragma unroll
+        for (int l = 0; l < NLV; ++l) w[l] = act ? a.w0[e * a.ldw + l * a.n + nn] : 0.f;
+      }
+#pragma unroll
+      for (int k = 0; k < AB; ++k) {
+        if (FIRST) {
+          float wl = w[0];
+#pragma unroll
+          for (int l = 1; l < NLV; ++l) wl = (vl[k] == l) ? w[l] : wl;
+          v[k] = (ab + k < DIN) ? wl * __ldg(&a.Y[e * DENV + vy[k]]) : 0.f;
+        } else {
+          v[k] = (act && ab + k < DIN) ? a.Vin[(e * DIN + ab + k) * a.n + nn] : 0.f;
+        }
+        float acc = 0.f;
+#pragma unroll
+        for (int cc = 0; cc < DOUT; ++cc) {
+          acc = fmaf(Ms[(k * DOUT + cc) * 32 + lane], tbar[cc], acc);
+          Mb[k * DOUT + cc] = fmaf(v[k], tbar[cc], Mb[k * DOUT + cc]);
+        }
+        vb[k] = acc;
+      }
+      if (FIRST) {
+        float wb[NLV], pp[AB];
+#pragma unroll
+        for (int l = 0; l < NLV; ++l) wb[l] = 0.f;
+#pragma unroll
+        for (int k = 0; k < AB; ++k) {
+          float y = __ldg(&a.Y[e * DENV + vy[k]]);
+          float wl = w[0];
+          bool valid = ab + k < DIN;
+#pragma unroll
+          for (int l = 0; l < NLV; ++l) {
+            bool mm = valid && (vl[k] == l);
+            wb[l] = mm ? fmaf(vb[k], y, wb[l]) : wb[l];
+            wl = (vl[k] == l) ? w[l] : wl;
+          }
+          pp[k] = valid ? wl * vb[k] : 0.f;
+        }
+        // (an invalid tail slot aliases vy of the last component and contributes exactly 0)
+        ybar_accumulate<AB>(Yb + e * DENV, pp, vy, lane);
+        if (act)
+#pragma unroll
+          for (int l = 0; l < NLV; ++l) a.w0bar[e * a.ldob + l * a.n + nn] += wb[l];
+      } else if (act) {
+#pragma unroll
+        for (int k = 0; k < AB; ++k)
+          if (ab + k < DIN) a.Vbar_prev[(e * DIN + ab + k) * a.n + nn] = vb[k];
+      }
+    }
+    // Gamma-bar += K . M-bar(block)
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < AB * DOUT; ++k) Ms[k * 32 + lane] = Mb[k];
+    __syncwarp();
+    for (int k = tb.ptr[ab]; k < tb.ptr[aend]; ++k) {
+      int pk = tb.pack[k];
+      int idx = ((pk & 255) - ab) * DOUT + ((pk >> 8) & 255);
+      Gbs[(pk >> 16) * 32 + lane] = fmaf(tb.val[k], Ms[idx * 32 + lane], Gbs[(pk >> 16) * 32 + lane]);
+    }
+    __syncwarp();
+  }
+  float Gb[DENV];
+  int ident[DENV];
+#pragma unroll
+  for (int b = 0; b < DENV; ++b) { Gb[b] = a.c_env * Gbs[b * 32 + lane]; ident[b] = b; }
+  for (int64_t e = e0; e < e1; ++e) {
+    float om[NLV];
+#pragma unroll
+    for (int l = 0; l < NLV; ++l) om[l] = act ? a.om[e * a.ldo + l * a.n + nn] : 0.f;
+    float pp[DENV];
+#pragma unroll
+    for (int l = 0; l < NLV; ++l) {
+      float ob = 0.f;
+#pragma unroll
+      for (int b = l * l; b < (l + 1) * (l + 1); ++b) {
+        ob = fmaf(Gb[b], __ldg(&a.Y[e * DENV + b]), ob);
+        pp[b] = om[l] * Gb[b];
+      }
+      if (act) a.ombar[e * a.ldob + l * a.n + nn] = ob;
+    }
+    ybar_accumulate<DENV>(Yb + e * DENV, pp, ident, lane);
+  }
+}
+
+template <int DENV, int DIN, int DOUT, int CB, bool FIRST>
+int launch_bfwd(allegro_model* m, const TPW& a) {
+  size_t sm = (size_t)WARPS_PER_BLOCK * (DENV + DIN * CB) * 32 * 4 + (size_t)a.t.nnz * 8 + (DOUT + 1) * 4 + 16;
+  static bool set = false;
+  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tpb_fwd<DENV, DIN, DOUT, CB, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  int64_t warps = (int64_t)a.nc * a.ngroups;
+  k_tpb_fwd<DENV, DIN, DOUT, CB, FIRST><<<(unsigned)((warps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, sm, m->stream>>>(a);
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
+}
+template <int DENV, int DIN, int DOUT, int AB, bool FIRST>
+int launch_bbwd(allegro_model* m, const TPW& a) {
+  size_t sm = (size_t)WARPS_PER_BLOCK * (2 * DENV + AB * DOUT) * 32 * 4 + (size_t)a.t.nnz * 8 + (DIN + 1) * 4 + 16;
+  static bool set = false;
+  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tpb_bwd<DENV, DIN, DOUT, AB, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  int64_t warps = (int64_t)a.nc * a.ngroups;
+  k_tpb_bwd<DENV, DIN, DOUT, AB, FIRST><<<(unsigned)((warps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, sm, m->stream>>>(a);
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
+}
+
 template <int DENV, int DIN, int DOUT, bool FIRST>
 int launch_fwd(allegro_model* m, const TPW& a) {
   size_t sm = (size_t)WARPS_PER_BLOCK * (DENV + DIN * DOUT) * 32 * 4 + (size_t)a.t.nnz * 12 + 16;
@@ -329,6 +586,17 @@ int tpw_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   a.Tout = Tout; a.xs = xs; a.ldx = ldx; a.gamma_out = (float*)w.gamma.p;
   const int DENV = m->Denv, Din = a.t.Din, Dout = a.t.Dout;
   if (Vin == nullptr) { TPW_DISPATCH(launch_fwd, true) } else { TPW_DISPATCH(launch_fwd, false) }
+  if (DENV == 16) {   // l_max = 3: blocked kernels
+    if (Vin == nullptr) {
+      if (Din == 16 && Dout == 31) return launch_bfwd<16, 16, 31, 8, true>(m, a);
+      if (Din == 16 && Dout == 16) return launch_bfwd<16, 16, 16, 8, true>(m, a);
+      if (Din == 16 && Dout == 1) return launch_bfwd<16, 16, 1, 1, true>(m, a);
+    } else {
+      if (Din == 31 && Dout == 16) return launch_bfwd<16, 31, 16, 4, false>(m, a);
+      if (Din == 16 && Dout == 16) return launch_bfwd<16, 16, 16, 8, false>(m, a);
+      if (Din == 16 && Dout == 1) return launch_bfwd<16, 16, 1, 1, false>(m, a);
+    }
+  }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }
 
@@ -340,5 +608,16 @@ int tpw_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   a.Ybar = (float*)w.Ybar.p; a.ybar_gstride = (int64_t)w.cap_edges * m->Denv;
   const int DENV = m->Denv, Din = a.t.Din, Dout = a.t.Dout;
   if (Vin == nullptr) { TPW_DISPATCH(launch_bwd, true) } else { TPW_DISPATCH(launch_bwd, false) }
+  if (DENV == 16) {
+    if (Vin == nullptr) {
+      if (Din == 16 && Dout == 31) return launch_bbwd<16, 16, 31, 4, true>(m, a);
+      if (Din == 16 && Dout == 16) return launch_bbwd<16, 16, 16, 8, true>(m, a);
+      if (Din == 16 && Dout == 1) return launch_bbwd<16, 16, 1, 16, true>(m, a);
+    } else {
+      if (Din == 31 && Dout == 16) return launch_bbwd<16, 31, 16, 8, false>(m, a);
+      if (Din == 16 && Dout == 16) return launch_bbwd<16, 16, 16, 8, false>(m, a);
+      if (Din == 16 && Dout == 1) return launch_bbwd<16, 16, 1, 16, false>(m, a);
+    }
+  }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }
