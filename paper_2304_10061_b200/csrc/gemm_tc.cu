@@ -19,6 +19,16 @@
 
 namespace {
 
+#ifndef EPI_DIRECT
+#define EPI_DIRECT 0
+#endif
+#if EPI_DIRECT
+#define AUX1(i) (*reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col))
+#define AUX2(i) (*reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col))
+#else
+#define AUX1(i) ax1[i]
+#define AUX2(i) ax2[i]
+#endif
 constexpr int BM = 128;          // UMMA M (cta_group::1)
 constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
 constexpr int STAGES = 3;
@@ -202,16 +212,37 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       for (int c0 = chunk0 * 32; c0 < BN; c0 += 32 * (EPI_WARPS / 4)) {
         uint32_t r[32];
         tc_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN_MAX + c0, r);
+#if !EPI_DIRECT
 #pragma unroll
         for (int j = 0; j < 32; ++j) stg[lane * 33 + j] = __uint_as_float(r[j]);
         __syncwarp();
         const int col = nt * BN + c0 + c4;
         const bool col_ok = (col < g.N) && (c0 + c4 < BN);
+        // issue every aux load of this chunk up front (the stores below may alias, so the compiler cannot hoist them)
+        float4 ax1[8], ax2[8];
+        const bool need1 = (g.epi == EPI_LATENT || g.epi == EPI_MUL_DSILU || g.epi == EPI_ADD2);
+        const bool need2 = (g.epi == EPI_ADD2 || g.epi == EPI_ADD2R);
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
+          const int row = rbase + i * 4 + rsub;
+          const bool ok = row < M && col_ok;
+          ax1[i] = (need1 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax2[i] = (need2 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+#endif
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+#if EPI_DIRECT
+          const int row = rbase + lane;
+          const int col = nt * BN + c0 + i * 4;
+          const bool col_ok = (col < g.N) && (c0 + i * 4 < BN);
+          float v[4] = {__uint_as_float(r[i * 4]), __uint_as_float(r[i * 4 + 1]), __uint_as_float(r[i * 4 + 2]),
+                        __uint_as_float(r[i * 4 + 3])};
+#else
           const int rl = i * 4 + rsub;
           const int row = rbase + rl;
           float v[4] = {stg[rl * 33 + c4], stg[rl * 33 + c4 + 1], stg[rl * 33 + c4 + 2], stg[rl * 33 + c4 + 3]};
+#endif
           if (row < M && col_ok) {
             float o[4];
             switch (g.epi) {
@@ -221,7 +252,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(v[0], v[1], v[2], v[3]);
                 float us = (g.epi == EPI_SILU_BOTH) ? 1.0f : g.u[row];
                 if (g.epi == EPI_LATENT) {
-                  float4 x = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
+                  float4 x = AUX1(i);
                   float xo[4] = {x.x, x.y, x.z, x.w};
 #pragma unroll
                   for (int j = 0; j < 4; ++j) o[j] = g.c0 * xo[j] + g.c1 * us * silu_f(v[j]);
@@ -231,20 +262,20 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 }
               } break;
               case EPI_MUL_DSILU: {
-                float4 z = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
+                float4 z = AUX1(i);
                 float zz[4] = {z.x, z.y, z.z, z.w};
 #pragma unroll
                 for (int j = 0; j < 4; ++j) o[j] = v[j] * dsilu_f(zz[j]);
               } break;
               case EPI_ADD2: {
-                float4 x = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
-                float4 y = *reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col);
+                float4 x = AUX1(i);
+                float4 y = AUX2(i);
                 o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
                 o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
               } break;
               case EPI_ADD2R: {
                 float4 x = *reinterpret_cast<const float4*>(g.aux3 + col);
-                float4 y = *reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col);
+                float4 y = AUX2(i);
                 float cs = g.c0 * g.u[row];
                 o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
                 o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
