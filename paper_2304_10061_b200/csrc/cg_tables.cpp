@@ -230,6 +230,17 @@ int al_build_tp_tables(allegro_model* m, const std::vector<std::vector<float>>& 
       std::vector<int> af(t.aent_ptr.begin(), t.aent_ptr.end() - 1);
       for (int k = 0; k < t.nnz; ++k) { int a = t.ce_pack[k] & 255; t.ae_pack[af[a]] = t.ce_pack[k]; t.ae_val[af[a]++] = t.ce_val[k]; }
     }
+    // dense pair table (a-major, c-minor), empty pairs have zero length
+    t.dp_ptr.assign((size_t)t.Din * t.Dout + 1, 0); t.dp_b.clear(); t.dp_val.clear();
+    for (int a = 0; a < t.Din; ++a)
+      for (int c = 0; c < t.Dout; ++c) {
+        for (int b = 0; b < t.Denv; ++b)
+          if (pat[((size_t)a * t.Denv + b) * t.Dout + c]) {
+            t.dp_b.push_back(b);
+            t.dp_val.push_back((float)K[((size_t)a * t.Denv + b) * t.Dout + c]);
+          }
+        t.dp_ptr[(size_t)a * t.Dout + c + 1] = (int)t.dp_b.size();
+      }
     // CSR over c and over a
     t.c_ptr.assign(t.Dout + 1, 0); t.a_ptr.assign(t.Din + 1, 0); t.b_ptr.assign(t.Denv + 1, 0);
     for (int p = 0; p < t.npairs; ++p) { t.c_ptr[t.pair_c[p] + 1]++; t.a_ptr[t.pair_a[p] + 1]++; }

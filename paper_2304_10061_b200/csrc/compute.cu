@@ -16,7 +16,7 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
   if (M > w.cap_edges || w.XS.empty()) {
     auto R = [&](DevBuf& b, size_t floats) { return al_reserve(m, b, floats * 4 + 64); };
     AL_CHECK(R(w.ei, M)); AL_CHECK(R(w.ej, M)); AL_CHECK(R(w.geo, 4 * M)); AL_CHECK(R(w.u, M)); AL_CHECK(R(w.du, M)); AL_CHECK(R(w.sig, M));
-    AL_CHECK(R(w.B, M * m->NB)); AL_CHECK(R(w.dB, M * m->NB)); AL_CHECK(R(w.Y, M * m->Denv));
+    AL_CHECK(R(w.B, M * m->NB)); AL_CHECK(R(w.dB, M * m->NB)); AL_CHECK(R(w.Y, M * m->ldY));
     w.tb_z.resize(hp.n_twobody); w.tb_a.resize(hp.n_twobody);
     int maxw = d + n;
     for (int k = 0; k < hp.n_twobody; ++k) {
@@ -145,6 +145,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   AL_CHECK(k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom));
   // ---- step 11: backward -----------------------------------------------------------------------------------
   AL_CUDA(m, cudaMemsetAsync(w.ubar.p, 0, (size_t)m_cap * 4, st));
+  if (!tp2_eligible(m))                        // (the tp2 kernels write Y-bar before accumulating into it)
   for (int gq = 0; gq < (n + 31) / 32; ++gq)   // one partial Y-bar per 32-channel group (summed in fixed order in k_edge_bwd)
     AL_CUDA(m, cudaMemsetAsync((float*)w.Ybar.p + (size_t)gq * w.cap_edges * m->Denv, 0, (size_t)m_cap * m->Denv * 4, st));
   float* xb = (float*)w.XB0.p; float* xb_o = (float*)w.XB1.p;
@@ -311,7 +312,7 @@ extern "C" int allegro_debug_tensor(allegro_model* m, const char* name, float* o
   std::string s(name);
   const float* src = nullptr; int width = 0, ld = 0; int64_t rows = M;
   int d = m->d, n = m->n;
-  if (s == "Y") { src = (float*)w.Y.p; width = ld = m->Denv; }
+  if (s == "Y") { src = (float*)w.Y.p; width = m->Denv; ld = m->ldY; }
   else if (s == "u") { src = (float*)w.u.p; width = ld = 1; }
   else if (s == "B") { src = (float*)w.B.p; width = ld = m->NB; }
   else if (s == "geo") { src = (float*)w.geo.p; width = ld = 4; }

@@ -103,7 +103,7 @@ __global__ void k_set_mact(const int64_t* __restrict__ rowa, int nc, int* __rest
 
 __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, int* __restrict__ ei, int* __restrict__ ej,
                             float4* __restrict__ geo, float* __restrict__ u, float* __restrict__ du,
-                            float* __restrict__ B, float* __restrict__ dB, float* __restrict__ Y, int Denv,
+                            float* __restrict__ B, float* __restrict__ dB, float* __restrict__ Y, int Denv, int ldy,
                             int* __restrict__ flags, float* __restrict__ sig, const double* __restrict__ sigma) {
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= a.nc) return;
@@ -145,7 +145,7 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
       }
       float yy[16];
       sph_harm(hx, hy, hz, a.lmax, yy);
-      for (int q = 0; q < Denv; ++q) Y[o * Denv + q] = yy[q];
+      for (int q = 0; q < ldy; ++q) Y[o * ldy + q] = (q < Denv) ? yy[q] : 0.f;
     }
     cnt += __popc(mask);
   }
@@ -195,7 +195,7 @@ __global__ void k_twobody0(const int* __restrict__ m_ptr, const int* __restrict_
 struct TPArgs {
   const int64_t* rowa;
   const float* om; int ldo;       // omega^L  [M][(l,n)]
-  const float* Y; int Denv;
+  const float* Y; int Denv, ldy;
   const float* Vin;               // [M][Din][n] or null (FIRST)
   const float* w0; int ldw;       // FIRST: w^0 [M][(l,n)]
   const int *v0_l, *v0_y, *env_l;
@@ -215,7 +215,7 @@ struct TPArgs {
 
 template <bool FIRST>
 __device__ __forceinline__ float v_load(const TPArgs& a, int64_t e, int comp, int nn) {
-  if (FIRST) return a.w0[e * a.ldw + a.v0_l[comp] * a.n + nn] * a.Y[e * a.Denv + a.v0_y[comp]];
+  if (FIRST) return a.w0[e * a.ldw + a.v0_l[comp] * a.n + nn] * a.Y[e * a.ldy + a.v0_y[comp]];
   return a.Vin[(e * a.t.Din + comp) * a.n + nn];
 }
 
@@ -224,7 +224,7 @@ __device__ __forceinline__ void tp_gamma_M(const TPArgs& a, int64_t e0, int64_t 
   for (int idx = threadIdx.x; idx < a.Denv * n; idx += blockDim.x) {
     int b = idx / n, nn = idx - b * n, l = a.env_l[b];
     float acc = 0.f;
-    for (int64_t e = e0; e < e1; ++e) acc = fmaf(a.om[e * a.ldo + l * n + nn], a.Y[e * a.Denv + b], acc);
+    for (int64_t e = e0; e < e1; ++e) acc = fmaf(a.om[e * a.ldo + l * n + nn], a.Y[e * a.ldy + b], acc);
     G[idx] = a.c_env * acc;
   }
   __syncthreads();
@@ -315,7 +315,7 @@ __global__ void __launch_bounds__(256) k_tp_bwd(TPArgs a) {
     int el = idx / (nl * n), rem = idx - el * nl * n, l = rem / n, nn = rem - l * n;
     int64_t e = e0 + el;
     float acc = 0.f;
-    for (int b = l * l; b < (l + 1) * (l + 1); ++b) acc = fmaf(G[b * n + nn], a.Y[e * a.Denv + b], acc);
+    for (int b = l * l; b < (l + 1) * (l + 1); ++b) acc = fmaf(G[b * n + nn], a.Y[e * a.ldy + b], acc);
     a.ombar[e * a.ldob + l * n + nn] = a.c_env * acc;
   }
   // Y-bar_e[b] += c_env sum_n omega_e[l(b),n] Gamma-bar[b,n]
@@ -336,7 +336,7 @@ __global__ void __launch_bounds__(256) k_tp_bwd(TPArgs a) {
       int64_t e = e0 + el;
       float acc = 0.f;
       for (int aa = 0; aa < a.t.Din; ++aa)
-        if (a.v0_l[aa] == l) acc = fmaf(a.Vbar_prev[(e * a.t.Din + aa) * n + nn], a.Y[e * a.Denv + a.v0_y[aa]], acc);
+        if (a.v0_l[aa] == l) acc = fmaf(a.Vbar_prev[(e * a.t.Din + aa) * n + nn], a.Y[e * a.ldy + a.v0_y[aa]], acc);
       a.w0bar[e * a.ldob + l * n + nn] = acc;
     }
     for (int item = warp; item < deg * a.t.Din; item += nw) {
@@ -506,7 +506,7 @@ int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* r
   if (a.nc <= 0) return ALLEGRO_OK;
   k_geom_fill<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, rowa, (int*)w.ei.p, (int*)w.ej.p, (float4*)w.geo.p,
                                                            (float*)w.u.p, (float*)w.du.p, (float*)w.B.p, (float*)w.dB.p,
-                                                           (float*)w.Y.p, m->Denv, (int*)w.m_act.p, (float*)w.sig.p, m->sigma);
+                                                           (float*)w.Y.p, m->Denv, m->ldY, (int*)w.m_act.p, (float*)w.sig.p, m->sigma);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
@@ -528,7 +528,7 @@ static size_t tp_smem(const allegro_model* m, int L) { return (size_t)(m->Denv +
 static void tp_common(allegro_model* m, Work& w, int L, TPArgs& a, const float* om, int ldo, const float* Vin,
                       const float* w0, int ldw) {
   a.rowa = (const int64_t*)w.rowa.p;
-  a.om = om; a.ldo = ldo; a.Y = (const float*)w.Y.p; a.Denv = m->Denv;
+  a.om = om; a.ldo = ldo; a.Y = (const float*)w.Y.p; a.Denv = m->Denv; a.ldy = m->ldY;
   a.Vin = Vin; a.w0 = w0; a.ldw = ldw;
   a.v0_l = m->d_v0_l; a.v0_y = m->d_v0_y; a.env_l = m->d_env_l;
   a.t = m->tp[L - 1]; a.n = m->n; a.lmax = m->lmax; a.c_env = m->c_env;
@@ -539,12 +539,19 @@ int tpw_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
 int tpw_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
             const float* VbarL, const float* sbar, int lds, float* Vbar_prev, float* ombar, int ldob, float* w0bar);
 
+int tp2_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
+            float* Tout, float* xs, int ldx);
+int tp2_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
+            const float* VbarL, const float* sbar, int lds, float* Vbar_prev, float* ombar, int ldob, float* w0bar);
+
 int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin,
                     const float* w0, int ldw, float* Tout, float* xs, int ldx) {
   ProfScope _ps(m, PC_TP_FWD);
   if (nc <= 0) return ALLEGRO_OK;
   {
-    int rc = tpw_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);   // warp-per-(center, channel group) fast path
+    int rc = tp2_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);   // cp.async ring + FFMA2 (tp2_kernels.cu)
+    if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
+    rc = tpw_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);       // warp-per-(center, channel group) fallback
     if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
   }
   TPArgs a{};
@@ -568,7 +575,9 @@ int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
   ProfScope _ps(m, PC_TP_BWD);
   if (nc <= 0) return ALLEGRO_OK;
   {
-    int rc = tpw_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
+    int rc = tp2_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
+    if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
+    rc = tpw_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
     if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
   }
   TPArgs a{};

@@ -43,6 +43,8 @@ struct TPLayerHost {
   std::vector<int> ent_idx;                   // [nnz] a*Dout + c of the entry's pair
   // packed entry lists (a | c<<8 | b<<16, val): sorted by c (ce_*, cent_ptr[Dout+1]) and by a (ae_*, aent_ptr[Din+1])
   std::vector<int> ce_pack, cent_ptr, ae_pack, aent_ptr; std::vector<float> ce_val, ae_val;
+  // dense pair table: entries (b, val) of pair (a, c) are dp_b/dp_val[dp_ptr[a*Dout+c] .. dp_ptr[a*Dout+c+1])
+  std::vector<int> dp_ptr, dp_b; std::vector<float> dp_val;
   // CSR over output component c -> (a, pair)
   std::vector<int> c_ptr, c_a, c_p;
   // CSR over input component a -> (c, pair)
@@ -60,6 +62,7 @@ struct TPLayerDev {
   int *a_ptr, *a_c, *a_p;
   int *b_ptr, *b_p; float* b_val;
   int *ce_pack, *cent_ptr, *ae_pack, *aent_ptr; float *ce_val, *ae_val;
+  int *dp_ptr, *dp_b; float* dp_val;
 };
 
 struct Dense {
@@ -88,7 +91,7 @@ struct allegro_nbr {
 
 struct allegro_model {
   allegro_hparams hp;
-  int S, NB, d, n, lmax, NL, Denv, nA;
+  int S, NB, d, n, lmax, NL, Denv, nA, ldY;   // ldY = Denv rounded up to a multiple of 4 (float4 rows of Y)
   std::vector<TPLayerHost> tp_host;       // [NL]
   std::vector<TPLayerDev> tp;             // [NL]
   std::vector<int> D;                     // D_0..D_NL

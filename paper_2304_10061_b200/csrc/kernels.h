@@ -40,6 +40,7 @@ struct EdgeGeomArgs {
   int64_t c0; int nc;                                               // centers [c0, c0+nc)
 };
 
+bool tp2_eligible(const allegro_model* m);   // tp2_kernels.cu
 int k_launch_active_count(allegro_model* m, const EdgeGeomArgs& a, int* deg);
 int k_launch_set_mact(allegro_model* m, const int64_t* rowa, int nc, int* m_act);
 int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* rowa, Work& w);

@@ -160,7 +160,7 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
   m->hp = *hp;
   m->S = hp->n_species; m->NB = hp->n_bessel; m->d = hp->twobody_dims[hp->n_twobody - 1];
   m->n = hp->n_tensor; m->lmax = hp->l_max; m->NL = hp->n_layers;
-  m->Denv = (m->lmax + 1) * (m->lmax + 1); m->nA = m->n * (m->lmax + 1);
+  m->Denv = (m->lmax + 1) * (m->lmax + 1); m->nA = m->n * (m->lmax + 1); m->ldY = (m->Denv + 3) & ~3;
   int dev = 0; cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev);
   m->c_env = (float)(1.0 / std::sqrt(hp->avg_num_neighbors));
@@ -258,7 +258,8 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
         (rc = upload(m, &t.a_c, h.a_c)) || (rc = upload(m, &t.a_p, h.a_p)) || (rc = upload(m, &t.b_ptr, h.b_ptr)) ||
         (rc = upload(m, &t.b_p, h.b_p)) || (rc = upload(m, &t.b_val, h.b_val)) ||
         (rc = upload(m, &t.ce_pack, h.ce_pack)) || (rc = upload(m, &t.cent_ptr, h.cent_ptr)) || (rc = upload(m, &t.ce_val, h.ce_val)) ||
-        (rc = upload(m, &t.ae_pack, h.ae_pack)) || (rc = upload(m, &t.aent_ptr, h.aent_ptr)) || (rc = upload(m, &t.ae_val, h.ae_val)))
+        (rc = upload(m, &t.ae_pack, h.ae_pack)) || (rc = upload(m, &t.aent_ptr, h.aent_ptr)) || (rc = upload(m, &t.ae_val, h.ae_val)) ||
+        (rc = upload(m, &t.dp_ptr, h.dp_ptr)) || (rc = upload(m, &t.dp_b, h.dp_b)) || (rc = upload(m, &t.dp_val, h.dp_val)))
       return fail(rc);
   }
   std::vector<int> env_l;

@@ -67,7 +67,7 @@ __device__ __forceinline__ void ybar_accumulate(float* yrow, const float* p, con
 struct TPW {
   const int64_t* rowa; int nc;
   const float* om; int ldo;
-  const float* Y;
+  const float* Y; int ldy;
   const float* Vin;
   const float* w0; int ldw;
   const int *v0_l, *v0_y, *env_l;
@@ -105,7 +105,7 @@ __device__ __forceinline__ void gamma_and_M(const TPW& a, const SmemTables& tb, 
 #pragma unroll
     for (int l = 0; l < NLV; ++l)
 #pragma unroll
-      for (int b = l * l; b < (l + 1) * (l + 1); ++b) G[b] = fmaf(om[l], __ldg(&a.Y[e * DENV + b]), G[b]);
+      for (int b = l * l; b < (l + 1) * (l + 1); ++b) G[b] = fmaf(om[l], __ldg(&a.Y[e * a.ldy + b]), G[b]);
   }
 #pragma unroll
   for (int b = 0; b < DENV; ++b) Gs[b * 32 + lane] = a.c_env * G[b];
@@ -128,7 +128,7 @@ __device__ __forceinline__ void load_v(const TPW& a, int64_t e, int nn, bool act
       float wl = w[0];
 #pragma unroll
       for (int l = 1; l < NLV; ++l) wl = (vl[k] == l) ? w[l] : wl;
-      v[k] = wl * __ldg(&a.Y[e * DENV + vy[k]]);
+      v[k] = wl * __ldg(&a.Y[e * a.ldy + vy[k]]);
     }
   } else {
 #pragma unroll
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpw_bwd(TPW a) {
       float pp[DIN];
 #pragma unroll
       for (int k = 0; k < DIN; ++k) {
-        float y = __ldg(&a.Y[e * DENV + vy[k]]);
+        float y = __ldg(&a.Y[e * a.ldy + vy[k]]);
         float wl = w[0];
 #pragma unroll
         for (int l = 0; l < NLV; ++l) {
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpw_bwd(TPW a) {
       float ob = 0.f;
 #pragma unroll
       for (int b = l * l; b < (l + 1) * (l + 1); ++b) {
-        ob = fmaf(Gb[b], __ldg(&a.Y[e * DENV + b]), ob);
+        ob = fmaf(Gb[b], __ldg(&a.Y[e * a.ldy + b]), ob);
         pp[b] = om[l] * Gb[b];
       }
       if (act) a.ombar[e * a.ldob + l * a.n + nn] = ob;
@@ -312,7 +312,7 @@ __device__ __forceinline__ void gamma_only(const TPW& a, int64_t e0, int64_t e1,
 #pragma unroll
     for (int l = 0; l < NLV; ++l)
 #pragma unroll
-      for (int b = l * l; b < (l + 1) * (l + 1); ++b) G[b] = fmaf(om[l], __ldg(&a.Y[e * DENV + b]), G[b]);
+      for (int b = l * l; b < (l + 1) * (l + 1); ++b) G[b] = fmaf(om[l], __ldg(&a.Y[e * a.ldy + b]), G[b]);
   }
 #pragma unroll
   for (int b = 0; b < DENV; ++b) Gs[b * 32 + lane] = a.c_env * G[b];
@@ -440,7 +440,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpb_bwd(TPW a) {
           float wl = w[0];
 #pragma unroll
           for (int l = 1; l < NLV; ++l) wl = (vl[k] == l) ? w[l] : wl;
-          v[k] = (ab + k < DIN) ? wl * __ldg(&a.Y[e * DENV + vy[k]]) : 0.f;
+          v[k] = (ab + k < DIN) ? wl * __ldg(&a.Y[e * a.ldy + vy[k]]) : 0.f;
         } else {
           v[k] = (act && ab + k < DIN) ? a.Vin[(e * DIN + ab + k) * a.n + nn] : 0.f;
         }
@@ -458,7 +458,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpb_bwd(TPW a) {
         for (int l = 0; l < NLV; ++l) wb[l] = 0.f;
 #pragma unroll
         for (int k = 0; k < AB; ++k) {
-          float y = __ldg(&a.Y[e * DENV + vy[k]]);
+          float y = __ldg(&a.Y[e * a.ldy + vy[k]]);
           float wl = w[0];
           bool valid = ab + k < DIN;
 #pragma unroll
@@ -506,7 +506,7 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpb_bwd(TPW a) {
       float ob = 0.f;
 #pragma unroll
       for (int b = l * l; b < (l + 1) * (l + 1); ++b) {
-        ob = fmaf(Gb[b], __ldg(&a.Y[e * DENV + b]), ob);
+        ob = fmaf(Gb[b], __ldg(&a.Y[e * a.ldy + b]), ob);
         pp[b] = om[l] * Gb[b];
       }
       if (act) a.ombar[e * a.ldob + l * a.n + nn] = ob;
@@ -574,7 +574,7 @@ int launch_bwd(allegro_model* m, const TPW& a) {
 
 static void fill(allegro_model* m, Work& w, int L, int nc, TPW& a, const float* om, int ldo, const float* Vin,
                  const float* w0, int ldw) {
-  a.rowa = (const int64_t*)w.rowa.p; a.nc = nc; a.om = om; a.ldo = ldo; a.Y = (const float*)w.Y.p; a.Vin = Vin;
+  a.rowa = (const int64_t*)w.rowa.p; a.nc = nc; a.om = om; a.ldo = ldo; a.Y = (const float*)w.Y.p; a.ldy = m->ldY; a.Vin = Vin;
   a.w0 = w0; a.ldw = ldw; a.v0_l = m->d_v0_l; a.v0_y = m->d_v0_y; a.env_l = m->d_env_l; a.t = m->tp[L - 1];
   a.n = m->n; a.ngroups = (m->n + 31) / 32; a.c_env = m->c_env;
 }
