@@ -8,63 +8,70 @@
 //   * the per-edge operand rows (V_e / w0_e, Y_e, T-bar_e) stream through a per-warp cp.async ring in
 //     shared memory (NST stages of one edge each), so the loads in flight do not cost registers;
 //   * M_i (and the backward's M-bar_i) live in registers as float2 pairs over the output component and
-//     all inner products are packed FFMA2 (two fp32 FMAs per issue slot on sm_100);
+//     all inner products are packed FFMA2;
+//   * the sparsity pattern of K is a compile-time X-macro list (tp2_patterns.inc, generated at build time
+//     from cg_tables.cpp), so M_i = K.Gamma_i and Gamma-bar_i = K.M-bar_i are straight-line FFMAs with
+//     literal register indices; the values (which carry the path weights) come from the kernel parameters
+//     (constant bank);
 //   * wide features (l_max = 3) walk blocks of output components (forward) / input components (backward);
 //   * Y-bar is written, not accumulated, by the first kernel of a step that touches it (no memset).
-// Requirements (checked on the host, otherwise the kernels of tp_kernels.cu run): n % 32 == 0 and the
-// V^0 layout equal to the environment layout (always true for S_0 = env irreps).
+// Requirements (checked on the host, otherwise the kernels of tp_kernels.cu run): n % 32 == 0, V^0 layout
+// equal to the environment layout, and every layer's pattern equal to a generated one.
 #pragma once
 #include <cstdlib>
+#include <cstring>
 
 #include "kernels.h"
+#include "tp2_patterns.inc"
 #include "tp_common.cuh"
 
+enum { P_9_9_9 = 0, P_9_9_1, P_4_4_4, P_4_4_1, P_16_16_31, P_16_31_16, P_16_16_1, P_COUNT };
+template <int P> struct Pat;
+template <> struct Pat<P_9_9_9> { static constexpr int DENV = 9, DIN = 9, DOUT = 9, NNZ = TP2_NNZ_9_9_9; };
+template <> struct Pat<P_9_9_1> { static constexpr int DENV = 9, DIN = 9, DOUT = 1, NNZ = TP2_NNZ_9_9_1; };
+template <> struct Pat<P_4_4_4> { static constexpr int DENV = 4, DIN = 4, DOUT = 4, NNZ = TP2_NNZ_4_4_4; };
+template <> struct Pat<P_4_4_1> { static constexpr int DENV = 4, DIN = 4, DOUT = 1, NNZ = TP2_NNZ_4_4_1; };
+template <> struct Pat<P_16_16_31> { static constexpr int DENV = 16, DIN = 16, DOUT = 31, NNZ = TP2_NNZ_16_16_31; };
+template <> struct Pat<P_16_31_16> { static constexpr int DENV = 16, DIN = 31, DOUT = 16, NNZ = TP2_NNZ_16_31_16; };
+template <> struct Pat<P_16_16_1> { static constexpr int DENV = 16, DIN = 16, DOUT = 1, NNZ = TP2_NNZ_16_16_1; };
+
+// expands X(k, a, b, c) over the entries of pattern P (P is a template parameter at the point of use)
+#define TP2_EXPAND(P, X)                                            \
+  if constexpr (P == P_9_9_9) { TP2_PAT_9_9_9(X) }                  \
+  else if constexpr (P == P_9_9_1) { TP2_PAT_9_9_1(X) }             \
+  else if constexpr (P == P_4_4_4) { TP2_PAT_4_4_4(X) }             \
+  else if constexpr (P == P_4_4_1) { TP2_PAT_4_4_1(X) }             \
+  else if constexpr (P == P_16_16_31) { TP2_PAT_16_16_31(X) }       \
+  else if constexpr (P == P_16_31_16) { TP2_PAT_16_31_16(X) }       \
+  else if constexpr (P == P_16_16_1) { TP2_PAT_16_16_1(X) }
+
+template <int NNZ>
 struct TP2 {
   const int64_t* rowa; int nc;
   const float* om; int ldo;
   const float* Y; int ldy;
   const float* Vin;
   const float* w0; int ldw;
-  const int* dp_ptr; const int* dp_b; const float* dp_val; int nnz;
   int n, ngroups; float c_env;
   float* Tout; float* xs; int ldx; float* gamma_out;
   const float* VbarL; const float* sbar; int lds;
   float* Vbar_prev; float* ombar; int ldob; float* w0bar; float* Ybar; int64_t ybar_gstride;
+  float kv[NNZ];   // values of the fused tensor K in pattern order (dense pair table order)
 };
 
 __host__ __device__ constexpr int l_of(int k) { return k < 1 ? 0 : k < 4 ? 1 : k < 9 ? 2 : 3; }
 __host__ __device__ constexpr int nlv_of(int denv) { return denv == 1 ? 1 : denv == 4 ? 2 : denv == 9 ? 3 : 4; }
-__host__ __device__ constexpr int tab_ints(int din, int dout) { return (din * dout + 1 + 3) & ~3; }
-
-struct Tables { const int* ptr; const int* b; const float* val; };
-
-// block-wide: stage the dense pair table of the fused tensor K in shared memory
-template <int DIN, int DOUT>
-__device__ __forceinline__ Tables load_tables(const TP2& a, float* smem_tab) {
-  int* sp = (int*)smem_tab;
-  int* sb = sp + tab_ints(DIN, DOUT);
-  float* sv = (float*)(sb + a.nnz);
-  for (int k = threadIdx.x; k < DIN * DOUT + 1; k += blockDim.x) sp[k] = a.dp_ptr[k];
-  for (int k = threadIdx.x; k < a.nnz; k += blockDim.x) { sb[k] = a.dp_b[k]; sv[k] = a.dp_val[k]; }
-  __syncthreads();
-  return Tables{sp, sb, sv};
-}
-
-// M_i[a][c] for one (a, c) pair from Gamma_i in the warp's shared slice
-__device__ __forceinline__ float pair_val(const Tables& t, int p, const float* Gs, int lane) {
-  float acc = 0.f;
-  for (int k = t.ptr[p]; k < t.ptr[p + 1]; ++k) acc = fmaf(t.val[k], Gs[t.b[k] * 32 + lane], acc);
-  return acc;
-}
 
 template <int LDY>
 __device__ __forceinline__ float ycomp(const float4* y, int b) { return reinterpret_cast<const float*>(y)[b]; }
 
-// Gamma_i[b] = c_env sum_e omega_e[l(b)] Y_e[b]  ->  Gs[b*32 + lane]   (direct loads, 4 edges in flight)
-template <int DENV>
-__device__ __forceinline__ void gamma_pass(const TP2& a, int64_t e0, int64_t e1, int nn, int lane, float* Gs) {
+// element (r, cc) of a register matrix stored as float2 pairs over the second index, W pairs per row
+#define TP2_REF(M, W, r, cc) (((cc) & 1) ? M[(r) * (W) + ((cc) >> 1)].y : M[(r) * (W) + ((cc) >> 1)].x)
+
+// Gamma_i[b] = c_env sum_e omega_e[l(b)] Y_e[b]   (direct loads, 4 edges in flight)
+template <int DENV, class A>
+__device__ __forceinline__ void gamma_pass(const A& a, int64_t e0, int64_t e1, int nn, float* G) {
   constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3;
-  float G[DENV];
 #pragma unroll
   for (int b = 0; b < DENV; ++b) G[b] = 0.f;
   for (int64_t e = e0; e < e1; e += 4) {
@@ -86,30 +93,27 @@ __device__ __forceinline__ void gamma_pass(const TP2& a, int64_t e0, int64_t e1,
     }
   }
 #pragma unroll
-  for (int b = 0; b < DENV; ++b) Gs[b * 32 + lane] = a.c_env * G[b];
-  __syncwarp();
+  for (int b = 0; b < DENV; ++b) G[b] *= a.c_env;
 }
 
 // ======================================================================================================
 // forward:  T_e[c] = sum_a V_e[a] M_i[a][c]   (c-blocks of CB output components; CB == DOUT: one pass)
 // ======================================================================================================
-template <int DENV, int DIN, int DOUT, int CB, bool FIRST, int NST, int WPB>
-static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(TP2 a) {
+template <int P, int CB, bool FIRST, int NST, int WPB>
+static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(const __grid_constant__ TP2<Pat<P>::NNZ> a) {
+  constexpr int DENV = Pat<P>::DENV, DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
   constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3, CBH = (CB + 1) / 2;
   constexpr int SF = FIRST ? NLV * 32 + LDY : DIN * 32;   // floats per ring stage (one edge)
-  constexpr int SCR = CBH * 64;                           // one row of M as float2 per lane (lane-private scratch)
-  constexpr int WSL = DENV * 32 + SCR + NST * SF;         // floats per warp slice
+  constexpr int WSL = DENV * 32 + NST * SF;               // floats per warp slice
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const Tables tb = load_tables<DIN, DOUT>(a, smem + WPB * WSL);
   const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * a.ngroups) return;
   const int c = (int)(wg / a.ngroups), grp = (int)(wg - (int64_t)c * a.ngroups);
   const int nn = grp * 32 + lane;
   float* Gs = smem + wib * WSL;
-  float* scr = Gs + DENV * 32;
-  float* ring = scr + SCR;
+  float* ring = Gs + DENV * 32;
   const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
   const int deg = (int)(e1 - e0);
   if (deg <= 0) return;
@@ -128,24 +132,29 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(TP2 a) {
     if (s < deg) issue(e0 + s, ring + s * SF);
     tp_cp_commit();
   }
-  gamma_pass<DENV>(a, e0, e1, nn, lane, Gs);
-  if (a.gamma_out)
+  {
+    float G[DENV];
+    gamma_pass<DENV>(a, e0, e1, nn, G);
 #pragma unroll
-    for (int b = 0; b < DENV; ++b) a.gamma_out[((size_t)c * DENV + b) * a.n + nn] = Gs[b * 32 + lane];
+    for (int b = 0; b < DENV; ++b) Gs[b * 32 + lane] = G[b];
+    if (a.gamma_out)
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) a.gamma_out[((size_t)c * DENV + b) * a.n + nn] = G[b];
+  }
 
+#pragma unroll
   for (int cb = 0; cb < DOUT; cb += CB) {
-    // M block -> registers, one row at a time through the lane-private scratch (rolled loops: the fully
-    // unrolled build overflowed the instruction cache, ncu "no_instructions" 60 %)
     float2 Mr[DIN * CBH];
+    {
+      float G[DENV];
 #pragma unroll
-    for (int k = 0; k < DIN; ++k) {
-#pragma unroll 1
-      for (int cc = 0; cc < 2 * CBH; ++cc) {
-        const int ca = cb + cc;
-        scr[((cc >> 1) * 32 + lane) * 2 + (cc & 1)] = (cc < CB && ca < DOUT) ? pair_val(tb, k * DOUT + ca, Gs, lane) : 0.f;
-      }
+      for (int b = 0; b < DENV; ++b) G[b] = Gs[b * 32 + lane];
 #pragma unroll
-      for (int j = 0; j < CBH; ++j) Mr[k * CBH + j] = reinterpret_cast<const float2*>(scr)[j * 32 + lane];
+      for (int k = 0; k < DIN * CBH; ++k) Mr[k] = make_float2(0.f, 0.f);
+#define X(k, a_, b_, c_) \
+  if ((c_) >= cb && (c_) < cb + CB) TP2_REF(Mr, CBH, a_, (c_) - cb) = fmaf(a.kv[k], G[b_], TP2_REF(Mr, CBH, a_, (c_) - cb));
+      TP2_EXPAND(P, X)
+#undef X
     }
     if (cb > 0) {   // restart the ring for this block of output components
       __syncwarp();
@@ -196,18 +205,17 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(TP2 a) {
 //   FIRST (V^0 = w^0 (x) Y):  w0-bar_e[l] = sum_{a in l} V-bar^0_e[a] Y_e[a] ;  Y-bar_e[a] += sum_n w0_e[l(a)] V-bar^0_e[a]
 // a-blocks of AB input components; M block in registers (MREG) or in the warp's shared slice.
 // ======================================================================================================
-template <int DENV, int DIN, int DOUT, int AB, bool FIRST, bool HASVB, bool MREG, bool YINIT, int NST, int WPB>
-static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
+template <int P, int AB, bool FIRST, bool HASVB, bool MREG, bool YINIT, int NST, int WPB>
+static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_constant__ TP2<Pat<P>::NNZ> a) {
+  constexpr int DENV = Pat<P>::DENV, DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
   constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3, CH = (DOUT + 1) / 2;
   constexpr int SV = FIRST ? NLV * 32 + LDY : AB * 32;      // operand part of a stage
   constexpr int SF = SV + (HASVB ? DOUT * 32 : 0) + 32;     // + T-bar rows + s-bar row
   constexpr int MSL = MREG ? 0 : AB * CH * 64;              // M block as float2 per lane
-  constexpr int SCR = CH * 64;                              // one row of M / M-bar (lane-private scratch)
-  constexpr int WSL = 2 * DENV * 32 + MSL + SCR + NST * SF;
+  constexpr int WSL = 2 * DENV * 32 + MSL + NST * SF;
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const Tables tb = load_tables<DIN, DOUT>(a, smem + WPB * WSL);
   const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * a.ngroups) return;
   const int c = (int)(wg / a.ngroups), grp = (int)(wg - (int64_t)c * a.ngroups);
@@ -215,8 +223,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
   float* Gs = smem + wib * WSL;
   float* Gbs = Gs + DENV * 32;
   float2* Ms = reinterpret_cast<float2*>(Gbs + DENV * 32);
-  float* scr = Gbs + DENV * 32 + MSL;
-  float* ring = scr + SCR;
+  float* ring = Gbs + DENV * 32 + MSL;
   const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
   const int deg = (int)(e1 - e0);
   if (deg <= 0) return;
@@ -239,32 +246,46 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
     if (s < deg) issue(e0 + s, ring + s * SF, 0);
     tp_cp_commit();
   }
-  gamma_pass<DENV>(a, e0, e1, nn, lane, Gs);
+  {
+    float G[DENV];
+    gamma_pass<DENV>(a, e0, e1, nn, G);
 #pragma unroll
-  for (int b = 0; b < DENV; ++b) Gbs[b * 32 + lane] = 0.f;
+    for (int b = 0; b < DENV; ++b) { Gs[b * 32 + lane] = G[b]; Gbs[b * 32 + lane] = 0.f; }
+  }
 
+#pragma unroll
   for (int ab = 0; ab < DIN; ab += AB) {
     // for a ragged last block the staged rows start at a0 = DIN - AB; slot k of the block reads row k + (ab - a0)
     const int a0 = (FIRST || ab + AB <= DIN) ? ab : DIN - AB;
     const int roff = ab - a0;
     float2 Mr[MREG ? AB * CH : 1];
     float2 Mb[AB * CH];
-    if constexpr (MREG) {
+    {
+      float G[DENV];
 #pragma unroll
-      for (int k = 0; k < AB; ++k) {
-#pragma unroll 1
-        for (int cc = 0; cc < 2 * CH; ++cc)
-          scr[((cc >> 1) * 32 + lane) * 2 + (cc & 1)] = (cc < DOUT && ab + k < DIN) ? pair_val(tb, (ab + k) * DOUT + cc, Gs, lane) : 0.f;
+      for (int b = 0; b < DENV; ++b) G[b] = Gs[b * 32 + lane];
+      if constexpr (MREG) {
 #pragma unroll
-        for (int j = 0; j < CH; ++j) Mr[k * CH + j] = reinterpret_cast<const float2*>(scr)[j * 32 + lane];
+        for (int k = 0; k < AB * CH; ++k) Mr[k] = make_float2(0.f, 0.f);
+#define X(k, a_, b_, c_) \
+  if ((a_) >= ab && (a_) < ab + AB) TP2_REF(Mr, CH, (a_) - ab, c_) = fmaf(a.kv[k], G[b_], TP2_REF(Mr, CH, (a_) - ab, c_));
+        TP2_EXPAND(P, X)
+#undef X
+      } else {
+        // one row of the block at a time: accumulate in registers, park in the warp's shared slice
+#pragma unroll
+        for (int r = 0; r < AB; ++r) {
+          float2 row[CH];
+#pragma unroll
+          for (int j = 0; j < CH; ++j) row[j] = make_float2(0.f, 0.f);
+#define X(k, a_, b_, c_) \
+  if ((a_) == ab + r) TP2_REF(row, CH, 0, c_) = fmaf(a.kv[k], G[b_], TP2_REF(row, CH, 0, c_));
+          TP2_EXPAND(P, X)
+#undef X
+#pragma unroll
+          for (int j = 0; j < CH; ++j) Ms[(r * CH + j) * 32 + lane] = row[j];
+        }
       }
-    } else {
-#pragma unroll 1
-      for (int k = 0; k < AB; ++k)
-#pragma unroll 1
-        for (int cc = 0; cc < 2 * CH; ++cc)
-          reinterpret_cast<float*>(Ms)[((k * CH + (cc >> 1)) * 32 + lane) * 2 + (cc & 1)] =
-              (cc < DOUT && ab + k < DIN) ? pair_val(tb, (ab + k) * DOUT + cc, Gs, lane) : 0.f;
     }
 #pragma unroll
     for (int k = 0; k < AB * CH; ++k) Mb[k] = make_float2(0.f, 0.f);
@@ -276,7 +297,6 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
         tp_cp_commit();
       }
     }
-    __syncwarp();
     int slot = 0;
     for (int i = 0; i < deg; ++i) {
       tp_cp_wait<NST - 2>();
@@ -309,9 +329,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
         float v, y = 0.f, wl = 0.f;
         if (FIRST) {
           y = st[NLV * 32 + ka];
-          wl = w[0];
-#pragma unroll
-          for (int l = 1; l < NLV; ++l) wl = (l_of(ka) == l) ? w[l] : wl;
+          wl = w[l_of(ka)];
           v = valid ? wl * y : 0.f;
         } else {
           v = valid ? st[(k + roff) * 32 + lane] : 0.f;
@@ -327,8 +345,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
         }
         vb[k] = s2.x + s2.y;
         if (FIRST) {
-#pragma unroll
-          for (int l = 0; l < NLV; ++l) wb[l] = (valid && l_of(ka) == l) ? fmaf(vb[k], y, wb[l]) : wb[l];
+          if (valid) wb[l_of(ka)] = fmaf(vb[k], y, wb[l_of(ka)]);
           pp[k] = valid ? wl * vb[k] : 0.f;
         }
       }
@@ -337,8 +354,13 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
         tp_ybar_rows<AB, YINIT>(Yb + e * DENV, pp, ab, nvalid, lane);
 #pragma unroll
         for (int l = 0; l < NLV; ++l) {
-          float* p = a.w0bar + e * a.ldob + l * a.n + nn;
-          if (ab == 0) *p = wb[l]; else *p += wb[l];
+          // (a block only touches the l values of its own components; the first toucher stores)
+          const bool touched = l_of(ab) <= l && l <= l_of((ab + AB - 1 < DIN) ? ab + AB - 1 : DIN - 1);
+          const bool first_touch = (ab == 0) || l_of(ab - 1) < l;
+          if (touched) {
+            float* p = a.w0bar + e * a.ldob + l * a.n + nn;
+            if (first_touch) *p = wb[l]; else *p += wb[l];
+          }
         }
       } else {
 #pragma unroll
@@ -348,19 +370,16 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
       if (++slot == NST) slot = 0;
     }
     // Gamma-bar += K . M-bar(block)
+    {
+      float Gb[DENV];
 #pragma unroll
-    for (int k = 0; k < AB; ++k) {
+      for (int b = 0; b < DENV; ++b) Gb[b] = Gbs[b * 32 + lane];
+#define X(k, a_, b_, c_) \
+  if ((a_) >= ab && (a_) < ab + AB) Gb[b_] = fmaf(a.kv[k], TP2_REF(Mb, CH, (a_) - ab, c_), Gb[b_]);
+      TP2_EXPAND(P, X)
+#undef X
 #pragma unroll
-      for (int j = 0; j < CH; ++j) reinterpret_cast<float2*>(scr)[j * 32 + lane] = Mb[k * CH + j];
-      if (ab + k < DIN) {
-#pragma unroll 1
-        for (int cc = 0; cc < DOUT; ++cc) {
-          const float mb = scr[((cc >> 1) * 32 + lane) * 2 + (cc & 1)];
-          const int p0 = (ab + k) * DOUT + cc;
-          for (int q = tb.ptr[p0]; q < tb.ptr[p0 + 1]; ++q)
-            Gbs[tb.b[q] * 32 + lane] = fmaf(tb.val[q], mb, Gbs[tb.b[q] * 32 + lane]);
-        }
-      }
+      for (int b = 0; b < DENV; ++b) Gbs[b * 32 + lane] = Gb[b];
     }
   }
   // pass 2 (direct loads, 2 edges in flight): omega-bar_e and the environment part of Y-bar_e
@@ -399,31 +418,33 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(TP2 a) {
 }
 
 // ---- host side ---------------------------------------------------------------------------------------------
-template <int DENV, int DIN, int DOUT, int CB, bool FIRST, int NST, int WPB>
-int launch_fwd2(allegro_model* m, const TP2& a) {
+template <int P, int CB, bool FIRST, int NST, int WPB>
+int launch_fwd2(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
+  constexpr int DENV = Pat<P>::DENV, DIN = Pat<P>::DIN;
   constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3;
   constexpr int SF = FIRST ? NLV * 32 + LDY : DIN * 32;
-  constexpr int WSL = DENV * 32 + ((CB + 1) / 2) * 64 + NST * SF;
-  size_t sm = (size_t)WPB * WSL * 4 + (size_t)tab_ints(DIN, DOUT) * 4 + (size_t)a.nnz * 8 + 16;
+  constexpr int WSL = DENV * 32 + NST * SF;
+  size_t sm = (size_t)WPB * WSL * 4 + 16;
   static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp2_fwd<DENV, DIN, DOUT, CB, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp2_fwd<P, CB, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
   int64_t warps = (int64_t)a.nc * a.ngroups;
-  k_tp2_fwd<DENV, DIN, DOUT, CB, FIRST, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
+  k_tp2_fwd<P, CB, FIRST, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
 }
 
-template <int DENV, int DIN, int DOUT, int AB, bool FIRST, bool HASVB, bool MREG, int NST, int WPB>
-int launch_bwd2(allegro_model* m, const TP2& a) {
+template <int P, int AB, bool FIRST, bool HASVB, bool MREG, int NST, int WPB>
+int launch_bwd2(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
+  constexpr int DENV = Pat<P>::DENV, DOUT = Pat<P>::DOUT;
   constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3, CH = (DOUT + 1) / 2;
   constexpr int SV = FIRST ? NLV * 32 + LDY : AB * 32;
   constexpr int SF = SV + (HASVB ? DOUT * 32 : 0) + 32;
   constexpr int MSL = MREG ? 0 : AB * CH * 64;
-  constexpr int WSL = 2 * DENV * 32 + MSL + CH * 64 + NST * SF;
-  size_t sm = (size_t)WPB * WSL * 4 + (size_t)tab_ints(DIN, DOUT) * 4 + (size_t)a.nnz * 8 + 16;
+  constexpr int WSL = 2 * DENV * 32 + MSL + NST * SF;
+  size_t sm = (size_t)WPB * WSL * 4 + 16;
   // Y-bar is initialised by the first backward kernel of the step, which is the one without a V-bar input
-  auto kern = k_tp2_bwd<DENV, DIN, DOUT, AB, FIRST, HASVB, MREG, !HASVB, NST, WPB>;
+  auto kern = k_tp2_bwd<P, AB, FIRST, HASVB, MREG, !HASVB, NST, WPB>;
   static bool set = false;
   if (!set) { AL_CUDA(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
   int64_t warps = (int64_t)a.nc * a.ngroups;
@@ -433,10 +454,23 @@ int launch_bwd2(allegro_model* m, const TP2& a) {
   return ALLEGRO_OK;
 }
 
-inline void fill2(allegro_model* m, Work& w, int L, int nc, TP2& a, const float* om, int ldo, const float* Vin, const float* w0, int ldw) {
-  const TPLayerDev& t = m->tp[L - 1];
-  a.rowa = (const int64_t*)w.rowa.p; a.nc = nc; a.om = om; a.ldo = ldo; a.Y = (const float*)w.Y.p; a.ldy = m->ldY;
-  a.Vin = Vin; a.w0 = w0; a.ldw = ldw; a.dp_ptr = t.dp_ptr; a.dp_b = t.dp_b; a.dp_val = t.dp_val; a.nnz = t.nnz;
-  a.n = m->n; a.ngroups = m->n / 32; a.c_env = m->c_env;
-}
+// common arguments of one layer; the values of K are copied into the parameter block
+struct TP2Common {
+  Work* w; int L, nc; const float* om; int ldo; const float* Vin; const float* w0; int ldw;
+  float* Tout; float* xs; int ldx;
+  const float* VbarL; const float* sbar; int lds; float* Vbar_prev; float* ombar; int ldob; float* w0bar;
+};
 
+template <int NNZ>
+int fill2(allegro_model* m, const TP2Common& q, TP2<NNZ>& a) {
+  const TPLayerHost& h = m->tp_host[q.L - 1];
+  if ((int)h.dp_val.size() != NNZ) { al_set_error(m, "tp2: pattern size mismatch"); return ALLEGRO_ERR_BAD_ARG; }
+  Work& w = *q.w;
+  a.rowa = (const int64_t*)w.rowa.p; a.nc = q.nc; a.om = q.om; a.ldo = q.ldo; a.Y = (const float*)w.Y.p; a.ldy = m->ldY;
+  a.Vin = q.Vin; a.w0 = q.w0; a.ldw = q.ldw; a.n = m->n; a.ngroups = m->n / 32; a.c_env = m->c_env;
+  a.Tout = q.Tout; a.xs = q.xs; a.ldx = q.ldx; a.gamma_out = (float*)w.gamma.p;
+  a.VbarL = q.VbarL; a.sbar = q.sbar; a.lds = q.lds; a.Vbar_prev = q.Vbar_prev; a.ombar = q.ombar; a.ldob = q.ldob;
+  a.w0bar = q.w0bar; a.Ybar = (float*)w.Ybar.p; a.ybar_gstride = (int64_t)w.cap_edges * m->Denv;
+  memcpy(a.kv, h.dp_val.data(), sizeof(float) * NNZ);
+  return ALLEGRO_OK;
+}

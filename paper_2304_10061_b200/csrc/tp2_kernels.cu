@@ -3,64 +3,109 @@
 // translation units: they dominate the compile time).
 #include "tp2_impl.cuh"
 
-int tp2_l3_fwd(allegro_model* m, const TP2& a, int Din, int Dout, bool first);
-int tp2_l3_bwd(allegro_model* m, const TP2& a, int Din, int Dout, bool first, bool hasvb);
+int tp2_l3_fwd(allegro_model* m, const TP2Common& q, int pat);
+int tp2_l3_bwd(allegro_model* m, const TP2Common& q, int pat);
 
-static bool shape_ok(int de, int di, int dout, bool first, bool last) {
-  if (de == 4 || de == 9) return di == de && ((dout == de && !last) || (dout == 1 && last));
-  if (de == 16)
-    return (first && di == 16 && dout == 31 && !last) || (!first && di == 31 && dout == 16 && !last) ||
-           (!first && di == 16 && dout == 1 && last);
-  return false;
+namespace {
+
+struct Ent { short a, b, c; };
+#define XH(k, a, b, c) {a, b, c},
+const Ent pat_9_9_9[] = {TP2_PAT_9_9_9(XH)};
+const Ent pat_9_9_1[] = {TP2_PAT_9_9_1(XH)};
+const Ent pat_4_4_4[] = {TP2_PAT_4_4_4(XH)};
+const Ent pat_4_4_1[] = {TP2_PAT_4_4_1(XH)};
+const Ent pat_16_16_31[] = {TP2_PAT_16_16_31(XH)};
+const Ent pat_16_31_16[] = {TP2_PAT_16_31_16(XH)};
+const Ent pat_16_16_1[] = {TP2_PAT_16_16_1(XH)};
+#undef XH
+struct PatDesc { const Ent* e; int nnz, denv, din, dout; };
+const PatDesc pats[P_COUNT] = {
+    {pat_9_9_9, TP2_NNZ_9_9_9, 9, 9, 9},        {pat_9_9_1, TP2_NNZ_9_9_1, 9, 9, 1},
+    {pat_4_4_4, TP2_NNZ_4_4_4, 4, 4, 4},        {pat_4_4_1, TP2_NNZ_4_4_1, 4, 4, 1},
+    {pat_16_16_31, TP2_NNZ_16_16_31, 16, 16, 31}, {pat_16_31_16, TP2_NNZ_16_31_16, 16, 31, 16},
+    {pat_16_16_1, TP2_NNZ_16_16_1, 16, 16, 1}};
+
+// index of the generated pattern equal to this layer's dense pair table, or -1
+int match_pattern(const TPLayerHost& h) {
+  for (int p = 0; p < P_COUNT; ++p) {
+    const PatDesc& d = pats[p];
+    if (d.denv != h.Denv || d.din != h.Din || d.dout != h.Dout || d.nnz != h.nnz || (int)h.dp_b.size() != d.nnz) continue;
+    bool ok = true;
+    int k = 0;
+    for (int a = 0; a < h.Din && ok; ++a)
+      for (int c = 0; c < h.Dout && ok; ++c)
+        for (int q = h.dp_ptr[a * h.Dout + c]; q < h.dp_ptr[a * h.Dout + c + 1]; ++q, ++k)
+          if (d.e[k].a != a || d.e[k].b != h.dp_b[q] || d.e[k].c != c) { ok = false; break; }
+    if (ok && k == d.nnz) return p;
+  }
+  return -1;
 }
 
+}  // namespace
+
 // The kernels apply when every lane of a warp owns a channel, V^0 has the environment layout and every
-// layer has one of the instantiated shapes; otherwise tp_kernels.cu / the generic kernels run.
+// layer's sparsity pattern is one of the generated ones with the expected role (first / middle / last
+// layer); otherwise tp_kernels.cu / the generic kernels run.
 bool tp2_eligible(const allegro_model* m) {
   static const bool off = getenv("B200_ALLEGRO_TP_OLD") != nullptr;
   if (off || m->n % 32 != 0 || (int)m->v0_l.size() != m->Denv) return false;
   for (int k = 0; k < m->Denv; ++k)
     if (m->v0_y[k] != k || m->v0_l[k] != l_of(k)) return false;
-  for (int L = 1; L <= m->NL; ++L)
-    if (!shape_ok(m->Denv, m->tp[L - 1].Din, m->tp[L - 1].Dout, L == 1, L == m->NL)) return false;
+  for (int L = 1; L <= m->NL; ++L) {
+    int p = match_pattern(m->tp_host[L - 1]);
+    const bool first = (L == 1), last = (L == m->NL);
+    bool ok = false;
+    switch (p) {
+      case P_9_9_9: case P_4_4_4: ok = !last; break;
+      case P_9_9_1: case P_4_4_1: ok = last; break;
+      case P_16_16_31: ok = first && !last; break;
+      case P_16_31_16: ok = !first && !last; break;
+      case P_16_16_1: ok = !first && last; break;
+      default: ok = false;
+    }
+    if (!ok) return false;
+  }
   return true;
 }
+
+#define FILL(P)                                \
+  TP2<Pat<P>::NNZ> a{};                        \
+  { int rc = fill2(m, q, a); if (rc) return rc; }
 
 int tp2_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
             float* Tout, float* xs, int ldx) {
   if (!tp2_eligible(m)) return ALLEGRO_ERR_UNIMPLEMENTED;
-  TP2 a{};
-  fill2(m, w, L, nc, a, om, ldo, Vin, w0, ldw);
-  a.Tout = Tout; a.xs = xs; a.ldx = ldx; a.gamma_out = (float*)w.gamma.p;
-  const int DENV = m->Denv, Din = m->tp[L - 1].Din, Dout = m->tp[L - 1].Dout;
+  TP2Common q{};
+  q.w = &w; q.L = L; q.nc = nc; q.om = om; q.ldo = ldo; q.Vin = Vin; q.w0 = w0; q.ldw = ldw; q.Tout = Tout; q.xs = xs; q.ldx = ldx;
+  const int p = match_pattern(m->tp_host[L - 1]);
   const bool first = (Vin == nullptr);
-  if (DENV == 16) return tp2_l3_fwd(m, a, Din, Dout, first);
-  if (DENV == 9 && Dout == 9) return first ? launch_fwd2<9, 9, 9, 9, true, 4, 4>(m, a) : launch_fwd2<9, 9, 9, 9, false, 4, 4>(m, a);
-  if (DENV == 9 && Dout == 1) return first ? launch_fwd2<9, 9, 1, 1, true, 4, 4>(m, a) : launch_fwd2<9, 9, 1, 1, false, 4, 4>(m, a);
-  if (DENV == 4 && Dout == 4) return first ? launch_fwd2<4, 4, 4, 4, true, 4, 4>(m, a) : launch_fwd2<4, 4, 4, 4, false, 4, 4>(m, a);
-  if (DENV == 4 && Dout == 1) return first ? launch_fwd2<4, 4, 1, 1, true, 4, 4>(m, a) : launch_fwd2<4, 4, 1, 1, false, 4, 4>(m, a);
+  if (p == P_16_16_31 || p == P_16_31_16 || p == P_16_16_1) return tp2_l3_fwd(m, q, p);
+  if (p == P_9_9_9) { FILL(P_9_9_9) return first ? launch_fwd2<P_9_9_9, 9, true, 4, 4>(m, a) : launch_fwd2<P_9_9_9, 9, false, 4, 4>(m, a); }
+  if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_fwd2<P_9_9_1, 1, true, 4, 4>(m, a) : launch_fwd2<P_9_9_1, 1, false, 4, 4>(m, a); }
+  if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_fwd2<P_4_4_4, 4, true, 4, 4>(m, a) : launch_fwd2<P_4_4_4, 4, false, 4, 4>(m, a); }
+  if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_fwd2<P_4_4_1, 1, true, 4, 4>(m, a) : launch_fwd2<P_4_4_1, 1, false, 4, 4>(m, a); }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }
 
 int tp2_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
             const float* VbarL, const float* sbar, int lds, float* Vbar_prev, float* ombar, int ldob, float* w0bar) {
   if (!tp2_eligible(m)) return ALLEGRO_ERR_UNIMPLEMENTED;
-  TP2 a{};
-  fill2(m, w, L, nc, a, om, ldo, Vin, w0, ldw);
-  a.VbarL = VbarL; a.sbar = sbar; a.lds = lds; a.Vbar_prev = Vbar_prev; a.ombar = ombar; a.ldob = ldob; a.w0bar = w0bar;
-  a.Ybar = (float*)w.Ybar.p; a.ybar_gstride = (int64_t)w.cap_edges * m->Denv;
-  const int DENV = m->Denv, Din = m->tp[L - 1].Din, Dout = m->tp[L - 1].Dout;
+  TP2Common q{};
+  q.w = &w; q.L = L; q.nc = nc; q.om = om; q.ldo = ldo; q.Vin = Vin; q.w0 = w0; q.ldw = ldw;
+  q.VbarL = VbarL; q.sbar = sbar; q.lds = lds; q.Vbar_prev = Vbar_prev; q.ombar = ombar; q.ldob = ldob; q.w0bar = w0bar;
+  const int p = match_pattern(m->tp_host[L - 1]);
   const bool first = (Vin == nullptr), hasvb = (VbarL != nullptr);
   // Y-bar is initialised by the kernel without a V-bar input, which must be the first of the step (L = NL)
   if (hasvb != (L < m->NL)) { al_set_error(m, "tp2_bwd: unexpected V-bar input"); return ALLEGRO_ERR_BAD_ARG; }
-  if (DENV == 16) return tp2_l3_bwd(m, a, Din, Dout, first, hasvb);
-  static const bool mreg = getenv("B200_ALLEGRO_TP_MSMEM") == nullptr;
-  if (DENV == 9 && Dout == 9) {
-    if (mreg) return first ? launch_bwd2<9, 9, 9, 9, true, true, true, 3, 4>(m, a) : launch_bwd2<9, 9, 9, 9, false, true, true, 3, 4>(m, a);
-    return first ? launch_bwd2<9, 9, 9, 9, true, true, false, 3, 4>(m, a) : launch_bwd2<9, 9, 9, 9, false, true, false, 3, 4>(m, a);
+  if (p == P_16_16_31 || p == P_16_31_16 || p == P_16_16_1) return tp2_l3_bwd(m, q, p);
+  static const bool mreg = getenv("B200_ALLEGRO_TP_MREG") != nullptr;   // default: M block in shared memory (168 vs 251 registers; measured faster)
+  if (p == P_9_9_9) {
+    FILL(P_9_9_9)
+    if (mreg) return first ? launch_bwd2<P_9_9_9, 9, true, true, true, 3, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, true, 3, 4>(m, a);
+    return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 3, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 3, 4>(m, a);
   }
-  if (DENV == 9 && Dout == 1) return first ? launch_bwd2<9, 9, 1, 9, true, false, true, 3, 4>(m, a) : launch_bwd2<9, 9, 1, 9, false, false, true, 3, 4>(m, a);
-  if (DENV == 4 && Dout == 4) return first ? launch_bwd2<4, 4, 4, 4, true, true, true, 3, 4>(m, a) : launch_bwd2<4, 4, 4, 4, false, true, true, 3, 4>(m, a);
-  if (DENV == 4 && Dout == 1) return first ? launch_bwd2<4, 4, 1, 4, true, false, true, 3, 4>(m, a) : launch_bwd2<4, 4, 1, 4, false, false, true, 3, 4>(m, a);
+  if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_bwd2<P_9_9_1, 9, true, false, true, 3, 4>(m, a) : launch_bwd2<P_9_9_1, 9, false, false, true, 3, 4>(m, a); }
+  if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_bwd2<P_4_4_4, 4, true, true, true, 3, 4>(m, a) : launch_bwd2<P_4_4_4, 4, false, true, true, 3, 4>(m, a); }
+  if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_bwd2<P_4_4_1, 4, true, false, true, 3, 4>(m, a) : launch_bwd2<P_4_4_1, 4, false, false, true, 3, 4>(m, a); }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }

@@ -1,9 +1,9 @@
 // l_max = 3 backward instantiations of the second-generation tensor-track kernels (tp2_impl.cuh).
 #include "tp2_impl.cuh"
 
-int tp2_l3_bwd(allegro_model* m, const TP2& a, int Din, int Dout, bool first, bool hasvb) {
-  if (first && hasvb && Din == 16 && Dout == 31) return launch_bwd2<16, 16, 31, 4, true, true, false, 2, 2>(m, a);
-  if (!first && hasvb && Din == 31 && Dout == 16) return launch_bwd2<16, 31, 16, 8, false, true, false, 2, 2>(m, a);
-  if (!first && !hasvb && Din == 16 && Dout == 1) return launch_bwd2<16, 16, 1, 16, false, false, true, 2, 4>(m, a);
+int tp2_l3_bwd(allegro_model* m, const TP2Common& q, int pat) {
+  if (pat == P_16_16_31) { TP2<Pat<P_16_16_31>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd2<P_16_16_31, 4, true, true, false, 2, 2>(m, a); }
+  if (pat == P_16_31_16) { TP2<Pat<P_16_31_16>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd2<P_16_31_16, 8, false, true, false, 2, 2>(m, a); }
+  if (pat == P_16_16_1) { TP2<Pat<P_16_16_1>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd2<P_16_16_1, 16, false, false, true, 2, 4>(m, a); }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }
