@@ -43,7 +43,7 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     AL_CHECK(R(w.ZB0, (size_t)M * maxw)); AL_CHECK(R(w.ZB1, (size_t)M * maxw));
     AL_CHECK(R(w.G, (size_t)M * (d + n))); AL_CHECK(R(w.OB, (size_t)M * 2 * nA));
     AL_CHECK(R(w.VB0, (size_t)M * Dmax * n)); AL_CHECK(R(w.VB1, (size_t)M * Dmax * n));
-    AL_CHECK(R(w.ubar, M)); AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * ((n + 31) / 32))); AL_CHECK(R(w.ge, (size_t)3 * M));
+    AL_CHECK(R(w.ubar, M)); AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * ((n + 31) / 32) * (NL + 1))); AL_CHECK(R(w.ge, (size_t)3 * M));
     w.cap_edges = M;
   }
   if (Nc > w.cap_centers) {
@@ -145,9 +145,11 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   AL_CHECK(k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom));
   // ---- step 11: backward -----------------------------------------------------------------------------------
   AL_CUDA(m, cudaMemsetAsync(w.ubar.p, 0, (size_t)m_cap * 4, st));
-  if (!tp2_eligible(m))                        // (the tp2 kernels write Y-bar before accumulating into it)
-  for (int gq = 0; gq < (n + 31) / 32; ++gq)   // one partial Y-bar per 32-channel group (summed in fixed order in k_edge_bwd)
-    AL_CUDA(m, cudaMemsetAsync((float*)w.Ybar.p + (size_t)gq * w.cap_edges * m->Denv, 0, (size_t)m_cap * m->Denv * 4, st));
+  // Y-bar partials [group][slot 0..NL][M][Denv], summed in fixed order by k_edge_bwd.  The tp2 kernels store every
+  // partial; the fallback kernels accumulate into slot 0 of each group, so all partials are zeroed for them.
+  if (!tp2_eligible(m))
+    for (int gq = 0; gq < ((n + 31) / 32) * (NL + 1); ++gq)
+      AL_CUDA(m, cudaMemsetAsync((float*)w.Ybar.p + (size_t)gq * w.cap_edges * m->Denv, 0, (size_t)m_cap * m->Denv * 4, st));
   float* xb = (float*)w.XB0.p; float* xb_o = (float*)w.XB1.p;
   float* vb = nullptr; float* vb_a = (float*)w.VB0.p; float* vb_b = (float*)w.VB1.p;
   bool rank1 = true;   // x-bar^{NL} = sigma_e * w_eff is never materialised

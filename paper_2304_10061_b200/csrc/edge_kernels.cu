@@ -413,7 +413,7 @@ __global__ void k_bwd_prep(const int* __restrict__ m_ptr, const float* __restric
 __global__ void k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz, const float* __restrict__ W,
                            int S, int NB, int H, const float4* __restrict__ geo, const float* __restrict__ du,
                            const float* __restrict__ dB, const float* __restrict__ ubar, const float* __restrict__ Ybar,
-                           int ngroups, int64_t ybar_gstride, int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
+                           int nparts, int64_t ybar_pstride, int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
                            float* __restrict__ ge, double* __restrict__ force) {
   const int M = *m_ptr;
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -432,7 +432,7 @@ __global__ void k_edge_bwd(const int* __restrict__ m_ptr, const float* __restric
     float yb[16];
     for (int q = 0; q < Denv; ++q) {
       float acc = 0.f;
-      for (int gq = 0; gq < ngroups; ++gq) acc += Ybar[gq * ybar_gstride + e * Denv + q];   // fixed order: deterministic
+      for (int gq = 0; gq < nparts; ++gq) acc += Ybar[gq * ybar_pstride + e * Denv + q];   // fixed order: deterministic
       yb[q] = acc;
     }
     float vx, vy, vz;
@@ -630,7 +630,7 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
   (void)single;
   k_edge_bwd<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>(
       (int*)w.m_act.p, zb1, ldz, L0.W, m->S, m->NB, L0.fo, (float4*)w.geo.p, (float*)w.du.p, (float*)w.dB.p,
-      (float*)w.ubar.p, (float*)w.Ybar.p, (m->n + 31) / 32, (int64_t)w.cap_edges * m->Denv, m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
+      (float*)w.ubar.p, (float*)w.Ybar.p, ((m->n + 31) / 32) * (m->NL + 1), (int64_t)w.cap_edges * m->Denv, m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }

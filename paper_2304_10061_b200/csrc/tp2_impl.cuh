@@ -14,7 +14,8 @@
 //     literal register indices; the values (which carry the path weights) come from the kernel parameters
 //     (constant bank);
 //   * wide features (l_max = 3) walk blocks of output components (forward) / input components (backward);
-//   * Y-bar is written, not accumulated, by the first kernel of a step that touches it (no memset).
+//   * every Y-bar contribution (per channel group: V^0 part, environment part of each layer) is a plain
+//     store into its own partial buffer; k_edge_bwd sums the partials in fixed order (no memset, no RMW).
 // Requirements (checked on the host, otherwise the kernels of tp_kernels.cu run): n % 32 == 0, V^0 layout
 // equal to the environment layout, and every layer's pattern equal to a generated one.
 #pragma once
@@ -55,7 +56,8 @@ struct TP2 {
   int n, ngroups; float c_env;
   float* Tout; float* xs; int ldx; float* gamma_out;
   const float* VbarL; const float* sbar; int lds;
-  float* Vbar_prev; float* ombar; int ldob; float* w0bar; float* Ybar; int64_t ybar_gstride;
+  float* Vbar_prev; float* ombar; int ldob; float* w0bar;
+  float* Ybar; int64_t ybar_pstride; int ybar_slots, ybar_slot;   // Y-bar partials [group][slot][M][DENV], plain stores
   float kv[NNZ];   // values of the fused tensor K in pattern order (dense pair table order)
 };
 
@@ -205,7 +207,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(const __grid_consta
 //   FIRST (V^0 = w^0 (x) Y):  w0-bar_e[l] = sum_{a in l} V-bar^0_e[a] Y_e[a] ;  Y-bar_e[a] += sum_n w0_e[l(a)] V-bar^0_e[a]
 // a-blocks of AB input components; M block in registers (MREG) or in the warp's shared slice.
 // ======================================================================================================
-template <int P, int AB, bool FIRST, bool HASVB, bool MREG, bool YINIT, int NST, int WPB>
+template <int P, int AB, bool FIRST, bool HASVB, bool MREG, int NST, int WPB>
 static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_constant__ TP2<Pat<P>::NNZ> a) {
   constexpr int DENV = Pat<P>::DENV, DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
   constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3, CH = (DOUT + 1) / 2;
@@ -227,7 +229,9 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
   const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
   const int deg = (int)(e1 - e0);
   if (deg <= 0) return;
-  float* Yb = a.Ybar + (size_t)grp * a.ybar_gstride;
+  // slot 0 of the group: V^0 part (FIRST); slot L: environment part of layer L
+  float* Yb0 = a.Ybar + (size_t)grp * a.ybar_slots * a.ybar_pstride;
+  float* YbL = Yb0 + (size_t)a.ybar_slot * a.ybar_pstride;
 
   auto issue = [&](int64_t e, float* st, int ab) {
     if (FIRST) {
@@ -351,7 +355,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
       }
       if (FIRST) {
         const int nvalid = (DIN - ab < AB) ? DIN - ab : AB;
-        tp_ybar_rows<AB, YINIT>(Yb + e * DENV, pp, ab, nvalid, lane);
+        tp_ybar_rows<AB, true>(Yb0 + e * DENV, pp, ab, nvalid, lane);
 #pragma unroll
         for (int l = 0; l < NLV; ++l) {
           // (a block only touches the l values of its own components; the first toucher stores)
@@ -411,7 +415,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
           }
           a.ombar[(e + i) * a.ldob + l * a.n + nn] = ob;
         }
-        tp_ybar_rows<DENV, (YINIT && !FIRST)>(Yb + (e + i) * DENV, pp, 0, DENV, lane);
+        tp_ybar_rows<DENV, true>(YbL + (e + i) * DENV, pp, 0, DENV, lane);
       }
     }
   }
@@ -443,8 +447,7 @@ int launch_bwd2(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int MSL = MREG ? 0 : AB * CH * 64;
   constexpr int WSL = 2 * DENV * 32 + MSL + NST * SF;
   size_t sm = (size_t)WPB * WSL * 4 + 16;
-  // Y-bar is initialised by the first backward kernel of the step, which is the one without a V-bar input
-  auto kern = k_tp2_bwd<P, AB, FIRST, HASVB, MREG, !HASVB, NST, WPB>;
+  auto kern = k_tp2_bwd<P, AB, FIRST, HASVB, MREG, NST, WPB>;
   static bool set = false;
   if (!set) { AL_CUDA(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
   int64_t warps = (int64_t)a.nc * a.ngroups;
@@ -470,7 +473,8 @@ int fill2(allegro_model* m, const TP2Common& q, TP2<NNZ>& a) {
   a.Vin = q.Vin; a.w0 = q.w0; a.ldw = q.ldw; a.n = m->n; a.ngroups = m->n / 32; a.c_env = m->c_env;
   a.Tout = q.Tout; a.xs = q.xs; a.ldx = q.ldx; a.gamma_out = (float*)w.gamma.p;
   a.VbarL = q.VbarL; a.sbar = q.sbar; a.lds = q.lds; a.Vbar_prev = q.Vbar_prev; a.ombar = q.ombar; a.ldob = q.ldob;
-  a.w0bar = q.w0bar; a.Ybar = (float*)w.Ybar.p; a.ybar_gstride = (int64_t)w.cap_edges * m->Denv;
+  a.w0bar = q.w0bar; a.Ybar = (float*)w.Ybar.p; a.ybar_pstride = (int64_t)w.cap_edges * m->Denv;
+  a.ybar_slots = m->NL + 1; a.ybar_slot = q.L;
   memcpy(a.kv, h.dp_val.data(), sizeof(float) * NNZ);
   return ALLEGRO_OK;
 }

@@ -80,10 +80,10 @@ int tp2_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   const int p = match_pattern(m->tp_host[L - 1]);
   const bool first = (Vin == nullptr);
   if (p == P_16_16_31 || p == P_16_31_16 || p == P_16_16_1) return tp2_l3_fwd(m, q, p);
-  if (p == P_9_9_9) { FILL(P_9_9_9) return first ? launch_fwd2<P_9_9_9, 9, true, 4, 4>(m, a) : launch_fwd2<P_9_9_9, 9, false, 4, 4>(m, a); }
-  if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_fwd2<P_9_9_1, 1, true, 4, 4>(m, a) : launch_fwd2<P_9_9_1, 1, false, 4, 4>(m, a); }
-  if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_fwd2<P_4_4_4, 4, true, 4, 4>(m, a) : launch_fwd2<P_4_4_4, 4, false, 4, 4>(m, a); }
-  if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_fwd2<P_4_4_1, 1, true, 4, 4>(m, a) : launch_fwd2<P_4_4_1, 1, false, 4, 4>(m, a); }
+  if (p == P_9_9_9) { FILL(P_9_9_9) return first ? launch_fwd2<P_9_9_9, 9, true, 8, 4>(m, a) : launch_fwd2<P_9_9_9, 9, false, 4, 4>(m, a); }
+  if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_fwd2<P_9_9_1, 1, true, 8, 4>(m, a) : launch_fwd2<P_9_9_1, 1, false, 4, 4>(m, a); }
+  if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_fwd2<P_4_4_4, 4, true, 8, 4>(m, a) : launch_fwd2<P_4_4_4, 4, false, 4, 4>(m, a); }
+  if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_fwd2<P_4_4_1, 1, true, 8, 4>(m, a) : launch_fwd2<P_4_4_1, 1, false, 4, 4>(m, a); }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }
 
@@ -95,17 +95,16 @@ int tp2_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   q.VbarL = VbarL; q.sbar = sbar; q.lds = lds; q.Vbar_prev = Vbar_prev; q.ombar = ombar; q.ldob = ldob; q.w0bar = w0bar;
   const int p = match_pattern(m->tp_host[L - 1]);
   const bool first = (Vin == nullptr), hasvb = (VbarL != nullptr);
-  // Y-bar is initialised by the kernel without a V-bar input, which must be the first of the step (L = NL)
   if (hasvb != (L < m->NL)) { al_set_error(m, "tp2_bwd: unexpected V-bar input"); return ALLEGRO_ERR_BAD_ARG; }
   if (p == P_16_16_31 || p == P_16_31_16 || p == P_16_16_1) return tp2_l3_bwd(m, q, p);
   static const bool mreg = getenv("B200_ALLEGRO_TP_MREG") != nullptr;   // default: M block in shared memory (168 vs 251 registers; measured faster)
   if (p == P_9_9_9) {
     FILL(P_9_9_9)
-    if (mreg) return first ? launch_bwd2<P_9_9_9, 9, true, true, true, 3, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, true, 3, 4>(m, a);
-    return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 3, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 3, 4>(m, a);
+    if (mreg) return first ? launch_bwd2<P_9_9_9, 9, true, true, true, 4, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, true, 4, 4>(m, a);
+    return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 4, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 4, 4>(m, a);
   }
-  if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_bwd2<P_9_9_1, 9, true, false, true, 3, 4>(m, a) : launch_bwd2<P_9_9_1, 9, false, false, true, 3, 4>(m, a); }
-  if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_bwd2<P_4_4_4, 4, true, true, true, 3, 4>(m, a) : launch_bwd2<P_4_4_4, 4, false, true, true, 3, 4>(m, a); }
-  if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_bwd2<P_4_4_1, 4, true, false, true, 3, 4>(m, a) : launch_bwd2<P_4_4_1, 4, false, false, true, 3, 4>(m, a); }
+  if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_bwd2<P_9_9_1, 9, true, false, true, 4, 4>(m, a) : launch_bwd2<P_9_9_1, 9, false, false, true, 4, 4>(m, a); }
+  if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_bwd2<P_4_4_4, 4, true, true, true, 4, 4>(m, a) : launch_bwd2<P_4_4_4, 4, false, true, true, 4, 4>(m, a); }
+  if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_bwd2<P_4_4_1, 4, true, false, true, 4, 4>(m, a) : launch_bwd2<P_4_4_1, 4, false, false, true, 4, 4>(m, a); }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }
