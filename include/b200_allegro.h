@@ -147,6 +147,10 @@ int allegro_launch_count(const allegro_model* m, int64_t* launches);
 /* Total number of active (r < r_cut) edges, over all chunks, of the last allegro_compute (synchronises the stream). */
 int allegro_last_active_edges(allegro_model* m, int64_t* n_active);
 
+/* Debug mode (tests only; default off): keep every intermediate tensor that allegro_debug_tensor can name.
+ * Without it the final latent x^{NL} is consumed inside the epilogue of the last latent GEMM and never stored. */
+int allegro_set_debug(allegro_model* m, int on);
+
 /* Debug/parity taps (tests only): copy an intermediate tensor of the LAST chunk of the last
  * allegro_compute to host as fp32.  name: "Y", "u", "x0", "x1".., "V1".., "gamma1".., "ebar".
  * n_floats: in = capacity of out, out = floats written. */

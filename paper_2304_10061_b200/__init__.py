@@ -72,7 +72,7 @@ EXPORTS = [
     "allegro_set_allocator", "allegro_set_chunk_edges", "allegro_neighbors", "allegro_neighbors_host",
     "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
-    "allegro_launch_count", "allegro_last_active_edges", "allegro_debug_tensor",
+    "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_debug_tensor",
     "allegro_last_error",
 ]
 
@@ -97,6 +97,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_set_stream.argtypes = [vp, vp]
     lib.allegro_set_allocator.argtypes = [vp, _ALLOC_FN, _FREE_FN, vp]
     lib.allegro_set_chunk_edges.argtypes = [vp, i64]
+    lib.allegro_set_debug.argtypes = [vp, C.c_int]
     lib.allegro_neighbors.argtypes = [vp, vp, i64, P(C.c_double), C.c_double, P(vp)]
     lib.allegro_neighbors_host.argtypes = [vp, vp, i64, P(C.c_double), C.c_double, P(vp)]
     lib.allegro_nbr_info.argtypes = [vp, P(i64), P(i64), P(vp), P(vp), P(vp)]
@@ -327,6 +328,10 @@ class Allegro:
         ms, n = C.c_double(0), C.c_int64(0)
         self._check(self._lib.allegro_profile_read(self._h, name.encode(), C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def set_debug(self, on: bool = True):
+        """Keep every tensor debug_tensor() can name (tests only)."""
+        self._check(self._lib.allegro_set_debug(self._h, 1 if on else 0))
 
     def debug_tensor(self, name: str, max_floats: int = 1 << 26):
         import numpy as np

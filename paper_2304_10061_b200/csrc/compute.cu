@@ -43,7 +43,10 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     AL_CHECK(R(w.ZB0, (size_t)M * maxw)); AL_CHECK(R(w.ZB1, (size_t)M * maxw));
     AL_CHECK(R(w.G, (size_t)M * (d + n))); AL_CHECK(R(w.OB, (size_t)M * 2 * nA));
     AL_CHECK(R(w.VB0, (size_t)M * Dmax * n)); AL_CHECK(R(w.VB1, (size_t)M * Dmax * n));
-    AL_CHECK(R(w.ubar, M)); AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * ((n + 31) / 32) * (NL + 1))); AL_CHECK(R(w.ge, (size_t)3 * M));
+    w.n_eparts = (d % 32 == 0) ? al_gemm_row_parts(m, d) : 0;   // > 0: last latent layer fused with energy / z-bar (EPI_LATENT_LAST)
+    w.n_uparts = w.n_eparts + 1;
+    AL_CHECK(R(w.ubar, (size_t)M * w.n_uparts)); AL_CHECK(R(w.epart, (size_t)2 * M * std::max(w.n_eparts, 1)));
+    AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * ((n + 31) / 32) * (NL + 1))); AL_CHECK(R(w.ge, (size_t)3 * M));
     w.cap_edges = M;
   }
   if (Nc > w.cap_centers) {
@@ -65,7 +68,7 @@ void al_work_free(allegro_model* m) {
   Work& w = *m->work;
   std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.sig, &w.B, &w.dB, &w.Y,
                               &w.XF, &w.WE, &w.gamma, &w.XB0, &w.XB1, &w.ZB0, &w.ZB1, &w.G, &w.OB, &w.VB0, &w.VB1,
-                              &w.ubar, &w.Ybar, &w.ge, &w.eatom};
+                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom};
   for (auto* b : all) al_release(m, *b);
   for (auto* v : {&w.tb_z, &w.tb_a, &w.XS, &w.OM, &w.T}) for (auto& b : *v) al_release(m, b);
   for (auto* vv : {&w.lat_z, &w.lat_a}) for (auto& v : *vv) for (auto& b : v) al_release(m, b);
@@ -97,6 +100,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   }
   const int* mp = (const int*)w.m_act.p;
   cudaStream_t st = m->stream;
+  const bool fused_last = w.n_eparts > 0;
   EdgeGeomArgs ga{};
   ga.pos = pos; ga.species = species; memcpy(ga.box, box, 24); ga.rc = hp.r_cut; ga.p = hp.poly_p; ga.NB = m->NB;
   ga.lmax = m->lmax; ga.row_ptr = (const int64_t*)nb->row_ptr.p; ga.j = (const int32_t*)nb->j.p;
@@ -136,6 +140,14 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       GemmArgs g = mk(A, lda, m->latent[L - 1][k], false, C, ldc, m_cap, mp, last ? EPI_LATENT : EPI_SILU_BOTH);
       g.out2 = (float*)w.lat_z[L - 1][k].p; g.ldo2 = hp.latent_dims[k];
       g.u = (float*)w.u.p; g.aux1 = (float*)w.XS[L - 1].p; g.ld1 = d + n; g.c0 = m->c_old[L - 1]; g.c1 = m->c_new[L - 1];
+      if (last && L == NL && fused_last) {
+        // x^{NL} is consumed in the epilogue: edge-energy partials, z-bar^{NL} (in place of z) and u-bar partials
+        g.epi = EPI_LATENT_LAST;
+        if (!m->debug_keep) g.C = nullptr;
+        g.out2 = (float*)w.ZB0.p; g.ldo2 = d;
+        g.sig = (float*)w.sig.p; g.aux3 = m->w_eff_f; g.w_eff_d = m->w_eff_d;
+        g.epart = (double*)w.epart.p; g.upart = (float*)w.ubar.p; g.part_stride = w.cap_edges;
+      }
       AL_CHECK(al_gemm(m, g));
     }
     if (L < NL)
@@ -144,7 +156,8 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   // ---- steps 9-10: edge energy, per-atom energy (fp64) -----------------------------------------------------
   AL_CHECK(k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom));
   // ---- step 11: backward -----------------------------------------------------------------------------------
-  AL_CUDA(m, cudaMemsetAsync(w.ubar.p, 0, (size_t)m_cap * 4, st));
+  // u-bar partials: [0, n_eparts) stored by EPI_LATENT_LAST, the last one accumulated by k_bwd_prep
+  AL_CUDA(m, cudaMemsetAsync((float*)w.ubar.p + (size_t)(w.n_uparts - 1) * w.cap_edges, 0, (size_t)m_cap * 4, st));
   // Y-bar partials [group][slot 0..NL][M][Denv], summed in fixed order by k_edge_bwd.  The tp2 kernels store every
   // partial; the fallback kernels accumulate into slot 0 of each group, so all partials are zeroed for them.
   if (!tp2_eligible(m))
@@ -155,7 +168,8 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   bool rank1 = true;   // x-bar^{NL} = sigma_e * w_eff is never materialised
   for (int L = NL; L >= 1; --L) {
     float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
-    AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
+    if (!(rank1 && fused_last))   // (fused: z-bar^{NL} was written by the forward epilogue)
+      AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
     for (int k = nlat - 1; k >= 1; --k) {
       GemmArgs g = mk(zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
       g.aux1 = (float*)w.lat_z[L - 1][k - 1].p; g.ld1 = hp.latent_dims[k - 1];

@@ -152,42 +152,49 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
 }
 
 // ---- first two-body layer: one-hot rows + Bessel matvec ----------------------------------
-constexpr int TB0_EPB = 8;
-__global__ void k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int* __restrict__ ej,
-                           const int32_t* __restrict__ species, const float* __restrict__ B, const float* __restrict__ u,
-                           const float* __restrict__ W, int S, int NB, int H, float* __restrict__ z, float* __restrict__ act,
-                           int ldact, int scale_u) {
+// z_0[e, :] = W[Z_i, :] + W[S + Z_j, :] + sum_q B_q(e) W[2S + q, :]; a thread owns 4 consecutive outputs
+// (float4 I/O, the weight rows come from L1) of one edge at a time.
+constexpr int TB0_EDGES = 64;
+__global__ void __launch_bounds__(256)
+k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int* __restrict__ ej,
+           const int32_t* __restrict__ species, const float* __restrict__ B, const float* __restrict__ u,
+           const float* __restrict__ W, int S, int NB, int H, float* __restrict__ z, float* __restrict__ act, int ldact,
+           int scale_u) {
   const int M = *m_ptr;
-  int e0 = blockIdx.x * TB0_EPB;
-  if (e0 >= M) return;
-  __shared__ float sB[TB0_EPB][16];
-  __shared__ int sZi[TB0_EPB], sZj[TB0_EPB];
-  __shared__ float sU[TB0_EPB];
-  int tid = threadIdx.x;
-  if (tid < TB0_EPB * NB) {
-    int e = e0 + tid / NB;
-    sB[tid / NB][tid % NB] = (e < M) ? B[(size_t)e * NB + tid % NB] : 0.f;
+  const int64_t e_base = (int64_t)blockIdx.x * TB0_EDGES;
+  if (e_base >= M) return;
+  __shared__ float sB[TB0_EDGES][16];
+  __shared__ int sZi[TB0_EDGES], sZj[TB0_EDGES];
+  __shared__ float sU[TB0_EDGES];
+  const int tid = threadIdx.x;
+  for (int idx = tid; idx < TB0_EDGES * NB; idx += 256) {
+    int r = idx / NB, q = idx - r * NB;
+    sB[r][q] = (e_base + r < M) ? B[(e_base + r) * NB + q] : 0.f;
   }
-  if (tid < TB0_EPB) {
-    int e = e0 + tid;
+  if (tid < TB0_EDGES) {
+    int64_t e = e_base + tid;
     sZi[tid] = (e < M) ? species[ei[e]] : 0;
     sZj[tid] = (e < M) ? species[ej[e]] : 0;
     sU[tid] = (e < M) ? u[e] : 0.f;
   }
   __syncthreads();
-  for (int k = tid; k < H; k += blockDim.x) {
-    float wb[16];
-    for (int q = 0; q < NB; ++q) wb[q] = W[(size_t)(2 * S + q) * H + k];
-#pragma unroll
-    for (int t = 0; t < TB0_EPB; ++t) {
-      int e = e0 + t;
-      if (e >= M) break;
-      float acc = W[(size_t)sZi[t] * H + k] + W[(size_t)(S + sZj[t]) * H + k];
-      for (int q = 0; q < NB; ++q) acc = fmaf(sB[t][q], wb[q], acc);
-      z[(size_t)e * H + k] = acc;
-      float s = silu_f(acc);
-      act[(size_t)e * ldact + k] = scale_u ? sU[t] * s : s;
+  const int H4 = H >> 2;
+  for (int idx = tid; idx < TB0_EDGES * H4; idx += 256) {
+    const int r = idx / H4, k4 = (idx - r * H4) * 4;
+    const int64_t e = e_base + r;
+    if (e >= M) break;
+    float4 a0 = __ldg(reinterpret_cast<const float4*>(W + (size_t)sZi[r] * H + k4));
+    float4 a1 = __ldg(reinterpret_cast<const float4*>(W + (size_t)(S + sZj[r]) * H + k4));
+    float4 acc = make_float4(a0.x + a1.x, a0.y + a1.y, a0.z + a1.z, a0.w + a1.w);
+    for (int q = 0; q < NB; ++q) {
+      float4 w4 = __ldg(reinterpret_cast<const float4*>(W + (size_t)(2 * S + q) * H + k4));
+      float b = sB[r][q];
+      acc.x = fmaf(b, w4.x, acc.x); acc.y = fmaf(b, w4.y, acc.y); acc.z = fmaf(b, w4.z, acc.z); acc.w = fmaf(b, w4.w, acc.w);
     }
+    *reinterpret_cast<float4*>(z + e * H + k4) = acc;
+    const float us = scale_u ? sU[r] : 1.0f;
+    *reinterpret_cast<float4*>(act + e * ldact + k4) =
+        make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
   }
 }
 
@@ -368,6 +375,27 @@ __global__ void k_energy(const int64_t* __restrict__ rowa, int nc, int64_t c0, c
   }
 }
 
+// E-hat_i from the edge-energy partials written by the last latent GEMM (EPI_LATENT_LAST): lanes take the
+// center's edges, each sums its partials in fixed order, then a fixed-order warp reduction in fp64.
+__global__ void k_energy_parts(const int64_t* __restrict__ rowa, int nc, int64_t c0, const double* __restrict__ epart,
+                               int nparts, int64_t pstride, const int32_t* __restrict__ species,
+                               const double* __restrict__ sigma, const double* __restrict__ mu, double* __restrict__ e_atom) {
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= nc) return;
+  int64_t e0 = rowa[warp], e1 = rowa[warp + 1];
+  double acc = 0.0;
+  for (int64_t e = e0 + lane; e < e1; e += 32) {
+    double s = 0.0;
+    for (int p = 0; p < nparts; ++p) s += epart[(int64_t)p * pstride + e];
+    acc += s;
+  }
+  acc = warp_sum_d(acc);
+  if (lane == 0) {
+    int z = species[c0 + warp];
+    e_atom[c0 + warp] = sigma[z] * acc + mu[z];
+  }
+}
+
 __global__ void k_sum_f64(const double* __restrict__ x, int64_t n, double* __restrict__ out) {
   __shared__ double sh[1024];
   double s = 0.0;
@@ -410,44 +438,89 @@ __global__ void k_bwd_prep(const int* __restrict__ m_ptr, const float* __restric
 }
 
 // Last backward stage: B-bar through the first two-body layer, r-bar, angular part, dE/dr_e, force scatter.
-__global__ void k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz, const float* __restrict__ W,
-                           int S, int NB, int H, const float4* __restrict__ geo, const float* __restrict__ du,
-                           const float* __restrict__ dB, const float* __restrict__ ubar, const float* __restrict__ Ybar,
-                           int nparts, int64_t ybar_pstride, int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
-                           float* __restrict__ ge, double* __restrict__ force) {
+// Block = 32 edges x 8 lanes.  The block stages its 32 rows of z-bar_0 [H] and the Bessel rows of the first
+// two-body weight matrix in shared memory; lane q of an edge forms B-bar_q = <z-bar_0, W[2S+q,:]> (and q+8 when
+// n_bessel > 8), the 8 lanes then share the sums over the u-bar and Y-bar partial buffers (fixed order), one
+// lane evaluates the spherical-harmonic vjp and six lanes issue the fp64 force atomics (F_i += g, F_j -= g).
+constexpr int EB_EDGES = 32;
+__global__ void __launch_bounds__(256)
+k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz, const float* __restrict__ W, int S, int NB,
+           int H, const float4* __restrict__ geo, const float* __restrict__ du, const float* __restrict__ dB,
+           const float* __restrict__ ubar, int n_uparts, int64_t ubar_pstride, const float* __restrict__ Ybar, int nparts,
+           int64_t ybar_pstride, int Denv, int lmax, const int* __restrict__ ei, const int* __restrict__ ej,
+           float* __restrict__ ge, double* __restrict__ force) {
+  extern __shared__ float4 eb_smem4[];
+  float* Ws = reinterpret_cast<float*>(eb_smem4);     // [NB][H + 4]
+  const int HP = H + 4;
+  float* zs = Ws + NB * HP;                           // [32][H + 4]
   const int M = *m_ptr;
-  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (warp >= M) return;
-  int64_t e = warp;
-  float rbar = 0.f;
-  for (int q = 0; q < NB; ++q) {
-    float acc = 0.f;
-    for (int k = lane; k < H; k += 32) acc = fmaf(zb1[e * ldz + k], W[(size_t)(2 * S + q) * H + k], acc);
-    acc = warp_sum(acc);
-    rbar = fmaf(acc, dB[e * NB + q], rbar);
+  const int64_t e_base = (int64_t)blockIdx.x * EB_EDGES;
+  if (e_base >= M) return;
+  const int tid = threadIdx.x;
+  for (int idx = tid; idx < NB * (H / 4); idx += 256) {
+    int q = idx / (H / 4), k4 = (idx - q * (H / 4)) * 4;
+    *reinterpret_cast<float4*>(Ws + q * HP + k4) = __ldg(reinterpret_cast<const float4*>(W + (size_t)(2 * S + q) * H + k4));
   }
-  if (lane == 0) {
-    rbar = fmaf(ubar[e], du[e], rbar);
-    float4 g4 = geo[e];
-    float yb[16];
-    for (int q = 0; q < Denv; ++q) {
-      float acc = 0.f;
-      for (int gq = 0; gq < nparts; ++gq) acc += Ybar[gq * ybar_pstride + e * Denv + q];   // fixed order: deterministic
-      yb[q] = acc;
+  for (int idx = tid; idx < EB_EDGES * (H / 4); idx += 256) {
+    int r = idx / (H / 4), k4 = (idx - r * (H / 4)) * 4;
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (e_base + r < M) v = *reinterpret_cast<const float4*>(zb1 + (e_base + r) * ldz + k4);
+    *reinterpret_cast<float4*>(zs + r * HP + k4) = v;
+  }
+  __syncthreads();
+  const int el = tid >> 3, q = tid & 7, lane = tid & 31;
+  const int64_t e = e_base + el;
+  const bool live = e < M;
+  const int64_t ee = live ? e : (int64_t)M - 1;
+  // B-bar_q . dB_q
+  float pr = 0.f;
+  for (int qq = q; qq < NB; qq += 8) {
+    float acc = 0.f;
+    const float* zr = zs + el * HP;
+    const float* wr = Ws + qq * HP;
+    for (int k4 = 0; k4 < H; k4 += 4) {
+      float4 z4 = *reinterpret_cast<const float4*>(zr + k4);
+      float4 w4 = *reinterpret_cast<const float4*>(wr + k4);
+      acc = fmaf(z4.x, w4.x, acc); acc = fmaf(z4.y, w4.y, acc); acc = fmaf(z4.z, w4.z, acc); acc = fmaf(z4.w, w4.w, acc);
     }
+    pr = fmaf(acc, dB[ee * NB + qq], pr);
+  }
+  // u-bar partials: lane q takes parts q, q+8, ...
+  float ub = 0.f;
+  for (int p = q; p < n_uparts; p += 8) ub += ubar[(int64_t)p * ubar_pstride + ee];
+  pr = fmaf(ub, du[ee], pr);
+  // Y-bar partials: lane q sums components q and q+8 over the parts in fixed order
+  float ys0 = 0.f, ys1 = 0.f;
+  for (int p = 0; p < nparts; ++p) {
+    const float* yp = Ybar + (int64_t)p * ybar_pstride + ee * Denv;
+    if (q < Denv) ys0 += yp[q];
+    if (q + 8 < Denv) ys1 += yp[q + 8];
+  }
+#pragma unroll
+  for (int o = 1; o < 8; o <<= 1) pr += __shfl_xor_sync(FULLMASK, pr, o);   // r-bar (all 8 lanes of the edge hold it)
+  float yb[16];
+#pragma unroll
+  for (int b = 0; b < 16; ++b) yb[b] = __shfl_sync(FULLMASK, (b < 8) ? ys0 : ys1, (lane & ~7) + (b & 7));
+  float gx = 0.f, gy = 0.f, gz = 0.f;
+  if (q == 0) {
+    float4 g4 = geo[ee];
     float vx, vy, vz;
     sph_harm_vjp(g4.x, g4.y, g4.z, lmax, yb, vx, vy, vz);
     float dot = vx * g4.x + vy * g4.y + vz * g4.z;
     float ir = 1.0f / g4.w;
-    float gx = rbar * g4.x + (vx - dot * g4.x) * ir;
-    float gy = rbar * g4.y + (vy - dot * g4.y) * ir;
-    float gz = rbar * g4.z + (vz - dot * g4.z) * ir;
-    if (ge) { ge[3 * e] = gx; ge[3 * e + 1] = gy; ge[3 * e + 2] = gz; }
-    int i = ei[e], j = ej[e];
-    atomicAdd(&force[3 * (int64_t)i + 0], (double)gx); atomicAdd(&force[3 * (int64_t)i + 1], (double)gy);
-    atomicAdd(&force[3 * (int64_t)i + 2], (double)gz);
-    atomicAdd(&force[3 * (int64_t)j + 0], -(double)gx); atomicAdd(&force[3 * (int64_t)j + 1], -(double)gy);
-    atomicAdd(&force[3 * (int64_t)j + 2], -(double)gz);
+    gx = pr * g4.x + (vx - dot * g4.x) * ir;
+    gy = pr * g4.y + (vy - dot * g4.y) * ir;
+    gz = pr * g4.z + (vz - dot * g4.z) * ir;
+    if (ge && live) { ge[3 * e] = gx; ge[3 * e + 1] = gy; ge[3 * e + 2] = gz; }
+  }
+  // lanes 0-2: F_i[k] += g[k] ; lanes 3-5: F_j[k] -= g[k]
+  const int src = lane & ~7;
+  gx = __shfl_sync(FULLMASK, gx, src); gy = __shfl_sync(FULLMASK, gy, src); gz = __shfl_sync(FULLMASK, gz, src);
+  if (live && q < 6) {
+    const int k = (q < 3) ? q : q - 3;
+    const float g = (k == 0) ? gx : (k == 1) ? gy : gz;
+    const int atom = (q < 3) ? ei[e] : ej[e];
+    atomicAdd(&force[3 * (int64_t)atom + k], (q < 3) ? (double)g : -(double)g);
   }
 }
 
@@ -516,7 +589,7 @@ int k_launch_twobody0(allegro_model* m, Work& w, const int32_t* species, const D
   if (m_cap <= 0) return ALLEGRO_OK;
   float* act = single ? (float*)w.XS[0].p : (float*)w.tb_a[0].p;
   int ld = single ? (m->d + m->n) : L0.fo;
-  k_twobody0<<<(m_cap + TB0_EPB - 1) / TB0_EPB, 128, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, (int*)w.ej.p, species,
+  k_twobody0<<<(m_cap + TB0_EDGES - 1) / TB0_EDGES, 256, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, (int*)w.ej.p, species,
                                                                     (float*)w.B.p, (float*)w.u.p, L0.W, m->S, m->NB, L0.fo,
                                                                     (float*)w.tb_z[0].p, act, ld, single ? 1 : 0);
   LAUNCH_CHECK(m);
@@ -599,8 +672,12 @@ int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
 int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c0, int nc, const float* xf, double* e_atom) {
   ProfScope _ps(m, PC_ENERGY);
   if (nc <= 0) return ALLEGRO_OK;
-  k_energy<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, xf, m->d, m->w_eff_d, species,
-                                                        m->sigma, m->mu, e_atom);
+  if (w.n_eparts > 0 && xf != nullptr)
+    k_energy_parts<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, (const double*)w.epart.p,
+                                                                w.n_eparts, (int64_t)w.cap_edges, species, m->sigma, m->mu, e_atom);
+  else
+    k_energy<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, xf, m->d, m->w_eff_d, species,
+                                                          m->sigma, m->mu, e_atom);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
@@ -618,7 +695,7 @@ int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, con
   if (m_cap <= 0) return ALLEGRO_OK;
   k_bwd_prep<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>((int*)w.m_act.p, xbar, ldx, z, ldz,
                                                                                   (float*)w.u.p, c, zb, ldzb, width,
-                                                                                  (float*)w.ubar.p, (float*)w.sig.p, m->w_eff_f);
+                                                                                  (float*)w.ubar.p + (size_t)(w.n_uparts - 1) * w.cap_edges, (float*)w.sig.p, m->w_eff_f);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
@@ -628,9 +705,14 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
   ProfScope _ps(m, PC_EDGE_BWD);
   if (m_cap <= 0) return ALLEGRO_OK;
   (void)single;
-  k_edge_bwd<<<(unsigned)(((int64_t)m_cap * 32 + 255) / 256), 256, 0, m->stream>>>(
-      (int*)w.m_act.p, zb1, ldz, L0.W, m->S, m->NB, L0.fo, (float4*)w.geo.p, (float*)w.du.p, (float*)w.dB.p,
-      (float*)w.ubar.p, (float*)w.Ybar.p, ((m->n + 31) / 32) * (m->NL + 1), (int64_t)w.cap_edges * m->Denv, m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
+  const int H = L0.fo;
+  size_t sm = (size_t)(m->NB + EB_EDGES) * (H + 4) * sizeof(float);
+  static size_t sm_set = 0;
+  if (sm > sm_set) { AL_CUDA(m, cudaFuncSetAttribute(k_edge_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); sm_set = sm; }
+  k_edge_bwd<<<(unsigned)((m_cap + EB_EDGES - 1) / EB_EDGES), 256, sm, m->stream>>>(
+      (int*)w.m_act.p, zb1, ldz, L0.W, m->S, m->NB, H, (float4*)w.geo.p, (float*)w.du.p, (float*)w.dB.p, (float*)w.ubar.p,
+      w.n_uparts, (int64_t)w.cap_edges, (float*)w.Ybar.p, ((m->n + 31) / 32) * (m->NL + 1), (int64_t)w.cap_edges * m->Denv,
+      m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }

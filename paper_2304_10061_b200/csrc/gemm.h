@@ -13,7 +13,14 @@ enum GemmEpi {
   EPI_LATENT = 3,     // out2 = acc ; C = c0 * aux1[m,n] + c1 * u[m] * silu(acc)        (x^L residual update)
   EPI_MUL_DSILU = 4,  // C = acc * silu'(aux1[m,n])                                    (backward through SiLU)
   EPI_ADD2 = 5,       // C = acc + c0 * aux1[m,n] + aux2[m,n]                           (x-bar accumulation)
-  EPI_ADD2R = 6       // C = acc + c0 * u[m] * aux3[n] + aux2[m,n]   (rank-1 incoming gradient sigma_e * w_eff)
+  EPI_ADD2R = 6,      // C = acc + c0 * u[m] * aux3[n] + aux2[m,n]   (rank-1 incoming gradient sigma_e * w_eff)
+  // Last latent layer, forward and the start of the backward in one epilogue (x-bar^{NL} = sigma_e w_eff is
+  // known a priori): with x = c0 * aux1 + c1 * u * silu(acc),
+  //   out2  = c1 * u[m] * sig[m] * aux3[n] * silu'(acc)                     (z-bar of this layer; replaces z)
+  //   upart[p][m] = c1 * sig[m] * sum_{n in chunk p} aux3[n] * silu(acc)     (u-bar partial, fp32)
+  //   epart[p][m] = sum_{n in chunk p} x * w_eff_d[n]                        (edge-energy partial, fp64)
+  //   C = x only if C != nullptr (debug tap); chunks are 32 columns, see al_gemm_row_parts()
+  EPI_LATENT_LAST = 7
 };
 
 struct GemmArgs {
@@ -29,10 +36,14 @@ struct GemmArgs {
   const float* aux3; int ld3;
   float* out2; int ldo2;
   const float* u;                 // per-row scalar
-  float* ubar;                    // per-row accumulation target (EPI_LATENT_BWD)
+  const float* sig;               // per-row sigma_{Z_i(e)} (EPI_LATENT_LAST)
+  const double* w_eff_d;          // [N] fp64 folded edge-MLP vector (EPI_LATENT_LAST)
+  double* epart; float* upart; int64_t part_stride;   // [parts][part_stride] row partials (EPI_LATENT_LAST)
   float c0, c1;
 };
 
 // precision: 0 fp32 FFMA, 1 TF32 tcgen05, 2 BF16 tcgen05 (A converted on the fly is not possible with
 // TMA-fed operands, so precision 2 uses TF32 for fp32-resident activations).
 int al_gemm(struct allegro_model* m, const GemmArgs& g);
+// number of 32-column row partials the EPI_LATENT_LAST epilogue of the active GEMM kernel writes for N columns
+int al_gemm_row_parts(const struct allegro_model* m, int N);

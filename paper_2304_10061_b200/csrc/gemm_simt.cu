@@ -62,12 +62,22 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
     }
     __syncthreads();
   }
-  const int col = col0 + tx * TN;
-  if (col >= g.N) return;
+  int col = col0 + tx * TN;
+  // EPI_LATENT_LAST reduces over lanes with full-warp shuffles: no lane may exit early there; out-of-range
+  // lanes compute on clamped coordinates and store nothing.
+  const bool cok = col < g.N;
+  if (!cok) {
+    if (g.epi != EPI_LATENT_LAST) return;
+    col = 0;
+  }
 #pragma unroll
   for (int i = 0; i < TM; ++i) {
     int row = row0 + ty * TM + i;
-    if (row >= M) break;
+    const bool rok = row < M;
+    if (!rok) {
+      if (g.epi != EPI_LATENT_LAST) break;
+      row = M - 1;   // keep the lanes alive for the shuffles below; nothing is stored for this row
+    }
     float v[4] = {acc[i][0], acc[i][1], acc[i][2], acc[i][3]};
     float o[4];
     switch (g.epi) {
@@ -109,15 +119,50 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
         o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
         o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
       } break;
+      case EPI_LATENT_LAST: {
+        float4 x = *reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col);
+        float4 w = *reinterpret_cast<const float4*>(g.aux3 + col);
+        float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w.x, w.y, w.z, w.w}, zb[4];
+        const float us = g.u[row], sg = g.sig[row];
+        float up = 0.f; double ep = 0.0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          const float sgm = 1.0f / (1.0f + expf(-v[j]));   // one sigmoid serves silu and silu'
+          const float sl = v[j] * sgm;
+          o[j] = g.c0 * xo[j] + g.c1 * us * sl;
+          zb[j] = g.c1 * us * sg * we[j] * (sgm * (1.0f + v[j] * (1.0f - sgm)));
+          up = fmaf(we[j], sl, up);
+          ep += (double)o[j] * g.w_eff_d[col + j];
+        }
+        if (!cok) { up = 0.f; ep = 0.0; }
+        if (rok && cok) *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(zb[0], zb[1], zb[2], zb[3]);
+        // 8 consecutive lanes (tx = 8p .. 8p+7) hold the 32 columns of one chunk of this row
+#pragma unroll
+        for (int off = 1; off < 8; off <<= 1) {
+          up += __shfl_xor_sync(0xffffffffu, up, off);
+          ep += __shfl_xor_sync(0xffffffffu, ep, off);
+        }
+        if ((tx & 7) == 0 && rok && cok) {
+          const int p = col >> 5;
+          g.upart[(int64_t)p * g.part_stride + row] = g.c1 * sg * up;
+          g.epart[(int64_t)p * g.part_stride + row] = ep;
+        }
+      } break;
       default:
 #pragma unroll
         for (int j = 0; j < 4; ++j) o[j] = v[j];
     }
-    *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+    if (g.C && rok && cok) *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
   }
 }
 
 }  // namespace
+
+int al_gemm_tc_row_parts(int N);
+
+int al_gemm_row_parts(const allegro_model* m, int N) {
+  return (m->hp.precision >= 1) ? al_gemm_tc_row_parts(N) : (N + 31) / 32;
+}
 
 int al_gemm(allegro_model* m, const GemmArgs& g) {
   ProfScope _ps(m, PC_GEMM);

@@ -220,7 +220,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         const bool col_ok = (col < g.N) && (c0 + c4 < BN);
         // issue every aux load of this chunk up front (the stores below may alias, so the compiler cannot hoist them)
         float4 ax1[8], ax2[8];
-        const bool need1 = (g.epi == EPI_LATENT || g.epi == EPI_MUL_DSILU || g.epi == EPI_ADD2);
+        const bool need1 = (g.epi == EPI_LATENT || g.epi == EPI_LATENT_LAST || g.epi == EPI_MUL_DSILU || g.epi == EPI_ADD2);
         const bool need2 = (g.epi == EPI_ADD2 || g.epi == EPI_ADD2R);
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -243,7 +243,43 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           const int row = rbase + rl;
           float v[4] = {stg[rl * 33 + c4], stg[rl * 33 + c4 + 1], stg[rl * 33 + c4 + 2], stg[rl * 33 + c4 + 3]};
 #endif
-          if (row < M && col_ok) {
+          if (g.epi == EPI_LATENT_LAST) {
+            // all 32 lanes stay in step for the shuffles; out-of-range lanes contribute 0 and store nothing
+            const bool ok = row < M && col_ok;
+            const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
+            float4 x = AUX1(i);
+            float4 w = *reinterpret_cast<const float4*>(g.aux3 + cc);
+            const float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w.x, w.y, w.z, w.w};
+            const float us = g.u[rr], sg = g.sig[rr];
+            float o[4], zb[4], up = 0.f, ep4 = 0.f;
+            const float cu = g.c1 * us, cus = cu * sg;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              // one sigmoid serves silu and silu'
+              const float sgm = __fdividef(1.0f, 1.0f + __expf(-v[j]));
+              const float sl = v[j] * sgm;
+              o[j] = fmaf(g.c0, xo[j], cu * sl);
+              zb[j] = cus * we[j] * (sgm * fmaf(v[j], 1.0f - sgm, 1.0f));
+              up = fmaf(we[j], sl, up);
+              ep4 = fmaf(o[j], we[j], ep4);     // 4 terms in fp32 (w_eff rounded to fp32), the rest of the sum in fp64
+            }
+            double ep = ok ? (double)ep4 : 0.0;
+            if (!ok) up = 0.f;
+#pragma unroll
+            for (int off = 1; off < 8; off <<= 1) {
+              up += __shfl_xor_sync(0xffffffffu, up, off);
+              ep += __shfl_xor_sync(0xffffffffu, ep, off);
+            }
+            if (ok) {
+              *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(zb[0], zb[1], zb[2], zb[3]);
+              if (g.C) *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+              if ((lane & 7) == 0) {
+                const int64_t p = (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
+                g.upart[p * g.part_stride + row] = g.c1 * sg * up;
+                g.epart[p * g.part_stride + row] = ep;
+              }
+            }
+          } else if (row < M && col_ok) {
             float o[4];
             switch (g.epi) {
               case EPI_SILU_BOTH:
@@ -361,6 +397,12 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
+}
+
+int al_gemm_tc_row_parts(int N) {
+  int ntn = (N + BN_MAX - 1) / BN_MAX;
+  int BN = ((N + ntn - 1) / ntn + 15) & ~15;
+  return ntn * ((BN + 31) >> 5);
 }
 
 int al_upload_bf16(allegro_model* m, void** dst, const std::vector<float>& h) {

@@ -110,6 +110,7 @@ struct allegro_model {
   cudaStream_t stream = 0;
   allegro_alloc_fn alloc_fn = nullptr; allegro_free_fn free_fn = nullptr; void* alloc_user = nullptr;
   int64_t chunk_edges = 1 << 20;
+  bool debug_keep = false;                // allegro_set_debug: also store tensors that are otherwise consumed on chip
   int64_t launches = 0;
   std::string err;
   int sm_count = 148;

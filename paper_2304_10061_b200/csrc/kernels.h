@@ -27,7 +27,9 @@ struct Work {
   DevBuf G;                                 // [M][d+n] = [x-bar part | s-bar]
   DevBuf OB;                                // [M][2 nA] omega-bar (and w0-bar)
   DevBuf VB0, VB1;                          // V-bar ping-pong [M][Dmax][n]
-  DevBuf ubar, Ybar;                        // [M], [M][Denv]
+  DevBuf ubar, Ybar;                        // u-bar partials [n_uparts][M]; Y-bar partials [groups*(NL+1)][M][Denv]
+  int n_uparts = 1;
+  DevBuf epart; int n_eparts = 0;           // f64 edge-energy partials [n_eparts][M] (EPI_LATENT_LAST)
   DevBuf ge;                                // float[M][3] dE/dr_e (debug tap)
   DevBuf eatom;                             // f64[N] when the caller passes e_atom = NULL
   int64_t eatom_cap = 0;

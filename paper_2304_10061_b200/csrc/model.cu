@@ -294,6 +294,12 @@ extern "C" int allegro_set_allocator(allegro_model* m, allegro_alloc_fn a, alleg
   return ALLEGRO_OK;
 }
 
+extern "C" int allegro_set_debug(allegro_model* m, int on) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  m->debug_keep = on != 0;
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_set_chunk_edges(allegro_model* m, int64_t e) {
   if (!m || e < 1024) return ALLEGRO_ERR_BAD_ARG;
   m->chunk_edges = e;

@@ -87,6 +87,7 @@ def test_intermediates_cfg0():
     cfg = scaled_config(0, 192)
     pos, sp, box = make_system(cfg)
     model, oracle = make_both(cfg)
+    model.set_debug(True)
     got, nb = gpu_eval(model, pos, sp, box)
     ei, ej, es = O.neighbor_list(pos, box, cfg.hp.r_cut)
     t = torch.from_numpy
