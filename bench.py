@@ -148,6 +148,7 @@ def main():
     ap.add_argument("--precision", type=int, default=1, help="0 fp32 FFMA, 1 TF32 tensor cores")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
     args = ap.parse_args()
     K, W = args.steps, max(args.warmup, 3)
     rank = int(os.environ.get("RANK", "0"))
@@ -201,7 +202,7 @@ def main():
     N = pos.shape[0]
     chp = P.hparams_from(cfg.hp, args.precision)
     blob = make_blob(cfg.hp, P.path_fan(chp), [cfg.sigma] * cfg.hp.n_species, cfg.mu(), cfg.weight_seed)
-    model = P.Allegro(chp, blob)
+    model = P.Allegro(chp, blob, chunk_edges=args.chunk_edges) if args.chunk_edges else P.Allegro(chp, blob)
     dev = torch.device("cuda", local_rank)
     p = torch.from_numpy(pos.copy()).to(dev); v = torch.from_numpy(vel.copy()).to(dev)
     s = torch.from_numpy(sp).to(dev); mass = torch.from_numpy(masses_for(cfg)).to(dev)

@@ -2,6 +2,7 @@
 // stack (2), §8(a) steps 2-11).  No host synchronisation inside; the number of active edges of a chunk
 // lives on the device (Work::m_act) and every kernel grid is sized for the chunk's candidate count.
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 
 #include "gemm.h"
@@ -44,7 +45,8 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     AL_CHECK(R(w.G, (size_t)M * (d + n))); AL_CHECK(R(w.OB, (size_t)M * 2 * nA));
     AL_CHECK(R(w.VB0, (size_t)M * Dmax * n)); AL_CHECK(R(w.VB1, (size_t)M * Dmax * n));
     w.n_eparts = (d % 32 == 0) ? al_gemm_row_parts(m, d) : 0;   // > 0: last latent layer fused with energy / z-bar (EPI_LATENT_LAST)
-    w.n_uparts = w.n_eparts + 1;
+    // u-bar partial slots: [0, P) EPI_LATENT_LAST, then P per fused prep stage (NL of them), then one accumulated by k_bwd_prep
+    w.n_uparts = (w.n_eparts > 0) ? w.n_eparts * (NL + 1) + 1 : 1;
     AL_CHECK(R(w.ubar, (size_t)M * w.n_uparts)); AL_CHECK(R(w.epart, (size_t)2 * M * std::max(w.n_eparts, 1)));
     AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * ((n + 31) / 32) * (NL + 1))); AL_CHECK(R(w.ge, (size_t)3 * M));
     w.cap_edges = M;
@@ -166,9 +168,15 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   float* xb = (float*)w.XB0.p; float* xb_o = (float*)w.XB1.p;
   float* vb = nullptr; float* vb_a = (float*)w.VB0.p; float* vb_b = (float*)w.VB1.p;
   bool rank1 = true;   // x-bar^{NL} = sigma_e * w_eff is never materialised
+  // With fused_last every z-bar that starts an MLP's backward comes out of a GEMM epilogue (EPI_LATENT_LAST for
+  // layer NL, the prep stage of EPI_ADD2/ADD2R for the others); otherwise k_bwd_prep computes it.
+  bool zb_ready = fused_last;
+  static const bool no_prep = getenv("B200_ALLEGRO_NO_PREP") != nullptr;   // experiment switch: keep k_bwd_prep for L < NL
+  const bool fuse_prep = fused_last && !no_prep;
+  int prep_slot = 1;
   for (int L = NL; L >= 1; --L) {
     float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
-    if (!(rank1 && fused_last))   // (fused: z-bar^{NL} was written by the forward epilogue)
+    if (!zb_ready)
       AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
     for (int k = nlat - 1; k >= 1; --k) {
       GemmArgs g = mk(zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
@@ -190,13 +198,24 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
                     rank1 ? EPI_ADD2R : EPI_ADD2);
     g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = (float*)w.G.p; g.ld2 = d + n;
     g.u = (float*)w.sig.p; g.aux3 = m->w_eff_f;
+    if (fuse_prep) {
+      // prep stage: z-bar of the MLP below (latent MLP of layer L-1, or the two-body MLP when L = 1)
+      g.prep = 1;
+      g.zp = (L > 1) ? (float*)w.lat_z[L - 2][nlat - 1].p : (float*)w.tb_z[ntb - 1].p; g.ldzp = d;
+      g.zbp = (float*)w.ZB0.p; g.ldzbp = d; g.pu = (float*)w.u.p; g.cp = (L > 1) ? m->c_new[L - 2] : 1.0f;
+      g.upart = (float*)w.ubar.p; g.part_stride = w.cap_edges; g.pbase = prep_slot * w.n_eparts;
+      ++prep_slot;
+      if (L == 1 && !m->debug_keep) g.C = nullptr;   // x-bar^0 itself is not needed afterwards
+    }
     AL_CHECK(al_gemm(m, g));
     std::swap(xb, xb_o);
     rank1 = false;
+    zb_ready = fuse_prep;
   }
   {
     float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
-    AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.tb_z[ntb - 1].p, d, 1.0f, zb, d, d, m_cap));
+    if (!zb_ready)
+      AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.tb_z[ntb - 1].p, d, 1.0f, zb, d, d, m_cap));
     for (int k = ntb - 1; k >= 1; --k) {
       GemmArgs g = mk(zb, hp.twobody_dims[k], m->twobody[k], true, zb_o, hp.twobody_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
       g.aux1 = (float*)w.tb_z[k - 1].p; g.ld1 = hp.twobody_dims[k - 1];

@@ -38,7 +38,12 @@ struct GemmArgs {
   const float* u;                 // per-row scalar
   const float* sig;               // per-row sigma_{Z_i(e)} (EPI_LATENT_LAST)
   const double* w_eff_d;          // [N] fp64 folded edge-MLP vector (EPI_LATENT_LAST)
-  double* epart; float* upart; int64_t part_stride;   // [parts][part_stride] row partials (EPI_LATENT_LAST)
+  double* epart; float* upart; int64_t part_stride;   // [parts][part_stride] row partials (EPI_LATENT_LAST, prep)
+  // Optional second stage of EPI_ADD2 / EPI_ADD2R (replaces k_bwd_prep): with xb = the epilogue's result (x-bar),
+  //   zbp[m,n] = cp * pu[m] * xb * silu'(zp[m,n])          (z-bar entering the next MLP to differentiate)
+  //   upart[pbase + chunk][m] = cp * sum_{n in chunk} xb * silu(zp[m,n])     (u-bar partial)
+  // C may be NULL when x-bar itself is not needed afterwards.
+  int prep; const float* zp; int ldzp; float* zbp; int ldzbp; const float* pu; float cp; int pbase;
   float c0, c1;
 };
 

@@ -66,8 +66,9 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
   // EPI_LATENT_LAST reduces over lanes with full-warp shuffles: no lane may exit early there; out-of-range
   // lanes compute on clamped coordinates and store nothing.
   const bool cok = col < g.N;
+  const bool shf = (g.epi == EPI_LATENT_LAST) || g.prep;   // epilogues with warp shuffles
   if (!cok) {
-    if (g.epi != EPI_LATENT_LAST) return;
+    if (!shf) return;
     col = 0;
   }
 #pragma unroll
@@ -75,7 +76,7 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
     int row = row0 + ty * TM + i;
     const bool rok = row < M;
     if (!rok) {
-      if (g.epi != EPI_LATENT_LAST) break;
+      if (!shf) break;
       row = M - 1;   // keep the lanes alive for the shuffles below; nothing is stored for this row
     }
     float v[4] = {acc[i][0], acc[i][1], acc[i][2], acc[i][3]};
@@ -151,6 +152,23 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
       default:
 #pragma unroll
         for (int j = 0; j < 4; ++j) o[j] = v[j];
+    }
+    if (g.prep) {
+      float4 zq = *reinterpret_cast<const float4*>(g.zp + (size_t)row * g.ldzp + col);
+      const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
+      const float cu = g.cp * g.pu[row];
+      float zb[4], up = 0.f;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const float sgm = 1.0f / (1.0f + expf(-zz[j]));
+        up = fmaf(o[j], zz[j] * sgm, up);
+        zb[j] = cu * o[j] * (sgm * (1.0f + zz[j] * (1.0f - sgm)));
+      }
+      if (!cok) up = 0.f;
+      if (rok && cok) *reinterpret_cast<float4*>(g.zbp + (size_t)row * g.ldzbp + col) = make_float4(zb[0], zb[1], zb[2], zb[3]);
+#pragma unroll
+      for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
+      if ((tx & 7) == 0 && rok && cok) g.upart[(int64_t)(g.pbase + (col >> 5)) * g.part_stride + row] = g.cp * up;
     }
     if (g.C && rok && cok) *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
   }

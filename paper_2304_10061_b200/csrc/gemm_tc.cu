@@ -19,26 +19,17 @@
 
 namespace {
 
-#ifndef EPI_DIRECT
-#define EPI_DIRECT 0
-#endif
-#if EPI_DIRECT
-#define AUX1(i) (*reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col))
-#define AUX2(i) (*reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col))
-#else
-#define AUX1(i) ax1[i]
-#define AUX2(i) ax2[i]
-#endif
+#define AUX1(i) ax1[(i) & 3]
+#define AUX2(i) ax2[(i) & 3]
 constexpr int BM = 128;          // UMMA M (cta_group::1)
 constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
-constexpr int STAGES = 3;
 constexpr int BN_MAX = 256;
-constexpr int EPI_WARPS = 16;     // 2 per TMEM lane quarter, alternating 32-column chunks
-constexpr int NTHREADS = 64 + 32 * EPI_WARPS;
 constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
 constexpr uint32_t B_STAGE_BYTES = BN_MAX * BKF * 4;       // 32 KB (allocated for the largest BN)
-constexpr uint32_t STG_BYTES = EPI_WARPS * 32 * 33 * 4;             // epilogue transpose staging, one 32x33 tile per warp
-constexpr uint32_t SMEM_BYTES = STAGES * (A_STAGE_BYTES + B_STAGE_BYTES) + 1024 /*align*/ + 256 /*barriers*/ + STG_BYTES;
+// epilogue transpose staging: one 32x32 fp32 tile per warp, float4-granular XOR swizzle (conflict-free both ways)
+constexpr uint32_t smem_bytes(int stages, int epi_warps) {
+  return stages * (A_STAGE_BYTES + B_STAGE_BYTES) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
+}
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -118,7 +109,8 @@ __device__ __forceinline__ float dsilu_f(float z) {
   return s * fmaf(z, 1.0f - s, 1.0f);
 }
 
-__global__ void __launch_bounds__(NTHREADS, 1)
+template <int STAGES, int EPI_WARPS>
+__global__ void __launch_bounds__(64 + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, GemmArgs g, int BN, int ntn) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
@@ -205,44 +197,43 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       // Each 32-column chunk: TMEM -> registers (lane = row) -> padded smem -> registers in the
       // "coalesced domain" (8 lanes x float4 cover one row's 128 B, 4 rows per warp instruction), so
       // every global load/store of the epilogue touches 4 lines per instruction instead of 32.
-      float* stg = stage_buf + (warp - 2) * (32 * 33);
+      float4* stg4 = reinterpret_cast<float4*>(stage_buf) + (warp - 2) * (32 * 8);
       const int chunk0 = (warp - 2) >> 2;   // this warp takes chunks chunk0, chunk0 + EPI_WARPS/4, ...
       const int rsub = lane >> 3, c4 = (lane & 7) * 4;
       const int rbase = mt * BM + q * 32;
       for (int c0 = chunk0 * 32; c0 < BN; c0 += 32 * (EPI_WARPS / 4)) {
         uint32_t r[32];
         tc_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN_MAX + c0, r);
-#if !EPI_DIRECT
 #pragma unroll
-        for (int j = 0; j < 32; ++j) stg[lane * 33 + j] = __uint_as_float(r[j]);
+        for (int gq = 0; gq < 8; ++gq)
+          stg4[lane * 8 + (gq ^ (lane & 7))] = make_float4(__uint_as_float(r[4 * gq]), __uint_as_float(r[4 * gq + 1]),
+                                                           __uint_as_float(r[4 * gq + 2]), __uint_as_float(r[4 * gq + 3]));
         __syncwarp();
         const int col = nt * BN + c0 + c4;
         const bool col_ok = (col < g.N) && (c0 + c4 < BN);
-        // issue every aux load of this chunk up front (the stores below may alias, so the compiler cannot hoist them)
-        float4 ax1[8], ax2[8];
+        // Two halves of 16 rows: issue every aux load of a half up front (the stores below may alias, so the compiler
+        // cannot hoist them), then process it.  Halving keeps the register count low enough for 16 epilogue warps.
         const bool need1 = (g.epi == EPI_LATENT || g.epi == EPI_LATENT_LAST || g.epi == EPI_MUL_DSILU || g.epi == EPI_ADD2);
         const bool need2 = (g.epi == EPI_ADD2 || g.epi == EPI_ADD2R);
+#pragma unroll 1
+        for (int h = 0; h < 2; ++h) {
+        float4 ax1[4], ax2[4], ax3[4];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
+        for (int ii = 0; ii < 4; ++ii) {
+          const int i = h * 4 + ii;
           const int row = rbase + i * 4 + rsub;
           const bool ok = row < M && col_ok;
-          ax1[i] = (need1 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax2[i] = (need2 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax1[ii] = (need1 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax2[ii] = (need2 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax3[ii] = (g.prep && ok) ? __ldg(reinterpret_cast<const float4*>(g.zp + (size_t)row * g.ldzp + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
-#endif
 #pragma unroll
-        for (int i = 0; i < 8; ++i) {
-#if EPI_DIRECT
-          const int row = rbase + lane;
-          const int col = nt * BN + c0 + i * 4;
-          const bool col_ok = (col < g.N) && (c0 + i * 4 < BN);
-          float v[4] = {__uint_as_float(r[i * 4]), __uint_as_float(r[i * 4 + 1]), __uint_as_float(r[i * 4 + 2]),
-                        __uint_as_float(r[i * 4 + 3])};
-#else
+        for (int ii = 0; ii < 4; ++ii) {
+          const int i = h * 4 + ii;
           const int rl = i * 4 + rsub;
           const int row = rbase + rl;
-          float v[4] = {stg[rl * 33 + c4], stg[rl * 33 + c4 + 1], stg[rl * 33 + c4 + 2], stg[rl * 33 + c4 + 3]};
-#endif
+          const float4 v4 = stg4[rl * 8 + ((lane & 7) ^ (rl & 7))];
+          float v[4] = {v4.x, v4.y, v4.z, v4.w};
           if (g.epi == EPI_LATENT_LAST) {
             // all 32 lanes stay in step for the shuffles; out-of-range lanes contribute 0 and store nothing
             const bool ok = row < M && col_ok;
@@ -277,6 +268,43 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 const int64_t p = (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.c1 * sg * up;
                 g.epart[p * g.part_stride + row] = ep;
+              }
+            }
+          } else if (g.prep) {
+            // EPI_ADD2 / EPI_ADD2R followed by the z-bar / u-bar stage of the next MLP (all lanes stay in step)
+            const bool ok = row < M && col_ok;
+            const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
+            float o[4];
+            const float4 y = AUX2(i);
+            if (g.epi == EPI_ADD2) {
+              const float4 x = AUX1(i);
+              o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
+              o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
+            } else {
+              const float4 x = *reinterpret_cast<const float4*>(g.aux3 + cc);
+              const float cs = g.c0 * g.u[rr];
+              o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
+              o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
+            }
+            const float4 zq = ax3[ii];
+            const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
+            const float cu = g.cp * g.pu[rr];
+            float zb[4], up = 0.f;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+              const float sgm = __fdividef(1.0f, 1.0f + __expf(-zz[j]));
+              up = fmaf(o[j], zz[j] * sgm, up);
+              zb[j] = cu * o[j] * (sgm * fmaf(zz[j], 1.0f - sgm, 1.0f));
+            }
+            if (!ok) up = 0.f;
+#pragma unroll
+            for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
+            if (ok) {
+              *reinterpret_cast<float4*>(g.zbp + (size_t)row * g.ldzbp + col) = make_float4(zb[0], zb[1], zb[2], zb[3]);
+              if (g.C) *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+              if ((lane & 7) == 0) {
+                const int64_t p = g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
+                g.upart[p * g.part_stride + row] = g.cp * up;
               }
             }
           } else if (row < M && col_ok) {
@@ -323,6 +351,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
           }
         }
+        }   // halves
         __syncwarp();
       }
       tc_fence_before();
@@ -386,14 +415,22 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
   CUtensorMap tmA, tmB;
   AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, &tmA));
   AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, &tmB));
-  static bool attr_set = false;
-  if (!attr_set) {
-    AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_BYTES));
-    attr_set = true;
-  }
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  k_gemm_tf32<<<grid, NTHREADS, SMEM_BYTES, m->stream>>>(tmA, tmB, g, BN, ntn);
+  static const int variant = getenv("B200_ALLEGRO_GEMM_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM_VARIANT")) : 0;   // 0: 16 epilogue warps (measured best), 1: 8, 2: 12
+#define GEMM_LAUNCH(ST, EW)                                                                                              \
+  {                                                                                                                      \
+    static bool attr_set = false;                                                                                        \
+    if (!attr_set) {                                                                                                     \
+      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<ST, EW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(ST, EW))); \
+      attr_set = true;                                                                                                   \
+    }                                                                                                                    \
+    k_gemm_tf32<ST, EW><<<grid, 64 + 32 * EW, smem_bytes(ST, EW), m->stream>>>(tmA, tmB, g, BN, ntn);                     \
+  }
+  if (variant == 0) GEMM_LAUNCH(3, 16)
+  else if (variant == 2) GEMM_LAUNCH(3, 12)
+  else GEMM_LAUNCH(3, 8)
+#undef GEMM_LAUNCH
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
