@@ -46,28 +46,54 @@ def gemm_macs_per_edge(hp):
 def gemm_bytes_per_edge(hp):
     """Algorithmic HBM bytes per ACTIVE edge of the GEMM kernel group (fp32 storage): every launch reads its A
     operand once and writes its outputs once; aux operands of the fused epilogues are read once.  Weights are
-    L2-resident and not counted.  Mirrors the launch list of csrc/compute.cu::run_chunk."""
+    L2-resident and not counted.  Mirrors the launch list of csrc/compute.cu::run_chunk (default path: last latent
+    layer fused with the energy / z-bar epilogue, z-bar prep stage fused into the x-bar GEMMs)."""
     d, n, nA, NL = hp.twobody_dims[-1], hp.n_tensor, hp.n_tensor * (hp.l_max + 1), hp.n_layers
     tb, lat = list(hp.twobody_dims), list(hp.latent_dims)
-    fl = 0
+    parts = 12.0 * ((d + 31) // 32) / 4.0             # fp64 energy + fp32 u-bar partial per 32 columns, in floats
+    fl = 0.0
     for k in range(1, len(tb)):                       # two-body forward: A, C (activation), out2 (pre-activation)
         fl += tb[k - 1] + 2 * tb[k]
     fl += d + 2 * nA                                  # [w0 | omega1]
     for L in range(1, NL + 1):
         for k in range(len(lat)):
             K = d + n if k == 0 else lat[k - 1]
-            fl += K + 2 * lat[k] + (d if k == len(lat) - 1 else 0)      # last: residual x^{L-1} read
+            last = k == len(lat) - 1
+            if last and L == NL:
+                fl += K + lat[k] + d + parts          # A, z-bar out, residual x^{L-1} read, row partials (x^{NL} not stored)
+            else:
+                fl += K + 2 * lat[k] + (d if last else 0)
         if L < NL:
             fl += d + nA
     for L in range(NL, 0, -1):                        # backward
         for k in range(len(lat) - 1, 0, -1):
             fl += lat[k] + 2 * lat[k - 1]             # A, aux z, C
-        fl += lat[0] + (d + n)
+        fl += lat[0] + (d + n)                        # dX of the first latent layer -> [x-bar part | s-bar]
         Kx = 2 * nA if L == 1 else nA
-        fl += Kx + d * (2 if L == NL else 3)          # A, aux2 (+ aux1 unless rank-1), C
+        # x-bar GEMM + prep stage: A, aux2 (+ aux1 unless rank-1), z of the MLP below, z-bar out, u-bar partials,
+        # C = x-bar (not stored for L = 1)
+        fl += Kx + d + (0 if L == NL else d) + d + d + parts / 3.0 + (d if L > 1 else 0)
     for k in range(len(tb) - 1, 0, -1):
         fl += tb[k] + 2 * tb[k - 1]
-    return 4 * fl
+    return 4.0 * fl
+
+
+def tp_bytes_per_edge(hp):
+    """Algorithmic HBM bytes per ACTIVE edge of the tensor-track kernels (fp32 storage; every operand row read or
+    written once, Y rows and per-center quantities not counted).  D_L from the pruned irreps."""
+    n, nl = hp.n_tensor, hp.l_max + 1
+    D = {(1, 1): [4, 1], (2, 2): [9, 9, 1], (3, 3): [16, 31, 16, 1]}.get((hp.l_max, hp.n_layers))
+    if D is None:
+        return {"tp_fwd": 0.0, "tp_bwd": 0.0}
+    fwd = bwd = 0.0
+    for L in range(1, hp.n_layers + 1):
+        din, dout = D[L - 1], D[L]
+        vin = nl if L == 1 else din                   # layer 1 reads w0 (one value per l), not V^0
+        tout = dout if L < hp.n_layers else 0         # last layer writes only the scalars
+        fwd += n * (nl + vin + tout + 1)              # omega, V (or w0), T, s
+        # backward: omega, V (or w0), V-bar^L, s-bar in; V-bar^{L-1} (or w0-bar), omega-bar out
+        bwd += n * (nl + vin + tout + 1 + vin + nl)
+    return {"tp_fwd": 4.0 * fwd, "tp_bwd": 4.0 * bwd}
 
 
 class ClockSampler(threading.Thread):
@@ -251,6 +277,7 @@ def main():
 
     # ---- roofline of the dominant kernel group: second pass of K steps with per-group CUDA events
     groups = ["gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd", "neighbors", "nve"]
+    tp_bytes = tp_bytes_per_edge(cfg.hp)
     model.profile_enable(True)
     for _ in range(K):
         model.step_nve(p, v, f, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, e, ek)
@@ -275,12 +302,24 @@ def main():
     hbm = {"bound": "hbm", "achieved": gemm_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm,
            "peak_note": f"copy bandwidth ({pk['src']}); algorithmic bytes = {gemm_bytes_per_edge(cfg.hp)} B per active edge"}
     top = hbm if f_hbm > f_compute else comp       # the binding roofline is the one with the larger fraction
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
+    if os.path.exists(tpath):   # dram__bytes_read+write per GEMM launch from the committed ncu --set full capture
+        tj = json.load(open(tpath)).get(f"config{cfg.index}_precision{args.precision}")
+        if tj:
+            traffic = tj["gemm_dram_bytes_per_launch"]
     roofline = {"bound": top["bound"], "kernel": "MLP GEMM group (fwd+bwd), k_gemm_tf32" if args.precision else "MLP GEMM group (fwd+bwd), k_gemm_simt",
-                "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"], "traffic": None,
+                "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"], "traffic": traffic,
+                "algorithmic_bytes_per_launch": gemm_bytes_per_edge(cfg.hp) * n_active * K / max(gemm_n, 1),
                 "peak_note": top["peak_note"], "compute_roofline": comp, "hbm_roofline": hbm,
                 "launches_per_step": gemm_n / K, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
                 "share_of_step": gemm_ms / tot_prof if tot_prof else None,
-                "groups_ms_per_step": {g: round(t / K, 4) for g, (t, _) in prof.items()}}
+                "groups_ms_per_step": {g: round(t / K, 4) for g, (t, _) in prof.items()},
+                # the tensor-track kernels against the HBM roofline (north_star: gather/tensor-product/scatter >= 50 %)
+                "tensor_track_hbm": {k: {"achieved": tp_bytes[k] * n_active * K / (prof[k][0] * 1e-3) / 1e9 if prof[k][0] > 0 else 0.0,
+                                         "peak": pk["hbm_gbs"], "unit": "GB/s",
+                                         "frac": (tp_bytes[k] * n_active * K / (prof[k][0] * 1e-3) / 1e9 / pk["hbm_gbs"]) if prof[k][0] > 0 else 0.0,
+                                         "algorithmic_bytes_per_edge": tp_bytes[k]} for k in ("tp_fwd", "tp_bwd")}}
 
     out = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
