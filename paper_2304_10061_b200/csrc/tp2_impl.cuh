@@ -120,18 +120,21 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(const __grid_consta
   const int deg = (int)(e1 - e0);
   if (deg <= 0) return;
 
-  auto issue = [&](int64_t e, float* st) {
-    if (FIRST) {
-      tp_cp_rows<NLV>(st, a.w0 + e * a.ldw + grp * 32, a.n, lane);
-      if (lane < LDY / 4) tp_cp16(st + NLV * 32 + lane * 4, a.Y + e * a.ldy + lane * 4);
-    } else {
-      tp_cp_rows<DIN>(st, a.Vin + e * DIN * a.n + grp * 32, a.n, lane);
-    }
+  // per-center base pointers and hoisted per-lane chunk offsets: the edge loop only adds il * stride
+  constexpr int OPROWS = FIRST ? NLV : DIN;
+  int off_op[(OPROWS * 8 + 31) / 32];
+  tp_row_offsets<OPROWS>(off_op, a.n, lane);
+  const float* opc = FIRST ? a.w0 + e0 * a.ldw + grp * 32 : a.Vin + e0 * DIN * a.n + grp * 32;
+  const int op_stride = FIRST ? a.ldw : DIN * a.n;
+  const float* Yc = a.Y + e0 * a.ldy + lane * 4;
+  auto issue = [&](int il, float* st) {
+    tp_cp_rows_pre<OPROWS>(st, opc + il * op_stride, off_op, lane);
+    if (FIRST && lane < LDY / 4) tp_cp16(st + NLV * 32 + lane * 4, Yc + il * a.ldy);
   };
   // start streaming the first edges while Gamma_i is being summed
 #pragma unroll
   for (int s = 0; s < NST - 1; ++s) {
-    if (s < deg) issue(e0 + s, ring + s * SF);
+    if (s < deg) issue(s, ring + s * SF);
     tp_cp_commit();
   }
   {
@@ -162,22 +165,23 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(const __grid_consta
       __syncwarp();
 #pragma unroll
       for (int s = 0; s < NST - 1; ++s) {
-        if (s < deg) issue(e0 + s, ring + s * SF);
+        if (s < deg) issue(s, ring + s * SF);
         tp_cp_commit();
       }
     }
     int slot = 0;
+    float* xsp = a.xs + e0 * a.ldx + nn;
+    float* Tp = a.Tout ? a.Tout + (e0 * DOUT + cb) * a.n + nn : nullptr;
     for (int i = 0; i < deg; ++i) {
       tp_cp_wait<NST - 2>();
       __syncwarp();
       {
         const int nx = i + NST - 1;
         int ns = slot + NST - 1; if (ns >= NST) ns -= NST;
-        if (nx < deg) issue(e0 + nx, ring + ns * SF);
+        if (nx < deg) issue(nx, ring + ns * SF);
         tp_cp_commit();
       }
       const float* st = ring + slot * SF;
-      const int64_t e = e0 + i;
       float2 acc[CBH];
 #pragma unroll
       for (int j = 0; j < CBH; ++j) acc[j] = make_float2(0.f, 0.f);
@@ -188,11 +192,12 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(const __grid_consta
 #pragma unroll
         for (int j = 0; j < CBH; ++j) acc[j] = tp_fma2(v2, Mr[k * CBH + j], acc[j]);
       }
-      if (cb == 0) a.xs[e * a.ldx + nn] = acc[0].x;
-      if (a.Tout) {
+      if (cb == 0) { *xsp = acc[0].x; xsp += a.ldx; }
+      if (Tp) {
 #pragma unroll
         for (int cc = 0; cc < CB; ++cc)
-          if (cb + cc < DOUT) a.Tout[(e * DOUT + cb + cc) * a.n + nn] = (cc & 1) ? acc[cc >> 1].y : acc[cc >> 1].x;
+          if (cb + cc < DOUT) Tp[cc * a.n] = (cc & 1) ? acc[cc >> 1].y : acc[cc >> 1].x;
+        Tp += DOUT * a.n;
       }
       if (++slot == NST) slot = 0;
     }
@@ -233,21 +238,27 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
   float* Yb0 = a.Ybar + (size_t)grp * a.ybar_slots * a.ybar_pstride;
   float* YbL = Yb0 + (size_t)a.ybar_slot * a.ybar_pstride;
 
-  auto issue = [&](int64_t e, float* st, int ab) {
-    if (FIRST) {
-      tp_cp_rows<NLV>(st, a.w0 + e * a.ldw + grp * 32, a.n, lane);
-      if (lane < LDY / 4) tp_cp16(st + NLV * 32 + lane * 4, a.Y + e * a.ldy + lane * 4);
-    } else {
-      // rows ab .. ab+AB-1 of V_e (a ragged last block re-reads valid rows of the same edge)
-      const int a0 = (ab + AB <= DIN) ? ab : DIN - AB;
-      tp_cp_rows<AB>(st, a.Vin + (e * DIN + a0) * a.n + grp * 32, a.n, lane);
-    }
-    if (HASVB) tp_cp_rows<DOUT>(st + SV, a.VbarL + e * DOUT * a.n + grp * 32, a.n, lane);
-    if (lane < 8) tp_cp16(st + SF - 32 + lane * 4, a.sbar + e * a.lds + grp * 32 + lane * 4);
+  // per-center base pointers and hoisted per-lane chunk offsets: the edge loop only adds il * stride
+  constexpr int OPROWS = FIRST ? NLV : AB;
+  int off_op[(OPROWS * 8 + 31) / 32], off_vb[HASVB ? (DOUT * 8 + 31) / 32 : 1];
+  tp_row_offsets<OPROWS>(off_op, a.n, lane);
+  if (HASVB) tp_row_offsets<DOUT>(off_vb, a.n, lane);
+  const float* opc = FIRST ? a.w0 + e0 * a.ldw + grp * 32 : a.Vin + e0 * DIN * a.n + grp * 32;
+  const int op_stride = FIRST ? a.ldw : DIN * a.n;
+  const float* Yc = a.Y + e0 * a.ldy + lane * 4;
+  const float* vbc = HASVB ? a.VbarL + e0 * DOUT * a.n + grp * 32 : nullptr;
+  const float* sbc = a.sbar + e0 * a.lds + grp * 32 + (lane & 7) * 4;
+  auto issue = [&](int il, float* st, int ab) {
+    // FIRST: w0 rows + Y; else rows ab .. ab+AB-1 of V_e (a ragged last block re-reads valid rows of the same edge)
+    const int a0 = (FIRST || ab + AB <= DIN) ? ab : DIN - AB;
+    tp_cp_rows_pre<OPROWS>(st, opc + il * op_stride + (FIRST ? 0 : a0 * a.n), off_op, lane);
+    if (FIRST && lane < LDY / 4) tp_cp16(st + NLV * 32 + lane * 4, Yc + il * a.ldy);
+    if (HASVB) tp_cp_rows_pre<DOUT>(st + SV, vbc + il * (DOUT * a.n), off_vb, lane);
+    if (lane < 8) tp_cp16(st + SF - 32 + lane * 4, sbc + il * a.lds);
   };
 #pragma unroll
   for (int s = 0; s < NST - 1; ++s) {
-    if (s < deg) issue(e0 + s, ring + s * SF, 0);
+    if (s < deg) issue(s, ring + s * SF, 0);
     tp_cp_commit();
   }
   {
@@ -297,22 +308,23 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
       __syncwarp();
 #pragma unroll
       for (int s = 0; s < NST - 1; ++s) {
-        if (s < deg) issue(e0 + s, ring + s * SF, ab);
+        if (s < deg) issue(s, ring + s * SF, ab);
         tp_cp_commit();
       }
     }
     int slot = 0;
+    float* yb0p = Yb0 + e0 * DENV;
+    float* outp = FIRST ? a.w0bar + e0 * a.ldob + nn : a.Vbar_prev + (e0 * DIN + ab) * a.n + nn;
     for (int i = 0; i < deg; ++i) {
       tp_cp_wait<NST - 2>();
       __syncwarp();
       {
         const int nx = i + NST - 1;
         int ns = slot + NST - 1; if (ns >= NST) ns -= NST;
-        if (nx < deg) issue(e0 + nx, ring + ns * SF, ab);
+        if (nx < deg) issue(nx, ring + ns * SF, ab);
         tp_cp_commit();
       }
       const float* st = ring + slot * SF;
-      const int64_t e = e0 + i;
       float2 t2[CH];
 #pragma unroll
       for (int j = 0; j < CH; ++j) {
@@ -355,21 +367,24 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
       }
       if (FIRST) {
         const int nvalid = (DIN - ab < AB) ? DIN - ab : AB;
-        tp_ybar_rows<AB, true>(Yb0 + e * DENV, pp, ab, nvalid, lane);
+        tp_ybar_rows<AB, true>(yb0p, pp, ab, nvalid, lane);
+        yb0p += DENV;
 #pragma unroll
         for (int l = 0; l < NLV; ++l) {
           // (a block only touches the l values of its own components; the first toucher stores)
           const bool touched = l_of(ab) <= l && l <= l_of((ab + AB - 1 < DIN) ? ab + AB - 1 : DIN - 1);
           const bool first_touch = (ab == 0) || l_of(ab - 1) < l;
           if (touched) {
-            float* p = a.w0bar + e * a.ldob + l * a.n + nn;
+            float* p = outp + l * a.n;
             if (first_touch) *p = wb[l]; else *p += wb[l];
           }
         }
+        outp += a.ldob;
       } else {
 #pragma unroll
         for (int k = 0; k < AB; ++k)
-          if (ab + k < DIN) a.Vbar_prev[(e * DIN + ab + k) * a.n + nn] = vb[k];
+          if (ab + k < DIN) outp[k * a.n] = vb[k];
+        outp += DIN * a.n;
       }
       if (++slot == NST) slot = 0;
     }

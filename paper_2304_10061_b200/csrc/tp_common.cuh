@@ -73,6 +73,24 @@ __device__ __forceinline__ void tp_cp_rows(float* dst, const float* src, int rst
   }
 }
 
+// Same copy with the per-lane source offsets (in floats) hoisted out of the edge loop:
+//   off[it] = row * rstride + 4 * (chunk within the row), for chunk i = 32 it + lane; destination offset = 4 i.
+template <int ROWS>
+__device__ __forceinline__ void tp_row_offsets(int* off, int rstride, int lane) {
+#pragma unroll
+  for (int it = 0; it < (ROWS * 8 + 31) / 32; ++it) {
+    int i = it * 32 + lane;
+    off[it] = (i >> 3) * rstride + (i & 7) * 4;
+  }
+}
+template <int ROWS>
+__device__ __forceinline__ void tp_cp_rows_pre(float* dst, const float* src, const int* off, int lane) {
+#pragma unroll
+  for (int it = 0; it < (ROWS * 8 + 31) / 32; ++it) {
+    if (it * 32 + lane < ROWS * 8) tp_cp16(dst + (it * 32 + lane) * 4, src + off[it]);
+  }
+}
+
 #ifndef TP_FFMA2
 #define TP_FFMA2 1
 #endif
