@@ -101,6 +101,10 @@ int tp2_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   if (p == P_9_9_9) {
     FILL(P_9_9_9)
     if (mreg) return first ? launch_bwd2<P_9_9_9, 9, true, true, true, 4, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, true, 4, 4>(m, a);
+    static const int bv = getenv("B200_ALLEGRO_TP_BWDV") ? atoi(getenv("B200_ALLEGRO_TP_BWDV")) : 1;   // 1 (2 ring stages, 12 warps/SM) measured best
+    if (bv == 1) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 2, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 2, 4>(m, a);
+    if (bv == 2) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 3, 2>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 3, 2>(m, a);
+    if (bv == 3) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 2, 2>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 2, 2>(m, a);
     return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 4, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 4, 4>(m, a);
   }
   if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_bwd2<P_9_9_1, 9, true, false, true, 4, 4>(m, a) : launch_bwd2<P_9_9_1, 9, false, false, true, 4, 4>(m, a); }
