@@ -171,7 +171,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--precision", type=int, default=1, help="0 fp32 FFMA, 1 TF32 tensor cores")
+    ap.add_argument("--precision", type=int, default=1, help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores, 3 fp32 FFMA")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
@@ -288,11 +288,16 @@ def main():
     gemm_ms, gemm_n = prof["gemm"]
     flops_per_step = 2.0 * gemm_macs_per_edge(cfg.hp) * n_active
     gemm_tflops = flops_per_step * K / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
-    if args.precision == 0:
+    if args.precision == 3:
         # fp32 FFMA peak = SMs x 128 lanes x 2 flop x max SM clock (unit counts: blackwell guide; clock: MEASURED_PEAKS)
         nsm = torch.cuda.get_device_properties(dev).multi_processor_count
         peak, bound = nsm * FFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12, "alu"
         peak_note = f"{nsm} SMs x {FFMA_LANES_PER_SM} FFMA lanes x 2 x {pk['sm_max_mhz']} MHz"
+    elif args.precision == 0:
+        # 3xTF32: three TF32 MMAs per algorithmic MAC, so the useful-flop peak is a third of the TF32 figure
+        peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16 / 3.0, "tensor"
+        peak_note = (f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16} / 3 "
+                     f"(3xTF32 split operands: 3 MMAs per MAC)")
     else:
         peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16, "tensor"
         peak_note = f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16}"
@@ -308,7 +313,7 @@ def main():
         tj = json.load(open(tpath)).get(f"config{cfg.index}_precision{args.precision}")
         if tj:
             traffic = tj["gemm_dram_bytes_per_launch"]
-    roofline = {"bound": top["bound"], "kernel": "MLP GEMM group (fwd+bwd), k_gemm_tf32" if args.precision else "MLP GEMM group (fwd+bwd), k_gemm_simt",
+    roofline = {"bound": top["bound"], "kernel": {0: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., SPLIT> (3xTF32)", 1: "MLP GEMM group (fwd+bwd), k_gemm_tf32", 2: "MLP GEMM group (fwd+bwd), k_gemm_tf32", 3: "MLP GEMM group (fwd+bwd), k_gemm_simt"}[args.precision],
                 "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"], "traffic": traffic,
                 "algorithmic_bytes_per_launch": gemm_bytes_per_edge(cfg.hp) * n_active * K / max(gemm_n, 1),
                 "peak_note": top["peak_note"], "compute_roofline": comp, "hbm_roofline": hbm,
@@ -324,7 +329,7 @@ def main():
     out = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": {0: "f32", 1: "tf32", 2: "bf16"}[args.precision], "data": "synthetic",
+        "dtype": {0: "f32 (3xtf32)", 1: "tf32", 2: "bf16", 3: "f32"}[args.precision], "data": "synthetic",
         "config": {"workload": workload, "n_atoms": N, "active_edges": n_active, "candidate_edges": nb.n_edges,
                    "precision_mode": args.precision, "dt_fs": cfg.dt_fs, "rebuild_every": cfg.rebuild_every, "skin": cfg.skin,
                    "l2": "per-step working set (edge activations, several GB) is far larger than the 126 MB L2",

@@ -56,8 +56,10 @@ typedef struct {
   int32_t edge_dims[8];    /* hidden widths; the final ->1 layer is implicit */
   double avg_num_neighbors; /* c_env = 1/sqrt(this)                  (S7) */
   double resid_alpha[8];    /* per layer residual mixing coefficient (S7) */
-  int32_t precision;        /* MLP GEMM arithmetic: 0 fp32 (FFMA), 1 TF32 tensor cores, 2 BF16 tensor
-                               cores; accumulation is fp32 in all modes */
+  int32_t precision;        /* MLP GEMM arithmetic (accumulation is fp32 in all modes):
+                               0 fp32 on the tensor cores (3xTF32 split operands, meets the fp32 tolerances),
+                               1 TF32 tensor cores (the paper's scheme), 2 reserved (BF16 operands),
+                               3 fp32 on the FFMA pipes (slowest, most accurate) */
   int64_t max_atoms, max_edges; /* capacity hints, 0 = grow on demand (+5 %) */
 } allegro_hparams;
 

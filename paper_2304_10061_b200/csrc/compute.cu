@@ -84,8 +84,8 @@ static GemmArgs mk(const float* A, int lda, const Dense& D, bool transposed_weig
   // transposed_weight = true : backward dX = dY W^T -> Bt = W  [fi][fo], N = fi, K = fo
   GemmArgs g{};
   g.A = A; g.lda = lda;
-  if (!transposed_weight) { g.Bt = D.Wt; g.Bt16 = D.Wth; g.ldb = D.fi; g.N = D.fo; g.K = D.fi; }
-  else { g.Bt = D.W; g.Bt16 = D.Wh; g.ldb = D.fo; g.N = D.fi; g.K = D.fo; }
+  if (!transposed_weight) { g.Bt = D.Wt; g.Bt16 = D.Wth; g.Bt_hi = D.Wt_hi; g.Bt_lo = D.Wt_lo; g.ldb = D.fi; g.N = D.fo; g.K = D.fi; }
+  else { g.Bt = D.W; g.Bt16 = D.Wh; g.Bt_hi = D.W_hi; g.Bt_lo = D.W_lo; g.ldb = D.fo; g.N = D.fi; g.K = D.fo; }
   g.C = C; g.ldc = ldc; g.m_cap = m_cap; g.m_ptr = m_ptr; g.epi = epi;
   return g;
 }

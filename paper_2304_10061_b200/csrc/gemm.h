@@ -27,6 +27,7 @@ struct GemmArgs {
   const float* A; int lda;
   const float* Bt; int ldb;       // fp32 weights [N][K]
   const void* Bt16;               // bf16 weights [N][K] (precision 2) or null
+  const float *Bt_hi, *Bt_lo;     // TF32-exact / remainder split of Bt (precision 0 on tensor cores) or null
   float* C; int ldc;
   int N, K;
   int m_cap; const int* m_ptr;

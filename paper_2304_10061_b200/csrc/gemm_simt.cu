@@ -1,5 +1,7 @@
 // fp32 FFMA GEMM with fused epilogues (precision mode 0: "F32" matmuls of PAPER.md Table IV, needed
 // for the 1e-5 force tolerance).  128x64x16 tiles, 256 threads, 8x4 outputs per thread, float4 I/O.
+#include <cstdlib>
+
 #include "gemm.h"
 #include "internal.h"
 
@@ -176,10 +178,19 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
 
 }  // namespace
 
-int al_gemm_tc_row_parts(int N);
+int al_gemm_tc3(allegro_model* m, const GemmArgs& g);  // gemm_tc.cu (tcgen05, 3xTF32 split operands)
+int al_gemm_tc_row_parts(int N, bool split);
+
+// precision 0 runs on the tensor cores as 3xTF32; precision 3 (or B200_ALLEGRO_FP32_SIMT with precision 0) runs
+// the plain FFMA kernel below
+static bool fp32_simt(const allegro_model* m) {
+  static const bool v = getenv("B200_ALLEGRO_FP32_SIMT") != nullptr;
+  return m->hp.precision == 3 || (m->hp.precision == 0 && v);
+}
 
 int al_gemm_row_parts(const allegro_model* m, int N) {
-  return (m->hp.precision >= 1) ? al_gemm_tc_row_parts(N) : (N + 31) / 32;
+  if (fp32_simt(m)) return (N + 31) / 32;
+  return al_gemm_tc_row_parts(N, m->hp.precision == 0);
 }
 
 int al_gemm(allegro_model* m, const GemmArgs& g) {
@@ -189,7 +200,7 @@ int al_gemm(allegro_model* m, const GemmArgs& g) {
     al_set_error(m, "gemm: dimensions must be multiples of 4");
     return ALLEGRO_ERR_BAD_HPARAMS;
   }
-  if (m->hp.precision >= 1) return al_gemm_tc(m, g);
+  if (!fp32_simt(m)) return (m->hp.precision == 0) ? al_gemm_tc3(m, g) : al_gemm_tc(m, g);
   dim3 grid((g.m_cap + BM - 1) / BM, (g.N + BN - 1) / BN);
   k_gemm_simt<<<grid, NT, 0, m->stream>>>(g);
   m->launches++;

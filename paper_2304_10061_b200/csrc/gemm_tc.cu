@@ -23,12 +23,17 @@ namespace {
 #define AUX2(i) ax2[(i) & 3]
 constexpr int BM = 128;          // UMMA M (cta_group::1)
 constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
-constexpr int BN_MAX = 256;
 constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
-constexpr uint32_t B_STAGE_BYTES = BN_MAX * BKF * 4;       // 32 KB (allocated for the largest BN)
+// SPLIT = 3xTF32 (precision 0 on tensor cores): every operand is carried as hi + lo, hi = rn_tf32(x),
+// lo = rn_tf32(x - hi), and  A*B ~= A_hi*B_hi + A_hi*B_lo + A_lo*B_hi  (the dropped lo*lo term and the rounding of
+// the lo parts are each <= 2^-24 relative: the same order as one fp32 rounding).  B_hi / B_lo are prepared at create time; four "splitter" warps turn each landed A
+// stage into A_hi (in place) and A_lo (second buffer) before the MMA warp may read it.
+__host__ __device__ constexpr int bn_max(bool split) { return split ? 128 : 256; }
+__host__ __device__ constexpr uint32_t b_stage_bytes(bool split) { return bn_max(split) * BKF * 4; }   // allocated for the largest BN
+__host__ __device__ constexpr uint32_t stage_bytes(bool split) { return split ? 2 * A_STAGE_BYTES + 2 * b_stage_bytes(true) : A_STAGE_BYTES + b_stage_bytes(false); }
 // epilogue transpose staging: one 32x32 fp32 tile per warp, float4-granular XOR swizzle (conflict-free both ways)
-constexpr uint32_t smem_bytes(int stages, int epi_warps) {
-  return stages * (A_STAGE_BYTES + B_STAGE_BYTES) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
+constexpr uint32_t smem_bytes(int stages, int epi_warps, bool split) {
+  return stages * stage_bytes(split) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -109,20 +114,32 @@ __device__ __forceinline__ float dsilu_f(float z) {
   return s * fmaf(z, 1.0f - s, 1.0f);
 }
 
-template <int STAGES, int EPI_WARPS>
-__global__ void __launch_bounds__(64 + 32 * EPI_WARPS, 1)
-k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, GemmArgs g, int BN, int ntn) {
+// round to the nearest TF32 value (10 explicit mantissa bits; ties away from zero), result exact in TF32 so the
+// MMA's own truncation of the operand is a no-op
+__device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u); }
+
+template <int STAGES, int EPI_WARPS, bool SPLIT>
+__global__ void __launch_bounds__(64 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
+k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+            const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
+  constexpr int BN_MAX = bn_max(SPLIT);
+  constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT), STAGE_BYTES = stage_bytes(SPLIT);
+  constexpr int EW0 = SPLIT ? 6 : 2;     // first epilogue warp (warps 2..5 are the splitter in SPLIT mode)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t* sA = smem;
-  uint8_t* sB = smem + STAGES * A_STAGE_BYTES;
-  uint64_t* bars = (uint64_t*)(smem + STAGES * (A_STAGE_BYTES + B_STAGE_BYTES));
-  uint64_t* full = bars;                 // [STAGES]
-  uint64_t* empty = bars + STAGES;       // [STAGES]
-  uint64_t* tfull = bars + 2 * STAGES;   // [2]
-  uint64_t* tempty = bars + 2 * STAGES + 2;   // [2]
-  uint32_t* tmem_slot = (uint32_t*)(bars + 2 * STAGES + 4);
-  float* stage_buf = (float*)(smem + STAGES * (A_STAGE_BYTES + B_STAGE_BYTES) + 256);
+  // stage s: [A | (A_lo) | B (B_hi) | (B_lo)]
+  auto sA = [&](int s) { return smem + s * STAGE_BYTES; };
+  auto sAlo = [&](int s) { return smem + s * STAGE_BYTES + A_STAGE_BYTES; };
+  auto sB = [&](int s) { return smem + s * STAGE_BYTES + (SPLIT ? 2 : 1) * A_STAGE_BYTES; };
+  auto sBlo = [&](int s) { return smem + s * STAGE_BYTES + 2 * A_STAGE_BYTES + B_STAGE_BYTES; };
+  uint64_t* bars = (uint64_t*)(smem + STAGES * STAGE_BYTES);
+  uint64_t* full = bars;                 // [STAGES]  TMA -> (splitter | MMA)
+  uint64_t* empty = bars + STAGES;       // [STAGES]  MMA -> TMA
+  uint64_t* ready = bars + 2 * STAGES;   // [STAGES]  splitter -> MMA (SPLIT only)
+  uint64_t* tfull = bars + 3 * STAGES;   // [2]
+  uint64_t* tempty = bars + 3 * STAGES + 2;   // [2]
+  uint32_t* tmem_slot = (uint32_t*)(bars + 3 * STAGES + 4);
+  float* stage_buf = (float*)(smem + STAGES * STAGE_BYTES + 256);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = *g.m_ptr;
@@ -131,7 +148,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   const int num_kb = (g.K + BKF - 1) / BKF;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); mbar_init(&ready[s], 4); }
     for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], EPI_WARPS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -148,14 +165,15 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // ===== TMA producer =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      const uint32_t bytes = A_STAGE_BYTES + (uint32_t)BN * BKF * 4;
+      const uint32_t bytes = A_STAGE_BYTES + (SPLIT ? 2u : 1u) * (uint32_t)BN * BKF * 4;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         int mt = tile / ntn, nt = tile - mt * ntn;
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&empty[stage], phase ^ 1);
           mbar_expect_tx(&full[stage], bytes);
-          tma_load_2d(sA + stage * A_STAGE_BYTES, &tmA, &full[stage], kb * BKF, mt * BM);
-          tma_load_2d(sB + stage * B_STAGE_BYTES, &tmB, &full[stage], kb * BKF, nt * BN);
+          tma_load_2d(sA(stage), &tmA, &full[stage], kb * BKF, mt * BM);
+          tma_load_2d(sB(stage), &tmB, &full[stage], kb * BKF, nt * BN);
+          if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &full[stage], kb * BKF, nt * BN);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
@@ -172,17 +190,49 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         tc_fence_after();
         uint32_t d_tmem = tmem_base + acc * BN_MAX;
         for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(&full[stage], phase);
+          mbar_wait(SPLIT ? &ready[stage] : &full[stage], phase);
           tc_fence_after();
-          uint64_t da = make_desc(smem_u32(sA + stage * A_STAGE_BYTES));
-          uint64_t db = make_desc(smem_u32(sB + stage * B_STAGE_BYTES));
+          uint64_t da = make_desc(smem_u32(sA(stage)));
+          uint64_t db = make_desc(smem_u32(sB(stage)));
 #pragma unroll
           for (int k = 0; k < BKF / 8; ++k)   // UMMA_K = 8 tf32 = 32 bytes -> +2 in the (addr >> 4) field
             tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+          if (SPLIT) {
+            uint64_t dal = make_desc(smem_u32(sAlo(stage)));
+            uint64_t dbl = make_desc(smem_u32(sBlo(stage)));
+#pragma unroll
+            for (int k = 0; k < BKF / 8; ++k) {
+              tc_mma_tf32(d_tmem, da + 2 * k, dbl + 2 * k, idesc, 1u);    // A_hi * B_lo
+              tc_mma_tf32(d_tmem, dal + 2 * k, db + 2 * k, idesc, 1u);    // A_lo * B_hi
+            }
+          }
           tc_commit(&empty[stage]);
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
         tc_commit(&tfull[acc]);
+      }
+    }
+  } else if (SPLIT && warp < EW0) {
+    // ===== splitter warps (3xTF32): A -> A_hi (in place, low 13 mantissa bits cleared) and A_lo = A - A_hi =====
+    const int t = threadIdx.x - 64;       // 0..127
+    int stage = 0; uint32_t phase = 0;
+    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int kb = 0; kb < num_kb; ++kb) {
+        mbar_wait(&full[stage], phase);
+        float4* pa = reinterpret_cast<float4*>(sA(stage));
+        float4* pl = reinterpret_cast<float4*>(sAlo(stage));
+#pragma unroll
+        for (int i = 0; i < (int)(A_STAGE_BYTES / 16) / 128; ++i) {
+          float4 v = pa[t + i * 128];
+          float4 h = make_float4(tf32_rn(v.x), tf32_rn(v.y), tf32_rn(v.z), tf32_rn(v.w));
+          pa[t + i * 128] = h;
+          pl[t + i * 128] = make_float4(tf32_rn(v.x - h.x), tf32_rn(v.y - h.y), tf32_rn(v.z - h.z), tf32_rn(v.w - h.w));
+        }
+        // generic-proxy writes -> visible to the async proxy (tcgen05.mma reads shared memory through it)
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&ready[stage]);
+        if (++stage == STAGES) { stage = 0; phase ^= 1; }
       }
     }
   } else {
@@ -197,8 +247,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       // Each 32-column chunk: TMEM -> registers (lane = row) -> padded smem -> registers in the
       // "coalesced domain" (8 lanes x float4 cover one row's 128 B, 4 rows per warp instruction), so
       // every global load/store of the epilogue touches 4 lines per instruction instead of 32.
-      float4* stg4 = reinterpret_cast<float4*>(stage_buf) + (warp - 2) * (32 * 8);
-      const int chunk0 = (warp - 2) >> 2;   // this warp takes chunks chunk0, chunk0 + EPI_WARPS/4, ...
+      float4* stg4 = reinterpret_cast<float4*>(stage_buf) + (warp - EW0) * (32 * 8);
+      const int chunk0 = (warp - EW0) >> 2;   // this warp takes chunks chunk0, chunk0 + EPI_WARPS/4, ...
       const int rsub = lane >> 3, c4 = (lane & 7) * 4;
       const int rbase = mt * BM + q * 32;
       for (int c0 = chunk0 * 32; c0 < BN; c0 += 32 * (EPI_WARPS / 4)) {
@@ -373,14 +423,16 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 EncodeTiledFn g_encode = nullptr;
 
-typedef std::tuple<const void*, long long, long long, long long, int> TmKey;   // ptr, rows, K, ld, box_rows
+typedef std::tuple<const void*, long long, long long, long long, int, int> TmKey;   // ptr, rows, K, ld, box_rows, exact
 std::map<TmKey, CUtensorMap>& tm_cache() {
   static thread_local std::map<TmKey, CUtensorMap> c;
   return c;
 }
 
-int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, long long ld, int box_rows, CUtensorMap* out) {
-  TmKey key(ptr, rows, K, ld, box_rows);
+// exact = true: plain fp32 load (the 3xTF32 path splits the operand itself); false: TFLOAT32 map, i.e. the load
+// rounds to nearest TF32 (the MMA alone would truncate: measured 2-3x larger error)
+int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, long long ld, int box_rows, bool exact, CUtensorMap* out) {
+  TmKey key(ptr, rows, K, ld, box_rows, exact ? 1 : 0);
   auto& c = tm_cache();
   auto it = c.find(key);
   if (it != c.end()) { *out = it->second; return ALLEGRO_OK; }
@@ -396,8 +448,7 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
   cuuint32_t box[2] = {(cuuint32_t)BKF, (cuuint32_t)box_rows};
   cuuint32_t estr[2] = {1, 1};
   CUtensorMap tm;
-  static const bool f32map = getenv("B200_ALLEGRO_TMAP_F32") != nullptr;   // experiment: plain fp32 load (MMA truncates)
-  CUresult r = g_encode(&tm, f32map ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_TFLOAT32, 2, const_cast<void*>(ptr), gdim, gstr, box, estr,
+  CUresult r = g_encode(&tm, exact ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_TFLOAT32, 2, const_cast<void*>(ptr), gdim, gstr, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { al_set_error(m, "cuTensorMapEncodeTiled failed, code " + std::to_string((int)r)); return ALLEGRO_ERR_CUDA; }
@@ -409,35 +460,58 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 
 }  // namespace
 
-int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
-  int ntn = (g.N + BN_MAX - 1) / BN_MAX;
-  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
-  CUtensorMap tmA, tmB;
-  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, &tmA));
-  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, &tmB));
-  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
-  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  static const int variant = getenv("B200_ALLEGRO_GEMM_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM_VARIANT")) : 0;   // 0: 16 epilogue warps (measured best), 1: 8, 2: 12
-#define GEMM_LAUNCH(ST, EW)                                                                                              \
+#define GEMM_LAUNCH(ST, EW, SP)                                                                                          \
   {                                                                                                                      \
     static bool attr_set = false;                                                                                        \
     if (!attr_set) {                                                                                                     \
-      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<ST, EW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(ST, EW))); \
+      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<ST, EW, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                                      (int)smem_bytes(ST, EW, SP)));                                                     \
       attr_set = true;                                                                                                   \
     }                                                                                                                    \
-    k_gemm_tf32<ST, EW><<<grid, 64 + 32 * EW, smem_bytes(ST, EW), m->stream>>>(tmA, tmB, g, BN, ntn);                     \
+    k_gemm_tf32<ST, EW, SP><<<grid, 64 + (SP ? 128 : 0) + 32 * EW, smem_bytes(ST, EW, SP), m->stream>>>(tmA, tmB, tmB2, g, BN, ntn); \
   }
-  if (variant == 0) GEMM_LAUNCH(3, 16)
-  else if (variant == 2) GEMM_LAUNCH(3, 12)
-  else GEMM_LAUNCH(3, 8)
-#undef GEMM_LAUNCH
+
+// precision 1: TF32 operands (rounded to nearest by the TMA load), fp32 accumulation
+int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
+  int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
+  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  CUtensorMap tmA, tmB, tmB2;
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, false, &tmA));
+  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, false, &tmB));
+  tmB2 = tmB;
+  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
+  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
+  static const int variant = getenv("B200_ALLEGRO_GEMM_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM_VARIANT")) : 0;   // 0: 16 epilogue warps (measured best), 1: 8, 2: 12
+  if (variant == 0) GEMM_LAUNCH(3, 16, false)
+  else if (variant == 2) GEMM_LAUNCH(3, 12, false)
+  else GEMM_LAUNCH(3, 8, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
 }
 
-int al_gemm_tc_row_parts(int N) {
-  int ntn = (N + BN_MAX - 1) / BN_MAX;
+// precision 0 on tensor cores: 3xTF32 split operands (fp32-level accuracy), tiles 128 x <=128
+int al_gemm_tc3(allegro_model* m, const GemmArgs& g) {
+  if (!g.Bt_hi || !g.Bt_lo) { al_set_error(m, "3xTF32 GEMM: split weights missing"); return ALLEGRO_ERR_BAD_ARG; }
+  int ntn = (g.N + bn_max(true) - 1) / bn_max(true);
+  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  CUtensorMap tmA, tmB, tmB2;
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, true, &tmA));
+  AL_CHECK(get_tmap(m, g.Bt_hi, g.N, g.K, g.ldb, BN, true, &tmB));
+  AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, true, &tmB2));
+  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
+  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
+  static const int variant = getenv("B200_ALLEGRO_GEMM3_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM3_VARIANT")) : 0;
+  if (variant == 0) GEMM_LAUNCH(3, 8, true)
+  else GEMM_LAUNCH(2, 16, true)
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
+}
+#undef GEMM_LAUNCH
+
+int al_gemm_tc_row_parts(int N, bool split) {
+  int ntn = (N + bn_max(split) - 1) / bn_max(split);
   int BN = ((N + ntn - 1) / ntn + 15) & ~15;
   return ntn * ((BN + 31) >> 5);
 }

@@ -71,6 +71,8 @@ struct Dense {
   float* Wt = nullptr;   // [fo][fi] row-major  (B operand of Y = X * W, K-major over fi)
   void* Wh = nullptr;    // bf16 copies for precision 2 (same two layouts), else null
   void* Wth = nullptr;
+  // precision 0 on tensor cores (3xTF32): W_hi = rn_tf32(W), W_lo = rn_tf32(W - W_hi); same two layouts
+  float *W_hi = nullptr, *W_lo = nullptr, *Wt_hi = nullptr, *Wt_lo = nullptr;
 };
 
 struct DevBuf {

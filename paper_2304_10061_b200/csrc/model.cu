@@ -63,7 +63,7 @@ static int check_hp(const allegro_hparams* hp) {
   for (int k = 0; k < hp->n_edge; ++k) if (hp->edge_dims[k] < 1) return bad("edge_dims");
   if (hp->latent_dims[hp->n_latent - 1] != hp->twobody_dims[hp->n_twobody - 1]) return bad("last latent width must equal d");
   if (!(hp->avg_num_neighbors > 0)) return bad("avg_num_neighbors");
-  if (hp->precision < 0 || hp->precision > 2) return bad("precision");
+  if (hp->precision < 0 || hp->precision > 3) return bad("precision");
   return ALLEGRO_OK;
 }
 
@@ -137,6 +137,21 @@ static int upload_dense(allegro_model* m, Dense& D, const std::vector<float>& W,
   if (m->hp.precision == 2) {
     AL_CHECK(al_upload_bf16(m, &D.Wh, W));
     AL_CHECK(al_upload_bf16(m, &D.Wth, Wt));
+  }
+  if (m->hp.precision == 0) {
+    auto split = [](const std::vector<float>& x, std::vector<float>& hi, std::vector<float>& lo) {
+      hi.resize(x.size()); lo.resize(x.size());
+      auto rn = [](float v) { uint32_t b; memcpy(&b, &v, 4); b = (b + 0x1000u) & 0xFFFFE000u; float r; memcpy(&r, &b, 4); return r; };
+      for (size_t k = 0; k < x.size(); ++k) {
+        hi[k] = rn(x[k]);
+        lo[k] = rn(x[k] - hi[k]);
+      }
+    };
+    std::vector<float> hi, lo;
+    split(W, hi, lo);
+    AL_CHECK(upload(m, &D.W_hi, hi)); AL_CHECK(upload(m, &D.W_lo, lo));
+    split(Wt, hi, lo);
+    AL_CHECK(upload(m, &D.Wt_hi, hi)); AL_CHECK(upload(m, &D.Wt_lo, lo));
   }
   return ALLEGRO_OK;
 }
