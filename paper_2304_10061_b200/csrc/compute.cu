@@ -48,7 +48,7 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     // u-bar partial slots: [0, P) EPI_LATENT_LAST, then P per fused prep stage (NL of them), then one accumulated by k_bwd_prep
     w.n_uparts = (w.n_eparts > 0) ? w.n_eparts * (NL + 1) + 1 : 1;
     AL_CHECK(R(w.ubar, (size_t)M * w.n_uparts)); AL_CHECK(R(w.epart, (size_t)2 * M * std::max(w.n_eparts, 1)));
-    AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * ((n + 31) / 32) * (NL + 1))); AL_CHECK(R(w.ge, (size_t)3 * M));
+    { int part0[AL_MAX_LAYERS + 1]; AL_CHECK(R(w.Ybar, (size_t)M * m->Denv * al_ybar_layout(m, part0))); } AL_CHECK(R(w.ge, (size_t)3 * M));
     w.cap_edges = M;
   }
   if (Nc > w.cap_centers) {
@@ -160,10 +160,10 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   // ---- step 11: backward -----------------------------------------------------------------------------------
   // u-bar partials: [0, n_eparts) stored by EPI_LATENT_LAST, the last one accumulated by k_bwd_prep
   AL_CUDA(m, cudaMemsetAsync((float*)w.ubar.p + (size_t)(w.n_uparts - 1) * w.cap_edges, 0, (size_t)m_cap * 4, st));
-  // Y-bar partials [group][slot 0..NL][M][Denv], summed in fixed order by k_edge_bwd.  The tp2 kernels store every
-  // partial; the fallback kernels accumulate into slot 0 of each group, so all partials are zeroed for them.
+  // Y-bar partials [part][M][Denv] (al_ybar_layout), summed in fixed order by k_edge_bwd.  The tp2/tp3 kernels
+  // store every partial; the fallback kernels accumulate into one part per 32-channel group, zeroed here.
   if (!tp2_eligible(m))
-    for (int gq = 0; gq < ((n + 31) / 32) * (NL + 1); ++gq)
+    for (int gq = 0; gq < (n + 31) / 32; ++gq)
       AL_CUDA(m, cudaMemsetAsync((float*)w.Ybar.p + (size_t)gq * w.cap_edges * m->Denv, 0, (size_t)m_cap * m->Denv * 4, st));
   float* xb = (float*)w.XB0.p; float* xb_o = (float*)w.XB1.p;
   float* vb = nullptr; float* vb_a = (float*)w.VB0.p; float* vb_b = (float*)w.VB1.p;

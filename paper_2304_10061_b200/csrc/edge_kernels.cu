@@ -709,9 +709,11 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
   size_t sm = (size_t)(m->NB + EB_EDGES) * (H + 4) * sizeof(float);
   static size_t sm_set = 0;
   if (sm > sm_set) { AL_CUDA(m, cudaFuncSetAttribute(k_edge_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); sm_set = sm; }
+  int ypart0[AL_MAX_LAYERS + 1];
+  const int n_yparts = al_ybar_layout(m, ypart0);
   k_edge_bwd<<<(unsigned)((m_cap + EB_EDGES - 1) / EB_EDGES), 256, sm, m->stream>>>(
       (int*)w.m_act.p, zb1, ldz, L0.W, m->S, m->NB, H, (float4*)w.geo.p, (float*)w.du.p, (float*)w.dB.p, (float*)w.ubar.p,
-      w.n_uparts, (int64_t)w.cap_edges, (float*)w.Ybar.p, ((m->n + 31) / 32) * (m->NL + 1), (int64_t)w.cap_edges * m->Denv,
+      w.n_uparts, (int64_t)w.cap_edges, (float*)w.Ybar.p, n_yparts, (int64_t)w.cap_edges * m->Denv,
       m->Denv, m->lmax, (int*)w.ei.p, (int*)w.ej.p, (float*)w.ge.p, force);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;

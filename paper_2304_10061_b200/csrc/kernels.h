@@ -43,6 +43,9 @@ struct EdgeGeomArgs {
 };
 
 bool tp2_eligible(const allegro_model* m);   // tp2_kernels.cu
+// Y-bar partial buffers: part0[0] = first part of the V^0 contribution, part0[L] = first part of layer L's
+// environment contribution (one part per channel group of the kernel that writes it); returns the total count.
+int al_ybar_layout(const allegro_model* m, int* part0);
 int k_launch_active_count(allegro_model* m, const EdgeGeomArgs& a, int* deg);
 int k_launch_set_mact(allegro_model* m, const int64_t* rowa, int nc, int* m_act);
 int k_launch_geom_fill(allegro_model* m, const EdgeGeomArgs& a, const int64_t* rowa, Work& w);

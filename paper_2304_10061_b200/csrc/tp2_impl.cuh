@@ -57,7 +57,9 @@ struct TP2 {
   float* Tout; float* xs; int ldx; float* gamma_out;
   const float* VbarL; const float* sbar; int lds;
   float* Vbar_prev; float* ombar; int ldob; float* w0bar;
-  float* Ybar; int64_t ybar_pstride; int ybar_slots, ybar_slot;   // Y-bar partials [group][slot][M][DENV], plain stores
+  // Y-bar partials [part][M][DENV], plain stores: part = ybar_part0 + group for the V^0 contribution (FIRST, pass 1),
+  // ybar_partL + group for this layer's environment contribution (pass 2); see al_ybar_layout()
+  float* Ybar; int64_t ybar_pstride; int ybar_part0, ybar_partL;
   float kv[NNZ];   // values of the fused tensor K in pattern order (dense pair table order)
 };
 
@@ -234,9 +236,8 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
   const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
   const int deg = (int)(e1 - e0);
   if (deg <= 0) return;
-  // slot 0 of the group: V^0 part (FIRST); slot L: environment part of layer L
-  float* Yb0 = a.Ybar + (size_t)grp * a.ybar_slots * a.ybar_pstride;
-  float* YbL = Yb0 + (size_t)a.ybar_slot * a.ybar_pstride;
+  float* Yb0 = a.Ybar + (size_t)(a.ybar_part0 + grp) * a.ybar_pstride;
+  float* YbL = a.Ybar + (size_t)(a.ybar_partL + grp) * a.ybar_pstride;
 
   // per-center base pointers and hoisted per-lane chunk offsets: the edge loop only adds il * stride
   constexpr int OPROWS = FIRST ? NLV : AB;
@@ -489,7 +490,7 @@ int fill2(allegro_model* m, const TP2Common& q, TP2<NNZ>& a) {
   a.Tout = q.Tout; a.xs = q.xs; a.ldx = q.ldx; a.gamma_out = (float*)w.gamma.p;
   a.VbarL = q.VbarL; a.sbar = q.sbar; a.lds = q.lds; a.Vbar_prev = q.Vbar_prev; a.ombar = q.ombar; a.ldob = q.ldob;
   a.w0bar = q.w0bar; a.Ybar = (float*)w.Ybar.p; a.ybar_pstride = (int64_t)w.cap_edges * m->Denv;
-  a.ybar_slots = m->NL + 1; a.ybar_slot = q.L;
+  { int part[AL_MAX_LAYERS + 1]; al_ybar_layout(m, part); a.ybar_part0 = part[0]; a.ybar_partL = part[q.L]; }
   memcpy(a.kv, h.dp_val.data(), sizeof(float) * NNZ);
   return ALLEGRO_OK;
 }

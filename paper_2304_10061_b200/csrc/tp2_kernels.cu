@@ -68,6 +68,24 @@ bool tp2_eligible(const allegro_model* m) {
   return true;
 }
 
+// channel groups of the kernel that runs layer L's backward: 8-channel warps for the lane-split l_max = 3 kernels
+// (tp3_impl.cuh), 32-channel warps otherwise
+static int bwd_groups(const allegro_model* m, int L) {
+  int p = match_pattern(m->tp_host[L - 1]);
+  return (p == P_16_16_31 || p == P_16_31_16) ? m->n / 8 : m->n / 32;
+}
+
+int al_ybar_layout(const allegro_model* m, int* part0) {
+  if (!tp2_eligible(m)) {   // fallback kernels accumulate into one part per 32-channel group
+    for (int L = 0; L <= m->NL; ++L) part0[L] = 0;
+    return (m->n + 31) / 32;
+  }
+  int tot = 0;
+  part0[0] = tot; tot += bwd_groups(m, 1);
+  for (int L = 1; L <= m->NL; ++L) { part0[L] = tot; tot += bwd_groups(m, L); }
+  return tot;
+}
+
 #define FILL(P)                                \
   TP2<Pat<P>::NNZ> a{};                        \
   { int rc = fill2(m, q, a); if (rc) return rc; }

@@ -1,9 +1,10 @@
-// l_max = 3 backward instantiations of the second-generation tensor-track kernels (tp2_impl.cuh).
-#include "tp2_impl.cuh"
+// l_max = 3 backward instantiations: lane-split kernels (tp3_impl.cuh) for the wide layers, the 32-channel
+// kernel of tp2_impl.cuh for the scalar-output last layer.
+#include "tp3_impl.cuh"
 
 int tp2_l3_bwd(allegro_model* m, const TP2Common& q, int pat) {
-  if (pat == P_16_16_31) { TP2<Pat<P_16_16_31>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd2<P_16_16_31, 4, true, true, false, 2, 2>(m, a); }
-  if (pat == P_16_31_16) { TP2<Pat<P_16_31_16>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd2<P_16_31_16, 8, false, true, false, 2, 2>(m, a); }
+  if (pat == P_16_16_31) { TP2<Pat<P_16_16_31>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd3<P_16_16_31, true, 4, 4>(m, a); }
+  if (pat == P_16_31_16) { TP2<Pat<P_16_31_16>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd3<P_16_31_16, false, 4, 4>(m, a); }
   if (pat == P_16_16_1) { TP2<Pat<P_16_16_1>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_bwd2<P_16_16_1, 16, false, false, true, 2, 4>(m, a); }
   return ALLEGRO_ERR_UNIMPLEMENTED;
 }

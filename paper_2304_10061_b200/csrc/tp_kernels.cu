@@ -605,7 +605,7 @@ int tpw_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   TPW a{};
   fill(m, w, L, nc, a, om, ldo, Vin, w0, ldw);
   a.VbarL = VbarL; a.sbar = sbar; a.lds = lds; a.Vbar_prev = Vbar_prev; a.ombar = ombar; a.ldob = ldob; a.w0bar = w0bar;
-  a.Ybar = (float*)w.Ybar.p; a.ybar_gstride = (int64_t)(m->NL + 1) * w.cap_edges * m->Denv;   // slot 0 of each group
+  a.Ybar = (float*)w.Ybar.p; a.ybar_gstride = (int64_t)w.cap_edges * m->Denv;   // one part per 32-channel group
   const int DENV = m->Denv, Din = a.t.Din, Dout = a.t.Dout;
   if (Vin == nullptr) { TPW_DISPATCH(launch_bwd, true) } else { TPW_DISPATCH(launch_bwd, false) }
   if (DENV == 16) {
