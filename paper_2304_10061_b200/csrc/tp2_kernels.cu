@@ -1,7 +1,7 @@
 // Dispatch of the second-generation tensor-track kernels (tp2_impl.cuh) for l_max <= 2, and the
 // eligibility test.  The l_max = 3 instantiations live in tp2_l3_fwd.cu / tp2_l3_bwd.cu (separate
 // translation units: they dominate the compile time).
-#include "tp2_impl.cuh"
+#include "tp3_impl.cuh"
 
 int tp2_l3_fwd(allegro_model* m, const TP2Common& q, int pat);
 int tp2_l3_bwd(allegro_model* m, const TP2Common& q, int pat);
@@ -72,7 +72,8 @@ bool tp2_eligible(const allegro_model* m) {
 // (tp3_impl.cuh), 32-channel warps otherwise
 static int bwd_groups(const allegro_model* m, int L) {
   int p = match_pattern(m->tp_host[L - 1]);
-  return (p == P_16_16_31 || p == P_16_31_16) ? m->n / 8 : m->n / 32;
+  const int lq = t3_bwd_lq();
+  return ((p == P_16_16_31 || p == P_16_31_16) && lq) ? m->n / (32 >> lq) : m->n / 32;
 }
 
 int al_ybar_layout(const allegro_model* m, int* part0) {

@@ -14,7 +14,15 @@
 #pragma once
 #include "tp2_impl.cuh"
 
-constexpr int T3_CPW = 8;   // channels per warp
+constexpr int T3_CPW = 8;      // channels per warp of the forward kernels (4 blocks)
+// Backward: the lane-split kernel below exists for 2^LQ = 4 and 8 blocks per warp, but neither beat the blocked
+// 32-channel kernel of tp2_impl.cuh on config 4 (84 ms per step): LQ = 2 keeps the M block in shared memory and
+// is LDS-bound (88 ms, ncu l1tex 70 %), LQ = 3 holds M and M-bar in registers but moves 16-byte rows (124 ms).
+// B200_ALLEGRO_TP3_BWD = 2 | 3 selects them for experiments; the default (0) is the tp2 kernel.
+inline int t3_bwd_lq() {
+  static const int v = getenv("B200_ALLEGRO_TP3_BWD") ? atoi(getenv("B200_ALLEGRO_TP3_BWD")) : 0;
+  return (v == 2 || v == 3) ? v : 0;
+}
 
 // ROWS rows of 8 floats (32 B): smem dst row r at dst + 8 r, global row r at src + r * rstride
 template <int ROWS>
@@ -148,92 +156,147 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_fwd(const __grid_consta
   }
 }
 
-// sum over the 8 channel lanes (xor 1, 2, 4): every lane of the q-group ends with the total
-__device__ __forceinline__ float t3_sum_ch(float v) {
-  v += __shfl_xor_sync(TP_FULLMASK, v, 1);
-  v += __shfl_xor_sync(TP_FULLMASK, v, 2);
-  v += __shfl_xor_sync(TP_FULLMASK, v, 4);
+// ======================================================================================================
+// backward:  NBK = 2^LQ blocks per warp, CPW = 32 / NBK channels; lane (ch, q) owns input components
+// [q AB, (q+1) AB): V-bar rows, M / M-bar blocks (both in registers for LQ = 3, M in shared memory for LQ = 2)
+// and environment components [q GB, (q+1) GB) in the Gamma pass and in pass 2.
+// ======================================================================================================
+template <int CPW>
+__device__ __forceinline__ float t3_sum_ch(float v) {   // sum over the CPW channel lanes of a block
+#pragma unroll
+  for (int o = 1; o < CPW; o <<= 1) v += __shfl_xor_sync(TP_FULLMASK, v, o);
   return v;
 }
-
-// Per-l sums from the (first, rest) split of the four component groups: group q contributes xa to l(4q) and xb
-// to l(4q+1), i.e. l=0: a(0); l=1: b(0); l=2: a(1)+b(1)+a(2); l=3: b(2)+a(3)+b(3).  Lane (ch, q) returns l = q.
-__device__ __forceinline__ float t3_gather_l(float xa, float xb, int ch, int q) {
-  float a0 = __shfl_sync(TP_FULLMASK, xa, ch), b0 = __shfl_sync(TP_FULLMASK, xb, ch);
-  float a1 = __shfl_sync(TP_FULLMASK, xa, ch + 8), b1 = __shfl_sync(TP_FULLMASK, xb, ch + 8);
-  float a2 = __shfl_sync(TP_FULLMASK, xa, ch + 16), b2 = __shfl_sync(TP_FULLMASK, xb, ch + 16);
-  float a3 = __shfl_sync(TP_FULLMASK, xa, ch + 24), b3 = __shfl_sync(TP_FULLMASK, xb, ch + 24);
-  return q == 0 ? a0 : q == 1 ? b0 : q == 2 ? (a1 + b1) + a2 : (b2 + a3) + b3;
+// xa belongs to l = lA, xb to l = lB (of this lane's environment components); returns, in the lane with q = l,
+// the sum over the blocks of everything that belongs to l (fixed order: xor tree over the block bits)
+template <int CPW>
+__device__ __forceinline__ float t3_gather_l(float xa, float xb, int lA, int lB, int q) {
+  float c[4];
+#pragma unroll
+  for (int l = 0; l < 4; ++l) c[l] = ((lA == l) ? xa : 0.f) + ((lB == l) ? xb : 0.f);
+#pragma unroll
+  for (int o = CPW; o < 32; o <<= 1)
+#pragma unroll
+    for (int l = 0; l < 4; ++l) c[l] += __shfl_xor_sync(TP_FULLMASK, c[l], o);
+  return q == 0 ? c[0] : q == 1 ? c[1] : q == 2 ? c[2] : c[3];
 }
 
-// ======================================================================================================
-// backward:  lane (ch, q) owns input components [q AB, (q+1) AB): V-bar rows, M / M-bar blocks
-// ======================================================================================================
-template <int P, bool FIRST, int NST, int WPB>
+// rows of CPW floats: smem dst row r at dst + CPW r
+template <int ROWS, int CPW>
+__device__ __forceinline__ void t3_cp_rows_w(float* dst, const float* src, int rstride, int lane) {
+  constexpr int CPR = CPW / 4;   // 16-byte chunks per row
+#pragma unroll
+  for (int i0 = 0; i0 < ROWS * CPR; i0 += 32) {
+    int i = i0 + lane;
+    if (i < ROWS * CPR) tp_cp16(dst + i * 4, src + (i / CPR) * rstride + (i % CPR) * 4);
+  }
+}
+
+template <int P, bool FIRST, int LQ, int NST, int WPB>
 static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_constant__ TP2<Pat<P>::NNZ> a) {
   constexpr int DENV = Pat<P>::DENV, DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
   static_assert(DENV == 16, "lane-split kernels are written for l_max = 3");
   static_assert(!FIRST || DIN == 16, "FIRST: V^0 has the environment layout");
-  constexpr int AB = (DIN + 3) / 4, CH = (DOUT + 1) / 2;
-  constexpr int SV = FIRST ? 4 * 8 + 16 : DIN * 8;          // operand part of a stage
-  constexpr int SF = SV + DOUT * 8 + 8;                      // + V-bar^L rows + s-bar row
-  constexpr int MSL = AB * CH * 64;                          // M block, float2 per lane
-  constexpr int WSL = DENV * 8 + MSL + NST * SF;
+  constexpr int NBK = 1 << LQ, CPW = 32 / NBK, GB = DENV / NBK;
+  constexpr bool MREG = (LQ == 3);
+  constexpr int AB = (DIN + NBK - 1) / NBK, CH = (DOUT + 1) / 2;
+  static_assert(!FIRST || AB == GB, "FIRST: input blocks coincide with the environment component groups");
+  constexpr int SV = FIRST ? 4 * CPW + 16 : DIN * CPW;       // operand part of a stage
+  constexpr int SF = SV + DOUT * CPW + CPW;                   // + V-bar^L rows + s-bar row
+  constexpr int MSL = MREG ? 0 : AB * CH * 64;                // M block, float2 per lane
+  constexpr int WSL = DENV * CPW + MSL + NST * SF;
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
-  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, ch = lane & 7, q = lane >> 3;
-  const int ngroups = a.n / T3_CPW;
+  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, ch = lane & (CPW - 1), q = lane / CPW;
+  const int ngroups = a.n / CPW;
   const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * ngroups) return;
   const int c = (int)(wg / ngroups), grp = (int)(wg - (int64_t)c * ngroups);
-  const int nn = grp * T3_CPW + ch;
+  const int nn = grp * CPW + ch;
   float* Gs = smem + wib * WSL;
-  float2* Ms = reinterpret_cast<float2*>(Gs + DENV * 8);
-  float* ring = Gs + DENV * 8 + MSL;
+  float2* Ms = reinterpret_cast<float2*>(Gs + DENV * CPW);
+  float* ring = Gs + DENV * CPW + MSL;
   const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
   const int deg = (int)(e1 - e0);
   if (deg <= 0) return;
   float* Yb0 = a.Ybar + (size_t)(a.ybar_part0 + grp) * a.ybar_pstride;
   float* YbL = a.Ybar + (size_t)(a.ybar_partL + grp) * a.ybar_pstride;
+  const int lA = l_of(GB * q), lB = l_of(GB * q + 1);
 
-  const float* opc = FIRST ? a.w0 + e0 * a.ldw + grp * T3_CPW : a.Vin + e0 * DIN * a.n + grp * T3_CPW;
+  const float* opc = FIRST ? a.w0 + e0 * a.ldw + grp * CPW : a.Vin + e0 * DIN * a.n + grp * CPW;
   const int op_stride = FIRST ? a.ldw : DIN * a.n;
   const float* Yc = a.Y + e0 * a.ldy + lane * 4;
-  const float* vbc = a.VbarL + e0 * DOUT * a.n + grp * T3_CPW;
-  const float* sbc = a.sbar + e0 * a.lds + grp * T3_CPW + (lane & 1) * 4;
+  const float* vbc = a.VbarL + e0 * DOUT * a.n + grp * CPW;
+  const float* sbc = a.sbar + e0 * a.lds + grp * CPW + lane * 4;
   auto issue = [&](int il, float* st) {
     if (FIRST) {
-      t3_cp_rows<4>(st, opc + il * op_stride, a.n, lane);
-      if (lane < 4) tp_cp16(st + 32 + lane * 4, Yc + il * a.ldy);
+      t3_cp_rows_w<4, CPW>(st, opc + il * op_stride, a.n, lane);
+      if (lane < 4) tp_cp16(st + 4 * CPW + lane * 4, Yc + il * a.ldy);
     } else {
-      t3_cp_rows<DIN>(st, opc + il * op_stride, a.n, lane);
+      t3_cp_rows_w<DIN, CPW>(st, opc + il * op_stride, a.n, lane);
     }
-    t3_cp_rows<DOUT>(st + SV, vbc + il * (DOUT * a.n), a.n, lane);
-    if (lane < 2) tp_cp16(st + SF - 8 + lane * 4, sbc + il * a.lds);
+    t3_cp_rows_w<DOUT, CPW>(st + SV, vbc + il * (DOUT * a.n), a.n, lane);
+    if (lane < CPW / 4) tp_cp16(st + SF - CPW + lane * 4, sbc + il * a.lds);
   };
 #pragma unroll
   for (int s = 0; s < NST - 1; ++s) {
     if (s < deg) issue(s, ring + s * SF);
     tp_cp_commit();
   }
-  t3_gamma(a, e0, e1, nn, q, ch, Gs);
+  // Gamma_i: lane (ch, q) sums its GB environment components -> Gs[b * CPW + ch]
+  {
+    float g[GB];
+#pragma unroll
+    for (int j = 0; j < GB; ++j) g[j] = 0.f;
+    for (int64_t e = e0; e < e1; e += 4) {
+      float oa[4], ob[4], y[4][GB];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
+        oa[i] = a.om[ee * a.ldo + lA * a.n + nn];
+        ob[i] = a.om[ee * a.ldo + lB * a.n + nn];
+#pragma unroll
+        for (int j = 0; j < GB; ++j) y[i][j] = __ldg(a.Y + ee * a.ldy + GB * q + j);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        if (e + i < e1) {
+          g[0] = fmaf(oa[i], y[i][0], g[0]);
+#pragma unroll
+          for (int j = 1; j < GB; ++j) g[j] = fmaf(ob[i], y[i][j], g[j]);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < GB; ++j) Gs[(GB * q + j) * CPW + ch] = a.c_env * g[j];
+    __syncwarp();
+  }
 
-  // M block of this lane (rows q AB + r) -> the lane's shared slice, one row at a time
+  // M block of this lane (rows q AB + r): entries of block blk are FFMAs predicated on q == blk
+  float2 Mr[MREG ? AB * CH : 1];
   {
     float G[DENV];
 #pragma unroll
-    for (int b = 0; b < DENV; ++b) G[b] = Gs[b * 8 + ch];
+    for (int b = 0; b < DENV; ++b) G[b] = Gs[b * CPW + ch];
+    if constexpr (MREG) {
 #pragma unroll
-    for (int r = 0; r < AB; ++r) {
-      float2 row[CH];
-#pragma unroll
-      for (int j = 0; j < CH; ++j) row[j] = make_float2(0.f, 0.f);
+      for (int k = 0; k < AB * CH; ++k) Mr[k] = make_float2(0.f, 0.f);
 #define X(k, a_, b_, c_) \
-  if ((a_) % AB == r) { if (q == (a_) / AB) TP2_REF(row, CH, 0, c_) = fmaf(a.kv[k], G[b_], TP2_REF(row, CH, 0, c_)); }
+  if (q == (a_) / AB) TP2_REF(Mr, CH, (a_) % AB, c_) = fmaf(a.kv[k], G[b_], TP2_REF(Mr, CH, (a_) % AB, c_));
       TP2_EXPAND(P, X)
 #undef X
+    } else {
 #pragma unroll
-      for (int j = 0; j < CH; ++j) Ms[(r * CH + j) * 32 + lane] = row[j];
+      for (int r = 0; r < AB; ++r) {
+        float2 row[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) row[j] = make_float2(0.f, 0.f);
+#define X(k, a_, b_, c_) \
+  if ((a_) % AB == r) { if (q == (a_) / AB) TP2_REF(row, CH, 0, c_) = fmaf(a.kv[k], G[b_], TP2_REF(row, CH, 0, c_)); }
+        TP2_EXPAND(P, X)
+#undef X
+#pragma unroll
+        for (int j = 0; j < CH; ++j) Ms[(r * CH + j) * 32 + lane] = row[j];
+      }
     }
   }
   float2 Mb[AB * CH];
@@ -243,8 +306,8 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_consta
   // FIRST: shared-memory offsets of w0[l(ab + k)] for this lane's components
   int wrow[AB];
 #pragma unroll
-  for (int k = 0; k < AB; ++k) wrow[k] = l_of((ab + k < DIN) ? ab + k : DIN - 1) * 8 + ch;
-  float* yb0p = Yb0 + e0 * DENV + 4 * q;
+  for (int k = 0; k < AB; ++k) wrow[k] = l_of((ab + k < DIN) ? ab + k : DIN - 1) * CPW + ch;
+  float* yb0p = Yb0 + e0 * DENV + GB * q;
   float* outp = FIRST ? a.w0bar + e0 * a.ldob + q * a.n + nn : a.Vbar_prev + (e0 * DIN + ab) * a.n + nn;
   int slot = 0;
   for (int i = 0; i < deg; ++i) {
@@ -260,39 +323,47 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_consta
     float2 t2[CH];
 #pragma unroll
     for (int j = 0; j < CH; ++j) {
-      t2[j].x = st[SV + (2 * j) * 8 + ch];
-      t2[j].y = (2 * j + 1 < DOUT) ? st[SV + (2 * j + 1) * 8 + ch] : 0.f;
+      t2[j].x = st[SV + (2 * j) * CPW + ch];
+      t2[j].y = (2 * j + 1 < DOUT) ? st[SV + (2 * j + 1) * CPW + ch] : 0.f;
     }
-    t2[0].x += st[SF - 8 + ch];
+    t2[0].x += st[SF - CPW + ch];
     float vb[AB], y[AB], wl[AB];
 #pragma unroll
     for (int k = 0; k < AB; ++k) {
       const bool valid = ab + k < DIN;
       float v;
       if (FIRST) {
-        y[k] = st[32 + ab + k];
+        y[k] = st[4 * CPW + ab + k];
         wl[k] = st[wrow[k]];
         v = wl[k] * y[k];
       } else {
-        v = valid ? st[(ab + k) * 8 + ch] : 0.f;
+        v = valid ? st[(ab + k) * CPW + ch] : 0.f;
       }
       const float2 v2 = make_float2(v, v);
       float2 s2 = make_float2(0.f, 0.f);
 #pragma unroll
       for (int j = 0; j < CH; ++j) {
-        const float2 m2 = Ms[(k * CH + j) * 32 + lane];
+        float2 m2;
+        if constexpr (MREG) m2 = Mr[k * CH + j]; else m2 = Ms[(k * CH + j) * 32 + lane];
         s2 = tp_fma2(m2, t2[j], s2);
         Mb[k * CH + j] = tp_fma2(v2, t2[j], Mb[k * CH + j]);
       }
       vb[k] = s2.x + s2.y;
     }
     if (FIRST) {
-      // w0-bar[l] = sum_{a in l} V-bar^0[a] Y[a];  Y-bar[a] (V^0 part) = sum_n w0[l(a)] V-bar^0[a]   (AB == 4)
-      const float xa = vb[0] * y[0], xb = fmaf(vb[1], y[1], fmaf(vb[2], y[2], vb[3] * y[3]));
-      *outp = t3_gather_l(xa, xb, ch, q);
+      // w0-bar[l] = sum_{a in l} V-bar^0[a] Y[a];  Y-bar[a] (V^0 part) = sum_n w0[l(a)] V-bar^0[a]   (AB == GB)
+      float xa = vb[0] * y[0], xb = 0.f;
+#pragma unroll
+      for (int k = 1; k < AB; ++k) xb = fmaf(vb[k], y[k], xb);
+      const float wsum = t3_gather_l<CPW>(xa, xb, lA, lB, q);
+      if (q < 4) *outp = wsum;
       outp += a.ldob;
-      float4 p4 = make_float4(t3_sum_ch(wl[0] * vb[0]), t3_sum_ch(wl[1] * vb[1]), t3_sum_ch(wl[2] * vb[2]), t3_sum_ch(wl[3] * vb[3]));
-      if (ch == 0) *reinterpret_cast<float4*>(yb0p) = p4;
+      float pj[AB];
+#pragma unroll
+      for (int k = 0; k < AB; ++k) pj[k] = t3_sum_ch<CPW>(wl[k] * vb[k]);
+      if (ch == 0)
+#pragma unroll
+        for (int k = 0; k < AB; ++k) yb0p[k] = pj[k];
       yb0p += DENV;
     } else {
 #pragma unroll
@@ -302,7 +373,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_consta
     }
     if (++slot == NST) slot = 0;
   }
-  // Gamma-bar = K . M-bar: this lane's block, then the sum over the four blocks of the channel
+  // Gamma-bar = K . M-bar: this lane's block, then the sum over the blocks of the channel
   float Gb[DENV];
 #pragma unroll
   for (int b = 0; b < DENV; ++b) Gb[b] = 0.f;
@@ -311,37 +382,43 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_consta
   TP2_EXPAND(P, X)
 #undef X
 #pragma unroll
-  for (int b = 0; b < DENV; ++b) {
-    Gb[b] += __shfl_xor_sync(TP_FULLMASK, Gb[b], 8);
-    Gb[b] += __shfl_xor_sync(TP_FULLMASK, Gb[b], 16);
-  }
-  // pass 2: lane (ch, q) takes environment components [4q, 4q+4): omega-bar_e[l], Y-bar_e[b] (environment part)
-  float gq[4];
+  for (int b = 0; b < DENV; ++b)
 #pragma unroll
-  for (int j = 0; j < 4; ++j) {
+    for (int o = CPW; o < 32; o <<= 1) Gb[b] += __shfl_xor_sync(TP_FULLMASK, Gb[b], o);
+  // pass 2: lane (ch, q) takes environment components [q GB, (q+1) GB): omega-bar_e[l], Y-bar_e[b] (environment part)
+  float gq[GB];
+#pragma unroll
+  for (int j = 0; j < GB; ++j) {
     float v = Gb[j];
 #pragma unroll
-    for (int qq = 1; qq < 4; ++qq) v = (q == qq) ? Gb[4 * qq + j] : v;
+    for (int qq = 1; qq < NBK; ++qq) v = (q == qq) ? Gb[GB * qq + j] : v;
     gq[j] = a.c_env * v;
   }
-  const int lA = l_of(4 * q), lB = l_of(4 * q + 1);
   for (int64_t e = e0; e < e1; e += 2) {
-    float oa[2], ob[2];
-    float4 y[2];
+    float oa[2], ob[2], y[2][GB];
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
       const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
       oa[i] = a.om[ee * a.ldo + lA * a.n + nn];
       ob[i] = a.om[ee * a.ldo + lB * a.n + nn];
-      y[i] = __ldg(reinterpret_cast<const float4*>(a.Y + ee * a.ldy + 4 * q));
+#pragma unroll
+      for (int j = 0; j < GB; ++j) y[i][j] = __ldg(a.Y + ee * a.ldy + GB * q + j);
     }
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
       if (e + i < e1) {   // (warp-uniform)
-        const float xa = gq[0] * y[i].x, xb = fmaf(gq[1], y[i].y, fmaf(gq[2], y[i].z, gq[3] * y[i].w));
-        a.ombar[(e + i) * a.ldob + q * a.n + nn] = t3_gather_l(xa, xb, ch, q);
-        float4 p4 = make_float4(t3_sum_ch(oa[i] * gq[0]), t3_sum_ch(ob[i] * gq[1]), t3_sum_ch(ob[i] * gq[2]), t3_sum_ch(ob[i] * gq[3]));
-        if (ch == 0) *reinterpret_cast<float4*>(YbL + (e + i) * DENV + 4 * q) = p4;
+        float xa = gq[0] * y[i][0], xb = 0.f;
+#pragma unroll
+        for (int j = 1; j < GB; ++j) xb = fmaf(gq[j], y[i][j], xb);
+        const float osum = t3_gather_l<CPW>(xa, xb, lA, lB, q);
+        if (q < 4) a.ombar[(e + i) * a.ldob + q * a.n + nn] = osum;
+        float pj[GB];
+        pj[0] = t3_sum_ch<CPW>(oa[i] * gq[0]);
+#pragma unroll
+        for (int j = 1; j < GB; ++j) pj[j] = t3_sum_ch<CPW>(ob[i] * gq[j]);
+        if (ch == 0)
+#pragma unroll
+          for (int j = 0; j < GB; ++j) YbL[(e + i) * DENV + GB * q + j] = pj[j];
       }
     }
   }
@@ -363,18 +440,19 @@ int launch_fwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   return ALLEGRO_OK;
 }
 
-template <int P, bool FIRST, int NST, int WPB>
+template <int P, bool FIRST, int LQ, int NST, int WPB>
 int launch_bwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
-  constexpr int AB = (DIN + 3) / 4, CH = (DOUT + 1) / 2;
-  constexpr int SV = FIRST ? 4 * 8 + 16 : DIN * 8;
-  constexpr int SF = SV + DOUT * 8 + 8;
-  constexpr int WSL = 16 * 8 + AB * CH * 64 + NST * SF;
+  constexpr int NBK = 1 << LQ, CPW = 32 / NBK;
+  constexpr int AB = (DIN + NBK - 1) / NBK, CH = (DOUT + 1) / 2;
+  constexpr int SV = FIRST ? 4 * CPW + 16 : DIN * CPW;
+  constexpr int SF = SV + DOUT * CPW + CPW;
+  constexpr int WSL = 16 * CPW + (LQ == 3 ? 0 : AB * CH * 64) + NST * SF;
   size_t sm = (size_t)WPB * WSL * 4 + 16;
   static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_bwd<P, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
-  int64_t warps = (int64_t)a.nc * (a.n / T3_CPW);
-  k_tp3_bwd<P, FIRST, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
+  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_bwd<P, FIRST, LQ, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  int64_t warps = (int64_t)a.nc * (a.n / CPW);
+  k_tp3_bwd<P, FIRST, LQ, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
