@@ -30,10 +30,11 @@ constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
 // stage into A_hi (in place) and A_lo (second buffer) before the MMA warp may read it.
 __host__ __device__ constexpr int bn_max(bool split) { return split ? 128 : 256; }
 __host__ __device__ constexpr uint32_t b_stage_bytes(bool split) { return bn_max(split) * BKF * 4; }   // allocated for the largest BN
-__host__ __device__ constexpr uint32_t stage_bytes(bool split) { return split ? 2 * A_STAGE_BYTES + 2 * b_stage_bytes(true) : A_STAGE_BYTES + b_stage_bytes(false); }
+__host__ __device__ constexpr uint32_t a_ring_stage(bool split) { return (split ? 2 : 1) * A_STAGE_BYTES; }
+__host__ __device__ constexpr uint32_t b_ring_stage(bool split) { return (split ? 2 : 1) * b_stage_bytes(split); }
 // epilogue transpose staging: one 32x32 fp32 tile per warp, float4-granular XOR swizzle (conflict-free both ways)
-constexpr uint32_t smem_bytes(int stages, int epi_warps, bool split) {
-  return stages * stage_bytes(split) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
+constexpr uint32_t smem_bytes(int ast, int bst, int epi_warps, bool split) {
+  return ast * a_ring_stage(split) + bst * b_ring_stage(split) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -118,28 +119,34 @@ __device__ __forceinline__ float dsilu_f(float z) {
 // MMA's own truncation of the operand is a no-op
 __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u); }
 
-template <int STAGES, int EPI_WARPS, bool SPLIT>
-__global__ void __launch_bounds__(64 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
+template <int AST, int BST, int EPI_WARPS, bool SPLIT>
+__global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
             const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
   constexpr int BN_MAX = bn_max(SPLIT);
-  constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT), STAGE_BYTES = stage_bytes(SPLIT);
-  constexpr int EW0 = SPLIT ? 6 : 2;     // first epilogue warp (warps 2..5 are the splitter in SPLIT mode)
+  constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT);
+  constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT);
+  constexpr int EW0 = SPLIT ? 7 : 3;     // first epilogue warp (warps 3..6 are the splitter in SPLIT mode)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  // stage s: [A | (A_lo) | B (B_hi) | (B_lo)]
-  auto sA = [&](int s) { return smem + s * STAGE_BYTES; };
-  auto sAlo = [&](int s) { return smem + s * STAGE_BYTES + A_STAGE_BYTES; };
-  auto sB = [&](int s) { return smem + s * STAGE_BYTES + (SPLIT ? 2 : 1) * A_STAGE_BYTES; };
-  auto sBlo = [&](int s) { return smem + s * STAGE_BYTES + 2 * A_STAGE_BYTES + B_STAGE_BYTES; };
-  uint64_t* bars = (uint64_t*)(smem + STAGES * STAGE_BYTES);
-  uint64_t* full = bars;                 // [STAGES]  TMA -> (splitter | MMA)
-  uint64_t* empty = bars + STAGES;       // [STAGES]  MMA -> TMA
-  uint64_t* ready = bars + 2 * STAGES;   // [STAGES]  splitter -> MMA (SPLIT only)
-  uint64_t* tfull = bars + 3 * STAGES;   // [2]
-  uint64_t* tempty = bars + 3 * STAGES + 2;   // [2]
-  uint32_t* tmem_slot = (uint32_t*)(bars + 3 * STAGES + 4);
-  float* stage_buf = (float*)(smem + STAGES * STAGE_BYTES + 256);
+  // Two independent rings: A (activations, from HBM: deep, AST stages of [A | (A_lo)]) and B (weights, from L2:
+  // shallow, BST stages of [B (B_hi) | (B_lo)]).  The bytes of A in flight set the achieved HBM bandwidth (a probe
+  // with the same tile-shaped access pattern reaches 2.5 TB/s with 16 KB in flight per SM and 6.1 TB/s with 64 KB).
+  auto sA = [&](int s) { return smem + s * A_RING_STAGE; };
+  auto sAlo = [&](int s) { return smem + s * A_RING_STAGE + A_STAGE_BYTES; };
+  auto sB = [&](int s) { return smem + AST * A_RING_STAGE + s * B_RING_STAGE; };
+  auto sBlo = [&](int s) { return smem + AST * A_RING_STAGE + s * B_RING_STAGE + B_STAGE_BYTES; };
+  uint64_t* bars = (uint64_t*)(smem + AST * A_RING_STAGE + BST * B_RING_STAGE);
+  uint64_t* fullA = bars;                    // [AST]  TMA -> (splitter | MMA)
+  uint64_t* emptyA = bars + AST;             // [AST]  MMA -> TMA
+  uint64_t* readyA = bars + 2 * AST;         // [AST]  splitter -> MMA (SPLIT only)
+  uint64_t* fullB = bars + 3 * AST;          // [BST]
+  uint64_t* emptyB = bars + 3 * AST + BST;   // [BST]
+  uint64_t* tfull = bars + 3 * AST + 2 * BST;        // [2]
+  uint64_t* tempty = bars + 3 * AST + 2 * BST + 2;   // [2]
+  uint32_t* tmem_slot = (uint32_t*)(bars + 3 * AST + 2 * BST + 4);
+  static_assert((3 * AST + 2 * BST + 5) * 8 <= 256, "barrier block");
+  float* stage_buf = (float*)(smem + AST * A_RING_STAGE + BST * B_RING_STAGE + 256);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = *g.m_ptr;
@@ -148,7 +155,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   const int num_kb = (g.K + BKF - 1) / BKF;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); mbar_init(&ready[s], 4); }
+    for (int s = 0; s < AST; ++s) { mbar_init(&fullA[s], 1); mbar_init(&emptyA[s], 1); mbar_init(&readyA[s], 4); }
+    for (int s = 0; s < BST; ++s) { mbar_init(&fullB[s], 1); mbar_init(&emptyB[s], 1); }
     for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], EPI_WARPS); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -162,19 +170,32 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   const uint32_t tmem_base = *tmem_slot;
 
   if (warp == 0) {
-    // ===== TMA producer =====
+    // ===== TMA producer, A ring =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      const uint32_t bytes = A_STAGE_BYTES + (SPLIT ? 2u : 1u) * (uint32_t)BN * BKF * 4;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        int mt = tile / ntn;
+        for (int kb = 0; kb < num_kb; ++kb) {
+          mbar_wait(&emptyA[stage], phase ^ 1);
+          mbar_expect_tx(&fullA[stage], A_STAGE_BYTES);
+          tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKF, mt * BM);
+          if (++stage == AST) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 2) {
+    // ===== TMA producer, B ring =====
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      const uint32_t bytes = (SPLIT ? 2u : 1u) * (uint32_t)BN * BKF * 4;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         int mt = tile / ntn, nt = tile - mt * ntn;
         for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1);
-          mbar_expect_tx(&full[stage], bytes);
-          tma_load_2d(sA(stage), &tmA, &full[stage], kb * BKF, mt * BM);
-          tma_load_2d(sB(stage), &tmB, &full[stage], kb * BKF, nt * BN);
-          if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &full[stage], kb * BKF, nt * BN);
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          mbar_wait(&emptyB[stage], phase ^ 1);
+          mbar_expect_tx(&fullB[stage], bytes);
+          tma_load_2d(sB(stage), &tmB, &fullB[stage], kb * BKF, nt * BN);
+          if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &fullB[stage], kb * BKF, nt * BN);
+          if (++stage == BST) { stage = 0; phase ^= 1; }
         }
       }
     }
@@ -183,42 +204,45 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     if (lane == 0) {
       // instruction descriptor: D=f32, A=B=tf32, K-major both, N>>3, M>>4
       const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
-      int stage = 0; uint32_t phase = 0; int it = 0;
+      int sa = 0, sb = 0; uint32_t pa = 0, pb = 0; int it = 0;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
         int acc = it & 1;
         mbar_wait(&tempty[acc], ((it >> 1) & 1) ^ 1);
         tc_fence_after();
         uint32_t d_tmem = tmem_base + acc * BN_MAX;
         for (int kb = 0; kb < num_kb; ++kb) {
-          mbar_wait(SPLIT ? &ready[stage] : &full[stage], phase);
+          mbar_wait(SPLIT ? &readyA[sa] : &fullA[sa], pa);
+          mbar_wait(&fullB[sb], pb);
           tc_fence_after();
-          uint64_t da = make_desc(smem_u32(sA(stage)));
-          uint64_t db = make_desc(smem_u32(sB(stage)));
+          uint64_t da = make_desc(smem_u32(sA(sa)));
+          uint64_t db = make_desc(smem_u32(sB(sb)));
 #pragma unroll
           for (int k = 0; k < BKF / 8; ++k)   // UMMA_K = 8 tf32 = 32 bytes -> +2 in the (addr >> 4) field
             tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
           if (SPLIT) {
-            uint64_t dal = make_desc(smem_u32(sAlo(stage)));
-            uint64_t dbl = make_desc(smem_u32(sBlo(stage)));
+            uint64_t dal = make_desc(smem_u32(sAlo(sa)));
+            uint64_t dbl = make_desc(smem_u32(sBlo(sb)));
 #pragma unroll
             for (int k = 0; k < BKF / 8; ++k) {
               tc_mma_tf32(d_tmem, da + 2 * k, dbl + 2 * k, idesc, 1u);    // A_hi * B_lo
               tc_mma_tf32(d_tmem, dal + 2 * k, db + 2 * k, idesc, 1u);    // A_lo * B_hi
             }
           }
-          tc_commit(&empty[stage]);
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          tc_commit(&emptyA[sa]);
+          tc_commit(&emptyB[sb]);
+          if (++sa == AST) { sa = 0; pa ^= 1; }
+          if (++sb == BST) { sb = 0; pb ^= 1; }
         }
         tc_commit(&tfull[acc]);
       }
     }
   } else if (SPLIT && warp < EW0) {
     // ===== splitter warps (3xTF32): A -> A_hi (in place, low 13 mantissa bits cleared) and A_lo = A - A_hi =====
-    const int t = threadIdx.x - 64;       // 0..127
+    const int t = threadIdx.x - 96;       // 0..127
     int stage = 0; uint32_t phase = 0;
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
       for (int kb = 0; kb < num_kb; ++kb) {
-        mbar_wait(&full[stage], phase);
+        mbar_wait(&fullA[stage], phase);
         float4* pa = reinterpret_cast<float4*>(sA(stage));
         float4* pl = reinterpret_cast<float4*>(sAlo(stage));
 #pragma unroll
@@ -231,8 +255,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         // generic-proxy writes -> visible to the async proxy (tcgen05.mma reads shared memory through it)
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
-        if (lane == 0) mbar_arrive(&ready[stage]);
-        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        if (lane == 0) mbar_arrive(&readyA[stage]);
+        if (++stage == AST) { stage = 0; phase ^= 1; }
       }
     }
   } else {
@@ -460,15 +484,16 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 
 }  // namespace
 
-#define GEMM_LAUNCH(ST, EW, SP)                                                                                          \
+#define GEMM_LAUNCH(AS, BS, EW, SP)                                                                                      \
   {                                                                                                                      \
+    static_assert(smem_bytes(AS, BS, EW, SP) <= 232448, "shared memory budget (227 KB)");                                \
     static bool attr_set = false;                                                                                        \
     if (!attr_set) {                                                                                                     \
-      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<ST, EW, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
-                                      (int)smem_bytes(ST, EW, SP)));                                                     \
+      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
+                                      (int)smem_bytes(AS, BS, EW, SP)));                                                 \
       attr_set = true;                                                                                                   \
     }                                                                                                                    \
-    k_gemm_tf32<ST, EW, SP><<<grid, 64 + (SP ? 128 : 0) + 32 * EW, smem_bytes(ST, EW, SP), m->stream>>>(tmA, tmB, tmB2, g, BN, ntn); \
+    k_gemm_tf32<AS, BS, EW, SP><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>(tmA, tmB, tmB2, g, BN, ntn); \
   }
 
 // precision 1: TF32 operands (rounded to nearest by the TMA load), fp32 accumulation
@@ -481,10 +506,10 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
   tmB2 = tmB;
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  static const int variant = getenv("B200_ALLEGRO_GEMM_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM_VARIANT")) : 0;   // 0: 16 epilogue warps (measured best), 1: 8, 2: 12
-  if (variant == 0) GEMM_LAUNCH(3, 16, false)
-  else if (variant == 2) GEMM_LAUNCH(3, 12, false)
-  else GEMM_LAUNCH(3, 8, false)
+  static const int variant = getenv("B200_ALLEGRO_GEMM_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM_VARIANT")) : 0;   // A/B ring depths: 0 = 4/3 (default), 1 = 6/2, 2 = 3/3 -- all within 1 % of each other: the rings are not the limiter
+  if (variant == 1) GEMM_LAUNCH(6, 2, 16, false)
+  else if (variant == 2) GEMM_LAUNCH(3, 3, 16, false)
+  else GEMM_LAUNCH(4, 3, 16, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
@@ -502,8 +527,8 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g) {
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
   static const int variant = getenv("B200_ALLEGRO_GEMM3_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM3_VARIANT")) : 0;
-  if (variant == 0) GEMM_LAUNCH(3, 8, true)
-  else GEMM_LAUNCH(2, 16, true)
+  if (variant == 0) GEMM_LAUNCH(4, 2, 8, true)
+  else GEMM_LAUNCH(3, 3, 8, true)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
