@@ -167,9 +167,9 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
   __shared__ int sZi[TB0_EDGES], sZj[TB0_EDGES];
   __shared__ float sU[TB0_EDGES];
   const int tid = threadIdx.x;
-  for (int idx = tid; idx < TB0_EDGES * NB; idx += 256) {
-    int r = idx / NB, q = idx - r * NB;
-    sB[r][q] = (e_base + r < M) ? B[(e_base + r) * NB + q] : 0.f;
+  for (int idx = tid; idx < TB0_EDGES * 16; idx += 256) {
+    int r = idx >> 4, q = idx & 15;
+    sB[r][q] = (q < NB && e_base + r < M) ? B[(e_base + r) * NB + q] : 0.f;
   }
   if (tid < TB0_EDGES) {
     int64_t e = e_base + tid;
@@ -179,6 +179,31 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
   }
   __syncthreads();
   const int H4 = H >> 2;
+  if (256 % H4 == 0 && NB <= 8) {
+    // a thread keeps its 4 output columns for all its edges: the Bessel weight rows stay in registers
+    const int k4 = (tid % H4) * 4, rstep = 256 / H4;
+    float4 wb[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q)
+      wb[q] = (q < NB) ? __ldg(reinterpret_cast<const float4*>(W + (size_t)(2 * S + q) * H + k4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int r = tid / H4; r < TB0_EDGES; r += rstep) {
+      const int64_t e = e_base + r;
+      if (e >= M) break;
+      float4 a0 = __ldg(reinterpret_cast<const float4*>(W + (size_t)sZi[r] * H + k4));
+      float4 a1 = __ldg(reinterpret_cast<const float4*>(W + (size_t)(S + sZj[r]) * H + k4));
+      float4 acc = make_float4(a0.x + a1.x, a0.y + a1.y, a0.z + a1.z, a0.w + a1.w);
+#pragma unroll
+      for (int q = 0; q < 8; ++q) {
+        const float b = sB[r][q];   // (zero beyond NB)
+        acc.x = fmaf(b, wb[q].x, acc.x); acc.y = fmaf(b, wb[q].y, acc.y); acc.z = fmaf(b, wb[q].z, acc.z); acc.w = fmaf(b, wb[q].w, acc.w);
+      }
+      *reinterpret_cast<float4*>(z + e * H + k4) = acc;
+      const float us = scale_u ? sU[r] : 1.0f;
+      *reinterpret_cast<float4*>(act + e * ldact + k4) =
+          make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
+    }
+    return;
+  }
   for (int idx = tid; idx < TB0_EDGES * H4; idx += 256) {
     const int r = idx / H4, k4 = (idx - r * H4) * 4;
     const int64_t e = e_base + r;
