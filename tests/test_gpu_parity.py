@@ -269,3 +269,41 @@ def test_full_size_subsystem_parity(ci, precision):
 
 def test_config3_million_atoms_subsystem_parity():
     _subsystem_check(3, 8, 1)
+
+
+# ---------------------------------------------------------------------------------------------------
+# hyper-parameter shapes outside the five configs: deeper MLPs (the paper's own model has three latent layers,
+# PAPER.md:222), a single two-body layer, other (l_max, layers) combinations -> other kernel dispatch paths
+# ---------------------------------------------------------------------------------------------------
+def _variant(base_index, n_atoms, **hp_changes):
+    import dataclasses
+    c = scaled_config(base_index, n_atoms)
+    c.hp = dataclasses.replace(c.hp, **hp_changes)
+    return c
+
+
+VARIANTS = {
+    "deep_mlps": (1, 768, dict(twobody_dims=(32, 64, 64, 128), latent_dims=(96, 64, 128), edge_dims=(32, 16))),
+    "one_twobody_layer": (1, 768, dict(twobody_dims=(64,), latent_dims=(64,), edge_dims=(8,))),
+    "lmax2_three_layers": (1, 768, dict(n_layers=3, resid_alpha=(0.5, 0.5, 0.5), twobody_dims=(32, 64), latent_dims=(64,))),
+    "lmax1_two_layers_n32": (0, 384, dict(n_layers=2, n_tensor=32, resid_alpha=(0.5, 0.5))),
+    "lmax3_two_layers": (4, 600, dict(n_layers=2, n_tensor=32, resid_alpha=(0.5, 0.5), twobody_dims=(32, 64), latent_dims=(64,))),
+    "odd_channels_n24": (1, 768, dict(n_tensor=24, twobody_dims=(32, 64), latent_dims=(64,))),
+}
+
+
+@pytest.mark.parametrize("name", sorted(VARIANTS))
+@pytest.mark.parametrize("precision", [0, 1])
+def test_other_hyperparameter_shapes(name, precision):
+    base, n, changes = VARIANTS[name]
+    cfg = _variant(base, n, **changes)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg, precision=precision)
+    (E, Ea, F), nb = gpu_eval(model, pos, sp, box)
+    E0, Ea0, F0 = O.energy_forces(oracle, pos, sp, box, O.neighbor_list(pos, box, cfg.hp.r_cut))
+    if precision == 0:
+        _check_EF((E, Ea, F), (E0, Ea0, F0), n, f"{name} fp32")
+    else:
+        mu = np.array(cfg.mu())[sp]
+        assert abs(E - E0) <= 2e-3 * np.abs(Ea0 - mu).sum()
+        assert np.abs(F - F0).max() <= 2e-3 * np.abs(F0).max()
