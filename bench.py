@@ -175,6 +175,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
+    ap.add_argument("--pair-cutoffs", default="none", choices=["none", "water"],
+                    help="ordered species-pair cutoffs (PAPER.md:172-182, :222); 'water' = the paper's H/O values, configs 0-1 only")
     args = ap.parse_args()
     K, W = args.steps, max(args.warmup, 3)
     rank = int(os.environ.get("RANK", "0"))
@@ -185,6 +187,12 @@ def main():
     from synthetic.systems import masses_for
     cfg = CONFIGS[args.config]
     workload = f"config{cfg.index}:{cfg.name}"
+    if args.pair_cutoffs == "water":
+        import dataclasses
+        from synthetic.configs import WATER_PAIR_CUTOFFS
+        assert cfg.index in (0, 1), "the water pair cutoffs need the (H, O) species of configs 0-1"
+        cfg = dataclasses.replace(cfg, hp=dataclasses.replace(cfg.hp, r_cut_pair=WATER_PAIR_CUTOFFS))
+        workload += " + ordered species-pair cutoffs (H-H 3.0, H-O 1.25, O-H 3.0, O-O 4.0)"
     metric, unit = "atom-steps/s (energy+forces, 1 B200)", "atom-steps/s"
 
     # ---------------------------------------------------------------- reference arm = the oracle on host cores
@@ -229,6 +237,8 @@ def main():
     chp = P.hparams_from(cfg.hp, args.precision)
     blob = make_blob(cfg.hp, P.path_fan(chp), [cfg.sigma] * cfg.hp.n_species, cfg.mu(), cfg.weight_seed)
     model = P.Allegro(chp, blob, chunk_edges=args.chunk_edges) if args.chunk_edges else P.Allegro(chp, blob)
+    if cfg.hp.r_cut_pair is not None:
+        model.set_pair_cutoffs(cfg.hp.r_cut_pair)
     dev = torch.device("cuda", local_rank)
     p = torch.from_numpy(pos.copy()).to(dev); v = torch.from_numpy(vel.copy()).to(dev)
     s = torch.from_numpy(sp).to(dev); mass = torch.from_numpy(masses_for(cfg)).to(dev)

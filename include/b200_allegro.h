@@ -149,6 +149,13 @@ int allegro_launch_count(const allegro_model* m, int64_t* launches);
 /* Total number of active (r < r_cut) edges, over all chunks, of the last allegro_compute (synchronises the stream). */
 int allegro_last_active_edges(allegro_model* m, int64_t* n_active);
 
+/* Ordered species-pair cutoffs ("independent cutoffs for each *ordered* species pair", values
+ * :222): rc_pair is a HOST array [n_species][n_species], row = species of the centre i, column = species of the
+ * neighbour j, every entry in (0, r_cut].  The ordered pair (i, j) is an edge iff r_ij < rc_pair[Z_i][Z_j]; the
+ * envelope argument and the Bessel functions of that edge use the pair's own cutoff.  NULL restores the flat
+ * r_cut.  Neighbor lists are still built at a cutoff >= r_cut (the largest pair cutoff). */
+int allegro_set_pair_cutoffs(allegro_model* m, const double* rc_pair);
+
 /* Debug mode (tests only; default off): keep every intermediate tensor that allegro_debug_tensor can name.
  * Without it the final latent x^{NL} is consumed inside the epilogue of the last latent GEMM and never stored. */
 int allegro_set_debug(allegro_model* m, int on);

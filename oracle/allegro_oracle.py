@@ -49,10 +49,14 @@ def poly_cutoff(x: torch.Tensor, p: int) -> torch.Tensor:
     return torch.where(x < 1.0, u, torch.zeros_like(u))
 
 
-def bessel_basis(r: torch.Tensor, r_cut: float, n_bessel: int) -> torch.Tensor:
-    """b_n(r) = sqrt(2/r_c) sin(n pi r / r_c) / r, n = 1..N_B.  Returns [..., N_B]."""
+def bessel_basis(r: torch.Tensor, r_cut, n_bessel: int) -> torch.Tensor:
+    """b_n(r) = sqrt(2/r_c) sin(n pi r / r_c) / r, n = 1..N_B.  Returns [..., N_B].
+    r_cut: a float, or a tensor of the shape of r (one cutoff per edge: ordered species-pair cutoffs)."""
     n = torch.arange(1, n_bessel + 1, dtype=torch.float64)
-    return math.sqrt(2.0 / r_cut) * torch.sin(n * math.pi * r[..., None] / r_cut) / r[..., None]
+    rc = torch.as_tensor(r_cut, dtype=torch.float64)
+    if rc.ndim:
+        rc = rc[..., None]
+    return torch.sqrt(2.0 / rc) * torch.sin(n * math.pi * r[..., None] / rc) / r[..., None]
 
 
 # ----------------------------------------------------------------------------------------------
@@ -390,16 +394,24 @@ class OracleModel:
         n, lmax, NL, d = hp.n_tensor, hp.l_max, hp.n_layers, hp.d
         rvec = pos[ej] - pos[ei] + es.to(torch.float64) * box                  # S1 convention
         r = torch.sqrt((rvec * rvec).sum(-1))
-        keep = r < hp.r_cut                                                    # skin lists (S9 last line)
+        # cutoff of each ordered pair (i centre, j neighbour): r_c, or r_c[Z_i][Z_j] with ordered species-pair
+        # cutoffs (NEXT-1 reading in DESIGN.md: the pair's own cutoff enters the edge
+        # criterion, the envelope argument x = r / r_c[Z_i][Z_j] and the Bessel functions)
+        pair = getattr(hp, "r_cut_pair", None)
+        if pair is None:
+            rc = torch.full_like(r, hp.r_cut)
+        else:
+            rc = torch.tensor(pair, dtype=torch.float64)[species[ei], species[ej]]
+        keep = r < rc                                                          # skin lists (S9 last line)
         full_E = r.shape[0]
         idx = torch.nonzero(keep).reshape(-1)
-        ei, ej, rvec, r = ei[idx], ej[idx], rvec[idx], r[idx]
+        ei, ej, rvec, r, rc = ei[idx], ej[idx], rvec[idx], r[idx], rc[idx]
         E = r.shape[0]
         cent, ec = torch.unique(ei, return_inverse=True)      # local centre numbering for the env sum
         n_cent = cent.shape[0]
-        x = r / hp.r_cut
+        x = r / rc
         u = poly_cutoff(x, hp.poly_p)                                           # S2
-        B = bessel_basis(r, hp.r_cut, hp.n_bessel) * u[:, None]
+        B = bessel_basis(r, rc, hp.n_bessel) * u[:, None]
         onehot = torch.eye(hp.n_species, dtype=torch.float64)
         h = torch.cat([onehot[species[ei]], onehot[species[ej]], B], dim=1)     # S3
         for W in self.twobody:

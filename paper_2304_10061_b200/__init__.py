@@ -72,7 +72,7 @@ EXPORTS = [
     "allegro_set_allocator", "allegro_set_chunk_edges", "allegro_neighbors", "allegro_neighbors_host",
     "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
-    "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_debug_tensor",
+    "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
     "allegro_last_error",
 ]
 
@@ -98,6 +98,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_set_allocator.argtypes = [vp, _ALLOC_FN, _FREE_FN, vp]
     lib.allegro_set_chunk_edges.argtypes = [vp, i64]
     lib.allegro_set_debug.argtypes = [vp, C.c_int]
+    lib.allegro_set_pair_cutoffs.argtypes = [vp, vp]
     lib.allegro_neighbors.argtypes = [vp, vp, i64, P(C.c_double), C.c_double, P(vp)]
     lib.allegro_neighbors_host.argtypes = [vp, vp, i64, P(C.c_double), C.c_double, P(vp)]
     lib.allegro_nbr_info.argtypes = [vp, P(i64), P(i64), P(vp), P(vp), P(vp)]
@@ -328,6 +329,16 @@ class Allegro:
         ms, n = C.c_double(0), C.c_int64(0)
         self._check(self._lib.allegro_profile_read(self._h, name.encode(), C.byref(ms), C.byref(n)))
         return ms.value, n.value
+
+    def set_pair_cutoffs(self, rc_pair):
+        """Ordered species-pair cutoffs rc_pair[Z_centre][Z_neighbour]; None = flat r_cut."""
+        import numpy as np
+        if rc_pair is None:
+            self._check(self._lib.allegro_set_pair_cutoffs(self._h, None))
+            return
+        a = np.ascontiguousarray(rc_pair, dtype=np.float64)
+        assert a.shape == (self.hp.n_species, self.hp.n_species)
+        self._check(self._lib.allegro_set_pair_cutoffs(self._h, a.ctypes.data))
 
     def set_debug(self, on: bool = True):
         """Keep every tensor debug_tensor() can name (tests only)."""

@@ -107,6 +107,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   ga.pos = pos; ga.species = species; memcpy(ga.box, box, 24); ga.rc = hp.r_cut; ga.p = hp.poly_p; ga.NB = m->NB;
   ga.lmax = m->lmax; ga.row_ptr = (const int64_t*)nb->row_ptr.p; ga.j = (const int32_t*)nb->j.p;
   ga.shift = (const int8_t*)nb->shift.p; ga.c0 = ch.c0; ga.nc = nc;
+  ga.rc_pair = m->d_rc_pair; ga.S = m->S;
   // ---- step 2: compaction + geometry ----------------------------------------------------------------
   AL_CHECK(k_launch_active_count(m, ga, (int*)w.deg.p));
   AL_CHECK(al_exclusive_scan_i64(m, (int*)w.deg.p, (int64_t*)w.rowa.p, nc, w.scan_tmp));

@@ -71,14 +71,16 @@ __device__ __forceinline__ void sph_harm_vjp(float x, float y, float z, int lmax
 }
 
 // ---- active-edge count / compaction + geometry ------------------------------------------------------
+// rc: the cutoff of this ordered pair, r_cut or r_c[Z_i][Z_j] (allegro_set_pair_cutoffs)
 __device__ __forceinline__ bool edge_vec(const EdgeGeomArgs& a, int i, int64_t e, int& j, double& dx, double& dy,
-                                         double& dz, double& r2) {
+                                         double& dz, double& r2, double& rc) {
   j = a.j[e];
+  rc = a.rc_pair ? a.rc_pair[a.species[i] * a.S + a.species[j]] : a.rc;
   dx = (a.pos[3 * (int64_t)j + 0] - a.pos[3 * (int64_t)i + 0]) + (double)a.shift[3 * e + 0] * a.box[0];
   dy = (a.pos[3 * (int64_t)j + 1] - a.pos[3 * (int64_t)i + 1]) + (double)a.shift[3 * e + 1] * a.box[1];
   dz = (a.pos[3 * (int64_t)j + 2] - a.pos[3 * (int64_t)i + 2]) + (double)a.shift[3 * e + 2] * a.box[2];
   r2 = dx * dx + dy * dy + dz * dz;
-  return r2 < a.rc * a.rc;
+  return r2 < rc * rc;
 }
 
 __global__ void k_active_count(EdgeGeomArgs a, int* __restrict__ deg) {
@@ -88,8 +90,8 @@ __global__ void k_active_count(EdgeGeomArgs a, int* __restrict__ deg) {
   int64_t b = a.row_ptr[i], e = a.row_ptr[i + 1];
   int cnt = 0;
   for (int64_t k = b + lane; k < e; k += 32) {
-    int j; double dx, dy, dz, r2;
-    cnt += edge_vec(a, i, k, j, dx, dy, dz, r2) ? 1 : 0;
+    int j; double dx, dy, dz, r2, rc;
+    cnt += edge_vec(a, i, k, j, dx, dy, dz, r2, rc) ? 1 : 0;
   }
   cnt = (int)warp_sum((float)cnt);
   if (lane == 0) deg[warp] = cnt;
@@ -113,8 +115,8 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
   int cnt = 0;
   for (int64_t kb = b; kb < e; kb += 32) {
     int64_t k = kb + lane;
-    int j = 0; double dx = 0, dy = 0, dz = 0, r2 = 0;
-    bool ok = (k < e) && edge_vec(a, i, k, j, dx, dy, dz, r2);
+    int j = 0; double dx = 0, dy = 0, dz = 0, r2 = 0, rc = a.rc;
+    bool ok = (k < e) && edge_vec(a, i, k, j, dx, dy, dz, r2, rc);
     unsigned mask = __ballot_sync(FULLMASK, ok);
     if (ok) {
       int64_t o = out0 + cnt + __popc(mask & ((1u << lane) - 1u));
@@ -126,18 +128,18 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
       sig[o] = (float)sigma[a.species[i]];
       geo[o] = make_float4(hx, hy, hz, (float)r);
       // envelope (fp64; PAPER.md:222 via SURVEY S2)
-      double x = r / a.rc, p = (double)a.p;
+      double x = r / rc, p = (double)a.p;
       double xp1 = pow(x, p - 1.0), xp = xp1 * x;
       double uu = 1.0 - 0.5 * (p + 1.0) * (p + 2.0) * xp + p * (p + 2.0) * xp * x - 0.5 * p * (p + 1.0) * xp * x * x;
-      double dud = -0.5 * p * (p + 1.0) * (p + 2.0) * xp1 * (1.0 - x) * (1.0 - x) / a.rc;
+      double dud = -0.5 * p * (p + 1.0) * (p + 2.0) * xp1 * (1.0 - x) * (1.0 - x) / rc;
       u[o] = (float)uu; du[o] = (float)dud;
       // Bessel basis by the angle-addition recurrence in fp64
       double th = M_PI * x, s1, c1;
       sincos(th, &s1, &c1);
-      double sn = s1, cn = c1, pref = sqrt(2.0 / a.rc);
+      double sn = s1, cn = c1, pref = sqrt(2.0 / rc);
       for (int nb = 1; nb <= a.NB; ++nb) {
         double bn = pref * sn * inv;
-        double dbn = pref * ((double)nb * M_PI / a.rc * cn * inv - sn * inv * inv);
+        double dbn = pref * ((double)nb * M_PI / rc * cn * inv - sn * inv * inv);
         B[o * a.NB + nb - 1] = (float)(bn * uu);
         dB[o * a.NB + nb - 1] = (float)(dbn * uu + bn * dud);
         double s2 = sn * c1 + cn * s1, c2 = cn * c1 - sn * s1;

@@ -106,6 +106,7 @@ struct allegro_model {
   std::vector<std::vector<Dense>> latent; // [NL][n_latent]
   float* w_eff_f = nullptr; double* w_eff_d = nullptr;   // product of the edge-MLP layers, [d]
   double *sigma = nullptr, *mu = nullptr; // device [S]
+  double* d_rc_pair = nullptr;            // device [S][S] ordered species-pair cutoffs, or null (flat r_cut)
   std::vector<double> sigma_h, mu_h;
   float c_env; float c_old[AL_MAX_LAYERS], c_new[AL_MAX_LAYERS];
   // runtime

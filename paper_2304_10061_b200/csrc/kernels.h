@@ -38,6 +38,7 @@ struct Work {
 
 struct EdgeGeomArgs {
   const double* pos; const int32_t* species; double box[3]; double rc; int p; int NB; int lmax;
+  const double* rc_pair; int S;                                     // ordered species-pair cutoffs [S][S] or null
   const int64_t* row_ptr; const int32_t* j; const int8_t* shift;   // candidate list (global)
   int64_t c0; int nc;                                               // centers [c0, c0+nc)
 };

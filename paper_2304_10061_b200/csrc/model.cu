@@ -309,6 +309,23 @@ extern "C" int allegro_set_allocator(allegro_model* m, allegro_alloc_fn a, alleg
   return ALLEGRO_OK;
 }
 
+extern "C" int allegro_set_pair_cutoffs(allegro_model* m, const double* rc_pair) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  if (!rc_pair) { m->d_rc_pair = nullptr; return ALLEGRO_OK; }   // (the device array stays owned by the model)
+  const int S = m->S;
+  for (int k = 0; k < S * S; ++k)
+    if (!(rc_pair[k] > 0) || rc_pair[k] > m->hp.r_cut) {
+      al_set_error(m, "pair cutoffs must be in (0, r_cut]");
+      return ALLEGRO_ERR_BAD_HPARAMS;
+    }
+  std::vector<double> h(rc_pair, rc_pair + (size_t)S * S);
+  double* d = nullptr;
+  AL_CHECK(upload(m, &d, h));
+  m->d_rc_pair = d;
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_set_debug(allegro_model* m, int on) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   m->debug_keep = on != 0;

@@ -6,7 +6,7 @@ from __future__ import annotations
 
 import dataclasses
 import math
-from typing import List, Tuple
+from typing import List, Optional, Tuple
 
 
 @dataclasses.dataclass
@@ -23,6 +23,8 @@ class Hparams:
     edge_dims: Tuple[int, ...]         # edge-energy MLP hidden widths; final ->1 implicit
     avg_num_neighbors: float           # c_env = 1/sqrt(this)
     resid_alpha: Tuple[float, ...]     # per layer
+    # optional ordered species-pair cutoffs r_c[Z_centre][Z_neighbour] <= r_cut; None = flat r_cut
+    r_cut_pair: Optional[Tuple[Tuple[float, ...], ...]] = None
 
     @property
     def d(self) -> int:
@@ -80,6 +82,11 @@ CONFIGS: List[Config] = [
     Config(4, "tpstress50k", _hp(4, 3, 3, 64, [128, 256], [256], [128], 6.0, _AVG6),
            50000, 0.08, "random4", ("H", "C", "N", "O"), 1.0, 10, 0.5, 300.0, 1004, 2004),
 ]
+
+
+# The paper's ordered-pair cutoffs restricted to water ("H-H 3.0, H-C 1.25, H-O 1.25, O-H 3.0", all
+# others 4.0 Angstrom); species order of configs 0/1 is (H, O), rows = centre species.
+WATER_PAIR_CUTOFFS = ((3.0, 1.25), (3.0, 4.0))
 
 
 def get_config(index: int) -> Config:

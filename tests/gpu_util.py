@@ -15,6 +15,8 @@ def make_both(cfg, precision=0, sigma=None, chunk_edges=None):
     s = cfg.sigma if sigma is None else sigma
     blob = make_blob(hp, fan_gpu, [s] * hp.n_species, cfg.mu(), cfg.weight_seed)
     model = P.Allegro(chp, blob, chunk_edges=chunk_edges)
+    if getattr(hp, "r_cut_pair", None) is not None:
+        model.set_pair_cutoffs(hp.r_cut_pair)
     oracle = O.OracleModel(hp, blob)
     return model, oracle
 

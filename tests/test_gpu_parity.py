@@ -307,3 +307,35 @@ def test_other_hyperparameter_shapes(name, precision):
         mu = np.array(cfg.mu())[sp]
         assert abs(E - E0) <= 2e-3 * np.abs(Ea0 - mu).sum()
         assert np.abs(F - F0).max() <= 2e-3 * np.abs(F0).max()
+
+
+# ---------------------------------------------------------------------------------------------------
+# NEXT-1: ordered species-pair cutoffs (values :222) on the water configs
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ci,n,precision", [(0, 192, 0), (1, 1536, 0), (1, 1536, 3), (1, 1536, 1)])
+def test_ordered_pair_cutoffs(ci, n, precision):
+    import dataclasses
+    from synthetic.configs import WATER_PAIR_CUTOFFS
+    cfg = scaled_config(ci, n)
+    cfg.hp = dataclasses.replace(cfg.hp, r_cut_pair=WATER_PAIR_CUTOFFS)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg, precision=precision)
+    # skin list: candidates beyond every pair cutoff must drop out in the compaction
+    (E, Ea, F), nb = gpu_eval(model, pos, sp, box, cutoff=cfg.hp.r_cut + 0.5)
+    oi, oj, os_ = O.neighbor_list(pos, box, cfg.hp.r_cut)
+    rvec = pos[oj] - pos[oi] + os_ * box
+    rc = np.array(WATER_PAIR_CUTOFFS)[sp[oi], sp[oj]]
+    assert model.last_active_edges() == int((np.sqrt((rvec ** 2).sum(1)) < rc).sum())      # integer work: exact
+    want = O.energy_forces(oracle, pos, sp, box, (oi, oj, os_))
+    if precision in (0, 3):
+        _check_EF((E, Ea, F), want, n, f"pair cutoffs cfg{ci} prec{precision}")
+    else:
+        mu = np.array(cfg.mu())[sp]
+        assert abs(E - want[0]) <= 2e-3 * np.abs(want[1] - mu).sum()
+        assert np.abs(F - want[2]).max() <= 2e-3 * np.abs(want[2]).max()
+    # NULL restores the flat cutoff
+    model.set_pair_cutoffs(None)
+    got0, _ = gpu_eval(model, pos, sp, box)
+    if precision in (0, 3):
+        _, flat = make_both(scaled_config(ci, n), precision=precision)         # same seeded blob, no pair cutoffs
+        _check_EF(got0, O.energy_forces(flat, pos, sp, box, (oi, oj, os_)), n, "flat again")
