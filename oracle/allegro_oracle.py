@@ -49,14 +49,39 @@ def poly_cutoff(x: torch.Tensor, p: int) -> torch.Tensor:
     return torch.where(x < 1.0, u, torch.zeros_like(u))
 
 
-def bessel_basis(r: torch.Tensor, r_cut, n_bessel: int) -> torch.Tensor:
-    """b_n(r) = sqrt(2/r_c) sin(n pi r / r_c) / r, n = 1..N_B.  Returns [..., N_B].
-    r_cut: a float, or a tensor of the shape of r (one cutoff per edge: ordered species-pair cutoffs)."""
+def bessel_basis(r: torch.Tensor, r_cut, n_bessel: int, freq=None) -> torch.Tensor:
+    """b_n(r) = sqrt(2/r_c) sin(w_n r) / r, n = 1..N_B, with w_n = n pi / r_c unless `freq` is given.  Returns [..., N_B].
+    r_cut: a float, or a tensor of the shape of r (one cutoff per edge: ordered species-pair cutoffs).
+    freq: optional tensor [..., N_B] of angular frequencies in 1/Angstrom, one row per edge (the "trainable
+    per-ordered-species-pair radial basis" of PAPER.md:222: the trained values of w_n for the edge's pair)."""
     n = torch.arange(1, n_bessel + 1, dtype=torch.float64)
     rc = torch.as_tensor(r_cut, dtype=torch.float64)
     if rc.ndim:
         rc = rc[..., None]
-    return torch.sqrt(2.0 / rc) * torch.sin(n * math.pi * r[..., None] / rc) / r[..., None]
+    w = n * math.pi / rc if freq is None else freq
+    return torch.sqrt(2.0 / rc) * torch.sin(w * r[..., None]) / r[..., None]
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4. ZBL pair repulsion ("We also add a repulsive Ziegler-Biersack-Littmark (ZBL) term to the
+#     potential").  The paper gives no formula; reading: the universal screened-Coulomb form
+#         phi_ij(r) = k_e Z_i Z_j / r * Phi(r / a_ij) * u(r / r_c),   a_ij = 0.46850 / (Z_i^0.23 + Z_j^0.23) Angstrom,
+#         Phi(x) = 0.18175 e^{-3.19980 x} + 0.50986 e^{-0.94229 x} + 0.28022 e^{-0.40290 x} + 0.02817 e^{-0.20162 x},
+#     times the model's own polynomial envelope u at the FLAT cutoff r_c (a pair potential must be symmetric in
+#     (i, j), which the ordered pair cutoffs are not), E_ZBL = 1/2 sum over ordered pairs, split evenly between the
+#     two atoms, not scaled by sigma_Z.
+# ----------------------------------------------------------------------------------------------
+KE_EV_A = 14.399645478425668   # e^2 / (4 pi eps0) in eV * Angstrom
+ZBL_C = (0.18175, 0.50986, 0.28022, 0.02817)
+ZBL_D = (3.19980, 0.94229, 0.40290, 0.20162)
+
+
+def zbl_pair_energy(r: torch.Tensor, zi: torch.Tensor, zj: torch.Tensor, r_cut: float, p: int) -> torch.Tensor:
+    """phi_ij(r) of the reading above, elementwise; zi, zj are atomic numbers (float64)."""
+    a = 0.46850 / (zi ** 0.23 + zj ** 0.23)
+    x = r / a
+    Phi = sum(c * torch.exp(-dd * x) for c, dd in zip(ZBL_C, ZBL_D))
+    return KE_EV_A * zi * zj / r * Phi * poly_cutoff(r / r_cut, p)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -411,7 +436,9 @@ class OracleModel:
         n_cent = cent.shape[0]
         x = r / rc
         u = poly_cutoff(x, hp.poly_p)                                           # S2
-        B = bessel_basis(r, rc, hp.n_bessel) * u[:, None]
+        fq = getattr(hp, "bessel_freq_pair", None)                              # [S][S][N_B] or None
+        fq = None if fq is None else torch.tensor(fq, dtype=torch.float64)[species[ei], species[ej]]
+        B = bessel_basis(r, rc, hp.n_bessel, fq) * u[:, None]
         onehot = torch.eye(hp.n_species, dtype=torch.float64)
         h = torch.cat([onehot[species[ei]], onehot[species[ej]], B], dim=1)     # S3
         for W in self.twobody:
@@ -451,6 +478,13 @@ class OracleModel:
         Ee = self.edge_energies(pos, species, box, ei, ej, es)
         Ei = _zeros(N).index_add(0, ei, Ee)
         Ehat = self.sigma[species] * Ei + self.mu[species]
+        zn = getattr(self.hp, "zbl_Z", None)
+        if zn is not None:                                                     # NEXT-4: ZBL, 1/2 phi_ij to the centre
+            zn = torch.tensor(zn, dtype=torch.float64)
+            rvec = pos[ej] - pos[ei] + es.to(torch.float64) * box
+            r = torch.sqrt((rvec * rvec).sum(-1))
+            phi = zbl_pair_energy(r, zn[species[ei]], zn[species[ej]], self.hp.r_cut, self.hp.poly_p)
+            Ehat = Ehat + _zeros(N).index_add(0, ei, 0.5 * phi)
         if centers is not None:
             Ehat = Ehat * centers
         return Ehat
@@ -517,3 +551,38 @@ def nve_step(force_fn, pos, vel, force, mass_per_atom, dt_fs):
     e_pot, force = force_fn(pos)
     vel = nve_half_kick(vel, force, mass_per_atom, dt_fs)
     return pos, vel, force, e_pot
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT-4. thermostatted MD ("stable temperature around thermostat setting of 300K"; the paper does not
+#     name the thermostat).  Reading: one Nose-Hoover thermostat variable xi (1/fs) of relaxation time
+#     tau, Q = g k_B T0 tau^2, g = 3N degrees of freedom, integrated by the symmetric Trotter splitting
+#         [thermostat dt/2] [velocity-Verlet NVE step dt] [thermostat dt/2],
+#     thermostat half step:  xi += dt/4 * G(K);  v *= s = exp(-xi dt/2) (K *= s^2);  xi += dt/4 * G(K),
+#     G(K) = (2 K - g k_B T0) / Q.   Conserved: K + E_pot + Q xi^2 / 2 + g k_B T0 eta,  d(eta)/dt = xi.
+# ----------------------------------------------------------------------------------------------
+def nh_half_step(vel, xi, eta, e_kin, n_dof, t0_K, tau_fs, dt_fs):
+    """One thermostat half step.  Returns vel, xi, eta, e_kin (all after the half step)."""
+    gkt = n_dof * KB_EV * t0_K
+    Q = gkt * tau_fs * tau_fs
+    xi = xi + 0.25 * dt_fs * (2.0 * e_kin - gkt) / Q
+    s = math.exp(-xi * 0.5 * dt_fs)
+    eta = eta + xi * 0.5 * dt_fs
+    vel = vel * s
+    e_kin = e_kin * s * s
+    xi = xi + 0.25 * dt_fs * (2.0 * e_kin - gkt) / Q
+    return vel, xi, eta, e_kin
+
+
+def nvt_step(force_fn, pos, vel, force, mass_per_atom, dt_fs, xi, eta, t0_K, tau_fs):
+    """Nose-Hoover NVT step of the reading above.  Returns pos, vel, force, e_pot, e_kin, xi, eta."""
+    g = 3 * pos.shape[0]
+    vel, xi, eta, _ = nh_half_step(vel, xi, eta, kinetic_energy(vel, mass_per_atom), g, t0_K, tau_fs, dt_fs)
+    pos, vel, force, e_pot = nve_step(force_fn, pos, vel, force, mass_per_atom, dt_fs)
+    vel, xi, eta, e_kin = nh_half_step(vel, xi, eta, kinetic_energy(vel, mass_per_atom), g, t0_K, tau_fs, dt_fs)
+    return pos, vel, force, e_pot, e_kin, xi, eta
+
+
+def nh_conserved(e_pot, e_kin, xi, eta, n_dof, t0_K, tau_fs):
+    gkt = n_dof * KB_EV * t0_K
+    return e_pot + e_kin + 0.5 * gkt * tau_fs * tau_fs * xi * xi + gkt * eta

@@ -25,6 +25,11 @@ class Hparams:
     resid_alpha: Tuple[float, ...]     # per layer
     # optional ordered species-pair cutoffs r_c[Z_centre][Z_neighbour] <= r_cut; None = flat r_cut
     r_cut_pair: Optional[Tuple[Tuple[float, ...], ...]] = None
+    # optional trained Bessel angular frequencies w_n[Z_centre][Z_neighbour][n] in 1/A ("trainable
+    # per-ordered-species-pair radial basis"); None = n pi / r_c of the pair
+    bessel_freq_pair: Optional[Tuple[Tuple[Tuple[float, ...], ...], ...]] = None
+    # optional atomic numbers per species: adds the ZBL pair repulsion; None = no ZBL term
+    zbl_Z: Optional[Tuple[float, ...]] = None
 
     @property
     def d(self) -> int:
@@ -87,6 +92,9 @@ CONFIGS: List[Config] = [
 # The paper's ordered-pair cutoffs restricted to water ("H-H 3.0, H-C 1.25, H-O 1.25, O-H 3.0", all
 # others 4.0 Angstrom); species order of configs 0/1 is (H, O), rows = centre species.
 WATER_PAIR_CUTOFFS = ((3.0, 1.25), (3.0, 4.0))
+
+
+ATOMIC_NUMBERS = {"H": 1.0, "C": 6.0, "N": 7.0, "O": 8.0, "S": 16.0}
 
 
 def get_config(index: int) -> Config:
