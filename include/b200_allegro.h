@@ -110,7 +110,8 @@ int allegro_nbr_free(allegro_model* m, allegro_nbr* n);
 /* Energy and forces (PAPER.md:128 energy decomposition; Eq. (2) PAPER.md:132-138 layers
  * fp64 final stage; forces F_i = -dE/dr_i by the hand-written analytic backward).
  * The list may have been built at cutoff >= r_cut (Verlet skin); edges with r >= r_cut are dropped.
- * pos f64[N*3], species i32[N], e_total f64[1], e_atom f64[N] or NULL, force f64[N*3] (device). */
+ * pos f64[N*3], species i32[N], e_total f64[1], e_atom f64[N] or NULL, force f64[N*3] (device), or NULL for an
+ * energy-only evaluation (the backward pass is skipped). */
 int allegro_compute(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
                     const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force);
 int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
@@ -155,6 +156,34 @@ int allegro_last_active_edges(allegro_model* m, int64_t* n_active);
  * envelope argument and the Bessel functions of that edge use the pair's own cutoff.  NULL restores the flat
  * r_cut.  Neighbor lists are still built at a cutoff >= r_cut (the largest pair cutoff). */
 int allegro_set_pair_cutoffs(allegro_model* m, const double* rc_pair);
+
+/* Trained Bessel angular frequencies of the "trainable per-ordered-species-pair radial basis":
+ * freq is a HOST array [n_species][n_species][n_bessel] in 1/Angstrom (row = centre species, column = neighbour
+ * species); b_n(r) = sqrt(2 / r_c) sin(freq_n r) / r with r_c the pair's cutoff.  NULL restores n pi / r_c. */
+int allegro_set_bessel_frequencies(allegro_model* m, const double* freq);
+
+/* ZBL pair repulsion ("We also add a repulsive Ziegler-Biersack-Littmark (ZBL) term"; formula: DESIGN.md
+ * section 2): atomic_numbers is a HOST array [n_species]; adds 1/2 sum_j phi_ij(r_ij) to every E-hat_i (not scaled by
+ * sigma) and the matching forces, phi_ij = k_e Z_i Z_j / r Phi(r / a_ij) u(r / r_cut), over all ordered pairs with
+ * r < r_cut (the flat cutoff, also when ordered pair cutoffs are set).  NULL switches the term off. */
+int allegro_set_zbl(allegro_model* m, const double* atomic_numbers);
+
+/* Per-edge energies E_ij ("E_i = sum_j E_ij", before the sigma/mu scaling and without ZBL), forward pass
+ * only: e_edge is a DEVICE array f64[n_edges of nbr], in the order of the list; candidates that are not edges
+ * (r >= the pair's cutoff) receive 0.  e_total f64[1] (device) receives the total energy as allegro_compute does. */
+int allegro_edge_energies(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                          const double box[3], const allegro_nbr* nbr, double* e_total, double* e_edge);
+
+/* One thermostatted (NVT) step ("thermostat setting of 300K"; reading: DESIGN.md section 2): a single
+ * Nose-Hoover variable, Q = g k_B T0 tau^2 with g = 3 n_atoms, split as [thermostat dt/2][allegro_step_nve][thermostat
+ * dt/2]; thermostat half step: xi += dt/4 (2K - g k_B T0)/Q; v *= exp(-xi dt/2); xi += dt/4 (2K' - g k_B T0)/Q.
+ * nh_state: DEVICE f64[2] = {xi (1/fs), eta = integral of xi dt}, zero-initialised by the caller; the conserved
+ * quantity is e_kin + e_pot + Q xi^2/2 + g k_B T0 eta.  All other arguments as allegro_step_nve; e_kin receives the
+ * kinetic energy after the final thermostat half step. */
+int allegro_step_nvt(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                     const double* mass, int64_t n_atoms, const double box[3], double dt_fs, int32_t rebuild_every,
+                     double skin, allegro_nbr** nbr, int64_t* step_counter, double* e_pot, double* e_kin,
+                     double* nh_state, double t0_K, double tau_fs);
 
 /* Debug mode (tests only; default off): keep every intermediate tensor that allegro_debug_tensor can name.
  * Without it the final latent x^{NL} is consumed inside the epilogue of the last latent GEMM and never stored. */

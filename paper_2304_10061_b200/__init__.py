@@ -73,6 +73,7 @@ EXPORTS = [
     "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
+    "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt",
     "allegro_last_error",
 ]
 
@@ -109,6 +110,10 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_step_nve.argtypes = [vp, vp, vp, vp, vp, vp, i64, P(C.c_double), C.c_double, i32, C.c_double, P(vp),
                                      P(i64), vp, vp]
     lib.allegro_step_nve_host.argtypes = lib.allegro_step_nve.argtypes
+    lib.allegro_step_nvt.argtypes = lib.allegro_step_nve.argtypes + [vp, C.c_double, C.c_double]
+    lib.allegro_edge_energies.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp]
+    lib.allegro_set_bessel_frequencies.argtypes = [vp, vp]
+    lib.allegro_set_zbl.argtypes = [vp, vp]
     lib.allegro_profile_enable.argtypes = [vp, i32]
     lib.allegro_profile_read.argtypes = [vp, C.c_char_p, P(C.c_double), P(i64)]
     lib.allegro_launch_count.argtypes = [vp, P(i64)]
@@ -263,8 +268,10 @@ class Allegro:
                                                 C.byref(nb._h)))
         return nb
 
-    def compute(self, pos, species, box: Sequence[float], nbr: NeighborList, want_atom_energies: bool = True):
-        """allegro_compute -> (e_total f64[1], e_atom f64[N] | None, force f64[N,3]) CUDA tensors."""
+    def compute(self, pos, species, box: Sequence[float], nbr: NeighborList, want_atom_energies: bool = True,
+                want_forces: bool = True):
+        """allegro_compute -> (e_total f64[1], e_atom f64[N] | None, force f64[N,3] | None) CUDA tensors.
+        want_forces=False: energy-only evaluation (no backward pass)."""
         t = self._torch
         assert pos.is_cuda and pos.dtype == t.float64 and pos.is_contiguous()
         assert species.is_cuda and species.dtype == t.int32 and species.is_contiguous()
@@ -272,10 +279,23 @@ class Allegro:
         N = pos.shape[0]
         e = t.empty(1, dtype=t.float64, device=pos.device)
         ea = t.empty(N, dtype=t.float64, device=pos.device) if want_atom_energies else None
-        f = t.empty((N, 3), dtype=t.float64, device=pos.device)
+        f = t.empty((N, 3), dtype=t.float64, device=pos.device) if want_forces else None
         self._check(self._lib.allegro_compute(self._h, pos.data_ptr(), species.data_ptr(), N, _box3(box), nbr._h,
-                                              e.data_ptr(), ea.data_ptr() if ea is not None else None, f.data_ptr()))
+                                              e.data_ptr(), ea.data_ptr() if ea is not None else None,
+                                              f.data_ptr() if f is not None else None))
         return e, ea, f
+
+    def edge_energies(self, pos, species, box: Sequence[float], nbr: NeighborList):
+        """allegro_edge_energies -> (e_total f64[1], e_edge f64[nbr.n_edges]) CUDA tensors, list order."""
+        t = self._torch
+        assert pos.is_cuda and pos.dtype == t.float64 and pos.is_contiguous()
+        assert species.is_cuda and species.dtype == t.int32 and species.is_contiguous()
+        self._sync_stream()
+        e = t.empty(1, dtype=t.float64, device=pos.device)
+        ee = t.zeros(max(nbr.n_edges, 1), dtype=t.float64, device=pos.device)
+        self._check(self._lib.allegro_edge_energies(self._h, pos.data_ptr(), species.data_ptr(), pos.shape[0], _box3(box),
+                                                    nbr._h, e.data_ptr(), ee.data_ptr()))
+        return e, ee[:nbr.n_edges]
 
     def compute_into(self, pos, species, box3, nbr: NeighborList, e, ea, f):
         """allegro_compute into preallocated tensors (no allocation: bench inner loop)."""
@@ -313,6 +333,16 @@ class Allegro:
                                                float(dt_fs), int(rebuild_every), float(skin), C.byref(nbr._h),
                                                C.byref(step_counter), e_pot.data_ptr(), e_kin.data_ptr()))
 
+    def step_nvt(self, pos, vel, force, species, mass, box, dt_fs: float, rebuild_every: int, skin: float,
+                 nbr: NeighborList, step_counter: C.c_int64, e_pot, e_kin, nh_state, t0_K: float, tau_fs: float):
+        """allegro_step_nvt (Nose-Hoover); nh_state = CUDA float64 [2] = {xi, eta}, updated in place."""
+        assert nh_state.is_cuda and nh_state.dtype == self._torch.float64 and nh_state.numel() == 2
+        self._check(self._lib.allegro_step_nvt(self._h, pos.data_ptr(), vel.data_ptr(), force.data_ptr(),
+                                               species.data_ptr(), mass.data_ptr(), pos.shape[0], _box3(box),
+                                               float(dt_fs), int(rebuild_every), float(skin), C.byref(nbr._h),
+                                               C.byref(step_counter), e_pot.data_ptr(), e_kin.data_ptr(),
+                                               nh_state.data_ptr(), float(t0_K), float(tau_fs)))
+
     def step_nve_host(self, pos, vel, force, species, mass, box, dt_fs, rebuild_every, skin, nbr, step_counter,
                       e_pot, e_kin):
         """allegro_step_nve_host: all arrays are HOST buffers (numpy arrays or pinned CPU torch tensors)."""
@@ -339,6 +369,26 @@ class Allegro:
         a = np.ascontiguousarray(rc_pair, dtype=np.float64)
         assert a.shape == (self.hp.n_species, self.hp.n_species)
         self._check(self._lib.allegro_set_pair_cutoffs(self._h, a.ctypes.data))
+
+    def set_bessel_frequencies(self, freq):
+        """Trained Bessel angular frequencies freq[Z_centre][Z_neighbour][n] in 1/A; None = n pi / r_c."""
+        import numpy as np
+        if freq is None:
+            self._check(self._lib.allegro_set_bessel_frequencies(self._h, None))
+            return
+        a = np.ascontiguousarray(freq, dtype=np.float64)
+        assert a.shape == (self.hp.n_species, self.hp.n_species, self.hp.n_bessel)
+        self._check(self._lib.allegro_set_bessel_frequencies(self._h, a.ctypes.data))
+
+    def set_zbl(self, atomic_numbers):
+        """ZBL pair repulsion with these atomic numbers per species; None = off."""
+        import numpy as np
+        if atomic_numbers is None:
+            self._check(self._lib.allegro_set_zbl(self._h, None))
+            return
+        a = np.ascontiguousarray(atomic_numbers, dtype=np.float64)
+        assert a.shape == (self.hp.n_species,)
+        self._check(self._lib.allegro_set_zbl(self._h, a.ctypes.data))
 
     def set_debug(self, on: bool = True):
         """Keep every tensor debug_tensor() can name (tests only)."""

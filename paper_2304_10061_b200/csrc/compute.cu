@@ -91,7 +91,7 @@ static GemmArgs mk(const float* A, int lda, const Dense& D, bool transposed_weig
 }
 
 static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* pos, const int32_t* species,
-                     const double box[3], const allegro_nbr* nb, double* e_atom, double* force) {
+                     const double box[3], const allegro_nbr* nb, double* e_atom, double* force, double* e_edge) {
   const allegro_hparams& hp = m->hp;
   const int d = m->d, n = m->n, nA = m->nA, NL = m->NL, ntb = hp.n_twobody, nlat = hp.n_latent;
   const int nc = (int)(ch.c1 - ch.c0);
@@ -107,7 +107,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   ga.pos = pos; ga.species = species; memcpy(ga.box, box, 24); ga.rc = hp.r_cut; ga.p = hp.poly_p; ga.NB = m->NB;
   ga.lmax = m->lmax; ga.row_ptr = (const int64_t*)nb->row_ptr.p; ga.j = (const int32_t*)nb->j.p;
   ga.shift = (const int8_t*)nb->shift.p; ga.c0 = ch.c0; ga.nc = nc;
-  ga.rc_pair = m->d_rc_pair; ga.S = m->S;
+  ga.rc_pair = m->d_rc_pair; ga.S = m->S; ga.bfreq = m->d_bfreq;
   // ---- step 2: compaction + geometry ----------------------------------------------------------------
   AL_CHECK(k_launch_active_count(m, ga, (int*)w.deg.p));
   AL_CHECK(al_exclusive_scan_i64(m, (int*)w.deg.p, (int64_t*)w.rowa.p, nc, w.scan_tmp));
@@ -158,6 +158,9 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   }
   // ---- steps 9-10: edge energy, per-atom energy (fp64) -----------------------------------------------------
   AL_CHECK(k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom));
+  if (m->d_zbl_Z) AL_CHECK(k_launch_zbl(m, ga, m->d_zbl_Z, e_atom, force));           // NEXT-4: ZBL pair repulsion
+  if (e_edge) AL_CHECK(k_launch_edge_energy_out(m, ga, w, (float*)w.XF.p, e_edge));   // NEXT-4: per-edge energies
+  if (!force) return ALLEGRO_OK;                                                       // NEXT-4: energy only
   // ---- step 11: backward -----------------------------------------------------------------------------------
   // u-bar partials: [0, n_eparts) stored by EPI_LATENT_LAST, the last one accumulated by k_bwd_prep
   AL_CUDA(m, cudaMemsetAsync((float*)w.ubar.p + (size_t)(w.n_uparts - 1) * w.cap_edges, 0, (size_t)m_cap * 4, st));
@@ -229,21 +232,21 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
 }
 
 int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t N, const double box[3],
-                    const allegro_nbr* nb, double* e_total, double* e_atom, double* force) {
-  if (!m || !pos || !species || !box || !nb || !e_total || !force) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+                    const allegro_nbr* nb, double* e_total, double* e_atom, double* force, double* e_edge) {
+  if (!m || !pos || !species || !box || !nb || !e_total) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
   if (nb->n_atoms != N) { al_set_error(m, "neighbor list was built for a different n_atoms"); return ALLEGRO_ERR_BAD_ARG; }
   if (nb->cutoff < m->hp.r_cut) { al_set_error(m, "neighbor list cutoff < r_cut"); return ALLEGRO_ERR_BAD_ARG; }
   AL_CHECK(work_reserve(m, nb, N));
   Work& w = *m->work;
   double* ea = e_atom ? e_atom : (double*)w.eatom.p;
-  AL_CHECK(k_launch_zero_f64(m, force, 3 * N));
+  if (force) AL_CHECK(k_launch_zero_f64(m, force, 3 * N));
   AL_CUDA(m, cudaMemsetAsync((int*)w.m_act.p + 2, 0, 8, m->stream));   // total active edges of this call
   for (const Chunk& ch : nb->chunks) {
     if (ch.e1 == ch.e0) {
       // no candidate edges at all: make rowa all-zero so k_energy yields mu_Z
       AL_CUDA(m, cudaMemsetAsync(w.rowa.p, 0, (size_t)(ch.c1 - ch.c0 + 1) * 8, m->stream));
     }
-    AL_CHECK(run_chunk(m, w, ch, pos, species, box, nb, ea, force));
+    AL_CHECK(run_chunk(m, w, ch, pos, species, box, nb, ea, force, e_edge));
   }
   AL_CHECK(k_launch_sum_f64(m, ea, N, e_total));
   return ALLEGRO_OK;
@@ -251,13 +254,19 @@ int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species,
 
 extern "C" int allegro_compute(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
                                const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force) {
-  return al_compute_impl(m, pos, species, n_atoms, box, nbr, e_total, e_atom, force);
+  return al_compute_impl(m, pos, species, n_atoms, box, nbr, e_total, e_atom, force, nullptr);
+}
+
+extern "C" int allegro_edge_energies(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                                     const double box[3], const allegro_nbr* nbr, double* e_total, double* e_edge) {
+  if (!e_edge) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+  return al_compute_impl(m, pos, species, n_atoms, box, nbr, e_total, nullptr, nullptr, e_edge);
 }
 
 extern "C" int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* species, int64_t N,
                                     const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom,
                                     double* force) {
-  if (!m || !pos || !species || !e_total || !force) return ALLEGRO_ERR_BAD_ARG;
+  if (!m || !pos || !species || !e_total) return ALLEGRO_ERR_BAD_ARG;
   void *dp = nullptr, *ds = nullptr, *de = nullptr, *dea = nullptr, *df = nullptr;
   int rc = ALLEGRO_OK;
   cudaStream_t st = m->stream;
@@ -266,11 +275,11 @@ extern "C" int allegro_compute_host(allegro_model* m, const double* pos, const i
     goto done;
   cudaMemcpyAsync(dp, pos, N * 24, cudaMemcpyHostToDevice, st);
   cudaMemcpyAsync(ds, species, N * 4, cudaMemcpyHostToDevice, st);
-  rc = al_compute_impl(m, (double*)dp, (int32_t*)ds, N, box, nbr, (double*)de, (double*)dea, (double*)df);
+  rc = al_compute_impl(m, (double*)dp, (int32_t*)ds, N, box, nbr, (double*)de, (double*)dea, force ? (double*)df : nullptr, nullptr);
   if (rc == ALLEGRO_OK) {
     cudaMemcpyAsync(e_total, de, 8, cudaMemcpyDeviceToHost, st);
     if (e_atom) cudaMemcpyAsync(e_atom, dea, N * 8, cudaMemcpyDeviceToHost, st);
-    cudaMemcpyAsync(force, df, N * 24, cudaMemcpyDeviceToHost, st);
+    if (force) cudaMemcpyAsync(force, df, N * 24, cudaMemcpyDeviceToHost, st);
     cudaError_t e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { al_set_error(m, cudaGetErrorString(e)); rc = ALLEGRO_ERR_CUDA; }
     else {
@@ -305,10 +314,27 @@ extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, doub
   AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, true));
   if (*nbr == nullptr || (*step_counter % rebuild_every) == 0)
     AL_CHECK(al_neighbors_impl(m, pos, N, box, m->hp.r_cut + skin, nbr));
-  AL_CHECK(al_compute_impl(m, pos, species, N, box, *nbr, e_pot, nullptr, force));
+  AL_CHECK(al_compute_impl(m, pos, species, N, box, *nbr, e_pot, nullptr, force, nullptr));
   AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, false));
   AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, m->work->scan_tmp));
   (*step_counter)++;
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_step_nvt(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                                const double* mass, int64_t N, const double box[3], double dt_fs, int32_t rebuild_every,
+                                double skin, allegro_nbr** nbr, int64_t* step_counter, double* e_pot, double* e_kin,
+                                double* nh_state, double t0_K, double tau_fs) {
+  if (!m || !vel || !species || !mass || !e_kin || !nh_state) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+  if (!(t0_K > 0) || !(tau_fs > 0) || N < 1) { al_set_error(m, "t0_K > 0, tau_fs > 0, n_atoms >= 1 required"); return ALLEGRO_ERR_BAD_ARG; }
+  static thread_local DevBuf tmp, scal;
+  AL_CHECK(al_reserve(m, scal, 64));
+  const double g = 3.0 * (double)N;
+  // [thermostat dt/2] [velocity-Verlet NVE step] [thermostat dt/2]
+  AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, tmp));
+  AL_CHECK(k_launch_nh_half(m, vel, N, nh_state, e_kin, g, t0_K, tau_fs, dt_fs, (double*)scal.p));
+  AL_CHECK(allegro_step_nve(m, pos, vel, force, species, mass, N, box, dt_fs, rebuild_every, skin, nbr, step_counter, e_pot, e_kin));
+  AL_CHECK(k_launch_nh_half(m, vel, N, nh_state, e_kin, g, t0_K, tau_fs, dt_fs, (double*)scal.p));
   return ALLEGRO_OK;
 }
 

@@ -133,17 +133,31 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
       double uu = 1.0 - 0.5 * (p + 1.0) * (p + 2.0) * xp + p * (p + 2.0) * xp * x - 0.5 * p * (p + 1.0) * xp * x * x;
       double dud = -0.5 * p * (p + 1.0) * (p + 2.0) * xp1 * (1.0 - x) * (1.0 - x) / rc;
       u[o] = (float)uu; du[o] = (float)dud;
-      // Bessel basis by the angle-addition recurrence in fp64
-      double th = M_PI * x, s1, c1;
-      sincos(th, &s1, &c1);
-      double sn = s1, cn = c1, pref = sqrt(2.0 / rc);
-      for (int nb = 1; nb <= a.NB; ++nb) {
-        double bn = pref * sn * inv;
-        double dbn = pref * ((double)nb * M_PI / rc * cn * inv - sn * inv * inv);
-        B[o * a.NB + nb - 1] = (float)(bn * uu);
-        dB[o * a.NB + nb - 1] = (float)(dbn * uu + bn * dud);
-        double s2 = sn * c1 + cn * s1, c2 = cn * c1 - sn * s1;
-        sn = s2; cn = c2;
+      double pref = sqrt(2.0 / rc);
+      if (a.bfreq) {
+        // trained per-ordered-pair angular frequencies w_n: b_n = sqrt(2/rc) sin(w_n r) / r
+        const double* wq = a.bfreq + ((size_t)a.species[i] * a.S + a.species[j]) * a.NB;
+        for (int nb = 0; nb < a.NB; ++nb) {
+          double wn = wq[nb], sn, cn;
+          sincos(wn * r, &sn, &cn);
+          double bn = pref * sn * inv;
+          double dbn = pref * (wn * cn * inv - sn * inv * inv);
+          B[o * a.NB + nb] = (float)(bn * uu);
+          dB[o * a.NB + nb] = (float)(dbn * uu + bn * dud);
+        }
+      } else {
+        // Bessel basis by the angle-addition recurrence in fp64
+        double th = M_PI * x, s1, c1;
+        sincos(th, &s1, &c1);
+        double sn = s1, cn = c1;
+        for (int nb = 1; nb <= a.NB; ++nb) {
+          double bn = pref * sn * inv;
+          double dbn = pref * ((double)nb * M_PI / rc * cn * inv - sn * inv * inv);
+          B[o * a.NB + nb - 1] = (float)(bn * uu);
+          dB[o * a.NB + nb - 1] = (float)(dbn * uu + bn * dud);
+          double s2 = sn * c1 + cn * s1, c2 = cn * c1 - sn * s1;
+          sn = s2; cn = c2;
+        }
       }
       float yy[16];
       sph_harm(hx, hy, hz, a.lmax, yy);
@@ -571,6 +585,92 @@ __global__ void k_nve(double* pos, double* vel, const double* force, const int32
   }
 }
 
+// ---- ZBL pair repulsion (reading in DESIGN.md section 2) -------------------------------------------
+// phi_ij(r) = k_e Z_i Z_j / r * Phi(r / a_ij) * u(r / r_c) at the FLAT cutoff; E_i += 1/2 sum_j phi_ij and, since the
+// list holds both orders of every pair, F_i = sum_j phi'(r_ij) rhat_ij is a pure gather over the centre's own row.
+__global__ void k_zbl(EdgeGeomArgs a, const double* __restrict__ zn, double* __restrict__ e_atom, double* __restrict__ force) {
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= a.nc) return;
+  int i = (int)(a.c0 + warp);
+  int64_t b = a.row_ptr[i], e = a.row_ptr[i + 1];
+  const double zi = zn[a.species[i]], p = (double)a.p;
+  double es = 0.0, fx = 0.0, fy = 0.0, fz = 0.0;
+  for (int64_t k = b + lane; k < e; k += 32) {
+    int j = a.j[k];
+    double dx = (a.pos[3 * (int64_t)j + 0] - a.pos[3 * (int64_t)i + 0]) + (double)a.shift[3 * k + 0] * a.box[0];
+    double dy = (a.pos[3 * (int64_t)j + 1] - a.pos[3 * (int64_t)i + 1]) + (double)a.shift[3 * k + 1] * a.box[1];
+    double dz = (a.pos[3 * (int64_t)j + 2] - a.pos[3 * (int64_t)i + 2]) + (double)a.shift[3 * k + 2] * a.box[2];
+    double r2 = dx * dx + dy * dy + dz * dz;
+    if (!(r2 < a.rc * a.rc) || !(r2 > 0.0)) continue;
+    double r = sqrt(r2), inv = 1.0 / r;
+    double zj = zn[a.species[j]];
+    double ia = (pow(zi, 0.23) + pow(zj, 0.23)) / 0.46850, xs = r * ia;
+    double e1 = 0.18175 * exp(-3.19980 * xs), e2 = 0.50986 * exp(-0.94229 * xs), e3 = 0.28022 * exp(-0.40290 * xs),
+           e4 = 0.02817 * exp(-0.20162 * xs);
+    double Phi = e1 + e2 + e3 + e4;
+    double dPhi = -(3.19980 * e1 + 0.94229 * e2 + 0.40290 * e3 + 0.20162 * e4) * ia;
+    double x = r / a.rc;
+    double xp1 = pow(x, p - 1.0), xp = xp1 * x;
+    double uu = 1.0 - 0.5 * (p + 1.0) * (p + 2.0) * xp + p * (p + 2.0) * xp * x - 0.5 * p * (p + 1.0) * xp * x * x;
+    double dud = -0.5 * p * (p + 1.0) * (p + 2.0) * xp1 * (1.0 - x) * (1.0 - x) / a.rc;
+    double c = 14.399645478425668 * zi * zj;
+    double phi = c * inv * Phi * uu;
+    double dphi = c * (-inv * inv * Phi * uu + inv * dPhi * uu + inv * Phi * dud);
+    es += 0.5 * phi;
+    fx += dphi * dx * inv; fy += dphi * dy * inv; fz += dphi * dz * inv;
+  }
+  es = warp_sum_d(es); fx = warp_sum_d(fx); fy = warp_sum_d(fy); fz = warp_sum_d(fz);
+  if (lane == 0) {
+    e_atom[i] += es;                     // this warp is the only writer of atom i in this kernel
+    if (force) { force[3 * (int64_t)i] += fx; force[3 * (int64_t)i + 1] += fy; force[3 * (int64_t)i + 2] += fz; }
+  }
+}
+
+// ---- per-edge energies in candidate order: redo the compaction walk of k_geom_fill, E_ij = sum of the fp64 partials
+__global__ void k_edge_energy_out(EdgeGeomArgs a, const int64_t* __restrict__ rowa, const double* __restrict__ epart,
+                                  int nparts, int64_t pstride, const float* __restrict__ xf, int d,
+                                  const double* __restrict__ w_eff, double* __restrict__ e_edge) {
+  int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (warp >= a.nc) return;
+  int i = (int)(a.c0 + warp);
+  int64_t b = a.row_ptr[i], e = a.row_ptr[i + 1];
+  int64_t out0 = rowa[warp];
+  int cnt = 0;
+  for (int64_t kb = b; kb < e; kb += 32) {
+    int64_t k = kb + lane;
+    int j = 0; double dx = 0, dy = 0, dz = 0, r2 = 0, rc = a.rc;
+    bool ok = (k < e) && edge_vec(a, i, k, j, dx, dy, dz, r2, rc);
+    unsigned mask = __ballot_sync(FULLMASK, ok);
+    if (k < e) {
+      double v = 0.0;
+      if (ok) {
+        int64_t o = out0 + cnt + __popc(mask & ((1u << lane) - 1u));
+        if (nparts > 0) for (int q = 0; q < nparts; ++q) v += epart[(int64_t)q * pstride + o];
+        else for (int q = 0; q < d; ++q) v += (double)xf[o * d + q] * w_eff[q];
+      }
+      e_edge[k] = v;
+    }
+    cnt += __popc(mask);
+  }
+}
+
+// ---- Nose-Hoover thermostat half step (reading in DESIGN.md section 2) ----------------------------
+// st = {xi, eta}; scratch[0] receives the velocity scale s = exp(-xi dt/2); e_kin *= s^2.
+__global__ void k_nh_scalar(double* st, double* e_kin, double n_dof, double t0, double tau, double dt, double* scratch) {
+  const double gkt = n_dof * 8.617333262e-5 * t0, Q = gkt * tau * tau;
+  double xi = st[0], K = *e_kin;
+  xi = xi + 0.25 * dt * (2.0 * K - gkt) / Q;
+  double s = exp(-xi * 0.5 * dt);
+  st[1] = st[1] + xi * 0.5 * dt;
+  K = K * s * s;
+  xi = xi + 0.25 * dt * (2.0 * K - gkt) / Q;
+  st[0] = xi; *e_kin = K; scratch[0] = s;
+}
+__global__ void k_scale_vel(double* vel, int64_t n3, const double* __restrict__ s) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (i < n3) vel[i] *= s[0];
+}
+
 __global__ void k_kin(const double* vel, const int32_t* species, const double* mass, int64_t n, double* out) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -772,4 +872,34 @@ int k_launch_kinetic(allegro_model* m, const double* vel, const int32_t* species
     LAUNCH_CHECK(m);
   }
   return k_launch_sum_f64(m, (double*)tmp.p, n, e_kin);
+}
+
+
+int k_launch_zbl(allegro_model* m, const EdgeGeomArgs& a, const double* zbl_Z, double* e_atom, double* force) {
+  ProfScope _ps(m, PC_ENERGY);
+  if (a.nc <= 0) return ALLEGRO_OK;
+  k_zbl<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, zbl_Z, e_atom, force);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_edge_energy_out(allegro_model* m, const EdgeGeomArgs& a, Work& w, const float* xf, double* e_edge) {
+  ProfScope _ps(m, PC_ENERGY);
+  if (a.nc <= 0) return ALLEGRO_OK;
+  k_edge_energy_out<<<(a.nc * 32 + 255) / 256, 256, 0, m->stream>>>(a, (const int64_t*)w.rowa.p, (const double*)w.epart.p,
+                                                                 w.n_eparts, (int64_t)w.cap_edges, xf, m->d, m->w_eff_d, e_edge);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
+int k_launch_nh_half(allegro_model* m, double* vel, int64_t n, double* nh_state, double* e_kin, double n_dof, double t0_K,
+                     double tau_fs, double dt_fs, double* scratch) {
+  ProfScope _ps(m, PC_NVE);
+  k_nh_scalar<<<1, 1, 0, m->stream>>>(nh_state, e_kin, n_dof, t0_K, tau_fs, dt_fs, scratch);
+  LAUNCH_CHECK(m);
+  if (n > 0) {
+    k_scale_vel<<<(unsigned)((3 * n + 255) / 256), 256, 0, m->stream>>>(vel, 3 * n, scratch);
+    LAUNCH_CHECK(m);
+  }
+  return ALLEGRO_OK;
 }

@@ -107,6 +107,8 @@ struct allegro_model {
   float* w_eff_f = nullptr; double* w_eff_d = nullptr;   // product of the edge-MLP layers, [d]
   double *sigma = nullptr, *mu = nullptr; // device [S]
   double* d_rc_pair = nullptr;            // device [S][S] ordered species-pair cutoffs, or null (flat r_cut)
+  double* d_bfreq = nullptr;              // device [S][S][NB] trained Bessel angular frequencies, or null (n pi / r_c)
+  double* d_zbl_Z = nullptr;              // device [S] atomic numbers: ZBL pair repulsion on, or null
   std::vector<double> sigma_h, mu_h;
   float c_env; float c_old[AL_MAX_LAYERS], c_new[AL_MAX_LAYERS];
   // runtime
@@ -149,6 +151,7 @@ void al_enumerate(int lmax, int NL, std::vector<std::vector<Irrep>>& S,
 int al_neighbors_impl(allegro_model* m, const double* pos, int64_t n_atoms, const double box[3], double cutoff,
                       allegro_nbr** inout);
 int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
-                    const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force);
+                    const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force /*null: energy only*/,
+                    double* e_edge /*null or f64[nbr->n_edges]*/);
 int al_exclusive_scan_i64(allegro_model* m, const int32_t* in, int64_t* out, int64_t n, DevBuf& tmp);  // out[n] = total
 void al_work_free(allegro_model* m);

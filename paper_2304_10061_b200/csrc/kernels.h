@@ -39,6 +39,7 @@ struct Work {
 struct EdgeGeomArgs {
   const double* pos; const int32_t* species; double box[3]; double rc; int p; int NB; int lmax;
   const double* rc_pair; int S;                                     // ordered species-pair cutoffs [S][S] or null
+  const double* bfreq;                                              // Bessel angular frequencies [S][S][NB] or null
   const int64_t* row_ptr; const int32_t* j; const int8_t* shift;   // candidate list (global)
   int64_t c0; int nc;                                               // centers [c0, c0+nc)
 };
@@ -64,6 +65,13 @@ int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, con
 int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, const Dense& L0, bool single,
                       double* force, int m_cap);
 int k_launch_zero_f64(allegro_model* m, double* p, int64_t n);
+// ZBL pair repulsion over the candidate rows of the chunk's centres: e_atom[i] += 1/2 sum phi, force[i] += sum phi' rhat
+int k_launch_zbl(allegro_model* m, const EdgeGeomArgs& a, const double* zbl_Z, double* e_atom, double* force);
+// per-edge energies E_ij in candidate-list order (0 for dropped candidates)
+int k_launch_edge_energy_out(allegro_model* m, const EdgeGeomArgs& a, Work& w, const float* xf, double* e_edge);
+// Nose-Hoover thermostat half step on device scalars, then v *= s
+int k_launch_nh_half(allegro_model* m, double* vel, int64_t n, double* nh_state, double* e_kin, double n_dof, double t0_K,
+                     double tau_fs, double dt_fs, double* scratch);
 int k_launch_nve_kick_drift(allegro_model* m, double* pos, double* vel, const double* force, const int32_t* species,
                             const double* mass, int64_t n, double dt, bool drift);
 int k_launch_kinetic(allegro_model* m, const double* vel, const int32_t* species, const double* mass, int64_t n,

@@ -326,6 +326,33 @@ extern "C" int allegro_set_pair_cutoffs(allegro_model* m, const double* rc_pair)
   return ALLEGRO_OK;
 }
 
+extern "C" int allegro_set_bessel_frequencies(allegro_model* m, const double* freq) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  if (!freq) { m->d_bfreq = nullptr; return ALLEGRO_OK; }
+  const size_t cnt = (size_t)m->S * m->S * m->NB;
+  for (size_t k = 0; k < cnt; ++k)
+    if (!(freq[k] > 0) || !std::isfinite(freq[k])) { al_set_error(m, "Bessel frequencies must be finite and > 0"); return ALLEGRO_ERR_BAD_HPARAMS; }
+  std::vector<double> h(freq, freq + cnt);
+  double* d = nullptr;
+  AL_CHECK(upload(m, &d, h));
+  m->d_bfreq = d;
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_set_zbl(allegro_model* m, const double* atomic_numbers) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  if (!atomic_numbers) { m->d_zbl_Z = nullptr; return ALLEGRO_OK; }
+  for (int k = 0; k < m->S; ++k)
+    if (!(atomic_numbers[k] > 0) || !std::isfinite(atomic_numbers[k])) { al_set_error(m, "atomic numbers must be > 0"); return ALLEGRO_ERR_BAD_HPARAMS; }
+  std::vector<double> h(atomic_numbers, atomic_numbers + m->S);
+  double* d = nullptr;
+  AL_CHECK(upload(m, &d, h));
+  m->d_zbl_Z = d;
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_set_debug(allegro_model* m, int on) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   m->debug_keep = on != 0;

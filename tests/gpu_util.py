@@ -17,6 +17,10 @@ def make_both(cfg, precision=0, sigma=None, chunk_edges=None):
     model = P.Allegro(chp, blob, chunk_edges=chunk_edges)
     if getattr(hp, "r_cut_pair", None) is not None:
         model.set_pair_cutoffs(hp.r_cut_pair)
+    if getattr(hp, "bessel_freq_pair", None) is not None:
+        model.set_bessel_frequencies(hp.bessel_freq_pair)
+    if getattr(hp, "zbl_Z", None) is not None:
+        model.set_zbl(hp.zbl_Z)
     oracle = O.OracleModel(hp, blob)
     return model, oracle
 
