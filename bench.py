@@ -43,11 +43,12 @@ def gemm_macs_per_edge(hp):
     return fwd + bwd
 
 
-def gemm_bytes_per_edge(hp):
+def gemm_bytes_per_edge(hp, kcat=True):
     """Algorithmic HBM bytes per ACTIVE edge of the GEMM kernel group (fp32 storage): every launch reads its A
     operand once and writes its outputs once; aux operands of the fused epilogues are read once.  Weights are
     L2-resident and not counted.  Mirrors the launch list of csrc/compute.cu::run_chunk (default path: last latent
-    layer fused with the energy / z-bar epilogue, z-bar prep stage fused into the x-bar GEMMs)."""
+    layer fused with the energy / z-bar epilogue, z-bar prep stage fused into the x-bar GEMMs, and -- kcat, the tensor-core
+    modes -- the x-bar part of the first latent layer's dX folded into the x-bar GEMM by K-concatenation)."""
     d, n, nA, NL = hp.twobody_dims[-1], hp.n_tensor, hp.n_tensor * (hp.l_max + 1), hp.n_layers
     tb, lat = list(hp.twobody_dims), list(hp.latent_dims)
     parts = 12.0 * ((d + 31) // 32) / 4.0             # fp64 energy + fp32 u-bar partial per 32 columns, in floats
@@ -68,11 +69,17 @@ def gemm_bytes_per_edge(hp):
     for L in range(NL, 0, -1):                        # backward
         for k in range(len(lat) - 1, 0, -1):
             fl += lat[k] + 2 * lat[k - 1]             # A, aux z, C
-        fl += lat[0] + (d + n)                        # dX of the first latent layer -> [x-bar part | s-bar]
         Kx = 2 * nA if L == 1 else nA
-        # x-bar GEMM + prep stage: A, aux2 (+ aux1 unless rank-1), z of the MLP below, z-bar out, u-bar partials,
-        # C = x-bar (not stored for L = 1)
-        fl += Kx + d + (0 if L == NL else d) + d + d + parts / 3.0 + (d if L > 1 else 0)
+        if kcat:
+            # s-bar GEMM: A = z-bar, C = s-bar only; then ONE x-bar GEMM over the concatenated K axis [z-bar | omega-bar]
+            # (+ prep stage): A, aux1 unless rank-1, z of the MLP below, z-bar out, u-bar partials, C = x-bar (not for L = 1)
+            fl += lat[0] + n
+            fl += (lat[0] + Kx) + (0 if L == NL else d) + d + d + parts / 3.0 + (d if L > 1 else 0)
+        else:
+            fl += lat[0] + (d + n)                    # dX of the first latent layer -> [x-bar part | s-bar]
+            # x-bar GEMM + prep stage: A, aux2 (+ aux1 unless rank-1), z of the MLP below, z-bar out, u-bar partials,
+            # C = x-bar (not stored for L = 1)
+            fl += Kx + d + (0 if L == NL else d) + d + d + parts / 3.0 + (d if L > 1 else 0)
     for k in range(len(tb) - 1, 0, -1):
         fl += tb[k] + 2 * tb[k - 1]
     return 4.0 * fl
@@ -311,11 +318,14 @@ def main():
     else:
         peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16, "tensor"
         peak_note = f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16}"
-    gemm_gbs = gemm_bytes_per_edge(cfg.hp) * n_active * K / (gemm_ms * 1e-3) / 1e9 if gemm_ms > 0 else 0.0
+    # K-concatenated x-bar GEMM: tensor-core modes with a 32-multiple first latent width, unless switched off
+    kcat = args.precision != 3 and cfg.hp.latent_dims[0] % 32 == 0 and not os.environ.get("B200_ALLEGRO_NO_KCAT") \
+        and not os.environ.get("B200_ALLEGRO_FP32_SIMT")
+    gemm_gbs = gemm_bytes_per_edge(cfg.hp, kcat) * n_active * K / (gemm_ms * 1e-3) / 1e9 if gemm_ms > 0 else 0.0
     f_compute, f_hbm = gemm_tflops / peak, gemm_gbs / pk["hbm_gbs"]
     comp = {"bound": bound, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s", "frac": f_compute, "peak_note": peak_note}
     hbm = {"bound": "hbm", "achieved": gemm_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm,
-           "peak_note": f"copy bandwidth ({pk['src']}); algorithmic bytes = {gemm_bytes_per_edge(cfg.hp)} B per active edge"}
+           "peak_note": f"copy bandwidth ({pk['src']}); algorithmic bytes = {gemm_bytes_per_edge(cfg.hp, kcat)} B per active edge"}
     top = hbm if f_hbm > f_compute else comp       # the binding roofline is the one with the larger fraction
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
@@ -325,7 +335,7 @@ def main():
             traffic = tj["gemm_dram_bytes_per_launch"]
     roofline = {"bound": top["bound"], "kernel": {0: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., SPLIT> (3xTF32)", 1: "MLP GEMM group (fwd+bwd), k_gemm_tf32", 2: "MLP GEMM group (fwd+bwd), k_gemm_tf32", 3: "MLP GEMM group (fwd+bwd), k_gemm_simt"}[args.precision],
                 "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"], "traffic": traffic,
-                "algorithmic_bytes_per_launch": gemm_bytes_per_edge(cfg.hp) * n_active * K / max(gemm_n, 1),
+                "algorithmic_bytes_per_launch": gemm_bytes_per_edge(cfg.hp, kcat) * n_active * K / max(gemm_n, 1),
                 "peak_note": top["peak_note"], "compute_roofline": comp, "hbm_roofline": hbm,
                 "launches_per_step": gemm_n / K, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
                 "share_of_step": gemm_ms / tot_prof if tot_prof else None,

@@ -178,8 +178,13 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   static const bool no_prep = getenv("B200_ALLEGRO_NO_PREP") != nullptr;   // experiment switch: keep k_bwd_prep for L < NL
   const bool fuse_prep = fused_last && !no_prep;
   int prep_slot = 1;
+  // K-concatenated x-bar GEMM (tensor-core kernels): x-bar^{L-1} = [z-bar | omega-bar] [W_x | A]^T in one launch, so
+  // the x-bar part of dX of the first latent layer never goes through HBM; s-bar comes from its own N = n GEMM.
+  static const bool no_kcat = getenv("B200_ALLEGRO_NO_KCAT") != nullptr;
+  const bool kcat = !no_kcat && al_gemm_supports_kcat(m) && (hp.latent_dims[0] % 32 == 0);
+  float* zstart = (float*)w.ZB0.p;   // where the z-bar entering the next MLP to differentiate lives
   for (int L = NL; L >= 1; --L) {
-    float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
+    float* zb = zstart; float* zb_o = (zstart == (float*)w.ZB0.p) ? (float*)w.ZB1.p : (float*)w.ZB0.p;
     if (!zb_ready)
       AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
     for (int k = nlat - 1; k >= 1; --k) {
@@ -188,7 +193,10 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       AL_CHECK(al_gemm(m, g));
       std::swap(zb, zb_o);
     }
-    AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->latent[L - 1][0], true, (float*)w.G.p, d + n, m_cap, mp, EPI_PLAIN)));
+    if (kcat)   // s-bar only: [M, h] x W_lat0[d:, :]^T -> G[:, d:]
+      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->sbar[L - 1], true, (float*)w.G.p + d, d + n, m_cap, mp, EPI_PLAIN)));
+    else
+      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->latent[L - 1][0], true, (float*)w.G.p, d + n, m_cap, mp, EPI_PLAIN)));
     const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
     int ldo = (L == 1) ? 2 * nA : nA;
     const float* Vin = (L == 1) ? nullptr : (float*)w.T[L - 1].p;
@@ -202,11 +210,20 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
                     rank1 ? EPI_ADD2R : EPI_ADD2);
     g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = (float*)w.G.p; g.ld2 = d + n;
     g.u = (float*)w.sig.p; g.aux3 = m->w_eff_f;
+    if (kcat) {
+      const int h = hp.latent_dims[0];
+      GemmArgs gc = mk(zb, h, m->xcat[L - 1], true, xb_o, d, m_cap, mp, g.epi);
+      gc.A2 = (float*)w.OB.p; gc.lda2 = ldob; gc.K1 = h;
+      gc.aux1 = g.aux1; gc.ld1 = g.ld1; gc.c0 = g.c0; gc.aux2 = nullptr; gc.ld2 = 0; gc.u = g.u; gc.aux3 = g.aux3;
+      g = gc;
+    }
+    // the prep stage must not overwrite the z-bar this GEMM still reads as its A operand (kcat): use the other buffer
+    float* zb_next = (zb == (float*)w.ZB0.p) ? (float*)w.ZB1.p : (float*)w.ZB0.p;
     if (fuse_prep) {
       // prep stage: z-bar of the MLP below (latent MLP of layer L-1, or the two-body MLP when L = 1)
       g.prep = 1;
       g.zp = (L > 1) ? (float*)w.lat_z[L - 2][nlat - 1].p : (float*)w.tb_z[ntb - 1].p; g.ldzp = d;
-      g.zbp = (float*)w.ZB0.p; g.ldzbp = d; g.pu = (float*)w.u.p; g.cp = (L > 1) ? m->c_new[L - 2] : 1.0f;
+      g.zbp = zb_next; g.ldzbp = d; g.pu = (float*)w.u.p; g.cp = (L > 1) ? m->c_new[L - 2] : 1.0f;
       g.upart = (float*)w.ubar.p; g.part_stride = w.cap_edges; g.pbase = prep_slot * w.n_eparts;
       ++prep_slot;
       if (L == 1 && !m->debug_keep) g.C = nullptr;   // x-bar^0 itself is not needed afterwards
@@ -215,9 +232,10 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     std::swap(xb, xb_o);
     rank1 = false;
     zb_ready = fuse_prep;
+    zstart = fuse_prep ? zb_next : (float*)w.ZB0.p;
   }
   {
-    float* zb = (float*)w.ZB0.p; float* zb_o = (float*)w.ZB1.p;
+    float* zb = zstart; float* zb_o = (zstart == (float*)w.ZB0.p) ? (float*)w.ZB1.p : (float*)w.ZB0.p;
     if (!zb_ready)
       AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.tb_z[ntb - 1].p, d, 1.0f, zb, d, d, m_cap));
     for (int k = ntb - 1; k >= 1; --k) {

@@ -25,6 +25,9 @@ enum GemmEpi {
 
 struct GemmArgs {
   const float* A; int lda;
+  // Optional K-concatenation of two activation tensors (tensor-core kernels only): columns [0, K1) of the A operand
+  // come from A, columns [K1, K) from A2 (row stride lda2); K1 must be a multiple of 32.  A2 = null: plain A.
+  const float* A2; int lda2; int K1;
   const float* Bt; int ldb;       // fp32 weights [N][K]
   const void* Bt16;               // bf16 weights [N][K] (precision 2) or null
   const float *Bt_hi, *Bt_lo;     // TF32-exact / remainder split of Bt (precision 0 on tensor cores) or null
@@ -53,3 +56,5 @@ struct GemmArgs {
 int al_gemm(struct allegro_model* m, const GemmArgs& g);
 // number of 32-column row partials the EPI_LATENT_LAST epilogue of the active GEMM kernel writes for N columns
 int al_gemm_row_parts(const struct allegro_model* m, int N);
+// true when al_gemm runs a kernel that honours GemmArgs::A2 (the tcgen05 kernels)
+bool al_gemm_supports_kcat(const struct allegro_model* m);

@@ -193,9 +193,15 @@ int al_gemm_row_parts(const allegro_model* m, int N) {
   return al_gemm_tc_row_parts(N, m->hp.precision == 0);
 }
 
+bool al_gemm_supports_kcat(const allegro_model* m) { return !fp32_simt(m); }
+
 int al_gemm(allegro_model* m, const GemmArgs& g) {
   ProfScope _ps(m, PC_GEMM);
   if (g.m_cap <= 0) return ALLEGRO_OK;
+  if (g.A2 && (fp32_simt(m) || (g.K1 & 31) || g.K1 <= 0 || g.K1 >= g.K || (g.lda2 & 3))) {
+    al_set_error(m, "gemm: K-concatenated A needs a tensor-core mode and K1 % 32 == 0");
+    return ALLEGRO_ERR_BAD_HPARAMS;
+  }
   if ((g.K & 3) || (g.N & 3) || (g.lda & 3) || (g.ldb & 3) || (g.ldc & 3)) {
     al_set_error(m, "gemm: dimensions must be multiples of 4");
     return ALLEGRO_ERR_BAD_HPARAMS;

@@ -121,8 +121,8 @@ __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__fl
 
 template <int AST, int BST, int EPI_WARPS, bool SPLIT>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
-k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-            const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
+k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
+            const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
   constexpr int BN_MAX = bn_max(SPLIT);
   constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT);
   constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT);
@@ -173,12 +173,14 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // ===== TMA producer, A ring =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
+      const int kb1 = g.A2 ? g.K1 / BKF : num_kb;   // k-blocks [kb1, num_kb) come from the second activation tensor
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         int mt = tile / ntn;
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyA[stage], phase ^ 1);
           mbar_expect_tx(&fullA[stage], A_STAGE_BYTES);
-          tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKF, mt * BM);
+          if (kb < kb1) tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKF, mt * BM);
+          else tma_load_2d(sA(stage), &tmA2, &fullA[stage], (kb - kb1) * BKF, mt * BM);
           if (++stage == AST) { stage = 0; phase ^= 1; }
         }
       }
@@ -288,7 +290,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         // Two halves of 16 rows: issue every aux load of a half up front (the stores below may alias, so the compiler
         // cannot hoist them), then process it.  Halving keeps the register count low enough for 16 epilogue warps.
         const bool need1 = (g.epi == EPI_LATENT || g.epi == EPI_LATENT_LAST || g.epi == EPI_MUL_DSILU || g.epi == EPI_ADD2);
-        const bool need2 = (g.epi == EPI_ADD2 || g.epi == EPI_ADD2R);
+        const bool need2 = (g.epi == EPI_ADD2 || g.epi == EPI_ADD2R) && g.aux2 != nullptr;   // null: the term is in the K-concatenation
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
         float4 ax1[4], ax2[4], ax3[4];
@@ -493,15 +495,17 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
                                       (int)smem_bytes(AS, BS, EW, SP)));                                                 \
       attr_set = true;                                                                                                   \
     }                                                                                                                    \
-    k_gemm_tf32<AS, BS, EW, SP><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>(tmA, tmB, tmB2, g, BN, ntn); \
+    k_gemm_tf32<AS, BS, EW, SP><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>(tmA, tmA2, tmB, tmB2, g, BN, ntn); \
   }
 
 // precision 1: TF32 operands (rounded to nearest by the TMA load), fp32 accumulation
 int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
   int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
   int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
-  CUtensorMap tmA, tmB, tmB2;
-  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, false, &tmA));
+  CUtensorMap tmA, tmA2, tmB, tmB2;
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, false, &tmA));
+  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, false, &tmA2));
+  else tmA2 = tmA;
   AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, false, &tmB));
   tmB2 = tmB;
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
@@ -520,8 +524,10 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g) {
   if (!g.Bt_hi || !g.Bt_lo) { al_set_error(m, "3xTF32 GEMM: split weights missing"); return ALLEGRO_ERR_BAD_ARG; }
   int ntn = (g.N + bn_max(true) - 1) / bn_max(true);
   int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
-  CUtensorMap tmA, tmB, tmB2;
-  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.K, g.lda, BM, true, &tmA));
+  CUtensorMap tmA, tmA2, tmB, tmB2;
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, true, &tmA));
+  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, true, &tmA2));
+  else tmA2 = tmA;
   AL_CHECK(get_tmap(m, g.Bt_hi, g.N, g.K, g.ldb, BN, true, &tmB));
   AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, true, &tmB2));
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;

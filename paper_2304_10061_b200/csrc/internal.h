@@ -104,6 +104,9 @@ struct allegro_model {
   Dense emb01;                            // [A0 | A1] : d -> 2 nA, columns permuted to (l, n)
   std::vector<Dense> emb;                 // emb[L] = A^{L+1} for L >= 1 (index 0 unused)
   std::vector<std::vector<Dense>> latent; // [NL][n_latent]
+  // backward of layer L: x-bar^{L-1} = z-bar W_x^T + omega-bar A^T as ONE GEMM over the concatenated K axis,
+  // xcat[L-1].W = [W_lat0[:d, :] | A] ([d][h + Kx]); sbar[L-1].W = W_lat0[d:, :] ([n][h]) gives s-bar alone
+  std::vector<Dense> xcat, sbar;
   float* w_eff_f = nullptr; double* w_eff_d = nullptr;   // product of the edge-MLP layers, [d]
   double *sigma = nullptr, *mu = nullptr; // device [S]
   double* d_rc_pair = nullptr;            // device [S][S] ordered species-pair cutoffs, or null (flat r_cut)

@@ -212,6 +212,8 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
   n_paths_of(hp, npaths);
   m->emb.resize(m->NL + 1);
   m->latent.resize(m->NL);
+  m->xcat.resize(m->NL); m->sbar.resize(m->NL);
+  std::vector<float> A01_keep;
   for (int L = 1; L <= m->NL; ++L) {
     std::vector<float> AL = permute(take((size_t)m->d * m->nA));
     alphas[L - 1] = take(npaths[L - 1]);
@@ -222,6 +224,7 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
         memcpy(&A01[(size_t)r * 2 * m->nA + m->nA], &AL[(size_t)r * m->nA], m->nA * 4);
       }
       if ((rc = upload_dense(m, m->emb01, A01, m->d, 2 * m->nA))) return fail(rc);
+      A01_keep = A01;
     } else {
       if ((rc = upload_dense(m, m->emb[L - 1], AL, m->d, m->nA))) return fail(rc);
     }
@@ -229,7 +232,21 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
     m->latent[L - 1].resize(hp->n_latent);
     for (int k = 0; k < hp->n_latent; ++k) {
       int fo = hp->latent_dims[k];
-      if ((rc = upload_dense(m, m->latent[L - 1][k], take((size_t)fi * fo), fi, fo))) return fail(rc);
+      std::vector<float> Wk = take((size_t)fi * fo);
+      if ((rc = upload_dense(m, m->latent[L - 1][k], Wk, fi, fo))) return fail(rc);
+      if (k == 0) {
+        // K-concatenated weights of the x-bar GEMM and the s-bar rows (see internal.h)
+        const std::vector<float>& Ae = (L == 1) ? A01_keep : AL;
+        const int Kx = (L == 1) ? 2 * m->nA : m->nA, h = fo, d = m->d;
+        std::vector<float> cat((size_t)d * (h + Kx)), sb((size_t)m->n * h);
+        for (int r = 0; r < d; ++r) {
+          memcpy(&cat[(size_t)r * (h + Kx)], &Wk[(size_t)r * h], (size_t)h * 4);
+          memcpy(&cat[(size_t)r * (h + Kx) + h], &Ae[(size_t)r * Kx], (size_t)Kx * 4);
+        }
+        memcpy(sb.data(), &Wk[(size_t)d * h], (size_t)m->n * h * 4);
+        if ((rc = upload_dense(m, m->xcat[L - 1], cat, d, h + Kx))) return fail(rc);
+        if ((rc = upload_dense(m, m->sbar[L - 1], sb, m->n, h))) return fail(rc);
+      }
       fi = fo;
     }
   }

@@ -43,6 +43,9 @@ CASES = [
     ("gemm_rings_6_2_tf32", {"B200_ALLEGRO_GEMM_VARIANT": "1"}, 2, 3000, 1),       # other TMA ring depths
     ("gemm3_rings_3_3", {"B200_ALLEGRO_GEMM3_VARIANT": "1"}, 2, 3000, 0),
     ("fp32_simt_env", {"B200_ALLEGRO_FP32_SIMT": "1"}, 1, 1536, 0),
+    ("no_kcat_cfg1", {"B200_ALLEGRO_NO_KCAT": "1"}, 1, 1536, 0),        # separate dX-latent and x-bar GEMMs
+    ("no_kcat_tf32_cfg4", {"B200_ALLEGRO_NO_KCAT": "1"}, 4, 1200, 1),
+    ("no_kcat_no_prep", {"B200_ALLEGRO_NO_KCAT": "1", "B200_ALLEGRO_NO_PREP": "1"}, 2, 3000, 0),
 ]
 
 
