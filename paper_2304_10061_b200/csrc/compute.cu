@@ -70,7 +70,7 @@ void al_work_free(allegro_model* m) {
   Work& w = *m->work;
   std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.sig, &w.B, &w.dB, &w.Y,
                               &w.XF, &w.WE, &w.gamma, &w.XB0, &w.XB1, &w.ZB0, &w.ZB1, &w.G, &w.OB, &w.VB0, &w.VB1,
-                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom};
+                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom, &w.nh_scal};
   for (auto* b : all) al_release(m, *b);
   for (auto* v : {&w.tb_z, &w.tb_a, &w.XS, &w.OM, &w.T}) for (auto& b : *v) al_release(m, b);
   for (auto* vv : {&w.lat_z, &w.lat_a}) for (auto& v : *vv) for (auto& b : v) al_release(m, b);
@@ -345,14 +345,15 @@ extern "C" int allegro_step_nvt(allegro_model* m, double* pos, double* vel, doub
                                 double* nh_state, double t0_K, double tau_fs) {
   if (!m || !vel || !species || !mass || !e_kin || !nh_state) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
   if (!(t0_K > 0) || !(tau_fs > 0) || N < 1) { al_set_error(m, "t0_K > 0, tau_fs > 0, n_atoms >= 1 required"); return ALLEGRO_ERR_BAD_ARG; }
-  static thread_local DevBuf tmp, scal;
-  AL_CHECK(al_reserve(m, scal, 64));
+  if (!m->work) { al_set_error(m, "call allegro_compute once before the first step (force must hold F(r))"); return ALLEGRO_ERR_BAD_ARG; }
+  Work& w = *m->work;
+  AL_CHECK(al_reserve(m, w.nh_scal, 64));
   const double g = 3.0 * (double)N;
   // [thermostat dt/2] [velocity-Verlet NVE step] [thermostat dt/2]
-  AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, tmp));
-  AL_CHECK(k_launch_nh_half(m, vel, N, nh_state, e_kin, g, t0_K, tau_fs, dt_fs, (double*)scal.p));
+  AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, w.scan_tmp));
+  AL_CHECK(k_launch_nh_half(m, vel, N, nh_state, e_kin, g, t0_K, tau_fs, dt_fs, (double*)w.nh_scal.p));
   AL_CHECK(allegro_step_nve(m, pos, vel, force, species, mass, N, box, dt_fs, rebuild_every, skin, nbr, step_counter, e_pot, e_kin));
-  AL_CHECK(k_launch_nh_half(m, vel, N, nh_state, e_kin, g, t0_K, tau_fs, dt_fs, (double*)scal.p));
+  AL_CHECK(k_launch_nh_half(m, vel, N, nh_state, e_kin, g, t0_K, tau_fs, dt_fs, (double*)m->work->nh_scal.p));
   return ALLEGRO_OK;
 }
 

@@ -32,6 +32,7 @@ struct Work {
   DevBuf epart; int n_eparts = 0;           // f64 edge-energy partials [n_eparts][M] (EPI_LATENT_LAST)
   DevBuf ge;                                // float[M][3] dE/dr_e (debug tap)
   DevBuf eatom;                             // f64[N] when the caller passes e_atom = NULL
+  DevBuf nh_scal;                           // f64[1]: velocity scale of the Nose-Hoover half step
   int64_t eatom_cap = 0;
   int last_nc = 0;
 };
