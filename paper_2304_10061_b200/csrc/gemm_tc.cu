@@ -119,7 +119,9 @@ __device__ __forceinline__ float dsilu_f(float z) {
 // MMA's own truncation of the operand is a no-op
 __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xFFFFE000u); }
 
-template <int AST, int BST, int EPI_WARPS, bool SPLIT>
+// EPI (GemmEpi) and PREP (the z-bar / u-bar stage of EPI_ADD2 / EPI_ADD2R) are compile-time: one kernel per epilogue,
+// so the epilogue carries no run-time dispatch, no dead operands and no re-loaded argument fields.
+template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
             const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
@@ -289,8 +291,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         const bool col_ok = (col < g.N) && (c0 + c4 < BN);
         // Two halves of 16 rows: issue every aux load of a half up front (the stores below may alias, so the compiler
         // cannot hoist them), then process it.  Halving keeps the register count low enough for 16 epilogue warps.
-        const bool need1 = (g.epi == EPI_LATENT || g.epi == EPI_LATENT_LAST || g.epi == EPI_MUL_DSILU || g.epi == EPI_ADD2);
-        const bool need2 = (g.epi == EPI_ADD2 || g.epi == EPI_ADD2R) && g.aux2 != nullptr;   // null: the term is in the K-concatenation
+        constexpr bool need1 = (EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_MUL_DSILU || EPI == EPI_ADD2);
+        constexpr bool need2 = (EPI == EPI_ADD2 || EPI == EPI_ADD2R) && AUX2;   // no aux2: the term is in the K-concatenation
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
         float4 ax1[4], ax2[4], ax3[4];
@@ -301,7 +303,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           const bool ok = row < M && col_ok;
           ax1[ii] = (need1 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
           ax2[ii] = (need2 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax3[ii] = (g.prep && ok) ? __ldg(reinterpret_cast<const float4*>(g.zp + (size_t)row * g.ldzp + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax3[ii] = (PREP && ok) ? __ldg(reinterpret_cast<const float4*>(g.zp + (size_t)row * g.ldzp + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
@@ -310,7 +312,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           const int row = rbase + rl;
           const float4 v4 = stg4[rl * 8 + ((lane & 7) ^ (rl & 7))];
           float v[4] = {v4.x, v4.y, v4.z, v4.w};
-          if (g.epi == EPI_LATENT_LAST) {
+          if (EPI == EPI_LATENT_LAST) {
             // all 32 lanes stay in step for the shuffles; out-of-range lanes contribute 0 and store nothing
             const bool ok = row < M && col_ok;
             const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
@@ -346,13 +348,13 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 g.epart[p * g.part_stride + row] = ep;
               }
             }
-          } else if (g.prep) {
+          } else if (PREP) {
             // EPI_ADD2 / EPI_ADD2R followed by the z-bar / u-bar stage of the next MLP (all lanes stay in step)
             const bool ok = row < M && col_ok;
             const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
             float o[4];
             const float4 y = AUX2(i);
-            if (g.epi == EPI_ADD2) {
+            if (EPI == EPI_ADD2) {
               const float4 x = AUX1(i);
               o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
               o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
@@ -385,13 +387,13 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             }
           } else if (row < M && col_ok) {
             float o[4];
-            switch (g.epi) {
+            switch (EPI) {
               case EPI_SILU_BOTH:
               case EPI_SILU_U:
               case EPI_LATENT: {
                 *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(v[0], v[1], v[2], v[3]);
-                float us = (g.epi == EPI_SILU_BOTH) ? 1.0f : g.u[row];
-                if (g.epi == EPI_LATENT) {
+                float us = (EPI == EPI_SILU_BOTH) ? 1.0f : g.u[row];
+                if (EPI == EPI_LATENT) {
                   float4 x = AUX1(i);
                   float xo[4] = {x.x, x.y, x.z, x.w};
 #pragma unroll
@@ -486,16 +488,40 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 
 }  // namespace
 
-#define GEMM_LAUNCH(AS, BS, EW, SP)                                                                                      \
+#define GEMM_LAUNCH(AS, BS, EW, SP, EP, PR, A2)                                                                          \
   {                                                                                                                      \
     static_assert(smem_bytes(AS, BS, EW, SP) <= 232448, "shared memory budget (227 KB)");                                \
     static bool attr_set = false;                                                                                        \
     if (!attr_set) {                                                                                                     \
-      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
+      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
                                       (int)smem_bytes(AS, BS, EW, SP)));                                                 \
       attr_set = true;                                                                                                   \
     }                                                                                                                    \
-    k_gemm_tf32<AS, BS, EW, SP><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>(tmA, tmA2, tmB, tmB2, g, BN, ntn); \
+    k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>( \
+        tmA, tmA2, tmB, tmB2, g, BN, ntn);                                                                               \
+  }
+// one instantiation per epilogue (PREP only exists for the two x-bar epilogues)
+#define GEMM_DISPATCH(AS, BS, EW, SP)                                                                                    \
+  switch (g.epi) {                                                                                                       \
+    case EPI_PLAIN: GEMM_LAUNCH(AS, BS, EW, SP, EPI_PLAIN, false, false) break;                                                 \
+    case EPI_SILU_BOTH: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_BOTH, false, false) break;                                         \
+    case EPI_SILU_U: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_U, false, false) break;                                               \
+    case EPI_LATENT: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT, false, false) break;                                               \
+    case EPI_MUL_DSILU: GEMM_LAUNCH(AS, BS, EW, SP, EPI_MUL_DSILU, false, false) break;                                         \
+    case EPI_LATENT_LAST: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT_LAST, false, false) break;                                     \
+    case EPI_ADD2:                                                                                                       \
+      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, true)                                            \
+      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, false)                                                \
+      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, true)                                                \
+      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, false)                                                           \
+      break;                                                                                                             \
+    case EPI_ADD2R:                                                                                                      \
+      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, true)                                           \
+      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, false)                                               \
+      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, true)                                               \
+      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, false)                                                          \
+      break;                                                                                                             \
+    default: al_set_error(m, "gemm: unknown epilogue"); return ALLEGRO_ERR_BAD_ARG;                                      \
   }
 
 // precision 1: TF32 operands (rounded to nearest by the TMA load), fp32 accumulation
@@ -510,10 +536,8 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
   tmB2 = tmB;
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  static const int variant = getenv("B200_ALLEGRO_GEMM_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM_VARIANT")) : 0;   // A/B ring depths: 0 = 4/3 (default), 1 = 6/2, 2 = 3/3 -- all within 1 % of each other: the rings are not the limiter
-  if (variant == 1) GEMM_LAUNCH(6, 2, 16, false)
-  else if (variant == 2) GEMM_LAUNCH(3, 3, 16, false)
-  else GEMM_LAUNCH(4, 3, 16, false)
+  // A/B ring depths 4/3; 6/2 and 3/3 measured within 1 % of it (the rings are not the limiter)
+  GEMM_DISPATCH(4, 3, 16, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
@@ -532,13 +556,12 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g) {
   AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, true, &tmB2));
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  static const int variant = getenv("B200_ALLEGRO_GEMM3_VARIANT") ? atoi(getenv("B200_ALLEGRO_GEMM3_VARIANT")) : 0;
-  if (variant == 0) GEMM_LAUNCH(4, 2, 8, true)
-  else GEMM_LAUNCH(3, 3, 8, true)
+  GEMM_DISPATCH(4, 2, 8, true)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
 }
+#undef GEMM_DISPATCH
 #undef GEMM_LAUNCH
 
 int al_gemm_tc_row_parts(int N, bool split) {

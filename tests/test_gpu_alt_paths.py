@@ -40,8 +40,6 @@ CASES = [
     ("tp_mreg_cfg1", {"B200_ALLEGRO_TP_MREG": "1"}, 1, 1536, 0),        # 9x9x9 backward with M in registers
     ("tp3_bwd2_cfg4", {"B200_ALLEGRO_TP3_BWD": "2"}, 4, 1200, 0),       # lane-split l_max = 3 backward, 4 blocks
     ("tp3_bwd3_cfg4", {"B200_ALLEGRO_TP3_BWD": "3"}, 4, 1200, 0),       # ... 8 blocks
-    ("gemm_rings_6_2_tf32", {"B200_ALLEGRO_GEMM_VARIANT": "1"}, 2, 3000, 1),       # other TMA ring depths
-    ("gemm3_rings_3_3", {"B200_ALLEGRO_GEMM3_VARIANT": "1"}, 2, 3000, 0),
     ("fp32_simt_env", {"B200_ALLEGRO_FP32_SIMT": "1"}, 1, 1536, 0),
     ("no_kcat_cfg1", {"B200_ALLEGRO_NO_KCAT": "1"}, 1, 1536, 0),        # separate dX-latent and x-bar GEMMs
     ("no_kcat_tf32_cfg4", {"B200_ALLEGRO_NO_KCAT": "1"}, 4, 1200, 1),
