@@ -292,6 +292,19 @@ def main():
     h2d = 3 * N * 24 + N * 4 + cfg.hp.n_species * 8
     d2h = 3 * N * 24 + 16
 
+    # ---- allegro_compute alone and allegro_neighbors alone, outside the timed region above
+    def _ev_ms(fn, reps):
+        fn(); torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ts = []
+        for _ in range(reps):
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return sorted(ts)[len(ts) // 2]
+    compute_ms = _ev_ms(lambda: model.compute(p, s, box, nb, want_atom_energies=False), 5)
+    energy_only_ms = _ev_ms(lambda: model.compute(p, s, box, nb, want_atom_energies=False, want_forces=False), 5)
+    neighbors_ms = _ev_ms(lambda: model.neighbors(p, box, cfg.hp.r_cut + cfg.skin, reuse=nb), 3)
+
     # ---- roofline of the dominant kernel group: second pass of K steps with per-group CUDA events
     groups = ["gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd", "neighbors", "nve"]
     tp_bytes = tp_bytes_per_edge(cfg.hp)
@@ -356,6 +369,8 @@ def main():
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "timesteps_per_s": K / (ms_max * 1e-3), "ns_per_day": K / (ms_max * 1e-3) * cfg.dt_fs * 0.0864,
         "e_pot": e_pot, "e_kin": e_kin,
+        # medians of 5 / 5 / 3 calls, CUDA events: energy+forces alone, energy only (no backward), list build alone
+        "compute_only_ms": compute_ms, "energy_only_ms": energy_only_ms, "neighbors_only_ms": neighbors_ms,
         "gpu_launches": launches,
         "clocks": sampler.summary(),
         "e2e": {"value": e2e_val, "unit": unit, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
