@@ -128,6 +128,14 @@ int allegro_step_nve(allegro_model* m, double* pos, double* vel, double* force, 
                      int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
                      double* e_pot, double* e_kin);
 
+/* allegro_step_nve replays the steps that do not rebuild the list from a CUDA graph: a step whose arguments, list and
+ * configuration are those of the previous (eagerly run) step is captured once and relaunched as one graph from then on
+ * (the small configs are launch-bound: ~36 kernels of a few microseconds each); any change of an argument, a rebuild, a
+ * setter call or a buffer growth falls back to eager launches and re-captures.  The environment variable
+ * B200_ALLEGRO_NO_GRAPH disables it.  n receives the number of steps served by a graph launch so far, -1 if graph
+ * capture failed and was switched off (host). */
+int allegro_graph_steps(const allegro_model* m, int64_t* n);
+
 /* Same step with HOST arrays (pos, vel, force f64[N*3], species i32[N], mass f64[n_species], e_pot,
  * e_kin f64[1]): copies state host->device, runs allegro_step_nve, copies state and energies back,
  * and synchronises.  Pinned host memory makes the copies asynchronous. */

@@ -73,7 +73,7 @@ EXPORTS = [
     "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
-    "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt",
+    "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps",
     "allegro_last_error",
 ]
 
@@ -117,6 +117,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_profile_enable.argtypes = [vp, i32]
     lib.allegro_profile_read.argtypes = [vp, C.c_char_p, P(C.c_double), P(i64)]
     lib.allegro_launch_count.argtypes = [vp, P(i64)]
+    lib.allegro_graph_steps.argtypes = [vp, P(i64)]
     lib.allegro_last_active_edges.argtypes = [vp, P(i64)]
     lib.allegro_debug_tensor.argtypes = [vp, C.c_char_p, vp, P(i64)]
     lib.allegro_last_error.argtypes = [vp]
@@ -251,6 +252,13 @@ class Allegro:
     def launches(self) -> int:
         v = C.c_int64(0)
         self._lib.allegro_launch_count(self._h, C.byref(v))
+        return v.value
+
+    @property
+    def graph_steps(self) -> int:
+        """Number of MD steps served by a CUDA-graph launch so far (-1: capture failed and was switched off)."""
+        v = C.c_int64(0)
+        self._check(self._lib.allegro_graph_steps(self._h, C.byref(v)))
         return v.value
 
     def last_active_edges(self) -> int:

@@ -6,6 +6,7 @@
 #include <cstring>
 
 #include "gemm.h"
+#include <vector>
 #include "kernels.h"
 
 static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
@@ -321,6 +322,52 @@ extern "C" int allegro_last_active_edges(allegro_model* m, int64_t* n_active) {
   return ALLEGRO_OK;
 }
 
+// The part of an MD step that follows the (optional) list rebuild.  `with_first_kick`: the half kick + drift that
+// precedes the rebuild is included (steps without a rebuild, the ones a CUDA graph can replay).
+static int step_tail(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species, const double* mass,
+                     int64_t N, const double box[3], double dt_fs, const allegro_nbr* nbr, double* e_pot, double* e_kin,
+                     bool with_first_kick) {
+  if (with_first_kick) AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, true));
+  AL_CHECK(al_compute_impl(m, pos, species, N, box, nbr, e_pot, nullptr, force, nullptr));
+  AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, false));
+  AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, m->work->scan_tmp));
+  return ALLEGRO_OK;
+}
+
+// Capture one no-rebuild step into a CUDA graph (on a private stream: the caller's may be the legacy default stream,
+// which cannot be captured), instantiate or update the executable graph and launch it on the caller's stream.
+static int step_capture_and_launch(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
+                                   const double* mass, int64_t N, const double box[3], double dt_fs, const allegro_nbr* nbr,
+                                   double* e_pot, double* e_kin, const std::vector<uint64_t>& key) {
+  auto& sg = m->sg;
+  auto give_up = [&](const char* why) { cudaGetLastError(); sg.disabled = true; (void)why; return ALLEGRO_ERR_CUDA; };
+  if (!sg.cap && cudaStreamCreateWithFlags(&sg.cap, cudaStreamNonBlocking) != cudaSuccess) return give_up("stream");
+  cudaStream_t user = m->stream;
+  const int64_t l0 = m->launches;
+  if (cudaStreamBeginCapture(sg.cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) return give_up("begin");
+  m->stream = sg.cap;
+  int rc = step_tail(m, pos, vel, force, species, mass, N, box, dt_fs, nbr, e_pot, e_kin, true);
+  m->stream = user;
+  cudaGraph_t graph = nullptr;
+  cudaError_t e = cudaStreamEndCapture(sg.cap, &graph);
+  const int64_t nl = m->launches - l0;
+  m->launches = l0;                                    // nothing ran yet
+  if (rc != ALLEGRO_OK || e != cudaSuccess || !graph) {
+    if (graph) cudaGraphDestroy(graph);
+    return give_up("capture");
+  }
+  if (sg.exec) {
+    cudaGraphExecUpdateResultInfo info;
+    if (cudaGraphExecUpdate(sg.exec, graph, &info) != cudaSuccess) { cudaGetLastError(); cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; }
+  }
+  if (!sg.exec && cudaGraphInstantiate(&sg.exec, graph, 0) != cudaSuccess) { cudaGraphDestroy(graph); sg.exec = nullptr; return give_up("instantiate"); }
+  cudaGraphDestroy(graph);
+  if (cudaGraphLaunch(sg.exec, user) != cudaSuccess) { cudaGraphExecDestroy(sg.exec); sg.exec = nullptr; return give_up("launch"); }
+  sg.key = key; sg.nlaunch = nl;
+  m->launches += nl;
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, double* force, const int32_t* species,
                                 const double* mass, int64_t N, const double box[3], double dt_fs, int32_t rebuild_every,
                                 double skin, allegro_nbr** nbr, int64_t* step_counter, double* e_pot, double* e_kin) {
@@ -329,13 +376,46 @@ extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, doub
     return ALLEGRO_ERR_BAD_ARG;
   }
   if (rebuild_every < 1 || skin < 0) { al_set_error(m, "rebuild_every >= 1 and skin >= 0 required"); return ALLEGRO_ERR_BAD_ARG; }
+  const bool rebuild = (*nbr == nullptr || (*step_counter % rebuild_every) == 0);
+  static const bool no_graph = getenv("B200_ALLEGRO_NO_GRAPH") != nullptr;
+  const bool graphs = !no_graph && !m->prof && !m->sg.disabled;
+  auto make_key = [&]() {
+    auto bits = [](double x) { uint64_t b; memcpy(&b, &x, 8); return b; };
+    return std::vector<uint64_t>{(uint64_t)pos, (uint64_t)vel, (uint64_t)force, (uint64_t)species, (uint64_t)mass, (uint64_t)N,
+                                 bits(box[0]), bits(box[1]), bits(box[2]), bits(dt_fs), (uint64_t)*nbr, (*nbr)->version,
+                                 (uint64_t)e_pot, (uint64_t)e_kin, (uint64_t)m->stream, m->config_gen, m->alloc_gen};
+  };
+  if (!rebuild && graphs && m->work) {
+    const std::vector<uint64_t> key = make_key();
+    if (m->sg.exec && key == m->sg.key) {
+      if (cudaGraphLaunch(m->sg.exec, m->stream) == cudaSuccess) {
+        m->launches += m->sg.nlaunch;
+        m->sg.steps++;
+        (*step_counter)++;
+        return ALLEGRO_OK;
+      }
+      cudaGetLastError();
+      m->sg.disabled = true;
+    } else if (key == m->sg.warm) {
+      // a step with exactly this state already ran eagerly (every buffer is sized, every kernel attribute set): capture
+      if (step_capture_and_launch(m, pos, vel, force, species, mass, N, box, dt_fs, *nbr, e_pot, e_kin, key) == ALLEGRO_OK) {
+        m->sg.steps++;
+        (*step_counter)++;
+        return ALLEGRO_OK;
+      }
+    }
+  }
   AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, true));
-  if (*nbr == nullptr || (*step_counter % rebuild_every) == 0)
-    AL_CHECK(al_neighbors_impl(m, pos, N, box, m->hp.r_cut + skin, nbr));
-  AL_CHECK(al_compute_impl(m, pos, species, N, box, *nbr, e_pot, nullptr, force, nullptr));
-  AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, false));
-  AL_CHECK(k_launch_kinetic(m, vel, species, mass, N, e_kin, m->work->scan_tmp));
+  if (rebuild) AL_CHECK(al_neighbors_impl(m, pos, N, box, m->hp.r_cut + skin, nbr));
+  AL_CHECK(step_tail(m, pos, vel, force, species, mass, N, box, dt_fs, *nbr, e_pot, e_kin, false));
+  if (graphs && !m->sg.disabled) m->sg.warm = make_key();   // the state the next step will see if nothing changes
   (*step_counter)++;
+  return ALLEGRO_OK;
+}
+
+extern "C" int allegro_graph_steps(const allegro_model* m, int64_t* n) {
+  if (!m || !n) return ALLEGRO_ERR_BAD_ARG;
+  *n = m->sg.disabled ? -1 : m->sg.steps;
   return ALLEGRO_OK;
 }
 

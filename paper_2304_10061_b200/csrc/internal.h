@@ -82,6 +82,7 @@ struct DevBuf {
 struct Chunk { int64_t c0, c1; int64_t e0, e1; };   // centers [c0,c1), candidate edges [e0,e1)
 
 struct allegro_nbr {
+  uint64_t version = 0;                // incremented by every build (keys the CUDA-graph replay of the MD step)
   int64_t n_atoms = 0, n_edges = 0;
   double cutoff = 0; double box[3] = {0, 0, 0};
   DevBuf row_ptr, j, shift, keys;      // int64[N+1], int32[E], int8[3E], uint64[E] scratch
@@ -130,6 +131,14 @@ struct allegro_model {
   std::vector<ProfRec> prof_recs;
   std::vector<cudaEvent_t> prof_pool;
   std::vector<void*> owned;               // device allocations made through al_alloc (weights/tables)
+  // CUDA-graph replay of the steps of allegro_step_nve that do not rebuild the list (launch-bound small systems):
+  // a step whose key (all arguments, list version, configuration and allocation generations) was seen once eagerly
+  // is captured the next time and replayed from then on.
+  struct StepGraph {
+    cudaGraphExec_t exec = nullptr; cudaStream_t cap = nullptr;
+    std::vector<uint64_t> key, warm; int64_t nlaunch = 0, steps = 0; bool disabled = false;
+  } sg;
+  uint64_t config_gen = 0, alloc_gen = 0; // bumped by every setter / every (re)allocation of a work buffer
 };
 
 // ---- profiling ------------------------------------------------------------------------------------

@@ -35,6 +35,7 @@ void al_free(allegro_model* m, void* p) {
 int al_reserve(allegro_model* m, DevBuf& b, size_t bytes) {
   if (b.bytes >= bytes && b.p) return ALLEGRO_OK;
   if (b.p) { cudaStreamSynchronize(m->stream); al_free(m, b.p); b.p = nullptr; b.bytes = 0; }
+  if (m) m->alloc_gen++;
   size_t want = bytes + bytes / 20 + 256;   // +5 % head-room (avoid allocator churn)
   AL_CHECK(al_alloc(m, &b.p, want));
   b.bytes = want;
@@ -309,13 +310,15 @@ extern "C" int allegro_destroy(allegro_model* m) {
   for (auto& r : m->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : m->prof_pool) cudaEventDestroy(e);
   for (void* p : m->owned) cudaFree(p);
+  if (m->sg.exec) cudaGraphExecDestroy(m->sg.exec);
+  if (m->sg.cap) cudaStreamDestroy(m->sg.cap);
   delete m;
   return ALLEGRO_OK;
 }
 
 extern "C" int allegro_set_stream(allegro_model* m, void* s) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
-  m->stream = (cudaStream_t)s;
+  m->stream = (cudaStream_t)s;   // (part of the step-graph key itself)
   return ALLEGRO_OK;
 }
 
@@ -323,12 +326,14 @@ extern "C" int allegro_set_allocator(allegro_model* m, allegro_alloc_fn a, alleg
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   if (m->work) { al_set_error(m, "allocator must be set before the first compute call"); return ALLEGRO_ERR_BAD_ARG; }
   m->alloc_fn = a; m->free_fn = f; m->alloc_user = user;
+  m->config_gen++;
   return ALLEGRO_OK;
 }
 
 extern "C" int allegro_set_pair_cutoffs(allegro_model* m, const double* rc_pair) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  m->config_gen++;
   if (!rc_pair) { m->d_rc_pair = nullptr; return ALLEGRO_OK; }   // (the device array stays owned by the model)
   const int S = m->S;
   for (int k = 0; k < S * S; ++k)
@@ -346,6 +351,7 @@ extern "C" int allegro_set_pair_cutoffs(allegro_model* m, const double* rc_pair)
 extern "C" int allegro_set_bessel_frequencies(allegro_model* m, const double* freq) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  m->config_gen++;
   if (!freq) { m->d_bfreq = nullptr; return ALLEGRO_OK; }
   const size_t cnt = (size_t)m->S * m->S * m->NB;
   for (size_t k = 0; k < cnt; ++k)
@@ -360,6 +366,7 @@ extern "C" int allegro_set_bessel_frequencies(allegro_model* m, const double* fr
 extern "C" int allegro_set_zbl(allegro_model* m, const double* atomic_numbers) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  m->config_gen++;
   if (!atomic_numbers) { m->d_zbl_Z = nullptr; return ALLEGRO_OK; }
   for (int k = 0; k < m->S; ++k)
     if (!(atomic_numbers[k] > 0) || !std::isfinite(atomic_numbers[k])) { al_set_error(m, "atomic numbers must be > 0"); return ALLEGRO_ERR_BAD_HPARAMS; }
@@ -373,12 +380,14 @@ extern "C" int allegro_set_zbl(allegro_model* m, const double* atomic_numbers) {
 extern "C" int allegro_set_debug(allegro_model* m, int on) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   m->debug_keep = on != 0;
+  m->config_gen++;
   return ALLEGRO_OK;
 }
 
 extern "C" int allegro_set_chunk_edges(allegro_model* m, int64_t e) {
   if (!m || e < 1024) return ALLEGRO_ERR_BAD_ARG;
   m->chunk_edges = e;
+  m->config_gen++;
   return ALLEGRO_OK;
 }
 
@@ -409,6 +418,7 @@ extern "C" int allegro_profile_enable(allegro_model* m, int32_t on) {
   for (auto& r : m->prof_recs) { m->prof_pool.push_back(r.a); m->prof_pool.push_back(r.b); }
   m->prof_recs.clear();
   m->prof = on != 0;
+  m->config_gen++;
   return ALLEGRO_OK;
 }
 

@@ -213,6 +213,7 @@ int al_neighbors_impl(allegro_model* m, const double* pos, int64_t N, const doub
   allegro_nbr* nb = *inout ? *inout : new allegro_nbr();
   *inout = nb;
   nb->n_atoms = N; nb->cutoff = cutoff;
+  nb->version++;
   memcpy(nb->box, box, 24);
   NbrGeom g;
   g.cut2 = cutoff * cutoff;

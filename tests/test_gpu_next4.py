@@ -169,3 +169,52 @@ def test_nvt_steps_match_oracle():
     H = O.nh_conserved(e.item(), ek.item(), xi_g, eta_g, 3 * 192, t0, tau)
     H_o = O.nh_conserved(e_o, ek_o, xi, eta, 3 * 192, t0, tau)
     assert abs(H - H_o) < 192 * 2e-6 + 2 * tol_ek
+
+
+def test_md_steps_replayed_from_a_cuda_graph_match_the_oracle():
+    """14 NVE steps with a rebuild every 6: steps 0, 6, 12 run eagerly (list rebuild), 1, 7, 13 are captured, the others
+    are graph replays; the trajectory must still be the oracle's."""
+    import os
+    cfg = _cfg(0, 192)
+    pos, sp, box = make_system(cfg)
+    vel = maxwell_boltzmann(cfg, sp)
+    model, oracle = make_both(cfg)
+    mass = masses_for(cfg)
+    dt, nsteps = 0.5, 14
+
+    def force_fn(p):
+        E, _, F = O.energy_forces(oracle, p, sp, box, O.neighbor_list(p, box, cfg.hp.r_cut))
+        return E, F
+    p_o, v_o = pos.copy(), vel.copy()
+    e_o, f_o = force_fn(p_o)
+    for _ in range(nsteps):
+        p_o, v_o, f_o, e_o = O.nve_step(force_fn, p_o, v_o, f_o, mass[sp], dt)
+    p = torch.from_numpy(pos.copy()).cuda(); v = torch.from_numpy(vel.copy()).cuda()
+    s = torch.from_numpy(sp).cuda(); mg = torch.from_numpy(mass).cuda()
+    nb = model.neighbors(p, box, cfg.hp.r_cut + 1.0)
+    e, _, f = model.compute(p, s, box, nb)
+    ek = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ctr = ctypes.c_int64(0)
+    per_step = []
+    for _ in range(nsteps):
+        l0 = model.launches
+        model.step_nve(p, v, f, s, mg, box, dt, 6, 1.0, nb, ctr, e, ek)
+        per_step.append(model.launches - l0)
+    torch.cuda.synchronize()
+    if os.environ.get("B200_ALLEGRO_NO_GRAPH"):
+        assert model.graph_steps == 0
+    else:
+        assert model.graph_steps == nsteps - 3, model.graph_steps          # all but the three rebuild steps
+        assert len(set(per_step[k] for k in range(nsteps) if k % 6)) == 1   # replayed steps count the same launches
+    np.testing.assert_allclose(p.cpu().numpy(), p_o, atol=2e-7)
+    np.testing.assert_allclose(v.cpu().numpy(), v_o, atol=2e-7)
+    assert abs(e.item() - e_o) / 192 < 2e-6
+    # a setter invalidates the captured step: the next step runs eagerly with the new configuration
+    g0 = model.graph_steps
+    model.set_zbl((1.0, 8.0))
+    model.step_nve(p, v, f, s, mg, box, dt, 6, 1.0, nb, ctr, e, ek)       # step 14: no rebuild, but not the captured state
+    torch.cuda.synchronize()
+    assert model.graph_steps == g0
+    e_chk, _, f_chk = model.compute(p, s, box, nb)
+    torch.cuda.synchronize()
+    assert abs(e_chk.item() - e.item()) < 1e-9 and (f_chk - f).abs().max().item() < 1e-9   # forces include the ZBL term
