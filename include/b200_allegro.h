@@ -118,6 +118,19 @@ int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* spe
                          const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom,
                          double* force);
 
+/* Energy and forces of a spatial domain (the paper runs one rank per GPU over LAMMPS's
+ * spatial decomposition).  The first n_local atoms are the domain's own atoms and the only
+ * centres; atoms n_local .. n_atoms-1 are ghosts (copies, with their image shift applied, of atoms owned by other
+ * domains or by this one across a periodic face) and appear as neighbours only.  e_total = sum of E-hat_i over the local
+ * atoms, e_atom[i] = 0 for ghosts, force f64[n_atoms*3] = -d(e_total)/dr for local AND ghost atoms: the ghost part is what
+ * the reverse exchange returns to the owners, after which every owner holds its complete force (strict locality,
+ * PAPER.md:138).  With ZBL on, local atoms receive their complete pair force and ghosts none.  box is the periodic cell
+ * of the coordinates passed in: for a domain it must exceed the extent of local + ghost atoms by more than the cutoff
+ * in every direction, so that no pair is found through the boundary.  The list must have been built from the same
+ * n_atoms positions.  Arguments otherwise as allegro_compute. */
+int allegro_compute_local(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms, int64_t n_local,
+                          const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force);
+
 /* One velocity-Verlet NVE step: v += dt/2 F/m; r += dt v; [rebuild list at cutoff
  * r_cut+skin if *step_counter % rebuild_every == 0]; F; v += dt/2 F/m.  `force` f64[N*3] (device) must
  * hold F(r) of the current positions on entry (call allegro_compute once before the first step) and

@@ -73,7 +73,7 @@ EXPORTS = [
     "allegro_nbr_info", "allegro_nbr_copy_host", "allegro_nbr_free", "allegro_compute", "allegro_compute_host",
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
-    "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps",
+    "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps", "allegro_compute_local",
     "allegro_last_error",
 ]
 
@@ -111,6 +111,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
                                      P(i64), vp, vp]
     lib.allegro_step_nve_host.argtypes = lib.allegro_step_nve.argtypes
     lib.allegro_step_nvt.argtypes = lib.allegro_step_nve.argtypes + [vp, C.c_double, C.c_double]
+    lib.allegro_compute_local.argtypes = [vp, vp, vp, i64, i64, P(C.c_double), vp, vp, vp, vp]
     lib.allegro_edge_energies.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp]
     lib.allegro_set_bessel_frequencies.argtypes = [vp, vp]
     lib.allegro_set_zbl.argtypes = [vp, vp]
@@ -291,6 +292,20 @@ class Allegro:
         self._check(self._lib.allegro_compute(self._h, pos.data_ptr(), species.data_ptr(), N, _box3(box), nbr._h,
                                               e.data_ptr(), ea.data_ptr() if ea is not None else None,
                                               f.data_ptr() if f is not None else None))
+        return e, ea, f
+
+    def compute_local(self, pos, species, n_local: int, box: Sequence[float], nbr: NeighborList):
+        """allegro_compute_local: atoms [0, n_local) are centres, the rest ghosts -> (e_total, e_atom, force) CUDA."""
+        t = self._torch
+        assert pos.is_cuda and pos.dtype == t.float64 and pos.is_contiguous()
+        assert species.is_cuda and species.dtype == t.int32 and species.is_contiguous()
+        self._sync_stream()
+        N = pos.shape[0]
+        e = t.empty(1, dtype=t.float64, device=pos.device)
+        ea = t.empty(N, dtype=t.float64, device=pos.device)
+        f = t.empty((N, 3), dtype=t.float64, device=pos.device)
+        self._check(self._lib.allegro_compute_local(self._h, pos.data_ptr(), species.data_ptr(), N, int(n_local), _box3(box),
+                                                    nbr._h, e.data_ptr(), ea.data_ptr(), f.data_ptr()))
         return e, ea, f
 
     def edge_energies(self, pos, species, box: Sequence[float], nbr: NeighborList):

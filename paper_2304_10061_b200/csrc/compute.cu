@@ -252,7 +252,16 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
 
 int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t N, const double box[3],
                     const allegro_nbr* nb, double* e_total, double* e_atom, double* force, double* e_edge) {
+  return al_compute_local_impl(m, pos, species, N, N, box, nb, e_total, e_atom, force, e_edge);
+}
+
+// n_local < N: only the first n_local atoms are centres (the local atoms of a spatial domain); the others are ghosts that
+// appear as neighbours and receive the force -dE_local/dr_ghost.
+int al_compute_local_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t N, int64_t n_local,
+                          const double box[3], const allegro_nbr* nb, double* e_total, double* e_atom, double* force,
+                          double* e_edge) {
   if (!m || !pos || !species || !box || !nb || !e_total) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+  if (n_local < 0 || n_local > N) { al_set_error(m, "n_local out of range"); return ALLEGRO_ERR_BAD_ARG; }
   if (nb->n_atoms != N) { al_set_error(m, "neighbor list was built for a different n_atoms"); return ALLEGRO_ERR_BAD_ARG; }
   if (nb->cutoff < m->hp.r_cut) { al_set_error(m, "neighbor list cutoff < r_cut"); return ALLEGRO_ERR_BAD_ARG; }
   AL_CHECK(work_reserve(m, nb, N));
@@ -260,20 +269,32 @@ int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species,
   double* ea = e_atom ? e_atom : (double*)w.eatom.p;
   if (force) AL_CHECK(k_launch_zero_f64(m, force, 3 * N));
   AL_CUDA(m, cudaMemsetAsync((int*)w.m_act.p + 2, 0, 8, m->stream));   // total active edges of this call
-  for (const Chunk& ch : nb->chunks) {
+  for (Chunk ch : nb->chunks) {
+    if (ch.c0 >= n_local) break;
+    if (ch.c1 > n_local) {   // the chunk that straddles the local / ghost boundary: keep its local centres only
+      ch.c1 = n_local;
+      ch.e1 = nb->row_ptr_host[n_local];
+    }
     if (ch.e1 == ch.e0) {
       // no candidate edges at all: make rowa all-zero so k_energy yields mu_Z
       AL_CUDA(m, cudaMemsetAsync(w.rowa.p, 0, (size_t)(ch.c1 - ch.c0 + 1) * 8, m->stream));
     }
     AL_CHECK(run_chunk(m, w, ch, pos, species, box, nb, ea, force, e_edge));
   }
-  AL_CHECK(k_launch_sum_f64(m, ea, N, e_total));
+  if (n_local < N) AL_CHECK(k_launch_zero_f64(m, ea + n_local, N - n_local));   // ghosts carry no energy here
+  AL_CHECK(k_launch_sum_f64(m, ea, n_local, e_total));
   return ALLEGRO_OK;
 }
 
 extern "C" int allegro_compute(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
                                const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force) {
   return al_compute_impl(m, pos, species, n_atoms, box, nbr, e_total, e_atom, force, nullptr);
+}
+
+extern "C" int allegro_compute_local(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
+                                     int64_t n_local, const double box[3], const allegro_nbr* nbr, double* e_total,
+                                     double* e_atom, double* force) {
+  return al_compute_local_impl(m, pos, species, n_atoms, n_local, box, nbr, e_total, e_atom, force, nullptr);
 }
 
 extern "C" int allegro_edge_energies(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,

@@ -165,5 +165,8 @@ int al_neighbors_impl(allegro_model* m, const double* pos, int64_t n_atoms, cons
 int al_compute_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms,
                     const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force /*null: energy only*/,
                     double* e_edge /*null or f64[nbr->n_edges]*/);
+int al_compute_local_impl(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms, int64_t n_local,
+                          const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force,
+                          double* e_edge);
 int al_exclusive_scan_i64(allegro_model* m, const int32_t* in, int64_t* out, int64_t n, DevBuf& tmp);  // out[n] = total
 void al_work_free(allegro_model* m);
