@@ -172,6 +172,64 @@ def oracle_sample(cfg, pos, sp, box, n_centers):
     return run, centers.size, torch.get_num_threads()
 
 
+def run_decomposed(args, cfg, model, p, v, s, mass, box, dist, dev, rank, world, local_rank, K, W, metric, unit, workload):
+    """NEXT-3: the same NVE step with ONE system split over the ranks by spatial domains
+    (paper_2304_10061_b200/domain.py): halo forward / reverse exchange over NCCL all_to_all_single, migration at every
+    list rebuild, energy all-reduce.  Strong scaling: value = total atoms x steps / max-over-ranks time."""
+    import torch
+    from paper_2304_10061_b200.domain import Domain, DomainGrid, TorchComm, auto_grid
+    N = p.shape[0]
+    grid = auto_grid(world, box)
+    dom = Domain(DomainGrid(box, grid), rank, cfg.hp.r_cut + cfg.skin, cfg.hp.r_cut, model=model)
+    gid = dom.take_owned(p, s)
+    vel = v[gid].contiguous()
+    comm = TorchComm()
+    e, f = dom.energy_forces(comm)
+    f = f.contiguous()
+    state = {"vel": vel, "f": f, "e": e, "k": 0}
+
+    def step():
+        rebuild = state["k"] % cfg.rebuild_every == 0
+        state["e"], state["vel"], state["f"] = dom.nve_step(comm, state["vel"], state["f"], mass, cfg.dt_fs, rebuild)
+        state["k"] += 1
+
+    for _ in range(W):
+        step()
+    dist.barrier(); torch.cuda.synchronize()
+    l0 = model.launches
+    sampler = ClockSampler(local_rank); sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    dist.barrier(); torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(K):
+        step()
+    ev1.record()
+    dist.barrier(); torch.cuda.synchronize()
+    sampler.stop_flag = True
+    ms = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    cnt = torch.tensor([float(dom.pos.shape[0]), float(sum(dom.recv_counts))], dtype=torch.float64, device=dev)
+    cmax = cnt.clone(); dist.all_reduce(cmax, op=dist.ReduceOp.MAX)
+    dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+    ek = model.kinetic_energy(state["vel"], dom.species, mass)
+    dist.all_reduce(ek, op=dist.ReduceOp.SUM)
+    if rank == 0:
+        print(json.dumps({
+            "metric": metric, "value": N * K / (ms_max * 1e-3), "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": {0: "f32 (3xtf32)", 1: "tf32", 2: "bf16", 3: "f32"}[args.precision], "data": "synthetic",
+            "config": {"workload": workload, "n_atoms": N, "precision_mode": args.precision, "dt_fs": cfg.dt_fs,
+                       "rebuild_every": cfg.rebuild_every, "skin": cfg.skin,
+                       "parallelism": f"spatial decomposition {grid[0]}x{grid[1]}x{grid[2]}, halo {cfg.hp.r_cut + cfg.skin} A",
+                       "local_atoms_max": int(cmax[0].item()), "ghost_atoms_max": int(cmax[1].item()),
+                       "ghost_atoms_total": int(cnt[1].item())},
+            "timesteps_per_s": K / (ms_max * 1e-3), "ns_per_day": K / (ms_max * 1e-3) * cfg.dt_fs * 0.0864,
+            "e_pot": float(state["e"].item()), "e_kin": float(ek.item()),
+            "gpu_launches": model.launches - l0, "clocks": sampler.summary()}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -182,6 +240,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
+    ap.add_argument("--decompose", action="store_true",
+                    help="NEXT-3: ONE system split over the N GPUs by spatial domains with halo exchange (strong scaling) "
+                         "instead of N replicas; at N = 1 the single domain exchanges its periodic images with itself")
     ap.add_argument("--pair-cutoffs", default="none", choices=["none", "water"],
                     help="ordered species-pair cutoffs (PAPER.md:172-182, :222); 'water' = the paper's H/O values, configs 0-1 only")
     args = ap.parse_args()
@@ -229,9 +290,13 @@ def main():
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: the hot path has no CPU fallback"
     torch.cuda.set_device(local_rank)
     dist = None
-    if world > 1:
+    if world > 1 or args.decompose:
         import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if world == 1:
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29577")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local_rank))
+        else:
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     def barrier():
         if dist is not None:
@@ -249,6 +314,10 @@ def main():
     dev = torch.device("cuda", local_rank)
     p = torch.from_numpy(pos.copy()).to(dev); v = torch.from_numpy(vel.copy()).to(dev)
     s = torch.from_numpy(sp).to(dev); mass = torch.from_numpy(masses_for(cfg)).to(dev)
+    if args.decompose:
+        run_decomposed(args, cfg, model, p, v, s, mass, box, dist, dev, rank, world, local_rank, K, W, metric, unit, workload)
+        dist.destroy_process_group()
+        return
     nb = model.neighbors(p, box, cfg.hp.r_cut + cfg.skin)
     e, _, f = model.compute(p, s, box, nb, want_atom_energies=False)
     ek = torch.zeros(1, dtype=torch.float64, device=dev)

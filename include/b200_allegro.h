@@ -141,6 +141,14 @@ int allegro_step_nve(allegro_model* m, double* pos, double* vel, double* force, 
                      int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
                      double* e_pot, double* e_kin);
 
+/* The two halves of the velocity-Verlet step on their own, for drivers that put something between them (the domain-
+ * decomposed step exchanges halos there): v += dt/2 F/m * 9.648533212e-3 and, if drift != 0, r += dt v.
+ * allegro_kinetic_energy: e_kin = sum_i m_i v_i^2 / 2 in eV (device f64[1]), fixed-order reduction.  Device pointers. */
+int allegro_nve_kick(allegro_model* m, double* pos, double* vel, const double* force, const int32_t* species,
+                     const double* mass, int64_t n_atoms, double dt_fs, int32_t drift);
+int allegro_kinetic_energy(allegro_model* m, const double* vel, const int32_t* species, const double* mass,
+                           int64_t n_atoms, double* e_kin);
+
 /* allegro_step_nve replays the steps that do not rebuild the list from a CUDA graph: a step whose arguments, list and
  * configuration are those of the previous (eagerly run) step is captured once and relaunched as one graph from then on
  * (the small configs are launch-bound: ~36 kernels of a few microseconds each); any change of an argument, a rebuild, a

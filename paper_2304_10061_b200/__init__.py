@@ -74,6 +74,7 @@ EXPORTS = [
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
     "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps", "allegro_compute_local",
+    "allegro_nve_kick", "allegro_kinetic_energy",
     "allegro_last_error",
 ]
 
@@ -111,6 +112,8 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
                                      P(i64), vp, vp]
     lib.allegro_step_nve_host.argtypes = lib.allegro_step_nve.argtypes
     lib.allegro_step_nvt.argtypes = lib.allegro_step_nve.argtypes + [vp, C.c_double, C.c_double]
+    lib.allegro_nve_kick.argtypes = [vp, vp, vp, vp, vp, vp, i64, C.c_double, i32]
+    lib.allegro_kinetic_energy.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.allegro_compute_local.argtypes = [vp, vp, vp, i64, i64, P(C.c_double), vp, vp, vp, vp]
     lib.allegro_edge_energies.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp]
     lib.allegro_set_bessel_frequencies.argtypes = [vp, vp]
@@ -355,6 +358,20 @@ class Allegro:
                                                species.data_ptr(), mass.data_ptr(), pos.shape[0], _box3(box),
                                                float(dt_fs), int(rebuild_every), float(skin), C.byref(nbr._h),
                                                C.byref(step_counter), e_pot.data_ptr(), e_kin.data_ptr()))
+
+    def nve_kick(self, pos, vel, force, species, mass, dt_fs: float, drift: bool):
+        """allegro_nve_kick: half kick (and drift) in place on CUDA tensors."""
+        self._sync_stream()
+        self._check(self._lib.allegro_nve_kick(self._h, pos.data_ptr(), vel.data_ptr(), force.data_ptr(), species.data_ptr(),
+                                               mass.data_ptr(), vel.shape[0], float(dt_fs), 1 if drift else 0))
+
+    def kinetic_energy(self, vel, species, mass):
+        """allegro_kinetic_energy -> CUDA float64 [1] (eV)."""
+        self._sync_stream()
+        ek = self._torch.empty(1, dtype=self._torch.float64, device=vel.device)
+        self._check(self._lib.allegro_kinetic_energy(self._h, vel.data_ptr(), species.data_ptr(), mass.data_ptr(),
+                                                     vel.shape[0], ek.data_ptr()))
+        return ek
 
     def step_nvt(self, pos, vel, force, species, mass, box, dt_fs: float, rebuild_every: int, skin: float,
                  nbr: NeighborList, step_counter: C.c_int64, e_pot, e_kin, nh_state, t0_K: float, tau_fs: float):

@@ -434,6 +434,19 @@ extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, doub
   return ALLEGRO_OK;
 }
 
+extern "C" int allegro_nve_kick(allegro_model* m, double* pos, double* vel, const double* force, const int32_t* species,
+                                const double* mass, int64_t N, double dt_fs, int32_t drift) {
+  if (!m || !vel || !force || !species || !mass || (drift && !pos)) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+  return k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, drift != 0);
+}
+
+extern "C" int allegro_kinetic_energy(allegro_model* m, const double* vel, const int32_t* species, const double* mass,
+                                      int64_t N, double* e_kin) {
+  if (!m || !vel || !species || !mass || !e_kin) { al_set_error(m, "NULL argument"); return ALLEGRO_ERR_BAD_ARG; }
+  if (!m->work) m->work = new Work();
+  return k_launch_kinetic(m, vel, species, mass, N, e_kin, m->work->scan_tmp);
+}
+
 extern "C" int allegro_graph_steps(const allegro_model* m, int64_t* n) {
   if (!m || !n) return ALLEGRO_ERR_BAD_ARG;
   *n = m->sg.disabled ? -1 : m->sg.steps;

@@ -102,7 +102,7 @@ class Domain:
 
     compute_local(pos_all f64[n,3], species_all i32[n], n_local, box_local[3]) -> (e_local f64 scalar tensor,
     force_all f64[n,3]) evaluates the local centres; the default binds `Allegro.neighbors` + `Allegro.compute_local`
-    (CUDA; there is no CPU fallback), the CPU tests pass the oracle."""
+    (CUDA; there is no CPU fallback); the multi-process CPU tests inject their own evaluator."""
 
     def __init__(self, grid: DomainGrid, rank: int, halo: float, r_cut: float, model=None,
                  compute_local: Optional[Callable] = None):
@@ -215,6 +215,20 @@ class Domain:
         if returned.numel():
             f.index_add_(0, self.send_idx, returned)
         return f
+
+    # ---- one velocity-Verlet NVE step of this domain's atoms (kicks and drift by the library's kernels) ---------------
+    def nve_step(self, comm: "TorchComm", vel: torch.Tensor, force: torch.Tensor, mass: torch.Tensor, dt_fs: float,
+                 rebuild: bool):
+        """v += dt/2 a; r += dt v; [migrate + new ghost lists if rebuild]; halo exchange + forces; v += dt/2 a.
+        vel / force belong to this rank's atoms and come back re-ordered when atoms migrated.  Returns
+        (e_pot all-reduced f64[1], vel, force)."""
+        self.model.nve_kick(self.pos, vel, force, self.species, mass, dt_fs, True)
+        if rebuild:
+            vel = self.migrate(comm, vel).reshape(-1, 3).contiguous()
+        e, force = self.energy_forces(comm, rebuild=rebuild)
+        force = force.contiguous()
+        self.model.nve_kick(self.pos, vel, force, self.species, mass, dt_fs, False)
+        return e, vel, force
 
     # ---- the whole evaluation over a communicator ----------------------------------------------------------------------
     def energy_forces(self, comm: TorchComm, rebuild: bool = True):

@@ -173,3 +173,21 @@ def test_domains_on_one_gpu_match_the_single_domain_result(ci, n, grid, precisio
         assert abs(E - E0) / n <= 1e-6 and np.abs(F - F0).max() <= 1e-5 * fs
     else:
         assert np.abs(F - F1).max() <= 2e-3 * np.abs(F1).max()
+
+
+@pytest.mark.gpu
+def test_decomposed_md_over_nccl_world1_matches_the_plain_step():
+    """`bench.py --decompose` at one rank: the single domain exchanges its periodic images with itself through the real
+    NCCL all_to_all_single path (migration at every rebuild included); after 8 MD steps the energies must be those of
+    the plain allegro_step_nve run."""
+    import json
+    import subprocess
+    outs = []
+    for extra in (["--decompose"], ["--no-cpu-baseline"]):
+        r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "0", "--steps", "5", "--warmup", "3"] + extra,
+                           capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-3000:]
+        outs.append(json.loads(r.stdout.strip().splitlines()[-1]))
+    dec, std = outs
+    assert dec["scaling"] == "strong" and dec["config"]["ghost_atoms_max"] > 0 and dec["gpu_launches"] > 0
+    assert abs(dec["e_pot"] - std["e_pot"]) < 192 * 2e-6 and abs(dec["e_kin"] - std["e_kin"]) < 1e-4
