@@ -233,8 +233,10 @@ def run_decomposed(args, cfg, model, p, v, s, mass, box, dist, dev, rank, world,
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=5)
+    # defaults: >= 20 warm-up steps (the paper discards ~200) and a timed region long
+    # enough (0.6 s at config 1) for several nvidia-smi clock samples
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--precision", type=int, default=1, help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores, 3 fp32 FFMA")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
