@@ -219,11 +219,18 @@ class Allegro:
         if use_torch_allocator:
             dev = torch.cuda.current_device()
 
+            alloc_fn, delete_fn, stream_fn = (torch.cuda.caching_allocator_alloc, torch.cuda.caching_allocator_delete,
+                                              torch.cuda.current_stream)
+
             def _alloc(nbytes, _user):
-                return torch.cuda.caching_allocator_alloc(int(nbytes), dev, torch.cuda.current_stream(dev))
+                return alloc_fn(int(nbytes), dev, stream_fn(dev))
 
             def _free(ptr, _user):
-                torch.cuda.caching_allocator_delete(ptr)
+                # bound at creation: at interpreter shutdown the torch.cuda module attributes may already be gone
+                try:
+                    delete_fn(ptr)
+                except Exception:
+                    pass
 
             a, f = _ALLOC_FN(_alloc), _FREE_FN(_free)
             self._keep += [a, f]
