@@ -218,3 +218,41 @@ def test_md_steps_replayed_from_a_cuda_graph_match_the_oracle():
     e_chk, _, f_chk = model.compute(p, s, box, nb)
     torch.cuda.synchronize()
     assert abs(e_chk.item() - e.item()) < 1e-9 and (f_chk - f).abs().max().item() < 1e-9   # forces include the ZBL term
+
+
+def test_edge_cases_of_the_new_entry_points():
+    """n_local = N is allegro_compute, n_local = 0 evaluates nothing; a centre whose candidates all lie beyond its pair
+    cutoffs gets mu_Z (+ ZBL); an isolated system has no edges at all."""
+    cfg = _cfg(0, 192, zbl_Z=(1.0, 8.0))
+    pos, sp, box = make_system(cfg)
+    model, _ = make_both(cfg)
+    p = torch.from_numpy(pos).cuda(); s = torch.from_numpy(sp).cuda()
+    nb = model.neighbors(p, box, cfg.hp.r_cut + 0.5)
+    e, ea, f = model.compute(p, s, box, nb)
+    eN, eaN, fN = model.compute_local(p, s, 192, box, nb)
+    e0, ea0, f0 = model.compute_local(p, s, 0, box, nb)
+    eh, eah, fh = model.compute_local(p, s, 100, box, nb)
+    torch.cuda.synchronize()
+    assert eN.item() == e.item() and torch.equal(ea, eaN) and (f - fN).abs().max().item() < 1e-12
+    assert e0.item() == 0.0 and ea0.abs().max().item() == 0.0 and f0.abs().max().item() == 0.0
+    assert torch.equal(eah[:100], ea[:100]) and eah[100:].abs().max().item() == 0.0
+    assert abs(eh.item() - ea[:100].sum().item()) < 1e-9
+    # tiny pair cutoffs: no edge survives the compaction although every row has candidates
+    model.set_pair_cutoffs(((0.2, 0.2), (0.2, 0.2)))
+    model.set_zbl(None)
+    e1, ea1, f1 = model.compute(p, s, box, nb)
+    e_e, ee = model.edge_energies(p, s, box, nb)
+    torch.cuda.synchronize()
+    mu = np.array(cfg.mu())[sp]
+    assert model.last_active_edges() == 0
+    assert np.array_equal(ea1.cpu().numpy(), mu) and f1.abs().max().item() == 0.0 and ee.abs().max().item() == 0.0
+    # two atoms further apart than the cutoff in a big box: empty list
+    model.set_pair_cutoffs(None)
+    p2 = torch.tensor([[1.0, 1.0, 1.0], [9.0, 9.0, 9.0]], dtype=torch.float64, device="cuda")
+    s2 = torch.tensor([0, 1], dtype=torch.int32, device="cuda")
+    nb2 = model.neighbors(p2, [30.0, 30.0, 30.0], cfg.hp.r_cut)
+    assert nb2.n_edges == 0
+    e2, ea2, f2 = model.compute(p2, s2, [30.0, 30.0, 30.0], nb2)
+    e3, ee3 = model.edge_energies(p2, s2, [30.0, 30.0, 30.0], nb2)
+    torch.cuda.synchronize()
+    assert np.array_equal(ea2.cpu().numpy(), np.array(cfg.mu())) and f2.abs().max().item() == 0.0 and ee3.numel() == 0
