@@ -41,6 +41,7 @@ CASES = [
     ("tp3_bwd2_cfg4", {"B200_ALLEGRO_TP3_BWD": "2"}, 4, 1200, 0),       # lane-split l_max = 3 backward, 4 blocks
     ("tp3_bwd3_cfg4", {"B200_ALLEGRO_TP3_BWD": "3"}, 4, 1200, 0),       # ... 8 blocks
     ("fp32_simt_env", {"B200_ALLEGRO_FP32_SIMT": "1"}, 1, 1536, 0),
+    ("tp3_no_mma_tf32_cfg4", {"B200_ALLEGRO_TP3_NO_MMA": "1"}, 4, 1200, 1),   # FFMA forward for l_max = 3 in TF32 mode
     ("no_kcat_cfg1", {"B200_ALLEGRO_NO_KCAT": "1"}, 1, 1536, 0),        # separate dX-latent and x-bar GEMMs
     ("no_kcat_tf32_cfg4", {"B200_ALLEGRO_NO_KCAT": "1"}, 4, 1200, 1),
     ("no_kcat_no_prep", {"B200_ALLEGRO_NO_KCAT": "1", "B200_ALLEGRO_NO_PREP": "1"}, 2, 3000, 0),
