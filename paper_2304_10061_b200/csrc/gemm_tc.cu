@@ -108,6 +108,16 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
   return d;
 }
 
+// epilogue operands are streamed (read or written once per launch): keep them out of L1
+__device__ __forceinline__ float4 ep_ld4(const float* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void ep_st4(float* p, const float4 v) {
+  asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
 // tensor-core modes: fast-math sigmoid (ex2.approx + rcp.approx), error ~1e-7 << TF32 rounding
 __device__ __forceinline__ float silu_f(float z) { return __fdividef(z, 1.0f + __expf(-z)); }
 __device__ __forceinline__ float dsilu_f(float z) {
@@ -301,9 +311,9 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           const int i = h * 4 + ii;
           const int row = rbase + i * 4 + rsub;
           const bool ok = row < M && col_ok;
-          ax1[ii] = (need1 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux1 + (size_t)row * g.ld1 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax2[ii] = (need2 && ok) ? __ldg(reinterpret_cast<const float4*>(g.aux2 + (size_t)row * g.ld2 + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax3[ii] = (PREP && ok) ? __ldg(reinterpret_cast<const float4*>(g.zp + (size_t)row * g.ldzp + col)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax1[ii] = (need1 && ok) ? ep_ld4(g.aux1 + (size_t)row * g.ld1 + col) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax2[ii] = (need2 && ok) ? ep_ld4(g.aux2 + (size_t)row * g.ld2 + col) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax3[ii] = (PREP && ok) ? ep_ld4(g.zp + (size_t)row * g.ldzp + col) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
@@ -340,8 +350,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               ep += __shfl_xor_sync(0xffffffffu, ep, off);
             }
             if (ok) {
-              *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(zb[0], zb[1], zb[2], zb[3]);
-              if (g.C) *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+              ep_st4(g.out2 + (size_t)row * g.ldo2 + col, make_float4(zb[0], zb[1], zb[2], zb[3]));
+              if (g.C) ep_st4(g.C + (size_t)row * g.ldc + col, make_float4(o[0], o[1], o[2], o[3]));
               if ((lane & 7) == 0) {
                 const int64_t p = (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.c1 * sg * up;
@@ -378,8 +388,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
             for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
             if (ok) {
-              *reinterpret_cast<float4*>(g.zbp + (size_t)row * g.ldzbp + col) = make_float4(zb[0], zb[1], zb[2], zb[3]);
-              if (g.C) *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+              ep_st4(g.zbp + (size_t)row * g.ldzbp + col, make_float4(zb[0], zb[1], zb[2], zb[3]));
+              if (g.C) ep_st4(g.C + (size_t)row * g.ldc + col, make_float4(o[0], o[1], o[2], o[3]));
               if ((lane & 7) == 0) {
                 const int64_t p = g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.cp * up;
@@ -391,7 +401,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               case EPI_SILU_BOTH:
               case EPI_SILU_U:
               case EPI_LATENT: {
-                *reinterpret_cast<float4*>(g.out2 + (size_t)row * g.ldo2 + col) = make_float4(v[0], v[1], v[2], v[3]);
+                ep_st4(g.out2 + (size_t)row * g.ldo2 + col, make_float4(v[0], v[1], v[2], v[3]));
                 float us = (EPI == EPI_SILU_BOTH) ? 1.0f : g.u[row];
                 if (EPI == EPI_LATENT) {
                   float4 x = AUX1(i);
@@ -426,7 +436,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
                 for (int j = 0; j < 4; ++j) o[j] = v[j];
             }
-            *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + col) = make_float4(o[0], o[1], o[2], o[3]);
+            ep_st4(g.C + (size_t)row * g.ldc + col, make_float4(o[0], o[1], o[2], o[3]));
           }
         }
         }   // halves

@@ -12,11 +12,13 @@
 //   * the accumulators of the 8 channels stay in registers for two 8-column tiles at a time, so a lane also STORES whole
 //     32-byte sectors T[e][c][n0..n0+7].
 // Measured rates on this part: mma.sync TF32 279 TFLOP/s against 68 TFLOP/s for packed FFMA.
-// Measured result (config 4, forward of the tensor track): 29.5 ms against 30.3 ms for the FFMA kernels of tp3_impl.cuh --
-// the arithmetic is gone from the profile (tensor pipe 8 % busy) but both versions are bound by the L1 tag rate of
-// their 32-byte-sector accesses (l1tex 82 %): with channels fastest and 8 channels per warp every sector sits in its own
-// 128-byte line.  A layout with the 8-channel group fastest after the component ([edge][group][component][8]) would
-// make the 4 lanes of a fragment row read one line; that, and the backward, are the open part of NEXT-2.
+// Measured result (config 4, forward of the tensor track): 24.3 ms against 30.3 ms for the FFMA kernels of tp3_impl.cuh.
+// The arithmetic is gone from the profile (tensor pipe 8 % busy, 4x fewer instructions); what remains is the L1: with
+// channels fastest and 8 channels per warp every 32-byte sector sits in its own 128-byte line (l1tex 82 % busy).
+// Marking the sector loads and stores L1::no_allocate took the kernel from 29.5 to 24.3 ms (66 % of the copy bandwidth);
+// the same hint on the 4-byte stores of the FFMA kernels changed nothing.  A layout with the 8-channel group fastest
+// after the component ([edge][group][component][8]) would make the 4 lanes of a fragment row read one line; that, and
+// the backward, are the open part of NEXT-2.
 #pragma once
 #include "tp3_impl.cuh"
 
@@ -30,11 +32,11 @@ __device__ __forceinline__ void t3m_mma(float* c, uint32_t a0, uint32_t a1, uint
 
 // one whole 32-byte sector per lane (sm_100: 256-bit global loads / stores); p must be 32-byte aligned
 __device__ __forceinline__ void t3m_ld256(const float* p, float4& lo, float4& hi) {
-  asm volatile("ld.global.nc.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+  asm volatile("ld.global.nc.L1::no_allocate.v8.f32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
                : "=f"(lo.x), "=f"(lo.y), "=f"(lo.z), "=f"(lo.w), "=f"(hi.x), "=f"(hi.y), "=f"(hi.z), "=f"(hi.w) : "l"(p));
 }
 __device__ __forceinline__ void t3m_st256(float* p, const float4& lo, const float4& hi) {
-  asm volatile("st.global.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w),
+  asm volatile("st.global.L1::no_allocate.v8.f32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"l"(p), "f"(lo.x), "f"(lo.y), "f"(lo.z), "f"(lo.w),
                "f"(hi.x), "f"(hi.y), "f"(hi.z), "f"(hi.w) : "memory");
 }
 
