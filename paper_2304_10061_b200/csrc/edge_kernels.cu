@@ -7,6 +7,15 @@
 #include "kernels.h"
 
 namespace {
+// streamed rows (written or read once per step): keep them out of L1
+__device__ __forceinline__ void ek_st4(float* p, const float4 v) {
+  asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ float4 ek_ld4(const float* p) {
+  float4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
 
 #define FULLMASK 0xffffffffu
 
@@ -224,10 +233,9 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
         const float b = sB[r][q];   // (zero beyond NB)
         acc.x = fmaf(b, wb[q].x, acc.x); acc.y = fmaf(b, wb[q].y, acc.y); acc.z = fmaf(b, wb[q].z, acc.z); acc.w = fmaf(b, wb[q].w, acc.w);
       }
-      *reinterpret_cast<float4*>(z + e * H + k4) = acc;
+      ek_st4(z + e * H + k4, acc);
       const float us = scale_u ? sU[r] : 1.0f;
-      *reinterpret_cast<float4*>(act + e * ldact + k4) =
-          make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
+      ek_st4(act + e * ldact + k4, make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w)));
     }
     return;
   }
@@ -243,10 +251,9 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
       float b = sB[r][q];
       acc.x = fmaf(b, w4.x, acc.x); acc.y = fmaf(b, w4.y, acc.y); acc.z = fmaf(b, w4.z, acc.z); acc.w = fmaf(b, w4.w, acc.w);
     }
-    *reinterpret_cast<float4*>(z + e * H + k4) = acc;
+    ek_st4(z + e * H + k4, acc);
     const float us = scale_u ? sU[r] : 1.0f;
-    *reinterpret_cast<float4*>(act + e * ldact + k4) =
-        make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
+    ek_st4(act + e * ldact + k4, make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w)));
   }
 }
 
@@ -516,7 +523,7 @@ k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz
   for (int idx = tid; idx < EB_EDGES * (H / 4); idx += 256) {
     int r = idx / (H / 4), k4 = (idx - r * (H / 4)) * 4;
     float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (e_base + r < M) v = *reinterpret_cast<const float4*>(zb1 + (e_base + r) * ldz + k4);
+    if (e_base + r < M) v = ek_ld4(zb1 + (e_base + r) * ldz + k4);
     *reinterpret_cast<float4*>(zs + r * HP + k4) = v;
   }
   __syncthreads();
