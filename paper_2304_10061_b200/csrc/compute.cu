@@ -115,6 +115,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   AL_CHECK(k_launch_set_mact(m, (int64_t*)w.rowa.p, nc, (int*)w.m_act.p));
   AL_CHECK(k_launch_geom_fill(m, ga, (int64_t*)w.rowa.p, w));
   // ---- step 3: two-body latent ------------------------------------------------------------------------
+  m->sweep_ctr = 1;   // k_twobody0 walks forward, so the first GEMM after it starts reversed (al_next_rev)
   AL_CHECK(k_launch_twobody0(m, w, species, m->twobody[0], ntb == 1, m_cap));
   for (int k = 1; k < ntb; ++k) {
     bool last = (k == ntb - 1);

@@ -49,6 +49,9 @@ struct GemmArgs {
   // C may be NULL when x-bar itself is not needed afterwards.
   int prep; const float* zp; int ldzp; float* zbp; int ldzbp; const float* pu; float cp; int pbase;
   float c0, c1;
+  // 1: the kernel walks its row tiles from the last to the first (set by the launcher, see al_next_rev(): consecutive
+  // edge-ordered kernels alternate direction so each starts on the rows its producer left in L2)
+  int rev;
 };
 
 // precision: 0 fp32 FFMA, 1 TF32 tcgen05, 2 BF16 tcgen05 (A converted on the fly is not possible with

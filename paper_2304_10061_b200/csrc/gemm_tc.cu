@@ -188,6 +188,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       const int kb1 = g.A2 ? g.K1 / BKF : num_kb;   // k-blocks [kb1, num_kb) come from the second activation tensor
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         int mt = tile / ntn;
+        if (g.rev) mt = num_mt - 1 - mt;
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyA[stage], phase ^ 1);
           mbar_expect_tx(&fullA[stage], A_STAGE_BYTES);
@@ -279,6 +280,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     int it = 0;
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
       int mt = tile / ntn, nt = tile - mt * ntn;
+      if (g.rev) mt = num_mt - 1 - mt;
       int acc = it & 1;
       mbar_wait(&tfull[acc], (it >> 1) & 1);
       tc_fence_after();
@@ -535,7 +537,9 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
   }
 
 // precision 1: TF32 operands (rounded to nearest by the TMA load), fp32 accumulation
-int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
+int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
+  GemmArgs g = g_in;
+  g.rev = al_next_rev(m);
   int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
   int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
   CUtensorMap tmA, tmA2, tmB, tmB2;
@@ -554,7 +558,9 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g) {
 }
 
 // precision 0 on tensor cores: 3xTF32 split operands (fp32-level accuracy), tiles 128 x <=128
-int al_gemm_tc3(allegro_model* m, const GemmArgs& g) {
+int al_gemm_tc3(allegro_model* m, const GemmArgs& g_in) {
+  GemmArgs g = g_in;
+  g.rev = al_next_rev(m);
   if (!g.Bt_hi || !g.Bt_lo) { al_set_error(m, "3xTF32 GEMM: split weights missing"); return ALLEGRO_ERR_BAD_ARG; }
   int ntn = (g.N + bn_max(true) - 1) / bn_max(true);
   int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;

@@ -1,5 +1,6 @@
 // Internal structures of libb200allegro (not part of the C ABI).
 #pragma once
+#include <cstdlib>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -121,6 +122,10 @@ struct allegro_model {
   int64_t chunk_edges = 1 << 20;
   bool debug_keep = false;                // allegro_set_debug: also store tensors that are otherwise consumed on chip
   int64_t launches = 0;
+  // Alternating sweep direction of the edge-ordered kernels (GEMM row tiles, tensor-track centres): every such launch
+  // walks the edge range opposite to the one before it, so it starts on the rows its producer wrote last (still in the
+  // 126 MB L2) instead of on rows evicted long ago.  Results do not depend on the order.  B200_ALLEGRO_SWEEP=0: off.
+  int sweep_mode = -1; unsigned sweep_ctr = 0;
   std::string err;
   int sm_count = 148;
   // workspace (per chunk), grown on demand
@@ -140,6 +145,12 @@ struct allegro_model {
   } sg;
   uint64_t config_gen = 0, alloc_gen = 0; // bumped by every setter / every (re)allocation of a work buffer
 };
+
+// direction of the next edge-ordered launch (0 forward, 1 reversed), see allegro_model::sweep_mode
+inline int al_next_rev(allegro_model* m) {
+  if (m->sweep_mode < 0) { const char* e = getenv("B200_ALLEGRO_SWEEP"); m->sweep_mode = e ? atoi(e) : 1; }
+  return m->sweep_mode ? (int)(m->sweep_ctr++ & 1u) : 0;
+}
 
 // ---- profiling ------------------------------------------------------------------------------------
 enum ProfCat { PC_GEMM = 0, PC_TP_FWD, PC_TP_BWD, PC_GEOM, PC_TWOBODY0, PC_ENERGY, PC_BWD_ELEM, PC_EDGE_BWD, PC_NEIGHBORS,

@@ -60,6 +60,7 @@ struct TP2 {
   // Y-bar partials [part][M][DENV], plain stores: part = ybar_part0 + group for the V^0 contribution (FIRST, pass 1),
   // ybar_partL + group for this layer's environment contribution (pass 2); see al_ybar_layout()
   float* Ybar; int64_t ybar_pstride; int ybar_part0, ybar_partL;
+  int rev;         // 1: warps take the (centre, group) pairs from the last to the first (allegro_model::sweep_mode)
   float kv[NNZ];   // values of the fused tensor K in pattern order (dense pair table order)
 };
 
@@ -112,8 +113,9 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_fwd(const __grid_consta
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
+  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * a.ngroups) return;
+  if (a.rev) wg = (int64_t)a.nc * a.ngroups - 1 - wg;
   const int c = (int)(wg / a.ngroups), grp = (int)(wg - (int64_t)c * a.ngroups);
   const int nn = grp * 32 + lane;
   float* Gs = smem + wib * WSL;
@@ -225,8 +227,9 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp2_bwd(const __grid_consta
   extern __shared__ float4 smem4[];
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
+  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * a.ngroups) return;
+  if (a.rev) wg = (int64_t)a.nc * a.ngroups - 1 - wg;
   const int c = (int)(wg / a.ngroups), grp = (int)(wg - (int64_t)c * a.ngroups);
   const int nn = grp * 32 + lane;
   float* Gs = smem + wib * WSL;
@@ -492,5 +495,6 @@ int fill2(allegro_model* m, const TP2Common& q, TP2<NNZ>& a) {
   a.w0bar = q.w0bar; a.Ybar = (float*)w.Ybar.p; a.ybar_pstride = (int64_t)w.cap_edges * m->Denv;
   { int part[AL_MAX_LAYERS + 1]; al_ybar_layout(m, part); a.ybar_part0 = part[0]; a.ybar_partL = part[q.L]; }
   memcpy(a.kv, h.dp_val.data(), sizeof(float) * NNZ);
+  a.rev = al_next_rev(m);
   return ALLEGRO_OK;
 }

@@ -76,8 +76,9 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_fwd(const __grid_consta
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, ch = lane & 7, q = lane >> 3;
   const int ngroups = a.n / T3_CPW;
-  const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
+  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * ngroups) return;
+  if (a.rev) wg = (int64_t)a.nc * ngroups - 1 - wg;
   const int c = (int)(wg / ngroups), grp = (int)(wg - (int64_t)c * ngroups);
   const int nn = grp * T3_CPW + ch;
   float* Gs = smem + wib * WSL;
@@ -209,8 +210,9 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_consta
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, ch = lane & (CPW - 1), q = lane / CPW;
   const int ngroups = a.n / CPW;
-  const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
+  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * ngroups) return;
+  if (a.rev) wg = (int64_t)a.nc * ngroups - 1 - wg;
   const int c = (int)(wg / ngroups), grp = (int)(wg - (int64_t)c * ngroups);
   const int nn = grp * CPW + ch;
   float* Gs = smem + wib * WSL;

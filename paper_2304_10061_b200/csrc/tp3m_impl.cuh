@@ -47,8 +47,9 @@ template <int P, int WPB>
 static __global__ void __launch_bounds__(WPB * 32) k_tp3m_gamma(const __grid_constant__ TP2<Pat<P>::NNZ> a) {
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int ng = a.n / 32;
-  const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
+  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * ng) return;
+  if (a.rev) wg = (int64_t)a.nc * ng - 1 - wg;
   const int c = (int)(wg / ng), nn = (int)(wg - (int64_t)c * ng) * 32 + lane;
   const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
   float G[16];
@@ -74,8 +75,9 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3m_fwd(const __grid_const
   float* smem = reinterpret_cast<float*>(smem4);
   const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, ch = lane & 7, q = lane >> 3;
   const int ngroups = a.n / T3_CPW;
-  const int64_t wg = (int64_t)blockIdx.x * WPB + wib;
+  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
   if (wg >= (int64_t)a.nc * ngroups) return;
+  if (a.rev) wg = (int64_t)a.nc * ngroups - 1 - wg;
   const int c = (int)(wg / ngroups), grp = (int)(wg - (int64_t)c * ngroups);
   const int n0 = grp * T3_CPW, nn = n0 + ch;
   float* Gs = smem + wib * WSL;

@@ -44,6 +44,8 @@ CASES = [
     ("tp3_no_mma_tf32_cfg4", {"B200_ALLEGRO_TP3_NO_MMA": "1"}, 4, 1200, 1),   # FFMA forward for l_max = 3 in TF32 mode
     ("no_kcat_cfg1", {"B200_ALLEGRO_NO_KCAT": "1"}, 1, 1536, 0),        # separate dX-latent and x-bar GEMMs
     ("no_kcat_tf32_cfg4", {"B200_ALLEGRO_NO_KCAT": "1"}, 4, 1200, 1),
+    ("no_sweep_cfg1", {"B200_ALLEGRO_SWEEP": "0"}, 1, 1536, 1),         # every kernel walks the edges forward
+    ("no_sweep_cfg4", {"B200_ALLEGRO_SWEEP": "0"}, 4, 1200, 0),
     ("no_kcat_no_prep", {"B200_ALLEGRO_NO_KCAT": "1", "B200_ALLEGRO_NO_PREP": "1"}, 2, 3000, 0),
 ]
 
