@@ -364,6 +364,9 @@ def main():
     d2h = 3 * N * 24 + 16
 
     # ---- allegro_compute alone and allegro_neighbors alone, outside the timed region above
+    # the e2e loop above advanced its own host copy of the system and rebuilt `nb` there: rebuild the list for the
+    # device-resident positions `p` before timing single calls (a list from other positions has fewer active edges)
+    nb = model.neighbors(p, box, cfg.hp.r_cut + cfg.skin, reuse=nb)
     def _ev_ms(fn, reps):
         fn(); torch.cuda.synchronize()
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
