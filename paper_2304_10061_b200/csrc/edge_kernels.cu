@@ -516,9 +516,28 @@ k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz
   const int64_t e_base = (int64_t)blockIdx.x * EB_EDGES;
   if (e_base >= M) return;
   const int tid = threadIdx.x;
+  const int el = tid >> 3, q = tid & 7, lane = tid & 31;
+  const int64_t e = e_base + el;
+  const bool live = e < M;
+  const int64_t ee = live ? e : (int64_t)M - 1;
+  // Per-edge operands first: the first batch of u-bar partials (lane q takes parts q, q+8, ...), of Y-bar partials
+  // (lane q sums components q and q+8 over the parts), du and dB are independent loads issued before the staging
+  // loops, so their latency overlaps the staging (ncu had 65 % of this kernel's stall samples on the serial
+  // partial-sum loops that used to follow the barrier).  The order of every sum is fixed.
+  float ut[4], ya[4], yc[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    const int pu = q + 8 * k;
+    ut[k] = (pu < n_uparts) ? ubar[(int64_t)pu * ubar_pstride + ee] : 0.f;
+    const float* yp = Ybar + (int64_t)k * ybar_pstride + ee * Denv;
+    ya[k] = (k < nparts && q < Denv) ? yp[q] : 0.f;
+    yc[k] = (k < nparts && q + 8 < Denv) ? yp[q + 8] : 0.f;
+  }
+  const float duv = du[ee];
+  const float dB0 = (q < NB) ? dB[ee * NB + q] : 0.f, dB1 = (q + 8 < NB) ? dB[ee * NB + q + 8] : 0.f;
   for (int idx = tid; idx < NB * (H / 4); idx += 256) {
-    int q = idx / (H / 4), k4 = (idx - q * (H / 4)) * 4;
-    *reinterpret_cast<float4*>(Ws + q * HP + k4) = __ldg(reinterpret_cast<const float4*>(W + (size_t)(2 * S + q) * H + k4));
+    int qw = idx / (H / 4), k4 = (idx - qw * (H / 4)) * 4;
+    *reinterpret_cast<float4*>(Ws + qw * HP + k4) = __ldg(reinterpret_cast<const float4*>(W + (size_t)(2 * S + qw) * H + k4));
   }
   for (int idx = tid; idx < EB_EDGES * (H / 4); idx += 256) {
     int r = idx / (H / 4), k4 = (idx - r * (H / 4)) * 4;
@@ -527,10 +546,6 @@ k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz
     *reinterpret_cast<float4*>(zs + r * HP + k4) = v;
   }
   __syncthreads();
-  const int el = tid >> 3, q = tid & 7, lane = tid & 31;
-  const int64_t e = e_base + el;
-  const bool live = e < M;
-  const int64_t ee = live ? e : (int64_t)M - 1;
   // B-bar_q . dB_q
   float pr = 0.f;
   for (int qq = q; qq < NB; qq += 8) {
@@ -542,18 +557,28 @@ k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz
       float4 w4 = *reinterpret_cast<const float4*>(wr + k4);
       acc = fmaf(z4.x, w4.x, acc); acc = fmaf(z4.y, w4.y, acc); acc = fmaf(z4.z, w4.z, acc); acc = fmaf(z4.w, w4.w, acc);
     }
-    pr = fmaf(acc, dB[ee * NB + qq], pr);
+    pr = fmaf(acc, (qq == q) ? dB0 : (qq == q + 8) ? dB1 : dB[ee * NB + qq], pr);
   }
-  // u-bar partials: lane q takes parts q, q+8, ...
-  float ub = 0.f;
-  for (int p = q; p < n_uparts; p += 8) ub += ubar[(int64_t)p * ubar_pstride + ee];
-  pr = fmaf(ub, du[ee], pr);
-  // Y-bar partials: lane q sums components q and q+8 over the parts in fixed order
-  float ys0 = 0.f, ys1 = 0.f;
-  for (int p = 0; p < nparts; ++p) {
-    const float* yp = Ybar + (int64_t)p * ybar_pstride + ee * Denv;
-    if (q < Denv) ys0 += yp[q];
-    if (q + 8 < Denv) ys1 += yp[q + 8];
+  // remaining u-bar / Y-bar partials (more than 32 / 4 parts), four independent loads at a time
+  float ub = (ut[0] + ut[1]) + (ut[2] + ut[3]);
+  for (int p0 = q + 32; p0 < n_uparts; p0 += 32) {
+    float t[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) t[k] = (p0 + 8 * k < n_uparts) ? ubar[(int64_t)(p0 + 8 * k) * ubar_pstride + ee] : 0.f;
+    ub += (t[0] + t[1]) + (t[2] + t[3]);
+  }
+  pr = fmaf(ub, duv, pr);
+  float ys0 = (ya[0] + ya[1]) + (ya[2] + ya[3]), ys1 = (yc[0] + yc[1]) + (yc[2] + yc[3]);
+  for (int p0 = 4; p0 < nparts; p0 += 4) {
+    float a[4], b[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const float* yp = Ybar + (int64_t)(p0 + k) * ybar_pstride + ee * Denv;
+      a[k] = (p0 + k < nparts && q < Denv) ? yp[q] : 0.f;
+      b[k] = (p0 + k < nparts && q + 8 < Denv) ? yp[q + 8] : 0.f;
+    }
+    ys0 += (a[0] + a[1]) + (a[2] + a[3]);
+    ys1 += (b[0] + b[1]) + (b[2] + b[3]);
   }
 #pragma unroll
   for (int o = 1; o < 8; o <<= 1) pr += __shfl_xor_sync(FULLMASK, pr, o);   // r-bar (all 8 lanes of the edge hold it)
