@@ -73,28 +73,39 @@ __device__ __forceinline__ float ycomp(const float4* y, int b) { return reinterp
 // element (r, cc) of a register matrix stored as float2 pairs over the second index, W pairs per row
 #define TP2_REF(M, W, r, cc) (((cc) & 1) ? M[(r) * (W) + ((cc) >> 1)].y : M[(r) * (W) + ((cc) >> 1)].x)
 
-// Gamma_i[b] = c_env sum_e omega_e[l(b)] Y_e[b]   (direct loads, 4 edges in flight)
+// Gamma_i[b] = c_env sum_e omega_e[l(b)] Y_e[b]   (direct loads, 8 edges in flight).  Y_e is the same for every lane:
+// the warp loads the 8 rows as one contiguous block (LDY / 4 coalesced loads, one value per lane) and broadcasts the
+// components by shuffle, so a batch costs 8 NLV + LDY / 4 registers instead of 8 (NLV + LDY).  (ncu had 29 % of the
+// layer-1 forward's stall samples on this serial prologue with 4 edges in flight; holding two batches of 4 with
+// per-lane copies of Y took 164 registers in every kernel.)  nn = 32 * group + lane.
 template <int DENV, class A>
 __device__ __forceinline__ void gamma_pass(const A& a, int64_t e0, int64_t e1, int nn, float* G) {
-  constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3;
+  constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3, NR = LDY / 4;
+  const int lane = nn & 31;
+  const int64_t ylast = e1 * LDY - 1;
 #pragma unroll
   for (int b = 0; b < DENV; ++b) G[b] = 0.f;
-  for (int64_t e = e0; e < e1; e += 4) {
-    float om[4][NLV];
-    float4 yq[4][LDY / 4];
+  for (int64_t e = e0; e < e1; e += 8) {
+    float om[8][NLV], yr[NR];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < 8; ++i) {
       const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
 #pragma unroll
       for (int l = 0; l < NLV; ++l) om[i][l] = a.om[ee * a.ldo + l * a.n + nn];
-#pragma unroll
-      for (int q = 0; q < LDY / 4; ++q) yq[i][q] = __ldg(reinterpret_cast<const float4*>(a.Y + ee * a.ldy) + q);
     }
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int k = 0; k < NR; ++k) {
+      const int64_t idx = e * LDY + k * 32 + lane;     // rows beyond e1 are clamped into this centre's block (masked below)
+      yr[k] = __ldg(a.Y + (idx < ylast ? idx : ylast));
+    }
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
       const bool ok = e + i < e1;
 #pragma unroll
-      for (int b = 0; b < DENV; ++b) G[b] = fmaf(ok ? om[i][l_of(b)] : 0.f, ycomp<LDY>(yq[i], b), G[b]);
+      for (int b = 0; b < DENV; ++b) {
+        const float y = __shfl_sync(TP_FULLMASK, yr[(i * LDY + b) >> 5], (i * LDY + b) & 31);
+        G[b] = fmaf(ok ? om[i][l_of(b)] : 0.f, y, G[b]);
+      }
     }
   }
 #pragma unroll
