@@ -308,11 +308,19 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
         float4 ax1[4], ax2[4], ax3[4];
+        // per-row scalars (u, sigma, u of the prep stage) are prefetched with the aux rows: loaded at their point of use they
+        // were the top stall of the EPI_LATENT_LAST epilogue (ncu: long_scoreboard on the first multiply by u)
+        constexpr bool need_u = (EPI == EPI_SILU_U || EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R);
+        float ru[4], rs[4], rp[4];
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
           const int i = h * 4 + ii;
           const int row = rbase + i * 4 + rsub;
           const bool ok = row < M && col_ok;
+          const int rowc = (row < M) ? row : M - 1;
+          ru[ii] = need_u ? g.u[rowc] : 0.f;
+          rs[ii] = (EPI == EPI_LATENT_LAST) ? g.sig[rowc] : 0.f;
+          rp[ii] = PREP ? g.pu[rowc] : 0.f;
           ax1[ii] = (need1 && ok) ? ep_ld4(g.aux1 + (size_t)row * g.ld1 + col) : make_float4(0.f, 0.f, 0.f, 0.f);
           ax2[ii] = (need2 && ok) ? ep_ld4(g.aux2 + (size_t)row * g.ld2 + col) : make_float4(0.f, 0.f, 0.f, 0.f);
           ax3[ii] = (PREP && ok) ? ep_ld4(g.zp + (size_t)row * g.ldzp + col) : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -331,7 +339,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             float4 x = AUX1(i);
             float4 w = *reinterpret_cast<const float4*>(g.aux3 + cc);
             const float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w.x, w.y, w.z, w.w};
-            const float us = g.u[rr], sg = g.sig[rr];
+            const float us = ru[ii], sg = rs[ii];
             float o[4], zb[4], up = 0.f, ep4 = 0.f;
             const float cu = g.c1 * us, cus = cu * sg;
 #pragma unroll
@@ -372,13 +380,13 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
             } else {
               const float4 x = *reinterpret_cast<const float4*>(g.aux3 + cc);
-              const float cs = g.c0 * g.u[rr];
+              const float cs = g.c0 * ru[ii];
               o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
               o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
             }
             const float4 zq = ax3[ii];
             const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
-            const float cu = g.cp * g.pu[rr];
+            const float cu = g.cp * rp[ii];
             float zb[4], up = 0.f;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -404,7 +412,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               case EPI_SILU_U:
               case EPI_LATENT: {
                 ep_st4(g.out2 + (size_t)row * g.ldo2 + col, make_float4(v[0], v[1], v[2], v[3]));
-                float us = (EPI == EPI_SILU_BOTH) ? 1.0f : g.u[row];
+                float us = (EPI == EPI_SILU_BOTH) ? 1.0f : ru[ii];
                 if (EPI == EPI_LATENT) {
                   float4 x = AUX1(i);
                   float xo[4] = {x.x, x.y, x.z, x.w};
@@ -430,7 +438,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               case EPI_ADD2R: {
                 float4 x = *reinterpret_cast<const float4*>(g.aux3 + col);
                 float4 y = AUX2(i);
-                float cs = g.c0 * g.u[row];
+                float cs = g.c0 * ru[ii];
                 o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
                 o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
               } break;
