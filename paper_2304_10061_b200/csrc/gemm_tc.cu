@@ -305,6 +305,9 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         // cannot hoist them), then process it.  Halving keeps the register count low enough for 16 epilogue warps.
         constexpr bool need1 = (EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_MUL_DSILU || EPI == EPI_ADD2);
         constexpr bool need2 = (EPI == EPI_ADD2 || EPI == EPI_ADD2R) && AUX2;   // no aux2: the term is in the K-concatenation
+        // the column vector of the rank-1 / energy epilogues is the same for all 32 rows of the chunk: one load per chunk
+        float4 w3 = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R) w3 = *reinterpret_cast<const float4*>(g.aux3 + (col_ok ? col : 0));
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
         float4 ax1[4], ax2[4], ax3[4];
@@ -337,7 +340,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             const bool ok = row < M && col_ok;
             const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
             float4 x = AUX1(i);
-            float4 w = *reinterpret_cast<const float4*>(g.aux3 + cc);
+            const float4 w = w3;
             const float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w.x, w.y, w.z, w.w};
             const float us = ru[ii], sg = rs[ii];
             float o[4], zb[4], up = 0.f, ep4 = 0.f;
@@ -379,7 +382,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
               o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
             } else {
-              const float4 x = *reinterpret_cast<const float4*>(g.aux3 + cc);
+              const float4 x = w3;
               const float cs = g.c0 * ru[ii];
               o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
               o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
@@ -436,7 +439,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                 o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
               } break;
               case EPI_ADD2R: {
-                float4 x = *reinterpret_cast<const float4*>(g.aux3 + col);
+                float4 x = w3;
                 float4 y = AUX2(i);
                 float cs = g.c0 * ru[ii];
                 o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
