@@ -6,7 +6,9 @@ through the C ABI (`allegro_step_nve`): half-kick + drift, neighbor rebuild when
 `rebuild_every` steps at r_c + skin), active-edge compaction + edge basis, two-body MLP, Allegro layers,
 edge energies, fp64 sums, analytic backward, force scatter, half-kick, kinetic energy.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--precision 1] [--impl ours|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--precision 1] [--impl ours|reference]
+
+Default workload = config 3 (1,000,000 atoms, the largest single-GPU config of BASELINE.json); --config 0..4 selects the others.
 
 N > 1: launched by torchrun, one rank per GPU.  The path does not shard in this build (north_star: one
 GPU, no collectives) -> "replicas only": every rank runs an independent replica of the same workload;
@@ -30,7 +32,13 @@ if ROOT not in sys.path:
 import numpy as np
 
 FFMA_LANES_PER_SM = 128          # B200_PROFILING.md / blackwell guide: 4 SMSP x 32 fp32 FMA lanes
-TF32_OVER_BF16 = 0.5             # nominal dense ratio (B200_PROFILING.md table: 1.1 vs 2.25 PFLOP/s)
+TF32_OVER_BF16 = 0.5             # nominal dense ratio (B200_PROFILING.md table: 1.1 vs 2.25 PFLOP/s); fallback only
+
+
+def gemm_alg_bytes_per_edge(hp):
+    """ALGORITHMIC HBM bytes per active edge of the MLP group: "minimum bytes if only layer-boundary
+    tensors touch HBM: x^0 .. x^NL written once + read for the backward" = (NL + 1) * d * 4 B * 2."""
+    return 8.0 * (hp.n_layers + 1) * hp.twobody_dims[-1]
 
 
 def gemm_macs_per_edge(hp):
@@ -43,8 +51,9 @@ def gemm_macs_per_edge(hp):
     return fwd + bwd
 
 
-def gemm_bytes_per_edge(hp, kcat=True):
-    """Algorithmic HBM bytes per ACTIVE edge of the GEMM kernel group (fp32 storage): every launch reads its A
+def gemm_impl_bytes_per_edge(hp, kcat=True):
+    """IMPLEMENTATION HBM bytes per ACTIVE edge of the GEMM kernel group (fp32 storage) -- what this build's own launch
+    list moves, NOT the algorithmic minimum (gemm_alg_bytes_per_edge): every launch reads its A
     operand once and writes its outputs once; aux operands of the fused epilogues are read once.  Weights are
     L2-resident and not counted.  Mirrors the launch list of csrc/compute.cu::run_chunk (default path: last latent
     layer fused with the energy / z-bar epilogue, z-bar prep stage fused into the x-bar GEMMs, and -- kcat, the tensor-core
@@ -101,6 +110,46 @@ def tp_bytes_per_edge(hp):
         # backward: omega, V (or w0), V-bar^L, s-bar in; V-bar^{L-1} (or w0-bar), omega-bar out
         bwd += n * (nl + vin + tout + 1 + vin + nl)
     return {"tp_fwd": 4.0 * fwd, "tp_bwd": 4.0 * bwd}
+
+
+DTYPE = {0: "f32 (3xtf32)", 1: "tf32", 3: "f32"}      # precision 2 (BF16 operands) is refused by allegro_create
+
+
+def tp_flops_per_edge(hp):
+    """Algorithmic flops per ACTIVE edge of the tensor product: forward 3 nnz n per layer (K^L applied as
+    listed, 2 multiplies + 1 add per non-zero and channel), backward twice that (V-bar and Gamma-bar)."""
+    nnz = {(1, 1): [4], (2, 2): [83, 9], (3, 3): [611, 611, 16]}.get((hp.l_max, hp.n_layers))
+    if nnz is None:
+        return {"tp_fwd": 0.0, "tp_bwd": 0.0}
+    f = 3.0 * sum(nnz) * hp.n_tensor
+    return {"tp_fwd": f, "tp_bwd": 2.0 * f}
+
+
+def tf32_matmul_peak(dev, n=8192, sustain_s=4.0):
+    """MEASURED_PEAKS.json's procedure with TF32 allowed: torch.matmul fp32 n^3 (cuBLAS TF32 tensor cores), best of 10
+    (burst) and back to back for `sustain_s` seconds (sustained).  A library call used as a yardstick only."""
+    import torch
+    old = torch.backends.cuda.matmul.allow_tf32
+    torch.backends.cuda.matmul.allow_tf32 = True
+    try:
+        a = torch.randn(n, n, device=dev); b = torch.randn(n, n, device=dev); c = torch.empty(n, n, device=dev)
+        for _ in range(3):
+            torch.matmul(a, b, out=c)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = 1e30
+        for _ in range(10):
+            e0.record(); torch.matmul(a, b, out=c); e1.record(); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        reps = int(sustain_s * 1e3 / best) + 1
+        e0.record()
+        for _ in range(reps):
+            torch.matmul(a, b, out=c)
+        e1.record(); torch.cuda.synchronize()
+        fl = 2.0 * n ** 3
+        return {"burst": fl / (best * 1e-3) / 1e12, "sustained": fl * reps / (e0.elapsed_time(e1) * 1e-3) / 1e12}
+    finally:
+        torch.backends.cuda.matmul.allow_tf32 = old
 
 
 class ClockSampler(threading.Thread):
@@ -219,7 +268,7 @@ def run_decomposed(args, cfg, model, p, v, s, mass, box, dist, dev, rank, world,
         print(json.dumps({
             "metric": metric, "value": N * K / (ms_max * 1e-3), "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
-            "dtype": {0: "f32 (3xtf32)", 1: "tf32", 2: "bf16", 3: "f32"}[args.precision], "data": "synthetic",
+            "dtype": DTYPE[args.precision], "data": "synthetic",
             "config": {"workload": workload, "n_atoms": N, "precision_mode": args.precision, "dt_fs": cfg.dt_fs,
                        "rebuild_every": cfg.rebuild_every, "skin": cfg.skin,
                        "parallelism": f"spatial decomposition {grid[0]}x{grid[1]}x{grid[2]}, halo {cfg.hp.r_cut + cfg.skin} A",
@@ -233,12 +282,15 @@ def run_decomposed(args, cfg, model, p, v, s, mass, box, dist, dev, rank, world,
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    # defaults: >= 20 warm-up steps (the paper discards ~200) and a timed region long
-    # enough (0.6 s at config 1) for several nvidia-smi clock samples
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--config", type=int, default=1)
-    ap.add_argument("--precision", type=int, default=1, help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores, 3 fp32 FFMA")
+    # default = the contract line: config 3 (1 M atoms, the largest single-GPU config of BASELINE.json), 3 repeats of K steps
+    # after W warm-up steps; the timed region is seconds long, so nvidia-smi clock samples are plentiful
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--repeats", type=int, default=3, help="timed repeats of K steps each; the median is reported")
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--precision", type=int, default=1, choices=[0, 1, 3],
+                    help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores (the paper's scheme), 3 fp32 FFMA")
+    ap.add_argument("--no-peak-probe", action="store_true", help="skip the TF32 / FFMA peak measurements (~10 s)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
@@ -331,18 +383,23 @@ def main():
     for _ in range(W):
         step()
     barrier()
-    l0 = model.launches
     sampler = ClockSampler(local_rank); sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    ev0.record()
-    for _ in range(K):
-        step()
-    ev1.record()
-    barrier()
+    # R repeats of EXACTLY K steps, each bracketed by barrier + synchronize and timed with CUDA events on the launching
+    # stream; the reported region is the MEDIAN repeat ("median of >= 3 repeats")
+    reps = []
+    for _ in range(max(args.repeats, 1)):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = model.launches
+        barrier()
+        ev0.record()
+        for _ in range(K):
+            step()
+        ev1.record()
+        barrier()
+        reps.append((ev0.elapsed_time(ev1), model.launches - l0))
     sampler.stop_flag = True
-    ms = ev0.elapsed_time(ev1)
-    launches = model.launches - l0
+    model.status()                                     # deferred device-side errors (coincident atoms, bad species)
+    ms, launches = sorted(reps)[len(reps) // 2]
     n_active = model.last_active_edges()
     e_pot, e_kin = float(e.item()), float(ek.item())
     value, ms_max = aggregate_over_ranks(ms, N, K, dist, dev)
@@ -375,11 +432,11 @@ def main():
             a.record(); fn(); b.record(); torch.cuda.synchronize()
             ts.append(a.elapsed_time(b))
         return sorted(ts)[len(ts) // 2]
-    compute_ms = _ev_ms(lambda: model.compute(p, s, box, nb, want_atom_energies=False), 5)
-    energy_only_ms = _ev_ms(lambda: model.compute(p, s, box, nb, want_atom_energies=False, want_forces=False), 5)
+    compute_ms = _ev_ms(lambda: model.compute(p, s, box, nb, want_atom_energies=False), 3)
+    energy_only_ms = _ev_ms(lambda: model.compute(p, s, box, nb, want_atom_energies=False, want_forces=False), 3)
     neighbors_ms = _ev_ms(lambda: model.neighbors(p, box, cfg.hp.r_cut + cfg.skin, reuse=nb), 3)
 
-    # ---- roofline of the dominant kernel group: second pass of K steps with per-group CUDA events
+    # ---- roofline of the dominant kernel group: one more pass of K steps with per-group CUDA events on the launching stream
     groups = ["gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd", "neighbors", "nve"]
     tp_bytes = tp_bytes_per_edge(cfg.hp)
     model.profile_enable(True)
@@ -390,60 +447,103 @@ def main():
     tot_prof = sum(t for t, _ in prof.values())
     pk = peaks()
     gemm_ms, gemm_n = prof["gemm"]
-    flops_per_step = 2.0 * gemm_macs_per_edge(cfg.hp) * n_active
+    long_region = ms_max * 1e-3 > 2.0                  # seconds-long timed region runs under the power cap -> sustained peaks
+    which = "sustained" if long_region else "burst"
+
+    # measured peaks that MEASURED_PEAKS.json does not hold
+    probes = None
+    if not args.no_peak_probe:
+        probes = model.probe_peaks(2.0)                # the library's own FFMA and tcgen05 kind::tf32 issue-rate probes
+        probes["tf32_matmul_8192"] = tf32_matmul_peak(dev)   # MEASURED_PEAKS.json's procedure with TF32 allowed (cuBLAS)
+    macs = gemm_macs_per_edge(cfg.hp)
+    flops_per_step = 2.0 * macs * n_active
     gemm_tflops = flops_per_step * K / (gemm_ms * 1e-3) / 1e12 if gemm_ms > 0 else 0.0
+    nsm = torch.cuda.get_device_properties(dev).multi_processor_count
     if args.precision == 3:
-        # fp32 FFMA peak = SMs x 128 lanes x 2 flop x max SM clock (unit counts: blackwell guide; clock: MEASURED_PEAKS)
-        nsm = torch.cuda.get_device_properties(dev).multi_processor_count
-        peak, bound = nsm * FFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12, "alu"
-        peak_note = f"{nsm} SMs x {FFMA_LANES_PER_SM} FFMA lanes x 2 x {pk['sm_max_mhz']} MHz"
-    elif args.precision == 0:
-        # 3xTF32: three TF32 MMAs per algorithmic MAC, so the useful-flop peak is a third of the TF32 figure
-        peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16 / 3.0, "tensor"
-        peak_note = (f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16} / 3 "
-                     f"(3xTF32 split operands: 3 MMAs per MAC)")
+        bound = "alu"
+        if probes:
+            peak = probes["ffma"][which]
+            peak_note = (f"fp32 FFMA probe (allegro_probe_ffma), {which}: burst {probes['ffma']['burst']:.1f} / sustained "
+                         f"{probes['ffma']['sustained']:.1f} TFLOP/s; unit-count figure {nsm} SMs x {FFMA_LANES_PER_SM} lanes x 2 x "
+                         f"{pk['sm_max_mhz']} MHz = {nsm * FFMA_LANES_PER_SM * 2 * pk['sm_max_mhz'] * 1e6 / 1e12:.1f}")
+        else:
+            peak = nsm * FFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
+            peak_note = f"{nsm} SMs x {FFMA_LANES_PER_SM} FFMA lanes x 2 x {pk['sm_max_mhz']} MHz (not probed)"
     else:
-        peak, bound = pk["bf16_sustained"] * TF32_OVER_BF16, "tensor"
-        peak_note = f"bf16 sustained {pk['bf16_sustained']} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16}"
-    # K-concatenated x-bar GEMM: tensor-core modes with a 32-multiple first latent width, unless switched off
-    kcat = args.precision != 3 and cfg.hp.latent_dims[0] % 32 == 0 and not os.environ.get("B200_ALLEGRO_NO_KCAT") \
-        and not os.environ.get("B200_ALLEGRO_FP32_SIMT")
-    gemm_gbs = gemm_bytes_per_edge(cfg.hp, kcat) * n_active * K / (gemm_ms * 1e-3) / 1e9 if gemm_ms > 0 else 0.0
-    f_compute, f_hbm = gemm_tflops / peak, gemm_gbs / pk["hbm_gbs"]
-    comp = {"bound": bound, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s", "frac": f_compute, "peak_note": peak_note}
-    hbm = {"bound": "hbm", "achieved": gemm_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm,
-           "peak_note": f"copy bandwidth ({pk['src']}); algorithmic bytes = {gemm_bytes_per_edge(cfg.hp, kcat)} B per active edge"}
-    top = hbm if f_hbm > f_compute else comp       # the binding roofline is the one with the larger fraction
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r1_traffic.json")
-    if os.path.exists(tpath):   # dram__bytes_read+write per GEMM launch from the committed ncu --set full capture
+        bound = "tensor"
+        div = 3.0 if args.precision == 0 else 1.0      # 3xTF32: three TF32 MMAs per algorithmic MAC
+        if probes:
+            tm = probes["tf32_matmul_8192"]
+            peak = tm[which] / div
+            peak_note = (f"TF32 8192^3 torch.matmul (cuBLAS, allow_tf32), measured in this run the way MEASURED_PEAKS.json measures "
+                         f"bf16: burst {tm['burst']:.1f} / sustained {tm['sustained']:.1f} TFLOP/s, {which} used (timed region "
+                         f"{ms_max * 1e-3:.2f} s); tcgen05 kind::tf32 issue-rate probe {probes['tf32_mma']['burst']:.1f} / "
+                         f"{probes['tf32_mma']['sustained']:.1f}; bf16 {pk['bf16_burst']} / {pk['bf16_sustained']} ({pk['src']})"
+                         + (" ; / 3 for 3xTF32 split operands" if div > 1 else ""))
+        else:
+            base = pk["bf16_sustained"] if long_region else pk["bf16_burst"]
+            peak = base * TF32_OVER_BF16 / div
+            peak_note = f"FALLBACK (no probe): bf16 {which} {base} TF/s ({pk['src']}) x nominal tf32/bf16 ratio {TF32_OVER_BF16}" + (" / 3" if div > 1 else "")
+    # K-concatenated x-bar GEMM: tensor-core modes with a 32-multiple first latent width
+    kcat = args.precision != 3 and cfg.hp.latent_dims[0] % 32 == 0
+    alg_b, impl_b = gemm_alg_bytes_per_edge(cfg.hp), gemm_impl_bytes_per_edge(cfg.hp, kcat)
+    secs = gemm_ms * 1e-3
+    alg_gbs = alg_b * n_active * K / secs / 1e9 if gemm_ms > 0 else 0.0
+    impl_gbs = impl_b * n_active * K / secs / 1e9 if gemm_ms > 0 else 0.0
+    f_compute, f_hbm = gemm_tflops / peak, alg_gbs / pk["hbm_gbs"]
+    comp = {"bound": bound, "achieved": gemm_tflops, "peak": peak, "unit": "TFLOP/s", "frac": f_compute, "peak_note": peak_note,
+            "algorithmic_flops_per_edge": 2.0 * macs}
+    hbm = {"bound": "hbm", "achieved": alg_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm,
+           "peak_note": f"copy bandwidth ({pk['src']}); algorithmic bytes = 8 (NL+1) d = {alg_b:.0f} B per active edge "
+                        f"(SURVEY.md 8(d): x^0..x^NL written once + read once for the backward)"}
+    top = hbm if f_hbm > f_compute else comp           # a kernel's fraction = max(bytes / t / HBM, flops / t / peak)
+    traffic = traffic_src = None
+    tpath = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if os.path.exists(tpath):   # dram__bytes_read + write per GEMM launch from the committed ncu --set full capture
         tj = json.load(open(tpath)).get(f"config{cfg.index}_precision{args.precision}")
         if tj:
-            traffic = tj["gemm_dram_bytes_per_launch"]
-    roofline = {"bound": top["bound"], "kernel": {0: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., SPLIT> (3xTF32)", 1: "MLP GEMM group (fwd+bwd), k_gemm_tf32", 2: "MLP GEMM group (fwd+bwd), k_gemm_tf32", 3: "MLP GEMM group (fwd+bwd), k_gemm_simt"}[args.precision],
-                "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"], "traffic": traffic,
-                "algorithmic_bytes_per_launch": gemm_bytes_per_edge(cfg.hp, kcat) * n_active * K / max(gemm_n, 1),
+            traffic, traffic_src = tj["gemm_dram_bytes_per_launch"], tj.get("source")
+    kname = {0: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., SPLIT> (3xTF32)", 1: "MLP GEMM group (fwd+bwd), k_gemm_tf32",
+             3: "MLP GEMM group (fwd+bwd), k_gemm_simt"}[args.precision]
+    per_launch = K / max(gemm_n, 1)
+    roofline = {"bound": top["bound"], "kernel": kname,
+                "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"],
+                "traffic": traffic, "traffic_source": traffic_src,
+                "algorithmic_bytes_per_launch": alg_b * n_active * per_launch,
+                "algorithmic_flops_per_launch": flops_per_step * per_launch,
                 "peak_note": top["peak_note"], "compute_roofline": comp, "hbm_roofline": hbm,
+                # what this build's launch list actually moves (every A operand, aux operand and output once): NOT algorithmic
+                "implementation_bytes_per_edge": impl_b, "implementation_hbm_gbs": impl_gbs,
+                "implementation_hbm_frac": impl_gbs / pk["hbm_gbs"],
                 "launches_per_step": gemm_n / K, "avg_launch_ms": gemm_ms / max(gemm_n, 1),
                 "share_of_step": gemm_ms / tot_prof if tot_prof else None,
                 "groups_ms_per_step": {g: round(t / K, 4) for g, (t, _) in prof.items()},
+                "measured_peaks_tflops": probes,
                 # the tensor-track kernels against the HBM roofline (north_star: gather/tensor-product/scatter >= 50 %)
                 "tensor_track_hbm": {k: {"achieved": tp_bytes[k] * n_active * K / (prof[k][0] * 1e-3) / 1e9 if prof[k][0] > 0 else 0.0,
                                          "peak": pk["hbm_gbs"], "unit": "GB/s",
                                          "frac": (tp_bytes[k] * n_active * K / (prof[k][0] * 1e-3) / 1e9 / pk["hbm_gbs"]) if prof[k][0] > 0 else 0.0,
                                          "algorithmic_bytes_per_edge": tp_bytes[k]} for k in ("tp_fwd", "tp_bwd")}}
+    if probes and cfg.hp.l_max == 3:
+        # config 4: the tensor product is bound by the fp32 pipes, not HBM: report it against the FFMA probe too
+        fl = tp_flops_per_edge(cfg.hp)
+        roofline["tensor_track_alu"] = {k: {"achieved": fl[k] * n_active * K / (prof[k][0] * 1e-3) / 1e12 if prof[k][0] > 0 else 0.0,
+                                            "peak": probes["ffma"][which], "unit": "TFLOP/s",
+                                            "frac": (fl[k] * n_active * K / (prof[k][0] * 1e-3) / 1e12 / probes["ffma"][which]) if prof[k][0] > 0 else 0.0,
+                                            "algorithmic_flops_per_edge": fl[k]} for k in ("tp_fwd", "tp_bwd")}
 
     out = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": {0: "f32 (3xtf32)", 1: "tf32", 2: "bf16", 3: "f32"}[args.precision], "data": "synthetic",
+        "dtype": DTYPE[args.precision], "data": "synthetic",
         "config": {"workload": workload, "n_atoms": N, "active_edges": n_active, "candidate_edges": nb.n_edges,
                    "precision_mode": args.precision, "dt_fs": cfg.dt_fs, "rebuild_every": cfg.rebuild_every, "skin": cfg.skin,
                    "l2": "per-step working set (edge activations, several GB) is far larger than the 126 MB L2",
                    "parallelism": "replicas only" if world > 1 else "single GPU"},
         "timesteps_per_s": K / (ms_max * 1e-3), "ns_per_day": K / (ms_max * 1e-3) * cfg.dt_fs * 0.0864,
+        "repeats_ms_per_step": [round(t / K, 4) for t, _ in reps], "repeat_reported": "median",
         "e_pot": e_pot, "e_kin": e_kin,
-        # medians of 5 / 5 / 3 calls, CUDA events: energy+forces alone, energy only (no backward), list build alone
+        # medians of 3 calls, CUDA events: energy+forces alone, energy only (no backward), list build alone
         "compute_only_ms": compute_ms, "energy_only_ms": energy_only_ms, "neighbors_only_ms": neighbors_ms,
         "gpu_launches": launches,
         "clocks": sampler.summary(),
@@ -451,14 +551,26 @@ def main():
         "roofline": roofline,
     }
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        run, n_c, cores = oracle_sample(cfg, pos, sp, box, {0: 192, 1: 3072, 2: 512, 3: 512, 4: 256}[cfg.index])
-        run()
-        reps, tt = 0, 0.0
-        while tt < 10.0 and reps < 200:
-            tt += run(); reps += 1
-        out["cpu_baseline"] = {"value": n_c * reps / tt, "unit": unit, "cores": cores, "kind": "oracle",
-                               "sample": f"energy+forces of {n_c} contiguous centres (all their edges) of {workload}, "
-                                         f"{reps} repeats, {tt:.1f} s"}
+        n_all, n_one = {0: (192, 192), 1: (3072, 768), 2: (512, 128), 3: (512, 128), 4: (256, 64)}[cfg.index]
+        import torch as _t
+        ncores = _t.get_num_threads()
+
+        def timed(n_c, budget):
+            run, n_c, _ = oracle_sample(cfg, pos, sp, box, n_c)
+            run()
+            reps_, tt = 0, 0.0
+            while tt < budget and reps_ < 200:
+                tt += run(); reps_ += 1
+            return n_c * reps_ / tt, n_c, reps_, tt
+        v_all, nc_all, r_all, t_all = timed(n_all, 8.0)
+        _t.set_num_threads(1)
+        v_one, nc_one, r_one, t_one = timed(n_one, 8.0)
+        _t.set_num_threads(ncores)
+        out["cpu_baseline"] = {"value": v_all, "unit": unit, "cores": ncores, "kind": "oracle",
+                               "sample": f"energy+forces of {nc_all} contiguous centres (all their edges) of {workload}, "
+                                         f"{r_all} repeats, {t_all:.1f} s",
+                               "one_thread": {"value": v_one, "unit": unit, "cores": 1,
+                                              "sample": f"{nc_one} contiguous centres, {r_one} repeats, {t_one:.1f} s"}}
     if rank == 0:
         print(json.dumps(out))
     if dist is not None:

@@ -58,8 +58,8 @@ typedef struct {
   double resid_alpha[8];    /* per layer residual mixing coefficient (S7) */
   int32_t precision;        /* MLP GEMM arithmetic (accumulation is fp32 in all modes):
                                0 fp32 on the tensor cores (3xTF32 split operands, meets the fp32 tolerances),
-                               1 TF32 tensor cores (the paper's scheme), 2 reserved (BF16 operands),
-                               3 fp32 on the FFMA pipes (slowest, most accurate) */
+                               1 TF32 tensor cores (the paper's scheme), 2 BF16 operands: NOT BUILT, allegro_create returns
+                               ALLEGRO_ERR_UNIMPLEMENTED, 3 fp32 on the FFMA pipes (slowest, most accurate) */
   int64_t max_atoms, max_edges; /* capacity hints, 0 = grow on demand (+5 %) */
 } allegro_hparams;
 
@@ -131,6 +131,14 @@ int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* spe
 int allegro_compute_local(allegro_model* m, const double* pos, const int32_t* species, int64_t n_atoms, int64_t n_local,
                           const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom, double* force);
 
+/* Deferred errors of the device-pointer calls.  allegro_compute / allegro_compute_local / allegro_edge_energies /
+ * allegro_step_nve return after enqueueing, so what only the kernels can see -- coincident atoms (r = 0; the survey's
+ * ALLEGRO_ERR_NONFINITE) and species values outside [0, n_species) (ALLEGRO_ERR_BAD_ARG; table
+ * look-ups clamp, nothing is read out of bounds) -- is recorded in a device status word.  allegro_status synchronises the
+ * model's stream, returns the recorded error (ALLEGRO_OK if none) and clears it.  The same check runs inside every call
+ * that synchronises anyway: the _host variants, and allegro_step_nve on the steps that rebuild the list. */
+int allegro_status(allegro_model* m);
+
 /* One velocity-Verlet NVE step: v += dt/2 F/m; r += dt v; [rebuild list at cutoff
  * r_cut+skin if *step_counter % rebuild_every == 0]; F; v += dt/2 F/m.  `force` f64[N*3] (device) must
  * hold F(r) of the current positions on entry (call allegro_compute once before the first step) and
@@ -173,6 +181,15 @@ int allegro_step_nve_host(allegro_model* m, double* pos, double* vel, double* fo
  * flops are computed by the caller from allegro_last_active_edges).  host pointers. */
 int allegro_profile_enable(allegro_model* m, int32_t on);
 int allegro_profile_read(allegro_model* m, const char* name, double* ms, int64_t* launches);
+
+/* Roofline denominators for bench.py (the TF32 tensor-core and fp32 FFMA peaks are not in the
+ * driver's MEASURED_PEAKS.json and have to be measured on the box).  allegro_probe_ffma: fp32 FMA rate of the SIMT pipes
+ * (16 independent FMA chains per thread, no memory traffic).  allegro_probe_tf32: issue rate of tcgen05.mma kind::tf32
+ * (128 x 256 x 8 MMAs back to back on shared-memory-resident operands, one CTA per SM, no loads, no epilogue).  Each
+ * returns TFLOP/s (host f64): the best of 10 launches (burst) and the average over `sustain_s` seconds of back-to-back
+ * launches (sustained, i.e. under the power cap).  Synchronises the model's stream.  Not part of the hot path. */
+int allegro_probe_ffma(allegro_model* m, double sustain_s, double* burst_tflops, double* sustained_tflops);
+int allegro_probe_tf32(allegro_model* m, double sustain_s, double* burst_tflops, double* sustained_tflops);
 
 /* Counters for tests/bench: number of kernels launched by the library since creation (host). */
 int allegro_launch_count(const allegro_model* m, int64_t* launches);

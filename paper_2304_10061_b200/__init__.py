@@ -74,7 +74,7 @@ EXPORTS = [
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
     "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps", "allegro_compute_local",
-    "allegro_nve_kick", "allegro_kinetic_energy",
+    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32",
     "allegro_last_error",
 ]
 
@@ -124,6 +124,9 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_graph_steps.argtypes = [vp, P(i64)]
     lib.allegro_last_active_edges.argtypes = [vp, P(i64)]
     lib.allegro_debug_tensor.argtypes = [vp, C.c_char_p, vp, P(i64)]
+    lib.allegro_status.argtypes = [vp]
+    lib.allegro_probe_ffma.argtypes = [vp, C.c_double, P(C.c_double), P(C.c_double)]
+    lib.allegro_probe_tf32.argtypes = [vp, C.c_double, P(C.c_double), P(C.c_double)]
     lib.allegro_last_error.argtypes = [vp]
     lib.allegro_last_error.restype = C.c_char_p
     for name in EXPORTS:
@@ -195,9 +198,17 @@ class NeighborList:
         return rp, j, s
 
     def free(self):
-        if self._h:
+        # the list's buffers came from the model's allocator: free only while the model is alive (allegro_destroy does
+        # not own lists; a list that outlives its model is abandoned to the allocator's own teardown)
+        if self._h and self._model._h:
             self._model._lib.allegro_nbr_free(self._model._h, self._h)
-            self._h = C.c_void_p(None)
+        self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.free()
+        except Exception:
+            pass
 
 
 class Allegro:
@@ -271,6 +282,21 @@ class Allegro:
         v = C.c_int64(0)
         self._check(self._lib.allegro_graph_steps(self._h, C.byref(v)))
         return v.value
+
+    def status(self) -> None:
+        """allegro_status: synchronise the model's stream and raise what the device-pointer calls since the last check
+        flagged (coincident atoms -> ALLEGRO_ERR_NONFINITE, species out of range -> ALLEGRO_ERR_BAD_ARG)."""
+        self._check(self._lib.allegro_status(self._h))
+
+    def probe_peaks(self, sustain_s: float = 2.0) -> dict:
+        """allegro_probe_ffma / allegro_probe_tf32 -> TFLOP/s, burst and sustained (roofline denominators of bench.py)."""
+        self._sync_stream()
+        out = {}
+        for name, fn in (("ffma", self._lib.allegro_probe_ffma), ("tf32_mma", self._lib.allegro_probe_tf32)):
+            b, s = C.c_double(0), C.c_double(0)
+            self._check(fn(self._h, float(sustain_s), C.byref(b), C.byref(s)))
+            out[name] = {"burst": b.value, "sustained": s.value}
+        return out
 
     def last_active_edges(self) -> int:
         v = C.c_int64(0)

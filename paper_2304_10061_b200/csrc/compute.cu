@@ -71,7 +71,7 @@ void al_work_free(allegro_model* m) {
   Work& w = *m->work;
   std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.sig, &w.B, &w.dB, &w.Y,
                               &w.XF, &w.WE, &w.gamma, &w.XB0, &w.XB1, &w.ZB0, &w.ZB1, &w.G, &w.OB, &w.VB0, &w.VB1,
-                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom, &w.nh_scal};
+                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom, &w.nh_scal, &w.host_stage};
   for (auto* b : all) al_release(m, *b);
   for (auto* v : {&w.tb_z, &w.tb_a, &w.XS, &w.OM, &w.T}) for (auto& b : *v) al_release(m, b);
   for (auto* vv : {&w.lat_z, &w.lat_a}) for (auto& v : *vv) for (auto& b : v) al_release(m, b);
@@ -85,8 +85,8 @@ static GemmArgs mk(const float* A, int lda, const Dense& D, bool transposed_weig
   // transposed_weight = true : backward dX = dY W^T -> Bt = W  [fi][fo], N = fi, K = fo
   GemmArgs g{};
   g.A = A; g.lda = lda;
-  if (!transposed_weight) { g.Bt = D.Wt; g.Bt16 = D.Wth; g.Bt_hi = D.Wt_hi; g.Bt_lo = D.Wt_lo; g.ldb = D.fi; g.N = D.fo; g.K = D.fi; }
-  else { g.Bt = D.W; g.Bt16 = D.Wh; g.Bt_hi = D.W_hi; g.Bt_lo = D.W_lo; g.ldb = D.fo; g.N = D.fi; g.K = D.fo; }
+  if (!transposed_weight) { g.Bt = D.Wt; g.Bt_hi = D.Wt_hi; g.Bt_lo = D.Wt_lo; g.ldb = D.fi; g.N = D.fo; g.K = D.fi; }
+  else { g.Bt = D.W; g.Bt_hi = D.W_hi; g.Bt_lo = D.W_lo; g.ldb = D.fo; g.N = D.fi; g.K = D.fo; }
   g.C = C; g.ldc = ldc; g.m_cap = m_cap; g.m_ptr = m_ptr; g.epi = epi;
   return g;
 }
@@ -268,7 +268,7 @@ int al_compute_local_impl(allegro_model* m, const double* pos, const int32_t* sp
   AL_CHECK(work_reserve(m, nb, N));
   Work& w = *m->work;
   double* ea = e_atom ? e_atom : (double*)w.eatom.p;
-  if (force) AL_CHECK(k_launch_zero_f64(m, force, 3 * N));
+  AL_CHECK(k_launch_begin_compute(m, force, species, N, (int*)w.m_act.p));   // zero the forces, validate the species
   AL_CUDA(m, cudaMemsetAsync((int*)w.m_act.p + 2, 0, 8, m->stream));   // total active edges of this call
   for (Chunk ch : nb->chunks) {
     if (ch.c0 >= n_local) break;
@@ -304,6 +304,25 @@ extern "C" int allegro_edge_energies(allegro_model* m, const double* pos, const 
   return al_compute_impl(m, pos, species, n_atoms, box, nbr, e_total, nullptr, nullptr, e_edge);
 }
 
+// Status word written by the kernels (Work::m_act[1]): bit 0 = coincident atoms (r = 0), bit 1 = species out of range.
+// Reads it after synchronising the stream, clears it and turns it into an error code.
+int al_check_status(allegro_model* m) {
+  if (!m->work || !m->work->m_act.p) return ALLEGRO_OK;
+  int flags[2] = {0, 0};
+  AL_CUDA(m, cudaStreamSynchronize(m->stream));
+  AL_CUDA(m, cudaMemcpy(flags, m->work->m_act.p, 8, cudaMemcpyDeviceToHost));
+  if (!flags[1]) return ALLEGRO_OK;
+  AL_CUDA(m, cudaMemset((int*)m->work->m_act.p + 1, 0, 4));
+  if (flags[1] & 2) { al_set_error(m, "species value outside [0, n_species)"); return ALLEGRO_ERR_BAD_ARG; }
+  al_set_error(m, "coincident atoms (r = 0)");
+  return ALLEGRO_ERR_NONFINITE;
+}
+
+extern "C" int allegro_status(allegro_model* m) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  return al_check_status(m);
+}
+
 extern "C" int allegro_compute_host(allegro_model* m, const double* pos, const int32_t* species, int64_t N,
                                     const double box[3], const allegro_nbr* nbr, double* e_total, double* e_atom,
                                     double* force) {
@@ -314,20 +333,19 @@ extern "C" int allegro_compute_host(allegro_model* m, const double* pos, const i
   if ((rc = al_alloc(m, &dp, N * 24 + 16)) || (rc = al_alloc(m, &ds, N * 4 + 16)) || (rc = al_alloc(m, &de, 16)) ||
       (rc = al_alloc(m, &dea, N * 8 + 16)) || (rc = al_alloc(m, &df, N * 24 + 16)))
     goto done;
-  cudaMemcpyAsync(dp, pos, N * 24, cudaMemcpyHostToDevice, st);
-  cudaMemcpyAsync(ds, species, N * 4, cudaMemcpyHostToDevice, st);
+  {
+    cudaError_t e = cudaMemcpyAsync(dp, pos, N * 24, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ds, species, N * 4, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { al_set_error(m, std::string("allegro_compute_host, host->device copy: ") + cudaGetErrorString(e)); rc = ALLEGRO_ERR_CUDA; goto done; }
+  }
   rc = al_compute_impl(m, (double*)dp, (int32_t*)ds, N, box, nbr, (double*)de, (double*)dea, force ? (double*)df : nullptr, nullptr);
   if (rc == ALLEGRO_OK) {
-    cudaMemcpyAsync(e_total, de, 8, cudaMemcpyDeviceToHost, st);
-    if (e_atom) cudaMemcpyAsync(e_atom, dea, N * 8, cudaMemcpyDeviceToHost, st);
-    if (force) cudaMemcpyAsync(force, df, N * 24, cudaMemcpyDeviceToHost, st);
-    cudaError_t e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) { al_set_error(m, cudaGetErrorString(e)); rc = ALLEGRO_ERR_CUDA; }
-    else {
-      int flags[4];
-      cudaMemcpy(flags, m->work->m_act.p, 16, cudaMemcpyDeviceToHost);
-      if (flags[1] & 1) { al_set_error(m, "coincident atoms (r = 0)"); rc = ALLEGRO_ERR_NONFINITE; }
-    }
+    cudaError_t e = cudaMemcpyAsync(e_total, de, 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && e_atom) e = cudaMemcpyAsync(e_atom, dea, N * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && force) e = cudaMemcpyAsync(force, df, N * 24, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { al_set_error(m, std::string("allegro_compute_host, device->host copy: ") + cudaGetErrorString(e)); rc = ALLEGRO_ERR_CUDA; }
+    else rc = al_check_status(m);
   }
 done:
   cudaStreamSynchronize(st);
@@ -428,7 +446,10 @@ extern "C" int allegro_step_nve(allegro_model* m, double* pos, double* vel, doub
     }
   }
   AL_CHECK(k_launch_nve_kick_drift(m, pos, vel, force, species, mass, N, dt_fs, true));
-  if (rebuild) AL_CHECK(al_neighbors_impl(m, pos, N, box, m->hp.r_cut + skin, nbr));
+  if (rebuild) {
+    AL_CHECK(al_neighbors_impl(m, pos, N, box, m->hp.r_cut + skin, nbr));
+    AL_CHECK(al_check_status(m));   // the list build synchronised: surface what the steps since the last rebuild flagged
+  }
   AL_CHECK(step_tail(m, pos, vel, force, species, mass, N, box, dt_fs, *nbr, e_pot, e_kin, false));
   if (graphs && !m->sg.disabled) m->sg.warm = make_key();   // the state the next step will see if nothing changes
   (*step_counter)++;
@@ -477,7 +498,8 @@ extern "C" int allegro_step_nve_host(allegro_model* m, double* pos, double* vel,
                                      int32_t rebuild_every, double skin, allegro_nbr** nbr, int64_t* step_counter,
                                      double* e_pot, double* e_kin) {
   if (!m || !pos || !vel || !force || !species || !mass || !e_pot || !e_kin) return ALLEGRO_ERR_BAD_ARG;
-  static thread_local DevBuf stage;   // [pos | vel | force | e_pot, e_kin | mass | species]
+  if (!m->work) m->work = new Work();
+  DevBuf& stage = m->work->host_stage;   // [pos | vel | force | e_pot, e_kin | mass | species], owned by the model
   size_t b3 = (size_t)N * 24, off_e = 3 * b3, off_m = off_e + 16, off_s = off_m + (size_t)m->S * 8;
   AL_CHECK(al_reserve(m, stage, off_s + (size_t)N * 4 + 64));
   char* d = (char*)stage.p;
@@ -496,7 +518,7 @@ extern "C" int allegro_step_nve_host(allegro_model* m, double* pos, double* vel,
   AL_CUDA(m, cudaMemcpyAsync(e_pot, d + off_e, 8, cudaMemcpyDeviceToHost, st));
   AL_CUDA(m, cudaMemcpyAsync(e_kin, d + off_e + 8, 8, cudaMemcpyDeviceToHost, st));
   AL_CUDA(m, cudaStreamSynchronize(st));
-  return ALLEGRO_OK;
+  return al_check_status(m);
 }
 
 extern "C" int allegro_debug_tensor(allegro_model* m, const char* name, float* out, int64_t* n_floats) {

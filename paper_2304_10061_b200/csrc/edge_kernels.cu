@@ -90,17 +90,23 @@ __device__ __forceinline__ double ipow_d(double x, int n) {
   return r;
 }
 
+// species index clamped into [0, S): an out-of-range value (caller error) is reported through the status flag by
+// k_zero_check (ALLEGRO_ERR_BAD_ARG at the next host synchronisation) and must never index a table out of bounds
+__device__ __forceinline__ int zc(int z, int S) { return min(max(z, 0), S - 1); }
+
 // ---- active-edge count / compaction + geometry ------------------------------------------------------
 // rc: the cutoff of this ordered pair, r_cut or r_c[Z_i][Z_j] (allegro_set_pair_cutoffs)
 __device__ __forceinline__ bool edge_vec(const EdgeGeomArgs& a, int i, int64_t e, int& j, double& dx, double& dy,
                                          double& dz, double& r2, double& rc) {
   j = a.j[e];
-  rc = a.rc_pair ? a.rc_pair[a.species[i] * a.S + a.species[j]] : a.rc;
-  dx = (a.pos[3 * (int64_t)j + 0] - a.pos[3 * (int64_t)i + 0]) + (double)a.shift[3 * e + 0] * a.box[0];
-  dy = (a.pos[3 * (int64_t)j + 1] - a.pos[3 * (int64_t)i + 1]) + (double)a.shift[3 * e + 1] * a.box[1];
-  dz = (a.pos[3 * (int64_t)j + 2] - a.pos[3 * (int64_t)i + 2]) + (double)a.shift[3 * e + 2] * a.box[2];
-  r2 = dx * dx + dy * dy + dz * dz;
-  return r2 < rc * rc;
+  rc = a.rc_pair ? a.rc_pair[zc(a.species[i], a.S) * a.S + zc(a.species[j], a.S)] : a.rc;
+  dx = __dadd_rn(a.pos[3 * (int64_t)j + 0] - a.pos[3 * (int64_t)i + 0], __dmul_rn((double)a.shift[3 * e + 0], a.box[0]));
+  dy = __dadd_rn(a.pos[3 * (int64_t)j + 1] - a.pos[3 * (int64_t)i + 1], __dmul_rn((double)a.shift[3 * e + 1], a.box[1]));
+  dz = __dadd_rn(a.pos[3 * (int64_t)j + 2] - a.pos[3 * (int64_t)i + 2], __dmul_rn((double)a.shift[3 * e + 2], a.box[2]));
+  // the canonical expression of the list build: (dx*dx + dy*dy) + dz*dz, fp64, no FMA contraction, so the
+  // active-edge decision r2 < rc^2 is the same one an IEEE host evaluation takes (bit-exact counts with pair cutoffs)
+  r2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+  return r2 < __dmul_rn(rc, rc);
 }
 
 __global__ void k_active_count(EdgeGeomArgs a, int* __restrict__ deg) {
@@ -145,7 +151,7 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
       double inv = 1.0 / r;
       float hx = (float)(dx * inv), hy = (float)(dy * inv), hz = (float)(dz * inv);
       ei[o] = i; ej[o] = j;
-      sig[o] = (float)sigma[a.species[i]];
+      sig[o] = (float)sigma[zc(a.species[i], a.S)];
       geo[o] = make_float4(hx, hy, hz, (float)r);
       // envelope (fp64; PAPER.md:222 via SURVEY S2)
       double x = r / rc, p = (double)a.p;
@@ -156,7 +162,7 @@ __global__ void k_geom_fill(EdgeGeomArgs a, const int64_t* __restrict__ rowa, in
       double pref = sqrt(2.0 / rc);
       if (a.bfreq) {
         // trained per-ordered-pair angular frequencies w_n: b_n = sqrt(2/rc) sin(w_n r) / r
-        const double* wq = a.bfreq + ((size_t)a.species[i] * a.S + a.species[j]) * a.NB;
+        const double* wq = a.bfreq + ((size_t)zc(a.species[i], a.S) * a.S + zc(a.species[j], a.S)) * a.NB;
         for (int nb = 0; nb < a.NB; ++nb) {
           double wn = wq[nb], sn, cn;
           sincos(wn * r, &sn, &cn);
@@ -209,8 +215,8 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
   }
   if (tid < TB0_EDGES) {
     int64_t e = e_base + tid;
-    sZi[tid] = (e < M) ? species[ei[e]] : 0;
-    sZj[tid] = (e < M) ? species[ej[e]] : 0;
+    sZi[tid] = (e < M) ? zc(species[ei[e]], S) : 0;
+    sZj[tid] = (e < M) ? zc(species[ej[e]], S) : 0;
     sU[tid] = (e < M) ? u[e] : 0.f;
   }
   __syncthreads();
@@ -419,7 +425,7 @@ __global__ void __launch_bounds__(256) k_tp_bwd(TPArgs a) {
 
 // ---- energies (fp64 final stage) -------------------------------------------------------------
 __global__ void k_energy(const int64_t* __restrict__ rowa, int nc, int64_t c0, const float* __restrict__ xf, int d,
-                         const double* __restrict__ w_eff, const int32_t* __restrict__ species,
+                         const double* __restrict__ w_eff, const int32_t* __restrict__ species, int S,
                          const double* __restrict__ sigma, const double* __restrict__ mu, double* __restrict__ e_atom) {
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= nc) return;
@@ -429,7 +435,7 @@ __global__ void k_energy(const int64_t* __restrict__ rowa, int nc, int64_t c0, c
     for (int k = lane; k < d; k += 32) acc += (double)xf[e * d + k] * w_eff[k];
   acc = warp_sum_d(acc);
   if (lane == 0) {
-    int z = species[c0 + warp];
+    int z = zc(species[c0 + warp], S);
     e_atom[c0 + warp] = sigma[z] * acc + mu[z];
   }
 }
@@ -437,7 +443,7 @@ __global__ void k_energy(const int64_t* __restrict__ rowa, int nc, int64_t c0, c
 // E-hat_i from the edge-energy partials written by the last latent GEMM (EPI_LATENT_LAST): lanes take the
 // center's edges, each sums its partials in fixed order, then a fixed-order warp reduction in fp64.
 __global__ void k_energy_parts(const int64_t* __restrict__ rowa, int nc, int64_t c0, const double* __restrict__ epart,
-                               int nparts, int64_t pstride, const int32_t* __restrict__ species,
+                               int nparts, int64_t pstride, const int32_t* __restrict__ species, int S,
                                const double* __restrict__ sigma, const double* __restrict__ mu, double* __restrict__ e_atom) {
   int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (warp >= nc) return;
@@ -450,7 +456,7 @@ __global__ void k_energy_parts(const int64_t* __restrict__ rowa, int nc, int64_t
   }
   acc = warp_sum_d(acc);
   if (lane == 0) {
-    int z = species[c0 + warp];
+    int z = zc(species[c0 + warp], S);
     e_atom[c0 + warp] = sigma[z] * acc + mu[z];
   }
 }
@@ -609,6 +615,11 @@ k_edge_bwd(const int* __restrict__ m_ptr, const float* __restrict__ zb1, int ldz
   }
 }
 
+__global__ void k_zero_check(double* force, int64_t n3, const int32_t* __restrict__ species, int64_t n, int S, int* flags) {
+  int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+  if (force && i < n3) force[i] = 0.0;
+  if (i < n && (unsigned)species[i] >= (unsigned)S) atomicOr(&flags[1], 2);
+}
 __global__ void k_zero_f64(double* p, int64_t n) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i < n) p[i] = 0.0;
@@ -616,11 +627,11 @@ __global__ void k_zero_f64(double* p, int64_t n) {
 
 // ---- NVE ---------------------------------------------------------------------------------
 #define ACC_CONV 9.648533212e-3
-__global__ void k_nve(double* pos, double* vel, const double* force, const int32_t* species, const double* mass, int64_t n,
-                      double dt, int drift) {
+__global__ void k_nve(double* pos, double* vel, const double* force, const int32_t* species, const double* mass, int S,
+                      int64_t n, double dt, int drift) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
-  double im = ACC_CONV / mass[species[i]];
+  double im = ACC_CONV / mass[zc(species[i], S)];
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     double v = vel[3 * i + k] + (0.5 * dt) * (force[3 * i + k] * im);
@@ -637,7 +648,7 @@ __global__ void k_zbl(EdgeGeomArgs a, const double* __restrict__ zn, double* __r
   if (warp >= a.nc) return;
   int i = (int)(a.c0 + warp);
   int64_t b = a.row_ptr[i], e = a.row_ptr[i + 1];
-  const double zi = zn[a.species[i]], p = (double)a.p;
+  const double zi = zn[zc(a.species[i], a.S)], p = (double)a.p;
   double es = 0.0, fx = 0.0, fy = 0.0, fz = 0.0;
   for (int64_t k = b + lane; k < e; k += 32) {
     int j = a.j[k];
@@ -647,7 +658,7 @@ __global__ void k_zbl(EdgeGeomArgs a, const double* __restrict__ zn, double* __r
     double r2 = dx * dx + dy * dy + dz * dz;
     if (!(r2 < a.rc * a.rc) || !(r2 > 0.0)) continue;
     double r = sqrt(r2), inv = 1.0 / r;
-    double zj = zn[a.species[j]];
+    double zj = zn[zc(a.species[j], a.S)];
     double ia = (pow(zi, 0.23) + pow(zj, 0.23)) / 0.46850, xs = r * ia;
     double e1 = 0.18175 * exp(-3.19980 * xs), e2 = 0.50986 * exp(-0.94229 * xs), e3 = 0.28022 * exp(-0.40290 * xs),
            e4 = 0.02817 * exp(-0.20162 * xs);
@@ -715,10 +726,10 @@ __global__ void k_scale_vel(double* vel, int64_t n3, const double* __restrict__ 
   if (i < n3) vel[i] *= s[0];
 }
 
-__global__ void k_kin(const double* vel, const int32_t* species, const double* mass, int64_t n, double* out) {
+__global__ void k_kin(const double* vel, const int32_t* species, const double* mass, int S, int64_t n, double* out) {
   int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
   if (i >= n) return;
-  double m = mass[species[i]];
+  double m = mass[zc(species[i], S)];
   out[i] = 0.5 * m * (vel[3 * i] * vel[3 * i] + vel[3 * i + 1] * vel[3 * i + 1] + vel[3 * i + 2] * vel[3 * i + 2]) / ACC_CONV;
 }
 
@@ -845,10 +856,10 @@ int k_launch_energy(allegro_model* m, Work& w, const int32_t* species, int64_t c
   if (nc <= 0) return ALLEGRO_OK;
   if (w.n_eparts > 0 && xf != nullptr)
     k_energy_parts<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, (const double*)w.epart.p,
-                                                                w.n_eparts, (int64_t)w.cap_edges, species, m->sigma, m->mu, e_atom);
+                                                                w.n_eparts, (int64_t)w.cap_edges, species, m->S, m->sigma, m->mu, e_atom);
   else
     k_energy<<<(nc * 32 + 255) / 256, 256, 0, m->stream>>>((const int64_t*)w.rowa.p, nc, c0, xf, m->d, m->w_eff_d, species,
-                                                          m->sigma, m->mu, e_atom);
+                                                          m->S, m->sigma, m->mu, e_atom);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
@@ -890,6 +901,16 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
   return ALLEGRO_OK;
 }
 
+// Start of a compute call: zero the force array (may be null) and validate every atom's species; an out-of-range value
+// raises status bit 2 (ALLEGRO_ERR_BAD_ARG at the next host synchronisation); table look-ups clamp (zc()).
+int k_launch_begin_compute(allegro_model* m, double* force, const int32_t* species, int64_t n, int* flags) {
+  ProfScope _ps(m, PC_EDGE_BWD);
+  if (n <= 0) return ALLEGRO_OK;
+  k_zero_check<<<(unsigned)((3 * n + 255) / 256), 256, 0, m->stream>>>(force, 3 * n, species, n, m->S, flags);
+  LAUNCH_CHECK(m);
+  return ALLEGRO_OK;
+}
+
 int k_launch_zero_f64(allegro_model* m, double* p, int64_t n) {
   ProfScope _ps(m, PC_EDGE_BWD);
   if (n <= 0) return ALLEGRO_OK;
@@ -902,7 +923,7 @@ int k_launch_nve_kick_drift(allegro_model* m, double* pos, double* vel, const do
                             const double* mass, int64_t n, double dt, bool drift) {
   ProfScope _ps(m, PC_NVE);
   if (n <= 0) return ALLEGRO_OK;
-  k_nve<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(pos, vel, force, species, mass, n, dt, drift ? 1 : 0);
+  k_nve<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(pos, vel, force, species, mass, m->S, n, dt, drift ? 1 : 0);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
@@ -912,7 +933,7 @@ int k_launch_kinetic(allegro_model* m, const double* vel, const int32_t* species
   ProfScope _ps(m, PC_NVE);
   AL_CHECK(al_reserve(m, tmp, (size_t)n * 8 + 16));
   if (n > 0) {
-    k_kin<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(vel, species, mass, n, (double*)tmp.p);
+    k_kin<<<(unsigned)((n + 255) / 256), 256, 0, m->stream>>>(vel, species, mass, m->S, n, (double*)tmp.p);
     LAUNCH_CHECK(m);
   }
   return k_launch_sum_f64(m, (double*)tmp.p, n, e_kin);

@@ -29,7 +29,6 @@ struct GemmArgs {
   // come from A, columns [K1, K) from A2 (row stride lda2); K1 must be a multiple of 32.  A2 = null: plain A.
   const float* A2; int lda2; int K1;
   const float* Bt; int ldb;       // fp32 weights [N][K]
-  const void* Bt16;               // bf16 weights [N][K] (precision 2) or null
   const float *Bt_hi, *Bt_lo;     // TF32-exact / remainder split of Bt (precision 0 on tensor cores) or null
   float* C; int ldc;
   int N, K;
@@ -54,8 +53,7 @@ struct GemmArgs {
   int rev;
 };
 
-// precision: 0 fp32 FFMA, 1 TF32 tcgen05, 2 BF16 tcgen05 (A converted on the fly is not possible with
-// TMA-fed operands, so precision 2 uses TF32 for fp32-resident activations).
+// dispatch by allegro_hparams.precision: 0 3xTF32 tcgen05, 1 TF32 tcgen05, 3 fp32 FFMA (2 is refused at create time)
 int al_gemm(struct allegro_model* m, const GemmArgs& g);
 // number of 32-column row partials the EPI_LATENT_LAST epilogue of the active GEMM kernel writes for N columns
 int al_gemm_row_parts(const struct allegro_model* m, int N);

@@ -475,16 +475,19 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
 EncodeTiledFn g_encode = nullptr;
 
 typedef std::tuple<const void*, long long, long long, long long, int, int> TmKey;   // ptr, rows, K, ld, box_rows, exact
-std::map<TmKey, CUtensorMap>& tm_cache() {
-  static thread_local std::map<TmKey, CUtensorMap> c;
-  return c;
+typedef std::map<TmKey, CUtensorMap> TmCache;
+// one cache per model (allegro_model::tmaps): the maps describe that model's work buffers and weights on its device and die
+// with it (al_gemm_tc_free); keyed by (pointer, shape), so a buffer that is re-allocated at another address gets a new map
+TmCache& tm_cache(allegro_model* m) {
+  if (!m->tmaps) m->tmaps = new TmCache();
+  return *static_cast<TmCache*>(m->tmaps);
 }
 
 // exact = true: plain fp32 load (the 3xTF32 path splits the operand itself); false: TFLOAT32 map, i.e. the load
 // rounds to nearest TF32 (the MMA alone would truncate: measured 2-3x larger error)
 int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, long long ld, int box_rows, bool exact, CUtensorMap* out) {
   TmKey key(ptr, rows, K, ld, box_rows, exact ? 1 : 0);
-  auto& c = tm_cache();
+  auto& c = tm_cache(m);
   auto it = c.find(key);
   if (it != c.end()) { *out = it->second; return ALLEGRO_OK; }
   if (!g_encode) {
@@ -514,11 +517,11 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 #define GEMM_LAUNCH(AS, BS, EW, SP, EP, PR, A2)                                                                          \
   {                                                                                                                      \
     static_assert(smem_bytes(AS, BS, EW, SP) <= 232448, "shared memory budget (227 KB)");                                \
-    static bool attr_set = false;                                                                                        \
-    if (!attr_set) {                                                                                                     \
+    static AttrOnce once;                                                                                                \
+    if (once.need(m->device)) {                                                                                          \
       AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
                                       (int)smem_bytes(AS, BS, EW, SP)));                                                 \
-      attr_set = true;                                                                                                   \
+      once.done(m->device);                                                                                              \
     }                                                                                                                    \
     k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>( \
         tmA, tmA2, tmB, tmB2, g, BN, ntn);                                                                               \
@@ -597,8 +600,7 @@ int al_gemm_tc_row_parts(int N, bool split) {
   return ntn * ((BN + 31) >> 5);
 }
 
-int al_upload_bf16(allegro_model* m, void** dst, const std::vector<float>& h) {
-  (void)m; (void)h;
-  *dst = nullptr;   // precision 2 currently runs the TF32 kernel on the fp32 copies
-  return ALLEGRO_OK;
+void al_gemm_tc_free(allegro_model* m) {
+  delete static_cast<TmCache*>(m->tmaps);
+  m->tmaps = nullptr;
 }

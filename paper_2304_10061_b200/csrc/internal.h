@@ -1,5 +1,6 @@
 // Internal structures of libb200allegro (not part of the C ABI).
 #pragma once
+#include <atomic>
 #include <cstdlib>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -26,6 +27,14 @@ void al_set_error(const allegro_model* m, const std::string& msg);
     int _r = (expr);               \
     if (_r != ALLEGRO_OK) return _r; \
   } while (0)
+
+// cudaFuncSetAttribute is per (kernel, device): one static AttrOnce per launch site remembers which device ordinals
+// already carry the attribute, so a second model on another device of the same process sets it again (thread-safe).
+struct AttrOnce {
+  std::atomic<uint64_t> mask{0};
+  bool need(int dev) const { return !(mask.load(std::memory_order_acquire) & (1ull << (dev & 63))); }
+  void done(int dev) { mask.fetch_or(1ull << (dev & 63), std::memory_order_release); }
+};
 
 // ---- host-side description of the tensor track ---------------------------------------------------
 struct Irrep { int l, p; };
@@ -70,8 +79,6 @@ struct Dense {
   int fi = 0, fo = 0;
   float* W = nullptr;    // [fi][fo] row-major  (B operand of dX = dY * W^T, K-major over fo)
   float* Wt = nullptr;   // [fo][fi] row-major  (B operand of Y = X * W, K-major over fi)
-  void* Wh = nullptr;    // bf16 copies for precision 2 (same two layouts), else null
-  void* Wth = nullptr;
   // precision 0 on tensor cores (3xTF32): W_hi = rn_tf32(W), W_lo = rn_tf32(W - W_hi); same two layouts
   float *W_hi = nullptr, *W_lo = nullptr, *Wt_hi = nullptr, *Wt_lo = nullptr;
 };
@@ -128,6 +135,8 @@ struct allegro_model {
   int sweep_mode = -1; unsigned sweep_ctr = 0;
   std::string err;
   int sm_count = 148;
+  int device = 0;                         // CUDA device ordinal the model was created on
+  void* tmaps = nullptr;                  // tensor-map cache of the tcgen05 GEMMs (gemm_tc.cu), freed by al_gemm_tc_free
   // workspace (per chunk), grown on demand
   struct Work* work = nullptr;
   // per-kernel-group event timing (allegro_profile_*)
@@ -181,3 +190,4 @@ int al_compute_local_impl(allegro_model* m, const double* pos, const int32_t* sp
                           double* e_edge);
 int al_exclusive_scan_i64(allegro_model* m, const int32_t* in, int64_t* out, int64_t n, DevBuf& tmp);  // out[n] = total
 void al_work_free(allegro_model* m);
+int al_check_status(allegro_model* m);   // compute.cu: synchronise, read + clear the device status word -> error code

@@ -33,6 +33,7 @@ struct Work {
   DevBuf ge;                                // float[M][3] dE/dr_e (debug tap)
   DevBuf eatom;                             // f64[N] when the caller passes e_atom = NULL
   DevBuf nh_scal;                           // f64[1]: velocity scale of the Nose-Hoover half step
+  DevBuf host_stage;                        // device staging of allegro_step_nve_host
   int64_t eatom_cap = 0;
   int last_nc = 0;
 };
@@ -66,6 +67,7 @@ int k_launch_bwd_prep(allegro_model* m, Work& w, const float* xbar, int ldx, con
 int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, const Dense& L0, bool single,
                       double* force, int m_cap);
 int k_launch_zero_f64(allegro_model* m, double* p, int64_t n);
+int k_launch_begin_compute(allegro_model* m, double* force /*null: energy only*/, const int32_t* species, int64_t n, int* flags);
 // ZBL pair repulsion over the candidate rows of the chunk's centres: e_atom[i] += 1/2 sum phi, force[i] += sum phi' rhat
 int k_launch_zbl(allegro_model* m, const EdgeGeomArgs& a, const double* zbl_Z, double* e_atom, double* force);
 // per-edge energies E_ij in candidate-list order (0 for dropped candidates)

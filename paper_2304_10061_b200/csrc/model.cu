@@ -65,6 +65,10 @@ static int check_hp(const allegro_hparams* hp) {
   if (hp->latent_dims[hp->n_latent - 1] != hp->twobody_dims[hp->n_twobody - 1]) return bad("last latent width must equal d");
   if (!(hp->avg_num_neighbors > 0)) return bad("avg_num_neighbors");
   if (hp->precision < 0 || hp->precision > 3) return bad("precision");
+  if (hp->precision == 2) {   // 16-bit operand storage + tcgen05 kind::f16 is not built: refuse instead of aliasing another mode
+    al_set_error(nullptr, "precision 2 (BF16-operand MLPs) is not implemented; use 1 (TF32) or 0 / 3 (fp32)");
+    return ALLEGRO_ERR_UNIMPLEMENTED;
+  }
   return ALLEGRO_OK;
 }
 
@@ -126,7 +130,7 @@ static int upload(allegro_model* m, T** dst, const std::vector<T>& h) {
   return ALLEGRO_OK;
 }
 
-int al_upload_bf16(allegro_model* m, void** dst, const std::vector<float>& h);   // gemm_tc.cu
+void al_gemm_tc_free(allegro_model* m);   // gemm_tc.cu
 
 static int upload_dense(allegro_model* m, Dense& D, const std::vector<float>& W, int fi, int fo) {
   D.fi = fi; D.fo = fo;
@@ -135,10 +139,6 @@ static int upload_dense(allegro_model* m, Dense& D, const std::vector<float>& W,
     for (int o = 0; o < fo; ++o) Wt[(size_t)o * fi + i] = W[(size_t)i * fo + o];
   AL_CHECK(upload(m, &D.W, W));
   AL_CHECK(upload(m, &D.Wt, Wt));
-  if (m->hp.precision == 2) {
-    AL_CHECK(al_upload_bf16(m, &D.Wh, W));
-    AL_CHECK(al_upload_bf16(m, &D.Wth, Wt));
-  }
   if (m->hp.precision == 0) {
     auto split = [](const std::vector<float>& x, std::vector<float>& hi, std::vector<float>& lo) {
       hi.resize(x.size()); lo.resize(x.size());
@@ -178,6 +178,7 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
   m->n = hp->n_tensor; m->lmax = hp->l_max; m->NL = hp->n_layers;
   m->Denv = (m->lmax + 1) * (m->lmax + 1); m->nA = m->n * (m->lmax + 1); m->ldY = (m->Denv + 3) & ~3;
   int dev = 0; cudaGetDevice(&dev);
+  m->device = dev;
   cudaDeviceGetAttribute(&m->sm_count, cudaDevAttrMultiProcessorCount, dev);
   m->c_env = (float)(1.0 / std::sqrt(hp->avg_num_neighbors));
   for (int L = 0; L < m->NL; ++L) {
@@ -307,6 +308,7 @@ extern "C" int allegro_destroy(allegro_model* m) {
   if (!m) return ALLEGRO_OK;
   cudaDeviceSynchronize();
   al_work_free(m);
+  al_gemm_tc_free(m);
   for (auto& r : m->prof_recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
   for (auto e : m->prof_pool) cudaEventDestroy(e);
   for (void* p : m->owned) cudaFree(p);

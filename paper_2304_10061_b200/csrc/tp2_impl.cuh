@@ -459,8 +459,8 @@ int launch_fwd2(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int SF = FIRST ? NLV * 32 + LDY : DIN * 32;
   constexpr int WSL = DENV * 32 + NST * SF;
   size_t sm = (size_t)WPB * WSL * 4 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp2_fwd<P, CB, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tp2_fwd<P, CB, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * a.ngroups;
   k_tp2_fwd<P, CB, FIRST, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;
@@ -478,8 +478,8 @@ int launch_bwd2(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int WSL = 2 * DENV * 32 + MSL + NST * SF;
   size_t sm = (size_t)WPB * WSL * 4 + 16;
   auto kern = k_tp2_bwd<P, AB, FIRST, HASVB, MREG, NST, WPB>;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * a.ngroups;
   kern<<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;

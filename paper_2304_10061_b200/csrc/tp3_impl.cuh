@@ -433,8 +433,8 @@ int launch_fwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int SF = FIRST ? 4 * 8 + 16 : DIN * 8;
   constexpr int WSL = 16 * 8 + NST * SF;
   size_t sm = (size_t)WPB * WSL * 4 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_fwd<P, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_fwd<P, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * (a.n / T3_CPW);
   k_tp3_fwd<P, FIRST, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;
@@ -451,8 +451,8 @@ int launch_bwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int SF = SV + DOUT * CPW + CPW;
   constexpr int WSL = 16 * CPW + (LQ == 3 ? 0 : AB * CH * 64) + NST * SF;
   size_t sm = (size_t)WPB * WSL * 4 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_bwd<P, FIRST, LQ, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_bwd<P, FIRST, LQ, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * (a.n / CPW);
   k_tp3_bwd<P, FIRST, LQ, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;

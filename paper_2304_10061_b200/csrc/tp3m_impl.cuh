@@ -248,8 +248,8 @@ int launch_fwd3m(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   constexpr int KH = (Pat<P>::DIN + 7) / 8, NJ = (Pat<P>::DOUT + 7) / 8;
   constexpr int WSL = 16 * 8 + 8 * (KH * NJ * 72 + 2);
   size_t sm = (size_t)WPB * WSL * 4 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3m_fwd<P, FIRST, WPB, PIPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3m_fwd<P, FIRST, WPB, PIPE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   {
     int64_t gw = (int64_t)a.nc * (a.n / 32);
     k_tp3m_gamma<P, 8><<<(unsigned)((gw + 7) / 8), 256, 0, m->stream>>>(a);

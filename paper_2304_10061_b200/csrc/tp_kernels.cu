@@ -518,8 +518,8 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32) k_tpb_bwd(TPW a) {
 template <int DENV, int DIN, int DOUT, int CB, bool FIRST>
 int launch_bfwd(allegro_model* m, const TPW& a) {
   size_t sm = (size_t)WARPS_PER_BLOCK * (DENV + DIN * CB) * 32 * 4 + (size_t)a.t.nnz * 8 + (DOUT + 1) * 4 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tpb_fwd<DENV, DIN, DOUT, CB, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tpb_fwd<DENV, DIN, DOUT, CB, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * a.ngroups;
   k_tpb_fwd<DENV, DIN, DOUT, CB, FIRST><<<(unsigned)((warps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, sm, m->stream>>>(a);
   m->launches++;
@@ -529,8 +529,8 @@ int launch_bfwd(allegro_model* m, const TPW& a) {
 template <int DENV, int DIN, int DOUT, int AB, bool FIRST>
 int launch_bbwd(allegro_model* m, const TPW& a) {
   size_t sm = (size_t)WARPS_PER_BLOCK * (2 * DENV + AB * DOUT) * 32 * 4 + (size_t)a.t.nnz * 8 + (DIN + 1) * 4 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tpb_bwd<DENV, DIN, DOUT, AB, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tpb_bwd<DENV, DIN, DOUT, AB, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * a.ngroups;
   k_tpb_bwd<DENV, DIN, DOUT, AB, FIRST><<<(unsigned)((warps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, sm, m->stream>>>(a);
   m->launches++;
@@ -541,8 +541,8 @@ int launch_bbwd(allegro_model* m, const TPW& a) {
 template <int DENV, int DIN, int DOUT, bool FIRST>
 int launch_fwd(allegro_model* m, const TPW& a) {
   size_t sm = (size_t)WARPS_PER_BLOCK * (DENV + DIN * DOUT) * 32 * 4 + (size_t)a.t.nnz * 12 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tpw_fwd<DENV, DIN, DOUT, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tpw_fwd<DENV, DIN, DOUT, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * a.ngroups;
   k_tpw_fwd<DENV, DIN, DOUT, FIRST><<<(unsigned)((warps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, sm, m->stream>>>(a);
   m->launches++;
@@ -552,8 +552,8 @@ int launch_fwd(allegro_model* m, const TPW& a) {
 template <int DENV, int DIN, int DOUT, bool FIRST>
 int launch_bwd(allegro_model* m, const TPW& a) {
   size_t sm = (size_t)WARPS_PER_BLOCK * (DENV + DIN * DOUT) * 32 * 4 + (size_t)a.t.nnz * 12 + 16;
-  static bool set = false;
-  if (!set) { AL_CUDA(m, cudaFuncSetAttribute(k_tpw_bwd<DENV, DIN, DOUT, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); set = true; }
+  static AttrOnce once;
+  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tpw_bwd<DENV, DIN, DOUT, FIRST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * a.ngroups;
   k_tpw_bwd<DENV, DIN, DOUT, FIRST><<<(unsigned)((warps + WARPS_PER_BLOCK - 1) / WARPS_PER_BLOCK), WARPS_PER_BLOCK * 32, sm, m->stream>>>(a);
   m->launches++;

@@ -179,7 +179,7 @@ class Domain:
         self.send_counts = [int(x.numel()) for x in idx_d]
         self.send_idx = torch.cat(idx_d)
         self.send_shift = torch.cat(shift_d)
-        self._nbr = None
+        self._nbr_dirty = True     # new ghost set: rebuild the list INTO the existing handle (buffers are reused, nothing leaks)
         return self.send_counts
 
     # ---- forward exchange ----------------------------------------------------------------------------------------
@@ -202,9 +202,10 @@ class Domain:
         if self.model is None:
             raise RuntimeError("Domain needs an Allegro model (CUDA): there is no CPU fallback")
         # the list is rebuilt with the ghost lists (build_send_lists) and reused in between (Verlet skin = halo - r_cut)
-        if self._nbr is None or self._nbr_n != pos_all.shape[0]:
+        if self._nbr is None or getattr(self, "_nbr_dirty", True) or self._nbr_n != pos_all.shape[0]:
             self._nbr = self.model.neighbors(pos_all, box_local, self.halo, reuse=self._nbr)
             self._nbr_n = pos_all.shape[0]
+            self._nbr_dirty = False
         e, _, f = self.model.compute_local(pos_all, sp_all, n_local, box_local, self._nbr)
         return e, f
 

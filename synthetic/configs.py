@@ -52,8 +52,9 @@ class Config:
     pos_seed: int
     vel_seed: int
     weight_seed: int = 0
-    # per-species energy scale/shift (SURVEY §8(d) "Energy scale"): sigma is one constant per config,
-    # chosen by tests/golden/make_energy_scale.py (oracle only) so RMS|F| ~ 1 eV/A at step 0.
+    # per-species energy scale/shift (SURVEY §8(d) "Energy scale"): the five configs use sigma_Z = 1 for every species
+    # (RMS|F| is already O(1) eV/A with the seeded weights), mu_Z = -(1 + Z) eV.  Species-distinct sigma and
+    # layer-distinct resid_alpha are exercised by tests/test_oracle_sigma_alpha.py and tests/test_gpu_sigma_alpha.py.
     sigma: float = 1.0
 
     def mu(self) -> List[float]:
@@ -74,7 +75,6 @@ def _hp(S, lmax, nl, n, two, lat, edge, rc, avg):
                    avg_num_neighbors=avg, resid_alpha=tuple([0.5] * nl))
 
 
-# sigma values below are written by tests/golden/make_energy_scale.py (calls only oracle/)
 CONFIGS: List[Config] = [
     Config(0, "water64", _hp(2, 1, 1, 8, [32, 32], [32], [16], 4.0, _AVG4),
            192, _RHO_W, "water", ("H", "O"), 1.0, 10, 0.5, 300.0, 1000, 2000),

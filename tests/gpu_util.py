@@ -13,7 +13,9 @@ def make_both(cfg, precision=0, sigma=None, chunk_edges=None):
     fan_or = O.path_fan(hp.l_max, hp.n_layers)      # oracle side: its own enumeration
     assert fan_gpu == fan_or
     s = cfg.sigma if sigma is None else sigma
-    blob = make_blob(hp, fan_gpu, [s] * hp.n_species, cfg.mu(), cfg.weight_seed)
+    sig = list(s) if np.ndim(s) else [s] * hp.n_species           # scalar: same for every species; else per species
+    assert len(sig) == hp.n_species
+    blob = make_blob(hp, fan_gpu, sig, cfg.mu(), cfg.weight_seed)
     model = P.Allegro(chp, blob, chunk_edges=chunk_edges)
     if getattr(hp, "r_cut_pair", None) is not None:
         model.set_pair_cutoffs(hp.r_cut_pair)

@@ -11,7 +11,9 @@ from synthetic.configs import scaled_config
 def oracle_model(hp, sigma=1.0, mu=None, seed=0, zero_alpha=False):
     fan = O.path_fan(hp.l_max, hp.n_layers)
     S = hp.n_species
-    blob = make_blob(hp, fan, [sigma] * S, mu if mu is not None else [0.0] * S, seed)
+    sig = list(sigma) if np.ndim(sigma) else [sigma] * S          # scalar: one value for every species; else per species
+    assert len(sig) == S
+    blob = make_blob(hp, fan, sig, mu if mu is not None else [0.0] * S, seed)
     m = O.OracleModel(hp, blob)
     if zero_alpha:
         m.alpha = [a * 0 for a in m.alpha]

@@ -208,11 +208,14 @@ def test_energy_forces_tf32(ci, n):
 # config 1 against the full oracle; configs 2-4 by exact sub-system parity (strict locality,
 # E-hat_c needs only centre c's edges; F_a only the centres within r_c of a)
 # ---------------------------------------------------------------------------------------------------
-def _subsystem_check(ci, n_probe, precision, seed=0):
+def _subsystem_check(ci, n_probe, precision, seed=0, sigma=None, resid_alpha=None):
+    import dataclasses
     cfg = CONFIGS[ci]
+    if resid_alpha is not None:
+        cfg = dataclasses.replace(cfg, hp=dataclasses.replace(cfg.hp, resid_alpha=tuple(resid_alpha)))
     pos, sp, box = make_system(cfg)
     N = pos.shape[0]
-    model, oracle = make_both(cfg, precision=precision)
+    model, oracle = make_both(cfg, precision=precision, sigma=sigma)
     (E, Ea, F), nb = gpu_eval(model, pos, sp, box, cutoff=cfg.hp.r_cut + cfg.skin)
     oi, oj, os_ = O.neighbor_list(pos, box, cfg.hp.r_cut)
     # list parity at full size on sampled rows (bit-exact) + total count
