@@ -183,7 +183,7 @@ def test_decomposed_md_over_nccl_world1_matches_the_plain_step():
     import json
     import subprocess
     outs = []
-    for extra in (["--decompose"], ["--no-cpu-baseline"]):
+    for extra in (["--decompose"], ["--no-cpu-baseline", "--repeats", "1", "--no-peak-probe"]):   # both: 3 + 5 steps
         r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--config", "0", "--steps", "5", "--warmup", "3"] + extra,
                            capture_output=True, text=True, timeout=600)
         assert r.returncode == 0, r.stderr[-3000:]
