@@ -177,13 +177,11 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   // With fused_last every z-bar that starts an MLP's backward comes out of a GEMM epilogue (EPI_LATENT_LAST for
   // layer NL, the prep stage of EPI_ADD2/ADD2R for the others); otherwise k_bwd_prep computes it.
   bool zb_ready = fused_last;
-  static const bool no_prep = getenv("B200_ALLEGRO_NO_PREP") != nullptr;   // experiment switch: keep k_bwd_prep for L < NL
-  const bool fuse_prep = fused_last && !no_prep;
+  const bool fuse_prep = fused_last;
   int prep_slot = 1;
   // K-concatenated x-bar GEMM (tensor-core kernels): x-bar^{L-1} = [z-bar | omega-bar] [W_x | A]^T in one launch, so
   // the x-bar part of dX of the first latent layer never goes through HBM; s-bar comes from its own N = n GEMM.
-  static const bool no_kcat = getenv("B200_ALLEGRO_NO_KCAT") != nullptr;
-  const bool kcat = !no_kcat && al_gemm_supports_kcat(m) && (hp.latent_dims[0] % 32 == 0);
+  const bool kcat = al_gemm_supports_kcat(m) && (hp.latent_dims[0] % 32 == 0);
   float* zstart = (float*)w.ZB0.p;   // where the z-bar entering the next MLP to differentiate lives
   for (int L = NL; L >= 1; --L) {
     float* zb = zstart; float* zb_o = (zstart == (float*)w.ZB0.p) ? (float*)w.ZB1.p : (float*)w.ZB0.p;

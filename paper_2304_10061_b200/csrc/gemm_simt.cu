@@ -181,12 +181,8 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
 int al_gemm_tc3(allegro_model* m, const GemmArgs& g);  // gemm_tc.cu (tcgen05, 3xTF32 split operands)
 int al_gemm_tc_row_parts(int N, bool split);
 
-// precision 0 runs on the tensor cores as 3xTF32; precision 3 (or B200_ALLEGRO_FP32_SIMT with precision 0) runs
-// the plain FFMA kernel below
-static bool fp32_simt(const allegro_model* m) {
-  static const bool v = getenv("B200_ALLEGRO_FP32_SIMT") != nullptr;
-  return m->hp.precision == 3 || (m->hp.precision == 0 && v);
-}
+// precision 0 runs on the tensor cores as 3xTF32; precision 3 runs the plain FFMA kernel below
+static bool fp32_simt(const allegro_model* m) { return m->hp.precision == 3; }
 
 int al_gemm_row_parts(const allegro_model* m, int N) {
   if (fp32_simt(m)) return (N + 31) / 32;

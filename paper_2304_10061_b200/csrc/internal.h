@@ -131,8 +131,8 @@ struct allegro_model {
   int64_t launches = 0;
   // Alternating sweep direction of the edge-ordered kernels (GEMM row tiles, tensor-track centres): every such launch
   // walks the edge range opposite to the one before it, so it starts on the rows its producer wrote last (still in the
-  // 126 MB L2) instead of on rows evicted long ago.  Results do not depend on the order.  B200_ALLEGRO_SWEEP=0: off.
-  int sweep_mode = -1; unsigned sweep_ctr = 0;
+  // 126 MB L2) instead of on rows evicted long ago.  Results do not depend on the order.
+  unsigned sweep_ctr = 0;
   std::string err;
   int sm_count = 148;
   int device = 0;                         // CUDA device ordinal the model was created on
@@ -156,10 +156,7 @@ struct allegro_model {
 };
 
 // direction of the next edge-ordered launch (0 forward, 1 reversed), see allegro_model::sweep_mode
-inline int al_next_rev(allegro_model* m) {
-  if (m->sweep_mode < 0) { const char* e = getenv("B200_ALLEGRO_SWEEP"); m->sweep_mode = e ? atoi(e) : 1; }
-  return m->sweep_mode ? (int)(m->sweep_ctr++ & 1u) : 0;
-}
+inline int al_next_rev(allegro_model* m) { return (int)(m->sweep_ctr++ & 1u); }
 
 // ---- profiling ------------------------------------------------------------------------------------
 enum ProfCat { PC_GEMM = 0, PC_TP_FWD, PC_TP_BWD, PC_GEOM, PC_TWOBODY0, PC_ENERGY, PC_BWD_ELEM, PC_EDGE_BWD, PC_NEIGHBORS,

@@ -47,8 +47,7 @@ int match_pattern(const TPLayerHost& h) {
 // layer's sparsity pattern is one of the generated ones with the expected role (first / middle / last
 // layer); otherwise tp_kernels.cu / the generic kernels run.
 bool tp2_eligible(const allegro_model* m) {
-  static const bool off = getenv("B200_ALLEGRO_TP_OLD") != nullptr;
-  if (off || m->n % 32 != 0 || (int)m->v0_l.size() != m->Denv) return false;
+  if (m->n % 32 != 0 || (int)m->v0_l.size() != m->Denv) return false;
   for (int k = 0; k < m->Denv; ++k)
     if (m->v0_y[k] != k || m->v0_l[k] != l_of(k)) return false;
   for (int L = 1; L <= m->NL; ++L) {
@@ -68,12 +67,11 @@ bool tp2_eligible(const allegro_model* m) {
   return true;
 }
 
-// channel groups of the kernel that runs layer L's backward: 8-channel warps for the lane-split l_max = 3 kernels
-// (tp3_impl.cuh), 32-channel warps otherwise
+// channel groups of the kernel that runs layer L's backward: 8-channel teams for the mma.sync l_max = 3 kernels
+// (tp3mb_impl.cuh, TF32 mode), 32-channel warps otherwise
 static int bwd_groups(const allegro_model* m, int L) {
   int p = match_pattern(m->tp_host[L - 1]);
-  const int lq = t3_bwd_lq();
-  return ((p == P_16_16_31 || p == P_16_31_16) && lq) ? m->n / (32 >> lq) : m->n / 32;
+  return ((p == P_16_16_31 || p == P_16_31_16) && tp3m_bwd_active(m)) ? m->n / 8 : m->n / 32;
 }
 
 int al_ybar_layout(const allegro_model* m, int* part0) {
@@ -116,16 +114,9 @@ int tp2_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
   const bool first = (Vin == nullptr), hasvb = (VbarL != nullptr);
   if (hasvb != (L < m->NL)) { al_set_error(m, "tp2_bwd: unexpected V-bar input"); return ALLEGRO_ERR_BAD_ARG; }
   if (p == P_16_16_31 || p == P_16_31_16 || p == P_16_16_1) return tp2_l3_bwd(m, q, p);
-  static const bool mreg = getenv("B200_ALLEGRO_TP_MREG") != nullptr;   // default: M block in shared memory (168 vs 251 registers; measured faster)
-  if (p == P_9_9_9) {
-    FILL(P_9_9_9)
-    if (mreg) return first ? launch_bwd2<P_9_9_9, 9, true, true, true, 4, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, true, 4, 4>(m, a);
-    static const int bv = getenv("B200_ALLEGRO_TP_BWDV") ? atoi(getenv("B200_ALLEGRO_TP_BWDV")) : 1;   // 1 (2 ring stages, 12 warps/SM) measured best
-    if (bv == 1) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 2, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 2, 4>(m, a);
-    if (bv == 2) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 3, 2>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 3, 2>(m, a);
-    if (bv == 3) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 2, 2>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 2, 2>(m, a);
-    return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 4, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 4, 4>(m, a);
-  }
+  // 9 x 9 x 9: M block in the warp's shared slice, 2 ring stages, 12 warps per SM (round-1 measurements: M in registers at
+  // 251 registers and deeper rings / smaller blocks were all slower)
+  if (p == P_9_9_9) { FILL(P_9_9_9) return first ? launch_bwd2<P_9_9_9, 9, true, true, false, 2, 4>(m, a) : launch_bwd2<P_9_9_9, 9, false, true, false, 2, 4>(m, a); }
   if (p == P_9_9_1) { FILL(P_9_9_1) return first ? launch_bwd2<P_9_9_1, 9, true, false, true, 4, 4>(m, a) : launch_bwd2<P_9_9_1, 9, false, false, true, 4, 4>(m, a); }
   if (p == P_4_4_4) { FILL(P_4_4_4) return first ? launch_bwd2<P_4_4_4, 4, true, true, true, 4, 4>(m, a) : launch_bwd2<P_4_4_4, 4, false, true, true, 4, 4>(m, a); }
   if (p == P_4_4_1) { FILL(P_4_4_1) return first ? launch_bwd2<P_4_4_1, 4, true, false, true, 4, 4>(m, a) : launch_bwd2<P_4_4_1, 4, false, false, true, 4, 4>(m, a); }

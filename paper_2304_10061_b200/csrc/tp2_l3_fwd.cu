@@ -4,8 +4,7 @@
 
 int tp2_l3_fwd(allegro_model* m, const TP2Common& q, int pat) {
   // TF32 mode (precision 1; the paper runs the tensor product in TF32): mma.sync kernels of tp3m_impl.cuh
-  static const bool no_mma = getenv("B200_ALLEGRO_TP3_NO_MMA") != nullptr;
-  if (m->hp.precision == 1 && !no_mma && m->d % 8 == 0) {   // (32-byte rows of the scalar output need d % 8 == 0)
+  if (m->hp.precision == 1 && m->d % 8 == 0) {   // (32-byte rows of the scalar output need d % 8 == 0)
     // software-pipelined chunks, 2 warps per block (8 warps per SM at 238 / 255 registers); without the pipeline
     // (166 registers, 10 warps per SM) 3 % slower, 3 warps per block 25 % slower
     if (pat == P_16_16_31) { TP2<Pat<P_16_16_31>::NNZ> a{}; AL_CHECK(fill2(m, q, a)); return launch_fwd3m<P_16_16_31, true, 2, true>(m, a); }

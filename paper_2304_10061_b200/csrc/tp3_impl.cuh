@@ -15,14 +15,9 @@
 #include "tp2_impl.cuh"
 
 constexpr int T3_CPW = 8;      // channels per warp of the forward kernels (4 blocks)
-// Backward: the lane-split kernel below exists for 2^LQ = 4 and 8 blocks per warp, but neither beat the blocked
-// 32-channel kernel of tp2_impl.cuh on config 4 (84 ms per step): LQ = 2 keeps the M block in shared memory and
-// is LDS-bound (88 ms, ncu l1tex 70 %), LQ = 3 holds M and M-bar in registers but moves 16-byte rows (124 ms).
-// B200_ALLEGRO_TP3_BWD = 2 | 3 selects them for experiments; the default (0) is the tp2 kernel.
-inline int t3_bwd_lq() {
-  static const int v = getenv("B200_ALLEGRO_TP3_BWD") ? atoi(getenv("B200_ALLEGRO_TP3_BWD")) : 0;
-  return (v == 2 || v == 3) ? v : 0;
-}
+// The l_max = 3 backward in TF32 mode runs on the tensor cores (tp3mb_impl.cuh: 8-channel teams, so the Y-bar partial
+// buffers of those layers are per 8-channel group); the fp32 modes keep the blocked 32-channel kernel of tp2_impl.cuh.
+inline bool tp3m_bwd_active(const allegro_model* m) { return m->hp.precision == 1; }
 
 // ROWS rows of 8 floats (32 B): smem dst row r at dst + 8 r, global row r at src + r * rstride
 template <int ROWS>
@@ -158,9 +153,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tp3_fwd(const __grid_consta
 }
 
 // ======================================================================================================
-// backward:  NBK = 2^LQ blocks per warp, CPW = 32 / NBK channels; lane (ch, q) owns input components
-// [q AB, (q+1) AB): V-bar rows, M / M-bar blocks (both in registers for LQ = 3, M in shared memory for LQ = 2)
-// and environment components [q GB, (q+1) GB) in the Gamma pass and in pass 2.
+// helpers of the lane-split backward passes (lane = (channel ch, component group q)); used by tp3mb_impl.cuh
 // ======================================================================================================
 template <int CPW>
 __device__ __forceinline__ float t3_sum_ch(float v) {   // sum over the CPW channel lanes of a block
@@ -193,239 +186,6 @@ __device__ __forceinline__ void t3_cp_rows_w(float* dst, const float* src, int r
   }
 }
 
-template <int P, bool FIRST, int LQ, int NST, int WPB>
-static __global__ void __launch_bounds__(WPB * 32) k_tp3_bwd(const __grid_constant__ TP2<Pat<P>::NNZ> a) {
-  constexpr int DENV = Pat<P>::DENV, DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
-  static_assert(DENV == 16, "lane-split kernels are written for l_max = 3");
-  static_assert(!FIRST || DIN == 16, "FIRST: V^0 has the environment layout");
-  constexpr int NBK = 1 << LQ, CPW = 32 / NBK, GB = DENV / NBK;
-  constexpr bool MREG = (LQ == 3);
-  constexpr int AB = (DIN + NBK - 1) / NBK, CH = (DOUT + 1) / 2;
-  static_assert(!FIRST || AB == GB, "FIRST: input blocks coincide with the environment component groups");
-  constexpr int SV = FIRST ? 4 * CPW + 16 : DIN * CPW;       // operand part of a stage
-  constexpr int SF = SV + DOUT * CPW + CPW;                   // + V-bar^L rows + s-bar row
-  constexpr int MSL = MREG ? 0 : AB * CH * 64;                // M block, float2 per lane
-  constexpr int WSL = DENV * CPW + MSL + NST * SF;
-  extern __shared__ float4 smem4[];
-  float* smem = reinterpret_cast<float*>(smem4);
-  const int wib = threadIdx.x >> 5, lane = threadIdx.x & 31, ch = lane & (CPW - 1), q = lane / CPW;
-  const int ngroups = a.n / CPW;
-  int64_t wg = (int64_t)blockIdx.x * WPB + wib;
-  if (wg >= (int64_t)a.nc * ngroups) return;
-  if (a.rev) wg = (int64_t)a.nc * ngroups - 1 - wg;
-  const int c = (int)(wg / ngroups), grp = (int)(wg - (int64_t)c * ngroups);
-  const int nn = grp * CPW + ch;
-  float* Gs = smem + wib * WSL;
-  float2* Ms = reinterpret_cast<float2*>(Gs + DENV * CPW);
-  float* ring = Gs + DENV * CPW + MSL;
-  const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
-  const int deg = (int)(e1 - e0);
-  if (deg <= 0) return;
-  float* Yb0 = a.Ybar + (size_t)(a.ybar_part0 + grp) * a.ybar_pstride;
-  float* YbL = a.Ybar + (size_t)(a.ybar_partL + grp) * a.ybar_pstride;
-  const int lA = l_of(GB * q), lB = l_of(GB * q + 1);
-
-  const float* opc = FIRST ? a.w0 + e0 * a.ldw + grp * CPW : a.Vin + e0 * DIN * a.n + grp * CPW;
-  const int op_stride = FIRST ? a.ldw : DIN * a.n;
-  const float* Yc = a.Y + e0 * a.ldy + lane * 4;
-  const float* vbc = a.VbarL + e0 * DOUT * a.n + grp * CPW;
-  const float* sbc = a.sbar + e0 * a.lds + grp * CPW + lane * 4;
-  auto issue = [&](int il, float* st) {
-    if (FIRST) {
-      t3_cp_rows_w<4, CPW>(st, opc + il * op_stride, a.n, lane);
-      if (lane < 4) tp_cp16(st + 4 * CPW + lane * 4, Yc + il * a.ldy);
-    } else {
-      t3_cp_rows_w<DIN, CPW>(st, opc + il * op_stride, a.n, lane);
-    }
-    t3_cp_rows_w<DOUT, CPW>(st + SV, vbc + il * (DOUT * a.n), a.n, lane);
-    if (lane < CPW / 4) tp_cp16(st + SF - CPW + lane * 4, sbc + il * a.lds);
-  };
-#pragma unroll
-  for (int s = 0; s < NST - 1; ++s) {
-    if (s < deg) issue(s, ring + s * SF);
-    tp_cp_commit();
-  }
-  // Gamma_i: lane (ch, q) sums its GB environment components -> Gs[b * CPW + ch]
-  {
-    float g[GB];
-#pragma unroll
-    for (int j = 0; j < GB; ++j) g[j] = 0.f;
-    for (int64_t e = e0; e < e1; e += 4) {
-      float oa[4], ob[4], y[4][GB];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
-        oa[i] = a.om[ee * a.ldo + lA * a.n + nn];
-        ob[i] = a.om[ee * a.ldo + lB * a.n + nn];
-#pragma unroll
-        for (int j = 0; j < GB; ++j) y[i][j] = __ldg(a.Y + ee * a.ldy + GB * q + j);
-      }
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-        if (e + i < e1) {
-          g[0] = fmaf(oa[i], y[i][0], g[0]);
-#pragma unroll
-          for (int j = 1; j < GB; ++j) g[j] = fmaf(ob[i], y[i][j], g[j]);
-        }
-    }
-#pragma unroll
-    for (int j = 0; j < GB; ++j) Gs[(GB * q + j) * CPW + ch] = a.c_env * g[j];
-    __syncwarp();
-  }
-
-  // M block of this lane (rows q AB + r): entries of block blk are FFMAs predicated on q == blk
-  float2 Mr[MREG ? AB * CH : 1];
-  {
-    float G[DENV];
-#pragma unroll
-    for (int b = 0; b < DENV; ++b) G[b] = Gs[b * CPW + ch];
-    if constexpr (MREG) {
-#pragma unroll
-      for (int k = 0; k < AB * CH; ++k) Mr[k] = make_float2(0.f, 0.f);
-#define X(k, a_, b_, c_) \
-  if (q == (a_) / AB) TP2_REF(Mr, CH, (a_) % AB, c_) = fmaf(a.kv[k], G[b_], TP2_REF(Mr, CH, (a_) % AB, c_));
-      TP2_EXPAND(P, X)
-#undef X
-    } else {
-#pragma unroll
-      for (int r = 0; r < AB; ++r) {
-        float2 row[CH];
-#pragma unroll
-        for (int j = 0; j < CH; ++j) row[j] = make_float2(0.f, 0.f);
-#define X(k, a_, b_, c_) \
-  if ((a_) % AB == r) { if (q == (a_) / AB) TP2_REF(row, CH, 0, c_) = fmaf(a.kv[k], G[b_], TP2_REF(row, CH, 0, c_)); }
-        TP2_EXPAND(P, X)
-#undef X
-#pragma unroll
-        for (int j = 0; j < CH; ++j) Ms[(r * CH + j) * 32 + lane] = row[j];
-      }
-    }
-  }
-  float2 Mb[AB * CH];
-#pragma unroll
-  for (int k = 0; k < AB * CH; ++k) Mb[k] = make_float2(0.f, 0.f);
-  const int ab = q * AB;
-  // FIRST: shared-memory offsets of w0[l(ab + k)] for this lane's components
-  int wrow[AB];
-#pragma unroll
-  for (int k = 0; k < AB; ++k) wrow[k] = l_of((ab + k < DIN) ? ab + k : DIN - 1) * CPW + ch;
-  float* yb0p = Yb0 + e0 * DENV + GB * q;
-  float* outp = FIRST ? a.w0bar + e0 * a.ldob + q * a.n + nn : a.Vbar_prev + (e0 * DIN + ab) * a.n + nn;
-  int slot = 0;
-  for (int i = 0; i < deg; ++i) {
-    tp_cp_wait<NST - 2>();
-    __syncwarp();
-    {
-      const int nx = i + NST - 1;
-      int ns = slot + NST - 1; if (ns >= NST) ns -= NST;
-      if (nx < deg) issue(nx, ring + ns * SF);
-      tp_cp_commit();
-    }
-    const float* st = ring + slot * SF;
-    float2 t2[CH];
-#pragma unroll
-    for (int j = 0; j < CH; ++j) {
-      t2[j].x = st[SV + (2 * j) * CPW + ch];
-      t2[j].y = (2 * j + 1 < DOUT) ? st[SV + (2 * j + 1) * CPW + ch] : 0.f;
-    }
-    t2[0].x += st[SF - CPW + ch];
-    float vb[AB], y[AB], wl[AB];
-#pragma unroll
-    for (int k = 0; k < AB; ++k) {
-      const bool valid = ab + k < DIN;
-      float v;
-      if (FIRST) {
-        y[k] = st[4 * CPW + ab + k];
-        wl[k] = st[wrow[k]];
-        v = wl[k] * y[k];
-      } else {
-        v = valid ? st[(ab + k) * CPW + ch] : 0.f;
-      }
-      const float2 v2 = make_float2(v, v);
-      float2 s2 = make_float2(0.f, 0.f);
-#pragma unroll
-      for (int j = 0; j < CH; ++j) {
-        float2 m2;
-        if constexpr (MREG) m2 = Mr[k * CH + j]; else m2 = Ms[(k * CH + j) * 32 + lane];
-        s2 = tp_fma2(m2, t2[j], s2);
-        Mb[k * CH + j] = tp_fma2(v2, t2[j], Mb[k * CH + j]);
-      }
-      vb[k] = s2.x + s2.y;
-    }
-    if (FIRST) {
-      // w0-bar[l] = sum_{a in l} V-bar^0[a] Y[a];  Y-bar[a] (V^0 part) = sum_n w0[l(a)] V-bar^0[a]   (AB == GB)
-      float xa = vb[0] * y[0], xb = 0.f;
-#pragma unroll
-      for (int k = 1; k < AB; ++k) xb = fmaf(vb[k], y[k], xb);
-      const float wsum = t3_gather_l<CPW>(xa, xb, lA, lB, q);
-      if (q < 4) *outp = wsum;
-      outp += a.ldob;
-      float pj[AB];
-#pragma unroll
-      for (int k = 0; k < AB; ++k) pj[k] = t3_sum_ch<CPW>(wl[k] * vb[k]);
-      if (ch == 0)
-#pragma unroll
-        for (int k = 0; k < AB; ++k) yb0p[k] = pj[k];
-      yb0p += DENV;
-    } else {
-#pragma unroll
-      for (int k = 0; k < AB; ++k)
-        if (ab + k < DIN) outp[k * a.n] = vb[k];
-      outp += DIN * a.n;
-    }
-    if (++slot == NST) slot = 0;
-  }
-  // Gamma-bar = K . M-bar: this lane's block, then the sum over the blocks of the channel
-  float Gb[DENV];
-#pragma unroll
-  for (int b = 0; b < DENV; ++b) Gb[b] = 0.f;
-#define X(k, a_, b_, c_) \
-  if (q == (a_) / AB) Gb[b_] = fmaf(a.kv[k], TP2_REF(Mb, CH, (a_) % AB, c_), Gb[b_]);
-  TP2_EXPAND(P, X)
-#undef X
-#pragma unroll
-  for (int b = 0; b < DENV; ++b)
-#pragma unroll
-    for (int o = CPW; o < 32; o <<= 1) Gb[b] += __shfl_xor_sync(TP_FULLMASK, Gb[b], o);
-  // pass 2: lane (ch, q) takes environment components [q GB, (q+1) GB): omega-bar_e[l], Y-bar_e[b] (environment part)
-  float gq[GB];
-#pragma unroll
-  for (int j = 0; j < GB; ++j) {
-    float v = Gb[j];
-#pragma unroll
-    for (int qq = 1; qq < NBK; ++qq) v = (q == qq) ? Gb[GB * qq + j] : v;
-    gq[j] = a.c_env * v;
-  }
-  for (int64_t e = e0; e < e1; e += 2) {
-    float oa[2], ob[2], y[2][GB];
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-      const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
-      oa[i] = a.om[ee * a.ldo + lA * a.n + nn];
-      ob[i] = a.om[ee * a.ldo + lB * a.n + nn];
-#pragma unroll
-      for (int j = 0; j < GB; ++j) y[i][j] = __ldg(a.Y + ee * a.ldy + GB * q + j);
-    }
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-      if (e + i < e1) {   // (warp-uniform)
-        float xa = gq[0] * y[i][0], xb = 0.f;
-#pragma unroll
-        for (int j = 1; j < GB; ++j) xb = fmaf(gq[j], y[i][j], xb);
-        const float osum = t3_gather_l<CPW>(xa, xb, lA, lB, q);
-        if (q < 4) a.ombar[(e + i) * a.ldob + q * a.n + nn] = osum;
-        float pj[GB];
-        pj[0] = t3_sum_ch<CPW>(oa[i] * gq[0]);
-#pragma unroll
-        for (int j = 1; j < GB; ++j) pj[j] = t3_sum_ch<CPW>(ob[i] * gq[j]);
-        if (ch == 0)
-#pragma unroll
-          for (int j = 0; j < GB; ++j) YbL[(e + i) * DENV + GB * q + j] = pj[j];
-      }
-    }
-  }
-}
-
 // ---- host side ---------------------------------------------------------------------------------------------
 template <int P, bool FIRST, int NST, int WPB>
 int launch_fwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
@@ -437,24 +197,6 @@ int launch_fwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
   if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_fwd<P, FIRST, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
   int64_t warps = (int64_t)a.nc * (a.n / T3_CPW);
   k_tp3_fwd<P, FIRST, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
-  m->launches++;
-  AL_CUDA(m, cudaGetLastError());
-  return ALLEGRO_OK;
-}
-
-template <int P, bool FIRST, int LQ, int NST, int WPB>
-int launch_bwd3(allegro_model* m, const TP2<Pat<P>::NNZ>& a) {
-  constexpr int DIN = Pat<P>::DIN, DOUT = Pat<P>::DOUT;
-  constexpr int NBK = 1 << LQ, CPW = 32 / NBK;
-  constexpr int AB = (DIN + NBK - 1) / NBK, CH = (DOUT + 1) / 2;
-  constexpr int SV = FIRST ? 4 * CPW + 16 : DIN * CPW;
-  constexpr int SF = SV + DOUT * CPW + CPW;
-  constexpr int WSL = 16 * CPW + (LQ == 3 ? 0 : AB * CH * 64) + NST * SF;
-  size_t sm = (size_t)WPB * WSL * 4 + 16;
-  static AttrOnce once;
-  if (once.need(m->device)) { AL_CUDA(m, cudaFuncSetAttribute(k_tp3_bwd<P, FIRST, LQ, NST, WPB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); once.done(m->device); }
-  int64_t warps = (int64_t)a.nc * (a.n / CPW);
-  k_tp3_bwd<P, FIRST, LQ, NST, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, sm, m->stream>>>(a);
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;

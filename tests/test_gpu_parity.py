@@ -292,6 +292,10 @@ VARIANTS = {
     "lmax1_two_layers_n32": (0, 384, dict(n_layers=2, n_tensor=32, resid_alpha=(0.5, 0.5))),
     "lmax3_two_layers": (4, 600, dict(n_layers=2, n_tensor=32, resid_alpha=(0.5, 0.5), twobody_dims=(32, 64), latent_dims=(64,))),
     "odd_channels_n24": (1, 768, dict(n_tensor=24, twobody_dims=(32, 64), latent_dims=(64,))),
+    # fallback paths of the launch list (csrc/compute.cu): d % 32 != 0 -> the last latent layer is NOT fused with the energy /
+    # z-bar epilogue (k_bwd_prep, k_energy run instead); first latent width % 32 != 0 -> no K-concatenated x-bar GEMM
+    "narrow_d48_unfused_last": (1, 768, dict(twobody_dims=(32, 48), latent_dims=(48,), edge_dims=(8,))),
+    "latent0_40_no_kcat": (1, 768, dict(twobody_dims=(32, 64), latent_dims=(40, 64))),
 }
 
 
