@@ -95,8 +95,21 @@ def gemm_impl_bytes_per_edge(hp, kcat=True):
 
 
 def tp_bytes_per_edge(hp):
-    """Algorithmic HBM bytes per ACTIVE edge of the tensor-track kernels (fp32 storage; every operand row read or
-    written once, Y rows and per-center quantities not counted).  D_L from the pruned irreps."""
+    """HBM bytes per ACTIVE edge the tensor-track kernels have to move (fp32 storage; Y rows and per-centre quantities not
+    counted).  Default kernels (tensor track contracted per centre, csrc/tpc_impl.cuh): only the per-edge scalars-by-l and
+    scalar blocks exist -- forward, per layer: omega^L (nl n) + w0 (nl n) read, s^L (n) written; backward, per layer:
+    s-bar^L (n) + w0 (nl n) read, omega^L (nl n) read, omega-bar^L (nl n) written; layer 1 also reads the other layers'
+    s-bar and writes w0-bar (nl n).  SURVEY.md section 8(d)'s figure for the per-edge product formulation (V read + T write,
+    2,304 + 2,304 B at config 2 layer 1) is what these kernels no longer move; it is reported as `survey_bytes_per_edge`."""
+    n, nl, NL = hp.n_tensor, hp.l_max + 1, hp.n_layers
+    fwd = NL * n * (2 * nl + 1)
+    bwd = NL * n * (1 + 3 * nl) + n * ((NL - 1) + nl)
+    return {"tp_fwd": 4.0 * fwd, "tp_bwd": 4.0 * bwd}
+
+
+def tp_survey_bytes_per_edge(hp):
+    """SURVEY.md section 8(d) figure for the tensor product as a per-edge product (V^{L-1} read + T^L written per layer, forward;
+    omega, V, V-bar, s-bar in and V-bar, omega-bar out, backward): what the round-1 kernels moved."""
     n, nl = hp.n_tensor, hp.l_max + 1
     D = {(1, 1): [4, 1], (2, 2): [9, 9, 1], (3, 3): [16, 31, 16, 1]}.get((hp.l_max, hp.n_layers))
     if D is None:
@@ -104,10 +117,9 @@ def tp_bytes_per_edge(hp):
     fwd = bwd = 0.0
     for L in range(1, hp.n_layers + 1):
         din, dout = D[L - 1], D[L]
-        vin = nl if L == 1 else din                   # layer 1 reads w0 (one value per l), not V^0
-        tout = dout if L < hp.n_layers else 0         # last layer writes only the scalars
-        fwd += n * (nl + vin + tout + 1)              # omega, V (or w0), T, s
-        # backward: omega, V (or w0), V-bar^L, s-bar in; V-bar^{L-1} (or w0-bar), omega-bar out
+        vin = nl if L == 1 else din
+        tout = dout if L < hp.n_layers else 0
+        fwd += n * (nl + vin + tout + 1)
         bwd += n * (nl + vin + tout + 1 + vin + nl)
     return {"tp_fwd": 4.0 * fwd, "tp_bwd": 4.0 * bwd}
 
@@ -291,6 +303,9 @@ def main():
     ap.add_argument("--precision", type=int, default=1, choices=[0, 1, 3],
                     help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores (the paper's scheme), 3 fp32 FFMA")
     ap.add_argument("--no-peak-probe", action="store_true", help="skip the TF32 / FFMA peak measurements (~10 s)")
+    ap.add_argument("--drift-steps", type=int, default=0,
+                    help="also run this many NVE steps from the initial state and report the drift of E_pot + E_kin "
+                         "(SURVEY.md section 8(d): config 1, 100 steps at 0.5 fs)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
@@ -376,6 +391,26 @@ def main():
     e, _, f = model.compute(p, s, box, nb, want_atom_energies=False)
     ek = torch.zeros(1, dtype=torch.float64, device=dev)
     ctr = ctypes.c_int64(0)
+
+    drift = None
+    if args.drift_steps > 0:
+        # NVE energy conservation from the initial state (the paper's stability claim, needs trained weights; with
+        # the seeded weights this checks that forces are the gradient of the energy the integrator sees)
+        p0, v0, f0 = p.clone(), v.clone(), f.clone()
+        c0 = ctypes.c_int64(0)
+        ek0 = model.kinetic_energy(v0, s, mass)
+        series = [float(e.item()) + float(ek0.item())]
+        kin = [float(ek0.item())]
+        for _ in range(args.drift_steps):
+            model.step_nve(p0, v0, f0, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, c0, e, ek)
+            series.append(float(e.item()) + float(ek.item())); kin.append(float(ek.item()))
+        a = np.asarray(series)
+        drift = {"steps": args.drift_steps, "dt_fs": cfg.dt_fs, "e_tot_first": a[0], "e_tot_last": a[-1],
+                 "drift_per_atom_eV": (a[-1] - a[0]) / N, "max_dev_per_atom_eV": float(np.abs(a - a[0]).max()) / N,
+                 "rms_fluct_per_atom_eV": float(a.std()) / N, "e_kin_first": kin[0], "e_kin_last": kin[-1],
+                 "e_kin_per_atom_eV": kin[0] / N}
+        nb = model.neighbors(p, box, cfg.hp.r_cut + cfg.skin, reuse=nb)
+        e, _, f = model.compute(p, s, box, nb, want_atom_energies=False)
 
     def step():
         model.step_nve(p, v, f, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, e, ek)
@@ -523,7 +558,8 @@ def main():
                 "tensor_track_hbm": {k: {"achieved": tp_bytes[k] * n_active * K / (prof[k][0] * 1e-3) / 1e9 if prof[k][0] > 0 else 0.0,
                                          "peak": pk["hbm_gbs"], "unit": "GB/s",
                                          "frac": (tp_bytes[k] * n_active * K / (prof[k][0] * 1e-3) / 1e9 / pk["hbm_gbs"]) if prof[k][0] > 0 else 0.0,
-                                         "algorithmic_bytes_per_edge": tp_bytes[k]} for k in ("tp_fwd", "tp_bwd")}}
+                                         "algorithmic_bytes_per_edge": tp_bytes[k],
+                                         "survey_bytes_per_edge": tp_survey_bytes_per_edge(cfg.hp)[k]} for k in ("tp_fwd", "tp_bwd")}}
     if probes and cfg.hp.l_max == 3:
         # config 4: the tensor product is bound by the fp32 pipes, not HBM: report it against the FFMA probe too
         fl = tp_flops_per_edge(cfg.hp)
@@ -550,6 +586,8 @@ def main():
         "e2e": {"value": e2e_val, "unit": unit, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "roofline": roofline,
     }
+    if drift is not None:
+        out["nve_drift"] = drift
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_all, n_one = {0: (192, 192), 1: (3072, 768), 2: (512, 128), 3: (512, 128), 4: (256, 64)}[cfg.index]
         import torch as _t

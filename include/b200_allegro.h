@@ -139,6 +139,24 @@ int allegro_compute_local(allegro_model* m, const double* pos, const int32_t* sp
  * that synchronises anyway: the _host variants, and allegro_step_nve on the steps that rebuild the list. */
 int allegro_status(allegro_model* m);
 
+/* Halo kernels of the spatial decomposition (NEXT-3; the paper's ghost-atom forward / reverse communication, PAPER.md:188,
+ * 214-216).  The messages themselves travel through torch.distributed (paper_2304_10061_b200/domain.py); these calls do
+ * the per-atom work on the device (all pointers DEVICE pointers, enqueued on the model's stream):
+ *   allegro_halo_pack: for the n_send ghosts this rank provides, out_rows[k] = {pos[idx[k]] + shift[k], (double)species[idx[k]]}
+ *     (f64[n_send*4]); idx int64[n_send] indexes the rank's own atoms, shift f64[n_send*3] is the periodic image shift.
+ *   allegro_halo_assemble: pos_all f64[(n_local+n_ghost)*3] = {own positions, received ghost rows} - origin (host f64[3]),
+ *     species_all int32[n_local+n_ghost] likewise: the arrays allegro_compute_local takes.
+ *   allegro_halo_accumulate: force_out f64[n_local*3] = force_all[0 : n_local] + sum over k of returned[k] at atom idx[k]
+ *     (returned f64[n_send*3]: what the other domains accumulated on the ghosts this rank provided; an atom may appear
+ *     several times, fp64 atomics). */
+int allegro_halo_pack(allegro_model* m, const double* pos, const int32_t* species, const int64_t* idx, const double* shift,
+                      int64_t n_send, double* out_rows);
+int allegro_halo_assemble(allegro_model* m, const double* pos, const int32_t* species, int64_t n_local,
+                          const double* ghost_rows, int64_t n_ghost, const double origin[3], double* pos_all,
+                          int32_t* species_all);
+int allegro_halo_accumulate(allegro_model* m, const double* force_all, int64_t n_local, const int64_t* idx,
+                            const double* returned, int64_t n_send, double* force_out);
+
 /* One velocity-Verlet NVE step: v += dt/2 F/m; r += dt v; [rebuild list at cutoff
  * r_cut+skin if *step_counter % rebuild_every == 0]; F; v += dt/2 F/m.  `force` f64[N*3] (device) must
  * hold F(r) of the current positions on entry (call allegro_compute once before the first step) and
@@ -230,6 +248,16 @@ int allegro_step_nvt(allegro_model* m, double* pos, double* vel, double* force, 
                      const double* mass, int64_t n_atoms, const double box[3], double dt_fs, int32_t rebuild_every,
                      double skin, allegro_nbr** nbr, int64_t* step_counter, double* e_pot, double* e_kin,
                      double* nh_state, double t0_K, double tau_fs);
+
+/* Which kernels run the tensor track (Eq. (2) :132-138; SURVEY.md section 8(a) steps 5-7 and their backward).
+ *   0 (default)  contracted per centre: because tensor features only ever leave the track through their scalar block,
+ *                s^L_e = V^0_e . (M^1_i ... M^{L-1}_i M^L_i e_0) with the per-centre operators contracted first; no
+ *                [edges, D, n] tensor is formed.  Used whenever the model's irreps match the generated
+ *                patterns (all five configs), up to 3 layers; other models fall back to mode 1 by themselves.
+ *   1            one D_{L-1} x D_L product per edge, channel and layer, V^L_e stored: FFMA kernels (fp32 modes) or warp-level
+ *                mma.sync TF32 (precision 1, l_max = 3: SURVEY NEXT-2, the paper's own TF32 tensor product).
+ * Same function either way (fp32 summation order differs).  Must be called before the first compute call. */
+int allegro_set_tensor_track(allegro_model* m, int32_t mode);
 
 /* Debug mode (tests only; default off): keep every intermediate tensor that allegro_debug_tensor can name.
  * Without it the final latent x^{NL} is consumed inside the epilogue of the last latent GEMM and never stored. */

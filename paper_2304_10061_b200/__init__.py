@@ -74,7 +74,7 @@ EXPORTS = [
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
     "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps", "allegro_compute_local",
-    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32",
+    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32", "allegro_halo_pack", "allegro_halo_assemble", "allegro_halo_accumulate", "allegro_set_tensor_track",
     "allegro_last_error",
 ]
 
@@ -125,6 +125,10 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_last_active_edges.argtypes = [vp, P(i64)]
     lib.allegro_debug_tensor.argtypes = [vp, C.c_char_p, vp, P(i64)]
     lib.allegro_status.argtypes = [vp]
+    lib.allegro_set_tensor_track.argtypes = [vp, i32]
+    lib.allegro_halo_pack.argtypes = [vp, vp, vp, vp, vp, i64, vp]
+    lib.allegro_halo_assemble.argtypes = [vp, vp, vp, i64, vp, i64, P(C.c_double), vp, vp]
+    lib.allegro_halo_accumulate.argtypes = [vp, vp, i64, vp, vp, i64, vp]
     lib.allegro_probe_ffma.argtypes = [vp, C.c_double, P(C.c_double), P(C.c_double)]
     lib.allegro_probe_tf32.argtypes = [vp, C.c_double, P(C.c_double), P(C.c_double)]
     lib.allegro_last_error.argtypes = [vp]
@@ -283,6 +287,10 @@ class Allegro:
         self._check(self._lib.allegro_graph_steps(self._h, C.byref(v)))
         return v.value
 
+    def set_tensor_track(self, mode: int) -> None:
+        """allegro_set_tensor_track: 0 contracted per centre (default), 1 per-edge products (before the first compute)."""
+        self._check(self._lib.allegro_set_tensor_track(self._h, int(mode)))
+
     def status(self) -> None:
         """allegro_status: synchronise the model's stream and raise what the device-pointer calls since the last check
         flagged (coincident atoms -> ALLEGRO_ERR_NONFINITE, species out of range -> ALLEGRO_ERR_BAD_ARG)."""
@@ -296,6 +304,37 @@ class Allegro:
             b, s = C.c_double(0), C.c_double(0)
             self._check(fn(self._h, float(sustain_s), C.byref(b), C.byref(s)))
             out[name] = {"burst": b.value, "sustained": s.value}
+        return out
+
+    # -- NEXT-3 halo kernels (domain.py) ------------------------------------------------------------------
+    def halo_pack(self, pos, species, idx, shift):
+        """allegro_halo_pack -> f64[n_send, 4] rows [x, y, z, species] of the ghosts this rank provides."""
+        t = self._torch
+        self._sync_stream()
+        k = int(idx.shape[0])
+        out = t.empty((k, 4), dtype=t.float64, device=pos.device)
+        self._check(self._lib.allegro_halo_pack(self._h, pos.data_ptr(), species.data_ptr(), idx.data_ptr(), shift.data_ptr(), k,
+                                                out.data_ptr()))
+        return out
+
+    def halo_assemble(self, pos, species, ghost_rows, origin):
+        """allegro_halo_assemble -> (pos_all f64[n_local + n_ghost, 3] in the local frame, species_all int32)."""
+        t = self._torch
+        self._sync_stream()
+        nl, ng = int(pos.shape[0]), int(ghost_rows.shape[0])
+        pos_all = t.empty((nl + ng, 3), dtype=t.float64, device=pos.device)
+        sp_all = t.empty(nl + ng, dtype=t.int32, device=pos.device)
+        self._check(self._lib.allegro_halo_assemble(self._h, pos.data_ptr(), species.data_ptr(), nl, ghost_rows.data_ptr(), ng,
+                                                    _box3(origin), pos_all.data_ptr(), sp_all.data_ptr()))
+        return pos_all, sp_all
+
+    def halo_accumulate(self, force_all, n_local, idx, returned):
+        """allegro_halo_accumulate -> f64[n_local, 3]: local forces + what came back for the ghosts this rank provided."""
+        t = self._torch
+        self._sync_stream()
+        out = t.empty((n_local, 3), dtype=t.float64, device=force_all.device)
+        self._check(self._lib.allegro_halo_accumulate(self._h, force_all.data_ptr(), int(n_local), idx.data_ptr(), returned.data_ptr(),
+                                                      int(idx.shape[0]), out.data_ptr()))
         return out
 
     def last_active_edges(self) -> int:

@@ -11,10 +11,13 @@
 
 static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
   if (!m->work) m->work = new Work();
+  m->work_sized = true;
   Work& w = *m->work;
   int64_t M = std::max<int64_t>(nb->max_chunk_edges, 1), Nc = std::max<int64_t>(nb->max_chunk_centers, 1);
   const allegro_hparams& hp = m->hp;
   int d = m->d, n = m->n, nA = m->nA, NL = m->NL;
+  const bool tpc = tpc_eligible(m);          // tensor track contracted per centre: no [edges, D, n] tensors at all
+  const bool kcat = al_gemm_supports_kcat(m) && (hp.latent_dims[0] % 32 == 0);
   if (M > w.cap_edges || w.XS.empty()) {
     auto R = [&](DevBuf& b, size_t floats) { return al_reserve(m, b, floats * 4 + 64); };
     AL_CHECK(R(w.ei, M)); AL_CHECK(R(w.ej, M)); AL_CHECK(R(w.geo, 4 * M)); AL_CHECK(R(w.u, M)); AL_CHECK(R(w.du, M)); AL_CHECK(R(w.sig, M));
@@ -31,7 +34,7 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     for (int L = 0; L < NL; ++L) {
       AL_CHECK(R(w.XS[L], (size_t)M * (d + n)));
       if (L >= 1) AL_CHECK(R(w.OM[L + 1], (size_t)M * nA));
-      if (L >= 1) AL_CHECK(R(w.T[L], (size_t)M * m->D[L] * n));
+      if (L >= 1 && !tpc) AL_CHECK(R(w.T[L], (size_t)M * m->D[L] * n));   // V^L: only the per-edge product kernels store it
       Dmax = std::max(Dmax, m->D[L]);
       w.lat_z[L].resize(hp.n_latent); w.lat_a[L].resize(hp.n_latent);
       for (int k = 0; k < hp.n_latent; ++k) {
@@ -44,7 +47,13 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     AL_CHECK(R(w.XB0, (size_t)M * d)); AL_CHECK(R(w.XB1, (size_t)M * d));
     AL_CHECK(R(w.ZB0, (size_t)M * maxw)); AL_CHECK(R(w.ZB1, (size_t)M * maxw));
     AL_CHECK(R(w.G, (size_t)M * (d + n))); AL_CHECK(R(w.OB, (size_t)M * 2 * nA));
-    AL_CHECK(R(w.VB0, (size_t)M * Dmax * n)); AL_CHECK(R(w.VB1, (size_t)M * Dmax * n));
+    if (!tpc) { AL_CHECK(R(w.VB0, (size_t)M * Dmax * n)); AL_CHECK(R(w.VB1, (size_t)M * Dmax * n)); }
+    if (tpc) {
+      // s-bar^L of every layer stays alive until layer 1's backward: its own [M][n] rows with the K-concatenated x-bar GEMM,
+      // else the whole [x-bar part | s-bar] buffer of each layer
+      if (kcat) AL_CHECK(R(w.SB, (size_t)NL * M * n));
+      else { w.Gl.resize(NL); for (int L = 0; L < NL; ++L) AL_CHECK(R(w.Gl[L], (size_t)M * (d + n))); }
+    }
     w.n_eparts = (d % 32 == 0) ? al_gemm_row_parts(m, d) : 0;   // > 0: last latent layer fused with energy / z-bar (EPI_LATENT_LAST)
     // u-bar partial slots: [0, P) EPI_LATENT_LAST, then P per fused prep stage (NL of them), then one accumulated by k_bwd_prep
     w.n_uparts = (w.n_eparts > 0) ? w.n_eparts * (NL + 1) + 1 : 1;
@@ -56,6 +65,10 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
     AL_CHECK(al_reserve(m, w.deg, (size_t)Nc * 4 + 64));
     AL_CHECK(al_reserve(m, w.rowa, (size_t)(Nc + 1) * 8 + 64));
     AL_CHECK(al_reserve(m, w.gamma, (size_t)Nc * m->Denv * n * 4 + 64));
+    if (tpc) {
+      const size_t per = (size_t)NL * Nc * m->Denv * n * 4 + 64;
+      AL_CHECK(al_reserve(m, w.tpc_gam, per)); AL_CHECK(al_reserve(m, w.tpc_nvec, per)); AL_CHECK(al_reserve(m, w.tpc_gacc, per));
+    }
     w.cap_centers = Nc;
   }
   if (!w.m_act.p) {
@@ -71,9 +84,9 @@ void al_work_free(allegro_model* m) {
   Work& w = *m->work;
   std::vector<DevBuf*> all = {&w.deg, &w.rowa, &w.scan_tmp, &w.m_act, &w.ei, &w.ej, &w.geo, &w.u, &w.du, &w.sig, &w.B, &w.dB, &w.Y,
                               &w.XF, &w.WE, &w.gamma, &w.XB0, &w.XB1, &w.ZB0, &w.ZB1, &w.G, &w.OB, &w.VB0, &w.VB1,
-                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom, &w.nh_scal, &w.host_stage};
+                              &w.ubar, &w.epart, &w.Ybar, &w.ge, &w.eatom, &w.nh_scal, &w.host_stage, &w.tpc_gam, &w.tpc_nvec, &w.tpc_gacc, &w.SB};
   for (auto* b : all) al_release(m, *b);
-  for (auto* v : {&w.tb_z, &w.tb_a, &w.XS, &w.OM, &w.T}) for (auto& b : *v) al_release(m, b);
+  for (auto* v : {&w.tb_z, &w.tb_a, &w.XS, &w.OM, &w.T, &w.Gl}) for (auto& b : *v) al_release(m, b);
   for (auto* vv : {&w.lat_z, &w.lat_a}) for (auto& v : *vv) for (auto& b : v) al_release(m, b);
   delete m->work;
   m->work = nullptr;
@@ -104,6 +117,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   const int* mp = (const int*)w.m_act.p;
   cudaStream_t st = m->stream;
   const bool fused_last = w.n_eparts > 0;
+  const bool tpc = tpc_eligible(m);
   EdgeGeomArgs ga{};
   ga.pos = pos; ga.species = species; memcpy(ga.box, box, 24); ga.rc = hp.r_cut; ga.p = hp.poly_p; ga.NB = m->NB;
   ga.lmax = m->lmax; ga.row_ptr = (const int64_t*)nb->row_ptr.p; ga.j = (const int32_t*)nb->j.p;
@@ -131,8 +145,8 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   for (int L = 1; L <= NL; ++L) {
     const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
     int ldo = (L == 1) ? 2 * nA : nA;
-    const float* Vin = (L == 1) ? nullptr : (float*)w.T[L - 1].p;
-    float* Tout = (L < NL) ? (float*)w.T[L].p : nullptr;
+    const float* Vin = (L == 1 || tpc) ? nullptr : (float*)w.T[L - 1].p;
+    float* Tout = (L < NL && !tpc) ? (float*)w.T[L].p : nullptr;
     AL_CHECK(k_launch_tp_fwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, Tout, (float*)w.XS[L - 1].p + d, d + n));
     for (int k = 0; k < nlat; ++k) {
       bool last = (k == nlat - 1);
@@ -193,22 +207,29 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       AL_CHECK(al_gemm(m, g));
       std::swap(zb, zb_o);
     }
-    if (kcat)   // s-bar only: [M, h] x W_lat0[d:, :]^T -> G[:, d:]
-      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->sbar[L - 1], true, (float*)w.G.p + d, d + n, m_cap, mp, EPI_PLAIN)));
+    // [x-bar part | s-bar] of this layer.  Contracted tensor track: s-bar^L of every layer must survive until layer 1's
+    // backward (V-bar^0_e = sum_L s-bar^L_e n^L), so each layer has its own rows (SB with the K-concatenated x-bar GEMM,
+    // a whole G buffer per layer otherwise); per-edge product kernels: one G buffer re-used by every layer.
+    float* Gp = (tpc && !kcat) ? (float*)w.Gl[L - 1].p : (float*)w.G.p;
+    float* sbp = (tpc && kcat) ? (float*)w.SB.p + (size_t)(L - 1) * w.cap_edges * n : Gp + d;
+    const int sbl = (tpc && kcat) ? n : d + n;
+    w.sb_ptr[L - 1] = sbp; w.sb_ld[L - 1] = sbl;
+    if (kcat)   // s-bar only: [M, h] x W_lat0[d:, :]^T
+      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->sbar[L - 1], true, sbp, sbl, m_cap, mp, EPI_PLAIN)));
     else
-      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->latent[L - 1][0], true, (float*)w.G.p, d + n, m_cap, mp, EPI_PLAIN)));
+      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->latent[L - 1][0], true, Gp, d + n, m_cap, mp, EPI_PLAIN)));
     const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
     int ldo = (L == 1) ? 2 * nA : nA;
-    const float* Vin = (L == 1) ? nullptr : (float*)w.T[L - 1].p;
+    const float* Vin = (L == 1 || tpc) ? nullptr : (float*)w.T[L - 1].p;
     int ldob = (L == 1) ? 2 * nA : nA;
     float* ombar = (L == 1) ? (float*)w.OB.p + nA : (float*)w.OB.p;
     float* vprev = (vb == vb_a) ? vb_b : vb_a;
-    AL_CHECK(k_launch_tp_bwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, vb, (float*)w.G.p + d, d + n, vprev, ombar,
+    AL_CHECK(k_launch_tp_bwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, vb, sbp, sbl, vprev, ombar,
                              ldob, (float*)w.OB.p));
     vb = vprev;
     GemmArgs g = mk((float*)w.OB.p, ldob, (L == 1) ? m->emb01 : m->emb[L - 1], true, xb_o, d, m_cap, mp,
                     rank1 ? EPI_ADD2R : EPI_ADD2);
-    g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = (float*)w.G.p; g.ld2 = d + n;
+    g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = Gp; g.ld2 = d + n;
     g.u = (float*)w.sig.p; g.aux3 = m->w_eff_f;
     if (kcat) {
       const int h = hp.latent_dims[0];
@@ -549,6 +570,7 @@ extern "C" int allegro_debug_tensor(allegro_model* m, const char* name, float* o
   } else if (s[0] == 'V' && s.size() == 2) {
     int L = s[1] - '0';
     if (L < 1 || L >= m->NL) return ALLEGRO_ERR_BAD_ARG;
+    if (!w.T[L].p) { al_set_error(m, "V^L is never formed by the per-centre-contracted tensor track (allegro_set_tensor_track 1 keeps it)"); return ALLEGRO_ERR_BAD_ARG; }
     src = (float*)w.T[L].p; width = ld = m->D[L] * n;
   } else if (s == "gamma") { src = (float*)w.gamma.p; width = ld = m->Denv * n; rows = w.last_nc; }
   else { al_set_error(m, "unknown debug tensor"); return ALLEGRO_ERR_BAD_ARG; }

@@ -794,6 +794,9 @@ int tpw_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, 
 int tpw_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
             const float* VbarL, const float* sbar, int lds, float* Vbar_prev, float* ombar, int ldob, float* w0bar);
 
+int tpc_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* w0, int ldw, float* xs, int ldx);
+int tpc_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* w0, int ldw, float* ombar, int ldob,
+            float* w0bar);
 int tp2_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
             float* Tout, float* xs, int ldx);
 int tp2_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* Vin, const float* w0, int ldw,
@@ -804,7 +807,9 @@ int k_launch_tp_fwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
   ProfScope _ps(m, PC_TP_FWD);
   if (nc <= 0) return ALLEGRO_OK;
   {
-    int rc = tp2_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);   // cp.async ring + FFMA2 (tp2_kernels.cu)
+    int rc = tpc_fwd(m, w, L, nc, om, ldo, w0, ldw, xs, ldx);              // contracted per centre (tpc_kernels.cu): the default
+    if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
+    rc = tp2_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);       // per-edge products: cp.async ring + FFMA2 / mma.sync
     if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
     rc = tpw_fwd(m, w, L, nc, om, ldo, Vin, w0, ldw, Tout, xs, ldx);       // warp-per-(center, channel group) fallback
     if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
@@ -830,7 +835,9 @@ int k_launch_tp_bwd(allegro_model* m, Work& w, int L, int nc, const float* om, i
   ProfScope _ps(m, PC_TP_BWD);
   if (nc <= 0) return ALLEGRO_OK;
   {
-    int rc = tp2_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
+    int rc = tpc_bwd(m, w, L, nc, om, ldo, w0, ldw, ombar, ldob, w0bar);
+    if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
+    rc = tp2_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
     if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;
     rc = tpw_bwd(m, w, L, nc, om, ldo, Vin, w0, ldw, VbarL, sbar, lds, Vbar_prev, ombar, ldob, w0bar);
     if (rc != ALLEGRO_ERR_UNIMPLEMENTED) return rc;

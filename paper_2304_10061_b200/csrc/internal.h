@@ -127,6 +127,7 @@ struct allegro_model {
   cudaStream_t stream = 0;
   allegro_alloc_fn alloc_fn = nullptr; allegro_free_fn free_fn = nullptr; void* alloc_user = nullptr;
   int64_t chunk_edges = 1 << 20;
+  int tt_mode = 0;                        // tensor track: 0 contracted per centre (tpc_impl.cuh), 1 per-edge products (allegro_set_tensor_track)
   bool debug_keep = false;                // allegro_set_debug: also store tensors that are otherwise consumed on chip
   int64_t launches = 0;
   // Alternating sweep direction of the edge-ordered kernels (GEMM row tiles, tensor-track centres): every such launch
@@ -139,6 +140,7 @@ struct allegro_model {
   void* tmaps = nullptr;                  // tensor-map cache of the tcgen05 GEMMs (gemm_tc.cu), freed by al_gemm_tc_free
   // workspace (per chunk), grown on demand
   struct Work* work = nullptr;
+  bool work_sized = false;                // the per-chunk buffers have been laid out (fixes the tensor-track mode)
   // per-kernel-group event timing (allegro_profile_*)
   bool prof = false;
   struct ProfRec { int cat; cudaEvent_t a, b; };

@@ -21,6 +21,11 @@ struct Work {
   std::vector<DevBuf> T;                    // [NL]: T^L = V^L for L < NL, [M][D_L][n]
   std::vector<std::vector<DevBuf>> lat_z, lat_a;   // [NL][n_latent]
   DevBuf gamma;                             // [Nc][Denv][n] of the layer being processed (debug tap)
+  // per-centre-contracted tensor track (tpc_impl.cuh): Gamma^L, n^L, Gamma-bar accumulators, each [NL][Nc][Denv][n];
+  // s-bar^L of every layer [NL][M][n] (layer 1's backward needs them all); sb_ptr / sb_ld: where each layer's s-bar lives
+  DevBuf tpc_gam, tpc_nvec, tpc_gacc, SB;
+  std::vector<DevBuf> Gl;                   // [NL] per-layer [x-bar part | s-bar] buffers when the x-bar GEMM is not K-concatenated
+  const float* sb_ptr[AL_MAX_LAYERS] = {}; int sb_ld[AL_MAX_LAYERS] = {};
   // backward
   DevBuf XB0, XB1;                          // x-bar ping-pong [M][d]
   DevBuf ZB0, ZB1;                          // z-bar ping-pong [M][max width]
@@ -47,6 +52,7 @@ struct EdgeGeomArgs {
 };
 
 bool tp2_eligible(const allegro_model* m);   // tp2_kernels.cu
+bool tpc_eligible(const allegro_model* m);   // tpc_kernels.cu: the per-centre-contracted kernels run (default when possible)
 // Y-bar partial buffers: part0[0] = first part of the V^0 contribution, part0[L] = first part of layer L's
 // environment contribution (one part per channel group of the kernel that writes it); returns the total count.
 int al_ybar_layout(const allegro_model* m, int* part0);

@@ -379,6 +379,14 @@ extern "C" int allegro_set_zbl(allegro_model* m, const double* atomic_numbers) {
   return ALLEGRO_OK;
 }
 
+extern "C" int allegro_set_tensor_track(allegro_model* m, int32_t mode) {
+  if (!m || (mode != 0 && mode != 1)) return ALLEGRO_ERR_BAD_ARG;
+  if (m->work_sized) { al_set_error(m, "the tensor-track mode must be set before the first compute call"); return ALLEGRO_ERR_BAD_ARG; }
+  m->tt_mode = mode;
+  m->config_gen++;
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_set_debug(allegro_model* m, int on) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   m->debug_keep = on != 0;

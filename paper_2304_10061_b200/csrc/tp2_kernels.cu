@@ -70,6 +70,7 @@ bool tp2_eligible(const allegro_model* m) {
 // channel groups of the kernel that runs layer L's backward: 8-channel teams for the mma.sync l_max = 3 kernels
 // (tp3mb_impl.cuh, TF32 mode), 32-channel warps otherwise
 static int bwd_groups(const allegro_model* m, int L) {
+  if (tpc_eligible(m)) return m->n / 32;   // contracted kernels: one warp per (centre, 32 channels) in every layer
   int p = match_pattern(m->tp_host[L - 1]);
   return ((p == P_16_16_31 || p == P_16_31_16) && tp3m_bwd_active(m)) ? m->n / 8 : m->n / 32;
 }

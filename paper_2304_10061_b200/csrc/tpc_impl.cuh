@@ -1,0 +1,378 @@
+// Tensor track, contracted per centre ("collapsed"): the default tensor-track kernels (SURVEY.md section 8(a) steps 5-7 and
+// their backward in step 11; Eq. (2) :132-138, fused path-weighted CG tensor :160-164, Fig. 3 :180).
+//
+// The paper sums the environment before the product because the tensor product is bilinear (Eq. (2) line 2).
+// The same linearity reaches across layers: tensor features never pass through a nonlinearity -- only the scalar block
+// s^L_e = V^L_e[(0,+)] leaves the tensor track -- so with  M^k_i[a,c] = sum_b K^k[a,b,c] Gamma^k_i[b]  (per centre
+// i and channel n, the same for all edges of the centre)
+//     V^L_e = V^0_e M^1_i M^2_i ... M^L_i        and        s^L_e = V^0_e . n^L_i,     n^L_i = M^1_i ... M^{L-1}_i M^L_i[:, 0].
+// Contracting the per-centre operators FIRST leaves one D_0-long dot product per edge, channel and layer, instead of a
+// D_{L-1} x D_L product per edge: V^L_e is never formed, nothing of size [edges, D, n] is read or written, and the work that
+// involves the sparse tensors K^k happens once per centre.  It is the same function up to the order of the fp32 sums
+// (the fp64 oracle follows the paper's order, layer by layer and edge by edge).  Matrix-free: M^k is never built either;
+// the three trilinear forms of K^k(Gamma^k) that are needed run straight off the compile-time sparsity pattern
+// (tp2_patterns.inc) with every operand in registers:
+//     fwd :  y[a]  = sum K[a,b,c] Gamma[b] x[c]      (y = M x)
+//     tr  :  v[c]  = sum K[a,b,c] Gamma[b] u[a]      (v = M^T u)
+//     gb  :  g[b]  = sum K[a,b,c] u[a] w[c]          (d(u^T M w) / dGamma)
+// Forward, layer L (one warp = centre x 32 channels, lane = channel):
+//     Gamma^L_i = c_env sum_e omega^L_e (x) Y_e  ->  n^L_i (needs Gamma^1..Gamma^L)  ->  s^L_e = sum_a w0_e[l(a)] Y_e[a] n^L_i[a].
+// Backward, layer L (reverse order), with s-bar^L_e from the latent MLP's backward:
+//     n-bar^L_i = sum_e s-bar^L_e V^0_e;   u_0 = n-bar^L, w_L = e_0, w_k = M^{k+1} w_{k+1}, u_k = M^{k T} u_{k-1}:
+//     Gamma-bar^k_i += gb_k(u_{k-1}, w_k) for k = 1..L   (contributions to k < L wait in a per-centre accumulator until layer
+//     k's own backward, which then has the complete Gamma-bar^k);
+//     pass B: omega-bar^L_e[l] = c_env sum_{m} Gamma-bar^L[(l,m)] Y_e[(l,m)],  Y-bar_e[b] += c_env sum_n omega^L_e[l(b)] Gamma-bar^L[b];
+//     layer 1 also: V-bar^0_e = sum_L s-bar^L_e n^L_i  ->  w0-bar_e[l] = sum_{a in l} V-bar^0_e[a] Y_e[a],  Y-bar_e[a] += sum_n w0_e[l(a)] V-bar^0_e[a].
+// HBM traffic per edge at config 2/3 (n = 64): forward 2 x (omega 768 + w0 768 + s 256 B), backward 6.3 KB, against
+// 7.4 + 12.0 KB for the per-edge product kernels (tp2_impl.cuh), and the [edges, D, n] buffers T, V-bar are not allocated.
+#pragma once
+#include "tp2_impl.cuh"
+
+constexpr int TPC_MAXL = 3;   // layers the contracted kernels are instantiated for
+
+// pattern of layer k (1-based) of an (l_max, NL) model: the eligibility test (tp2_eligible) guarantees these roles
+template <int LM, int NL, int K> struct TpcPat {
+  static constexpr int P = (LM == 1) ? (K < NL ? P_4_4_4 : P_4_4_1) : (LM == 2) ? (K < NL ? P_9_9_9 : P_9_9_1)
+                                     : (K == 1 ? P_16_16_31 : K == 2 ? P_16_31_16 : P_16_16_1);
+};
+template <int LM> struct TpcEnv { static constexpr int DENV = (LM + 1) * (LM + 1); };
+
+template <int LM, int NL>
+struct TPC {
+  static constexpr int NNZ1 = Pat<TpcPat<LM, NL, 1>::P>::NNZ;
+  static constexpr int NNZ2 = NL >= 2 ? Pat<TpcPat<LM, NL, (NL >= 2 ? 2 : 1)>::P>::NNZ : 1;
+  static constexpr int NNZ3 = NL >= 3 ? Pat<TpcPat<LM, NL, (NL >= 3 ? 3 : 1)>::P>::NNZ : 1;
+  const int64_t* rowa; int nc, n; float c_env; int rev;
+  const float* Y; int ldy;
+  const float* w0; int ldw;                   // w^0_e[l][n]
+  const float* om; int ldo;                   // omega^L_e[l][n] of THIS layer
+  float* xs; int ldx;                         // forward: s^L_e[n]
+  float* gam; float* nvec; float* gacc; int64_t cstride;   // per-centre [layer][centre][DENV][n]; cstride = centres * DENV * n
+  const float* sb[TPC_MAXL]; int lds[TPC_MAXL];            // backward: s-bar^k_e[n] of every layer k (layer 1 needs them all)
+  float* ombar; int ldob; float* w0bar;
+  float* Ybar; int64_t ybar_pstride; int ybar_part0, ybar_partL;
+  float kv1[NNZ1], kv2[NNZ2], kv3[NNZ3];      // values of K^1, K^2, K^3 in pattern order
+};
+
+// ---- the three trilinear sweeps over the pattern of P ------------------------------------------------------------------------
+// E0: the right-hand vector is e_0 (only the entries with c = 0 contribute)
+template <int P, bool E0, int NNZ>
+__device__ __forceinline__ void tpc_fwd(const float (&kv)[NNZ], const float* G, const float* x, float* y) {
+#pragma unroll
+  for (int a = 0; a < Pat<P>::DIN; ++a) y[a] = 0.f;
+#define X(k, a_, b_, c_) \
+  if (!E0) y[a_] = fmaf(kv[k] * G[b_], x[c_], y[a_]); else if ((c_) == 0) y[a_] = fmaf(kv[k], G[b_], y[a_]);
+  TP2_EXPAND(P, X)
+#undef X
+}
+template <int P, int NNZ>
+__device__ __forceinline__ void tpc_tr(const float (&kv)[NNZ], const float* G, const float* u, float* v) {
+#pragma unroll
+  for (int c = 0; c < Pat<P>::DOUT; ++c) v[c] = 0.f;
+#define X(k, a_, b_, c_) v[c_] = fmaf(kv[k] * G[b_], u[a_], v[c_]);
+  TP2_EXPAND(P, X)
+#undef X
+}
+// g[b] += ...  (accumulates)
+template <int P, bool E0, int NNZ>
+__device__ __forceinline__ void tpc_gb(const float (&kv)[NNZ], const float* u, const float* w, float* g) {
+#define X(k, a_, b_, c_) \
+  if (!E0) g[b_] = fmaf(kv[k] * u[a_], w[c_], g[b_]); else if ((c_) == 0) g[b_] = fmaf(kv[k], u[a_], g[b_]);
+  TP2_EXPAND(P, X)
+#undef X
+}
+
+// ---- one batch of up to 8 edges of a centre: NLV rows of 32 channels each + the Y rows (one contiguous block, one value per
+//      lane, components broadcast by shuffle as in gamma_pass) ------------------------------------------------------------------
+template <int DENV>
+struct TpcBatch {
+  static constexpr int NLV = nlv_of(DENV), LDY = (DENV + 3) & ~3, NR = LDY / 4;
+  float yr[NR];
+  __device__ __forceinline__ void load_y(const float* Y, int64_t e, int64_t e1, int lane) {
+    const int64_t ylast = e1 * LDY - 1;
+#pragma unroll
+    for (int k = 0; k < NR; ++k) {
+      const int64_t idx = e * LDY + k * 32 + lane;
+      yr[k] = __ldg(Y + (idx < ylast ? idx : ylast));
+    }
+  }
+  __device__ __forceinline__ float y(int i, int b) const { return __shfl_sync(TP_FULLMASK, yr[(i * LDY + b) >> 5], (i * LDY + b) & 31); }
+};
+
+// ======================================================================================================
+// forward of layer L
+// ======================================================================================================
+template <int LM, int NL, int L, int WPB>
+static __global__ void __launch_bounds__(WPB * 32) k_tpc_fwd(const __grid_constant__ TPC<LM, NL> a) {
+  constexpr int DENV = TpcEnv<LM>::DENV, NLV = nlv_of(DENV);
+  constexpr int P1 = TpcPat<LM, NL, 1>::P, P2 = TpcPat<LM, NL, (NL >= 2 ? 2 : 1)>::P, P3 = TpcPat<LM, NL, (NL >= 3 ? 3 : 1)>::P;
+  const int lane = threadIdx.x & 31, ng = a.n / 32;
+  int64_t wg = (int64_t)blockIdx.x * WPB + (threadIdx.x >> 5);
+  if (wg >= (int64_t)a.nc * ng) return;
+  if (a.rev) wg = (int64_t)a.nc * ng - 1 - wg;
+  const int c = (int)(wg / ng), nn = (int)(wg - (int64_t)c * ng) * 32 + lane;
+  const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
+  if (e1 <= e0) return;
+  float nv[DENV];
+  {
+    float G[L][DENV];
+    gamma_pass<DENV>(a, e0, e1, nn, G[L - 1]);                       // Gamma^L_i (Eq. (2) line 2: sum before product)
+    float* gp = a.gam + ((size_t)c * DENV) * a.n + nn;
+#pragma unroll
+    for (int b = 0; b < DENV; ++b) gp[(L - 1) * a.cstride + (size_t)b * a.n] = G[L - 1][b];
+#pragma unroll
+    for (int k = 0; k < L - 1; ++k)
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) G[k][b] = gp[k * a.cstride + (size_t)b * a.n];
+    // n^L = M^1 ... M^{L-1} M^L e_0
+    if constexpr (L == 1) {
+      tpc_fwd<P1, true>(a.kv1, G[0], nullptr, nv);
+    } else if constexpr (L == 2) {
+      float x1[Pat<P2>::DIN];
+      tpc_fwd<P2, true>(a.kv2, G[1], nullptr, x1);
+      tpc_fwd<P1, false>(a.kv1, G[0], x1, nv);
+    } else {
+      float x2[Pat<P3>::DIN], x1[Pat<P2>::DIN];
+      tpc_fwd<P3, true>(a.kv3, G[2], nullptr, x2);
+      tpc_fwd<P2, false>(a.kv2, G[1], x2, x1);
+      tpc_fwd<P1, false>(a.kv1, G[0], x1, nv);
+    }
+    float* np = a.nvec + (L - 1) * a.cstride + ((size_t)c * DENV) * a.n + nn;
+#pragma unroll
+    for (int b = 0; b < DENV; ++b) np[(size_t)b * a.n] = nv[b];
+  }
+  // s^L_e = sum_a w0_e[l(a)] Y_e[a] n^L[a], 8 edges in flight
+  for (int64_t e = e0; e < e1; e += 8) {
+    float w[8][NLV];
+    TpcBatch<DENV> yb;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
+#pragma unroll
+      for (int l = 0; l < NLV; ++l) w[i][l] = a.w0[ee * a.ldw + l * a.n + nn];
+    }
+    yb.load_y(a.Y, e, e1, lane);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      float t[NLV];
+#pragma unroll
+      for (int l = 0; l < NLV; ++l) t[l] = 0.f;
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) t[l_of(b)] = fmaf(yb.y(i, b), nv[b], t[l_of(b)]);
+      float s = 0.f;
+#pragma unroll
+      for (int l = 0; l < NLV; ++l) s = fmaf(w[i][l], t[l], s);
+      if (e + i < e1) a.xs[(e + i) * a.ldx + nn] = s;
+    }
+  }
+}
+
+// ======================================================================================================
+// backward of layer L
+// ======================================================================================================
+template <int LM, int NL, int L, int WPB>
+static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_constant__ TPC<LM, NL> a) {
+  constexpr int DENV = TpcEnv<LM>::DENV, NLV = nlv_of(DENV);
+  constexpr int P1 = TpcPat<LM, NL, 1>::P, P2 = TpcPat<LM, NL, (NL >= 2 ? 2 : 1)>::P, P3 = TpcPat<LM, NL, (NL >= 3 ? 3 : 1)>::P;
+  const int lane = threadIdx.x & 31, ng = a.n / 32;
+  int64_t wg = (int64_t)blockIdx.x * WPB + (threadIdx.x >> 5);
+  if (wg >= (int64_t)a.nc * ng) return;
+  if (a.rev) wg = (int64_t)a.nc * ng - 1 - wg;
+  const int c = (int)(wg / ng), grp = (int)(wg - (int64_t)c * ng), nn = grp * 32 + lane;
+  const int64_t e0 = a.rowa[c], e1 = a.rowa[c + 1];
+  if (e1 <= e0) return;
+  const size_t cb = ((size_t)c * DENV) * a.n + nn;                   // + layer * cstride + b * n
+  float* Yb0 = a.Ybar + (size_t)(a.ybar_part0 + grp) * a.ybar_pstride;
+  float* YbL = a.Ybar + (size_t)(a.ybar_partL + grp) * a.ybar_pstride;
+
+  // ---- pass A: n-bar^L[a] = sum_e s-bar^L_e w0_e[l(a)] Y_e[a]; layer 1 also turns V-bar^0_e = sum_k s-bar^k_e n^k into
+  //      w0-bar_e and the V^0 part of Y-bar_e --------------------------------------------------------------------------------------
+  float nb[DENV];
+#pragma unroll
+  for (int b = 0; b < DENV; ++b) nb[b] = 0.f;
+  {
+    constexpr int NK = (L == 1) ? NL : 1;                            // layers whose s-bar this pass reads
+    float nk[NK][DENV];                                              // layer 1: n^k of every layer
+    if constexpr (L == 1) {
+#pragma unroll
+      for (int k = 0; k < NL; ++k)
+#pragma unroll
+        for (int b = 0; b < DENV; ++b) nk[k][b] = a.nvec[k * a.cstride + cb + (size_t)b * a.n];
+    }
+    constexpr int EB = (L == 1) ? 4 : 8;                             // edges in flight
+    for (int64_t e = e0; e < e1; e += EB) {
+      float w[EB][NLV], sb[EB][NK];
+      TpcBatch<DENV> yb;
+#pragma unroll
+      for (int i = 0; i < EB; ++i) {
+        const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
+#pragma unroll
+        for (int l = 0; l < NLV; ++l) w[i][l] = a.w0[ee * a.ldw + l * a.n + nn];
+        if constexpr (L == 1) {
+#pragma unroll
+          for (int k = 0; k < NL; ++k) sb[i][k] = a.sb[k][ee * a.lds[k] + nn];
+        } else {
+          sb[i][0] = a.sb[L - 1][ee * a.lds[L - 1] + nn];
+        }
+      }
+      yb.load_y(a.Y, e, e1, lane);
+#pragma unroll
+      for (int i = 0; i < EB; ++i) {
+        const bool ok = e + i < e1;                                  // (warp-uniform)
+        const float s1 = ok ? sb[i][(L == 1) ? 0 : 0] : 0.f;         // s-bar of THIS layer
+        float ws[NLV];
+#pragma unroll
+        for (int l = 0; l < NLV; ++l) ws[l] = w[i][l] * s1;
+        if constexpr (L == 1) {
+          float wbar[NLV], pp[DENV];
+#pragma unroll
+          for (int l = 0; l < NLV; ++l) wbar[l] = 0.f;
+#pragma unroll
+          for (int b = 0; b < DENV; ++b) {
+            const float y = yb.y(i, b);
+            nb[b] = fmaf(ws[l_of(b)], y, nb[b]);
+            float vb = 0.f;                                          // V-bar^0_e[b]
+#pragma unroll
+            for (int k = 0; k < NL; ++k) vb = fmaf(sb[i][k], nk[k][b], vb);
+            wbar[l_of(b)] = fmaf(vb, y, wbar[l_of(b)]);
+            pp[b] = w[i][l_of(b)] * vb;
+          }
+          if (ok) {
+#pragma unroll
+            for (int l = 0; l < NLV; ++l) a.w0bar[(e + i) * a.ldob + l * a.n + nn] = wbar[l];
+            tp_ybar_rows<DENV, true>(Yb0 + (e + i) * DENV, pp, 0, DENV, lane);
+          }
+        } else {
+#pragma unroll
+          for (int b = 0; b < DENV; ++b) nb[b] = fmaf(ws[l_of(b)], yb.y(i, b), nb[b]);
+        }
+      }
+    }
+  }
+
+  // ---- per centre: Gamma-bar^k contributions of this layer's scalars, k = 1..L ------------------------------------------------------
+  float Gb[DENV];                                                    // Gamma-bar^L, complete after this block
+  {
+    float G[L][DENV];
+#pragma unroll
+    for (int k = 0; k < L; ++k)
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) G[k][b] = a.gam[k * a.cstride + cb + (size_t)b * a.n];
+    // what the later layers (processed before this one) left for Gamma-bar^L
+#pragma unroll
+    for (int b = 0; b < DENV; ++b) Gb[b] = (L < NL) ? a.gacc[(L - 1) * a.cstride + cb + (size_t)b * a.n] : 0.f;
+    auto put = [&](int k, const float* g) {                          // Gamma-bar^k accumulator, k < L: layer NL writes, the others add
+      float* p = a.gacc + (k - 1) * a.cstride + cb;
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) {
+        if (L == NL) p[(size_t)b * a.n] = g[b]; else p[(size_t)b * a.n] += g[b];
+      }
+    };
+    if constexpr (L == 1) {
+      tpc_gb<P1, true>(a.kv1, nb, nullptr, Gb);
+    } else if constexpr (L == 2) {
+      float w1[Pat<P2>::DIN], u1[Pat<P1>::DOUT], g1[DENV];
+      tpc_fwd<P2, true>(a.kv2, G[1], nullptr, w1);                   // w_1 = M^2 e_0
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) g1[b] = 0.f;
+      tpc_gb<P1, false>(a.kv1, nb, w1, g1);
+      put(1, g1);
+      tpc_tr<P1>(a.kv1, G[0], nb, u1);                               // u_1 = M^1T n-bar
+      tpc_gb<P2, true>(a.kv2, u1, nullptr, Gb);
+    } else {
+      float w2[Pat<P3>::DIN], w1[Pat<P2>::DIN], u1[Pat<P1>::DOUT], u2[Pat<P2>::DOUT], g[DENV];
+      tpc_fwd<P3, true>(a.kv3, G[2], nullptr, w2);                   // w_2 = M^3 e_0
+      tpc_fwd<P2, false>(a.kv2, G[1], w2, w1);                       // w_1 = M^2 w_2
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) g[b] = 0.f;
+      tpc_gb<P1, false>(a.kv1, nb, w1, g);
+      put(1, g);
+      tpc_tr<P1>(a.kv1, G[0], nb, u1);
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) g[b] = 0.f;
+      tpc_gb<P2, false>(a.kv2, u1, w2, g);
+      put(2, g);
+      tpc_tr<P2>(a.kv2, G[1], u1, u2);
+      tpc_gb<P3, true>(a.kv3, u2, nullptr, Gb);
+    }
+  }
+
+  // ---- pass B: omega-bar^L_e and the environment part of Y-bar_e (4 edges in flight) --------------------------------------------------
+#pragma unroll
+  for (int b = 0; b < DENV; ++b) Gb[b] *= a.c_env;
+  for (int64_t e = e0; e < e1; e += 4) {
+    float om[4][NLV];
+    TpcBatch<DENV> yb;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int64_t ee = (e + i < e1) ? e + i : e1 - 1;
+#pragma unroll
+      for (int l = 0; l < NLV; ++l) om[i][l] = a.om[ee * a.ldo + l * a.n + nn];
+    }
+    yb.load_y(a.Y, e, e1, lane);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      float ob[NLV], pp[DENV];
+#pragma unroll
+      for (int l = 0; l < NLV; ++l) ob[l] = 0.f;
+#pragma unroll
+      for (int b = 0; b < DENV; ++b) {
+        ob[l_of(b)] = fmaf(Gb[b], yb.y(i, b), ob[l_of(b)]);
+        pp[b] = om[i][l_of(b)] * Gb[b];
+      }
+      if (e + i < e1) {
+#pragma unroll
+        for (int l = 0; l < NLV; ++l) a.ombar[(e + i) * a.ldob + l * a.n + nn] = ob[l];
+        tp_ybar_rows<DENV, true>(YbL + (e + i) * DENV, pp, 0, DENV, lane);
+      }
+    }
+  }
+}
+
+// ---- host side ---------------------------------------------------------------------------------------------
+template <int LM, int NL>
+int tpc_fill(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* w0, int ldw, TPC<LM, NL>& a) {
+  a.rowa = (const int64_t*)w.rowa.p; a.nc = nc; a.n = m->n; a.c_env = m->c_env; a.rev = al_next_rev(m);
+  a.Y = (const float*)w.Y.p; a.ldy = m->ldY; a.w0 = w0; a.ldw = ldw; a.om = om; a.ldo = ldo;
+  a.gam = (float*)w.tpc_gam.p; a.nvec = (float*)w.tpc_nvec.p; a.gacc = (float*)w.tpc_gacc.p;
+  a.cstride = (int64_t)w.cap_centers * m->Denv * m->n;
+  for (int k = 0; k < TPC_MAXL; ++k) { a.sb[k] = w.sb_ptr[k]; a.lds[k] = w.sb_ld[k]; }
+  a.Ybar = (float*)w.Ybar.p; a.ybar_pstride = (int64_t)w.cap_edges * m->Denv;
+  { int part[AL_MAX_LAYERS + 1]; al_ybar_layout(m, part); a.ybar_part0 = part[0]; a.ybar_partL = part[L]; }
+  const int want[3] = {TPC<LM, NL>::NNZ1, TPC<LM, NL>::NNZ2, TPC<LM, NL>::NNZ3};
+  float* dst[3] = {a.kv1, a.kv2, a.kv3};
+  for (int k = 0; k < NL; ++k) {
+    const TPLayerHost& h = m->tp_host[k];
+    if ((int)h.dp_val.size() != want[k]) { al_set_error(m, "tpc: pattern size mismatch"); return ALLEGRO_ERR_BAD_ARG; }
+    memcpy(dst[k], h.dp_val.data(), sizeof(float) * want[k]);
+  }
+  return ALLEGRO_OK;
+}
+
+template <int LM, int NL, int L>
+int tpc_launch_fwd(allegro_model* m, Work& w, int nc, const float* om, int ldo, const float* w0, int ldw, float* xs, int ldx) {
+  TPC<LM, NL> a{};
+  AL_CHECK((tpc_fill<LM, NL>(m, w, L, nc, om, ldo, w0, ldw, a)));
+  a.xs = xs; a.ldx = ldx;
+  constexpr int WPB = 4;
+  const int64_t warps = (int64_t)nc * (m->n / 32);
+  k_tpc_fwd<LM, NL, L, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, 0, m->stream>>>(a);
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
+}
+
+template <int LM, int NL, int L>
+int tpc_launch_bwd(allegro_model* m, Work& w, int nc, const float* om, int ldo, const float* w0, int ldw, float* ombar, int ldob,
+                   float* w0bar) {
+  TPC<LM, NL> a{};
+  AL_CHECK((tpc_fill<LM, NL>(m, w, L, nc, om, ldo, w0, ldw, a)));
+  a.ombar = ombar; a.ldob = ldob; a.w0bar = w0bar;
+  constexpr int WPB = 4;
+  const int64_t warps = (int64_t)nc * (m->n / 32);
+  k_tpc_bwd<LM, NL, L, WPB><<<(unsigned)((warps + WPB - 1) / WPB), WPB * 32, 0, m->stream>>>(a);
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
+}
+

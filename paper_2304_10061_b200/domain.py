@@ -185,12 +185,23 @@ class Domain:
     # ---- forward exchange ----------------------------------------------------------------------------------------
     def pack_forward(self) -> torch.Tensor:
         """Rows [x, y, z, species] of the ghosts this rank provides, grouped by destination."""
+        if self._on_device():          # one library kernel (allegro_halo_pack) instead of gather + add + cast + cat
+            return self.model.halo_pack(self.pos, self.species, self.send_idx, self.send_shift)
         p = self.pos[self.send_idx] + self.send_shift
         return torch.cat([p, self.species[self.send_idx].to(p.dtype)[:, None]], dim=1)
+
+    def _on_device(self) -> bool:
+        """The per-atom halo work runs in the library's kernels whenever the domain's arrays are CUDA tensors and a model is
+        bound; the torch expressions below are the same operations for the CPU (gloo) tests of the exchange logic."""
+        return self.model is not None and self.pos.is_cuda and self.species.dtype == torch.int32
 
     def local_system(self, ghosts: torch.Tensor):
         """Local atoms followed by the received ghosts, in a frame whose periodic box cannot connect opposite faces."""
         n_local = self.pos.shape[0]
+        if self._on_device():          # allegro_halo_assemble: concatenate, shift into the local frame, cast the species
+            origin_h = self.lo - self.halo
+            pos_all, sp_all = self.model.halo_assemble(self.pos, self.species, ghosts.contiguous(), origin_h)
+            return pos_all, sp_all, n_local, (self.hi - self.lo) + 3.0 * self.halo + 1.0
         pos_all = torch.cat([self.pos, ghosts[:, :3]], dim=0)
         sp_all = torch.cat([self.species, ghosts[:, 3].round().to(self.species.dtype)], dim=0)
         origin = torch.as_tensor(self.lo - self.halo, dtype=pos_all.dtype, device=pos_all.device)
@@ -212,6 +223,8 @@ class Domain:
     # ---- reverse exchange ------------------------------------------------------------------------------------------
     def finish(self, f_all: torch.Tensor, returned: torch.Tensor) -> torch.Tensor:
         """Local part of the forces plus what the other domains accumulated on the ghosts this rank provided."""
+        if self._on_device() and f_all.is_cuda:          # allegro_halo_accumulate
+            return self.model.halo_accumulate(f_all.contiguous(), self.pos.shape[0], self.send_idx, returned.contiguous())
         f = f_all[: self.pos.shape[0]].clone()
         if returned.numel():
             f.index_add_(0, self.send_idx, returned)

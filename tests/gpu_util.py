@@ -6,7 +6,7 @@ from oracle import allegro_oracle as O
 from synthetic import make_blob
 
 
-def make_both(cfg, precision=0, sigma=None, chunk_edges=None):
+def make_both(cfg, precision=0, sigma=None, chunk_edges=None, tensor_track=0):
     hp = cfg.hp
     chp = P.hparams_from(hp, precision)
     fan_gpu = P.path_fan(chp)                       # product side: from the C library
@@ -17,6 +17,8 @@ def make_both(cfg, precision=0, sigma=None, chunk_edges=None):
     assert len(sig) == hp.n_species
     blob = make_blob(hp, fan_gpu, sig, cfg.mu(), cfg.weight_seed)
     model = P.Allegro(chp, blob, chunk_edges=chunk_edges)
+    if tensor_track:
+        model.set_tensor_track(tensor_track)          # 1: per-edge product kernels instead of the per-centre contraction
     if getattr(hp, "r_cut_pair", None) is not None:
         model.set_pair_cutoffs(hp.r_cut_pair)
     if getattr(hp, "bessel_freq_pair", None) is not None:

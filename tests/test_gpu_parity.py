@@ -85,6 +85,29 @@ def test_energy_forces_fp32(ci, n, precision):
     _check_EF(got, want, n, f"cfg{ci}")
 
 
+# the per-edge product kernels (allegro_set_tensor_track 1): FFMA kernels in the fp32 modes, mma.sync TF32 kernels for l_max = 3
+# in TF32 mode (NEXT-2, forward and backward); the default everywhere else in this suite is the per-centre contraction
+@pytest.mark.parametrize("ci,n,precision", [(0, 192, 0), (1, 1536, 0), (1, 1536, 1), (2, 3000, 1), (4, 1200, 0), (4, 1200, 1), (4, 1200, 3)])
+def test_per_edge_product_kernels(ci, n, precision):
+    cfg = scaled_config(ci, n)
+    pos, sp, box = make_system(cfg)
+    model, oracle = make_both(cfg, precision=precision, tensor_track=1)
+    (E, Ea, F), nb = gpu_eval(model, pos, sp, box)
+    E0, Ea0, F0 = O.energy_forces(oracle, pos, sp, box, O.neighbor_list(pos, box, cfg.hp.r_cut))
+    if precision in (0, 3):
+        _check_EF((E, Ea, F), (E0, Ea0, F0), n, f"per-edge products cfg{ci} prec{precision}")
+    else:
+        mu = np.array(cfg.mu())[sp]
+        assert abs(E - E0) <= 2e-3 * np.abs(Ea0 - mu).sum()
+        assert np.abs(F - F0).max() <= 2e-3 * np.abs(F0).max()
+        assert np.linalg.norm(F - F0) <= 2e-3 * np.linalg.norm(F0)
+    # and both tensor-track implementations compute the same function
+    model0, _ = make_both(cfg, precision=precision)
+    (E1, Ea1, F1), _ = gpu_eval(model0, pos, sp, box)
+    tol = 2e-5 if precision in (0, 3) else 4e-3
+    assert np.abs(F1 - F).max() <= tol * max(1.0, np.abs(F0).max()) and abs(E1 - E) / n <= (2e-6 if precision in (0, 3) else 1e-3)
+
+
 def test_intermediates_cfg0():
     cfg = scaled_config(0, 192)
     pos, sp, box = make_system(cfg)
