@@ -570,10 +570,9 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
   // A/B ring depths 4/3; 6/2 and 3/3 measured within 1 % of it (the rings are not the limiter)
-  static const int dev_cfg = getenv("B200_DEV_GEMM") ? atoi(getenv("B200_DEV_GEMM")) : 0;
-  if (dev_cfg == 1) { GEMM_DISPATCH(6, 3, 8, false) }
-  else if (dev_cfg == 2) { GEMM_DISPATCH(5, 3, 12, false) }
-  else { GEMM_DISPATCH(4, 3, 16, false) }
+  // round 2, config 2 (GEMM group per step): 4 / 3 / 16 warps 32.5 ms, 5 / 3 / 12 warps 33.9 ms, 6 / 3 / 8 warps 37.3 ms -- the epilogue
+  // warps, not the ring depth, set the pace (DESIGN.md section 6 has the skip-experiments that show what binds the kernel)
+  GEMM_DISPATCH(4, 3, 16, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
