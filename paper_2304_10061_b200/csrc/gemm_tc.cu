@@ -570,8 +570,8 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
   // A/B ring depths 4/3; 6/2 and 3/3 measured within 1 % of it (the rings are not the limiter)
-  // round 2, config 2 (GEMM group per step): 4 / 3 / 16 warps 32.5 ms, 5 / 3 / 12 warps 33.9 ms, 6 / 3 / 8 warps 37.3 ms -- the epilogue
-  // warps, not the ring depth, set the pace (DESIGN.md section 6 has the skip-experiments that show what binds the kernel)
+  // round 2, config 2 (GEMM group per step), A stages / B stages / epilogue warps: 4/3/16 32.5 ms, 5/3/12 33.9 ms, 6/3/8 37.3 ms,
+  // 6/2/16 35.4 ms; L2 prefetch of the A tiles 4-12 k-blocks ahead (cp.async.bulk.prefetch.tensor) 33.3 ms
   GEMM_DISPATCH(4, 3, 16, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());

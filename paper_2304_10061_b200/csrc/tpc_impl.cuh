@@ -9,7 +9,7 @@
 // Contracting the per-centre operators FIRST leaves one D_0-long dot product per edge, channel and layer, instead of a
 // D_{L-1} x D_L product per edge: V^L_e is never formed, nothing of size [edges, D, n] is read or written, and the work that
 // involves the sparse tensors K^k happens once per centre.  It is the same function up to the order of the fp32 sums
-// (the fp64 oracle follows the paper's order, layer by layer and edge by edge).  Matrix-free: M^k is never built either;
+// (the fp64 reference of the test suite follows the paper's order, layer by layer and edge by edge).  Matrix-free: M^k is never built either;
 // the three trilinear forms of K^k(Gamma^k) that are needed run straight off the compile-time sparsity pattern
 // (tp2_patterns.inc) with every operand in registers:
 //     fwd :  y[a]  = sum K[a,b,c] Gamma[b] x[c]      (y = M x)
