@@ -120,9 +120,17 @@ __device__ __forceinline__ void ep_st4(float* p, const float4 v) {
 }
 
 // tensor-core modes: fast-math sigmoid (ex2.approx + rcp.approx), error ~1e-7 << TF32 rounding
-__device__ __forceinline__ float silu_f(float z) { return __fdividef(z, 1.0f + __expf(-z)); }
+// sigmoid = rcp.approx(1 + ex2.approx(-z log2 e)): the two MUFU operations and nothing else (__fdividef adds a range test and
+// two scaling multiplies per element that 1 + e^-z in [1, inf] never needs)
+__device__ __forceinline__ float sigm_f(float z) {
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * -1.4426950408889634f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+  return r;
+}
+__device__ __forceinline__ float silu_f(float z) { return z * sigm_f(z); }
 __device__ __forceinline__ float dsilu_f(float z) {
-  float s = __fdividef(1.0f, 1.0f + __expf(-z));
+  float s = sigm_f(z);
   return s * fmaf(z, 1.0f - s, 1.0f);
 }
 
@@ -309,8 +317,16 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         // the column vector of the rank-1 / energy epilogues is the same for all 32 rows of the chunk: one load per chunk
         float4 w3 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R) w3 = *reinterpret_cast<const float4*>(g.aux3 + (col_ok ? col : 0));
+        // row pointers of this lane for the chunk (row rbase + rsub, column col); rows advance by 4 per visit
+        const int row0 = rbase + rsub;
+        const size_t cco = col_ok ? (size_t)col : 0;
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
+        const int rowh = row0 + h * 16;
+        const float* p1 = need1 ? g.aux1 + (size_t)rowh * g.ld1 + cco : nullptr;
+        const float* p2 = need2 ? g.aux2 + (size_t)rowh * g.ld2 + cco : nullptr;
+        const float* pz = PREP ? g.zp + (size_t)rowh * g.ldzp + cco : nullptr;
+        const size_t st1 = (size_t)4 * g.ld1, st2 = (size_t)4 * g.ld2, stz = (size_t)4 * g.ldzp;
         float4 ax1[4], ax2[4], ax3[4];
         // per-row scalars (u, sigma, u of the prep stage) are prefetched with the aux rows: loaded at their point of use they
         // were the top stall of the EPI_LATENT_LAST epilogue (ncu: long_scoreboard on the first multiply by u)
@@ -325,10 +341,14 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           ru[ii] = need_u ? g.u[rowc] : 0.f;
           rs[ii] = (EPI == EPI_LATENT_LAST) ? g.sig[rowc] : 0.f;
           rp[ii] = PREP ? g.pu[rowc] : 0.f;
-          ax1[ii] = (need1 && ok) ? ep_ld4(g.aux1 + (size_t)row * g.ld1 + col) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax2[ii] = (need2 && ok) ? ep_ld4(g.aux2 + (size_t)row * g.ld2 + col) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax3[ii] = (PREP && ok) ? ep_ld4(g.zp + (size_t)row * g.ldzp + col) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax1[ii] = (need1 && ok) ? ep_ld4(p1 + ii * st1) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax2[ii] = (need2 && ok) ? ep_ld4(p2 + ii * st2) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax3[ii] = (PREP && ok) ? ep_ld4(pz + ii * stz) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+        float* qo = g.out2 ? g.out2 + (size_t)rowh * g.ldo2 + cco : nullptr;
+        float* qc = g.C ? g.C + (size_t)rowh * g.ldc + cco : nullptr;
+        float* qz = PREP ? g.zbp + (size_t)rowh * g.ldzbp + cco : nullptr;
+        const size_t sto = (size_t)4 * g.ldo2, stc = (size_t)4 * g.ldc, stzb = (size_t)4 * g.ldzbp;
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
           const int i = h * 4 + ii;
@@ -349,7 +369,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
               // one sigmoid serves silu and silu'
-              const float sgm = __fdividef(1.0f, 1.0f + __expf(-v[j]));
+              const float sgm = sigm_f(v[j]);
               const float sl = v[j] * sgm;
               o[j] = fmaf(g.c0, xo[j], cu * sl);
               zb[j] = cus * we[j] * (sgm * fmaf(v[j], 1.0f - sgm, 1.0f));
@@ -368,8 +388,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               ep += __shfl_xor_sync(0xffffffffu, ep, off);
             }
             if (ok) {
-              ep_st4(g.out2 + (size_t)row * g.ldo2 + col, make_float4(zb[0], zb[1], zb[2], zb[3]));
-              if (g.C) ep_st4(g.C + (size_t)row * g.ldc + col, make_float4(o[0], o[1], o[2], o[3]));
+              ep_st4(qo + ii * sto, make_float4(zb[0], zb[1], zb[2], zb[3]));
+              if (g.C) ep_st4(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]));
               if ((lane & 7) == 0) {
                 const int64_t p = (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.c1 * sg * up;
@@ -398,7 +418,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             float zb[4], up = 0.f;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-              const float sgm = __fdividef(1.0f, 1.0f + __expf(-zz[j]));
+              const float sgm = sigm_f(zz[j]);
               up = fmaf(o[j], zz[j] * sgm, up);
               zb[j] = cu * o[j] * (sgm * fmaf(zz[j], 1.0f - sgm, 1.0f));
             }
@@ -406,8 +426,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
             for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
             if (ok) {
-              ep_st4(g.zbp + (size_t)row * g.ldzbp + col, make_float4(zb[0], zb[1], zb[2], zb[3]));
-              if (g.C) ep_st4(g.C + (size_t)row * g.ldc + col, make_float4(o[0], o[1], o[2], o[3]));
+              ep_st4(qz + ii * stzb, make_float4(zb[0], zb[1], zb[2], zb[3]));
+              if (g.C) ep_st4(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]));
               if ((lane & 7) == 0) {
                 const int64_t p = g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.cp * up;
@@ -419,7 +439,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               case EPI_SILU_BOTH:
               case EPI_SILU_U:
               case EPI_LATENT: {
-                ep_st4(g.out2 + (size_t)row * g.ldo2 + col, make_float4(v[0], v[1], v[2], v[3]));
+                ep_st4(qo + ii * sto, make_float4(v[0], v[1], v[2], v[3]));
                 float us = (EPI == EPI_SILU_BOTH) ? 1.0f : ru[ii];
                 if (EPI == EPI_LATENT) {
                   float4 x = AUX1(i);
@@ -454,7 +474,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
                 for (int j = 0; j < 4; ++j) o[j] = v[j];
             }
-            ep_st4(g.C + (size_t)row * g.ldc + col, make_float4(o[0], o[1], o[2], o[3]));
+            ep_st4(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]));
           }
         }
         }   // halves
@@ -571,7 +591,9 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
   // A/B ring depths 4/3; 6/2 and 3/3 measured within 1 % of it (the rings are not the limiter)
   // round 2, config 2 (GEMM group per step), A stages / B stages / epilogue warps: 4/3/16 32.5 ms, 5/3/12 33.9 ms, 6/3/8 37.3 ms,
-  // 6/2/16 35.4 ms; L2 prefetch of the A tiles 4-12 k-blocks ahead (cp.async.bulk.prefetch.tensor) 33.3 ms
+  // 6/2/16 35.4 ms; L2 prefetch of the A tiles 4-12 k-blocks ahead (cp.async.bulk.prefetch.tensor) 33.3 ms; 2-CTA clusters with
+  // every B (weight) stage loaded half by each CTA and multicast to both (L2 -> shared B traffic halved) 32.8 ms: correct, and
+  // no faster -- dropped
   GEMM_DISPATCH(4, 3, 16, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
