@@ -61,3 +61,20 @@ def test_product_never_imports_oracle():
     for f in ("oracle/allegro_oracle.py",):
         txt = open(os.path.join(ROOT, f)).read()
         assert "import paper_2304_10061_b200" not in txt and "from paper_2304_10061_b200" not in txt
+
+
+def test_precision_2_is_refused_not_aliased():
+    """BF16-operand MLPs are not built: allegro_create must say so (ALLEGRO_ERR_UNIMPLEMENTED = -7) instead of running
+    another mode under that name.  The hyper-parameter check runs before any device is touched, so this needs no GPU."""
+    import ctypes as C
+    import paper_2304_10061_b200 as P
+    from synthetic import CONFIGS
+    lib = P.load_library()
+    hp = P.hparams_from(CONFIGS[0].hp, 2)
+    h = C.c_void_p(None)
+    blob = C.create_string_buffer(16)
+    rc = lib.allegro_create(C.byref(hp), blob, 16, C.byref(h))
+    assert rc == -7 and not h
+    assert b"precision 2" in lib.allegro_last_error(None)
+    n = C.c_size_t(0)
+    assert lib.allegro_blob_size(C.byref(hp), C.byref(n)) == -7
