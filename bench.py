@@ -124,7 +124,7 @@ def tp_survey_bytes_per_edge(hp):
     return {"tp_fwd": 4.0 * fwd, "tp_bwd": 4.0 * bwd}
 
 
-DTYPE = {0: "f32 (3xtf32)", 1: "tf32", 3: "f32"}      # precision 2 (BF16 operands) is refused by allegro_create
+DTYPE = {0: "f32 (3xtf32)", 1: "tf32", 2: "bf16 operands (fp32 accumulate)", 3: "f32", 4: "fp16 operands (fp32 accumulate)"}
 
 
 def tp_flops_per_edge(hp):
@@ -300,8 +300,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--repeats", type=int, default=3, help="timed repeats of K steps each; the median is reported")
     ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--precision", type=int, default=1, choices=[0, 1, 3],
-                    help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores (the paper's scheme), 3 fp32 FFMA")
+    ap.add_argument("--precision", type=int, default=1, choices=[0, 1, 2, 3, 4],
+                    help="0 fp32 (3xTF32 on tensor cores), 1 TF32 tensor cores (the paper's scheme, the contract line), 3 fp32 FFMA, "
+                         "2 / 4 bf16 / fp16 operand storage for the MLPs (fp32 accumulate)")
     ap.add_argument("--no-peak-probe", action="store_true", help="skip the TF32 / FFMA peak measurements (~10 s)")
     ap.add_argument("--drift-steps", type=int, default=0,
                     help="also run this many NVE steps from the initial state and report the drift of E_pot + E_kin "
@@ -339,13 +340,13 @@ def main():
         pos, sp, box = make_system(cfg)
         n_c = {0: 192, 1: 3072, 2: 512, 3: 512, 4: 256}[cfg.index]
         run, n_c, cores = oracle_sample(cfg, pos, sp, box, n_c)
-        for _ in range(min(W, 3)):
+        for _ in range(W):
             run()
         t = sum(run() for _ in range(K))
         val = n_c * K / t
         print(json.dumps({
             "impl": "reference", "metric": metric, "value": val, "unit": unit, "n_gpus": args.gpus, "steps": K,
-            "warmup": min(W, 3), "ms_per_step": 1e3 * t / K, "higher_is_better": True, "scaling": "weak",
+            "warmup": W, "ms_per_step": 1e3 * t / K, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload, "n_atoms": int(pos.shape[0]), "sample": f"{n_c} contiguous centres per step"},
             "cpu_baseline": {"value": val, "unit": unit, "cores": cores, "kind": "oracle",
@@ -504,6 +505,10 @@ def main():
         else:
             peak = nsm * FFMA_LANES_PER_SM * 2 * pk["sm_max_mhz"] * 1e6 / 1e12
             peak_note = f"{nsm} SMs x {FFMA_LANES_PER_SM} FFMA lanes x 2 x {pk['sm_max_mhz']} MHz (not probed)"
+    elif args.precision in (2, 4):
+        bound = "tensor"
+        peak = pk["bf16_sustained"] if long_region else pk["bf16_burst"]
+        peak_note = f"16-bit dense matmul {which} {peak} TFLOP/s (MEASURED_PEAKS.json, {pk['src']}; fp16 and bf16 share the rate)"
     else:
         bound = "tensor"
         div = 3.0 if args.precision == 0 else 1.0      # 3xTF32: three TF32 MMAs per algorithmic MAC
@@ -539,7 +544,8 @@ def main():
         if tj:
             traffic, traffic_src = tj["gemm_dram_bytes_per_launch"], tj.get("source")
     kname = {0: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., SPLIT> (3xTF32)", 1: "MLP GEMM group (fwd+bwd), k_gemm_tf32",
-             3: "MLP GEMM group (fwd+bwd), k_gemm_simt"}[args.precision]
+             2: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., H16> (bf16 operands)", 3: "MLP GEMM group (fwd+bwd), k_gemm_simt",
+             4: "MLP GEMM group (fwd+bwd), k_gemm_tf32<.., H16> (fp16 operands)"}[args.precision]
     per_launch = K / max(gemm_n, 1)
     roofline = {"bound": top["bound"], "kernel": kname,
                 "achieved": top["achieved"], "peak": top["peak"], "unit": top["unit"], "frac": top["frac"],

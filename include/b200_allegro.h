@@ -58,8 +58,13 @@ typedef struct {
   double resid_alpha[8];    /* per layer residual mixing coefficient (S7) */
   int32_t precision;        /* MLP GEMM arithmetic (accumulation is fp32 in all modes):
                                0 fp32 on the tensor cores (3xTF32 split operands, meets the fp32 tolerances),
-                               1 TF32 tensor cores (the paper's scheme), 2 BF16 operands: NOT BUILT, allegro_create returns
-                               ALLEGRO_ERR_UNIMPLEMENTED, 3 fp32 on the FFMA pipes (slowest, most accurate) */
+                               1 TF32 tensor cores (the paper's scheme), 3 fp32 on the FFMA pipes (slowest, most accurate),
+                               2 / 4 16-bit operand MLPs: every tensor that only the MLP GEMMs and their epilogues touch
+                               (activations, pre-activations, latents x^L, their gradients) and the weights are stored as
+                               bfloat16 (2) or IEEE fp16 (4), tcgen05 kind::f16, fp32 accumulation, fp32 tensor track and fp64
+                               final stage as in the other modes; needs >= 2 two-body layers, d and n_tensor multiples of 32, a
+                               first latent width that is a multiple of 64 and a model the contracted tensor track covers
+                               (else ALLEGRO_ERR_BAD_HPARAMS at create / ALLEGRO_ERR_UNIMPLEMENTED at the first compute) */
   int64_t max_atoms, max_edges; /* capacity hints, 0 = grow on demand (+5 %) */
 } allegro_hparams;
 

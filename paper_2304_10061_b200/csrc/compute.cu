@@ -18,6 +18,10 @@ static int work_reserve(allegro_model* m, const allegro_nbr* nb, int64_t N) {
   int d = m->d, n = m->n, nA = m->nA, NL = m->NL;
   const bool tpc = tpc_eligible(m);          // tensor track contracted per centre: no [edges, D, n] tensors at all
   const bool kcat = al_gemm_supports_kcat(m) && (hp.latent_dims[0] % 32 == 0);
+  if (m->hfmt >= 0 && (!tpc || !kcat)) {
+    al_set_error(m, "16-bit operand modes need the per-centre-contracted tensor track (generated CG patterns, n % 32 == 0, <= 3 layers)");
+    return ALLEGRO_ERR_UNIMPLEMENTED;
+  }
   if (M > w.cap_edges || w.XS.empty()) {
     auto R = [&](DevBuf& b, size_t floats) { return al_reserve(m, b, floats * 4 + 64); };
     AL_CHECK(R(w.ei, M)); AL_CHECK(R(w.ej, M)); AL_CHECK(R(w.geo, 4 * M)); AL_CHECK(R(w.u, M)); AL_CHECK(R(w.du, M)); AL_CHECK(R(w.sig, M));
@@ -92,8 +96,10 @@ void al_work_free(allegro_model* m) {
   m->work = nullptr;
 }
 
-static GemmArgs mk(const float* A, int lda, const Dense& D, bool transposed_weight, float* C, int ldc, int m_cap,
-                   const int* m_ptr, int epi) {
+// io16 (precision 2 only): which epilogue tensors of this launch are stored as 16-bit (IO16_* below = gemm_tc.cu's bits)
+enum { IO16_C = 1, IO16_OUT2 = 2, IO16_ZBP = 4, IO16_AUX1 = 8, IO16_AUX2 = 16, IO16_ZP = 32 };
+static GemmArgs mk(const allegro_model* m, const float* A, int lda, const Dense& D, bool transposed_weight, float* C, int ldc, int m_cap,
+                   const int* m_ptr, int epi, int io16 = 0) {
   // transposed_weight = false: forward  Y = X W   -> Bt = Wt [fo][fi], N = fo, K = fi
   // transposed_weight = true : backward dX = dY W^T -> Bt = W  [fi][fo], N = fi, K = fo
   GemmArgs g{};
@@ -101,6 +107,7 @@ static GemmArgs mk(const float* A, int lda, const Dense& D, bool transposed_weig
   if (!transposed_weight) { g.Bt = D.Wt; g.Bt_hi = D.Wt_hi; g.Bt_lo = D.Wt_lo; g.ldb = D.fi; g.N = D.fo; g.K = D.fi; }
   else { g.Bt = D.W; g.Bt_hi = D.W_hi; g.Bt_lo = D.W_lo; g.ldb = D.fo; g.N = D.fi; g.K = D.fo; }
   g.C = C; g.ldc = ldc; g.m_cap = m_cap; g.m_ptr = m_ptr; g.epi = epi;
+  if (m->hfmt >= 0) { g.Bt16 = transposed_weight ? D.W16 : D.Wt16; g.hfmt = m->hfmt; g.io16 = io16; }
   return g;
 }
 
@@ -118,6 +125,8 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   cudaStream_t st = m->stream;
   const bool fused_last = w.n_eparts > 0;
   const bool tpc = tpc_eligible(m);
+  const bool h16 = m->hfmt >= 0;      // precision 2 / 4: every tensor that only GEMMs and their epilogues touch is 16-bit
+  auto el = [&](void* base, size_t elems) { return (float*)((char*)base + elems * (h16 ? 2 : 4)); };   // element offset
   EdgeGeomArgs ga{};
   ga.pos = pos; ga.species = species; memcpy(ga.box, box, 24); ga.rc = hp.r_cut; ga.p = hp.poly_p; ga.NB = m->NB;
   ga.lmax = m->lmax; ga.row_ptr = (const int64_t*)nb->row_ptr.p; ga.j = (const int32_t*)nb->j.p;
@@ -133,21 +142,21 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
   AL_CHECK(k_launch_twobody0(m, w, species, m->twobody[0], ntb == 1, m_cap));
   for (int k = 1; k < ntb; ++k) {
     bool last = (k == ntb - 1);
-    GemmArgs g = mk((float*)w.tb_a[k - 1].p, hp.twobody_dims[k - 1], m->twobody[k], false,
+    GemmArgs g = mk(m, (float*)w.tb_a[k - 1].p, hp.twobody_dims[k - 1], m->twobody[k], false,
                     last ? (float*)w.XS[0].p : (float*)w.tb_a[k].p, last ? d + n : hp.twobody_dims[k], m_cap, mp,
-                    last ? EPI_SILU_U : EPI_SILU_BOTH);
+                    last ? EPI_SILU_U : EPI_SILU_BOTH, IO16_C | IO16_OUT2);
     g.out2 = (float*)w.tb_z[k].p; g.ldo2 = hp.twobody_dims[k]; g.u = (float*)w.u.p;
     AL_CHECK(al_gemm(m, g));
   }
   // ---- step 4: embedding projections  [w^0 | omega^1] = x^0 [A^0 | A^1] ----------------------------------
-  AL_CHECK(al_gemm(m, mk((float*)w.XS[0].p, d + n, m->emb01, false, (float*)w.WE.p, 2 * nA, m_cap, mp, EPI_PLAIN)));
+  AL_CHECK(al_gemm(m, mk(m, (float*)w.XS[0].p, d + n, m->emb01, false, (float*)w.WE.p, 2 * nA, m_cap, mp, EPI_PLAIN)));
   // ---- steps 5-8: layers -----------------------------------------------------------------------------------
   for (int L = 1; L <= NL; ++L) {
     const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
     int ldo = (L == 1) ? 2 * nA : nA;
     const float* Vin = (L == 1 || tpc) ? nullptr : (float*)w.T[L - 1].p;
     float* Tout = (L < NL && !tpc) ? (float*)w.T[L].p : nullptr;
-    AL_CHECK(k_launch_tp_fwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, Tout, (float*)w.XS[L - 1].p + d, d + n));
+    AL_CHECK(k_launch_tp_fwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, Tout, el(w.XS[L - 1].p, d), d + n));
     for (int k = 0; k < nlat; ++k) {
       bool last = (k == nlat - 1);
       const float* A = (k == 0) ? (float*)w.XS[L - 1].p : (float*)w.lat_a[L - 1][k - 1].p;
@@ -156,13 +165,15 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       if (!last) { C = (float*)w.lat_a[L - 1][k].p; ldc = hp.latent_dims[k]; }
       else if (L < NL) { C = (float*)w.XS[L].p; ldc = d + n; }
       else { C = (float*)w.XF.p; ldc = d; }
-      GemmArgs g = mk(A, lda, m->latent[L - 1][k], false, C, ldc, m_cap, mp, last ? EPI_LATENT : EPI_SILU_BOTH);
+      GemmArgs g = mk(m, A, lda, m->latent[L - 1][k], false, C, ldc, m_cap, mp, last ? EPI_LATENT : EPI_SILU_BOTH,
+                      IO16_C | IO16_OUT2 | IO16_AUX1);
       g.out2 = (float*)w.lat_z[L - 1][k].p; g.ldo2 = hp.latent_dims[k];
       g.u = (float*)w.u.p; g.aux1 = (float*)w.XS[L - 1].p; g.ld1 = d + n; g.c0 = m->c_old[L - 1]; g.c1 = m->c_new[L - 1];
       if (last && L == NL && fused_last) {
         // x^{NL} is consumed in the epilogue: edge-energy partials, z-bar^{NL} (in place of z) and u-bar partials
         g.epi = EPI_LATENT_LAST;
         if (!m->debug_keep) g.C = nullptr;
+        g.io16 &= ~IO16_C;                         // the debug tap of x^{NL} stays fp32
         g.out2 = (float*)w.ZB0.p; g.ldo2 = d;
         g.sig = (float*)w.sig.p; g.aux3 = m->w_eff_f; g.w_eff_d = m->w_eff_d;
         g.epart = (double*)w.epart.p; g.upart = (float*)w.ubar.p; g.part_stride = w.cap_edges;
@@ -170,7 +181,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       AL_CHECK(al_gemm(m, g));
     }
     if (L < NL)
-      AL_CHECK(al_gemm(m, mk((float*)w.XS[L].p, d + n, m->emb[L], false, (float*)w.OM[L + 1].p, nA, m_cap, mp, EPI_PLAIN)));
+      AL_CHECK(al_gemm(m, mk(m, (float*)w.XS[L].p, d + n, m->emb[L], false, (float*)w.OM[L + 1].p, nA, m_cap, mp, EPI_PLAIN)));
   }
   // ---- steps 9-10: edge energy, per-atom energy (fp64) -----------------------------------------------------
   AL_CHECK(k_launch_energy(m, w, species, ch.c0, nc, (float*)w.XF.p, e_atom));
@@ -202,7 +213,8 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     if (!zb_ready)
       AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
     for (int k = nlat - 1; k >= 1; --k) {
-      GemmArgs g = mk(zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
+      GemmArgs g = mk(m, zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU,
+                      IO16_C | IO16_AUX1);
       g.aux1 = (float*)w.lat_z[L - 1][k - 1].p; g.ld1 = hp.latent_dims[k - 1];
       AL_CHECK(al_gemm(m, g));
       std::swap(zb, zb_o);
@@ -215,25 +227,25 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     const int sbl = (tpc && kcat) ? n : d + n;
     w.sb_ptr[L - 1] = sbp; w.sb_ld[L - 1] = sbl;
     if (kcat)   // s-bar only: [M, h] x W_lat0[d:, :]^T
-      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->sbar[L - 1], true, sbp, sbl, m_cap, mp, EPI_PLAIN)));
+      AL_CHECK(al_gemm(m, mk(m, zb, hp.latent_dims[0], m->sbar[L - 1], true, sbp, sbl, m_cap, mp, EPI_PLAIN)));
     else
-      AL_CHECK(al_gemm(m, mk(zb, hp.latent_dims[0], m->latent[L - 1][0], true, Gp, d + n, m_cap, mp, EPI_PLAIN)));
+      AL_CHECK(al_gemm(m, mk(m, zb, hp.latent_dims[0], m->latent[L - 1][0], true, Gp, d + n, m_cap, mp, EPI_PLAIN)));
     const float* om = (L == 1) ? (float*)w.WE.p + nA : (float*)w.OM[L].p;
     int ldo = (L == 1) ? 2 * nA : nA;
     const float* Vin = (L == 1 || tpc) ? nullptr : (float*)w.T[L - 1].p;
     int ldob = (L == 1) ? 2 * nA : nA;
-    float* ombar = (L == 1) ? (float*)w.OB.p + nA : (float*)w.OB.p;
+    float* ombar = (L == 1) ? el(w.OB.p, nA) : (float*)w.OB.p;   // (16-bit in the 16-bit modes: the x-bar GEMM's second A operand)
     float* vprev = (vb == vb_a) ? vb_b : vb_a;
     AL_CHECK(k_launch_tp_bwd(m, w, L, nc, om, ldo, Vin, (float*)w.WE.p, 2 * nA, vb, sbp, sbl, vprev, ombar,
                              ldob, (float*)w.OB.p));
     vb = vprev;
-    GemmArgs g = mk((float*)w.OB.p, ldob, (L == 1) ? m->emb01 : m->emb[L - 1], true, xb_o, d, m_cap, mp,
+    GemmArgs g = mk(m, (float*)w.OB.p, ldob, (L == 1) ? m->emb01 : m->emb[L - 1], true, xb_o, d, m_cap, mp,
                     rank1 ? EPI_ADD2R : EPI_ADD2);
     g.aux1 = xb; g.ld1 = d; g.c0 = m->c_old[L - 1]; g.aux2 = Gp; g.ld2 = d + n;
     g.u = (float*)w.sig.p; g.aux3 = m->w_eff_f;
     if (kcat) {
       const int h = hp.latent_dims[0];
-      GemmArgs gc = mk(zb, h, m->xcat[L - 1], true, xb_o, d, m_cap, mp, g.epi);
+      GemmArgs gc = mk(m, zb, h, m->xcat[L - 1], true, xb_o, d, m_cap, mp, g.epi, IO16_C | IO16_AUX1 | IO16_ZP | IO16_ZBP);
       gc.A2 = (float*)w.OB.p; gc.lda2 = ldob; gc.K1 = h;
       gc.aux1 = g.aux1; gc.ld1 = g.ld1; gc.c0 = g.c0; gc.aux2 = nullptr; gc.ld2 = 0; gc.u = g.u; gc.aux3 = g.aux3;
       g = gc;
@@ -260,7 +272,8 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     if (!zb_ready)
       AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.tb_z[ntb - 1].p, d, 1.0f, zb, d, d, m_cap));
     for (int k = ntb - 1; k >= 1; --k) {
-      GemmArgs g = mk(zb, hp.twobody_dims[k], m->twobody[k], true, zb_o, hp.twobody_dims[k - 1], m_cap, mp, EPI_MUL_DSILU);
+      GemmArgs g = mk(m, zb, hp.twobody_dims[k], m->twobody[k], true, zb_o, hp.twobody_dims[k - 1], m_cap, mp, EPI_MUL_DSILU,
+                      IO16_AUX1 | (k > 1 ? IO16_C : 0));   // the last z-bar (read by k_edge_bwd) stays fp32
       g.aux1 = (float*)w.tb_z[k - 1].p; g.ld1 = hp.twobody_dims[k - 1];
       AL_CHECK(al_gemm(m, g));
       std::swap(zb, zb_o);
@@ -543,6 +556,10 @@ extern "C" int allegro_step_nve_host(allegro_model* m, double* pos, double* vel,
 extern "C" int allegro_debug_tensor(allegro_model* m, const char* name, float* out, int64_t* n_floats) {
   if (!m || !name || !out || !n_floats || !m->work) return ALLEGRO_ERR_BAD_ARG;
   Work& w = *m->work;
+  if (m->hfmt >= 0 && name[0] != 'Y' && name[0] != 'u' && name[0] != 'B' && name[0] != 'g' && name[0] != 'e') {
+    al_set_error(m, "debug taps of latent tensors are fp32-only (16-bit operand mode)");
+    return ALLEGRO_ERR_UNIMPLEMENTED;
+  }
   int M = 0;
   AL_CUDA(m, cudaStreamSynchronize(m->stream));
   AL_CUDA(m, cudaMemcpy(&M, w.m_act.p, 4, cudaMemcpyDeviceToHost));

@@ -5,6 +5,7 @@
 #include <cmath>
 
 #include "kernels.h"
+#include "h16.cuh"
 
 namespace {
 // streamed rows (written or read once per step): keep them out of L1
@@ -201,7 +202,7 @@ __global__ void __launch_bounds__(256)
 k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int* __restrict__ ej,
            const int32_t* __restrict__ species, const float* __restrict__ B, const float* __restrict__ u,
            const float* __restrict__ W, int S, int NB, int H, float* __restrict__ z, float* __restrict__ act, int ldact,
-           int scale_u) {
+           int scale_u, int hfmt /* -1: fp32 outputs; 0 / 1: z and act stored as fp16 / bf16 (16-bit operand modes) */) {
   const int M = *m_ptr;
   const int64_t e_base = (int64_t)blockIdx.x * TB0_EDGES;
   if (e_base >= M) return;
@@ -239,9 +240,10 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
         const float b = sB[r][q];   // (zero beyond NB)
         acc.x = fmaf(b, wb[q].x, acc.x); acc.y = fmaf(b, wb[q].y, acc.y); acc.z = fmaf(b, wb[q].z, acc.z); acc.w = fmaf(b, wb[q].w, acc.w);
       }
-      ek_st4(z + e * H + k4, acc);
+      if (hfmt < 0) ek_st4(z + e * H + k4, acc); else h16_store4(z, (size_t)e * H + k4, acc, hfmt);
       const float us = scale_u ? sU[r] : 1.0f;
-      ek_st4(act + e * ldact + k4, make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w)));
+      { const float4 o4 = make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
+        if (hfmt < 0) ek_st4(act + e * ldact + k4, o4); else h16_store4(act, (size_t)e * ldact + k4, o4, hfmt); }
     }
     return;
   }
@@ -257,9 +259,10 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
       float b = sB[r][q];
       acc.x = fmaf(b, w4.x, acc.x); acc.y = fmaf(b, w4.y, acc.y); acc.z = fmaf(b, w4.z, acc.z); acc.w = fmaf(b, w4.w, acc.w);
     }
-    ek_st4(z + e * H + k4, acc);
+    if (hfmt < 0) ek_st4(z + e * H + k4, acc); else h16_store4(z, (size_t)e * H + k4, acc, hfmt);
     const float us = scale_u ? sU[r] : 1.0f;
-    ek_st4(act + e * ldact + k4, make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w)));
+    { const float4 o4 = make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
+        if (hfmt < 0) ek_st4(act + e * ldact + k4, o4); else h16_store4(act, (size_t)e * ldact + k4, o4, hfmt); }
   }
 }
 
@@ -773,7 +776,7 @@ int k_launch_twobody0(allegro_model* m, Work& w, const int32_t* species, const D
   int ld = single ? (m->d + m->n) : L0.fo;
   k_twobody0<<<(m_cap + TB0_EDGES - 1) / TB0_EDGES, 256, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, (int*)w.ej.p, species,
                                                                     (float*)w.B.p, (float*)w.u.p, L0.W, m->S, m->NB, L0.fo,
-                                                                    (float*)w.tb_z[0].p, act, ld, single ? 1 : 0);
+                                                                    (float*)w.tb_z[0].p, act, ld, single ? 1 : 0, m->hfmt);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }

@@ -179,6 +179,7 @@ __global__ void __launch_bounds__(NT) k_gemm_simt(GemmArgs g) {
 }  // namespace
 
 int al_gemm_tc3(allegro_model* m, const GemmArgs& g);  // gemm_tc.cu (tcgen05, 3xTF32 split operands)
+int al_gemm_h16(allegro_model* m, const GemmArgs& g);  // gemm_tc.cu (tcgen05 kind::f16, 16-bit operands: precision 2 / 4)
 int al_gemm_tc_row_parts(int N, bool split);
 
 // precision 0 runs on the tensor cores as 3xTF32; precision 3 runs the plain FFMA kernel below
@@ -202,6 +203,7 @@ int al_gemm(allegro_model* m, const GemmArgs& g) {
     al_set_error(m, "gemm: dimensions must be multiples of 4");
     return ALLEGRO_ERR_BAD_HPARAMS;
   }
+  if (m->hfmt >= 0) return al_gemm_h16(m, g);
   if (!fp32_simt(m)) return (m->hp.precision == 0) ? al_gemm_tc3(m, g) : al_gemm_tc(m, g);
   dim3 grid((g.m_cap + BM - 1) / BM, (g.N + BN - 1) / BN);
   k_gemm_simt<<<grid, NT, 0, m->stream>>>(g);

@@ -9,6 +9,8 @@
 // Warp roles: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM alloc), warps 2.. = epilogue (TMEM
 // lane quarter = warp_id % 4, EPI_WARPS/4 warps per quarter taking alternate 32-column chunks).  Persistent CTAs, static tile schedule, n fastest.
 #include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cstdlib>
 
 #include <map>
@@ -20,8 +22,8 @@
 
 namespace {
 
-#define AUX1(i) ax1[(i) & 3]
-#define AUX2(i) ax2[(i) & 3]
+#define AUX1(i) ep_cvt<H16>(ax1[(i) & 3], h1, g.hfmt)
+#define AUX2(i) ep_cvt<H16>(ax2[(i) & 3], h2, g.hfmt)
 constexpr int BM = 128;          // UMMA M (cta_group::1)
 constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
 constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
@@ -85,6 +87,16 @@ __device__ __forceinline__ void tc_mma_tf32(uint32_t tmem_d, uint64_t da, uint64
       "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
       : "memory");
 }
+__device__ __forceinline__ void tc_mma_f16(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
 __device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t* r) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -110,16 +122,53 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
 }
 
 // epilogue operands are streamed (read or written once per launch): keep them out of L1
-__device__ __forceinline__ float4 ep_ld4(const float* p) {
-  float4 v;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-  return v;
-}
 __device__ __forceinline__ void ep_st4(float* p, const float4 v) {
   asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
 }
 
 // tensor-core modes: fast-math sigmoid (ex2.approx + rcp.approx), error ~1e-7 << TF32 rounding
+// Precision 2 (16-bit operand storage): four consecutive elements = 8 bytes.  fmt 0: IEEE fp16 (10-bit mantissa, as TF32),
+// fmt 1: bfloat16 (7-bit mantissa, fp32 range).  GemmArgs::io16 says which epilogue tensors are stored that way.
+enum { IO16_C = 1, IO16_OUT2 = 2, IO16_ZBP = 4, IO16_AUX1 = 8, IO16_AUX2 = 16, IO16_ZP = 32 };
+__device__ __forceinline__ void ep_st4h(void* p, const float4 v, int fmt) {
+  uint2 o;
+  if (fmt == 0) {
+    __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
+    o.x = *reinterpret_cast<uint32_t*>(&a); o.y = *reinterpret_cast<uint32_t*>(&b);
+  } else {
+    __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+    o.x = *reinterpret_cast<uint32_t*>(&a); o.y = *reinterpret_cast<uint32_t*>(&b);
+  }
+  asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(p), "r"(o.x), "r"(o.y) : "memory");
+}
+// element-size aware versions used by the epilogue: `h` = this tensor is stored as 16-bit (only in H16 kernels).
+// The load returns the raw bits and the conversion happens where the value is used: with the conversion at the load every
+// prefetched aux row waited for its own memory latency (ncu r2m: 58 % long_scoreboard on the PRMT behind each load).
+template <bool H16>
+__device__ __forceinline__ uint4 ep_load(const char* p, bool h) {
+  uint4 v = make_uint4(0u, 0u, 0u, 0u);
+  if (H16 && h) asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
+  else asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+template <bool H16>
+__device__ __forceinline__ float4 ep_cvt(const uint4 v, bool h, int fmt) {
+  if (H16 && h) {
+    if (fmt == 0) {
+      const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
+      const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
+      return make_float4(a.x, a.y, b.x, b.y);
+    }
+    return make_float4(__uint_as_float(v.x << 16), __uint_as_float(v.x & 0xFFFF0000u),
+                       __uint_as_float(v.y << 16), __uint_as_float(v.y & 0xFFFF0000u));
+  }
+  return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
+}
+template <bool H16>
+__device__ __forceinline__ void ep_store(char* p, const float4 v, bool h, int fmt) {
+  if (H16 && h) ep_st4h(p, v, fmt); else ep_st4(reinterpret_cast<float*>(p), v);
+}
+
 // sigmoid = rcp.approx(1 + ex2.approx(-z log2 e)): the two MUFU operations and nothing else (__fdividef adds a range test and
 // two scaling multiplies per element that 1 + e^-z in [1, inf] never needs)
 __device__ __forceinline__ float sigm_f(float z) {
@@ -140,7 +189,9 @@ __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__fl
 
 // EPI (GemmEpi) and PREP (the z-bar / u-bar stage of EPI_ADD2 / EPI_ADD2R) are compile-time: one kernel per epilogue,
 // so the epilogue carries no run-time dispatch, no dead operands and no re-loaded argument fields.
-template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2>
+// H16 (precision 2): A and B operands are 16-bit in HBM (fp16 or bf16, GemmArgs::hfmt), one stage = 64 K-elements (the same
+// 128-byte rows), tcgen05.mma.kind::f16 with fp32 accumulation; the epilogue tensors flagged in GemmArgs::io16 are 16-bit too.
+template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, bool H16 = false>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
             const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
@@ -148,6 +199,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT);
   constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT);
   constexpr int EW0 = SPLIT ? 7 : 3;     // first epilogue warp (warps 3..6 are the splitter in SPLIT mode)
+  constexpr int BKE = H16 ? 2 * BKF : BKF;   // K elements per stage
+  static_assert(!(SPLIT && H16), "3xTF32 and 16-bit operands exclude each other");
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
   // Two independent rings: A (activations, from HBM: deep, AST stages of [A | (A_lo)]) and B (weights, from L2:
@@ -173,7 +226,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   const int M = *g.m_ptr;
   const int num_mt = (M + BM - 1) / BM;
   const int num_tiles = num_mt * ntn;
-  const int num_kb = (g.K + BKF - 1) / BKF;
+  const int num_kb = (g.K + BKE - 1) / BKE;
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < AST; ++s) { mbar_init(&fullA[s], 1); mbar_init(&emptyA[s], 1); mbar_init(&readyA[s], 4); }
@@ -194,15 +247,15 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // ===== TMA producer, A ring =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      const int kb1 = g.A2 ? g.K1 / BKF : num_kb;   // k-blocks [kb1, num_kb) come from the second activation tensor
+      const int kb1 = g.A2 ? g.K1 / BKE : num_kb;   // k-blocks [kb1, num_kb) come from the second activation tensor
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         int mt = tile / ntn;
         if (g.rev) mt = num_mt - 1 - mt;
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyA[stage], phase ^ 1);
           mbar_expect_tx(&fullA[stage], A_STAGE_BYTES);
-          if (kb < kb1) tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKF, mt * BM);
-          else tma_load_2d(sA(stage), &tmA2, &fullA[stage], (kb - kb1) * BKF, mt * BM);
+          if (kb < kb1) tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKE, mt * BM);
+          else tma_load_2d(sA(stage), &tmA2, &fullA[stage], (kb - kb1) * BKE, mt * BM);
           if (++stage == AST) { stage = 0; phase ^= 1; }
         }
       }
@@ -217,8 +270,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyB[stage], phase ^ 1);
           mbar_expect_tx(&fullB[stage], bytes);
-          tma_load_2d(sB(stage), &tmB, &fullB[stage], kb * BKF, nt * BN);
-          if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &fullB[stage], kb * BKF, nt * BN);
+          tma_load_2d(sB(stage), &tmB, &fullB[stage], kb * BKE, nt * BN);
+          if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &fullB[stage], kb * BKE, nt * BN);
           if (++stage == BST) { stage = 0; phase ^= 1; }
         }
       }
@@ -227,7 +280,9 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // ===== MMA issuer =====
     if (lane == 0) {
       // instruction descriptor: D=f32, A=B=tf32, K-major both, N>>3, M>>4
-      const uint32_t idesc = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+      // (A / B format field: 2 = tf32 for kind::tf32; kind::f16: 0 = f16, 1 = bf16)
+      const uint32_t ofmt = H16 ? (uint32_t)g.hfmt : 2u;
+      const uint32_t idesc = (1u << 4) | (ofmt << 7) | (ofmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
       int sa = 0, sb = 0; uint32_t pa = 0, pb = 0; int it = 0;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
         int acc = it & 1;
@@ -241,8 +296,10 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           uint64_t da = make_desc(smem_u32(sA(sa)));
           uint64_t db = make_desc(smem_u32(sB(sb)));
 #pragma unroll
-          for (int k = 0; k < BKF / 8; ++k)   // UMMA_K = 8 tf32 = 32 bytes -> +2 in the (addr >> 4) field
-            tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+          for (int k = 0; k < BKF / 8; ++k) {   // UMMA_K = 8 tf32 or 16 halves = 32 bytes -> +2 in the (addr >> 4) field
+            if (H16) tc_mma_f16(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+            else tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+          }
           if (SPLIT) {
             uint64_t dal = make_desc(smem_u32(sAlo(sa)));
             uint64_t dbl = make_desc(smem_u32(sBlo(sb)));
@@ -323,11 +380,15 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
         const int rowh = row0 + h * 16;
-        const float* p1 = need1 ? g.aux1 + (size_t)rowh * g.ld1 + cco : nullptr;
-        const float* p2 = need2 ? g.aux2 + (size_t)rowh * g.ld2 + cco : nullptr;
-        const float* pz = PREP ? g.zp + (size_t)rowh * g.ldzp + cco : nullptr;
-        const size_t st1 = (size_t)4 * g.ld1, st2 = (size_t)4 * g.ld2, stz = (size_t)4 * g.ldzp;
-        float4 ax1[4], ax2[4], ax3[4];
+        // (byte pointers: a tensor flagged in io16 has 2-byte elements in the H16 kernels)
+        const bool h1 = H16 && (g.io16 & IO16_AUX1), h2 = H16 && (g.io16 & IO16_AUX2), hz = H16 && (g.io16 & IO16_ZP);
+        const bool hc = H16 && (g.io16 & IO16_C), ho = H16 && (g.io16 & IO16_OUT2), hzb = H16 && (g.io16 & IO16_ZBP);
+        const size_t e1 = h1 ? 2 : 4, e2 = h2 ? 2 : 4, ez = hz ? 2 : 4, ec = hc ? 2 : 4, eo = ho ? 2 : 4, ezb = hzb ? 2 : 4;
+        const char* p1 = need1 ? reinterpret_cast<const char*>(g.aux1) + ((size_t)rowh * g.ld1 + cco) * e1 : nullptr;
+        const char* p2 = need2 ? reinterpret_cast<const char*>(g.aux2) + ((size_t)rowh * g.ld2 + cco) * e2 : nullptr;
+        const char* pz = PREP ? reinterpret_cast<const char*>(g.zp) + ((size_t)rowh * g.ldzp + cco) * ez : nullptr;
+        const size_t st1 = (size_t)4 * g.ld1 * e1, st2 = (size_t)4 * g.ld2 * e2, stz = (size_t)4 * g.ldzp * ez;
+        uint4 ax1[4], ax2[4], ax3[4];   // raw bits (fp32 x 4, or 16-bit x 4 in .x .y)
         // per-row scalars (u, sigma, u of the prep stage) are prefetched with the aux rows: loaded at their point of use they
         // were the top stall of the EPI_LATENT_LAST epilogue (ncu: long_scoreboard on the first multiply by u)
         constexpr bool need_u = (EPI == EPI_SILU_U || EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R);
@@ -341,14 +402,14 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           ru[ii] = need_u ? g.u[rowc] : 0.f;
           rs[ii] = (EPI == EPI_LATENT_LAST) ? g.sig[rowc] : 0.f;
           rp[ii] = PREP ? g.pu[rowc] : 0.f;
-          ax1[ii] = (need1 && ok) ? ep_ld4(p1 + ii * st1) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax2[ii] = (need2 && ok) ? ep_ld4(p2 + ii * st2) : make_float4(0.f, 0.f, 0.f, 0.f);
-          ax3[ii] = (PREP && ok) ? ep_ld4(pz + ii * stz) : make_float4(0.f, 0.f, 0.f, 0.f);
+          ax1[ii] = (need1 && ok) ? ep_load<H16>(p1 + ii * st1, h1) : make_uint4(0u, 0u, 0u, 0u);
+          ax2[ii] = (need2 && ok) ? ep_load<H16>(p2 + ii * st2, h2) : make_uint4(0u, 0u, 0u, 0u);
+          ax3[ii] = (PREP && ok) ? ep_load<H16>(pz + ii * stz, hz) : make_uint4(0u, 0u, 0u, 0u);
         }
-        float* qo = g.out2 ? g.out2 + (size_t)rowh * g.ldo2 + cco : nullptr;
-        float* qc = g.C ? g.C + (size_t)rowh * g.ldc + cco : nullptr;
-        float* qz = PREP ? g.zbp + (size_t)rowh * g.ldzbp + cco : nullptr;
-        const size_t sto = (size_t)4 * g.ldo2, stc = (size_t)4 * g.ldc, stzb = (size_t)4 * g.ldzbp;
+        char* qo = g.out2 ? reinterpret_cast<char*>(g.out2) + ((size_t)rowh * g.ldo2 + cco) * eo : nullptr;
+        char* qc = g.C ? reinterpret_cast<char*>(g.C) + ((size_t)rowh * g.ldc + cco) * ec : nullptr;
+        char* qz = PREP ? reinterpret_cast<char*>(g.zbp) + ((size_t)rowh * g.ldzbp + cco) * ezb : nullptr;
+        const size_t sto = (size_t)4 * g.ldo2 * eo, stc = (size_t)4 * g.ldc * ec, stzb = (size_t)4 * g.ldzbp * ezb;
 #pragma unroll
         for (int ii = 0; ii < 4; ++ii) {
           const int i = h * 4 + ii;
@@ -388,8 +449,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               ep += __shfl_xor_sync(0xffffffffu, ep, off);
             }
             if (ok) {
-              ep_st4(qo + ii * sto, make_float4(zb[0], zb[1], zb[2], zb[3]));
-              if (g.C) ep_st4(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]));
+              ep_store<H16>(qo + ii * sto, make_float4(zb[0], zb[1], zb[2], zb[3]), ho, g.hfmt);
+              if (g.C) ep_store<H16>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), hc, g.hfmt);
               if ((lane & 7) == 0) {
                 const int64_t p = (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.c1 * sg * up;
@@ -412,7 +473,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
               o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
             }
-            const float4 zq = ax3[ii];
+            const float4 zq = ep_cvt<H16>(ax3[ii], hz, g.hfmt);
             const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
             const float cu = g.cp * rp[ii];
             float zb[4], up = 0.f;
@@ -426,8 +487,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
             for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
             if (ok) {
-              ep_st4(qz + ii * stzb, make_float4(zb[0], zb[1], zb[2], zb[3]));
-              if (g.C) ep_st4(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]));
+              ep_store<H16>(qz + ii * stzb, make_float4(zb[0], zb[1], zb[2], zb[3]), hzb, g.hfmt);
+              if (g.C) ep_store<H16>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), hc, g.hfmt);
               if ((lane & 7) == 0) {
                 const int64_t p = g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
                 g.upart[p * g.part_stride + row] = g.cp * up;
@@ -439,7 +500,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               case EPI_SILU_BOTH:
               case EPI_SILU_U:
               case EPI_LATENT: {
-                ep_st4(qo + ii * sto, make_float4(v[0], v[1], v[2], v[3]));
+                ep_store<H16>(qo + ii * sto, make_float4(v[0], v[1], v[2], v[3]), ho, g.hfmt);
                 float us = (EPI == EPI_SILU_BOTH) ? 1.0f : ru[ii];
                 if (EPI == EPI_LATENT) {
                   float4 x = AUX1(i);
@@ -474,7 +535,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 #pragma unroll
                 for (int j = 0; j < 4; ++j) o[j] = v[j];
             }
-            ep_st4(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]));
+            ep_store<H16>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), hc, g.hfmt);
           }
         }
         }   // halves
@@ -510,8 +571,9 @@ TmCache& tm_cache(allegro_model* m) {
 
 // exact = true: plain fp32 load (the 3xTF32 path splits the operand itself); false: TFLOAT32 map, i.e. the load
 // rounds to nearest TF32 (the MMA alone would truncate: measured 2-3x larger error)
-int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, long long ld, int box_rows, bool exact, CUtensorMap* out) {
-  TmKey key(ptr, rows, K, ld, box_rows, exact ? 1 : 0);
+// kind 2 / 3: fp16 / bf16 operands of precision 2 (2-byte elements, 64 of them per 128-byte box row)
+int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, long long ld, int box_rows, int kind, CUtensorMap* out) {
+  TmKey key(ptr, rows, K, ld, box_rows, kind);
   auto& c = tm_cache(m);
   auto it = c.find(key);
   if (it != c.end()) { *out = it->second; return ALLEGRO_OK; }
@@ -523,11 +585,14 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
     g_encode = (EncodeTiledFn)fn;
   }
   cuuint64_t gdim[2] = {(cuuint64_t)K, (cuuint64_t)rows};
-  cuuint64_t gstr[1] = {(cuuint64_t)ld * 4};
-  cuuint32_t box[2] = {(cuuint32_t)BKF, (cuuint32_t)box_rows};
+  const int esz = kind >= 2 ? 2 : 4;
+  cuuint64_t gstr[1] = {(cuuint64_t)ld * esz};
+  cuuint32_t box[2] = {(cuuint32_t)(128 / esz), (cuuint32_t)box_rows};
+  const CUtensorMapDataType dt = kind == 0 ? CU_TENSOR_MAP_DATA_TYPE_TFLOAT32 : kind == 1 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32
+                               : kind == 2 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16;
   cuuint32_t estr[2] = {1, 1};
   CUtensorMap tm;
-  CUresult r = g_encode(&tm, exact ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_TFLOAT32, 2, const_cast<void*>(ptr), gdim, gstr, box, estr,
+  CUresult r = g_encode(&tm, dt, 2, const_cast<void*>(ptr), gdim, gstr, box, estr,
                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { al_set_error(m, "cuTensorMapEncodeTiled failed, code " + std::to_string((int)r)); return ALLEGRO_ERR_CUDA; }
@@ -539,38 +604,38 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 
 }  // namespace
 
-#define GEMM_LAUNCH(AS, BS, EW, SP, EP, PR, A2)                                                                          \
+#define GEMM_LAUNCH(AS, BS, EW, SP, EP, PR, A2, H6)                                                                        \
   {                                                                                                                      \
     static_assert(smem_bytes(AS, BS, EW, SP) <= 232448, "shared memory budget (227 KB)");                                \
     static AttrOnce once;                                                                                                \
     if (once.need(m->device)) {                                                                                          \
-      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
                                       (int)smem_bytes(AS, BS, EW, SP)));                                                 \
       once.done(m->device);                                                                                              \
     }                                                                                                                    \
-    k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>( \
+    k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>( \
         tmA, tmA2, tmB, tmB2, g, BN, ntn);                                                                               \
   }
 // one instantiation per epilogue (PREP only exists for the two x-bar epilogues)
-#define GEMM_DISPATCH(AS, BS, EW, SP)                                                                                    \
+#define GEMM_DISPATCH(AS, BS, EW, SP, H6)                                                                                  \
   switch (g.epi) {                                                                                                       \
-    case EPI_PLAIN: GEMM_LAUNCH(AS, BS, EW, SP, EPI_PLAIN, false, false) break;                                                 \
-    case EPI_SILU_BOTH: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_BOTH, false, false) break;                                         \
-    case EPI_SILU_U: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_U, false, false) break;                                               \
-    case EPI_LATENT: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT, false, false) break;                                               \
-    case EPI_MUL_DSILU: GEMM_LAUNCH(AS, BS, EW, SP, EPI_MUL_DSILU, false, false) break;                                         \
-    case EPI_LATENT_LAST: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT_LAST, false, false) break;                                     \
+    case EPI_PLAIN: GEMM_LAUNCH(AS, BS, EW, SP, EPI_PLAIN, false, false, H6) break;                                                 \
+    case EPI_SILU_BOTH: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_BOTH, false, false, H6) break;                                         \
+    case EPI_SILU_U: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_U, false, false, H6) break;                                               \
+    case EPI_LATENT: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT, false, false, H6) break;                                               \
+    case EPI_MUL_DSILU: GEMM_LAUNCH(AS, BS, EW, SP, EPI_MUL_DSILU, false, false, H6) break;                                         \
+    case EPI_LATENT_LAST: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT_LAST, false, false, H6) break;                                     \
     case EPI_ADD2:                                                                                                       \
-      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, true)                                            \
-      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, false)                                                \
-      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, true)                                                \
-      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, false)                                                           \
+      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, true, H6)                                            \
+      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, false, H6)                                                \
+      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, true, H6)                                                \
+      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, false, H6)                                                           \
       break;                                                                                                             \
     case EPI_ADD2R:                                                                                                      \
-      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, true)                                           \
-      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, false)                                               \
-      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, true)                                               \
-      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, false)                                                          \
+      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, true, H6)                                           \
+      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, false, H6)                                               \
+      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, true, H6)                                               \
+      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, false, H6)                                                          \
       break;                                                                                                             \
     default: al_set_error(m, "gemm: unknown epilogue"); return ALLEGRO_ERR_BAD_ARG;                                      \
   }
@@ -582,10 +647,10 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
   int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
   CUtensorMap tmA, tmA2, tmB, tmB2;
-  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, false, &tmA));
-  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, false, &tmA2));
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, 0, &tmA));
+  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, 0, &tmA2));
   else tmA2 = tmA;
-  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, false, &tmB));
+  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, 0, &tmB));
   tmB2 = tmB;
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
@@ -594,7 +659,33 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   // 6/2/16 35.4 ms; L2 prefetch of the A tiles 4-12 k-blocks ahead (cp.async.bulk.prefetch.tensor) 33.3 ms; 2-CTA clusters with
   // every B (weight) stage loaded half by each CTA and multicast to both (L2 -> shared B traffic halved) 32.8 ms: correct, and
   // no faster -- dropped
-  GEMM_DISPATCH(4, 3, 16, false)
+  GEMM_DISPATCH(4, 3, 16, false, false)
+  m->launches++;
+  AL_CUDA(m, cudaGetLastError());
+  return ALLEGRO_OK;
+}
+
+// precision 2: 16-bit operands (fp16 or bf16, g.hfmt) in HBM, tcgen05.mma.kind::f16, fp32 accumulation
+int al_gemm_h16(allegro_model* m, const GemmArgs& g_in) {
+  GemmArgs g = g_in;
+  g.rev = al_next_rev(m);
+  if (!g.Bt16) { al_set_error(m, "16-bit GEMM: 16-bit weights missing"); return ALLEGRO_ERR_BAD_ARG; }
+  if ((g.K & 7) || (g.lda & 7) || (g.ldb & 7) || (g.A2 && ((g.lda2 & 7) || (g.K1 & 63)))) {
+    al_set_error(m, "16-bit GEMM: K and the row strides must be multiples of 8 elements (K1 of 64)");
+    return ALLEGRO_ERR_BAD_HPARAMS;
+  }
+  const int kind = 2 + (g.hfmt ? 1 : 0);
+  int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
+  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  CUtensorMap tmA, tmA2, tmB, tmB2;
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, kind, &tmA));
+  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, kind, &tmA2));
+  else tmA2 = tmA;
+  AL_CHECK(get_tmap(m, g.Bt16, g.N, g.K, g.ldb, BN, kind, &tmB));
+  tmB2 = tmB;
+  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
+  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
+  GEMM_DISPATCH(4, 3, 16, false, true)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
@@ -608,14 +699,14 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g_in) {
   int ntn = (g.N + bn_max(true) - 1) / bn_max(true);
   int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
   CUtensorMap tmA, tmA2, tmB, tmB2;
-  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, true, &tmA));
-  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, true, &tmA2));
+  AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, 1, &tmA));
+  if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, 1, &tmA2));
   else tmA2 = tmA;
-  AL_CHECK(get_tmap(m, g.Bt_hi, g.N, g.K, g.ldb, BN, true, &tmB));
-  AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, true, &tmB2));
+  AL_CHECK(get_tmap(m, g.Bt_hi, g.N, g.K, g.ldb, BN, 1, &tmB));
+  AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, 1, &tmB2));
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  GEMM_DISPATCH(4, 2, 8, true)
+  GEMM_DISPATCH(4, 2, 8, true, false)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;

@@ -81,6 +81,8 @@ struct Dense {
   float* Wt = nullptr;   // [fo][fi] row-major  (B operand of Y = X * W, K-major over fi)
   // precision 0 on tensor cores (3xTF32): W_hi = rn_tf32(W), W_lo = rn_tf32(W - W_hi); same two layouts
   float *W_hi = nullptr, *W_lo = nullptr, *Wt_hi = nullptr, *Wt_lo = nullptr;
+  // 16-bit operand modes (precision 2 bf16 / 4 fp16): the same two layouts as 16-bit elements
+  void *W16 = nullptr, *Wt16 = nullptr;
 };
 
 struct DevBuf {
@@ -127,6 +129,7 @@ struct allegro_model {
   cudaStream_t stream = 0;
   allegro_alloc_fn alloc_fn = nullptr; allegro_free_fn free_fn = nullptr; void* alloc_user = nullptr;
   int64_t chunk_edges = 1 << 20;
+  int hfmt = -1;                          // 16-bit operand modes: 0 fp16 (precision 4), 1 bf16 (precision 2); -1: fp32 activations
   int tt_mode = 0;                        // tensor track: 0 contracted per centre (tpc_impl.cuh), 1 per-edge products (allegro_set_tensor_track)
   bool debug_keep = false;                // allegro_set_debug: also store tensors that are otherwise consumed on chip
   int64_t launches = 0;

@@ -3,6 +3,9 @@
 #include <cmath>
 #include <cstring>
 
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
 #include "internal.h"
 
 static thread_local std::string g_err;
@@ -64,10 +67,15 @@ static int check_hp(const allegro_hparams* hp) {
   for (int k = 0; k < hp->n_edge; ++k) if (hp->edge_dims[k] < 1) return bad("edge_dims");
   if (hp->latent_dims[hp->n_latent - 1] != hp->twobody_dims[hp->n_twobody - 1]) return bad("last latent width must equal d");
   if (!(hp->avg_num_neighbors > 0)) return bad("avg_num_neighbors");
-  if (hp->precision < 0 || hp->precision > 3) return bad("precision");
-  if (hp->precision == 2) {   // 16-bit operand storage + tcgen05 kind::f16 is not built: refuse instead of aliasing another mode
-    al_set_error(nullptr, "precision 2 (BF16-operand MLPs) is not implemented; use 1 (TF32) or 0 / 3 (fp32)");
-    return ALLEGRO_ERR_UNIMPLEMENTED;
+  if (hp->precision < 0 || hp->precision > 4) return bad("precision");
+  if (hp->precision == 2 || hp->precision == 4) {
+    // 16-bit operand MLPs (tcgen05 kind::f16): TMA rows of 16-bit tensors need 16-byte strides, the K-concatenated x-bar GEMM
+    // needs a first latent width that is a multiple of the 64-element k-block, and the fused last-latent epilogue d % 32 == 0
+    if (hp->n_twobody < 2) return bad("16-bit operand modes need at least two two-body layers");
+    for (int k = 0; k < hp->n_twobody; ++k) if (hp->twobody_dims[k] % 8) return bad("16-bit operand modes: twobody_dims multiples of 8");
+    for (int k = 0; k < hp->n_latent; ++k) if (hp->latent_dims[k] % 8) return bad("16-bit operand modes: latent_dims multiples of 8");
+    if (hp->latent_dims[0] % 64) return bad("16-bit operand modes: first latent width a multiple of 64");
+    if (hp->twobody_dims[hp->n_twobody - 1] % 32 || hp->n_tensor % 32) return bad("16-bit operand modes: d and n_tensor multiples of 32");
   }
   return ALLEGRO_OK;
 }
@@ -139,6 +147,19 @@ static int upload_dense(allegro_model* m, Dense& D, const std::vector<float>& W,
     for (int o = 0; o < fo; ++o) Wt[(size_t)o * fi + i] = W[(size_t)i * fo + o];
   AL_CHECK(upload(m, &D.W, W));
   AL_CHECK(upload(m, &D.Wt, Wt));
+  if (m->hfmt >= 0) {
+    auto conv = [&](const std::vector<float>& x) {
+      std::vector<uint16_t> h(x.size());
+      for (size_t k = 0; k < x.size(); ++k) {
+        if (m->hfmt == 0) { __half v = __float2half_rn(x[k]); memcpy(&h[k], &v, 2); }
+        else { __nv_bfloat16 v = __float2bfloat16_rn(x[k]); memcpy(&h[k], &v, 2); }
+      }
+      return h;
+    };
+    uint16_t* p16 = nullptr;
+    AL_CHECK(upload(m, &p16, conv(W))); D.W16 = p16;
+    AL_CHECK(upload(m, &p16, conv(Wt))); D.Wt16 = p16;
+  }
   if (m->hp.precision == 0) {
     auto split = [](const std::vector<float>& x, std::vector<float>& hi, std::vector<float>& lo) {
       hi.resize(x.size()); lo.resize(x.size());
@@ -174,6 +195,7 @@ extern "C" int allegro_create(const allegro_hparams* hp, const void* blob, size_
   }
   allegro_model* m = new allegro_model();
   m->hp = *hp;
+  m->hfmt = (hp->precision == 2) ? 1 : (hp->precision == 4) ? 0 : -1;
   m->S = hp->n_species; m->NB = hp->n_bessel; m->d = hp->twobody_dims[hp->n_twobody - 1];
   m->n = hp->n_tensor; m->lmax = hp->l_max; m->NL = hp->n_layers;
   m->Denv = (m->lmax + 1) * (m->lmax + 1); m->nA = m->n * (m->lmax + 1); m->ldY = (m->Denv + 3) & ~3;

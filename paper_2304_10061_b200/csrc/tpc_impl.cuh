@@ -26,6 +26,7 @@
 // HBM traffic per edge at config 2/3 (n = 64): forward 2 x (omega 768 + w0 768 + s 256 B), backward 6.3 KB, against
 // 7.4 + 12.0 KB for the per-edge product kernels (tp2_impl.cuh), and the [edges, D, n] buffers T, V-bar are not allocated.
 #pragma once
+#include "h16.cuh"
 #include "tp2_impl.cuh"
 
 constexpr int TPC_MAXL = 3;   // layers the contracted kernels are instantiated for
@@ -43,6 +44,7 @@ struct TPC {
   static constexpr int NNZ2 = NL >= 2 ? Pat<TpcPat<LM, NL, (NL >= 2 ? 2 : 1)>::P>::NNZ : 1;
   static constexpr int NNZ3 = NL >= 3 ? Pat<TpcPat<LM, NL, (NL >= 3 ? 3 : 1)>::P>::NNZ : 1;
   const int64_t* rowa; int nc, n; float c_env; int rev;
+  int hfmt;                                   // >= 0 (16-bit operand modes): xs, ombar, w0bar are 16-bit tensors (GEMM A operands)
   const float* Y; int ldy;
   const float* w0; int ldw;                   // w^0_e[l][n]
   const float* om; int ldo;                   // omega^L_e[l][n] of THIS layer
@@ -80,6 +82,17 @@ template <int P, bool E0, int NNZ>
 __device__ __forceinline__ void tpc_gb(const float (&kv)[NNZ], const float* u, const float* w, float* g) {
 #define X(k, a_, b_, c_) \
   if (!E0) g[b_] = fmaf(kv[k] * w[c_], u[a_], g[b_]); else if ((c_) == 0) g[b_] = fmaf(kv[k], u[a_], g[b_]);
+  TP2_EXPAND(P, X)
+#undef X
+}
+
+// tr and gb over the same pattern with the same left vector u in one sweep: v = M^T u and g[b] += sum K[a,b,c] u[a] w[c] share
+// the product kv[k] * u[a] (3 instead of 4 instructions per entry; the shared product lives for two instructions only)
+template <int P, int NNZ>
+__device__ __forceinline__ void tpc_tr_gb(const float (&kv)[NNZ], const float* G, const float* u, const float* w, float* v, float* g) {
+#pragma unroll
+  for (int c = 0; c < Pat<P>::DOUT; ++c) v[c] = 0.f;
+#define X(k, a_, b_, c_) { const float t_ = kv[k] * u[a_]; v[c_] = fmaf(t_, G[b_], v[c_]); g[b_] = fmaf(t_, w[c_], g[b_]); }
   TP2_EXPAND(P, X)
 #undef X
 }
@@ -289,7 +302,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_fwd(const __grid_consta
   }
   // s^L_e = sum_a w0_e[l(a)] Y_e[a] n^L[a]
   q.src1 = a.w0; q.ld1 = a.ldw;
-  float* xsp = a.xs + e0 * a.ldx + nn;
+  const size_t xs0 = (size_t)e0 * a.ldx + nn;
   tpc_stream<DENV, 0>(ring, q, e0, deg, grp * 32, lane, [&](int il, int, const float* st) {
     float t[NLV];
 #pragma unroll
@@ -299,7 +312,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_fwd(const __grid_consta
     float sv = 0.f;
 #pragma unroll
     for (int l = 0; l < NLV; ++l) sv = fmaf(st[l * 32 + lane], t[l], sv);
-    xsp[(int64_t)il * a.ldx] = sv;
+    h16_store(a.xs, xs0 + (size_t)il * a.ldx, sv, a.hfmt);
   }, [](int) {});
 }
 
@@ -386,7 +399,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_fwd_rb(const __grid_con
       float s = 0.f;
 #pragma unroll
       for (int l = 0; l < NLV; ++l) s = fmaf(w[i][l], t[l], s);
-      if (e + i < e1) a.xs[(e + i) * a.ldx + nn] = s;
+      if (e + i < e1) h16_store(a.xs, (size_t)(e + i) * a.ldx + nn, s, a.hfmt);
     }
   }
 }
@@ -431,7 +444,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
     }
     TpcSrc q{a.w0, a.ldw, a.sb[L - 1], a.lds[L - 1], (L == 1 && NL >= 2) ? a.sb[1] : nullptr, (L == 1 && NL >= 2) ? a.lds[1] : 0,
              a.Y, a.ldy, a.n};
-    float* wbp = (L == 1) ? a.w0bar + e0 * a.ldob + nn : nullptr;
+    size_t wbo = (size_t)e0 * a.ldob + nn;       // element offset into w0bar
     // Y-bar sums over the lanes: batched over four edges (l_max <= 2: 36 values per butterfly pass) or one tree per edge
     // (l_max = 3: the four-edge batch costs 64 registers and measured slower, 20.9 against 17.0 ms per step at config 4)
     constexpr bool BATCHY = DENV <= 9;
@@ -461,8 +474,8 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
           pp[BATCHY ? j : 0][b] = w[l_of(b)] * vb;
         }
 #pragma unroll
-        for (int l = 0; l < NLV; ++l) wbp[l * a.n] = wbar[l];
-        wbp += a.ldob;
+        for (int l = 0; l < NLV; ++l) h16_store(a.w0bar, wbo + (size_t)l * a.n, wbar[l], a.hfmt);
+        wbo += a.ldob;
         if constexpr (!BATCHY) tp_ybar_rows<DENV, true>(Yb0 + (int64_t)il * DENV, pp[0], 0, DENV, lane);
       } else {
 #pragma unroll
@@ -505,9 +518,8 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
       tpc_fwd<P2, true>(a.kv2, G[1], nullptr, w1);                   // w_1 = M^2 e_0
 #pragma unroll
       for (int b = 0; b < DENV; ++b) g1[b] = 0.f;
-      tpc_gb<P1, false>(a.kv1, nb, w1, g1);
+      tpc_tr_gb<P1>(a.kv1, G[0], nb, w1, u1, g1);                    // u_1 = M^1T n-bar;  Gamma-bar^1 += g_1(n-bar, w_1)
       put(1, g1);
-      tpc_tr<P1>(a.kv1, G[0], nb, u1);                               // u_1 = M^1T n-bar
       tpc_gb<P2, true>(a.kv2, u1, nullptr, Gb);
     } else {
       float w2[Pat<P3>::DIN], w1[Pat<P2>::DIN], u1[Pat<P1>::DOUT], u2[Pat<P2>::DOUT], g[DENV];
@@ -515,14 +527,12 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
       tpc_fwd<P2, false>(a.kv2, G[1], w2, w1);                       // w_1 = M^2 w_2
 #pragma unroll
       for (int b = 0; b < DENV; ++b) g[b] = 0.f;
-      tpc_gb<P1, false>(a.kv1, nb, w1, g);
+      tpc_tr_gb<P1>(a.kv1, G[0], nb, w1, u1, g);
       put(1, g);
-      tpc_tr<P1>(a.kv1, G[0], nb, u1);
 #pragma unroll
       for (int b = 0; b < DENV; ++b) g[b] = 0.f;
-      tpc_gb<P2, false>(a.kv2, u1, w2, g);
+      tpc_tr_gb<P2>(a.kv2, G[1], u1, w2, u2, g);
       put(2, g);
-      tpc_tr<P2>(a.kv2, G[1], u1, u2);
       tpc_gb<P3, true>(a.kv3, u2, nullptr, Gb);
     }
   }
@@ -532,7 +542,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
   for (int b = 0; b < DENV; ++b) Gb[b] *= a.c_env;
   {
     TpcSrc q{a.om, a.ldo, nullptr, 0, nullptr, 0, a.Y, a.ldy, a.n};
-    float* obp = a.ombar + e0 * a.ldob + nn;
+    size_t obo = (size_t)e0 * a.ldob + nn;       // element offset into ombar
     constexpr bool BATCHY = DENV <= 9;
     float pp[BATCHY ? 4 : 1][DENV];
     tpc_stream<DENV, 0>(ring, q, e0, deg, grp * 32, lane, [&](int il, int j, const float* st) {
@@ -545,8 +555,8 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
         pp[BATCHY ? j : 0][b] = om[l_of(b)] * Gb[b];
       }
 #pragma unroll
-      for (int l = 0; l < NLV; ++l) obp[l * a.n] = ob[l];
-      obp += a.ldob;
+      for (int l = 0; l < NLV; ++l) h16_store(a.ombar, obo + (size_t)l * a.n, ob[l], a.hfmt);
+      obo += a.ldob;
       if constexpr (!BATCHY) tp_ybar_rows<DENV, true>(YbL + (int64_t)il * DENV, pp[0], 0, DENV, lane);
     }, [&](int il0) {
       if constexpr (BATCHY) {
@@ -564,7 +574,7 @@ static __global__ void __launch_bounds__(WPB * 32) k_tpc_bwd(const __grid_consta
 // ---- host side ---------------------------------------------------------------------------------------------
 template <int LM, int NL>
 int tpc_fill(allegro_model* m, Work& w, int L, int nc, const float* om, int ldo, const float* w0, int ldw, TPC<LM, NL>& a) {
-  a.rowa = (const int64_t*)w.rowa.p; a.nc = nc; a.n = m->n; a.c_env = m->c_env; a.rev = al_next_rev(m);
+  a.rowa = (const int64_t*)w.rowa.p; a.nc = nc; a.n = m->n; a.c_env = m->c_env; a.rev = al_next_rev(m); a.hfmt = m->hfmt;
   a.Y = (const float*)w.Y.p; a.ldy = m->ldY; a.w0 = w0; a.ldw = ldw; a.om = om; a.ldo = ldo;
   a.gam = (float*)w.tpc_gam.p; a.nvec = (float*)w.tpc_nvec.p; a.gacc = (float*)w.tpc_gacc.p;
   a.cstride = (int64_t)w.cap_centers * m->Denv * m->n;

@@ -63,18 +63,23 @@ def test_product_never_imports_oracle():
         assert "import paper_2304_10061_b200" not in txt and "from paper_2304_10061_b200" not in txt
 
 
-def test_precision_2_is_refused_not_aliased():
-    """BF16-operand MLPs are not built: allegro_create must say so (ALLEGRO_ERR_UNIMPLEMENTED = -7) instead of running
-    another mode under that name.  The hyper-parameter check runs before any device is touched, so this needs no GPU."""
+def test_16bit_operand_modes_check_their_preconditions():
+    """Precision 2 / 4 (bf16 / fp16 operand MLPs) are real modes with shape preconditions (include/b200_allegro.h); a model
+    that does not meet them is refused with ALLEGRO_ERR_BAD_HPARAMS instead of silently running another mode.  The
+    hyper-parameter check runs before any device is touched, so this needs no GPU."""
     import ctypes as C
+    import dataclasses
     import paper_2304_10061_b200 as P
     from synthetic import CONFIGS
     lib = P.load_library()
-    hp = P.hparams_from(CONFIGS[0].hp, 2)
-    h = C.c_void_p(None)
-    blob = C.create_string_buffer(16)
-    rc = lib.allegro_create(C.byref(hp), blob, 16, C.byref(h))
-    assert rc == -7 and not h
-    assert b"precision 2" in lib.allegro_last_error(None)
     n = C.c_size_t(0)
-    assert lib.allegro_blob_size(C.byref(hp), C.byref(n)) == -7
+    for prec in (2, 4):
+        ok = P.hparams_from(CONFIGS[1].hp, prec)
+        assert lib.allegro_blob_size(C.byref(ok), C.byref(n)) == 0 and n.value > 0
+        one_layer = P.hparams_from(dataclasses.replace(CONFIGS[1].hp, twobody_dims=(256,)), prec)
+        assert lib.allegro_blob_size(C.byref(one_layer), C.byref(n)) == -1
+        odd_latent = P.hparams_from(dataclasses.replace(CONFIGS[1].hp, latent_dims=(96, 256)), prec)
+        assert lib.allegro_blob_size(C.byref(odd_latent), C.byref(n)) == -1
+        assert b"16-bit" in lib.allegro_last_error(None)
+    bad = P.hparams_from(CONFIGS[1].hp, 5)
+    assert lib.allegro_blob_size(C.byref(bad), C.byref(n)) == -1

@@ -17,7 +17,7 @@ from synthetic.configs import scaled_config
 from gpu_util import gpu_eval, make_both
 
 
-@pytest.mark.parametrize("ci,n,precision", [(1, 3072, 1), (1, 3072, 0), (4, 1200, 1), (2, 3000, 1)])
+@pytest.mark.parametrize("ci,n,precision", [(1, 3072, 1), (1, 3072, 0), (4, 1200, 1), (2, 3000, 1), (2, 3000, 4), (4, 1200, 2)])
 def test_run_to_run(ci, n, precision):
     cfg = scaled_config(ci, n)
     pos, sp, box = make_system(cfg)
