@@ -96,8 +96,10 @@ void al_work_free(allegro_model* m) {
   m->work = nullptr;
 }
 
-// io16 (precision 2 only): which epilogue tensors of this launch are stored as 16-bit (IO16_* below = gemm_tc.cu's bits)
-enum { IO16_C = 1, IO16_OUT2 = 2, IO16_ZBP = 4, IO16_AUX1 = 8, IO16_AUX2 = 16, IO16_ZP = 32 };
+// io16 (16-bit operand modes only): every epilogue tensor of a 16-bit GEMM (aux rows, second output, prep-stage tensors) is
+// 16-bit; its main output C is 16-bit only where a GEMM or an epilogue is the sole reader (IO16_C = gemm_tc.cu's bit) and
+// fp32 where the tensor track, k_edge_bwd or a debug tap reads it
+enum { IO16_C = 1 };
 static GemmArgs mk(const allegro_model* m, const float* A, int lda, const Dense& D, bool transposed_weight, float* C, int ldc, int m_cap,
                    const int* m_ptr, int epi, int io16 = 0) {
   // transposed_weight = false: forward  Y = X W   -> Bt = Wt [fo][fi], N = fo, K = fi
@@ -144,7 +146,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     bool last = (k == ntb - 1);
     GemmArgs g = mk(m, (float*)w.tb_a[k - 1].p, hp.twobody_dims[k - 1], m->twobody[k], false,
                     last ? (float*)w.XS[0].p : (float*)w.tb_a[k].p, last ? d + n : hp.twobody_dims[k], m_cap, mp,
-                    last ? EPI_SILU_U : EPI_SILU_BOTH, IO16_C | IO16_OUT2);
+                    last ? EPI_SILU_U : EPI_SILU_BOTH, IO16_C);
     g.out2 = (float*)w.tb_z[k].p; g.ldo2 = hp.twobody_dims[k]; g.u = (float*)w.u.p;
     AL_CHECK(al_gemm(m, g));
   }
@@ -166,7 +168,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       else if (L < NL) { C = (float*)w.XS[L].p; ldc = d + n; }
       else { C = (float*)w.XF.p; ldc = d; }
       GemmArgs g = mk(m, A, lda, m->latent[L - 1][k], false, C, ldc, m_cap, mp, last ? EPI_LATENT : EPI_SILU_BOTH,
-                      IO16_C | IO16_OUT2 | IO16_AUX1);
+                      IO16_C);
       g.out2 = (float*)w.lat_z[L - 1][k].p; g.ldo2 = hp.latent_dims[k];
       g.u = (float*)w.u.p; g.aux1 = (float*)w.XS[L - 1].p; g.ld1 = d + n; g.c0 = m->c_old[L - 1]; g.c1 = m->c_new[L - 1];
       if (last && L == NL && fused_last) {
@@ -214,7 +216,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       AL_CHECK(k_launch_bwd_prep(m, w, rank1 ? nullptr : xb, d, (float*)w.lat_z[L - 1][nlat - 1].p, d, m->c_new[L - 1], zb, d, d, m_cap));
     for (int k = nlat - 1; k >= 1; --k) {
       GemmArgs g = mk(m, zb, hp.latent_dims[k], m->latent[L - 1][k], true, zb_o, hp.latent_dims[k - 1], m_cap, mp, EPI_MUL_DSILU,
-                      IO16_C | IO16_AUX1);
+                      IO16_C);
       g.aux1 = (float*)w.lat_z[L - 1][k - 1].p; g.ld1 = hp.latent_dims[k - 1];
       AL_CHECK(al_gemm(m, g));
       std::swap(zb, zb_o);
@@ -245,7 +247,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
     g.u = (float*)w.sig.p; g.aux3 = m->w_eff_f;
     if (kcat) {
       const int h = hp.latent_dims[0];
-      GemmArgs gc = mk(m, zb, h, m->xcat[L - 1], true, xb_o, d, m_cap, mp, g.epi, IO16_C | IO16_AUX1 | IO16_ZP | IO16_ZBP);
+      GemmArgs gc = mk(m, zb, h, m->xcat[L - 1], true, xb_o, d, m_cap, mp, g.epi, IO16_C);
       gc.A2 = (float*)w.OB.p; gc.lda2 = ldob; gc.K1 = h;
       gc.aux1 = g.aux1; gc.ld1 = g.ld1; gc.c0 = g.c0; gc.aux2 = nullptr; gc.ld2 = 0; gc.u = g.u; gc.aux3 = g.aux3;
       g = gc;
@@ -273,7 +275,7 @@ static int run_chunk(allegro_model* m, Work& w, const Chunk& ch, const double* p
       AL_CHECK(k_launch_bwd_prep(m, w, xb, d, (float*)w.tb_z[ntb - 1].p, d, 1.0f, zb, d, d, m_cap));
     for (int k = ntb - 1; k >= 1; --k) {
       GemmArgs g = mk(m, zb, hp.twobody_dims[k], m->twobody[k], true, zb_o, hp.twobody_dims[k - 1], m_cap, mp, EPI_MUL_DSILU,
-                      IO16_AUX1 | (k > 1 ? IO16_C : 0));   // the last z-bar (read by k_edge_bwd) stays fp32
+                      (k > 1 ? IO16_C : 0));   // the last z-bar (read by k_edge_bwd) stays fp32
       g.aux1 = (float*)w.tb_z[k - 1].p; g.ld1 = hp.twobody_dims[k - 1];
       AL_CHECK(al_gemm(m, g));
       std::swap(zb, zb_o);

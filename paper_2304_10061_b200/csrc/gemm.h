@@ -51,8 +51,9 @@ struct GemmArgs {
   // 1: the kernel walks its row tiles from the last to the first (set by the launcher, see al_next_rev(): consecutive
   // edge-ordered kernels alternate direction so each starts on the rows its producer left in L2)
   int rev;
-  // precision 2 (16-bit operand storage): element format of A / B and of the epilogue tensors named in io16 (bit mask, see
-  // gemm_tc.cu IO16_*): 0 fp16, 1 bf16.  A, A2, Bt then point to 16-bit data (Bt16), lda / lda2 / ldb count elements.
+  // precision 4 / 2 (16-bit operand storage): hfmt = element format of A / B and of every epilogue tensor (aux1, aux2, out2,
+  // zp, zbp), 0 fp16, 1 bf16; io16 bit 0 (gemm_tc.cu IO16_C): C is 16-bit too, else fp32.  A, A2, Bt then point to 16-bit
+  // data (Bt16); lda / lda2 / ldb and the epilogue strides count elements.
   int hfmt, io16;
   const void* Bt16;
 };

@@ -22,8 +22,6 @@
 
 namespace {
 
-#define AUX1(i) ep_cvt<H16>(ax1[(i) & 3], h1, g.hfmt)
-#define AUX2(i) ep_cvt<H16>(ax2[(i) & 3], h2, g.hfmt)
 constexpr int BM = 128;          // UMMA M (cta_group::1)
 constexpr int BKF = 32;          // K floats per stage = one 128-byte swizzle atom
 constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
@@ -121,52 +119,81 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr) {
   return d;
 }
 
-// epilogue operands are streamed (read or written once per launch): keep them out of L1
-__device__ __forceinline__ void ep_st4(float* p, const float4 v) {
-  asm volatile("st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
-}
-
-// tensor-core modes: fast-math sigmoid (ex2.approx + rcp.approx), error ~1e-7 << TF32 rounding
-// Precision 2 (16-bit operand storage): four consecutive elements = 8 bytes.  fmt 0: IEEE fp16 (10-bit mantissa, as TF32),
-// fmt 1: bfloat16 (7-bit mantissa, fp32 range).  GemmArgs::io16 says which epilogue tensors are stored that way.
-enum { IO16_C = 1, IO16_OUT2 = 2, IO16_ZBP = 4, IO16_AUX1 = 8, IO16_AUX2 = 16, IO16_ZP = 32 };
-__device__ __forceinline__ void ep_st4h(void* p, const float4 v, int fmt) {
-  uint2 o;
-  if (fmt == 0) {
-    __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
-    o.x = *reinterpret_cast<uint32_t*>(&a); o.y = *reinterpret_cast<uint32_t*>(&b);
-  } else {
-    __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
-    o.x = *reinterpret_cast<uint32_t*>(&a); o.y = *reinterpret_cast<uint32_t*>(&b);
-  }
-  asm volatile("st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};" ::"l"(p), "r"(o.x), "r"(o.y) : "memory");
-}
-// element-size aware versions used by the epilogue: `h` = this tensor is stored as 16-bit (only in H16 kernels).
-// The load returns the raw bits and the conversion happens where the value is used: with the conversion at the load every
-// prefetched aux row waited for its own memory latency (ncu r2m: 58 % long_scoreboard on the PRMT behind each load).
-template <bool H16>
-__device__ __forceinline__ uint4 ep_load(const char* p, bool h) {
+// ---- epilogue memory operations -------------------------------------------------------------------------
+// Epilogue operands are streamed (read or written once per launch): L1::no_allocate.  Every access is PREDICATED inside the
+// asm statement and carries no "memory" clobber, so the 16-row half of a chunk is one basic block: with `if (ok) store`
+// branches and clobbering stores the four row groups of a half ran one after the other, each exposing its own shared-memory
+// load and MUFU chain (ncu r2m: 24 % `wait`, issue slots half idle at 4 epilogue warps per scheduler).
+// HF = 0: four fp32 (16 bytes); HF = 1 / 2: four IEEE fp16 / bfloat16 values (8 bytes), converted where they are used.
+enum { IO16_C = 1 };   // GemmArgs::io16: in the 16-bit kernels every epilogue tensor is 16-bit; C is, only if this bit is set
+template <int HF>
+__device__ __forceinline__ uint4 ep_load(const char* p, bool pred) {
   uint4 v = make_uint4(0u, 0u, 0u, 0u);
-  if (H16 && h) asm volatile("ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p));
-  else asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  if (HF)
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %3, 0;\n\t@q ld.global.nc.L1::no_allocate.v2.u32 {%0,%1}, [%2];\n\t}"
+                 : "+r"(v.x), "+r"(v.y) : "l"(p), "r"((int)pred));
+  else
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %5, 0;\n\t@q ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];\n\t}"
+                 : "+r"(v.x), "+r"(v.y), "+r"(v.z), "+r"(v.w) : "l"(p), "r"((int)pred));
   return v;
 }
-template <bool H16>
-__device__ __forceinline__ float4 ep_cvt(const uint4 v, bool h, int fmt) {
-  if (H16 && h) {
-    if (fmt == 0) {
-      const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
-      const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
-      return make_float4(a.x, a.y, b.x, b.y);
-    }
+template <int HF>
+__device__ __forceinline__ float4 ep_cvt(const uint4 v) {
+  if (HF == 1) {
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&v.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&v.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+  }
+  if (HF == 2)
     return make_float4(__uint_as_float(v.x << 16), __uint_as_float(v.x & 0xFFFF0000u),
                        __uint_as_float(v.y << 16), __uint_as_float(v.y & 0xFFFF0000u));
-  }
   return make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), __uint_as_float(v.w));
 }
-template <bool H16>
-__device__ __forceinline__ void ep_store(char* p, const float4 v, bool h, int fmt) {
-  if (H16 && h) ep_st4h(p, v, fmt); else ep_st4(reinterpret_cast<float*>(p), v);
+template <int HF>
+__device__ __forceinline__ void ep_store(char* p, const float4 v, bool pred) {
+  if (HF) {
+    uint2 o;
+    if (HF == 1) {
+      __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
+      o.x = *reinterpret_cast<uint32_t*>(&a); o.y = *reinterpret_cast<uint32_t*>(&b);
+    } else {
+      __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+      o.x = *reinterpret_cast<uint32_t*>(&a); o.y = *reinterpret_cast<uint32_t*>(&b);
+    }
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %3, 0;\n\t@q st.global.L1::no_allocate.v2.u32 [%0], {%1,%2};\n\t}"
+                 ::"l"(p), "r"(o.x), "r"(o.y), "r"((int)pred));
+  } else {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %5, 0;\n\t@q st.global.L1::no_allocate.v4.f32 [%0], {%1,%2,%3,%4};\n\t}"
+                 ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "r"((int)pred));
+  }
+}
+// C of a 16-bit kernel: 16-bit or fp32 by a launch-uniform flag -> two complementary predicated stores, no branch
+template <int HF>
+__device__ __forceinline__ void ep_store_c(char* p, const float4 v, bool pred, bool c16) {
+  if (HF) { ep_store<HF>(p, v, pred && c16); ep_store<0>(p, v, pred && !c16); }
+  else ep_store<0>(p, v, pred);
+}
+__device__ __forceinline__ void ep_st_f32(float* p, float v, bool pred) {
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t@q st.global.f32 [%0], %1;\n\t}" ::"l"(p), "f"(v), "r"((int)pred));
+}
+__device__ __forceinline__ void ep_st_f64(double* p, double v, bool pred) {
+  asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.b32 q, %2, 0;\n\t@q st.global.f64 [%0], %1;\n\t}" ::"l"(p), "d"(v), "r"((int)pred));
+}
+// staging tile of the TMEM -> coalesced-domain transposition, addressed as shared memory (a generic pointer costs LD.E / ST.E)
+__device__ __forceinline__ void sts128(uint32_t a, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+  asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+// Not volatile: the compiler may hoist it above the (volatile) global stores of the previous row group.  What keeps it behind
+// the warp barrier that follows the tile's st.shared is its address: derived from stg_fence()'s opaque result.
+__device__ __forceinline__ float4 lds128(uint32_t a) {
+  float4 v;
+  asm("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+  return v;
+}
+__device__ __forceinline__ uint32_t stg_fence(uint32_t a) {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %1;" : "=r"(r) : "r"(a) : "memory");
+  return r;
 }
 
 // sigmoid = rcp.approx(1 + ex2.approx(-z log2 e)): the two MUFU operations and nothing else (__fdividef adds a range test and
@@ -189,9 +216,9 @@ __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__fl
 
 // EPI (GemmEpi) and PREP (the z-bar / u-bar stage of EPI_ADD2 / EPI_ADD2R) are compile-time: one kernel per epilogue,
 // so the epilogue carries no run-time dispatch, no dead operands and no re-loaded argument fields.
-// H16 (precision 2): A and B operands are 16-bit in HBM (fp16 or bf16, GemmArgs::hfmt), one stage = 64 K-elements (the same
-// 128-byte rows), tcgen05.mma.kind::f16 with fp32 accumulation; the epilogue tensors flagged in GemmArgs::io16 are 16-bit too.
-template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, bool H16 = false>
+// HF = 1 / 2 (precision 4 / 2): A and B operands are fp16 / bf16 in HBM, one stage = 64 K-elements (the same
+// 128-byte rows), tcgen05.mma.kind::f16 with fp32 accumulation; every epilogue tensor is 16-bit too, C only if GemmArgs::io16 has IO16_C.
+template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, int HF = 0>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
             const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
@@ -199,6 +226,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT);
   constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT);
   constexpr int EW0 = SPLIT ? 7 : 3;     // first epilogue warp (warps 3..6 are the splitter in SPLIT mode)
+  constexpr bool H16 = HF != 0;              // HF = 1: IEEE fp16, 2: bfloat16 operands and epilogue tensors
   constexpr int BKE = H16 ? 2 * BKF : BKF;   // K elements per stage
   static_assert(!(SPLIT && H16), "3xTF32 and 16-bit operands exclude each other");
   extern __shared__ uint8_t smem_raw[];
@@ -281,7 +309,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     if (lane == 0) {
       // instruction descriptor: D=f32, A=B=tf32, K-major both, N>>3, M>>4
       // (A / B format field: 2 = tf32 for kind::tf32; kind::f16: 0 = f16, 1 = bf16)
-      const uint32_t ofmt = H16 ? (uint32_t)g.hfmt : 2u;
+      const uint32_t ofmt = H16 ? (uint32_t)(HF - 1) : 2u;
       const uint32_t idesc = (1u << 4) | (ofmt << 7) | (ofmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
       int sa = 0, sb = 0; uint32_t pa = 0, pb = 0; int it = 0;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
@@ -353,191 +381,178 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       // Each 32-column chunk: TMEM -> registers (lane = row) -> padded smem -> registers in the
       // "coalesced domain" (8 lanes x float4 cover one row's 128 B, 4 rows per warp instruction), so
       // every global load/store of the epilogue touches 4 lines per instruction instead of 32.
-      float4* stg4 = reinterpret_cast<float4*>(stage_buf) + (warp - EW0) * (32 * 8);
+      const uint32_t stg_s = smem_u32(stage_buf) + (uint32_t)(warp - EW0) * (32 * 8 * 16);
       const int chunk0 = (warp - EW0) >> 2;   // this warp takes chunks chunk0, chunk0 + EPI_WARPS/4, ...
       const int rsub = lane >> 3, c4 = (lane & 7) * 4;
       const int rbase = mt * BM + q * 32;
+      const bool c16 = H16 && (g.io16 & IO16_C);
+      const bool haveC = g.C != nullptr;
       for (int c0 = chunk0 * 32; c0 < BN; c0 += 32 * (EPI_WARPS / 4)) {
-        uint32_t r[32];
-        tc_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN_MAX + c0, r);
+        {
+          uint32_t r[32];
+          tc_ld32(tmem_base + ((uint32_t)(q * 32) << 16) + acc * BN_MAX + c0, r);
 #pragma unroll
-        for (int gq = 0; gq < 8; ++gq)
-          stg4[lane * 8 + (gq ^ (lane & 7))] = make_float4(__uint_as_float(r[4 * gq]), __uint_as_float(r[4 * gq + 1]),
-                                                           __uint_as_float(r[4 * gq + 2]), __uint_as_float(r[4 * gq + 3]));
+          for (int gq = 0; gq < 8; ++gq)
+            sts128(stg_s + (uint32_t)(lane * 8 + (gq ^ (lane & 7))) * 16, r[4 * gq], r[4 * gq + 1], r[4 * gq + 2], r[4 * gq + 3]);
+        }
         __syncwarp();
+        const uint32_t stg = stg_fence(stg_s);
         const int col = nt * BN + c0 + c4;
         const bool col_ok = (col < g.N) && (c0 + c4 < BN);
-        // Two halves of 16 rows: issue every aux load of a half up front (the stores below may alias, so the compiler
-        // cannot hoist them), then process it.  Halving keeps the register count low enough for 16 epilogue warps.
+        // Two halves of 16 rows: issue every aux load of a half up front, then process it.  Halving keeps the register
+        // count low enough for 16 epilogue warps.
         constexpr bool need1 = (EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_MUL_DSILU || EPI == EPI_ADD2);
         constexpr bool need2 = (EPI == EPI_ADD2 || EPI == EPI_ADD2R) && AUX2;   // no aux2: the term is in the K-concatenation
+        constexpr bool out2 = (EPI == EPI_SILU_BOTH || EPI == EPI_SILU_U || EPI == EPI_LATENT || EPI == EPI_LATENT_LAST);
         // the column vector of the rank-1 / energy epilogues is the same for all 32 rows of the chunk: one load per chunk
         float4 w3 = make_float4(0.f, 0.f, 0.f, 0.f);
         if (EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R) w3 = *reinterpret_cast<const float4*>(g.aux3 + (col_ok ? col : 0));
         // row pointers of this lane for the chunk (row rbase + rsub, column col); rows advance by 4 per visit
         const int row0 = rbase + rsub;
         const size_t cco = col_ok ? (size_t)col : 0;
+        constexpr size_t EH = H16 ? 2 : 4;        // element size of the aux / out2 / prep tensors
+        const size_t ec = c16 ? 2 : 4;            // element size of C
 #pragma unroll 1
         for (int h = 0; h < 2; ++h) {
-        const int rowh = row0 + h * 16;
-        // (byte pointers: a tensor flagged in io16 has 2-byte elements in the H16 kernels)
-        const bool h1 = H16 && (g.io16 & IO16_AUX1), h2 = H16 && (g.io16 & IO16_AUX2), hz = H16 && (g.io16 & IO16_ZP);
-        const bool hc = H16 && (g.io16 & IO16_C), ho = H16 && (g.io16 & IO16_OUT2), hzb = H16 && (g.io16 & IO16_ZBP);
-        const size_t e1 = h1 ? 2 : 4, e2 = h2 ? 2 : 4, ez = hz ? 2 : 4, ec = hc ? 2 : 4, eo = ho ? 2 : 4, ezb = hzb ? 2 : 4;
-        const char* p1 = need1 ? reinterpret_cast<const char*>(g.aux1) + ((size_t)rowh * g.ld1 + cco) * e1 : nullptr;
-        const char* p2 = need2 ? reinterpret_cast<const char*>(g.aux2) + ((size_t)rowh * g.ld2 + cco) * e2 : nullptr;
-        const char* pz = PREP ? reinterpret_cast<const char*>(g.zp) + ((size_t)rowh * g.ldzp + cco) * ez : nullptr;
-        const size_t st1 = (size_t)4 * g.ld1 * e1, st2 = (size_t)4 * g.ld2 * e2, stz = (size_t)4 * g.ldzp * ez;
-        uint4 ax1[4], ax2[4], ax3[4];   // raw bits (fp32 x 4, or 16-bit x 4 in .x .y)
-        // per-row scalars (u, sigma, u of the prep stage) are prefetched with the aux rows: loaded at their point of use they
-        // were the top stall of the EPI_LATENT_LAST epilogue (ncu: long_scoreboard on the first multiply by u)
-        constexpr bool need_u = (EPI == EPI_SILU_U || EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R);
-        float ru[4], rs[4], rp[4];
+          const int rowh = row0 + h * 16;
+          const char* p1 = need1 ? reinterpret_cast<const char*>(g.aux1) + ((size_t)rowh * g.ld1 + cco) * EH : nullptr;
+          const char* p2 = need2 ? reinterpret_cast<const char*>(g.aux2) + ((size_t)rowh * g.ld2 + cco) * EH : nullptr;
+          const char* pz = PREP ? reinterpret_cast<const char*>(g.zp) + ((size_t)rowh * g.ldzp + cco) * EH : nullptr;
+          const size_t st1 = (size_t)4 * g.ld1 * EH, st2 = (size_t)4 * g.ld2 * EH, stz = (size_t)4 * g.ldzp * EH;
+          uint4 ax1[4], ax2[4], ax3[4];   // raw bits (fp32 x 4, or 16-bit x 4 in .x .y)
+          // per-row scalars (u, sigma, u of the prep stage) are prefetched with the aux rows: loaded at their point of use they
+          // were the top stall of the EPI_LATENT_LAST epilogue (ncu: long_scoreboard on the first multiply by u)
+          constexpr bool need_u = (EPI == EPI_SILU_U || EPI == EPI_LATENT || EPI == EPI_LATENT_LAST || EPI == EPI_ADD2R);
+          float ru[4], rs[4], rp[4];
 #pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-          const int i = h * 4 + ii;
-          const int row = rbase + i * 4 + rsub;
-          const bool ok = row < M && col_ok;
-          const int rowc = (row < M) ? row : M - 1;
-          ru[ii] = need_u ? g.u[rowc] : 0.f;
-          rs[ii] = (EPI == EPI_LATENT_LAST) ? g.sig[rowc] : 0.f;
-          rp[ii] = PREP ? g.pu[rowc] : 0.f;
-          ax1[ii] = (need1 && ok) ? ep_load<H16>(p1 + ii * st1, h1) : make_uint4(0u, 0u, 0u, 0u);
-          ax2[ii] = (need2 && ok) ? ep_load<H16>(p2 + ii * st2, h2) : make_uint4(0u, 0u, 0u, 0u);
-          ax3[ii] = (PREP && ok) ? ep_load<H16>(pz + ii * stz, hz) : make_uint4(0u, 0u, 0u, 0u);
-        }
-        char* qo = g.out2 ? reinterpret_cast<char*>(g.out2) + ((size_t)rowh * g.ldo2 + cco) * eo : nullptr;
-        char* qc = g.C ? reinterpret_cast<char*>(g.C) + ((size_t)rowh * g.ldc + cco) * ec : nullptr;
-        char* qz = PREP ? reinterpret_cast<char*>(g.zbp) + ((size_t)rowh * g.ldzbp + cco) * ezb : nullptr;
-        const size_t sto = (size_t)4 * g.ldo2 * eo, stc = (size_t)4 * g.ldc * ec, stzb = (size_t)4 * g.ldzbp * ezb;
-#pragma unroll
-        for (int ii = 0; ii < 4; ++ii) {
-          const int i = h * 4 + ii;
-          const int rl = i * 4 + rsub;
-          const int row = rbase + rl;
-          const float4 v4 = stg4[rl * 8 + ((lane & 7) ^ (rl & 7))];
-          float v[4] = {v4.x, v4.y, v4.z, v4.w};
-          if (EPI == EPI_LATENT_LAST) {
-            // all 32 lanes stay in step for the shuffles; out-of-range lanes contribute 0 and store nothing
+          for (int ii = 0; ii < 4; ++ii) {
+            const int row = rowh + ii * 4;
             const bool ok = row < M && col_ok;
-            const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
-            float4 x = AUX1(i);
-            const float4 w = w3;
-            const float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w.x, w.y, w.z, w.w};
-            const float us = ru[ii], sg = rs[ii];
-            float o[4], zb[4], up = 0.f, ep4 = 0.f;
-            const float cu = g.c1 * us, cus = cu * sg;
+            const int rowc = (row < M) ? row : M - 1;
+            ru[ii] = need_u ? g.u[rowc] : 0.f;
+            rs[ii] = (EPI == EPI_LATENT_LAST) ? g.sig[rowc] : 0.f;
+            rp[ii] = PREP ? g.pu[rowc] : 0.f;
+            ax1[ii] = need1 ? ep_load<HF>(p1 + ii * st1, ok) : make_uint4(0u, 0u, 0u, 0u);
+            ax2[ii] = need2 ? ep_load<HF>(p2 + ii * st2, ok) : make_uint4(0u, 0u, 0u, 0u);
+            ax3[ii] = PREP ? ep_load<HF>(pz + ii * stz, ok) : make_uint4(0u, 0u, 0u, 0u);
+          }
+          char* qo = out2 ? reinterpret_cast<char*>(g.out2) + ((size_t)rowh * g.ldo2 + cco) * EH : nullptr;
+          char* qc = reinterpret_cast<char*>(g.C) + ((size_t)rowh * g.ldc + cco) * ec;
+          char* qz = PREP ? reinterpret_cast<char*>(g.zbp) + ((size_t)rowh * g.ldzbp + cco) * EH : nullptr;
+          const size_t sto = (size_t)4 * g.ldo2 * EH, stc = (size_t)4 * g.ldc * ec, stzb = (size_t)4 * g.ldzbp * EH;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              // one sigmoid serves silu and silu'
-              const float sgm = sigm_f(v[j]);
-              const float sl = v[j] * sgm;
-              o[j] = fmaf(g.c0, xo[j], cu * sl);
-              zb[j] = cus * we[j] * (sgm * fmaf(v[j], 1.0f - sgm, 1.0f));
-              up = fmaf(we[j], sl, up);
-              ep4 = fmaf(o[j], we[j], ep4);     // 4 terms in fp32 (w_eff rounded to fp32), the rest of the sum in fp64
-            }
-            // 3xTF32 (fp32-accurate mode): the 8-lane sum of the 32-column energy partial runs in fp64; TF32 mode: in fp32
-            // (32 terms, error ~1e-7 relative, far below the TF32 operand rounding) -- the fp64 shuffles and adds were the
-            // heaviest part of this epilogue (ncu: 794 us at 3.0 TB/s, 3.8e8 warp instructions per launch at config 3)
-            typedef typename std::conditional<SPLIT, double, float>::type ep_t;
-            ep_t ep = ok ? (ep_t)ep4 : (ep_t)0;
-            if (!ok) up = 0.f;
-#pragma unroll
-            for (int off = 1; off < 8; off <<= 1) {
-              up += __shfl_xor_sync(0xffffffffu, up, off);
-              ep += __shfl_xor_sync(0xffffffffu, ep, off);
-            }
-            if (ok) {
-              ep_store<H16>(qo + ii * sto, make_float4(zb[0], zb[1], zb[2], zb[3]), ho, g.hfmt);
-              if (g.C) ep_store<H16>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), hc, g.hfmt);
-              if ((lane & 7) == 0) {
-                const int64_t p = (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
-                g.upart[p * g.part_stride + row] = g.c1 * sg * up;
-                g.epart[p * g.part_stride + row] = (double)ep;
-              }
-            }
-          } else if (PREP) {
-            // EPI_ADD2 / EPI_ADD2R followed by the z-bar / u-bar stage of the next MLP (all lanes stay in step)
-            const bool ok = row < M && col_ok;
-            const int rr = (row < M) ? row : M - 1, cc = col_ok ? col : 0;
+          for (int ii = 0; ii < 4; ++ii) {
+            const int rl = (h * 4 + ii) * 4 + rsub;
+            const int row = rbase + rl;
+            const bool ok = row < M && col_ok;          // out-of-range lanes compute on zeros and store nothing
+            const float4 v4 = lds128(stg + (uint32_t)(rl * 8 + ((lane & 7) ^ (rl & 7))) * 16);
+            const float v[4] = {v4.x, v4.y, v4.z, v4.w};
             float o[4];
-            const float4 y = AUX2(i);
-            if (EPI == EPI_ADD2) {
-              const float4 x = AUX1(i);
-              o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
-              o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
-            } else {
-              const float4 x = w3;
-              const float cs = g.c0 * ru[ii];
-              o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
-              o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
-            }
-            const float4 zq = ep_cvt<H16>(ax3[ii], hz, g.hfmt);
-            const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
-            const float cu = g.cp * rp[ii];
-            float zb[4], up = 0.f;
+            if (EPI == EPI_LATENT_LAST) {
+              const float4 x = ep_cvt<HF>(ax1[ii]);
+              const float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w3.x, w3.y, w3.z, w3.w};
+              const float us = ru[ii], sg = rs[ii];
+              float zb[4], up = 0.f, ep4 = 0.f;
+              const float cu = g.c1 * us, cus = cu * sg;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const float sgm = sigm_f(zz[j]);
-              up = fmaf(o[j], zz[j] * sgm, up);
-              zb[j] = cu * o[j] * (sgm * fmaf(zz[j], 1.0f - sgm, 1.0f));
-            }
-            if (!ok) up = 0.f;
-#pragma unroll
-            for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
-            if (ok) {
-              ep_store<H16>(qz + ii * stzb, make_float4(zb[0], zb[1], zb[2], zb[3]), hzb, g.hfmt);
-              if (g.C) ep_store<H16>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), hc, g.hfmt);
-              if ((lane & 7) == 0) {
-                const int64_t p = g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5);
-                g.upart[p * g.part_stride + row] = g.cp * up;
+              for (int j = 0; j < 4; ++j) {
+                // one sigmoid serves silu and silu' = sgm + silu (1 - sgm)
+                const float sgm = sigm_f(v[j]);
+                const float sl = v[j] * sgm;
+                o[j] = fmaf(g.c0, xo[j], cu * sl);
+                zb[j] = (cus * we[j]) * fmaf(-sl, sgm, sgm + sl);
+                up = fmaf(we[j], sl, up);
+                ep4 = fmaf(o[j], we[j], ep4);     // 4 terms in fp32 (w_eff rounded to fp32), the rest of the sum in fp64
               }
-            }
-          } else if (row < M && col_ok) {
-            float o[4];
-            switch (EPI) {
-              case EPI_SILU_BOTH:
-              case EPI_SILU_U:
-              case EPI_LATENT: {
-                ep_store<H16>(qo + ii * sto, make_float4(v[0], v[1], v[2], v[3]), ho, g.hfmt);
-                float us = (EPI == EPI_SILU_BOTH) ? 1.0f : ru[ii];
-                if (EPI == EPI_LATENT) {
-                  float4 x = AUX1(i);
-                  float xo[4] = {x.x, x.y, x.z, x.w};
+              // 3xTF32 (fp32-accurate mode): the 8-lane sum of the 32-column energy partial runs in fp64; TF32 mode: in fp32
+              // (32 terms, error ~1e-7 relative, far below the TF32 operand rounding) -- the fp64 shuffles and adds were the
+              // heaviest part of this epilogue (ncu: 794 us at 3.0 TB/s, 3.8e8 warp instructions per launch at config 3)
+              typedef typename std::conditional<SPLIT, double, float>::type ep_t;
+              ep_t ep = ok ? (ep_t)ep4 : (ep_t)0;
+              if (!ok) up = 0.f;
 #pragma unroll
-                  for (int j = 0; j < 4; ++j) o[j] = g.c0 * xo[j] + g.c1 * us * silu_f(v[j]);
-                } else {
-#pragma unroll
-                  for (int j = 0; j < 4; ++j) o[j] = us * silu_f(v[j]);
-                }
-              } break;
-              case EPI_MUL_DSILU: {
-                float4 z = AUX1(i);
-                float zz[4] = {z.x, z.y, z.z, z.w};
-#pragma unroll
-                for (int j = 0; j < 4; ++j) o[j] = v[j] * dsilu_f(zz[j]);
-              } break;
-              case EPI_ADD2: {
-                float4 x = AUX1(i);
-                float4 y = AUX2(i);
+              for (int off = 1; off < 8; off <<= 1) {
+                up += __shfl_xor_sync(0xffffffffu, up, off);
+                ep += __shfl_xor_sync(0xffffffffu, ep, off);
+              }
+              ep_store<HF>(qo + ii * sto, make_float4(zb[0], zb[1], zb[2], zb[3]), ok);
+              ep_store_c<HF>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), ok && haveC, c16);
+              const int64_t pi = ((int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5)) * g.part_stride + (ok ? row : 0);
+              ep_st_f32(g.upart + pi, g.c1 * sg * up, ok && (lane & 7) == 0);
+              ep_st_f64(g.epart + pi, (double)ep, ok && (lane & 7) == 0);
+            } else if (PREP) {
+              // EPI_ADD2 / EPI_ADD2R followed by the z-bar / u-bar stage of the next MLP
+              const float4 y = ep_cvt<HF>(ax2[ii]);
+              if (EPI == EPI_ADD2) {
+                const float4 x = ep_cvt<HF>(ax1[ii]);
                 o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
                 o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
-              } break;
-              case EPI_ADD2R: {
-                float4 x = w3;
-                float4 y = AUX2(i);
-                float cs = g.c0 * ru[ii];
-                o[0] = v[0] + cs * x.x + y.x; o[1] = v[1] + cs * x.y + y.y;
-                o[2] = v[2] + cs * x.z + y.z; o[3] = v[3] + cs * x.w + y.w;
-              } break;
-              default:
+              } else {
+                const float cs = g.c0 * ru[ii];
+                o[0] = v[0] + cs * w3.x + y.x; o[1] = v[1] + cs * w3.y + y.y;
+                o[2] = v[2] + cs * w3.z + y.z; o[3] = v[3] + cs * w3.w + y.w;
+              }
+              const float4 zq = ep_cvt<HF>(ax3[ii]);
+              const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
+              const float cu = g.cp * rp[ii];
+              float zb[4], up = 0.f;
 #pragma unroll
-                for (int j = 0; j < 4; ++j) o[j] = v[j];
+              for (int j = 0; j < 4; ++j) {
+                const float sgm = sigm_f(zz[j]);
+                const float sl = zz[j] * sgm;
+                up = fmaf(o[j], sl, up);
+                zb[j] = (cu * o[j]) * fmaf(-sl, sgm, sgm + sl);
+              }
+              if (!ok) up = 0.f;
+#pragma unroll
+              for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
+              ep_store<HF>(qz + ii * stzb, make_float4(zb[0], zb[1], zb[2], zb[3]), ok);
+              ep_store_c<HF>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), ok && haveC, c16);
+              const int64_t pi = (g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5)) * g.part_stride + (ok ? row : 0);
+              ep_st_f32(g.upart + pi, g.cp * up, ok && (lane & 7) == 0);
+            } else {
+              switch (EPI) {
+                case EPI_SILU_BOTH:
+                case EPI_SILU_U:
+                case EPI_LATENT: {
+                  ep_store<HF>(qo + ii * sto, v4, ok);
+                  const float us = (EPI == EPI_SILU_BOTH) ? 1.0f : ru[ii];
+                  if (EPI == EPI_LATENT) {
+                    const float4 x = ep_cvt<HF>(ax1[ii]);
+                    const float xo[4] = {x.x, x.y, x.z, x.w};
+                    const float cu = g.c1 * us;
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) o[j] = fmaf(g.c0, xo[j], cu * silu_f(v[j]));
+                  } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) o[j] = us * silu_f(v[j]);
+                  }
+                } break;
+                case EPI_MUL_DSILU: {
+                  const float4 z = ep_cvt<HF>(ax1[ii]);
+                  const float zz[4] = {z.x, z.y, z.z, z.w};
+#pragma unroll
+                  for (int j = 0; j < 4; ++j) o[j] = v[j] * dsilu_f(zz[j]);
+                } break;
+                case EPI_ADD2: {
+                  const float4 x = ep_cvt<HF>(ax1[ii]);
+                  const float4 y = ep_cvt<HF>(ax2[ii]);
+                  o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
+                  o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
+                } break;
+                case EPI_ADD2R: {
+                  const float4 y = ep_cvt<HF>(ax2[ii]);
+                  const float cs = g.c0 * ru[ii];
+                  o[0] = v[0] + cs * w3.x + y.x; o[1] = v[1] + cs * w3.y + y.y;
+                  o[2] = v[2] + cs * w3.z + y.z; o[3] = v[3] + cs * w3.w + y.w;
+                } break;
+                default:
+#pragma unroll
+                  for (int j = 0; j < 4; ++j) o[j] = v[j];
+              }
+              ep_store_c<HF>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), ok, c16);
             }
-            ep_store<H16>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), hc, g.hfmt);
           }
-        }
         }   // halves
         __syncwarp();
       }
@@ -659,7 +674,7 @@ int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   // 6/2/16 35.4 ms; L2 prefetch of the A tiles 4-12 k-blocks ahead (cp.async.bulk.prefetch.tensor) 33.3 ms; 2-CTA clusters with
   // every B (weight) stage loaded half by each CTA and multicast to both (L2 -> shared B traffic halved) 32.8 ms: correct, and
   // no faster -- dropped
-  GEMM_DISPATCH(4, 3, 16, false, false)
+  GEMM_DISPATCH(4, 3, 16, false, 0)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
@@ -685,7 +700,7 @@ int al_gemm_h16(allegro_model* m, const GemmArgs& g_in) {
   tmB2 = tmB;
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  GEMM_DISPATCH(4, 3, 16, false, true)
+  if (g.hfmt == 0) { GEMM_DISPATCH(4, 3, 16, false, 1) } else { GEMM_DISPATCH(4, 3, 16, false, 2) }
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
@@ -706,7 +721,7 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g_in) {
   AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, 1, &tmB2));
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  GEMM_DISPATCH(4, 2, 8, true, false)
+  GEMM_DISPATCH(4, 2, 8, true, 0)
   m->launches++;
   AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
