@@ -197,18 +197,23 @@ __device__ __forceinline__ uint32_t stg_fence(uint32_t a) {
 }
 
 // sigmoid = rcp.approx(1 + ex2.approx(-z log2 e)): the two MUFU operations and nothing else (__fdividef adds a range test and
-// two scaling multiplies per element that 1 + e^-z in [1, inf] never needs)
-__device__ __forceinline__ float sigm_f(float z) {
-  float e, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * -1.4426950408889634f));
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+// two scaling multiplies per element that 1 + e^-z in [1, inf] never needs); error ~1e-7 << TF32 rounding.
+// Packed fp32 pairs (FMUL2 / FADD2 / FFMA2 of sm_100): the epilogue of the fused kernels is bound by issue slots, not by the
+// fp32 pipe (ncu r2n: selected + not_selected 45 % of the warp samples, 13.5 scalar FMUL / FADD / FFMA per output element);
+// a packed instruction takes one slot for two elements.  Roundings are those of the scalar code (IEEE rn per operation).
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 sigm2(float2 z) {
+  const float2 t = __fmul2_rn(z, f2(-1.4426950408889634f));
+  float2 e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e.x) : "f"(t.x));
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e.y) : "f"(t.y));
+  const float2 d = __fadd2_rn(e, f2(1.0f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r.x) : "f"(d.x));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r.y) : "f"(d.y));
   return r;
 }
-__device__ __forceinline__ float silu_f(float z) { return z * sigm_f(z); }
-__device__ __forceinline__ float dsilu_f(float z) {
-  float s = sigm_f(z);
-  return s * fmaf(z, 1.0f - s, 1.0f);
-}
+// silu'(z) = s + silu(z) (1 - s) from s = sigmoid(z) and sl = z s
+__device__ __forceinline__ float2 dsilu2(float2 s, float2 sl) { return __ffma2_rn(sl, __ffma2_rn(s, f2(-1.0f), f2(1.0f)), s); }
 
 // round to the nearest TF32 value (10 explicit mantissa bits; ties away from zero), result exact in TF32 so the
 // MMA's own truncation of the operand is a no-op
@@ -446,24 +451,29 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             const int row = rbase + rl;
             const bool ok = row < M && col_ok;          // out-of-range lanes compute on zeros and store nothing
             const float4 v4 = lds128(stg + (uint32_t)(rl * 8 + ((lane & 7) ^ (rl & 7))) * 16);
-            const float v[4] = {v4.x, v4.y, v4.z, v4.w};
             float o[4];
             if (EPI == EPI_LATENT_LAST) {
               const float4 x = ep_cvt<HF>(ax1[ii]);
-              const float xo[4] = {x.x, x.y, x.z, x.w}, we[4] = {w3.x, w3.y, w3.z, w3.w};
               const float us = ru[ii], sg = rs[ii];
-              float zb[4], up = 0.f, ep4 = 0.f;
               const float cu = g.c1 * us, cus = cu * sg;
+              const float2 vv[2] = {make_float2(v4.x, v4.y), make_float2(v4.z, v4.w)};
+              const float2 xx[2] = {make_float2(x.x, x.y), make_float2(x.z, x.w)};
+              const float2 ww[2] = {make_float2(w3.x, w3.y), make_float2(w3.z, w3.w)};
+              float2 oo[2], zz2[2], up2 = f2(0.f), ep2 = f2(0.f);
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                // one sigmoid serves silu and silu' = sgm + silu (1 - sgm)
-                const float sgm = sigm_f(v[j]);
-                const float sl = v[j] * sgm;
-                o[j] = fmaf(g.c0, xo[j], cu * sl);
-                zb[j] = (cus * we[j]) * fmaf(-sl, sgm, sgm + sl);
-                up = fmaf(we[j], sl, up);
-                ep4 = fmaf(o[j], we[j], ep4);     // 4 terms in fp32 (w_eff rounded to fp32), the rest of the sum in fp64
+              for (int j = 0; j < 2; ++j) {
+                // one sigmoid serves silu and silu'
+                const float2 sgm = sigm2(vv[j]);
+                const float2 sl = __fmul2_rn(vv[j], sgm);
+                oo[j] = __ffma2_rn(f2(g.c0), xx[j], __fmul2_rn(f2(cu), sl));
+                zz2[j] = __fmul2_rn(__fmul2_rn(f2(cus), ww[j]), dsilu2(sgm, sl));
+                up2 = __ffma2_rn(ww[j], sl, up2);
+                ep2 = __ffma2_rn(oo[j], ww[j], ep2);     // 4 terms in fp32 (w_eff rounded to fp32), the rest of the sum in fp64
               }
+              o[0] = oo[0].x; o[1] = oo[0].y; o[2] = oo[1].x; o[3] = oo[1].y;
+              const float zb[4] = {zz2[0].x, zz2[0].y, zz2[1].x, zz2[1].y};
+              float up = up2.x + up2.y;
+              const float ep4 = ep2.x + ep2.y;
               // 3xTF32 (fp32-accurate mode): the 8-lane sum of the 32-column energy partial runs in fp64; TF32 mode: in fp32
               // (32 terms, error ~1e-7 relative, far below the TF32 operand rounding) -- the fp64 shuffles and adds were the
               // heaviest part of this epilogue (ncu: 794 us at 3.0 TB/s, 3.8e8 warp instructions per launch at config 3)
@@ -482,27 +492,36 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               ep_st_f64(g.epart + pi, (double)ep, ok && (lane & 7) == 0);
             } else if (PREP) {
               // EPI_ADD2 / EPI_ADD2R followed by the z-bar / u-bar stage of the next MLP
-              const float4 y = ep_cvt<HF>(ax2[ii]);
+              const float2 vv[2] = {make_float2(v4.x, v4.y), make_float2(v4.z, v4.w)};
+              float2 oo[2];
               if (EPI == EPI_ADD2) {
                 const float4 x = ep_cvt<HF>(ax1[ii]);
-                o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
-                o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
+                oo[0] = __ffma2_rn(f2(g.c0), make_float2(x.x, x.y), vv[0]);
+                oo[1] = __ffma2_rn(f2(g.c0), make_float2(x.z, x.w), vv[1]);
               } else {
                 const float cs = g.c0 * ru[ii];
-                o[0] = v[0] + cs * w3.x + y.x; o[1] = v[1] + cs * w3.y + y.y;
-                o[2] = v[2] + cs * w3.z + y.z; o[3] = v[3] + cs * w3.w + y.w;
+                oo[0] = __ffma2_rn(f2(cs), make_float2(w3.x, w3.y), vv[0]);
+                oo[1] = __ffma2_rn(f2(cs), make_float2(w3.z, w3.w), vv[1]);
+              }
+              if (need2) {
+                const float4 y = ep_cvt<HF>(ax2[ii]);
+                oo[0] = __fadd2_rn(oo[0], make_float2(y.x, y.y));
+                oo[1] = __fadd2_rn(oo[1], make_float2(y.z, y.w));
               }
               const float4 zq = ep_cvt<HF>(ax3[ii]);
-              const float zz[4] = {zq.x, zq.y, zq.z, zq.w};
+              const float2 zq2[2] = {make_float2(zq.x, zq.y), make_float2(zq.z, zq.w)};
               const float cu = g.cp * rp[ii];
-              float zb[4], up = 0.f;
+              float2 zz2[2], up2 = f2(0.f);
 #pragma unroll
-              for (int j = 0; j < 4; ++j) {
-                const float sgm = sigm_f(zz[j]);
-                const float sl = zz[j] * sgm;
-                up = fmaf(o[j], sl, up);
-                zb[j] = (cu * o[j]) * fmaf(-sl, sgm, sgm + sl);
+              for (int j = 0; j < 2; ++j) {
+                const float2 sgm = sigm2(zq2[j]);
+                const float2 sl = __fmul2_rn(zq2[j], sgm);
+                up2 = __ffma2_rn(oo[j], sl, up2);
+                zz2[j] = __fmul2_rn(__fmul2_rn(f2(cu), oo[j]), dsilu2(sgm, sl));
               }
+              o[0] = oo[0].x; o[1] = oo[0].y; o[2] = oo[1].x; o[3] = oo[1].y;
+              const float zb[4] = {zz2[0].x, zz2[0].y, zz2[1].x, zz2[1].y};
+              float up = up2.x + up2.y;
               if (!ok) up = 0.f;
 #pragma unroll
               for (int off = 1; off < 8; off <<= 1) up += __shfl_xor_sync(0xffffffffu, up, off);
@@ -511,6 +530,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               const int64_t pi = (g.pbase + (int64_t)nt * ((BN + 31) >> 5) + (c0 >> 5)) * g.part_stride + (ok ? row : 0);
               ep_st_f32(g.upart + pi, g.cp * up, ok && (lane & 7) == 0);
             } else {
+              const float2 vv[2] = {make_float2(v4.x, v4.y), make_float2(v4.z, v4.w)};
+              float2 oo[2];
               switch (EPI) {
                 case EPI_SILU_BOTH:
                 case EPI_SILU_U:
@@ -519,37 +540,44 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
                   const float us = (EPI == EPI_SILU_BOTH) ? 1.0f : ru[ii];
                   if (EPI == EPI_LATENT) {
                     const float4 x = ep_cvt<HF>(ax1[ii]);
-                    const float xo[4] = {x.x, x.y, x.z, x.w};
+                    const float2 xx[2] = {make_float2(x.x, x.y), make_float2(x.z, x.w)};
                     const float cu = g.c1 * us;
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) o[j] = fmaf(g.c0, xo[j], cu * silu_f(v[j]));
+                    for (int j = 0; j < 2; ++j)
+                      oo[j] = __ffma2_rn(f2(g.c0), xx[j], __fmul2_rn(f2(cu), __fmul2_rn(vv[j], sigm2(vv[j]))));
+                  } else if (EPI == EPI_SILU_U) {
+#pragma unroll
+                    for (int j = 0; j < 2; ++j) oo[j] = __fmul2_rn(f2(us), __fmul2_rn(vv[j], sigm2(vv[j])));
                   } else {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j) o[j] = us * silu_f(v[j]);
+                    for (int j = 0; j < 2; ++j) oo[j] = __fmul2_rn(vv[j], sigm2(vv[j]));
                   }
                 } break;
                 case EPI_MUL_DSILU: {
                   const float4 z = ep_cvt<HF>(ax1[ii]);
-                  const float zz[4] = {z.x, z.y, z.z, z.w};
+                  const float2 zq2[2] = {make_float2(z.x, z.y), make_float2(z.z, z.w)};
 #pragma unroll
-                  for (int j = 0; j < 4; ++j) o[j] = v[j] * dsilu_f(zz[j]);
+                  for (int j = 0; j < 2; ++j) {
+                    const float2 sgm = sigm2(zq2[j]);
+                    oo[j] = __fmul2_rn(vv[j], dsilu2(sgm, __fmul2_rn(zq2[j], sgm)));
+                  }
                 } break;
                 case EPI_ADD2: {
                   const float4 x = ep_cvt<HF>(ax1[ii]);
                   const float4 y = ep_cvt<HF>(ax2[ii]);
-                  o[0] = v[0] + g.c0 * x.x + y.x; o[1] = v[1] + g.c0 * x.y + y.y;
-                  o[2] = v[2] + g.c0 * x.z + y.z; o[3] = v[3] + g.c0 * x.w + y.w;
+                  oo[0] = __fadd2_rn(__ffma2_rn(f2(g.c0), make_float2(x.x, x.y), vv[0]), make_float2(y.x, y.y));
+                  oo[1] = __fadd2_rn(__ffma2_rn(f2(g.c0), make_float2(x.z, x.w), vv[1]), make_float2(y.z, y.w));
                 } break;
                 case EPI_ADD2R: {
                   const float4 y = ep_cvt<HF>(ax2[ii]);
                   const float cs = g.c0 * ru[ii];
-                  o[0] = v[0] + cs * w3.x + y.x; o[1] = v[1] + cs * w3.y + y.y;
-                  o[2] = v[2] + cs * w3.z + y.z; o[3] = v[3] + cs * w3.w + y.w;
+                  oo[0] = __fadd2_rn(__ffma2_rn(f2(cs), make_float2(w3.x, w3.y), vv[0]), make_float2(y.x, y.y));
+                  oo[1] = __fadd2_rn(__ffma2_rn(f2(cs), make_float2(w3.z, w3.w), vv[1]), make_float2(y.z, y.w));
                 } break;
                 default:
-#pragma unroll
-                  for (int j = 0; j < 4; ++j) o[j] = v[j];
+                  oo[0] = vv[0]; oo[1] = vv[1];
               }
+              o[0] = oo[0].x; o[1] = oo[0].y; o[2] = oo[1].x; o[3] = oo[1].y;
               ep_store_c<HF>(qc + ii * stc, make_float4(o[0], o[1], o[2], o[3]), ok, c16);
             }
           }
