@@ -180,6 +180,19 @@ int allegro_nve_kick(allegro_model* m, double* pos, double* vel, const double* f
 int allegro_kinetic_energy(allegro_model* m, const double* vel, const int32_t* species, const double* mass,
                            int64_t n_atoms, double* e_kin);
 
+/* allegro_kinetic_energy without any allocation, for callers that may not call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same arguments (device pointers), same fixed-order reduction and the same
+ * value as allegro_kinetic_energy; the per-atom scratch that call reserves with cudaMalloc lives here in a fixed __device__
+ * array of ALLEGRO_KINETIC_NOALLOC_MAX_ATOMS doubles (8 MiB, held by every GPU that loads the library until the process
+ * exits).  n_atoms beyond that limit: ALLEGRO_ERR_CAPACITY, nothing launched.  The model's device must be current
+ * (ALLEGRO_ERR_BAD_ARG otherwise).  The call never calls cudaMalloc / cudaFree or an allocating library routine; the kernels
+ * run on the model's stream.  Every call on a device shares the one array and nothing in it needs to start at zero (a call
+ * reads only what it wrote), so calls ordered on one stream are safe, while calls that OVERLAP on the GPU (other streams, other
+ * models on the same device) race on it and must be serialised by the caller.  (csrc/noalloc.cu) */
+#define ALLEGRO_KINETIC_NOALLOC_MAX_ATOMS 1048576
+int allegro_kinetic_energy_noalloc(allegro_model* m, const double* vel, const int32_t* species, const double* mass,
+                                   int64_t n_atoms, double* e_kin);
+
 /* allegro_step_nve replays the steps that do not rebuild the list from a CUDA graph: a step whose arguments, list and
  * configuration are those of the previous (eagerly run) step is captured once and relaunched as one graph from then on
  * (the small configs are launch-bound: ~36 kernels of a few microseconds each); any change of an argument, a rebuild, a

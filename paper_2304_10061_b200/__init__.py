@@ -74,7 +74,7 @@ EXPORTS = [
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
     "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps", "allegro_compute_local",
-    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32", "allegro_halo_pack", "allegro_halo_assemble", "allegro_halo_accumulate", "allegro_set_tensor_track",
+    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_kinetic_energy_noalloc", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32", "allegro_halo_pack", "allegro_halo_assemble", "allegro_halo_accumulate", "allegro_set_tensor_track",
     "allegro_last_error",
 ]
 
@@ -114,6 +114,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_step_nvt.argtypes = lib.allegro_step_nve.argtypes + [vp, C.c_double, C.c_double]
     lib.allegro_nve_kick.argtypes = [vp, vp, vp, vp, vp, vp, i64, C.c_double, i32]
     lib.allegro_kinetic_energy.argtypes = [vp, vp, vp, vp, i64, vp]
+    lib.allegro_kinetic_energy_noalloc.argtypes = [vp, vp, vp, vp, i64, vp]
     lib.allegro_compute_local.argtypes = [vp, vp, vp, i64, i64, P(C.c_double), vp, vp, vp, vp]
     lib.allegro_edge_energies.argtypes = [vp, vp, vp, i64, P(C.c_double), vp, vp, vp]
     lib.allegro_set_bessel_frequencies.argtypes = [vp, vp]
@@ -444,6 +445,13 @@ class Allegro:
         self._check(self._lib.allegro_kinetic_energy(self._h, vel.data_ptr(), species.data_ptr(), mass.data_ptr(),
                                                      vel.shape[0], ek.data_ptr()))
         return ek
+
+    def kinetic_energy_noalloc(self, vel, species, mass, out):
+        """allegro_kinetic_energy_noalloc: writes e_kin (eV) into `out` (CUDA float64 [1], the caller's); allocates nothing."""
+        self._sync_stream()
+        self._check(self._lib.allegro_kinetic_energy_noalloc(self._h, vel.data_ptr(), species.data_ptr(), mass.data_ptr(),
+                                                             vel.shape[0], out.data_ptr()))
+        return out
 
     def step_nvt(self, pos, vel, force, species, mass, box, dt_fs: float, rebuild_every: int, skin: float,
                  nbr: NeighborList, step_counter: C.c_int64, e_pot, e_kin, nh_state, t0_K: float, tau_fs: float):

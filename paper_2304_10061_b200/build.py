@@ -16,7 +16,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libb200allegro.so")
 # gen_tp_patterns.cpp is a build-time host tool, not part of the library
 SOURCES = ["model.cu", "cg_tables.cpp", "neighbors.cu", "edge_kernels.cu", "tp_kernels.cu", "tp2_kernels.cu",
-           "tp2_l3_fwd.cu", "tp2_l3_bwd.cu", "tpc_kernels.cu", "tpc_l3.cu", "gemm_simt.cu", "gemm_tc.cu", "compute.cu", "probe.cu", "halo.cu"]
+           "tp2_l3_fwd.cu", "tp2_l3_bwd.cu", "tpc_kernels.cu", "tpc_l3.cu", "gemm_simt.cu", "gemm_tc.cu", "compute.cu", "probe.cu", "halo.cu", "noalloc.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
