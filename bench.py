@@ -309,6 +309,8 @@ def main():
                          "(SURVEY.md section 8(d): config 1, 100 steps at 0.5 fs)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra-modes", action="store_true",
+                    help="skip the fp16-operand sub-record that the default (TF32, one GPU) run appends (~10 s)")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
     ap.add_argument("--decompose", action="store_true",
                     help="NEXT-3: ONE system split over the N GPUs by spatial domains with halo exchange (strong scaling) "
@@ -594,6 +596,40 @@ def main():
     }
     if drift is not None:
         out["nve_drift"] = drift
+    if rank == 0 and world == 1 and args.precision == 1 and not args.no_extra_modes and not args.decompose:
+        # The same K steps in the fp16-operand MLP mode (precision 4: 16-bit storage of the MLP-only tensors, fp32 accumulate,
+        # inside north_star's 2e-3 tolerance, tests/test_gpu_16bit.py) as a sub-record; the line above stays the TF32 one.
+        try:
+            del model, nb
+            chp4 = P.hparams_from(cfg.hp, 4)
+            m4 = P.Allegro(chp4, blob, chunk_edges=args.chunk_edges) if args.chunk_edges else P.Allegro(chp4, blob)
+            if cfg.hp.r_cut_pair is not None:
+                m4.set_pair_cutoffs(cfg.hp.r_cut_pair)
+            p4 = torch.from_numpy(pos.copy()).to(dev); v4 = torch.from_numpy(vel.copy()).to(dev)
+            nb4 = m4.neighbors(p4, box, cfg.hp.r_cut + cfg.skin)
+            e4, _, f4 = m4.compute(p4, s, box, nb4, want_atom_energies=False)
+            ek4 = torch.zeros(1, dtype=torch.float64, device=dev); c4 = ctypes.c_int64(0)
+            for _ in range(W):
+                m4.step_nve(p4, v4, f4, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb4, c4, e4, ek4)
+            torch.cuda.synchronize()
+            smp = ClockSampler(local_rank); smp.start()
+            a4, b4 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            l4 = m4.launches
+            a4.record()
+            for _ in range(K):
+                m4.step_nve(p4, v4, f4, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb4, c4, e4, ek4)
+            b4.record(); torch.cuda.synchronize()
+            smp.stop_flag = True
+            m4.status()
+            ms4 = a4.elapsed_time(b4)
+            out["extra_modes"] = {"fp16_operands": {
+                "precision_mode": 4, "dtype": DTYPE[4], "steps": K, "warmup": W, "ms_per_step": ms4 / K,
+                "value": N * K / (ms4 * 1e-3), "unit": unit, "gpu_launches": m4.launches - l4, "e_pot": float(e4.item()),
+                "clocks": smp.summary(),
+                "note": "same workload and step as the line; extra mode, not the paper's F32-activation / TF32-matmul scheme"}}
+            del m4
+        except P.AllegroError as ex:
+            out["extra_modes"] = {"fp16_operands": {"unavailable": str(ex)}}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         n_all, n_one = {0: (192, 192), 1: (3072, 768), 2: (512, 128), 3: (512, 128), 4: (256, 64)}[cfg.index]
         import torch as _t

@@ -899,8 +899,13 @@ int k_launch_edge_bwd(allegro_model* m, Work& w, const float* zb1, int ldz, cons
   (void)single;
   const int H = L0.fo;
   size_t sm = (size_t)(m->NB + EB_EDGES) * (H + 4) * sizeof(float);
-  static size_t sm_set = 0;
-  if (sm > sm_set) { AL_CUDA(m, cudaFuncSetAttribute(k_edge_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)); sm_set = sm; }
+  // per device: the opt-in is a property of the kernel on one device, and the size depends on the model (largest seen so far)
+  static std::atomic<size_t> sm_set[64];
+  std::atomic<size_t>& cur = sm_set[m->device & 63];
+  if (sm > cur.load(std::memory_order_acquire)) {
+    AL_CUDA(m, cudaFuncSetAttribute(k_edge_bwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm));
+    cur.store(sm, std::memory_order_release);
+  }
   int ypart0[AL_MAX_LAYERS + 1];
   const int n_yparts = al_ybar_layout(m, ypart0);
   k_edge_bwd<<<(unsigned)((m_cap + EB_EDGES - 1) / EB_EDGES), 256, sm, m->stream>>>(
