@@ -309,6 +309,8 @@ def main():
                          "(SURVEY.md section 8(d): config 1, 100 steps at 0.5 fs)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nvtx", action="store_true",
+                    help="NVTX range per kernel group around the library's launches (for `ncu --nvtx --nvtx-include \"gemm/\"`)")
     ap.add_argument("--no-extra-modes", action="store_true",
                     help="skip the fp16-operand sub-record that the default (TF32, one GPU) run appends (~10 s)")
     ap.add_argument("--chunk-edges", type=int, default=0, help="override the per-chunk edge budget (0 = library default)")
@@ -383,6 +385,8 @@ def main():
     model = P.Allegro(chp, blob, chunk_edges=args.chunk_edges) if args.chunk_edges else P.Allegro(chp, blob)
     if cfg.hp.r_cut_pair is not None:
         model.set_pair_cutoffs(cfg.hp.r_cut_pair)
+    if args.nvtx:
+        model.profile_enable(False, nvtx=True)
     dev = torch.device("cuda", local_rank)
     p = torch.from_numpy(pos.copy()).to(dev); v = torch.from_numpy(vel.copy()).to(dev)
     s = torch.from_numpy(sp).to(dev); mass = torch.from_numpy(masses_for(cfg)).to(dev)
@@ -477,11 +481,11 @@ def main():
     # ---- roofline of the dominant kernel group: one more pass of K steps with per-group CUDA events on the launching stream
     groups = ["gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd", "neighbors", "nve"]
     tp_bytes = tp_bytes_per_edge(cfg.hp)
-    model.profile_enable(True)
+    model.profile_enable(True, nvtx=args.nvtx)
     for _ in range(K):
         model.step_nve(p, v, f, s, mass, box, cfg.dt_fs, cfg.rebuild_every, cfg.skin, nb, ctr, e, ek)
     prof = {g: model.profile_read(g) for g in groups}
-    model.profile_enable(False)
+    model.profile_enable(False, nvtx=args.nvtx)
     tot_prof = sum(t for t, _ in prof.values())
     pk = peaks()
     gemm_ms, gemm_n = prof["gemm"]

@@ -214,7 +214,10 @@ int allegro_step_nve_host(allegro_model* m, double* pos, double* vel, double* fo
  * returns, for group `name` ("gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem",
  * "edge_bwd", "neighbors", "nve"), the summed milliseconds and the launch count since enable, plus for
  * "gemm" the summed algorithmic FLOPs (2*M*N*K with M the chunk's candidate-edge capacity is NOT used:
- * flops are computed by the caller from allegro_last_active_edges).  host pointers. */
+ * flops are computed by the caller from allegro_last_active_edges).  host pointers.
+ * `on` is a bit mask: 1 = the CUDA-event timing above; 2 = an NVTX range named after the group around the launches of every
+ * group (host side, header-only nvtx3: costs nothing without a tool attached), so a profiler can select a group, e.g.
+ * `ncu --nvtx --nvtx-include "tp_bwd/"`. */
 int allegro_profile_enable(allegro_model* m, int32_t on);
 int allegro_profile_read(allegro_model* m, const char* name, double* ms, int64_t* launches);
 

@@ -472,8 +472,9 @@ class Allegro:
                                                     float(skin), C.byref(nbr._h), C.byref(step_counter), ptr(e_pot),
                                                     ptr(e_kin)))
 
-    def profile_enable(self, on: bool):
-        self._check(self._lib.allegro_profile_enable(self._h, 1 if on else 0))
+    def profile_enable(self, on, nvtx: bool = False):
+        """allegro_profile_enable: CUDA-event timing per kernel group (`on`) and / or NVTX ranges per group (`nvtx`)."""
+        self._check(self._lib.allegro_profile_enable(self._h, (1 if on else 0) | (2 if nvtx else 0)))
 
     def profile_read(self, name: str):
         ms, n = C.c_double(0), C.c_int64(0)

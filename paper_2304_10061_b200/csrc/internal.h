@@ -147,6 +147,7 @@ struct allegro_model {
   // per-kernel-group event timing (allegro_profile_*)
   bool prof = false;
   struct ProfRec { int cat; cudaEvent_t a, b; };
+  bool nvtx = false;                      // allegro_profile_enable bit 1: NVTX range per kernel group (host side)
   std::vector<ProfRec> prof_recs;
   std::vector<cudaEvent_t> prof_pool;
   std::vector<void*> owned;               // device allocations made through al_alloc (weights/tables)
@@ -167,7 +168,7 @@ inline int al_next_rev(allegro_model* m) { return (int)(m->sweep_ctr++ & 1u); }
 enum ProfCat { PC_GEMM = 0, PC_TP_FWD, PC_TP_BWD, PC_GEOM, PC_TWOBODY0, PC_ENERGY, PC_BWD_ELEM, PC_EDGE_BWD, PC_NEIGHBORS,
                PC_NVE, PC_COUNT };
 struct ProfScope {
-  allegro_model* m; int cat; cudaEvent_t a = nullptr;
+  allegro_model* m; int cat; cudaEvent_t a = nullptr; bool range = false;
   ProfScope(allegro_model* m_, int cat_);
   ~ProfScope();
 };

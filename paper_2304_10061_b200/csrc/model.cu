@@ -1,5 +1,6 @@
 // Model construction: hyper-parameter checks, blob parsing, weight upload, tensor-track tables.
 // (SURVEY.md §8(b) boundary and blob layout; PAPER.md:222 for what the MLPs are.)
+#include <nvtx3/nvToolsExt.h>
 #include <cmath>
 #include <cstring>
 
@@ -434,22 +435,25 @@ static cudaEvent_t prof_event(allegro_model* m) {
   if (!m->prof_pool.empty()) { cudaEvent_t e = m->prof_pool.back(); m->prof_pool.pop_back(); return e; }
   cudaEvent_t e; cudaEventCreate(&e); return e;
 }
+static const char* kProfNames[PC_COUNT] = {"gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd",
+                                           "neighbors", "nve"};
+
 ProfScope::ProfScope(allegro_model* m_, int cat_) : m(m_), cat(cat_) {
+  if (m && m->nvtx) { nvtxRangePushA(kProfNames[cat]); range = true; }   // e.g. ncu --nvtx --nvtx-include "gemm/"
   if (m && m->prof) { a = prof_event(m); cudaEventRecord(a, m->stream); }
 }
 ProfScope::~ProfScope() {
   if (a) { cudaEvent_t b = prof_event(m); cudaEventRecord(b, m->stream); m->prof_recs.push_back({cat, a, b}); }
+  if (range) nvtxRangePop();
 }
-
-static const char* kProfNames[PC_COUNT] = {"gemm", "tp_fwd", "tp_bwd", "geom", "twobody0", "energy", "bwd_elem", "edge_bwd",
-                                           "neighbors", "nve"};
 
 extern "C" int allegro_profile_enable(allegro_model* m, int32_t on) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   cudaStreamSynchronize(m->stream);
   for (auto& r : m->prof_recs) { m->prof_pool.push_back(r.a); m->prof_pool.push_back(r.b); }
   m->prof_recs.clear();
-  m->prof = on != 0;
+  m->prof = (on & 1) != 0;
+  m->nvtx = (on & 2) != 0;
   m->config_gen++;
   return ALLEGRO_OK;
 }

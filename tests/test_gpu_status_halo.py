@@ -73,3 +73,21 @@ def test_peak_probes_are_plausible():
     pk = model.probe_peaks(0.2)
     assert 30.0 < pk["ffma"]["burst"] < 90.0            # 148 SMs x 128 lanes x 2 x 1.965 GHz = 74.4 TFLOP/s
     assert 500.0 < pk["tf32_mma"]["burst"] < 1300.0     # nominal dense TF32 ~1.1 PFLOP/s
+
+
+def test_profile_groups_with_nvtx_ranges():
+    """allegro_profile_enable bit mask: 1 = CUDA-event timing per kernel group, 2 = NVTX range per group.  The ranges are host-side
+    markers (visible to a profiler only); here: both bits on, the result is unchanged and the group timers still fill."""
+    cfg = scaled_config(1, 768)
+    pos, sp, box = make_system(cfg)
+    model, _ = make_both(cfg, precision=1)
+    p = torch.from_numpy(pos).cuda(); s = torch.from_numpy(sp.astype(np.int32)).cuda()
+    nb = model.neighbors(p, box, cfg.hp.r_cut)
+    e0, _, f0 = model.compute(p, s, box, nb)
+    model.profile_enable(True, nvtx=True)
+    e1, _, f1 = model.compute(p, s, box, nb)
+    ms, n = model.profile_read("gemm")
+    model.profile_enable(False)
+    assert n > 0 and ms > 0.0
+    assert float(e0.item()) == float(e1.item())
+    assert (f0 - f1).abs().max().item() <= 1e-12 * f0.abs().max().item()
