@@ -74,7 +74,7 @@ EXPORTS = [
     "allegro_step_nve", "allegro_step_nve_host", "allegro_profile_enable", "allegro_profile_read",
     "allegro_launch_count", "allegro_last_active_edges", "allegro_set_debug", "allegro_set_pair_cutoffs", "allegro_debug_tensor",
     "allegro_set_bessel_frequencies", "allegro_set_zbl", "allegro_edge_energies", "allegro_step_nvt", "allegro_graph_steps", "allegro_compute_local",
-    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_kinetic_energy_noalloc", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32", "allegro_halo_pack", "allegro_halo_assemble", "allegro_halo_accumulate", "allegro_set_tensor_track",
+    "allegro_nve_kick", "allegro_kinetic_energy", "allegro_kinetic_energy_noalloc", "allegro_status", "allegro_probe_ffma", "allegro_probe_tf32", "allegro_halo_pack", "allegro_halo_assemble", "allegro_halo_accumulate", "allegro_set_tensor_track", "allegro_set_gemm_pairs",
     "allegro_last_error",
 ]
 
@@ -127,6 +127,7 @@ def load_library(path: Optional[str] = None) -> C.CDLL:
     lib.allegro_debug_tensor.argtypes = [vp, C.c_char_p, vp, P(i64)]
     lib.allegro_status.argtypes = [vp]
     lib.allegro_set_tensor_track.argtypes = [vp, i32]
+    lib.allegro_set_gemm_pairs.argtypes = [vp, i32]
     lib.allegro_halo_pack.argtypes = [vp, vp, vp, vp, vp, i64, vp]
     lib.allegro_halo_assemble.argtypes = [vp, vp, vp, i64, vp, i64, P(C.c_double), vp, vp]
     lib.allegro_halo_accumulate.argtypes = [vp, vp, i64, vp, vp, i64, vp]
@@ -471,6 +472,10 @@ class Allegro:
                                                     pos.shape[0], _box3(box), float(dt_fs), int(rebuild_every),
                                                     float(skin), C.byref(nbr._h), C.byref(step_counter), ptr(e_pot),
                                                     ptr(e_kin)))
+
+    def set_gemm_pairs(self, pairs: bool):
+        """allegro_set_gemm_pairs: MLP GEMMs on CTA pairs (256-row tiles, the default for large launches) or on single CTAs."""
+        self._check(self._lib.allegro_set_gemm_pairs(self._h, 1 if pairs else 0))
 
     def profile_enable(self, on, nvtx: bool = False):
         """allegro_profile_enable: CUDA-event timing per kernel group (`on`) and / or NVTX ranges per group (`nvtx`)."""

@@ -30,12 +30,13 @@ constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
 // the lo parts are each <= 2^-24 relative: the same order as one fp32 rounding).  B_hi / B_lo are prepared at create time; four "splitter" warps turn each landed A
 // stage into A_hi (in place) and A_lo (second buffer) before the MMA warp may read it.
 __host__ __device__ constexpr int bn_max(bool split) { return split ? 128 : 256; }
-__host__ __device__ constexpr uint32_t b_stage_bytes(bool split) { return bn_max(split) * BKF * 4; }   // allocated for the largest BN
+// CG = 2 (cta_group::2): a pair of CTAs works on one 256-row tile; each loads its own 128 rows of A and HALF of the B tile
+__host__ __device__ constexpr uint32_t b_stage_bytes(bool split, int cg = 1) { return bn_max(split) / cg * BKF * 4; }   // allocated for the largest BN
 __host__ __device__ constexpr uint32_t a_ring_stage(bool split) { return (split ? 2 : 1) * A_STAGE_BYTES; }
-__host__ __device__ constexpr uint32_t b_ring_stage(bool split) { return (split ? 2 : 1) * b_stage_bytes(split); }
+__host__ __device__ constexpr uint32_t b_ring_stage(bool split, int cg = 1) { return (split ? 2 : 1) * b_stage_bytes(split, cg); }
 // epilogue transpose staging: one 32x32 fp32 tile per warp, float4-granular XOR swizzle (conflict-free both ways)
-constexpr uint32_t smem_bytes(int ast, int bst, int epi_warps, bool split) {
-  return ast * a_ring_stage(split) + bst * b_ring_stage(split) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
+constexpr uint32_t smem_bytes(int ast, int bst, int epi_warps, bool split, int cg = 1) {
+  return ast * a_ring_stage(split) + bst * b_ring_stage(split, cg) + 1024 /*align*/ + 256 /*barriers*/ + epi_warps * 32 * 32 * 4;
 }
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -91,6 +92,61 @@ __device__ __forceinline__ void tc_mma_f16(uint32_t tmem_d, uint64_t da, uint64_
       ".reg .pred p;\n\t"
       "setp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+// ---- cta_group::2: two CTAs of a cluster (one TPC) run one MMA of M = 256.  Only the leader (cluster rank 0) issues MMAs and
+// commits; its full barriers collect the TMA bytes of both CTAs; commits arrive on the barriers of both (multicast).
+__device__ __forceinline__ uint32_t cluster_rank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t mapa_leader(uint32_t addr) {     // the same shared-memory offset in the CTA of rank 0
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(0));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_cluster(uint32_t cluster_addr, uint32_t bytes) {
+  // (default .release.cta semantics: with .release.cluster every arrive costs a MEMBAR + ERRBAR in the producer's loop)
+  asm volatile("mbarrier.arrive.expect_tx.shared::cluster.b64 _, [%0], %1;" ::"r"(cluster_addr), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_cg2(void* smem_dst, const CUtensorMap* tm, uint32_t bar_cluster_addr, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(tm), "r"(bar_cluster_addr), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void tc_commit_cg2(uint64_t* bar) {   // arrives on `bar` at the same offset in both CTAs
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+                   smem_u32(bar)),
+               "h"((uint16_t)3)
+               : "memory");
+}
+__device__ __forceinline__ void tc_mma_tf32_cg2(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::tf32 [%0], %1, %2, %3, p;\n\t"
+      "}" ::"r"(tmem_d),
+      "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void tc_mma_f16_cg2(uint32_t tmem_d, uint64_t da, uint64_t db, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n\t"
+      ".reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
       "}" ::"r"(tmem_d),
       "l"(da), "l"(db), "r"(idesc), "r"(accumulate)
       : "memory");
@@ -223,13 +279,20 @@ __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__fl
 // so the epilogue carries no run-time dispatch, no dead operands and no re-loaded argument fields.
 // HF = 1 / 2 (precision 4 / 2): A and B operands are fp16 / bf16 in HBM, one stage = 64 K-elements (the same
 // 128-byte rows), tcgen05.mma.kind::f16 with fp32 accumulation; every epilogue tensor is 16-bit too, C only if GemmArgs::io16 has IO16_C.
-template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, int HF = 0>
+// CG = 2: the kernel is launched in clusters of two CTAs (cta_group::2).  A pair owns 256-row tiles: CTA rank r loads rows
+// [256 t + 128 r, +128) of A and rows [BN r / 2, +BN / 2) of the B tile, the leader issues one M = 256 MMA per k-slice, each
+// CTA's TMEM receives its own 128 rows of the accumulator and each CTA runs the epilogue of its rows.  The weights cross the
+// L2 -> SM fabric once per 256 rows instead of once per 128: with 128-row tiles every large GEMM of the step ran at the
+// ~13.5 TB/s the L2 slices deliver to the SMs (A twice for the two column tiles + B per tile, B = 2 x A per k-slice), not
+// at an HBM limit (profiles/r2o_summary.md).
+template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, int HF = 0, int CG = 1>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
             const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
+  static_assert(CG == 1 || (CG == 2 && !SPLIT), "cta_group::2 is built for the non-split modes");
   constexpr int BN_MAX = bn_max(SPLIT);
-  constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT);
-  constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT);
+  constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT, CG);
+  constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT, CG);
   constexpr int EW0 = SPLIT ? 7 : 3;     // first epilogue warp (warps 3..6 are the splitter in SPLIT mode)
   constexpr bool H16 = HF != 0;              // HF = 1: IEEE fp16, 2: bfloat16 operands and epilogue tensors
   constexpr int BKE = H16 ? 2 * BKF : BKF;   // K elements per stage
@@ -257,22 +320,32 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int M = *g.m_ptr;
-  const int num_mt = (M + BM - 1) / BM;
+  const int rank = (CG == 2) ? (int)cluster_rank() : 0;       // position in the CTA pair
+  const int num_mt = (M + BM * CG - 1) / (BM * CG);           // row blocks of 128 CG rows
   const int num_tiles = num_mt * ntn;
   const int num_kb = (g.K + BKE - 1) / BKE;
+  const int tile0 = blockIdx.x / CG, tile_step = gridDim.x / CG;   // both CTAs of a pair walk the same tiles
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < AST; ++s) { mbar_init(&fullA[s], 1); mbar_init(&emptyA[s], 1); mbar_init(&readyA[s], 4); }
-    for (int s = 0; s < BST; ++s) { mbar_init(&fullB[s], 1); mbar_init(&emptyB[s], 1); }
-    for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], EPI_WARPS); }
+    // CG = 2: the leader's full barriers take one expect_tx arrival per CTA, its accumulator-empty barriers one arrival
+    // per epilogue warp of both CTAs; the empty / accumulator-full barriers of each CTA are hit by the multicast commits
+    for (int s = 0; s < AST; ++s) { mbar_init(&fullA[s], CG); mbar_init(&emptyA[s], 1); mbar_init(&readyA[s], 4); }
+    for (int s = 0; s < BST; ++s) { mbar_init(&fullB[s], CG); mbar_init(&emptyB[s], 1); }
+    for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], EPI_WARPS * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (CG == 2) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(tmem_slot)) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   tc_fence_before();
   __syncthreads();
+  if (CG == 2) cluster_sync_all();     // the peer's barriers are initialised before anything arrives on them
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
@@ -281,14 +354,22 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       const int kb1 = g.A2 ? g.K1 / BKE : num_kb;   // k-blocks [kb1, num_kb) come from the second activation tensor
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = tile0; tile < num_tiles; tile += tile_step) {
         int mt = tile / ntn;
         if (g.rev) mt = num_mt - 1 - mt;
+        const int row = (mt * CG + rank) * BM;      // (past M for the odd last block of a pair: TMA fills zeros)
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyA[stage], phase ^ 1);
-          mbar_expect_tx(&fullA[stage], A_STAGE_BYTES);
-          if (kb < kb1) tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKE, mt * BM);
-          else tma_load_2d(sA(stage), &tmA2, &fullA[stage], (kb - kb1) * BKE, mt * BM);
+          if (CG == 2) {
+            const uint32_t fb = mapa_leader(smem_u32(&fullA[stage]));
+            mbar_expect_tx_cluster(fb, A_STAGE_BYTES);
+            if (kb < kb1) tma_load_2d_cg2(sA(stage), &tmA, fb, kb * BKE, row);
+            else tma_load_2d_cg2(sA(stage), &tmA2, fb, (kb - kb1) * BKE, row);
+          } else {
+            mbar_expect_tx(&fullA[stage], A_STAGE_BYTES);
+            if (kb < kb1) tma_load_2d(sA(stage), &tmA, &fullA[stage], kb * BKE, row);
+            else tma_load_2d(sA(stage), &tmA2, &fullA[stage], (kb - kb1) * BKE, row);
+          }
           if (++stage == AST) { stage = 0; phase ^= 1; }
         }
       }
@@ -297,27 +378,33 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // ===== TMA producer, B ring =====
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      const uint32_t bytes = (SPLIT ? 2u : 1u) * (uint32_t)BN * BKF * 4;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      const uint32_t bytes = (SPLIT ? 2u : 1u) * (uint32_t)(BN / CG) * BKF * 4;
+      for (int tile = tile0; tile < num_tiles; tile += tile_step) {
         int mt = tile / ntn, nt = tile - mt * ntn;
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyB[stage], phase ^ 1);
-          mbar_expect_tx(&fullB[stage], bytes);
-          tma_load_2d(sB(stage), &tmB, &fullB[stage], kb * BKE, nt * BN);
-          if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &fullB[stage], kb * BKE, nt * BN);
+          if (CG == 2) {
+            const uint32_t fb = mapa_leader(smem_u32(&fullB[stage]));
+            mbar_expect_tx_cluster(fb, bytes);
+            tma_load_2d_cg2(sB(stage), &tmB, fb, kb * BKE, nt * BN + rank * (BN / 2));
+          } else {
+            mbar_expect_tx(&fullB[stage], bytes);
+            tma_load_2d(sB(stage), &tmB, &fullB[stage], kb * BKE, nt * BN);
+            if (SPLIT) tma_load_2d(sBlo(stage), &tmB2, &fullB[stage], kb * BKE, nt * BN);
+          }
           if (++stage == BST) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
     // ===== MMA issuer =====
-    if (lane == 0) {
-      // instruction descriptor: D=f32, A=B=tf32, K-major both, N>>3, M>>4
+    if (lane == 0 && rank == 0) {     // (CG = 2: the leader issues for the pair)
+      // instruction descriptor: D=f32, A=B=tf32, K-major both, N>>3, M>>4 (M = 256 across the pair for CG = 2)
       // (A / B format field: 2 = tf32 for kind::tf32; kind::f16: 0 = f16, 1 = bf16)
       const uint32_t ofmt = H16 ? (uint32_t)(HF - 1) : 2u;
-      const uint32_t idesc = (1u << 4) | (ofmt << 7) | (ofmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+      const uint32_t idesc = (1u << 4) | (ofmt << 7) | (ofmt << 10) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)((BM * CG) >> 4) << 24);
       int sa = 0, sb = 0; uint32_t pa = 0, pb = 0; int it = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+      for (int tile = tile0; tile < num_tiles; tile += tile_step, ++it) {
         int acc = it & 1;
         mbar_wait(&tempty[acc], ((it >> 1) & 1) ^ 1);
         tc_fence_after();
@@ -330,8 +417,13 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
           uint64_t db = make_desc(smem_u32(sB(sb)));
 #pragma unroll
           for (int k = 0; k < BKF / 8; ++k) {   // UMMA_K = 8 tf32 or 16 halves = 32 bytes -> +2 in the (addr >> 4) field
-            if (H16) tc_mma_f16(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
-            else tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+            if (CG == 2) {
+              if (H16) tc_mma_f16_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+              else tc_mma_tf32_cg2(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+            } else {
+              if (H16) tc_mma_f16(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+              else tc_mma_tf32(d_tmem, da + 2 * k, db + 2 * k, idesc, (kb | k) ? 1u : 0u);
+            }
           }
           if (SPLIT) {
             uint64_t dal = make_desc(smem_u32(sAlo(sa)));
@@ -342,19 +434,19 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
               tc_mma_tf32(d_tmem, dal + 2 * k, db + 2 * k, idesc, 1u);    // A_lo * B_hi
             }
           }
-          tc_commit(&emptyA[sa]);
-          tc_commit(&emptyB[sb]);
+          if (CG == 2) { tc_commit_cg2(&emptyA[sa]); tc_commit_cg2(&emptyB[sb]); }
+          else { tc_commit(&emptyA[sa]); tc_commit(&emptyB[sb]); }
           if (++sa == AST) { sa = 0; pa ^= 1; }
           if (++sb == BST) { sb = 0; pb ^= 1; }
         }
-        tc_commit(&tfull[acc]);
+        if (CG == 2) tc_commit_cg2(&tfull[acc]); else tc_commit(&tfull[acc]);
       }
     }
   } else if (SPLIT && warp < EW0) {
     // ===== splitter warps (3xTF32): A -> A_hi (in place, low 13 mantissa bits cleared) and A_lo = A - A_hi =====
     const int t = threadIdx.x - 96;       // 0..127
     int stage = 0; uint32_t phase = 0;
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    for (int tile = tile0; tile < num_tiles; tile += tile_step) {
       for (int kb = 0; kb < num_kb; ++kb) {
         mbar_wait(&fullA[stage], phase);
         float4* pa = reinterpret_cast<float4*>(sA(stage));
@@ -377,9 +469,10 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
     // ===== epilogue warps =====
     const int q = warp & 3;   // TMEM lane quarter
     int it = 0;
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x, ++it) {
+    for (int tile = tile0; tile < num_tiles; tile += tile_step, ++it) {
       int mt = tile / ntn, nt = tile - mt * ntn;
       if (g.rev) mt = num_mt - 1 - mt;
+      mt = mt * CG + rank;                 // this CTA's 128-row block
       int acc = it & 1;
       mbar_wait(&tfull[acc], (it >> 1) & 1);
       tc_fence_after();
@@ -586,14 +679,19 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&tempty[acc]);
+      if (lane == 0) {
+        if (CG == 2) mbar_arrive_cluster(mapa_leader(smem_u32(&tempty[acc])));
+        else mbar_arrive(&tempty[acc]);
+      }
     }
   }
   tc_fence_before();
   __syncthreads();
+  if (CG == 2) cluster_sync_all();     // both CTAs are done with the pair's TMEM and with each other's barriers
   if (warp == 1) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+    if (CG == 2) asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
+    else asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base) : "memory");
   }
 }
 
@@ -647,68 +745,103 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 
 }  // namespace
 
-#define GEMM_LAUNCH(AS, BS, EW, SP, EP, PR, A2, H6)                                                                        \
+#define GEMM_LAUNCH(AS, BS, EW, SP, EP, PR, A2, H6, CG_)                                                                  \
   {                                                                                                                      \
-    static_assert(smem_bytes(AS, BS, EW, SP) <= 232448, "shared memory budget (227 KB)");                                \
+    static_assert(smem_bytes(AS, BS, EW, SP, CG_) <= 232448, "shared memory budget (227 KB)");                           \
     static AttrOnce once;                                                                                                \
     if (once.need(m->device)) {                                                                                          \
-      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
-                                      (int)smem_bytes(AS, BS, EW, SP)));                                                 \
+      AL_CUDA(m, cudaFuncSetAttribute(k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6, CG_>,                                  \
+                                      cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes(AS, BS, EW, SP, CG_))); \
       once.done(m->device);                                                                                              \
     }                                                                                                                    \
-    k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6><<<grid, 96 + (SP ? 128 : 0) + 32 * EW, smem_bytes(AS, BS, EW, SP), m->stream>>>( \
-        tmA, tmA2, tmB, tmB2, g, BN, ntn);                                                                               \
+    cudaLaunchConfig_t lc = {};                                                                                          \
+    lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3(96 + (SP ? 128 : 0) + 32 * EW);                                \
+    lc.dynamicSmemBytes = smem_bytes(AS, BS, EW, SP, CG_); lc.stream = m->stream;                                        \
+    cudaLaunchAttribute la[1];                                                                                           \
+    la[0].id = cudaLaunchAttributeClusterDimension;                                                                      \
+    la[0].val.clusterDim.x = CG_; la[0].val.clusterDim.y = 1; la[0].val.clusterDim.z = 1;                                \
+    lc.attrs = la; lc.numAttrs = 1;                                                                                      \
+    if (CG_ == 2) {                                                                                                      \
+      /* persistent pairs: never more clusters than the device can hold at once (a GPC with an odd SM count leaves one   \
+         SM without a partner), or the tiles of the late clusters would run as a second wave */                          \
+      static int max_pairs[64] = {};                                                                                     \
+      int& mp = max_pairs[m->device & 63];                                                                               \
+      if (mp == 0) {                                                                                                     \
+        int nc = 0;                                                                                                      \
+        AL_CUDA(m, cudaOccupancyMaxActiveClusters(&nc, k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6, CG_>, &lc));          \
+        mp = nc > 0 ? nc : -1;                                                                                           \
+      }                                                                                                                  \
+      if (mp < 0) { al_set_error(m, "gemm: no CTA pair fits on this device"); return ALLEGRO_ERR_CUDA; }                 \
+      if (grid > 2 * mp) lc.gridDim = dim3((unsigned)(2 * mp));                                                          \
+    }                                                                                                                    \
+    AL_CUDA(m, cudaLaunchKernelEx(&lc, k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6, CG_>, tmA, tmA2, tmB, tmB2, g, BN, ntn)); \
   }
 // one instantiation per epilogue (PREP only exists for the two x-bar epilogues)
-#define GEMM_DISPATCH(AS, BS, EW, SP, H6)                                                                                  \
+#define GEMM_DISPATCH(AS, BS, EW, SP, H6, CG_)                                                                            \
   switch (g.epi) {                                                                                                       \
-    case EPI_PLAIN: GEMM_LAUNCH(AS, BS, EW, SP, EPI_PLAIN, false, false, H6) break;                                                 \
-    case EPI_SILU_BOTH: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_BOTH, false, false, H6) break;                                         \
-    case EPI_SILU_U: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_U, false, false, H6) break;                                               \
-    case EPI_LATENT: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT, false, false, H6) break;                                               \
-    case EPI_MUL_DSILU: GEMM_LAUNCH(AS, BS, EW, SP, EPI_MUL_DSILU, false, false, H6) break;                                         \
-    case EPI_LATENT_LAST: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT_LAST, false, false, H6) break;                                     \
+    case EPI_PLAIN: GEMM_LAUNCH(AS, BS, EW, SP, EPI_PLAIN, false, false, H6, CG_) break;                                 \
+    case EPI_SILU_BOTH: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_BOTH, false, false, H6, CG_) break;                         \
+    case EPI_SILU_U: GEMM_LAUNCH(AS, BS, EW, SP, EPI_SILU_U, false, false, H6, CG_) break;                               \
+    case EPI_LATENT: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT, false, false, H6, CG_) break;                               \
+    case EPI_MUL_DSILU: GEMM_LAUNCH(AS, BS, EW, SP, EPI_MUL_DSILU, false, false, H6, CG_) break;                         \
+    case EPI_LATENT_LAST: GEMM_LAUNCH(AS, BS, EW, SP, EPI_LATENT_LAST, false, false, H6, CG_) break;                     \
     case EPI_ADD2:                                                                                                       \
-      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, true, H6)                                            \
-      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, false, H6)                                                \
-      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, true, H6)                                                \
-      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, false, H6)                                                           \
+      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, true, H6, CG_)                                   \
+      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, true, false, H6, CG_)                                       \
+      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, true, H6, CG_)                                       \
+      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2, false, false, H6, CG_)                                                  \
       break;                                                                                                             \
     case EPI_ADD2R:                                                                                                      \
-      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, true, H6)                                           \
-      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, false, H6)                                               \
-      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, true, H6)                                               \
-      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, false, H6)                                                          \
+      if (g.prep && g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, true, H6, CG_)                                  \
+      else if (g.prep) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, true, false, H6, CG_)                                      \
+      else if (g.aux2) GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, true, H6, CG_)                                      \
+      else GEMM_LAUNCH(AS, BS, EW, SP, EPI_ADD2R, false, false, H6, CG_)                                                 \
       break;                                                                                                             \
     default: al_set_error(m, "gemm: unknown epilogue"); return ALLEGRO_ERR_BAD_ARG;                                      \
   }
+
+// Tile geometry shared by the non-split launchers.  CTA pairs (cta_group::2, 256-row tiles) whenever the problem has at least
+// one pair tile per pair of SMs; small problems keep 128-row tiles (twice as many tiles to spread over the SMs).
+struct TileGeom { int ntn, BN, cg, grid; };
+static TileGeom tile_geom(const allegro_model* m, const GemmArgs& g) {
+  TileGeom t;
+  t.ntn = (g.N + bn_max(false) - 1) / bn_max(false);
+  t.BN = ((g.N + t.ntn - 1) / t.ntn + 15) & ~15;
+  const int sms = m->sm_count & ~1;
+  const int pair_tiles = ((g.m_cap + 2 * BM - 1) / (2 * BM)) * t.ntn;
+  t.cg = (m->gemm_cta_pairs && pair_tiles * 2 >= sms && sms >= 2) ? 2 : 1;
+  if (t.cg == 2) t.grid = sms;
+  else {
+    const int tiles_cap = ((g.m_cap + BM - 1) / BM) * t.ntn;
+    t.grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
+  }
+  return t;
+}
 
 // precision 1: TF32 operands (rounded to nearest by the TMA load), fp32 accumulation
 int al_gemm_tc(allegro_model* m, const GemmArgs& g_in) {
   GemmArgs g = g_in;
   g.rev = al_next_rev(m);
-  int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
-  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  const TileGeom t = tile_geom(m, g);
+  const int ntn = t.ntn, BN = t.BN, grid = t.grid;
   CUtensorMap tmA, tmA2, tmB, tmB2;
   AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, 0, &tmA));
   if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, 0, &tmA2));
   else tmA2 = tmA;
-  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN, 0, &tmB));
+  AL_CHECK(get_tmap(m, g.Bt, g.N, g.K, g.ldb, BN / t.cg, 0, &tmB));
   tmB2 = tmB;
-  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
-  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  // A/B ring depths 4/3; 6/2 and 3/3 measured within 1 % of it (the rings are not the limiter)
-  // round 2, config 2 (GEMM group per step), A stages / B stages / epilogue warps: 4/3/16 32.5 ms, 5/3/12 33.9 ms, 6/3/8 37.3 ms,
-  // 6/2/16 35.4 ms; L2 prefetch of the A tiles 4-12 k-blocks ahead (cp.async.bulk.prefetch.tensor) 33.3 ms; 2-CTA clusters with
-  // every B (weight) stage loaded half by each CTA and multicast to both (L2 -> shared B traffic halved) 32.8 ms: correct, and
-  // no faster -- dropped
-  GEMM_DISPATCH(4, 3, 16, false, 0)
+  // Ring depths, 128-row tiles: A 4 x 16 KB, B 3 x 32 KB (6/2 and 3/3 within 1 %; round 2, config 2, GEMM group per step,
+  // A stages / B stages / epilogue warps: 4/3/16 32.5 ms, 5/3/12 33.9 ms, 6/3/8 37.3 ms, 6/2/16 35.4 ms; L2 prefetch of the A
+  // tiles 4-12 k-blocks ahead 33.3 ms; B stages multicast inside 2-CTA clusters (still cta_group::1) 32.8 ms: the multicast
+  // does not cut L2 traffic below cluster size 8).  CTA pairs: each CTA holds half of every B stage (16 KB), the shared
+  // memory that frees deepens the rings to A 6 / B 4.
+  if (t.cg == 2) { GEMM_DISPATCH(6, 4, 16, false, 0, 2) }
+  else { GEMM_DISPATCH(4, 3, 16, false, 0, 1) }
   m->launches++;
-  AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
 }
 
-// precision 2: 16-bit operands (fp16 or bf16, g.hfmt) in HBM, tcgen05.mma.kind::f16, fp32 accumulation
+// precision 2 / 4: 16-bit operands (fp16 or bf16, g.hfmt) in HBM, tcgen05.mma.kind::f16, fp32 accumulation
 int al_gemm_h16(allegro_model* m, const GemmArgs& g_in) {
   GemmArgs g = g_in;
   g.rev = al_next_rev(m);
@@ -718,19 +851,20 @@ int al_gemm_h16(allegro_model* m, const GemmArgs& g_in) {
     return ALLEGRO_ERR_BAD_HPARAMS;
   }
   const int kind = 2 + (g.hfmt ? 1 : 0);
-  int ntn = (g.N + bn_max(false) - 1) / bn_max(false);
-  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  const TileGeom t = tile_geom(m, g);
+  const int ntn = t.ntn, BN = t.BN, grid = t.grid;
   CUtensorMap tmA, tmA2, tmB, tmB2;
   AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, kind, &tmA));
   if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, kind, &tmA2));
   else tmA2 = tmA;
-  AL_CHECK(get_tmap(m, g.Bt16, g.N, g.K, g.ldb, BN, kind, &tmB));
+  AL_CHECK(get_tmap(m, g.Bt16, g.N, g.K, g.ldb, BN / t.cg, kind, &tmB));
   tmB2 = tmB;
-  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
-  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  if (g.hfmt == 0) { GEMM_DISPATCH(4, 3, 16, false, 1) } else { GEMM_DISPATCH(4, 3, 16, false, 2) }
+  if (t.cg == 2) {
+    if (g.hfmt == 0) { GEMM_DISPATCH(6, 4, 16, false, 1, 2) } else { GEMM_DISPATCH(6, 4, 16, false, 2, 2) }
+  } else {
+    if (g.hfmt == 0) { GEMM_DISPATCH(4, 3, 16, false, 1, 1) } else { GEMM_DISPATCH(4, 3, 16, false, 2, 1) }
+  }
   m->launches++;
-  AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
 }
 
@@ -749,9 +883,8 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g_in) {
   AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, 1, &tmB2));
   int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
   int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  GEMM_DISPATCH(4, 2, 8, true, 0)
+  GEMM_DISPATCH(4, 2, 8, true, 0, 1)
   m->launches++;
-  AL_CUDA(m, cudaGetLastError());
   return ALLEGRO_OK;
 }
 #undef GEMM_DISPATCH

@@ -147,6 +147,7 @@ struct allegro_model {
   // per-kernel-group event timing (allegro_profile_*)
   bool prof = false;
   struct ProfRec { int cat; cudaEvent_t a, b; };
+  bool gemm_cta_pairs = true;            // MLP GEMMs on CTA pairs (cta_group::2, 256-row tiles) when the problem is large enough
   bool nvtx = false;                      // allegro_profile_enable bit 1: NVTX range per kernel group (host side)
   std::vector<ProfRec> prof_recs;
   std::vector<cudaEvent_t> prof_pool;

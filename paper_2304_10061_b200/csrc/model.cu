@@ -447,6 +447,13 @@ ProfScope::~ProfScope() {
   if (range) nvtxRangePop();
 }
 
+extern "C" int allegro_set_gemm_pairs(allegro_model* m, int32_t pairs) {
+  if (!m) return ALLEGRO_ERR_BAD_ARG;
+  m->gemm_cta_pairs = pairs != 0;
+  m->config_gen++;          // a captured step graph holds the old launch shapes
+  return ALLEGRO_OK;
+}
+
 extern "C" int allegro_profile_enable(allegro_model* m, int32_t on) {
   if (!m) return ALLEGRO_ERR_BAD_ARG;
   cudaStreamSynchronize(m->stream);

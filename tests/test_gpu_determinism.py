@@ -31,3 +31,22 @@ def test_run_to_run(ci, n, precision):
         assert E == E0                                   # bit-identical
         assert np.array_equal(Ea, Ea0)                   # bit-identical per-atom energies
         assert np.abs(F - F0).max() <= 1e-12 * fmax      # fp64 atomics: order-dependent round-off only
+
+
+@pytest.mark.parametrize("ci,n,precision", [(2, 20000, 1), (2, 20000, 4), (4, 6000, 1), (1, 12288, 2)])
+def test_cta_pairs_match_single_cta_tiles(ci, n, precision):
+    """allegro_set_gemm_pairs: the MLP GEMMs on CTA pairs (cta_group::2, 256-row tiles, the default for large launches) and on
+    single CTAs (128-row tiles) accumulate over K in the same order, so energies are bit-identical and forces agree to the
+    round-off of their fp64 atomics.  Sizes chosen so that every launch is large enough for the pair path (ragged last tiles,
+    odd numbers of 128-row blocks included: 20,000 / 6,000 atoms give chunk sizes that are not multiples of 256)."""
+    cfg = scaled_config(ci, n)
+    pos, sp, box = make_system(cfg)
+    out = []
+    for pairs in (False, True):
+        model, _ = make_both(cfg, precision=precision, chunk_edges=150001)
+        model.set_gemm_pairs(pairs)
+        out.append(gpu_eval(model, pos, sp, box, cutoff=cfg.hp.r_cut + 0.5)[0])
+    (E0, Ea0, F0), (E1, Ea1, F1) = out
+    assert E0 == E1
+    assert np.array_equal(Ea0, Ea1)
+    assert np.abs(F0 - F1).max() <= 1e-12 * np.abs(F0).max()
