@@ -284,7 +284,7 @@ __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__fl
 // CTA's TMEM receives its own 128 rows of the accumulator and each CTA runs the epilogue of its rows.  The weights cross the
 // L2 -> SM fabric once per 256 rows instead of once per 128: with 128-row tiles every large GEMM of the step ran at the
 // ~13.5 TB/s the L2 slices deliver to the SMs (A twice for the two column tiles + B per tile, B = 2 x A per k-slice), not
-// at an HBM limit (profiles/r2o_summary.md).
+// at an HBM limit (profiles/r2r_summary.md).
 template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, int HF = 0, int CG = 1>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
