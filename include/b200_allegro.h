@@ -212,7 +212,7 @@ int allegro_step_nve_host(allegro_model* m, double* pos, double* vel, double* fo
 /* Tile shape of the tensor-core MLP GEMMs.  pairs != 0 (the default): launches large enough to give every pair of SMs a tile run
  * on CTA pairs (thread-block clusters of 2, tcgen05 cta_group::2): 256-row tiles, each CTA loads its 128 rows of the activations
  * and half of the weight tile, so the weights cross L2 -> SM once per 256 rows.  pairs == 0: 128-row tiles on single CTAs
- * everywhere (what small launches and the 3xTF32 mode always use).  Same arithmetic either way (the accumulation order over K
+ * everywhere (what small launches always use).  Same arithmetic either way (the accumulation order over K
  * is identical); meant for tests and A/B timing.  Host call, takes effect at the next launch. */
 int allegro_set_gemm_pairs(allegro_model* m, int32_t pairs);
 

@@ -29,9 +29,11 @@ constexpr uint32_t A_STAGE_BYTES = BM * BKF * 4;           // 16 KB
 // lo = rn_tf32(x - hi), and  A*B ~= A_hi*B_hi + A_hi*B_lo + A_lo*B_hi  (the dropped lo*lo term and the rounding of
 // the lo parts are each <= 2^-24 relative: the same order as one fp32 rounding).  B_hi / B_lo are prepared at create time; four "splitter" warps turn each landed A
 // stage into A_hi (in place) and A_lo (second buffer) before the MMA warp may read it.
-__host__ __device__ constexpr int bn_max(bool split) { return split ? 128 : 256; }
+// widest column tile: the accumulator is double-buffered in 512 TMEM columns -> 256; the 3xTF32 mode on single CTAs keeps
+// 128 (its weight stage holds B_hi and B_lo); on CTA pairs each CTA holds half a weight stage and 256 fits there too
+__host__ __device__ constexpr int bn_max(bool split, int cg = 1) { return (split && cg == 1) ? 128 : 256; }
 // CG = 2 (cta_group::2): a pair of CTAs works on one 256-row tile; each loads its own 128 rows of A and HALF of the B tile
-__host__ __device__ constexpr uint32_t b_stage_bytes(bool split, int cg = 1) { return bn_max(split) / cg * BKF * 4; }   // allocated for the largest BN
+__host__ __device__ constexpr uint32_t b_stage_bytes(bool split, int cg = 1) { return bn_max(split, cg) / cg * BKF * 4; }   // allocated for the largest BN
 __host__ __device__ constexpr uint32_t a_ring_stage(bool split) { return (split ? 2 : 1) * A_STAGE_BYTES; }
 __host__ __device__ constexpr uint32_t b_ring_stage(bool split, int cg = 1) { return (split ? 2 : 1) * b_stage_bytes(split, cg); }
 // epilogue transpose staging: one 32x32 fp32 tile per warp, float4-granular XOR swizzle (conflict-free both ways)
@@ -289,8 +291,8 @@ template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool 
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
             const __grid_constant__ CUtensorMap tmB, const __grid_constant__ CUtensorMap tmB2, GemmArgs g, int BN, int ntn) {
-  static_assert(CG == 1 || (CG == 2 && !SPLIT), "cta_group::2 is built for the non-split modes");
-  constexpr int BN_MAX = bn_max(SPLIT);
+  static_assert(CG == 1 || CG == 2, "CTA group size");
+  constexpr int BN_MAX = bn_max(SPLIT, CG);
   constexpr uint32_t A_RING_STAGE = a_ring_stage(SPLIT), B_RING_STAGE = b_ring_stage(SPLIT, CG);
   constexpr uint32_t B_STAGE_BYTES = b_stage_bytes(SPLIT, CG);
   constexpr int EW0 = SPLIT ? 7 : 3;     // first epilogue warp (warps 3..6 are the splitter in SPLIT mode)
@@ -329,7 +331,8 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
   if (threadIdx.x == 0) {
     // CG = 2: the leader's full barriers take one expect_tx arrival per CTA, its accumulator-empty barriers one arrival
     // per epilogue warp of both CTAs; the empty / accumulator-full barriers of each CTA are hit by the multicast commits
-    for (int s = 0; s < AST; ++s) { mbar_init(&fullA[s], CG); mbar_init(&emptyA[s], 1); mbar_init(&readyA[s], 4); }
+    // (3xTF32 on pairs: A lands on the CTA's own full barrier, its splitter warps hand the stage to the leader's ready barrier)
+    for (int s = 0; s < AST; ++s) { mbar_init(&fullA[s], SPLIT ? 1 : CG); mbar_init(&emptyA[s], 1); mbar_init(&readyA[s], 4 * CG); }
     for (int s = 0; s < BST; ++s) { mbar_init(&fullB[s], CG); mbar_init(&emptyB[s], 1); }
     for (int s = 0; s < 2; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], EPI_WARPS * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -360,7 +363,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         const int row = (mt * CG + rank) * BM;      // (past M for the odd last block of a pair: TMA fills zeros)
         for (int kb = 0; kb < num_kb; ++kb) {
           mbar_wait(&emptyA[stage], phase ^ 1);
-          if (CG == 2) {
+          if (CG == 2 && !SPLIT) {
             const uint32_t fb = mapa_leader(smem_u32(&fullA[stage]));
             mbar_expect_tx_cluster(fb, A_STAGE_BYTES);
             if (kb < kb1) tma_load_2d_cg2(sA(stage), &tmA, fb, kb * BKE, row);
@@ -387,6 +390,7 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             const uint32_t fb = mapa_leader(smem_u32(&fullB[stage]));
             mbar_expect_tx_cluster(fb, bytes);
             tma_load_2d_cg2(sB(stage), &tmB, fb, kb * BKE, nt * BN + rank * (BN / 2));
+            if (SPLIT) tma_load_2d_cg2(sBlo(stage), &tmB2, fb, kb * BKE, nt * BN + rank * (BN / 2));
           } else {
             mbar_expect_tx(&fullB[stage], bytes);
             tma_load_2d(sB(stage), &tmB, &fullB[stage], kb * BKE, nt * BN);
@@ -430,8 +434,13 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
             uint64_t dbl = make_desc(smem_u32(sBlo(sb)));
 #pragma unroll
             for (int k = 0; k < BKF / 8; ++k) {
-              tc_mma_tf32(d_tmem, da + 2 * k, dbl + 2 * k, idesc, 1u);    // A_hi * B_lo
-              tc_mma_tf32(d_tmem, dal + 2 * k, db + 2 * k, idesc, 1u);    // A_lo * B_hi
+              if (CG == 2) {
+                tc_mma_tf32_cg2(d_tmem, da + 2 * k, dbl + 2 * k, idesc, 1u);    // A_hi * B_lo
+                tc_mma_tf32_cg2(d_tmem, dal + 2 * k, db + 2 * k, idesc, 1u);    // A_lo * B_hi
+              } else {
+                tc_mma_tf32(d_tmem, da + 2 * k, dbl + 2 * k, idesc, 1u);    // A_hi * B_lo
+                tc_mma_tf32(d_tmem, dal + 2 * k, db + 2 * k, idesc, 1u);    // A_lo * B_hi
+              }
             }
           }
           if (CG == 2) { tc_commit_cg2(&emptyA[sa]); tc_commit_cg2(&emptyB[sb]); }
@@ -461,7 +470,10 @@ k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUt
         // generic-proxy writes -> visible to the async proxy (tcgen05.mma reads shared memory through it)
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
-        if (lane == 0) mbar_arrive(&readyA[stage]);
+        if (lane == 0) {
+          if (CG == 2) mbar_arrive_cluster(mapa_leader(smem_u32(&readyA[stage])));
+          else mbar_arrive(&readyA[stage]);
+        }
         if (++stage == AST) { stage = 0; phase ^= 1; }
       }
     }
@@ -803,15 +815,26 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
 // Tile geometry shared by the non-split launchers.  CTA pairs (cta_group::2, 256-row tiles) whenever the problem has at least
 // one pair tile per pair of SMs; small problems keep 128-row tiles (twice as many tiles to spread over the SMs).
 struct TileGeom { int ntn, BN, cg, grid; };
-static TileGeom tile_geom(const allegro_model* m, const GemmArgs& g) {
+static void tile_cols(int N, int bnmax, int* ntn, int* BN) {
+  *ntn = (N + bnmax - 1) / bnmax;
+  *BN = ((N + *ntn - 1) / *ntn + 15) & ~15;
+}
+static TileGeom tile_geom(const allegro_model* m, const GemmArgs& g, bool split = false) {
   TileGeom t;
-  t.ntn = (g.N + bn_max(false) - 1) / bn_max(false);
-  t.BN = ((g.N + t.ntn - 1) / t.ntn + 15) & ~15;
   const int sms = m->sm_count & ~1;
+  tile_cols(g.N, bn_max(split, 2), &t.ntn, &t.BN);
   const int pair_tiles = ((g.m_cap + 2 * BM - 1) / (2 * BM)) * t.ntn;
   t.cg = (m->gemm_cta_pairs && pair_tiles * 2 >= sms && sms >= 2) ? 2 : 1;
+  if (split && t.cg == 2) {
+    // the row-partial buffers of the fused epilogues are indexed by 32-column chunk and sized for the single-CTA tiling
+    // (al_gemm_tc_row_parts): the pair tiling may be used only where both tilings number the chunks alike
+    int n1, b1;
+    tile_cols(g.N, bn_max(true, 1), &n1, &b1);
+    if ((b1 & 31) || (t.BN & 31)) t.cg = 1;
+  }
   if (t.cg == 2) t.grid = sms;
   else {
+    tile_cols(g.N, bn_max(split, 1), &t.ntn, &t.BN);
     const int tiles_cap = ((g.m_cap + BM - 1) / BM) * t.ntn;
     t.grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
   }
@@ -873,17 +896,18 @@ int al_gemm_tc3(allegro_model* m, const GemmArgs& g_in) {
   GemmArgs g = g_in;
   g.rev = al_next_rev(m);
   if (!g.Bt_hi || !g.Bt_lo) { al_set_error(m, "3xTF32 GEMM: split weights missing"); return ALLEGRO_ERR_BAD_ARG; }
-  int ntn = (g.N + bn_max(true) - 1) / bn_max(true);
-  int BN = ((g.N + ntn - 1) / ntn + 15) & ~15;
+  const TileGeom t = tile_geom(m, g, true);
+  const int ntn = t.ntn, BN = t.BN, grid = t.grid;
   CUtensorMap tmA, tmA2, tmB, tmB2;
   AL_CHECK(get_tmap(m, g.A, g.m_cap, g.A2 ? g.K1 : g.K, g.lda, BM, 1, &tmA));
   if (g.A2) AL_CHECK(get_tmap(m, g.A2, g.m_cap, g.K - g.K1, g.lda2, BM, 1, &tmA2));
   else tmA2 = tmA;
-  AL_CHECK(get_tmap(m, g.Bt_hi, g.N, g.K, g.ldb, BN, 1, &tmB));
-  AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN, 1, &tmB2));
-  int tiles_cap = ((g.m_cap + BM - 1) / BM) * ntn;
-  int grid = tiles_cap < m->sm_count ? tiles_cap : m->sm_count;
-  GEMM_DISPATCH(4, 2, 8, true, 0, 1)
+  AL_CHECK(get_tmap(m, g.Bt_hi, g.N, g.K, g.ldb, BN / t.cg, 1, &tmB));
+  AL_CHECK(get_tmap(m, g.Bt_lo, g.N, g.K, g.ldb, BN / t.cg, 1, &tmB2));
+  // pairs: 256-column tiles (each CTA holds 128 rows of B_hi and of B_lo per stage: the shared-memory layout of the single-CTA
+  // kernel), weights cross L2 -> SM once per 256 rows and the activations twice instead of four times
+  if (t.cg == 2) { GEMM_DISPATCH(4, 2, 8, true, 0, 2) }
+  else { GEMM_DISPATCH(4, 2, 8, true, 0, 1) }
   m->launches++;
   return ALLEGRO_OK;
 }

@@ -33,7 +33,7 @@ def test_run_to_run(ci, n, precision):
         assert np.abs(F - F0).max() <= 1e-12 * fmax      # fp64 atomics: order-dependent round-off only
 
 
-@pytest.mark.parametrize("ci,n,precision", [(2, 20000, 1), (2, 20000, 4), (4, 6000, 1), (1, 12288, 2)])
+@pytest.mark.parametrize("ci,n,precision", [(2, 20000, 1), (2, 20000, 4), (4, 6000, 1), (1, 12288, 2), (2, 20000, 0), (4, 6000, 0)])
 def test_cta_pairs_match_single_cta_tiles(ci, n, precision):
     """allegro_set_gemm_pairs: the MLP GEMMs on CTA pairs (cta_group::2, 256-row tiles, the default for large launches) and on
     single CTAs (128-row tiles) accumulate over K in the same order, so energies are bit-identical and forces agree to the
