@@ -1,13 +1,17 @@
-// tcgen05 tensor-core GEMM for the edge-batched MLPs (precision modes 1/2; "TF32 for
-// matrix multiplications", Table IV).  sm_100a only: TMA (cp.async.bulk.tensor) stages K-major 128B-
-// swizzled operand tiles in shared memory, one elected thread issues tcgen05.mma.kind::tf32 with the
-// fp32 accumulator in TMEM (double-buffered, 2 x 256 columns), four epilogue warps read it back with
-// tcgen05.ld and apply the fused epilogue (SiLU / envelope / residual / SiLU') before storing fp32.
+// tcgen05 tensor-core GEMM for the edge-batched MLPs (precision modes 0 / 1 / 2 / 4; "TF32 for matrix
+// multiplications", Table IV).  sm_100a only: TMA (cp.async.bulk.tensor) stages K-major 128B-swizzled operand tiles in shared
+// memory (two rings: A = activations from HBM, B = weights from L2), one elected thread issues tcgen05.mma (kind::tf32, or
+// kind::f16 for 16-bit operand storage) with the fp32 accumulator in TMEM (double-buffered, 2 x 256 columns), sixteen epilogue
+// warps read it back with tcgen05.ld, transpose 32 x 32 blocks through shared memory into a coalesced domain and apply one of
+// the fused epilogues (SiLU / envelope / residual / SiLU' / energy and z-bar of the last layer / x-bar accumulation with the
+// next layer's z-bar) before storing.
 //
-//   C[M,N] = epi( A[M,K] * Bt[N,K]^T ),  A and Bt row-major (K contiguous) fp32 in HBM.
+//   C[M,N] = epi( A[M,K] * Bt[N,K]^T ),  A and Bt row-major (K contiguous) in HBM; K may be the concatenation of two A tensors.
 //
-// Warp roles: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM alloc), warps 2.. = epilogue (TMEM
-// lane quarter = warp_id % 4, EPI_WARPS/4 warps per quarter taking alternate 32-column chunks).  Persistent CTAs, static tile schedule, n fastest.
+// Warp roles: warp 0 = TMA producer of A, warp 2 = TMA producer of B, warp 1 = MMA issuer (+ TMEM alloc), (3xTF32: warps 3-6
+// split every landed A stage into hi / lo parts,) the remaining warps = epilogue (TMEM lane quarter = warp_id % 4, EPI_WARPS / 4
+// warps per quarter taking alternate 32-column chunks).  Persistent CTAs, static tile schedule, n fastest.  Large launches run
+// on CTA pairs (clusters of two, cta_group::2, 256-row tiles): see the comment above the kernel.
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
