@@ -309,6 +309,8 @@ def main():
                          "(SURVEY.md section 8(d): config 1, 100 steps at 0.5 fs)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--gemm-pairs", type=int, default=1, choices=[0, 1],
+                    help="MLP GEMMs on CTA pairs (tcgen05 cta_group::2, the default) or on single CTAs: allegro_set_gemm_pairs")
     ap.add_argument("--nvtx", action="store_true",
                     help="NVTX range per kernel group around the library's launches (for `ncu --nvtx --nvtx-include \"gemm/\"`)")
     ap.add_argument("--no-extra-modes", action="store_true",
@@ -385,6 +387,8 @@ def main():
     model = P.Allegro(chp, blob, chunk_edges=args.chunk_edges) if args.chunk_edges else P.Allegro(chp, blob)
     if cfg.hp.r_cut_pair is not None:
         model.set_pair_cutoffs(cfg.hp.r_cut_pair)
+    if not args.gemm_pairs:
+        model.set_gemm_pairs(False)
     if args.nvtx:
         model.profile_enable(False, nvtx=True)
     dev = torch.device("cuda", local_rank)

@@ -288,9 +288,9 @@ __device__ __forceinline__ float tf32_rn(float x) { return __uint_as_float((__fl
 // CG = 2: the kernel is launched in clusters of two CTAs (cta_group::2).  A pair owns 256-row tiles: CTA rank r loads rows
 // [256 t + 128 r, +128) of A and rows [BN r / 2, +BN / 2) of the B tile, the leader issues one M = 256 MMA per k-slice, each
 // CTA's TMEM receives its own 128 rows of the accumulator and each CTA runs the epilogue of its rows.  The weights cross the
-// L2 -> SM fabric once per 256 rows instead of once per 128: with 128-row tiles every large GEMM of the step ran at the
-// ~13.5 TB/s the L2 slices deliver to the SMs (A twice for the two column tiles + B per tile, B = 2 x A per k-slice), not
-// at an HBM limit (profiles/r2r_summary.md).
+// L2 -> SM fabric once per 256 rows instead of once per 128: with 128-row tiles the 13 GEMM launches of a config-3 chunk moved
+// 62 GB from L2 to the SMs (weights = 2 x the activation bytes per k-slice) for 32 GB of DRAM traffic, the two heaviest at the
+// ~12 TB/s the fabric delivers; pairs move 47 GB (profiles/r2r_summary.md).
 template <int AST, int BST, int EPI_WARPS, bool SPLIT, int EPI, bool PREP, bool AUX2, int HF = 0, int CG = 1>
 __global__ void __launch_bounds__(96 + (SPLIT ? 128 : 0) + 32 * EPI_WARPS, 1)
 k_gemm_tf32(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmA2,
