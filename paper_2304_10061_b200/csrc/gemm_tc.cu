@@ -780,12 +780,13 @@ int get_tmap(allegro_model* m, const void* ptr, long long rows, long long K, lon
     if (CG_ == 2) {                                                                                                      \
       /* persistent pairs: never more clusters than the device can hold at once (a GPC with an odd SM count leaves one   \
          SM without a partner), or the tiles of the late clusters would run as a second wave */                          \
-      static int max_pairs[64] = {};                                                                                     \
-      int& mp = max_pairs[m->device & 63];                                                                               \
+      static std::atomic<int> max_pairs[64];                                                                             \
+      int mp = max_pairs[m->device & 63].load(std::memory_order_acquire);                                                \
       if (mp == 0) {                                                                                                     \
         int nc = 0;                                                                                                      \
         AL_CUDA(m, cudaOccupancyMaxActiveClusters(&nc, k_gemm_tf32<AS, BS, EW, SP, EP, PR, A2, H6, CG_>, &lc));          \
         mp = nc > 0 ? nc : -1;                                                                                           \
+        max_pairs[m->device & 63].store(mp, std::memory_order_release);                                                  \
       }                                                                                                                  \
       if (mp < 0) { al_set_error(m, "gemm: no CTA pair fits on this device"); return ALLEGRO_ERR_CUDA; }                 \
       if (grid > 2 * mp) lc.gridDim = dim3((unsigned)(2 * mp));                                                          \
