@@ -21,6 +21,14 @@ __device__ __forceinline__ float4 ek_ld4(const float* p) {
 #define FULLMASK 0xffffffffu
 
 __device__ __forceinline__ float silu_f(float z) { return z / (1.0f + expf(-z)); }
+// tensor-core modes (TF32 / 16-bit operands): the value feeds a TF32 / fp16 MMA operand, ex2.approx + rcp.approx (error ~1e-7)
+// is far below its rounding; the fp32 modes keep expf and the IEEE division
+__device__ __forceinline__ float silu_fast(float z) {
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(z * -1.4426950408889634f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + e));
+  return z * r;
+}
 __device__ __forceinline__ float dsilu_f(float z) {
   float s = 1.0f / (1.0f + expf(-z));
   return s * (1.0f + z * (1.0f - s));
@@ -202,7 +210,8 @@ __global__ void __launch_bounds__(256)
 k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int* __restrict__ ej,
            const int32_t* __restrict__ species, const float* __restrict__ B, const float* __restrict__ u,
            const float* __restrict__ W, int S, int NB, int H, float* __restrict__ z, float* __restrict__ act, int ldact,
-           int scale_u, int hfmt /* -1: fp32 outputs; 0 / 1: z and act stored as fp16 / bf16 (16-bit operand modes) */) {
+           int scale_u, int hfmt /* -1: fp32 outputs; 0 / 1: z and act stored as fp16 / bf16 (16-bit operand modes) */,
+           int fast /* 1: silu_fast (tensor-core precision modes) */) {
   const int M = *m_ptr;
   const int64_t e_base = (int64_t)blockIdx.x * TB0_EDGES;
   if (e_base >= M) return;
@@ -242,7 +251,8 @@ k_twobody0(const int* __restrict__ m_ptr, const int* __restrict__ ei, const int*
       }
       if (hfmt < 0) ek_st4(z + e * H + k4, acc); else h16_store4(z, (size_t)e * H + k4, acc, hfmt);
       const float us = scale_u ? sU[r] : 1.0f;
-      { const float4 o4 = make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
+      { const float4 o4 = fast ? make_float4(us * silu_fast(acc.x), us * silu_fast(acc.y), us * silu_fast(acc.z), us * silu_fast(acc.w))
+                               : make_float4(us * silu_f(acc.x), us * silu_f(acc.y), us * silu_f(acc.z), us * silu_f(acc.w));
         if (hfmt < 0) ek_st4(act + e * ldact + k4, o4); else h16_store4(act, (size_t)e * ldact + k4, o4, hfmt); }
     }
     return;
@@ -776,7 +786,8 @@ int k_launch_twobody0(allegro_model* m, Work& w, const int32_t* species, const D
   int ld = single ? (m->d + m->n) : L0.fo;
   k_twobody0<<<(m_cap + TB0_EDGES - 1) / TB0_EDGES, 256, 0, m->stream>>>((int*)w.m_act.p, (int*)w.ei.p, (int*)w.ej.p, species,
                                                                     (float*)w.B.p, (float*)w.u.p, L0.W, m->S, m->NB, L0.fo,
-                                                                    (float*)w.tb_z[0].p, act, ld, single ? 1 : 0, m->hfmt);
+                                                                    (float*)w.tb_z[0].p, act, ld, single ? 1 : 0, m->hfmt,
+                                                                    (m->hp.precision == 1 || m->hfmt >= 0) ? 1 : 0);
   LAUNCH_CHECK(m);
   return ALLEGRO_OK;
 }
